@@ -1,0 +1,336 @@
+"""Pins of the oracle against things other than itself (-m "not gpu").
+
+Each test names what fixes the expected value: a cited golden file, exact rational arithmetic, a closed form,
+an invariant, a library routine the oracle does not use, or pure-Python brute force on a tiny input.
+"""
+from fractions import Fraction
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+import datagen
+import oracle
+
+GOLD = Path(__file__).resolve().parent / "golden"
+
+
+def _rows(name):
+    for line in (GOLD / name).read_text().splitlines():
+        line = line.strip()
+        if line and not line.startswith("#"):
+            yield line.split()
+
+
+def _exact_delay(freqs, c, dm, tsamp, b):
+    """north_star formula in exact rational arithmetic on the double-valued inputs; round half away from zero."""
+    f, f0 = Fraction(float(freqs[c])), Fraction(float(freqs[0]))
+    v = Fraction(4148808, 1000) * Fraction(float(dm)) * (1 / (f * f) - 1 / (f0 * f0)) / Fraction(float(tsamp)) / b
+    q = int(v)            # v >= 0
+    return q + (1 if v - q >= Fraction(1, 2) else 0), v
+
+
+# ------------------------------------------------------------------------------------------------ C2 delays
+def test_delay_golden_values():
+    for wl, c, dm, b, exp in _rows("delays.txt"):
+        w = datagen.get_workload(wl)
+        k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
+        assert oracle.delay(k[int(c)], float(dm), int(b)) == int(exp), (wl, c, dm, b)
+        assert _exact_delay(w.freqs_mhz, int(c), float(dm), w.tsamp_s, int(b))[0] == int(exp)
+
+
+@pytest.mark.parametrize("wl", ["tiny", "mid", "ska", "lowf"])
+def test_delay_matches_exact_rational_on_samples(wl):
+    w = datagen.get_workload(wl)
+    k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
+    rng = np.random.default_rng(11)
+    for r in w.ranges:
+        cs = np.concatenate([[0, 1, w.nchans - 1], rng.integers(0, w.nchans, 60)])
+        js = np.concatenate([[0, 1, r[2] - 1], rng.integers(0, r[2], 60)])
+        for c, i in zip(cs, js):
+            dm = oracle.dm_value(r[0], r[1], int(i))
+            exp, v = _exact_delay(w.freqs_mhz, int(c), dm, w.tsamp_s, r[3])
+            got = oracle.delay(k[int(c)], dm, r[3])
+            # double evaluation may differ from the exact value only within 1e-9 of a tie
+            assert got == exp or abs((v - int(v)) - Fraction(1, 2)) < Fraction(1, 10**9), (wl, c, i)
+
+
+def test_delay_zero_and_monotone():
+    w = datagen.get_workload("ska")
+    k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
+    assert k[0] == 0.0 and np.all(np.diff(k) > 0)
+    for r in w.ranges:
+        assert oracle.delay(k[0], r[0] + 5 * r[1], r[3]) == 0
+        assert oracle.delay(k[-1], 0.0, r[3]) == 0
+        d = [oracle.delay(kc, oracle.dm_value(r[0], r[1], r[2] - 1), r[3]) for kc in k[::37]]
+        assert all(a <= b for a, b in zip(d, d[1:]))
+        d = [oracle.delay(k[-1], oracle.dm_value(r[0], r[1], i), r[3]) for i in range(0, r[2], 13)]
+        assert all(a <= b for a, b in zip(d, d[1:]))
+
+
+def test_pulse_signal_model_equals_search_delay():
+    """datagen's pulse sweep (signal model) lands on the oracle's delay for bin 1, so an injected pulse is aligned."""
+    for wl in ("tiny", "mid", "ska"):
+        w = datagen.get_workload(wl)
+        k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
+        for dm in (0.0, 50.0, 123.456):
+            sw = datagen.pulse_sweep(w.freqs_mhz, dm, w.tsamp_s)
+            mine = np.array([oracle.delay(kc, dm, 1) for kc in k])
+            assert np.max(np.abs(sw - mine)) <= 1 and np.mean(sw == mine) > 0.999
+
+
+# ------------------------------------------------------------------------------------------------ C3 geometry
+def test_chunk_geometry_golden():
+    for wl, B, S, n_out, outputs in _rows("geometry.txt"):
+        w = datagen.get_workload(wl)
+        k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
+        g = oracle.chunk_geometry(k, w.ranges, w.nsamp)
+        assert (g["B"], g["S"], g["n_out"]) == (int(B), int(S), int(n_out))
+        assert sum(r[2] * (g["n_out"] // r[3]) for r in w.ranges) == int(outputs)
+        assert len(g["chunks"]) == 1
+
+
+def test_chunk_geometry_streaming_tiles_without_gap():
+    w = datagen.get_workload("stream")
+    k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
+    g = oracle.chunk_geometry(k, w.ranges, w.nsamp, chunk_len=1 << 20)
+    assert g["S"] == 32384 and g["n_out"] == (1 << 20) - 32384
+    pos = 0
+    for (start, L, n) in g["chunks"]:
+        assert start == pos and L % g["B"] == 0 and start % g["B"] == 0 and start + L <= w.nsamp
+        pos += n
+    assert len(g["chunks"]) == 10 and g["chunks"][-1][1] == 229272      # SURVEY §8(d) Streaming row
+    assert pos == 9342616                                                # SURVEY §8(d) n_out (stream total)
+
+
+# ------------------------------------------------------------------------------------------------ C4 binning
+@pytest.mark.parametrize("b", [1, 2, 4, 8])
+def test_binning_constant_and_sum_conservation(b):
+    x = np.full((3, 64), 7, np.uint8)
+    assert np.all(oracle.bin_time(x, 0, 64 // b, b) == 7 * b)
+    rng = np.random.default_rng(b)
+    x = rng.integers(0, 256, (5, 96), dtype=np.uint8)
+    xb = oracle.bin_time(x, 8, 80 // b, b)
+    assert np.array_equal(xb.sum(axis=1), x[:, 8:88].astype(np.int64).sum(axis=1))
+    assert np.array_equal(xb, x[:, 8:88].reshape(5, -1, b).astype(np.int64).sum(axis=2))   # numpy reshape-sum
+    assert np.all(oracle.bin_time(np.full((1, 16), 255, np.uint8), 0, 2, 8) == 2040)
+
+
+# ------------------------------------------------------------------------------------------------ C5 dedispersion
+def test_dm0_row_is_channel_sum(tiny):
+    w, x, k, g = tiny
+    xb = oracle.bin_time(x, 0, g["L"], 1)
+    D = oracle.dedisperse(xb, k, w.ranges[0], 0, 1, g["n_out"])
+    assert np.array_equal(D[0], x[:, :g["n_out"]].astype(np.int64).sum(axis=0))
+
+
+def test_dedisperse_vs_pure_python_brute_force():
+    rng = np.random.default_rng(5)
+    C, L = 4, 40
+    x = rng.integers(0, 256, (C, L), dtype=np.uint8)
+    freqs = np.array([400.0, 390.0, 380.0, 370.0])
+    k = oracle.delay_constants(freqs, 1e-3)
+    r = (0.0, 0.7, 6, 1)
+    dl = [[oracle.delay(k[c], r[0] + i * r[1], 1) for c in range(C)] for i in range(r[2])]
+    T = L - max(max(d) for d in dl)
+    assert T > 8 and dl[-1][-1] > 3 and len({tuple(d) for d in dl}) > 3       # a non-trivial case
+    D = oracle.dedisperse(oracle.bin_time(x, 0, L, 1), k, r, 0, r[2], T)
+    for i in range(r[2]):
+        for t in range(T):
+            assert D[i, t] == sum(int(x[c, t + dl[i][c]]) for c in range(C))
+
+
+def test_dedisperse_binned_vs_brute_force():
+    rng = np.random.default_rng(6)
+    C, L, b = 3, 64, 4
+    x = rng.integers(0, 256, (C, L), dtype=np.uint8)
+    k = oracle.delay_constants(np.array([300.0, 290.0, 280.0]), 1e-3)
+    r = (2.0, 1.5, 4, b)
+    dl = [[oracle.delay(k[c], r[0] + i * r[1], b) for c in range(C)] for i in range(r[2])]
+    T = L // b - max(max(d) for d in dl)
+    assert T >= 4 and dl[-1][-1] >= 2
+    D = oracle.dedisperse(oracle.bin_time(x, 0, L // b, b), k, r, 0, r[2], T)
+    for i in range(r[2]):
+        for t in range(T):
+            assert D[i, t] == sum(int(x[c, b * (t + dl[i][c]) + j]) for c in range(C) for j in range(b))
+
+
+def test_dedisperse_constant_input_closed_form():
+    w = datagen.get_workload("tiny")
+    k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
+    for b in (1, 2):
+        x = np.full((w.nchans, 512), 9, np.uint8)
+        r = (0.0, 1.0, 20, b)
+        T = 512 // b - oracle.delay(k[-1], 19.0, b)
+        D = oracle.dedisperse(oracle.bin_time(x, 0, 512 // b, b), k, r, 0, 20, T)
+        assert np.all(D == w.nchans * b * 9)
+
+
+def test_dedisperse_single_impulse_response():
+    w = datagen.get_workload("tiny")
+    k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
+    x = np.zeros((w.nchans, 600), np.uint8)
+    c0, t0 = 40, 300
+    x[c0, t0] = 200
+    r = (0.0, 1.0, 101, 1)
+    T = 600 - 65
+    D = oracle.dedisperse(oracle.bin_time(x, 0, 600, 1), k, r, 0, 101, T)
+    exp = np.zeros_like(D)
+    for i in range(101):
+        exp[i, t0 - oracle.delay(k[c0], float(i), 1)] = 200
+    assert np.array_equal(D, exp)
+
+
+def test_dedisperse_all_rows_moment_identity(tiny):
+    """SURVEY §8(c) pin (v): sum_t D and sum_t t*D from per-channel prefix sums (an O(C) route per row)."""
+    w, x, k, g = tiny
+    r, T = w.ranges[0], g["n_out"]
+    xb = oracle.bin_time(x, 0, g["L"], 1).astype(np.int64)
+    D = oracle.dedisperse(oracle.bin_time(x, 0, g["L"], 1), k, r, 0, r[2], T)
+    P = np.concatenate([np.zeros((w.nchans, 1), np.int64), np.cumsum(xb, axis=1)], axis=1)
+    Q = np.concatenate([np.zeros((w.nchans, 1), np.int64), np.cumsum(xb * np.arange(xb.shape[1]), axis=1)], axis=1)
+    tt = np.arange(T)
+    for i in range(r[2]):
+        d = np.array([oracle.delay(kc, float(i), 1) for kc in k])
+        ch = np.arange(w.nchans)
+        m0 = (P[ch, T + d] - P[ch, d]).sum()
+        m1 = ((Q[ch, T + d] - Q[ch, d]) - d * (P[ch, T + d] - P[ch, d])).sum()
+        assert D[i].sum() == m0 and (D[i] * tt).sum() == m1
+
+
+# ------------------------------------------------------------------------------------------------ C6 statistics
+def test_stats_two_valued_row_exact():
+    row = np.array([100] * 500 + [104] * 500)             # mean 102, population sigma 2, nothing beyond 3 sigma
+    mu, sg, n, it, lo, hi, deg = oracle.row_stats(row)
+    assert (mu, sg, n, deg) == (102.0, 2.0, 1000, False) and (lo, hi) == (96, 108) and it == 1
+
+
+def test_stats_uniform_closed_form():
+    M = 200
+    row = np.tile(np.arange(M + 1), 7)
+    mu, sg, n, *_ = oracle.row_stats(row)
+    assert n == row.size and mu == M / 2
+    assert abs(sg - np.sqrt(((M + 1) ** 2 - 1) / 12.0)) < 1e-12 * sg
+
+
+def test_stats_outlier_rejected_hand_worked():
+    # 100 x 10 and one 1000: pass 0 mu=19.80, sigma=98.02 -> keep [-274, 313] drops 1000 -> mu=10, sigma=0
+    mu, sg, n, it, lo, hi, deg = oracle.row_stats(np.array([10] * 100 + [1000]))
+    assert (mu, sg, n) == (10.0, 0.0, 100) and it == 2 and not deg
+    # 3:1 mixture of 0 and 40 with a burst of 5 huge samples
+    row = np.array(([0] * 3 + [40]) * 250 + [100000] * 5)
+    mu, sg, n, *_ = oracle.row_stats(row)
+    assert n == 1000 and mu == 10.0 and abs(sg - np.sqrt(300.0)) < 1e-12
+
+
+def test_stats_gaussian_fixed_point_closed_form():
+    """For Gaussian data the 3-sigma clip converges to r*sigma with r^2 = 1 - 2a*phi(a)/(2Phi(a)-1), a = 3r."""
+    from math import erf, exp, pi, sqrt
+    r = 1.0
+    for _ in range(200):
+        a = 3.0 * r
+        r = sqrt(1.0 - 2.0 * a * (exp(-a * a / 2) / sqrt(2 * pi)) / erf(a / sqrt(2)))
+    assert abs(r - 0.98485) < 2e-5                         # the constant SURVEY §8(c) C6 quotes
+    rng = np.random.default_rng(3)
+    n = 400_000
+    row = np.round(rng.normal(520000.0, 1024.0, n)).astype(np.int64)
+    mu, sg, cnt, it, *_ = oracle.row_stats(row)
+    assert abs(sg / 1024.0 - r) < 4.0 / sqrt(n) and abs(mu - 520000.0) < 5 * 1024 / sqrt(n)
+    assert 2 <= it <= 8
+
+
+def test_stats_order_and_pivot_invariance():
+    rng = np.random.default_rng(4)
+    row = np.round(rng.normal(8000.0, 130.0, 5000)).astype(np.int64)
+    row[::97] += 4000
+    a = oracle.row_stats(row)
+    b = oracle.row_stats(rng.permutation(row))
+    assert a[2:6] == b[2:6]                                # n, iterations, lo, hi identical
+    assert abs(a[0] - b[0]) < 1e-9 and abs(a[1] - b[1]) < 1e-9
+
+
+def test_stats_constant_row_sigma_zero():
+    mu, sg, n, it, lo, hi, deg = oracle.row_stats(np.full(300, 77))
+    assert (mu, sg, n) == (77.0, 0.0, 300)
+    S, wb = oracle.boxcar_snr(np.full(300, 77), [1, 2], mu, sg)
+    assert np.all(np.isneginf(S)) and np.all(wb == 0)
+
+
+# ------------------------------------------------------------------------------------------------ C7 boxcar / SNR
+def test_boxcar_hand_worked():
+    row = np.array([5, 5, 5, 9, 9, 5, 5, 5])
+    S, wb = oracle.boxcar_snr(row, [1, 2, 4], 5.0, 2.0)
+    # t=3: w=1 -> (9-5)/2 = 2; w=2 -> (18-10)/(sqrt2*2) = 2*sqrt2; w=4 -> (28-20)/4 = 2
+    assert wb[3] == 2 and abs(S[3] - 2 * np.sqrt(2)) < 1e-15
+    assert wb[2] == 4 and S[2] == 2.0                      # w=1: 0, w=2: 4/(2*sqrt2)=1.414, w=4: 8/4=2
+    assert wb[4] == 1 and S[4] == 2.0                      # w=2: 4/2.83=1.41, w=4: 4/4=1; tie-free
+    assert wb[7] == 1 and S[7] == 0.0 and wb[6] == 1       # only w=1 (and 2 at t=6) valid at the end; ties keep smallest
+    assert wb[5] == 1 and S[5] == 0.0
+
+
+def test_boxcar_direct_vs_numpy_convolve_and_prefix():
+    rng = np.random.default_rng(8)
+    row = rng.integers(500000, 540000, 700).astype(np.int64)
+    widths = [1, 2, 3, 8, 64, 256]
+    mu, sg = 520000.25, 11000.5
+    S, wb = oracle.boxcar_snr(row, widths, mu, sg)
+    best = np.full(row.size, -np.inf); bw = np.zeros(row.size, np.int32)
+    for w in widths:
+        B = np.convolve(row, np.ones(w, np.int64), mode="valid")                 # library routine
+        snr = (B - w * mu) / (np.sqrt(w) * sg)
+        upd = snr > best[:B.size]
+        best[:B.size][upd] = snr[upd]; bw[:B.size][upd] = w
+    assert np.array_equal(wb, bw) and np.allclose(S, best, rtol=1e-12, atol=1e-12)
+    S2, wb2 = oracle.boxcar_snr(row, widths, mu, sg, prefix=True)
+    assert np.array_equal(S, S2) and np.array_equal(wb, wb2)                    # bit-identical routes
+
+
+# ------------------------------------------------------------------------------------------------ C8 peaks
+def test_peaks_hand_built_maps():
+    ninf = -np.inf
+    S = np.array([[1, 1, 1, 1, 1, 1, 1, 9],
+                  [1, 7, 7, 1, 1, 8, 1, 1],
+                  [1, 7, 7, 1, 1, 1, 1, 1],
+                  [1, 1, 1, 1, ninf, 6.5, 1, 1],
+                  [9, 1, 1, 1, ninf, ninf, 1, 6]], dtype=np.float64)
+    rr, tt = oracle.find_peaks(S, 6.0)
+    got = sorted(zip(rr.tolist(), tt.tolist()))
+    # corner (0,7)=9; plateau of 7s -> its first point (1,1) only; (1,5)=8; (3,5)=6.5 next to -inf; corner (4,0)=9;
+    # (4,7)=6 is not > threshold 6 (strict)
+    assert got == [(0, 7), (1, 1), (1, 5), (3, 5), (4, 0)]
+    rr, tt = oracle.find_peaks(S, 6.0, 1, 4)               # halo rows 0 and 4 are neighbours but not reported
+    assert sorted(zip(rr.tolist(), tt.tolist())) == [(1, 1), (1, 5), (3, 5)]
+    S[0, 6] = 8.5                                          # a bigger neighbour in the halo row kills (1,5)
+    rr, tt = oracle.find_peaks(S, 6.0, 1, 4)
+    assert sorted(zip(rr.tolist(), tt.tolist())) == [(1, 1), (3, 5)]
+
+
+# ------------------------------------------------------------------------------------------------ end to end
+def test_tiny_injected_pulse_recovered(tiny):
+    """BASELINE.json config 1 + north_star 'must recover an injected dispersed pulse at its DM and time within one
+    sample'; SURVEY §8(c) C7 closed form SNR ~ A*sqrt(C*w)/16.0026/0.98485 = 12.18 (+- noise)."""
+    w, x, k, g = tiny
+    xb = oracle.bin_time(x, 0, g["L"], 1)
+    r = oracle.search_rows(xb, k, w.ranges[0], 0, g["n_out"], w.widths, w.threshold, 0, 0, w.ranges[0][2],
+                           want=("D", "stats"))
+    c = r["cands"]
+    top = c[np.argmax(c["snr"])]
+    assert abs(int(top["dm_index"]) - 50) <= 1 and abs(int(top["sample"]) - 3000) <= 1 and int(top["width"]) == 4
+    assert abs(float(top["snr"]) - 12.0 * np.sqrt(64 * 4) / 16.0026 / 0.98485) < 1.5
+    assert r["D"][50, 3000:3004].mean() - r["stats"][50, 0] > 4 * r["stats"][50, 1]     # the pulse is in D at t0
+    # noise rows: mu ~ 127*C, sigma ~ 0.98485*16.0026*sqrt(C) (SURVEY §8(c) C6 closed form)
+    assert abs(np.median(r["stats"][:, 0]) - 127.0 * 64) < 3.0
+    assert abs(np.median(r["stats"][:, 1]) / (0.98485 * 16.0026 * 8.0) - 1.0) < 0.02
+    # canonical order (range, dm_index, sample)
+    key = list(zip(c["dm_index"].tolist(), c["sample"].tolist()))
+    assert key == sorted(key)
+
+
+def test_band_search_equals_full_search(tiny):
+    """Searching a band of rows with halo reproduces the same rows of the full search (used for the big configs)."""
+    w, x, k, g = tiny
+    xb = oracle.bin_time(x, 0, g["L"], 1)
+    full = oracle.search_rows(xb, k, w.ranges[0], 0, g["n_out"], w.widths, w.threshold, 0, 0, 101, want=())
+    band = oracle.search_rows(xb, k, w.ranges[0], 0, g["n_out"], w.widths, w.threshold, 0, 47, 54, want=())
+    sel = full["cands"][(full["cands"]["dm_index"] >= 47) & (full["cands"]["dm_index"] < 54)]
+    assert len(sel) > 0 and np.array_equal(sel, band["cands"])
