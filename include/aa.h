@@ -1,0 +1,208 @@
+/*
+ * aa.h — C ABI of the B200-native dedispersion + single-pulse-search (SPS) hot path.
+ *
+ * What it mirrors. arXiv:1912.07704 describes AstroAccelerate's plan -> strategy -> pipeline pattern:
+ * the user fills a *plan* with search parameters, the API computes an immutable *strategy* ("how input data are
+ * split and processed on the GPU", PAPER.md:43 §3.1, :59 §3.2), the pipeline "iterates over the radio telescope
+ * input data in chunks" and reports a *status code* per iteration (§3.3); telescope data stay on the
+ * host under the user's ownership, device memory is encapsulated, results are owned by the API (§2.4);
+ * modules request device memory from a memory manager before use (§2.3). The call sequence below is the
+ * paper's 8-step list (§3.1). The function names and the arithmetic are BASELINE.json `north_star`.
+ *
+ * Conventions
+ *   - Plain C, no exceptions cross the boundary, no global mutable state except a thread-local error string.
+ *   - Every entry point returns aa_status: >= 0 success / progress, < 0 error. After an error,
+ *     aa_last_error() names the offending field ("the API provides user feedback").
+ *     Errors raised by aa_run_* are sticky on the strategy.
+ *   - "host" / "device" is stated for every pointer. No CUDA allocation happens inside aa_run_*; all device memory
+ *     is carved from ONE arena at aa_strategy_setup (north_star "memory-manager arena makes one allocation per run").
+ *   - Thread safety: distinct strategies may be used from distinct threads; one strategy is not re-entrant.
+ */
+#ifndef AA_H
+#define AA_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct aa_plan aa_plan;          /* opaque: the user's search parameters + metadata */
+typedef struct aa_strategy aa_strategy;  /* opaque: immutable GPU configuration + the chunk cursor */
+
+typedef enum {
+    AA_OK = 0,
+    AA_STATUS_CHUNK_DONE = 1,        /* this chunk finished, more chunks remain */
+    AA_STATUS_FINISHED = 2,          /* the last chunk finished */
+    AA_ERR_INVALID_ARG = -1,
+    AA_ERR_NOT_READY = -2,           /* run before a successful setup                   (PAPER.md:59 items 2, 4) */
+    AA_ERR_BUDGET_TOO_SMALL = -3,
+    AA_ERR_CUDA = -4,
+    AA_ERR_CANDIDATE_OVERFLOW = -5,  /* records beyond capacity were dropped, the count is still exact */
+    AA_ERR_ORDER = -6,               /* "another module still needs to run" */
+    AA_ERR_INTERNAL = -7
+} aa_status;
+
+/* One DM range: DM_i = dm_low + i*dm_step for i in [0, ndms); the range is searched on data decimated in time by
+ * `bin` in {1,2,4,8} (north_star "DM ranges that decimate in time by 1/2/4/8"; binning = SUM of bin samples). */
+typedef struct {
+    double dm_low, dm_step;
+    int32_t ndms;
+    int32_t bin;
+} aa_dm_range;
+
+/* One candidate (north_star "finds local peaks above a threshold into a candidate list"). */
+typedef struct {
+    uint64_t sample;    /* absolute UNBINNED start sample of the best boxcar */
+    float dm;           /* (float) DM_i */
+    float snr;          /* (float) best SNR over the plan's widths */
+    uint32_t width;     /* best boxcar width in UNBINNED samples (= w * bin) */
+    uint32_t range;     /* index into the plan's ranges */
+    uint32_t dm_index;  /* i within the range */
+} aa_candidate;
+
+/* Per-range geometry of one chunk, as decided by the strategy (read-only facts, PAPER.md:59 item 2). */
+typedef struct {
+    int32_t ndms, bin;
+    int64_t nt;            /* T_r: output samples per DM row per FULL chunk (binned units) = n_out / bin */
+    int64_t row_pitch;     /* int32 elements between consecutive DM rows of D_r on the device */
+    int64_t max_delay;     /* delay(C-1, last DM) in binned samples */
+    int32_t dm_tile, t_tile, chan_block, window;   /* dedispersion kernel tiling chosen for this range */
+} aa_range_info;
+
+typedef struct {
+    int32_t ready;             /* 1 once setup succeeded */
+    int32_t nchans, nranges, nwidths;
+    int32_t max_bin;           /* B */
+    int64_t nsamp_total;
+    int64_t overlap;           /* S: unbinned samples shared by consecutive chunks = max delay rounded up to B */
+    int64_t chunk_len;         /* L: unbinned input samples per full chunk (multiple of B, > S) */
+    int64_t n_out;             /* L - S: unbinned output span per full chunk */
+    int64_t nchunks;
+    int64_t next_chunk;        /* chunk cursor: index of the chunk the next aa_run_dedispersion will process */
+    size_t arena_bytes_used;   /* bytes carved from the arena */
+    size_t arena_bytes_total;
+    size_t max_candidates;
+    int32_t owns_arena;        /* 1 if the library made the (single) cudaMalloc */
+} aa_strategy_info;
+
+/* ------------------------------------------------------------------------------------------------ plan
+ * PAPER.md:47 steps 1,3 ("provide ... metadata", "configure each module with a plan"). All arrays are HOST memory and
+ * are copied; the caller may free them on return.
+ *   chan_freq_mhz [nchans]  strictly descending; [0] is f_top, the reference of every delay.
+ *   tsamp_s                 sampling time in seconds (> 0).
+ *   ranges [nranges]        ndms >= 1, dm_step > 0 (or ndms == 1), dm_low >= 0, bin in {1,2,4,8}.
+ *   boxcar_widths [nwidths] strictly ascending, >= 1, in BINNED samples of each range (north_star "widths 1..W").
+ *   snr_threshold           candidates need SNR > threshold (strict).
+ * Limits checked here: nchans*255*max(bin) < 2^23 (int32 sums with headroom for the packed accumulators) and
+ * max(width)*nchans*255*max(bin) < 2^31 (boxcar sums). Errors: AA_ERR_INVALID_ARG naming the field. */
+aa_status aa_plan_create(aa_plan** out, int32_t nchans, const double* chan_freq_mhz, double tsamp_s,
+                         const aa_dm_range* ranges, int32_t nranges,
+                         const int32_t* boxcar_widths, int32_t nwidths, float snr_threshold);
+void aa_plan_destroy(aa_plan* plan);
+
+/* ------------------------------------------------------------------------------------------------ strategy
+ * PAPER.md:47 steps 4-6 ("bind", "the API calculates the optimal strategy", "checks whether all modules are
+ * configured"). Host-side planning plus ONE device allocation (or none if the caller lends an arena):
+ *   delays:  k_c = (4.148808e3*(f_c^-2 - f_0^-2))/tsamp; delay(c,r,i) = llround((k_c*DM_ri)/bin_r)   [north_star]
+ *   chunks:  S = ceil_B(max_r bin_r*delay(C-1,r,last)); L multiple of B with arena(L) <= budget; n_out = L - S;
+ *            chunk j covers input [j*n_out, j*n_out + L) and outputs [j*n_out, (j+1)*n_out); the last chunk takes the
+ *            remaining input rounded down to a multiple of B (reading C3). chunk_len_hint > 0 forces L.
+ *   device_arena (DEVICE, may be NULL): caller-owned memory of arena_bytes (e.g. a torch uint8 tensor), 256-byte
+ *            aligned. NULL => the library makes exactly one cudaMalloc of the bytes it needs (<= budget_bytes;
+ *            budget_bytes == 0 means "no limit": a single chunk if it fits the device).
+ *   compute_stream / copy_stream: cudaStream_t handles (e.g. from torch); NULL => the library creates its own.
+ *   max_candidates: capacity of the device candidate buffer per chunk and of the host list.
+ * The plan may be destroyed afterwards. Errors: AA_ERR_INVALID_ARG, AA_ERR_BUDGET_TOO_SMALL (message states the
+ * bytes needed for the smallest legal chunk), AA_ERR_CUDA. */
+aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, uint64_t nsamp_total,
+                            void* device_arena, size_t arena_bytes, size_t budget_bytes,
+                            void* compute_stream, void* copy_stream, size_t max_candidates,
+                            uint64_t chunk_len_hint);
+void aa_strategy_destroy(aa_strategy* s);
+
+/* Host-only planning: the same delays, chunk geometry, kernel tiling and arena size as aa_strategy_setup, without touching
+ * the GPU. The result has ready == 0 ("query the strategy fields and ready-state"): getters work,
+ * aa_run_* return AA_ERR_NOT_READY. budget_bytes == 0 means unlimited (a single chunk). arena_bytes_used reports the bytes a
+ * real setup would carve. */
+aa_status aa_strategy_plan(aa_strategy** out, const aa_plan* plan, uint64_t nsamp_total, size_t budget_bytes,
+                           size_t max_candidates, uint64_t chunk_len_hint);
+
+/* Read-only queries (PAPER.md:59 item 2 "the user may query the strategy fields and ready-state"). */
+aa_status aa_strategy_get_info(const aa_strategy* s, aa_strategy_info* out);
+aa_status aa_strategy_get_range_info(const aa_strategy* s, int32_t range, aa_range_info* out);
+/* Chunk j: absolute start sample, input length L_j and output span n_out_j (unbinned). */
+aa_status aa_strategy_get_chunk(const aa_strategy* s, int64_t chunk, uint64_t* start, uint64_t* len, uint64_t* n_out);
+/* delay(c, range, dm_index) in binned samples, as used by the kernels. */
+aa_status aa_strategy_get_delay(const aa_strategy* s, int32_t range, int32_t dm_index, int32_t chan, int64_t* delay);
+/* Human-readable dump of chunking, tiling and arena layout into buf (HOST); returns bytes needed incl. NUL. */
+size_t aa_strategy_describe(const aa_strategy* s, char* buf, size_t buflen);
+/* Rewind the chunk cursor to 0 and forget all candidates (the configuration itself is immutable). */
+aa_status aa_strategy_reset(aa_strategy* s);
+
+/* ------------------------------------------------------------------------------------------------ pipeline
+ * PAPER.md:47 step 7. One call = one chunk of one module.
+ *
+ * aa_run_dedispersion: H2D of the cursor's chunk (unless a previous call prefetched it), prefetch of the following chunk
+ * into the other input buffer on the copy stream, time binning for ranges with bin > 1, then
+ *   D_r[i][t'] = sum_c x_b[c][t' + delay(c,r,i)]   (int32, bit-exact)            [north_star]
+ * for every range. Asynchronous: returns after enqueueing.
+ *   host_input (HOST, const, user-owned, never written): x[c][t] uint8, channel-major, the WHOLE observation
+ *              (nsamp_total samples per channel), row_stride_bytes between channels. Must stay valid until the
+ *              following aa_run_* call returns (prefetch). Pinned memory is needed for the copy to overlap compute.
+ * Returns AA_OK; AA_ERR_NOT_READY; AA_ERR_ORDER if the previous chunk's SPS has not run; AA_ERR_CUDA. */
+aa_status aa_run_dedispersion(aa_strategy* s, const uint8_t* host_input, size_t row_stride_bytes);
+
+/* Same, with the chunk already resident on the DEVICE: device_chunk points at sample `start` of chunk `cursor`
+ * (x[c][0..L_j)), row stride in bytes, at least 16-byte aligned rows; the data are copied device-to-device into the
+ * arena's input buffer (so the kernel's over-read slack exists). Used when the producer is another GPU stage. */
+aa_status aa_run_dedispersion_device(aa_strategy* s, const uint8_t* device_chunk, size_t row_stride_bytes);
+
+/* aa_run_sps: on the chunk just dedispersed — robust per-row mean/sigma, boxcar SNR, 3x3 local peaks above the
+ * threshold, appended to the device candidate buffer. Advances the chunk cursor.
+ * Returns AA_STATUS_CHUNK_DONE or AA_STATUS_FINISHED; AA_ERR_ORDER if no dedispersed chunk is pending. */
+aa_status aa_run_sps(aa_strategy* s);
+
+/* aa_get_candidates: synchronises, copies the device records to library-owned HOST memory, and returns ALL candidates
+ * of the chunks processed so far in canonical order (chunk, range, dm_index, sample). *out stays valid until the next
+ * aa_run_*, aa_strategy_reset or aa_strategy_destroy. Returns AA_OK, or AA_ERR_CANDIDATE_OVERFLOW when more
+ * candidates were found than max_candidates (the list holds the first max_candidates in arrival order, sorted; the true
+ * count is in aa_last_error()). */
+aa_status aa_get_candidates(aa_strategy* s, const aa_candidate** out, size_t* n);
+
+/* Parity hooks: copy one row of the CURRENT chunk (the one last dedispersed / searched) to library-owned HOST memory.
+ * Valid until the next call on this strategy. */
+aa_status aa_get_dedispersed_row(aa_strategy* s, int32_t range, int32_t dm_index, const int32_t** host_row, size_t* len);
+/* mu, sigma, n kept, clip iterations of a row, as computed by aa_run_sps for the current chunk. */
+aa_status aa_get_row_stats(aa_strategy* s, int32_t range, int32_t dm_index, double* mu, double* sigma,
+                           int64_t* n_kept, int32_t* iterations);
+/* Per-row moments sum_t D and sum_t t*D (int64) of every row of a range, computed on the device (test hook for the
+ * all-rows checksum). out arrays are HOST, length ndms. */
+aa_status aa_get_row_moments(aa_strategy* s, int32_t range, int64_t* sum_d, int64_t* sum_td);
+/* Device pointer of D_r for the current chunk and its row pitch in elements (read-only use by other GPU code). */
+aa_status aa_get_dedispersed_device(aa_strategy* s, int32_t range, const int32_t** device_ptr, int64_t* row_pitch);
+
+/* Block until everything enqueued on the strategy's streams has finished. */
+aa_status aa_synchronize(aa_strategy* s);
+
+/* ------------------------------------------------------------------------------------------------ measurement
+ * Sustained 32-bit integer add rate of this GPU (the roofline denominator): runs the K0
+ * microbenchmark for about `millis` ms on `stream` (NULL = default). Outputs (HOST): lane-adds per second with
+ * IADD3-only chains, with IADD3+IMAD mixed chains (both integer pipes), and the SM clock (MHz) observed via the cycle
+ * counter. */
+aa_status aa_measure_int_add_peak(void* stream, int32_t millis, double* iadd3_per_s, double* mixed_per_s, double* sm_mhz);
+
+/* CUDA-event time (ms) of the kernel classes of the last chunk: [0] binning, [1] dedispersion (all ranges),
+ * [2] SPS statistics, [3] SPS boxcar/peaks, [4] H2D of the chunk (0 if prefetched/overlapped). Synchronises. */
+aa_status aa_get_last_timings(aa_strategy* s, float ms_out[5]);
+/* Number of kernel launches issued by this strategy since setup / reset. */
+aa_status aa_get_launch_count(const aa_strategy* s, uint64_t* launches);
+
+const char* aa_last_error(void);   /* thread-local, never NULL */
+const char* aa_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AA_H */

@@ -1,0 +1,136 @@
+/*
+ * aa_internal.h — host-side objects behind the opaque handles of include/aa.h.
+ * plan = the user's parameters; strategy = immutable GPU configuration + chunk cursor;
+ * Arena = the memory manager from which every device buffer is carved once (§2.3).
+ */
+#ifndef AA_INTERNAL_H
+#define AA_INTERNAL_H
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/aa.h"
+#include "aa_kernels.h"
+
+namespace aa {
+
+void set_error(const char* fmt, ...);
+aa_status cuda_fail(cudaError_t e, const char* what);
+
+constexpr int kDmTile = 32;       /* must match k_dedisp.cu */
+constexpr int kTTile = 1024;
+constexpr size_t kSlack = 64 * 1024;   /* readable bytes after every input buffer (TMA windows over-read) */
+
+inline size_t round_up(size_t v, size_t m) { return (v + m - 1) / m * m; }
+
+struct Plan {
+    int32_t nchans = 0;
+    std::vector<double> freq;
+    double tsamp = 0.0;
+    std::vector<aa_dm_range> ranges;
+    std::vector<int32_t> widths;
+    float threshold = 0.f;
+};
+
+/* Single-allocation bump allocator over caller- or library-owned device memory. */
+struct Arena {
+    uint8_t* base = nullptr;
+    size_t size = 0, used = 0;
+    bool dry = false;             /* dry run: only measure */
+    void* take(size_t bytes) {
+        const size_t off = round_up(used, 256);
+        used = off + bytes;
+        if (dry || used > size) return nullptr;
+        return base + off;
+    }
+};
+
+struct Range {
+    aa_dm_range r;
+    int32_t index = 0;
+    int32_t in16 = 0, esz = 1, spw = 4, ncopy = 4;
+    int64_t max_delay = 0;        /* binned samples */
+    int64_t nt_full = 0;          /* T_r of a full chunk */
+    int64_t pitch = 0;            /* D row pitch, elements */
+    int32_t chan_block = 8, window_bytes = 0, spill_stages = 0, ndm_tiles = 0, nstages = 0;
+    std::vector<int32_t> delays;  /* [ndms][nchans], binned samples (host) */
+    int32_t* d_etab = nullptr;
+    int32_t* d_x0tab = nullptr;
+    int32_t* d_D = nullptr;
+    CUtensorMap maps[2][4];       /* [raw buffer parity][copy] */
+    size_t first_row = 0;         /* index of this range's first row in the row tables */
+};
+
+struct Chunk { uint64_t start, len, n_out; };
+
+struct Strategy {
+    bool ready = false;           /* false for a host-only strategy made by aa_strategy_plan */
+    Plan plan;
+    std::vector<double> k;        /* delay constants, samples per unit DM (unbinned) */
+    uint64_t nsamp_total = 0;
+    int32_t B = 1;
+    int64_t S = 0, L = 0, n_out = 0;
+    std::vector<Chunk> chunks;
+    std::vector<Range> ranges;
+    size_t nrows = 0;
+
+    /* device memory */
+    Arena arena;
+    bool owns_arena = false;
+    size_t in_pitch = 0;                     /* bytes per channel row of the uint8 buffers */
+    uint8_t* d_raw[2] = {nullptr, nullptr};  /* H2D targets (copy 0 of the uint8 input) */
+    uint8_t* d_shift[3] = {nullptr, nullptr, nullptr};   /* copies 1..3 of the uint8 input */
+    bool need_u8_copies = false;
+    size_t xb_pitch[9] = {0};                /* elements, indexed by bin */
+    uint16_t* d_xb[9][2] = {{nullptr}};      /* binned input, copies 0 and 1, indexed by bin */
+    aak_row_desc* d_rows[2] = {nullptr, nullptr};   /* [0] full chunk geometry, [1] last (short) chunk */
+    double* d_mu_sigma = nullptr;            /* [nrows][2] */
+    int64_t* d_n_iters = nullptr;            /* [nrows][2] */
+    aak_candidate* d_cands = nullptr;
+    unsigned long long* d_counter = nullptr;
+    long long* d_moments = nullptr;          /* [2][max ndms] */
+    size_t max_candidates = 0;
+
+    /* streams / events */
+    cudaStream_t compute = nullptr, copy = nullptr;
+    bool owns_compute = false, owns_copy = false;
+    cudaEvent_t ev_copied[2] = {nullptr, nullptr};    /* chunk landed in d_raw[b] (copy stream) */
+    cudaEvent_t ev_raw_free[2] = {nullptr, nullptr};  /* last reader of d_raw[b] finished (compute stream) */
+    cudaEvent_t ev_count = nullptr;                   /* candidate counter copied to the host */
+    cudaEvent_t ev_t[6] = {nullptr};                  /* timing marks on the compute stream */
+    cudaEvent_t ev_h2d[2] = {nullptr, nullptr};       /* timing marks on the copy stream */
+    bool h2d_timed = false;
+
+    /* cursor / state */
+    int64_t next_chunk = 0;
+    int64_t current_chunk = -1;        /* chunk whose D is on the device */
+    bool pending_sps = false;
+    int64_t raw_holds[2] = {-1, -1};   /* which chunk each raw buffer holds (or is receiving) */
+    bool raw_free_recorded[2] = {false, false};
+    bool harvest_pending = false;
+    int64_t harvest_chunk = -1;
+    aa_status sticky = AA_OK;
+    uint64_t launches = 0;
+    bool timed = false, stats_timed = false;
+
+    /* host results */
+    unsigned long long* h_counter = nullptr;    /* pinned */
+    std::vector<aa_candidate> cands;
+    uint64_t true_count = 0;
+    bool overflow = false;
+    std::vector<int32_t> host_row;
+};
+
+/* aa_strategy.cpp */
+int64_t delay_of(const Strategy& s, const Range& rg, int32_t chan, int32_t dm_index);
+
+}  // namespace aa
+
+struct aa_plan { aa::Plan p; };
+struct aa_strategy { aa::Strategy s; };
+
+#endif

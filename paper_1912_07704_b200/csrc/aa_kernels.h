@@ -1,0 +1,97 @@
+/*
+ * aa_kernels.h — C-style launch wrappers of the CUDA kernels (one per kernel class), called by the host runtime.
+ * Follows the separate-compilation practice of PAPER.md:25 (§2.1): CUDA code in its own translation units behind
+ * C wrapper functions; host code compiled by the host compiler.
+ *
+ * All pointers are DEVICE pointers unless named h_*. No wrapper allocates memory. Every wrapper returns the
+ * cudaError_t of the launch (cudaGetLastError), as an int.
+ */
+#ifndef AA_KERNELS_H
+#define AA_KERNELS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- K1: time binning, x_b[c][t'] = sum_{j<b} x[c][b*t'+j]  (uint8 -> uint16) --------------------------------- */
+int aak_bin_time(const uint8_t* x, size_t x_pitch, uint16_t* xb, size_t xb_pitch_elems, int32_t nchans,
+                 int64_t nbinned, int32_t bin, void* stream);
+/* ---- K1b: shifted copy, out[c][j] = in[c][j + shift_bytes] (1..3) for j in [0, row_bytes), rows `pitch` bytes apart.
+ * row_bytes and pitch are multiples of 16; the source must be readable up to row_bytes + 4 past each row start. */
+int aak_shift_copy(const uint8_t* in, uint8_t* out, size_t pitch, size_t row_bytes, int32_t nrows, int32_t shift_bytes,
+                   void* stream);
+
+/* ---- K2: dedispersion --------------------------------------------------------------------------------------------
+ * Tiled kernel: a CTA owns DM_TILE(=32) DM trials x T_TILE(=1024) output samples; channels stream through shared memory
+ * in blocks of `chan_block` via TMA (tensor map `tmap`, 128 opaque bytes, see aa_strategy.cpp), NSTAGE-deep mbarrier ring.
+ * The input exists as NCOPY = 4 (uint8) or 2 (uint16) sample-shifted copies in global memory, copy k = x[c][t+k];
+ * tmap points at NCOPY consecutive 128-byte CUtensorMaps (HOST memory), one per copy.
+ * etab  [ndm_tiles][nstages][chan_block][32] int32 : shared-memory byte offset of (channel, DM) inside a stage
+ * x0tab [ndm_tiles][nstages*chan_block]    int32 : 16-byte aligned BYTE offset of the channel window relative to the
+ *                                                  tile's first output sample */
+typedef struct {
+    const void* tmap;          /* HOST pointer to NCOPY 128-byte CUtensorMaps (copied into kernel params) */
+    const int32_t* etab;
+    const int32_t* x0tab;
+    int32_t* D;                /* [ndms][pitch] */
+    int64_t pitch;
+    int64_t nt;                /* T_r valid outputs per row */
+    int32_t ndms;
+    int32_t nchans;
+    int32_t chan_block;        /* 8, 4 or 2 */
+    int32_t window_bytes;      /* WB: bytes per (copy, channel) window in shared memory, multiple of 256 */
+    int32_t boxes_per_row;     /* 1 (one 3-D box covers the window) or WB/256 (one 2-D box per 256 bytes) */
+    int32_t spill_stages;      /* carry the 16-bit lanes every this many stages: (256/bin)/chan_block */
+    int32_t in16;              /* 0: uint8 input (bin 1), 1: uint16 input (binned) */
+    int32_t variant;           /* uint8 only: 1 = odd-byte lane adds issued as IMAD (FMA pipe), 0 = fused IADD3 */
+} aak_dedisp_args;
+int aak_dedisperse(const aak_dedisp_args* a, void* stream);
+size_t aak_dedisperse_smem_bytes(int32_t chan_block, int32_t window_bytes, int32_t in16);
+int aak_dedisperse_init(void);   /* sets the dynamic shared-memory attribute of every instantiation */
+
+/* Reference kernel (one thread per output, global loads): debugging / cross-check only. delays [ndms][nchans] int32. */
+int aak_dedisperse_naive(const void* x, size_t pitch_elems, int32_t in16, const int32_t* delays, int32_t nchans,
+                         int32_t ndms, int64_t nt, int32_t* D, int64_t pitch, void* stream);
+
+/* ---- K3: robust row statistics ---------------------------------------------------------------------------------
+ * rows: one entry per DM row of all ranges of the chunk. stats out: per row {mu, sigma} doubles and {n, iters} */
+typedef struct {
+    const int32_t* D;     /* row base */
+    int64_t nt;
+} aak_row_desc;
+int aak_row_stats(const aak_row_desc* rows, int32_t nrows, double* mu_sigma /* [nrows][2] */,
+                  int64_t* n_iters /* [nrows][2] */, void* stream);
+
+/* ---- K4: boxcar SNR + 3x3 peaks + candidate append ---------------------------------------------------------------- */
+typedef struct {
+    uint64_t sample; float dm; float snr; uint32_t width; uint32_t range; uint32_t dm_index;
+} aak_candidate;
+typedef struct {
+    const int32_t* D; int64_t pitch; int64_t nt; int32_t ndms; int32_t bin; int32_t range_index;
+    double dm_low, dm_step;
+    const double* mu_sigma;    /* [ndms][2] for this range */
+    uint64_t chunk_start;
+    int32_t widths[16]; int32_t nwidths;
+    double threshold;
+    aak_candidate* cands; unsigned long long* counter; unsigned long long capacity;
+} aak_sps_args;
+int aak_sps_peaks(const aak_sps_args* a, void* stream);
+int aak_sps_init(void);
+
+/* ---- K5 (test hook): per-row moments sum_t D, sum_t t*D ------------------------------------------------------------ */
+int aak_row_moments(const int32_t* D, int64_t pitch, int64_t nt, int32_t ndms, long long* sum_d, long long* sum_td,
+                    void* stream);
+
+/* ---- K0: integer-add peak microbenchmark ----------------------------------------------------------------------------
+ * mode 0: IADD3-only chains, mode 1: IADD3 + IMAD mixed chains. cycles_out [gridDim] receives per-CTA cycle counts. */
+int aak_peak_iadd(int32_t mode, int32_t iters, int32_t grid, int32_t threads, uint32_t* sink, unsigned long long* cycles_out,
+                  void* stream);
+#define AAK_PEAK_ADDS_PER_THREAD_ITER 16
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,358 @@
+/*
+ * aa_pipeline.cpp — the pipeline: "iterates over the radio telescope input data in chunks. On each iteration, the user may
+ * query the pipeline via a status code" (§3.3). One aa_run_* call = one module on one chunk; nothing here
+ * allocates device memory and the dedispersed data never leave the GPU between the modules.
+ * Host input is const and user-owned; results are copied into library-owned host memory.
+ */
+#include <algorithm>
+#include <cstring>
+
+#include "aa_internal.h"
+
+using namespace aa;
+
+namespace {
+
+#define AA_CUDA(call, what)                                              \
+    do {                                                                 \
+        cudaError_t e_ = (call);                                         \
+        if (e_ != cudaSuccess) { s.sticky = cuda_fail(e_, what); return s.sticky; } \
+    } while (0)
+#define AA_LAUNCH(call, what)                                            \
+    do {                                                                 \
+        int e_ = (call);                                                 \
+        ++s.launches;                                                    \
+        if (e_ != 0) { s.sticky = cuda_fail((cudaError_t)e_, what); return s.sticky; } \
+    } while (0)
+
+aa_status check_ready(aa_strategy* h, const char* fn) {
+    if (!h) { set_error("%s: strategy is NULL — configure a plan and call aa_strategy_setup first", fn); return AA_ERR_NOT_READY; }
+    if (!h->s.ready) { set_error("%s: this strategy was only planned (aa_strategy_plan); call aa_strategy_setup to make it ready", fn); return AA_ERR_NOT_READY; }
+    if (h->s.sticky < 0) { return h->s.sticky; }
+    return AA_OK;
+}
+
+/* Enqueue the H2D copy of chunk j into raw buffer b on the copy stream. */
+aa_status enqueue_h2d(Strategy& s, int64_t j, int b, const uint8_t* host_input, size_t row_stride, bool timed) {
+    const Chunk& c = s.chunks[(size_t)j];
+    if (s.raw_free_recorded[b]) AA_CUDA(cudaStreamWaitEvent(s.copy, s.ev_raw_free[b], 0), "cudaStreamWaitEvent");
+    if (timed) AA_CUDA(cudaEventRecord(s.ev_h2d[0], s.copy), "cudaEventRecord");
+    AA_CUDA(cudaMemcpy2DAsync(s.d_raw[b], s.in_pitch, host_input + c.start, row_stride, (size_t)c.len, (size_t)s.plan.nchans,
+                              cudaMemcpyHostToDevice, s.copy), "cudaMemcpy2DAsync (H2D chunk)");
+    if (timed) AA_CUDA(cudaEventRecord(s.ev_h2d[1], s.copy), "cudaEventRecord");
+    AA_CUDA(cudaEventRecord(s.ev_copied[b], s.copy), "cudaEventRecord");
+    s.raw_holds[b] = j;
+    return AA_OK;
+}
+
+/* Shifted copies, binning and the dedispersion launches for the chunk resident in raw buffer b. */
+aa_status enqueue_dedispersion(Strategy& s, int64_t j, int b) {
+    const Chunk& c = s.chunks[(size_t)j];
+    const int32_t C = s.plan.nchans;
+    AA_CUDA(cudaEventRecord(s.ev_t[0], s.compute), "cudaEventRecord");
+    if (s.need_u8_copies)
+        for (int k = 1; k <= 3; ++k)
+            AA_LAUNCH(aak_shift_copy(s.d_raw[b], s.d_shift[k - 1], s.in_pitch, s.in_pitch, C, k, s.compute), "shift copy (uint8)");
+    for (int bin = 2; bin <= 8; bin *= 2) {
+        if (!s.d_xb[bin][0]) continue;
+        const size_t pitch_bytes = s.xb_pitch[bin] * 2;
+        AA_LAUNCH(aak_bin_time(s.d_raw[b], s.in_pitch, s.d_xb[bin][0], s.xb_pitch[bin], C, (int64_t)(c.len / (uint64_t)bin), bin, s.compute), "time binning");
+        AA_LAUNCH(aak_shift_copy((const uint8_t*)s.d_xb[bin][0], (uint8_t*)s.d_xb[bin][1], pitch_bytes, pitch_bytes, C, 2, s.compute), "shift copy (uint16)");
+    }
+    AA_CUDA(cudaEventRecord(s.ev_t[1], s.compute), "cudaEventRecord");
+    for (Range& rg : s.ranges) {
+        aak_dedisp_args a;
+        a.tmap = &rg.maps[b][0];
+        a.etab = rg.d_etab; a.x0tab = rg.d_x0tab; a.D = rg.d_D; a.pitch = rg.pitch;
+        a.nt = (int64_t)(c.n_out / (uint64_t)rg.r.bin);
+        a.ndms = rg.r.ndms; a.nchans = C; a.chan_block = rg.chan_block; a.window_bytes = rg.window_bytes; a.boxes_per_row = 1;
+        a.spill_stages = rg.spill_stages; a.in16 = rg.in16; a.variant = 1;
+        AA_LAUNCH(aak_dedisperse(&a, s.compute), "dedispersion");
+    }
+    AA_CUDA(cudaEventRecord(s.ev_t[2], s.compute), "cudaEventRecord");
+    AA_CUDA(cudaEventRecord(s.ev_raw_free[b], s.compute), "cudaEventRecord");
+    s.raw_free_recorded[b] = true;
+    s.timed = true; s.stats_timed = false;
+    s.current_chunk = j;
+    s.pending_sps = true;
+    return AA_OK;
+}
+
+bool cand_less(const aa_candidate& a, const aa_candidate& b) {
+    if (a.range != b.range) return a.range < b.range;
+    if (a.dm_index != b.dm_index) return a.dm_index < b.dm_index;
+    return a.sample < b.sample;
+}
+
+/* Bring the candidates of the last searched chunk to the host (PAPER.md:47 step 8). Synchronises on the counter copy. */
+aa_status harvest(Strategy& s) {
+    if (!s.harvest_pending) return AA_OK;
+    AA_CUDA(cudaEventSynchronize(s.ev_count), "cudaEventSynchronize");
+    const unsigned long long found = *s.h_counter;
+    s.true_count += found;
+    unsigned long long take = std::min<unsigned long long>(found, s.max_candidates);
+    const size_t room = s.max_candidates - std::min(s.max_candidates, s.cands.size());
+    if (take > room) take = room;
+    if (take < found) s.overflow = true;
+    if (take) {
+        const size_t old = s.cands.size();
+        s.cands.resize(old + (size_t)take);
+        static_assert(sizeof(aa_candidate) == sizeof(aak_candidate), "candidate layouts must match");
+        AA_CUDA(cudaMemcpyAsync(s.cands.data() + old, s.d_cands, (size_t)take * sizeof(aa_candidate), cudaMemcpyDeviceToHost, s.compute), "candidate D2H");
+        AA_CUDA(cudaStreamSynchronize(s.compute), "cudaStreamSynchronize");
+        std::sort(s.cands.begin() + (ptrdiff_t)old, s.cands.end(), cand_less);   /* chunks arrive in order: canonical */
+    }
+    s.harvest_pending = false;
+    return AA_OK;
+}
+
+}  // namespace
+
+extern "C" aa_status aa_run_dedispersion(aa_strategy* h, const uint8_t* host_input, size_t row_stride_bytes) {
+    aa_status st = check_ready(h, "aa_run_dedispersion");
+    if (st != AA_OK) return st;
+    Strategy& s = h->s;
+    if (!host_input) { set_error("aa_run_dedispersion: host_input is NULL"); return AA_ERR_INVALID_ARG; }
+    if (row_stride_bytes < s.nsamp_total) { set_error("aa_run_dedispersion: row_stride_bytes = %zu is shorter than nsamp_total = %llu", row_stride_bytes, (unsigned long long)s.nsamp_total); return AA_ERR_INVALID_ARG; }
+    if (s.pending_sps) { set_error("aa_run_dedispersion: chunk %lld is dedispersed but aa_run_sps has not run on it yet", (long long)s.current_chunk); return AA_ERR_ORDER; }
+    if (s.next_chunk >= (int64_t)s.chunks.size()) { set_error("aa_run_dedispersion: all %zu chunks are done (aa_strategy_reset rewinds)", s.chunks.size()); return AA_ERR_ORDER; }
+    const int64_t j = s.next_chunk;
+    const int b = s.d_raw[1] ? (int)(j & 1) : 0;
+    s.h2d_timed = false;
+    if (s.raw_holds[b] != j) {
+        if ((st = enqueue_h2d(s, j, b, host_input, row_stride_bytes, true)) != AA_OK) return st;
+        s.h2d_timed = true;
+    }
+    AA_CUDA(cudaStreamWaitEvent(s.compute, s.ev_copied[b], 0), "cudaStreamWaitEvent");
+    if ((st = enqueue_dedispersion(s, j, b)) != AA_OK) return st;
+    /* double buffering: start moving chunk j+1 while chunk j computes (north_star "Streaming") */
+    if (s.d_raw[1] && j + 1 < (int64_t)s.chunks.size() && s.raw_holds[b ^ 1] != j + 1)
+        if ((st = enqueue_h2d(s, j + 1, b ^ 1, host_input, row_stride_bytes, false)) != AA_OK) return st;
+    return AA_OK;
+}
+
+extern "C" aa_status aa_run_dedispersion_device(aa_strategy* h, const uint8_t* device_chunk, size_t row_stride_bytes) {
+    aa_status st = check_ready(h, "aa_run_dedispersion_device");
+    if (st != AA_OK) return st;
+    Strategy& s = h->s;
+    if (!device_chunk) { set_error("aa_run_dedispersion_device: device_chunk is NULL"); return AA_ERR_INVALID_ARG; }
+    if (s.pending_sps) { set_error("aa_run_dedispersion_device: chunk %lld is dedispersed but aa_run_sps has not run on it yet", (long long)s.current_chunk); return AA_ERR_ORDER; }
+    if (s.next_chunk >= (int64_t)s.chunks.size()) { set_error("aa_run_dedispersion_device: all %zu chunks are done", s.chunks.size()); return AA_ERR_ORDER; }
+    const int64_t j = s.next_chunk;
+    const Chunk& c = s.chunks[(size_t)j];
+    if (row_stride_bytes < c.len) { set_error("aa_run_dedispersion_device: row_stride_bytes = %zu is shorter than the chunk (%llu)", row_stride_bytes, (unsigned long long)c.len); return AA_ERR_INVALID_ARG; }
+    const int b = s.d_raw[1] ? (int)(j & 1) : 0;
+    s.h2d_timed = false;
+    AA_CUDA(cudaMemcpy2DAsync(s.d_raw[b], s.in_pitch, device_chunk, row_stride_bytes, (size_t)c.len, (size_t)s.plan.nchans,
+                              cudaMemcpyDeviceToDevice, s.compute), "cudaMemcpy2DAsync (D2D chunk)");
+    s.raw_holds[b] = j;
+    return enqueue_dedispersion(s, j, b);
+}
+
+extern "C" aa_status aa_run_sps(aa_strategy* h) {
+    aa_status st = check_ready(h, "aa_run_sps");
+    if (st != AA_OK) return st;
+    Strategy& s = h->s;
+    if (!s.pending_sps) { set_error("aa_run_sps: no dedispersed chunk is pending — aa_run_dedispersion must run first"); return AA_ERR_ORDER; }
+    if ((st = harvest(s)) != AA_OK) return st;      /* previous chunk's records leave the device buffer first */
+    const int64_t j = s.current_chunk;
+    const Chunk& c = s.chunks[(size_t)j];
+    const bool is_short = c.len != (uint64_t)s.L;
+    AA_CUDA(cudaMemsetAsync(s.d_counter, 0, sizeof(unsigned long long), s.compute), "cudaMemsetAsync");
+    AA_CUDA(cudaEventRecord(s.ev_t[3], s.compute), "cudaEventRecord");
+    AA_LAUNCH(aak_row_stats(s.d_rows[is_short ? 1 : 0], (int32_t)s.nrows, s.d_mu_sigma, s.d_n_iters, s.compute), "row statistics");
+    AA_CUDA(cudaEventRecord(s.ev_t[4], s.compute), "cudaEventRecord");
+    for (Range& rg : s.ranges) {
+        aak_sps_args a;
+        a.D = rg.d_D; a.pitch = rg.pitch; a.nt = (int64_t)(c.n_out / (uint64_t)rg.r.bin); a.ndms = rg.r.ndms; a.bin = rg.r.bin;
+        a.range_index = rg.index; a.dm_low = rg.r.dm_low; a.dm_step = rg.r.dm_step;
+        a.mu_sigma = s.d_mu_sigma + 2 * rg.first_row; a.chunk_start = c.start;
+        a.nwidths = (int32_t)s.plan.widths.size();
+        for (int k = 0; k < 16; ++k) a.widths[k] = k < a.nwidths ? s.plan.widths[(size_t)k] : 0;
+        a.threshold = (double)s.plan.threshold;
+        a.cands = s.d_cands; a.counter = s.d_counter; a.capacity = s.max_candidates;
+        AA_LAUNCH(aak_sps_peaks(&a, s.compute), "sps peaks");
+    }
+    AA_CUDA(cudaEventRecord(s.ev_t[5], s.compute), "cudaEventRecord");
+    AA_CUDA(cudaMemcpyAsync(s.h_counter, s.d_counter, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s.compute), "counter D2H");
+    AA_CUDA(cudaEventRecord(s.ev_count, s.compute), "cudaEventRecord");
+    s.harvest_pending = true; s.harvest_chunk = j; s.stats_timed = true;
+    s.pending_sps = false;
+    s.next_chunk = j + 1;
+    return s.next_chunk >= (int64_t)s.chunks.size() ? AA_STATUS_FINISHED : AA_STATUS_CHUNK_DONE;
+}
+
+extern "C" aa_status aa_get_candidates(aa_strategy* h, const aa_candidate** out, size_t* n) {
+    aa_status st = check_ready(h, "aa_get_candidates");
+    if (st != AA_OK) return st;
+    Strategy& s = h->s;
+    if (!out || !n) { set_error("aa_get_candidates: NULL output argument"); return AA_ERR_INVALID_ARG; }
+    if ((st = harvest(s)) != AA_OK) return st;
+    *out = s.cands.data();
+    *n = s.cands.size();
+    if (s.overflow) {
+        set_error("aa_get_candidates: %llu candidates were found but max_candidates = %zu; %zu are returned", (unsigned long long)s.true_count, s.max_candidates, s.cands.size());
+        return AA_ERR_CANDIDATE_OVERFLOW;
+    }
+    return AA_OK;
+}
+
+extern "C" aa_status aa_strategy_reset(aa_strategy* h) {
+    if (!h) { set_error("aa_strategy_reset: strategy is NULL"); return AA_ERR_NOT_READY; }
+    Strategy& s = h->s;
+    cudaStreamSynchronize(s.compute);
+    cudaStreamSynchronize(s.copy);
+    s.next_chunk = 0; s.current_chunk = -1; s.pending_sps = false; s.harvest_pending = false;
+    s.raw_holds[0] = s.raw_holds[1] = -1;
+    s.cands.clear(); s.true_count = 0; s.overflow = false; s.launches = 0; s.timed = false; s.stats_timed = false;
+    if (s.sticky != AA_ERR_CUDA) s.sticky = AA_OK;
+    return AA_OK;
+}
+
+extern "C" aa_status aa_synchronize(aa_strategy* h) {
+    aa_status st = check_ready(h, "aa_synchronize");
+    if (st != AA_OK) return st;
+    Strategy& s = h->s;
+    AA_CUDA(cudaStreamSynchronize(s.compute), "cudaStreamSynchronize");
+    AA_CUDA(cudaStreamSynchronize(s.copy), "cudaStreamSynchronize");
+    return AA_OK;
+}
+
+extern "C" aa_status aa_get_dedispersed_row(aa_strategy* h, int32_t range, int32_t dm_index, const int32_t** host_row, size_t* len) {
+    aa_status st = check_ready(h, "aa_get_dedispersed_row");
+    if (st != AA_OK) return st;
+    Strategy& s = h->s;
+    if (s.current_chunk < 0) { set_error("aa_get_dedispersed_row: no chunk has been dedispersed yet"); return AA_ERR_ORDER; }
+    if (!host_row || !len || range < 0 || range >= (int32_t)s.ranges.size() || dm_index < 0 || dm_index >= s.ranges[(size_t)range].r.ndms) {
+        set_error("aa_get_dedispersed_row: range %d / dm_index %d out of bounds", range, dm_index); return AA_ERR_INVALID_ARG;
+    }
+    const Range& rg = s.ranges[(size_t)range];
+    const size_t nt = (size_t)(s.chunks[(size_t)s.current_chunk].n_out / (uint64_t)rg.r.bin);
+    s.host_row.resize(nt);
+    AA_CUDA(cudaMemcpyAsync(s.host_row.data(), rg.d_D + (size_t)dm_index * (size_t)rg.pitch, nt * 4, cudaMemcpyDeviceToHost, s.compute), "row D2H");
+    AA_CUDA(cudaStreamSynchronize(s.compute), "cudaStreamSynchronize");
+    *host_row = s.host_row.data();
+    *len = nt;
+    return AA_OK;
+}
+
+extern "C" aa_status aa_get_dedispersed_device(aa_strategy* h, int32_t range, const int32_t** device_ptr, int64_t* row_pitch) {
+    aa_status st = check_ready(h, "aa_get_dedispersed_device");
+    if (st != AA_OK) return st;
+    Strategy& s = h->s;
+    if (!device_ptr || !row_pitch || range < 0 || range >= (int32_t)s.ranges.size()) { set_error("aa_get_dedispersed_device: bad argument"); return AA_ERR_INVALID_ARG; }
+    *device_ptr = s.ranges[(size_t)range].d_D;
+    *row_pitch = s.ranges[(size_t)range].pitch;
+    return AA_OK;
+}
+
+extern "C" aa_status aa_get_row_stats(aa_strategy* h, int32_t range, int32_t dm_index, double* mu, double* sigma, int64_t* n_kept,
+                                      int32_t* iterations) {
+    aa_status st = check_ready(h, "aa_get_row_stats");
+    if (st != AA_OK) return st;
+    Strategy& s = h->s;
+    if (!s.stats_timed) { set_error("aa_get_row_stats: aa_run_sps has not run on the current chunk"); return AA_ERR_ORDER; }
+    if (range < 0 || range >= (int32_t)s.ranges.size() || dm_index < 0 || dm_index >= s.ranges[(size_t)range].r.ndms) {
+        set_error("aa_get_row_stats: range %d / dm_index %d out of bounds", range, dm_index); return AA_ERR_INVALID_ARG;
+    }
+    const size_t row = s.ranges[(size_t)range].first_row + (size_t)dm_index;
+    double ms[2]; int64_t ni[2];
+    AA_CUDA(cudaMemcpyAsync(ms, s.d_mu_sigma + 2 * row, sizeof ms, cudaMemcpyDeviceToHost, s.compute), "stats D2H");
+    AA_CUDA(cudaMemcpyAsync(ni, s.d_n_iters + 2 * row, sizeof ni, cudaMemcpyDeviceToHost, s.compute), "stats D2H");
+    AA_CUDA(cudaStreamSynchronize(s.compute), "cudaStreamSynchronize");
+    if (mu) *mu = ms[0];
+    if (sigma) *sigma = ms[1];
+    if (n_kept) *n_kept = ni[0];
+    if (iterations) *iterations = (int32_t)ni[1];
+    return AA_OK;
+}
+
+extern "C" aa_status aa_get_row_moments(aa_strategy* h, int32_t range, int64_t* sum_d, int64_t* sum_td) {
+    aa_status st = check_ready(h, "aa_get_row_moments");
+    if (st != AA_OK) return st;
+    Strategy& s = h->s;
+    if (s.current_chunk < 0) { set_error("aa_get_row_moments: no chunk has been dedispersed yet"); return AA_ERR_ORDER; }
+    if (!sum_d || !sum_td || range < 0 || range >= (int32_t)s.ranges.size()) { set_error("aa_get_row_moments: bad argument"); return AA_ERR_INVALID_ARG; }
+    const Range& rg = s.ranges[(size_t)range];
+    const int64_t nt = (int64_t)(s.chunks[(size_t)s.current_chunk].n_out / (uint64_t)rg.r.bin);
+    long long* a = s.d_moments;
+    long long* b = s.d_moments + rg.r.ndms;
+    AA_LAUNCH(aak_row_moments(rg.d_D, rg.pitch, nt, rg.r.ndms, a, b, s.compute), "row moments");
+    AA_CUDA(cudaMemcpyAsync(sum_d, a, (size_t)rg.r.ndms * 8, cudaMemcpyDeviceToHost, s.compute), "moments D2H");
+    AA_CUDA(cudaMemcpyAsync(sum_td, b, (size_t)rg.r.ndms * 8, cudaMemcpyDeviceToHost, s.compute), "moments D2H");
+    AA_CUDA(cudaStreamSynchronize(s.compute), "cudaStreamSynchronize");
+    return AA_OK;
+}
+
+extern "C" aa_status aa_get_last_timings(aa_strategy* h, float ms_out[5]) {
+    aa_status st = check_ready(h, "aa_get_last_timings");
+    if (st != AA_OK) return st;
+    Strategy& s = h->s;
+    if (!ms_out) { set_error("aa_get_last_timings: ms_out is NULL"); return AA_ERR_INVALID_ARG; }
+    for (int i = 0; i < 5; ++i) ms_out[i] = 0.f;
+    if (!s.timed) return AA_OK;
+    AA_CUDA(cudaStreamSynchronize(s.compute), "cudaStreamSynchronize");
+    AA_CUDA(cudaEventElapsedTime(&ms_out[0], s.ev_t[0], s.ev_t[1]), "cudaEventElapsedTime");
+    AA_CUDA(cudaEventElapsedTime(&ms_out[1], s.ev_t[1], s.ev_t[2]), "cudaEventElapsedTime");
+    if (s.stats_timed) {
+        AA_CUDA(cudaEventElapsedTime(&ms_out[2], s.ev_t[3], s.ev_t[4]), "cudaEventElapsedTime");
+        AA_CUDA(cudaEventElapsedTime(&ms_out[3], s.ev_t[4], s.ev_t[5]), "cudaEventElapsedTime");
+    }
+    if (s.h2d_timed) {
+        AA_CUDA(cudaStreamSynchronize(s.copy), "cudaStreamSynchronize");
+        AA_CUDA(cudaEventElapsedTime(&ms_out[4], s.ev_h2d[0], s.ev_h2d[1]), "cudaEventElapsedTime");
+    }
+    return AA_OK;
+}
+
+extern "C" aa_status aa_get_launch_count(const aa_strategy* h, uint64_t* launches) {
+    if (!h || !launches) { set_error("aa_get_launch_count: NULL argument"); return h ? AA_ERR_INVALID_ARG : AA_ERR_NOT_READY; }
+    *launches = h->s.launches;
+    return AA_OK;
+}
+
+extern "C" aa_status aa_measure_int_add_peak(void* stream, int32_t millis, double* iadd3_per_s, double* mixed_per_s, double* sm_mhz) {
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, nsm = 0;
+    cudaError_t e;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    if ((e = cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
+    const int threads = 1024, grid = nsm;
+    uint32_t* sink = nullptr; unsigned long long* cyc = nullptr;
+    if ((e = cudaMalloc(&sink, (size_t)grid * threads * 4)) != cudaSuccess) return cuda_fail(e, "cudaMalloc (peak scratch)");
+    if ((e = cudaMalloc(&cyc, (size_t)grid * 8)) != cudaSuccess) { cudaFree(sink); return cuda_fail(e, "cudaMalloc (peak scratch)"); }
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    std::vector<unsigned long long> hc((size_t)grid);
+    double rate[2] = {0, 0}, mhz = 0;
+    aa_status ret = AA_OK;
+    if (millis < 1) millis = 1;
+    for (int mode = 0; mode < 2 && ret == AA_OK; ++mode) {
+        int iters = 4096;
+        for (int pass = 0; pass < 2; ++pass) {       /* pass 0 calibrates the iteration count */
+            cudaEventRecord(e0, st);
+            int le = aak_peak_iadd(mode, iters, grid, threads, sink, cyc, st);
+            cudaEventRecord(e1, st);
+            if (le != 0 || (e = cudaEventSynchronize(e1)) != cudaSuccess) { ret = cuda_fail(le ? (cudaError_t)le : e, "peak microbenchmark"); break; }
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            if (pass == 0) {
+                double want = (double)iters * (double)millis / std::max(1e-3, (double)ms);
+                iters = (int)std::min(2.0e9, std::max(4096.0, want));
+            } else {
+                cudaMemcpy(hc.data(), cyc, (size_t)grid * 8, cudaMemcpyDeviceToHost);
+                double sum = 0;
+                for (unsigned long long v : hc) sum += (double)v;
+                rate[mode] = (double)AAK_PEAK_ADDS_PER_THREAD_ITER * iters * (double)threads * grid / ((double)ms * 1e-3);
+                mhz = (sum / grid) / ((double)ms * 1e-3) * 1e-6;
+            }
+        }
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(sink); cudaFree(cyc);
+    if (ret != AA_OK) return ret;
+    if (iadd3_per_s) *iadd3_per_s = rate[0];
+    if (mixed_per_s) *mixed_per_s = rate[1];
+    if (sm_mhz) *sm_mhz = mhz;
+    return AA_OK;
+}

@@ -1,0 +1,447 @@
+/*
+ * aa_strategy.cpp — strategy object: "how input data are split and processed on the GPU" (§3.1).
+ * Host-only planning (delays, chunk geometry, kernel tiling, offset tables, tensor maps) plus the memory manager
+ * (§2.3): every device buffer is carved from ONE arena here; aa_run_* never allocates.
+ *
+ * Arithmetic of the delays is BASELINE.json north_star, evaluated in IEEE double in the order of DESIGN.md reading C2
+ * (this file is compiled with -ffp-contract=off):
+ *     k_c = (4.148808e3 * (1/f_c^2 - 1/f_0^2)) / tsamp;  DM_i = dm_low + i*dm_step;  delay = llround((k_c*DM_i)/bin)
+ */
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "aa_internal.h"
+
+namespace aa {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+static double dm_of(const aa_dm_range& r, int32_t i) { return r.dm_low + (double)i * r.dm_step; }
+
+static int64_t delay_calc(double k_c, double dm, int32_t bin) { return (int64_t)llround((k_c * dm) / (double)bin); }
+
+int64_t delay_of(const Strategy& s, const Range& rg, int32_t chan, int32_t dm_index) {
+    return delay_calc(s.k[(size_t)chan], dm_of(rg.r, dm_index), rg.r.bin);
+}
+
+/* Channel rows seen as overlapping 256-byte segments: a {256, nseg, 1} box lands as one linear window (k_dedisp.cu). */
+static bool make_window_map(CUtensorMap* map, void* base, size_t pitch_bytes, int32_t nchans, int32_t window_bytes) {
+    EncodeTiledFn enc = encode_fn();
+    if (!enc) { set_error("aa_strategy_setup: cuTensorMapEncodeTiled is not available from this driver"); return false; }
+    const cuuint32_t nseg = (cuuint32_t)(window_bytes / 256);
+    cuuint64_t dims[3] = {(cuuint64_t)pitch_bytes, nseg, (cuuint64_t)nchans};
+    cuuint64_t strides[2] = {256, (cuuint64_t)pitch_bytes};
+    cuuint32_t box[3] = {256, nseg, 1};
+    cuuint32_t es[3] = {1, 1, 1};
+    const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { set_error("aa_strategy_setup: cuTensorMapEncodeTiled failed with CUresult %d", (int)r); return false; }
+    return true;
+}
+
+/* Everything that depends on the chunk length L. Carves (or, on a dry arena, only measures) the device buffers. */
+static void carve(Strategy& s, int64_t L, bool two_raw) {
+    Arena& a = s.arena;
+    a.used = 0;
+    s.in_pitch = round_up((size_t)L, 256);
+    const size_t raw_bytes = (size_t)s.plan.nchans * s.in_pitch + kSlack;
+    s.d_raw[0] = (uint8_t*)a.take(raw_bytes);
+    s.d_raw[1] = two_raw ? (uint8_t*)a.take(raw_bytes) : nullptr;
+    for (int k = 0; k < 3; ++k) s.d_shift[k] = s.need_u8_copies ? (uint8_t*)a.take(raw_bytes) : nullptr;
+    for (int b = 2; b <= 8; b *= 2) {
+        bool used = false;
+        for (const Range& rg : s.ranges) used = used || rg.r.bin == b;
+        s.xb_pitch[b] = used ? round_up((size_t)(L / b), 256) : 0;
+        for (int k = 0; k < 2; ++k)
+            s.d_xb[b][k] = used ? (uint16_t*)a.take((size_t)s.plan.nchans * s.xb_pitch[b] * 2 + kSlack) : nullptr;
+    }
+    const int64_t n_out = L - s.S;
+    for (Range& rg : s.ranges) {
+        rg.nt_full = n_out / rg.r.bin;
+        rg.pitch = (int64_t)round_up((size_t)rg.nt_full, 128);
+        rg.d_D = (int32_t*)a.take((size_t)rg.r.ndms * (size_t)rg.pitch * 4);
+        rg.d_etab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * kDmTile * 4);
+        rg.d_x0tab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * 4);
+    }
+    s.d_rows[0] = (aak_row_desc*)a.take(s.nrows * sizeof(aak_row_desc));
+    s.d_rows[1] = (aak_row_desc*)a.take(s.nrows * sizeof(aak_row_desc));
+    s.d_mu_sigma = (double*)a.take(s.nrows * 2 * sizeof(double));
+    s.d_n_iters = (int64_t*)a.take(s.nrows * 2 * sizeof(int64_t));
+    s.d_cands = (aak_candidate*)a.take(s.max_candidates * sizeof(aak_candidate));
+    s.d_counter = (unsigned long long*)a.take(256);
+    int32_t maxnd = 0;
+    for (const Range& rg : s.ranges) maxnd = std::max(maxnd, rg.r.ndms);
+    s.d_moments = (long long*)a.take((size_t)2 * maxnd * sizeof(long long));
+    a.used = round_up(a.used, 256);
+}
+
+static std::vector<Chunk> make_chunks(uint64_t nsamp, int64_t B, int64_t S, int64_t L) {
+    std::vector<Chunk> v;
+    const int64_t n_out = L - S;
+    const int64_t usable = (int64_t)(nsamp / (uint64_t)B) * B;
+    int64_t start = 0;
+    while (start < usable) {
+        const int64_t len = std::min<int64_t>(L, usable - start);
+        if (len <= S) break;
+        v.push_back(Chunk{(uint64_t)start, (uint64_t)len, (uint64_t)(len - S)});
+        if (len < L) break;
+        start += n_out;
+    }
+    return v;
+}
+
+/* Kernel tiling and offset tables of one range (host side). Returns false with the error set. */
+static bool plan_range(Strategy& s, Range& rg, std::vector<int32_t>& etab, std::vector<int32_t>& x0tab) {
+    const int32_t C = s.plan.nchans, nd = rg.r.ndms;
+    rg.in16 = rg.r.bin > 1; rg.esz = rg.in16 ? 2 : 1; rg.spw = 4 / rg.esz; rg.ncopy = rg.spw;
+    rg.delays.resize((size_t)nd * C);
+    for (int32_t i = 0; i < nd; ++i) {
+        const double dm = dm_of(rg.r, i);
+        int32_t* row = rg.delays.data() + (size_t)i * C;
+        for (int32_t c = 0; c < C; ++c) {
+            const int64_t d = delay_calc(s.k[(size_t)c], dm, rg.r.bin);
+            if (d < 0 || d > 0x3fffffff) { set_error("aa_strategy_setup: delay(%d, range %d, %d) = %lld out of range", c, rg.index, i, (long long)d); return false; }
+            row[c] = (int32_t)d;
+        }
+    }
+    rg.max_delay = rg.delays[(size_t)(nd - 1) * C + (C - 1)];
+    rg.ndm_tiles = (nd + kDmTile - 1) / kDmTile;
+    /* widest window: T_TILE + largest in-tile delay spread + alignment residue (< 16 bytes) */
+    int64_t omax = 0;
+    for (int32_t t = 0; t < rg.ndm_tiles; ++t) {
+        const int32_t i0 = t * kDmTile, i1 = std::min(nd - 1, i0 + kDmTile - 1);
+        const int32_t* a = rg.delays.data() + (size_t)i0 * C;
+        const int32_t* b = rg.delays.data() + (size_t)i1 * C;
+        for (int32_t c = 0; c < C; ++c) omax = std::max<int64_t>(omax, (int64_t)b[c] - a[c]);
+    }
+    const int64_t wsamp = kTTile + omax + 16 / rg.esz;
+    rg.window_bytes = (int32_t)round_up((size_t)(wsamp * rg.esz), 256);
+    if (rg.window_bytes > 65536) { set_error("aa_strategy_setup: range %d needs a %d-byte channel window per DM tile (> 65536): DM step too coarse for this band", rg.index, rg.window_bytes); return false; }
+    rg.chan_block = 0;
+    for (int cb = 8; cb >= 2; cb /= 2)
+        if (aak_dedisperse_smem_bytes(cb, rg.window_bytes, rg.in16) <= 227 * 1024) { rg.chan_block = cb; break; }
+    if (!rg.chan_block) { set_error("aa_strategy_setup: range %d: channel window of %d bytes does not fit shared memory", rg.index, rg.window_bytes); return false; }
+    rg.nstages = (C + rg.chan_block - 1) / rg.chan_block;
+    rg.spill_stages = (256 / rg.r.bin) / rg.chan_block;
+    const int32_t CB = rg.chan_block, Cpad = rg.nstages * CB, WB = rg.window_bytes;
+    etab.assign((size_t)rg.ndm_tiles * Cpad * kDmTile, 0);
+    x0tab.assign((size_t)rg.ndm_tiles * Cpad, 0);
+    for (int32_t t = 0; t < rg.ndm_tiles; ++t) {
+        const int32_t i0 = t * kDmTile;
+        for (int32_t c = 0; c < Cpad; ++c) {
+            int32_t* e = etab.data() + ((size_t)t * Cpad + c) * kDmTile;     /* [tile][stage][c_local][m] */
+            const int32_t cl = c % CB;
+            if (c >= C) {                                                   /* padding channel: TMA zero-fills it */
+                for (int m = 0; m < kDmTile; ++m) e[m] = cl * WB;
+                continue;
+            }
+            const int64_t d0 = rg.delays[(size_t)i0 * C + c];
+            const int64_t xs = d0 * rg.esz, xa = xs & ~(int64_t)15;
+            const int64_t res = (xs - xa) / rg.esz;                         /* samples folded into the offsets */
+            x0tab[(size_t)t * Cpad + c] = (int32_t)xa;
+            for (int m = 0; m < kDmTile; ++m) {
+                const int32_t i = std::min(nd - 1, i0 + m);
+                const int64_t o = (int64_t)rg.delays[(size_t)i * C + c] - d0 + res;
+                const int64_t copy = o & (rg.spw - 1);
+                e[m] = (int32_t)((copy * CB + cl) * WB + (o - copy) * rg.esz);
+            }
+        }
+    }
+    return true;
+}
+
+/* Host-only part of the setup: delays, overlap, tiling, tables, chunk length under `limit` bytes (0 = unlimited). */
+static aa_status plan_host(aa_strategy* h, const aa_plan* plan, uint64_t nsamp_total, size_t limit, size_t max_candidates,
+                           uint64_t chunk_len_hint, std::vector<std::vector<int32_t>>& etabs, std::vector<std::vector<int32_t>>& x0tabs,
+                           size_t* bytes_needed) {
+    Strategy& s = h->s;
+    s.plan = plan->p;
+    s.nsamp_total = nsamp_total;
+    s.max_candidates = max_candidates;
+    const int32_t C = s.plan.nchans;
+
+    /* delays and overlap (reading C2, C3) */
+    s.k.resize((size_t)C);
+    const double f0 = s.plan.freq[0];
+    for (int32_t c = 0; c < C; ++c) {
+        const double f = s.plan.freq[(size_t)c];
+        s.k[(size_t)c] = (4.148808e3 * (1.0 / (f * f) - 1.0 / (f0 * f0))) / s.plan.tsamp;
+    }
+    s.B = 1;
+    for (const aa_dm_range& r : s.plan.ranges) s.B = std::max(s.B, r.bin);
+    s.ranges.resize(s.plan.ranges.size());
+    etabs.resize(s.ranges.size()); x0tabs.resize(s.ranges.size());
+    int64_t smax = 0;
+    s.nrows = 0;
+    for (size_t r = 0; r < s.ranges.size(); ++r) {
+        Range& rg = s.ranges[r];
+        rg.r = s.plan.ranges[r];
+        rg.index = (int32_t)r;
+        if (!plan_range(s, rg, etabs[r], x0tabs[r])) return AA_ERR_INVALID_ARG;
+        smax = std::max<int64_t>(smax, rg.max_delay * rg.r.bin);
+        rg.first_row = s.nrows;
+        s.nrows += (size_t)rg.r.ndms;
+        if (rg.r.bin == 1) s.need_u8_copies = true;
+    }
+    s.S = (int64_t)round_up((size_t)smax, (size_t)s.B);
+    const int64_t usable = (int64_t)(nsamp_total / (uint64_t)s.B) * s.B;
+    if (usable <= s.S) {
+        set_error("aa_strategy_setup: nsamp_total = %llu is not longer than the maximum delay %lld samples", (unsigned long long)nsamp_total, (long long)s.S);
+        return AA_ERR_INVALID_ARG;
+    }
+
+    /* chunk length under the budget (reading C3): whole observation if it fits, else the largest power of two */
+    s.arena.dry = true; s.arena.base = nullptr; s.arena.size = 0;
+    auto need = [&](int64_t L) { const bool two = (L < usable); carve(s, L, two); return s.arena.used; };
+    int64_t L = 0;
+    if (chunk_len_hint) {
+        L = (int64_t)chunk_len_hint;
+        if (L % s.B || L <= s.S) { set_error("aa_strategy_setup: chunk_len_hint = %lld must be a multiple of %d and > overlap %lld", (long long)L, s.B, (long long)s.S); return AA_ERR_INVALID_ARG; }
+        if (L > usable) L = usable;
+        if (limit && need(L) > limit) { set_error("aa_strategy_setup: chunk_len_hint = %lld needs %zu bytes, budget is %zu", (long long)L, need(L), limit); return AA_ERR_BUDGET_TOO_SMALL; }
+    } else if (!limit || need(usable) <= limit) {
+        L = usable;
+    } else {
+        int64_t p2 = 1;
+        while (p2 <= s.S) p2 <<= 1;
+        if (p2 % s.B) p2 = (int64_t)round_up((size_t)p2, (size_t)s.B);
+        if (p2 >= usable || need(p2) > limit) {
+            set_error("aa_strategy_setup: budget of %zu bytes is too small: the smallest chunk (%lld samples, overlap %lld) needs %zu bytes",
+                      limit, (long long)p2, (long long)s.S, need(std::min(p2, usable)));
+            return AA_ERR_BUDGET_TOO_SMALL;
+        }
+        while (p2 * 2 < usable && need(p2 * 2) <= limit) p2 *= 2;
+        L = p2;
+    }
+    s.L = L;
+    s.n_out = L - s.S;
+    s.chunks = make_chunks(nsamp_total, s.B, s.S, L);
+    carve(s, L, s.chunks.size() > 1);
+    *bytes_needed = s.arena.used;
+    return AA_OK;
+}
+
+}  // namespace aa
+
+using namespace aa;
+
+extern "C" aa_status aa_strategy_plan(aa_strategy** out, const aa_plan* plan, uint64_t nsamp_total, size_t budget_bytes,
+                                      size_t max_candidates, uint64_t chunk_len_hint) {
+    if (!out) { set_error("aa_strategy_plan: out is NULL"); return AA_ERR_INVALID_ARG; }
+    *out = nullptr;
+    if (!plan) { set_error("aa_strategy_plan: plan is NULL (configure a plan first)"); return AA_ERR_NOT_READY; }
+    if (max_candidates < 1) { set_error("aa_strategy_plan: max_candidates must be >= 1"); return AA_ERR_INVALID_ARG; }
+    aa_strategy* h = new (std::nothrow) aa_strategy();
+    if (!h) { set_error("aa_strategy_plan: out of host memory"); return AA_ERR_INTERNAL; }
+    std::vector<std::vector<int32_t>> etabs, x0tabs;
+    size_t bytes = 0;
+    const aa_status st = plan_host(h, plan, nsamp_total, budget_bytes, max_candidates, chunk_len_hint, etabs, x0tabs, &bytes);
+    if (st != AA_OK) { delete h; return st; }
+    h->s.arena.size = 0;
+    h->s.ready = false;
+    *out = h;
+    return AA_OK;
+}
+
+extern "C" aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, uint64_t nsamp_total, void* device_arena,
+                                       size_t arena_bytes, size_t budget_bytes, void* compute_stream, void* copy_stream,
+                                       size_t max_candidates, uint64_t chunk_len_hint) {
+    if (!out) { set_error("aa_strategy_setup: out is NULL"); return AA_ERR_INVALID_ARG; }
+    *out = nullptr;
+    if (!plan) { set_error("aa_strategy_setup: plan is NULL (configure and bind a plan first)"); return AA_ERR_NOT_READY; }
+    if (max_candidates < 1) { set_error("aa_strategy_setup: max_candidates must be >= 1"); return AA_ERR_INVALID_ARG; }
+    if (device_arena && ((uintptr_t)device_arena & 255)) { set_error("aa_strategy_setup: device_arena must be 256-byte aligned"); return AA_ERR_INVALID_ARG; }
+    aa_strategy* h = new (std::nothrow) aa_strategy();
+    if (!h) { set_error("aa_strategy_setup: out of host memory"); return AA_ERR_INTERNAL; }
+    Strategy& s = h->s;
+    auto fail = [&](aa_status st) { aa_strategy_destroy(h); return st; };
+    size_t limit = budget_bytes;
+    if (device_arena) limit = limit ? std::min(limit, arena_bytes) : arena_bytes;
+    if (!device_arena && limit == 0) {
+        size_t fr = 0, tot = 0;
+        cudaError_t e0 = cudaMemGetInfo(&fr, &tot);
+        if (e0 != cudaSuccess) return fail(cuda_fail(e0, "cudaMemGetInfo"));
+        limit = fr - std::min<size_t>(fr / 16, (size_t)1 << 30);
+    }
+    std::vector<std::vector<int32_t>> etabs, x0tabs;
+    size_t bytes_needed = 0;
+    {
+        const aa_status st = plan_host(h, plan, nsamp_total, limit, max_candidates, chunk_len_hint, etabs, x0tabs, &bytes_needed);
+        if (st != AA_OK) return fail(st);
+    }
+    const int32_t C = s.plan.nchans;
+    const int64_t L = s.L;
+    const bool two_raw = s.chunks.size() > 1;
+
+    /* the single allocation (north_star "one allocation per run") */
+    if (device_arena) {
+        if (bytes_needed > arena_bytes) { set_error("aa_strategy_setup: arena of %zu bytes is too small, %zu needed", arena_bytes, bytes_needed); return fail(AA_ERR_BUDGET_TOO_SMALL); }
+        s.arena.base = (uint8_t*)device_arena; s.arena.size = arena_bytes; s.owns_arena = false;
+    } else {
+        void* p = nullptr;
+        cudaError_t e = cudaMalloc(&p, bytes_needed);
+        if (e != cudaSuccess) { cudaGetLastError(); set_error("aa_strategy_setup: cudaMalloc of %zu bytes failed: %s", bytes_needed, cudaGetErrorString(e)); return fail(AA_ERR_BUDGET_TOO_SMALL); }
+        s.arena.base = (uint8_t*)p; s.arena.size = bytes_needed; s.owns_arena = true;
+    }
+    s.arena.dry = false;
+    carve(s, L, two_raw);
+
+    /* streams, events, pinned counter */
+    cudaError_t e;
+    if (compute_stream) s.compute = (cudaStream_t)compute_stream;
+    else { if ((e = cudaStreamCreateWithFlags(&s.compute, cudaStreamNonBlocking)) != cudaSuccess) return fail(cuda_fail(e, "cudaStreamCreate")); s.owns_compute = true; }
+    if (copy_stream) s.copy = (cudaStream_t)copy_stream;
+    else { if ((e = cudaStreamCreateWithFlags(&s.copy, cudaStreamNonBlocking)) != cudaSuccess) return fail(cuda_fail(e, "cudaStreamCreate")); s.owns_copy = true; }
+    for (int b = 0; b < 2; ++b) {
+        if ((e = cudaEventCreateWithFlags(&s.ev_copied[b], cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
+        if ((e = cudaEventCreateWithFlags(&s.ev_raw_free[b], cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
+        if ((e = cudaEventCreate(&s.ev_h2d[b])) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
+    }
+    if ((e = cudaEventCreateWithFlags(&s.ev_count, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
+    for (int i = 0; i < 6; ++i)
+        if ((e = cudaEventCreate(&s.ev_t[i])) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
+    if ((e = cudaHostAlloc((void**)&s.h_counter, 64, cudaHostAllocDefault)) != cudaSuccess) return fail(cuda_fail(e, "cudaHostAlloc"));
+    *s.h_counter = 0;
+    if ((e = (cudaError_t)aak_dedisperse_init()) != cudaSuccess) return fail(cuda_fail(e, "kernel attribute setup (dedispersion)"));
+    if ((e = (cudaError_t)aak_sps_init()) != cudaSuccess) return fail(cuda_fail(e, "kernel attribute setup (sps)"));
+
+    /* upload tables, build tensor maps and row descriptors */
+    std::vector<aak_row_desc> rows_full(s.nrows), rows_last(s.nrows);
+    const Chunk& last = s.chunks.back();
+    for (size_t r = 0; r < s.ranges.size(); ++r) {
+        Range& rg = s.ranges[r];
+        if ((e = cudaMemcpyAsync(rg.d_etab, etabs[r].data(), etabs[r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
+        if ((e = cudaMemcpyAsync(rg.d_x0tab, x0tabs[r].data(), x0tabs[r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
+        for (int par = 0; par < 2; ++par) {
+            for (int k = 0; k < rg.ncopy; ++k) {
+                void* base; size_t pitch_bytes;
+                if (rg.in16) { base = s.d_xb[rg.r.bin][k]; pitch_bytes = s.xb_pitch[rg.r.bin] * 2; }
+                else { base = k == 0 ? (s.d_raw[par] ? s.d_raw[par] : s.d_raw[0]) : s.d_shift[k - 1]; pitch_bytes = s.in_pitch; }
+                if (!make_window_map(&rg.maps[par][k], base, pitch_bytes, C, rg.window_bytes)) return fail(AA_ERR_CUDA);
+            }
+        }
+        for (int32_t i = 0; i < rg.r.ndms; ++i) {
+            const int32_t* base = rg.d_D + (size_t)i * (size_t)rg.pitch;
+            rows_full[rg.first_row + i] = aak_row_desc{base, rg.nt_full};
+            rows_last[rg.first_row + i] = aak_row_desc{base, (int64_t)(last.n_out / (uint64_t)rg.r.bin)};
+        }
+    }
+    if ((e = cudaMemcpyAsync(s.d_rows[0], rows_full.data(), s.nrows * sizeof(aak_row_desc), cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "row table upload"));
+    if ((e = cudaMemcpyAsync(s.d_rows[1], rows_last.data(), s.nrows * sizeof(aak_row_desc), cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "row table upload"));
+    if ((e = cudaMemsetAsync(s.d_counter, 0, 256, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "cudaMemsetAsync"));
+    if ((e = cudaStreamSynchronize(s.compute)) != cudaSuccess) return fail(cuda_fail(e, "strategy upload"));   /* host tables go out of scope */
+    s.ready = true;
+    *out = h;
+    return AA_OK;
+}
+
+extern "C" void aa_strategy_destroy(aa_strategy* h) {
+    if (!h) return;
+    Strategy& s = h->s;
+    if (s.compute) cudaStreamSynchronize(s.compute);
+    if (s.copy) cudaStreamSynchronize(s.copy);
+    for (int b = 0; b < 2; ++b) {
+        if (s.ev_copied[b]) cudaEventDestroy(s.ev_copied[b]);
+        if (s.ev_raw_free[b]) cudaEventDestroy(s.ev_raw_free[b]);
+        if (s.ev_h2d[b]) cudaEventDestroy(s.ev_h2d[b]);
+    }
+    if (s.ev_count) cudaEventDestroy(s.ev_count);
+    for (int i = 0; i < 6; ++i) if (s.ev_t[i]) cudaEventDestroy(s.ev_t[i]);
+    if (s.owns_compute && s.compute) cudaStreamDestroy(s.compute);
+    if (s.owns_copy && s.copy) cudaStreamDestroy(s.copy);
+    if (s.h_counter) cudaFreeHost(s.h_counter);
+    if (s.owns_arena && s.arena.base) cudaFree(s.arena.base);
+    delete h;
+}
+
+extern "C" aa_status aa_strategy_get_info(const aa_strategy* h, aa_strategy_info* out) {
+    if (!h || !out) { set_error("aa_strategy_get_info: NULL argument"); return h ? AA_ERR_INVALID_ARG : AA_ERR_NOT_READY; }
+    const Strategy& s = h->s;
+    out->ready = s.ready ? 1 : 0;
+    out->nchans = s.plan.nchans; out->nranges = (int32_t)s.ranges.size(); out->nwidths = (int32_t)s.plan.widths.size();
+    out->max_bin = s.B; out->nsamp_total = (int64_t)s.nsamp_total; out->overlap = s.S; out->chunk_len = s.L; out->n_out = s.n_out;
+    out->nchunks = (int64_t)s.chunks.size(); out->next_chunk = s.next_chunk;
+    out->arena_bytes_used = s.arena.used; out->arena_bytes_total = s.arena.size; out->max_candidates = s.max_candidates;
+    out->owns_arena = s.owns_arena ? 1 : 0;
+    return AA_OK;
+}
+
+extern "C" aa_status aa_strategy_get_range_info(const aa_strategy* h, int32_t range, aa_range_info* out) {
+    if (!h) { set_error("aa_strategy_get_range_info: strategy is NULL"); return AA_ERR_NOT_READY; }
+    if (!out || range < 0 || range >= (int32_t)h->s.ranges.size()) { set_error("aa_strategy_get_range_info: range %d out of bounds", range); return AA_ERR_INVALID_ARG; }
+    const Range& rg = h->s.ranges[(size_t)range];
+    out->ndms = rg.r.ndms; out->bin = rg.r.bin; out->nt = rg.nt_full; out->row_pitch = rg.pitch; out->max_delay = rg.max_delay;
+    out->dm_tile = kDmTile; out->t_tile = kTTile; out->chan_block = rg.chan_block; out->window = rg.window_bytes;
+    return AA_OK;
+}
+
+extern "C" aa_status aa_strategy_get_chunk(const aa_strategy* h, int64_t chunk, uint64_t* start, uint64_t* len, uint64_t* n_out) {
+    if (!h) { set_error("aa_strategy_get_chunk: strategy is NULL"); return AA_ERR_NOT_READY; }
+    if (chunk < 0 || chunk >= (int64_t)h->s.chunks.size()) { set_error("aa_strategy_get_chunk: chunk %lld out of bounds (nchunks = %zu)", (long long)chunk, h->s.chunks.size()); return AA_ERR_INVALID_ARG; }
+    const Chunk& c = h->s.chunks[(size_t)chunk];
+    if (start) *start = c.start;
+    if (len) *len = c.len;
+    if (n_out) *n_out = c.n_out;
+    return AA_OK;
+}
+
+extern "C" aa_status aa_strategy_get_delay(const aa_strategy* h, int32_t range, int32_t dm_index, int32_t chan, int64_t* delay) {
+    if (!h) { set_error("aa_strategy_get_delay: strategy is NULL"); return AA_ERR_NOT_READY; }
+    const Strategy& s = h->s;
+    if (!delay || range < 0 || range >= (int32_t)s.ranges.size() || chan < 0 || chan >= s.plan.nchans || dm_index < 0 ||
+        dm_index >= s.ranges[(size_t)range].r.ndms) { set_error("aa_strategy_get_delay: index out of bounds"); return AA_ERR_INVALID_ARG; }
+    *delay = s.ranges[(size_t)range].delays[(size_t)dm_index * s.plan.nchans + chan];
+    return AA_OK;
+}
+
+extern "C" size_t aa_strategy_describe(const aa_strategy* h, char* buf, size_t buflen) {
+    if (!h) return 0;
+    const Strategy& s = h->s;
+    std::string o;
+    char line[512];
+    snprintf(line, sizeof line, "strategy: nchans=%d nsamp=%llu B=%d overlap S=%lld chunk L=%lld n_out=%lld nchunks=%zu\n", s.plan.nchans,
+             (unsigned long long)s.nsamp_total, s.B, (long long)s.S, (long long)s.L, (long long)s.n_out, s.chunks.size());
+    o += line;
+    snprintf(line, sizeof line, "arena: %zu bytes used of %zu (%s), input pitch %zu, raw buffers %d, uint8 shifted copies %s\n", s.arena.used,
+             s.arena.size, s.owns_arena ? "library-owned, one cudaMalloc" : "caller-owned", s.in_pitch, s.d_raw[1] ? 2 : 1,
+             s.need_u8_copies ? "3" : "none");
+    o += line;
+    for (const Range& rg : s.ranges) {
+        snprintf(line, sizeof line,
+                 "range %d: dm_low=%g step=%g ndms=%d bin=%d max_delay=%lld T=%lld pitch=%lld | tile %dx%d chan_block=%d window=%dB stages=%d "
+                 "dm_tiles=%d spill/%d smem=%zuB\n",
+                 rg.index, rg.r.dm_low, rg.r.dm_step, rg.r.ndms, rg.r.bin, (long long)rg.max_delay, (long long)rg.nt_full, (long long)rg.pitch,
+                 kDmTile, kTTile, rg.chan_block, rg.window_bytes, rg.nstages, rg.ndm_tiles, rg.spill_stages,
+                 aak_dedisperse_smem_bytes(rg.chan_block, rg.window_bytes, rg.in16));
+        o += line;
+    }
+    for (size_t j = 0; j < s.chunks.size() && j < 4; ++j) {
+        snprintf(line, sizeof line, "chunk %zu: start=%llu len=%llu n_out=%llu\n", j, (unsigned long long)s.chunks[j].start,
+                 (unsigned long long)s.chunks[j].len, (unsigned long long)s.chunks[j].n_out);
+        o += line;
+    }
+    if (s.chunks.size() > 4) {
+        const Chunk& c = s.chunks.back();
+        snprintf(line, sizeof line, "... chunk %zu: start=%llu len=%llu n_out=%llu\n", s.chunks.size() - 1, (unsigned long long)c.start,
+                 (unsigned long long)c.len, (unsigned long long)c.n_out);
+        o += line;
+    }
+    if (buf && buflen) { const size_t n = std::min(buflen - 1, o.size()); memcpy(buf, o.data(), n); buf[n] = 0; }
+    return o.size() + 1;
+}

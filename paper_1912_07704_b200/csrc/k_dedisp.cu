@@ -1,0 +1,348 @@
+/*
+ * k_dedisp.cu — K2, brute-force incoherent dedispersion for sm_100a.
+ *
+ *   D[i][t] = sum_{c<C} x_b[c][t + delay(c,i)]          (BASELINE.json north_star; every term is added individually)
+ *
+ * Design:
+ *   * A CTA owns DM_TILE = 32 DM trials x T_TILE = 1024 output samples. 16 compute warps each hold 2 DMs x 1024 samples
+ *     in registers; a 17th warp is the TMA producer. Channels stream through shared memory in blocks of CB channels,
+ *     NSTAGE-deep ring, full/empty mbarriers (no __syncthreads in the main loop).
+ *   * Shared memory holds SPW sample-shifted copies of every channel window (SPW = samples per 32-bit word: 4 for uint8,
+ *     2 for uint16), so that ANY sample offset t+delay is a word-aligned, bank-conflict-free LDS.32: copy k holds the
+ *     window shifted by k samples. TMA needs 16-byte aligned global coordinates (measured: an unaligned inner
+ *     coordinate raises an illegal-instruction fault on sm_100a), so the shifted copies exist in GLOBAL memory
+ *     (K1 writes them: x_k[c][t] = x[c][t+k]) and each is fetched by its own tensor map; the window start is aligned
+ *     down to 16 bytes and the residue is folded into the host-built offset table.
+ *   * One TMA per (copy, channel) moves the whole window: the tensor map views a channel row as OVERLAPPING 256-byte
+ *     segments (dims {pitch, nseg, C}, strides {256, pitch}), so a {256, nseg, 1} box lands as one linear run.
+ *   * Packed arithmetic (uint8): a loaded word w = (b0,b1,b2,b3) is four consecutive time samples of one channel.
+ *         A += w                      (whole word, lanes overlap at 8-bit spacing, wraps mod 2^32)
+ *         H += (b1, 0, b3, 0)         (one PRMT; two clean 16-bit lanes)
+ *     and L = A - (H << 8) = (b0 sums, b2 sums) is recovered exactly when the lanes are read, so one 32-bit add
+ *     instruction performs two (H) or four (A) algorithmic adds and only ONE unpack instruction is spent per four
+ *     samples. Two channels are folded per three-input IADD3 (A += w1 + w2); the H adds are issued as IMAD (x*1+y) so
+ *     that they run on the FMA pipe while PRMT/IADD3 use the ALU pipe. 16-bit lanes are carried into a second pair of
+ *     packed registers every 256/bin channels (255 + 256*255 = 65535 never overflows), so the result is bit-exact
+ *     int32 for any uint8 input.
+ *     uint16 (binned) input is already a pair of 16-bit lanes: A += w1 + w2, same carry rule.
+ *   * The per-(channel, DM) shared-memory offsets come from a host-built table (exact double delays), streamed with
+ *     the data by a 1-D bulk copy; inside the loop an address is one integer add.
+ */
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string.h>
+#include "aa_kernels.h"
+
+namespace {
+
+constexpr int NW = 16;               /* compute warps */
+constexpr int M = 2;                 /* DM trials per warp */
+constexpr int DM_TILE = NW * M;      /* 32 */
+constexpr int T_TILE = 1024;
+constexpr int NSTAGE = 3;
+constexpr int NTHREADS = (NW + 1) * 32;
+constexpr int SMEM_HEADER = 1024;    /* mbarriers live here; keeps the stages 1024-byte aligned */
+
+struct TmapPack { CUtensorMap m[4]; };   /* one per shifted copy */
+
+struct DedispParams {
+    const int32_t* etab;
+    const int32_t* x0tab;
+    int32_t* D;
+    long long pitch;
+    long long nt;
+    int ndms;
+    int nstages;
+    int window_bytes;
+    int boxes_per_row;
+    int spill_stages;
+    unsigned one;              /* always 1; a runtime value so that x*one+y stays an IMAD (FMA pipe) */
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "AA_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra AA_DONE;\n"
+        "bra AA_WAIT;\n"
+        "AA_DONE:\n"
+        "}\n" ::"r"(bar), "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int x, int y, int z, uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst),
+        "l"(reinterpret_cast<uint64_t>(map)), "r"(x), "r"(y), "r"(z), "r"(bar)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_load_1d(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+/* x*1 + y on the FMA pipe: `one` is a runtime 1 so ptxas keeps the IMAD. */
+__device__ __forceinline__ uint32_t add_fma_pipe(uint32_t x, uint32_t one, uint32_t y) {
+    uint32_t d;
+    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(x), "r"(one), "r"(y));
+    return d;
+}
+__device__ __forceinline__ uint32_t odd_bytes(uint32_t w) { /* (b1, 0, b3, 0) */
+    uint32_t d;
+    asm("prmt.b32 %0, %1, 0, 0x4341;" : "=r"(d) : "r"(w));
+    return d;
+}
+
+template <int IN16, int CB, int FMA_H>
+__global__ void __launch_bounds__(NTHREADS, 1)
+k_dedisperse(const __grid_constant__ TmapPack maps, const DedispParams p) {
+    constexpr int ESZ = IN16 ? 2 : 1;
+    constexpr int SPW = 4 / ESZ;                 /* samples per word */
+    constexpr int NCOPY = SPW;                   /* shifted copies */
+    constexpr int J = T_TILE / (32 * SPW);       /* words per thread per DM: 8 (u8) or 16 (u16) */
+    constexpr int ENT_BYTES = CB * DM_TILE * 4;
+
+    extern __shared__ __align__(1024) uint8_t smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int ndm_tiles = (p.ndms + DM_TILE - 1) / DM_TILE;
+    const int dt = blockIdx.x % ndm_tiles;       /* DM tile fastest: concurrent CTAs share the same input windows in L2 */
+    const int tt = blockIdx.x / ndm_tiles;
+    const long long t0 = (long long)tt * T_TILE;
+    const int WB = p.window_bytes;
+    const int data_bytes = NCOPY * CB * WB;
+    const int stage_bytes = data_bytes + ENT_BYTES;
+    const uint32_t bar_full = smem_u32(smem);            /* NSTAGE x 8 bytes */
+    const uint32_t bar_empty = bar_full + 8 * NSTAGE;
+    uint8_t* const stages = smem + SMEM_HEADER;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NSTAGE; ++s) {
+            mbar_init(bar_full + 8 * s, 1);
+            mbar_init(bar_empty + 8 * s, NW);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp == NW) {
+        /* ------------------------------------------------------------------ producer warp */
+        const int32_t* x0row = p.x0tab + (size_t)dt * (size_t)p.nstages * CB;
+        const int32_t* erow = p.etab + (size_t)dt * (size_t)p.nstages * (CB * DM_TILE);
+        const int c_local = lane % CB, copy = lane / CB;
+        const bool active = lane < NCOPY * CB;
+        const int box_bytes = WB / p.boxes_per_row;
+        int slot = 0; uint32_t ph = 0;
+        for (int s = 0; s < p.nstages; ++s) {
+            const int x0 = active ? __ldg(x0row + s * CB + c_local) : 0;
+            mbar_wait(bar_empty + 8 * slot, ph ^ 1u);
+            const uint32_t fb = bar_full + 8 * slot;
+            if (lane == 0) mbar_arrive_expect_tx(fb, (uint32_t)stage_bytes);
+            __syncwarp();
+            const uint32_t sbase = smem_u32(stages + (size_t)slot * stage_bytes);
+            if (active) {
+                const long long xs = t0 * ESZ + x0;                    /* 16-byte aligned byte coordinate of the window */
+                const int xi = xs > 0x7fff0000ll ? 0x7fff0000 : (int)xs; /* far out of bounds is zero-filled anyway */
+                const uint32_t dst = sbase + (uint32_t)((copy * CB + c_local) * WB);
+                for (int b = 0; b < p.boxes_per_row; ++b)
+                    tma_load_3d(dst + b * box_bytes, &maps.m[copy], xi + b * box_bytes, 0, s * CB + c_local, fb);
+            }
+            if (lane == 0) bulk_load_1d(sbase + data_bytes, erow + (size_t)s * (CB * DM_TILE), ENT_BYTES, fb);
+            if (++slot == NSTAGE) { slot = 0; ph ^= 1u; }
+        }
+        return;
+    }
+
+    /* ---------------------------------------------------------------------- compute warps */
+    const uint32_t one = p.one;
+    uint32_t A[M][J], C1[M][J];
+    uint32_t H[IN16 ? 1 : M][IN16 ? 1 : J], C2[IN16 ? 1 : M][IN16 ? 1 : J];
+#pragma unroll
+    for (int m = 0; m < M; ++m)
+#pragma unroll
+        for (int j = 0; j < J; ++j) {
+            A[m][j] = 0; C1[m][j] = 0;
+            if (!IN16) { H[m][j] = 0; C2[m][j] = 0; }
+        }
+
+    const int ent_off = data_bytes + warp * M * 4;
+    int until_spill = p.spill_stages;
+    int slot = 0; uint32_t ph = 0;
+    for (int s = 0; s < p.nstages; ++s) {
+        mbar_wait(bar_full + 8 * slot, ph);
+        const uint8_t* sb = stages + (size_t)slot * stage_bytes;
+        const uint8_t* db = sb + lane * 4;
+#pragma unroll
+        for (int cp = 0; cp < CB / 2; ++cp) {
+            const uint2 e1 = *reinterpret_cast<const uint2*>(sb + ent_off + (2 * cp) * (DM_TILE * 4));
+            const uint2 e2 = *reinterpret_cast<const uint2*>(sb + ent_off + (2 * cp + 1) * (DM_TILE * 4));
+#pragma unroll
+            for (int m = 0; m < M; ++m) {
+                const uint8_t* a1 = db + (m == 0 ? e1.x : e1.y);
+                const uint8_t* a2 = db + (m == 0 ? e2.x : e2.y);
+#pragma unroll
+                for (int j = 0; j < J; ++j) {
+                    const uint32_t w1 = *reinterpret_cast<const uint32_t*>(a1 + j * 128);
+                    const uint32_t w2 = *reinterpret_cast<const uint32_t*>(a2 + j * 128);
+                    A[m][j] = A[m][j] + w1 + w2;
+                    if (!IN16) {
+                        if (FMA_H) {
+                            H[m][j] = add_fma_pipe(odd_bytes(w1), one, H[m][j]);
+                            H[m][j] = add_fma_pipe(odd_bytes(w2), one, H[m][j]);
+                        } else {
+                            H[m][j] = H[m][j] + odd_bytes(w1) + odd_bytes(w2);
+                        }
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_empty + 8 * slot);
+        if (++slot == NSTAGE) { slot = 0; ph ^= 1u; }
+        if (--until_spill == 0) {
+            until_spill = p.spill_stages;
+#pragma unroll
+            for (int m = 0; m < M; ++m)
+#pragma unroll
+                for (int j = 0; j < J; ++j) {
+                    if (!IN16) {
+                        uint32_t L = A[m][j] - (H[m][j] << 8);
+                        C1[m][j] += (L >> 8) & 0x00FF00FFu;
+                        C2[m][j] += (H[m][j] >> 8) & 0x00FF00FFu;
+                        L &= 0x00FF00FFu;
+                        H[m][j] &= 0x00FF00FFu;
+                        A[m][j] = L + (H[m][j] << 8);
+                    } else {
+                        C1[m][j] += (A[m][j] >> 8) & 0x00FF00FFu;
+                        A[m][j] &= 0x00FF00FFu;
+                    }
+                }
+        }
+    }
+
+    /* ---------------------------------------------------------------------- unpack and store */
+#pragma unroll
+    for (int m = 0; m < M; ++m) {
+        const int i = dt * DM_TILE + warp * M + m;
+        if (i >= p.ndms) continue;
+        int32_t* row = p.D + (size_t)i * (size_t)p.pitch;
+#pragma unroll
+        for (int j = 0; j < J; ++j) {
+            const long long t = t0 + (long long)(j * 32 + lane) * SPW;
+            if (t >= p.nt) continue;
+            if (!IN16) {
+                const uint32_t L = A[m][j] - (H[m][j] << 8);
+                int4 v;
+                v.x = (int)((L & 0xFFFFu) + ((C1[m][j] & 0xFFFFu) << 8));
+                v.y = (int)((H[m][j] & 0xFFFFu) + ((C2[m][j] & 0xFFFFu) << 8));
+                v.z = (int)((L >> 16) + ((C1[m][j] >> 16) << 8));
+                v.w = (int)((H[m][j] >> 16) + ((C2[m][j] >> 16) << 8));
+                *reinterpret_cast<int4*>(row + t) = v;
+            } else {
+                int2 v;
+                v.x = (int)((A[m][j] & 0xFFFFu) + ((C1[m][j] & 0xFFFFu) << 8));
+                v.y = (int)((A[m][j] >> 16) + ((C1[m][j] >> 16) << 8));
+                *reinterpret_cast<int2*>(row + t) = v;
+            }
+        }
+    }
+}
+
+template <typename T>
+__global__ void k_dedisperse_naive(const T* __restrict__ x, size_t pitch, const int32_t* __restrict__ delays, int nchans,
+                                   int ndms, long long nt, int32_t* __restrict__ D, long long dpitch) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = blockIdx.y;
+    if (t >= nt || i >= ndms) return;
+    const int32_t* dl = delays + (size_t)i * nchans;
+    int acc = 0;
+    for (int c = 0; c < nchans; ++c) acc += (int)x[(size_t)c * pitch + (size_t)(t + dl[c])];
+    D[(size_t)i * dpitch + t] = acc;
+}
+
+template <int IN16, int CB, int FMA_H>
+int launch(const aak_dedisp_args* a, cudaStream_t st) {
+    constexpr int NCOPY = IN16 ? 2 : 4;
+    DedispParams p;
+    p.etab = a->etab; p.x0tab = a->x0tab; p.D = a->D; p.pitch = a->pitch; p.nt = a->nt; p.ndms = a->ndms;
+    p.nstages = (a->nchans + CB - 1) / CB;
+    p.window_bytes = a->window_bytes; p.boxes_per_row = a->boxes_per_row; p.spill_stages = a->spill_stages; p.one = 1u;
+    const size_t smem = SMEM_HEADER + (size_t)NSTAGE * ((size_t)NCOPY * CB * a->window_bytes + CB * DM_TILE * 4);
+    const long long ndm_tiles = (a->ndms + DM_TILE - 1) / DM_TILE;
+    const long long nt_tiles = (a->nt + T_TILE - 1) / T_TILE;
+    const long long grid = ndm_tiles * nt_tiles;
+    if (grid <= 0 || grid > 0x7fffffffll) return (int)cudaErrorInvalidConfiguration;
+    TmapPack maps;
+    memset(&maps, 0, sizeof(maps));
+    memcpy(&maps, a->tmap, sizeof(CUtensorMap) * NCOPY);
+    k_dedisperse<IN16, CB, FMA_H><<<(unsigned)grid, NTHREADS, smem, st>>>(maps, p);
+    return (int)cudaGetLastError();
+}
+
+template <int IN16, int CB, int FMA_H>
+int set_attr() {
+    return (int)cudaFuncSetAttribute(k_dedisperse<IN16, CB, FMA_H>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+}
+
+}  // namespace
+
+extern "C" size_t aak_dedisperse_smem_bytes(int32_t chan_block, int32_t window_bytes, int32_t in16) {
+    const size_t ncopy = in16 ? 2 : 4;
+    return SMEM_HEADER + (size_t)NSTAGE * (ncopy * chan_block * (size_t)window_bytes + (size_t)chan_block * DM_TILE * 4);
+}
+
+extern "C" int aak_dedisperse_init(void) {
+    int e = 0;
+    if ((e = set_attr<0, 8, 0>())) return e;
+    if ((e = set_attr<0, 4, 0>())) return e;
+    if ((e = set_attr<0, 2, 0>())) return e;
+    if ((e = set_attr<0, 8, 1>())) return e;
+    if ((e = set_attr<0, 4, 1>())) return e;
+    if ((e = set_attr<0, 2, 1>())) return e;
+    if ((e = set_attr<1, 8, 0>())) return e;
+    if ((e = set_attr<1, 4, 0>())) return e;
+    if ((e = set_attr<1, 2, 0>())) return e;
+    return 0;
+}
+
+extern "C" int aak_dedisperse(const aak_dedisp_args* a, void* stream) {
+    cudaStream_t st = (cudaStream_t)stream;
+    if (a->in16) {
+        switch (a->chan_block) {
+            case 8: return launch<1, 8, 0>(a, st);
+            case 4: return launch<1, 4, 0>(a, st);
+            case 2: return launch<1, 2, 0>(a, st);
+        }
+    } else {
+        switch (a->chan_block) {
+            case 8: return a->variant ? launch<0, 8, 1>(a, st) : launch<0, 8, 0>(a, st);
+            case 4: return a->variant ? launch<0, 4, 1>(a, st) : launch<0, 4, 0>(a, st);
+            case 2: return a->variant ? launch<0, 2, 1>(a, st) : launch<0, 2, 0>(a, st);
+        }
+    }
+    return (int)cudaErrorInvalidValue;
+}
+
+extern "C" int aak_dedisperse_naive(const void* x, size_t pitch_elems, int32_t in16, const int32_t* delays, int32_t nchans,
+                                    int32_t ndms, int64_t nt, int32_t* D, int64_t pitch, void* stream) {
+    cudaStream_t st = (cudaStream_t)stream;
+    dim3 grid((unsigned)((nt + 255) / 256), (unsigned)ndms);
+    if (in16)
+        k_dedisperse_naive<uint16_t><<<grid, 256, 0, st>>>((const uint16_t*)x, pitch_elems, delays, nchans, ndms, nt, D, pitch);
+    else
+        k_dedisperse_naive<uint8_t><<<grid, 256, 0, st>>>((const uint8_t*)x, pitch_elems, delays, nchans, ndms, nt, D, pitch);
+    return (int)cudaGetLastError();
+}

@@ -1,0 +1,152 @@
+/*
+ * k_misc.cu — K1 (time binning), K5 (row-moment test hook) and K0 (integer-add peak microbenchmark) for sm_100a.
+ */
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "aa_kernels.h"
+
+namespace {
+
+/* ---- K1: x_b[c][t'] = sum_{j<b} x[c][b*t'+j] (north_star "DM ranges that decimate in time by 1/2/4/8";
+ * DESIGN.md reading C4: binning is a SUM held in uint16). One thread turns 16 input bytes into 16/b outputs. */
+template <int B>
+__global__ void __launch_bounds__(256)
+k_bin_time(const uint8_t* __restrict__ x, size_t x_pitch, uint16_t* __restrict__ xb, size_t xb_pitch, long long ngroups) {
+    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= ngroups) return;
+    const int c = blockIdx.y;
+    const uint4 v = *reinterpret_cast<const uint4*>(x + (size_t)c * x_pitch + (size_t)g * 16);
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+    uint16_t o[16 / B];
+#pragma unroll
+    for (int k = 0; k < 16 / B; ++k) {
+        uint32_t s = 0;
+#pragma unroll
+        for (int j = 0; j < B; ++j) {
+            const int byte = k * B + j;
+            s += (w[byte >> 2] >> (8 * (byte & 3))) & 0xFFu;
+        }
+        o[k] = (uint16_t)s;
+    }
+    uint16_t* dst = xb + (size_t)c * xb_pitch + (size_t)g * (16 / B);
+    if (B == 2) {
+        uint4 r;
+        r.x = o[0] | ((uint32_t)o[1] << 16); r.y = o[2] | ((uint32_t)o[3] << 16);
+        r.z = o[4] | ((uint32_t)o[5] << 16); r.w = o[6] | ((uint32_t)o[7] << 16);
+        *reinterpret_cast<uint4*>(dst) = r;
+    } else if (B == 4) {
+        uint2 r;
+        r.x = o[0] | ((uint32_t)o[1] << 16); r.y = o[2] | ((uint32_t)o[3] << 16);
+        *reinterpret_cast<uint2*>(dst) = r;
+    } else {
+        *reinterpret_cast<uint32_t*>(dst) = o[0] | ((uint32_t)o[1] << 16);
+    }
+}
+
+/* ---- K1b: out[c][j] = in[c][j + shift] (shift = 1, 2 or 3 bytes): the sample-shifted copies K2's TMA loads need
+ * (TMA wants 16-byte aligned global coordinates, so a window at an odd sample offset is read from a shifted copy). */
+__global__ void __launch_bounds__(256)
+k_shift_copy(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, size_t pitch, long long ngroups, int shift) {
+    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= ngroups) return;
+    const uint8_t* src = in + (size_t)blockIdx.y * pitch + (size_t)g * 16;
+    const uint4 a = *reinterpret_cast<const uint4*>(src);
+    const uint32_t nx = *reinterpret_cast<const uint32_t*>(src + 16);
+    const int bs = shift * 8;
+    uint4 o;
+    o.x = __funnelshift_r(a.x, a.y, bs);
+    o.y = __funnelshift_r(a.y, a.z, bs);
+    o.z = __funnelshift_r(a.z, a.w, bs);
+    o.w = __funnelshift_r(a.w, nx, bs);
+    *reinterpret_cast<uint4*>(out + (size_t)blockIdx.y * pitch + (size_t)g * 16) = o;
+}
+
+/* ---- K5: sum_t D[i][t] and sum_t t*D[i][t] per row, int64 (all-rows checksum against the prefix-sum identity) */
+__global__ void __launch_bounds__(256)
+k_row_moments(const int32_t* __restrict__ D, long long pitch, long long nt, long long* __restrict__ sum_d,
+              long long* __restrict__ sum_td) {
+    __shared__ long long red[16];
+    const int32_t* row = D + (size_t)blockIdx.x * (size_t)pitch;
+    long long a = 0, b = 0;
+    for (long long t = threadIdx.x; t < nt; t += blockDim.x) { const long long v = row[t]; a += v; b += v * t; }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { a += __shfl_down_sync(0xffffffffu, a, o); b += __shfl_down_sync(0xffffffffu, b, o); }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) { red[warp * 2] = a; red[warp * 2 + 1] = b; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        long long sa = 0, sb = 0;
+        for (int w = 0; w < 8; ++w) { sa += red[w * 2]; sb += red[w * 2 + 1]; }
+        sum_d[blockIdx.x] = sa; sum_td[blockIdx.x] = sb;
+    }
+}
+
+/* ---- K0: sustained 32-bit integer add rate. 16 independent chains per thread, each step one add instruction.
+ * mode 0: every step an IADD3 (ALU pipe). mode 1: chains alternate IADD3 and IMAD (x*m + y with a runtime m = 1),
+ * which is how a kernel spreads integer adds over both 64-lane integer-capable pipes of an SM. */
+__global__ void __launch_bounds__(1024)
+k_peak_iadd(int mode, int iters, uint32_t* __restrict__ sink, unsigned long long* __restrict__ cycles, uint32_t b, uint32_t m) {
+    uint32_t a[AAK_PEAK_ADDS_PER_THREAD_ITER];
+#pragma unroll
+    for (int i = 0; i < AAK_PEAK_ADDS_PER_THREAD_ITER; ++i) a[i] = b * (i + 1) + threadIdx.x;
+    __syncthreads();
+    const unsigned long long t0 = clock64();
+    if (mode == 0) {
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int i = 0; i < AAK_PEAK_ADDS_PER_THREAD_ITER; ++i)
+                asm volatile("{.reg .u32 t; add.u32 t, %0, %1; add.u32 %0, t, %2;}" : "+r"(a[i]) : "r"(b), "r"(m));   /* one IADD3 */
+        }
+    } else {
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int i = 0; i < AAK_PEAK_ADDS_PER_THREAD_ITER; i += 2) {
+                asm volatile("{.reg .u32 t; add.u32 t, %0, %1; add.u32 %0, t, %2;}" : "+r"(a[i]) : "r"(b), "r"(m));
+                asm volatile("mad.lo.u32 %0, %1, %2, %0;" : "+r"(a[i + 1]) : "r"(b), "r"(m));                        /* IMAD */
+            }
+        }
+    }
+    const unsigned long long t1 = clock64();
+    uint32_t s = 0;
+#pragma unroll
+    for (int i = 0; i < AAK_PEAK_ADDS_PER_THREAD_ITER; ++i) s += a[i];
+    sink[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+    if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
+}
+
+}  // namespace
+
+extern "C" int aak_bin_time(const uint8_t* x, size_t x_pitch, uint16_t* xb, size_t xb_pitch_elems, int32_t nchans,
+                            int64_t nbinned, int32_t bin, void* stream) {
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long ngroups = (nbinned * bin + 15) / 16;
+    dim3 grid((unsigned)((ngroups + 255) / 256), (unsigned)nchans);
+    switch (bin) {
+        case 2: k_bin_time<2><<<grid, 256, 0, st>>>(x, x_pitch, xb, xb_pitch_elems, ngroups); break;
+        case 4: k_bin_time<4><<<grid, 256, 0, st>>>(x, x_pitch, xb, xb_pitch_elems, ngroups); break;
+        case 8: k_bin_time<8><<<grid, 256, 0, st>>>(x, x_pitch, xb, xb_pitch_elems, ngroups); break;
+        default: return (int)cudaErrorInvalidValue;
+    }
+    return (int)cudaGetLastError();
+}
+
+extern "C" int aak_shift_copy(const uint8_t* in, uint8_t* out, size_t pitch, size_t row_bytes, int32_t nrows, int32_t shift_bytes,
+                              void* stream) {
+    if (shift_bytes < 1 || shift_bytes > 3 || (row_bytes & 15) || (pitch & 15)) return (int)cudaErrorInvalidValue;
+    const long long ngroups = (long long)(row_bytes / 16);
+    dim3 grid((unsigned)((ngroups + 255) / 256), (unsigned)nrows);
+    k_shift_copy<<<grid, 256, 0, (cudaStream_t)stream>>>(in, out, pitch, ngroups, shift_bytes);
+    return (int)cudaGetLastError();
+}
+
+extern "C" int aak_row_moments(const int32_t* D, int64_t pitch, int64_t nt, int32_t ndms, long long* sum_d, long long* sum_td,
+                               void* stream) {
+    k_row_moments<<<(unsigned)ndms, 256, 0, (cudaStream_t)stream>>>(D, pitch, nt, sum_d, sum_td);
+    return (int)cudaGetLastError();
+}
+
+extern "C" int aak_peak_iadd(int32_t mode, int32_t iters, int32_t grid, int32_t threads, uint32_t* sink,
+                             unsigned long long* cycles_out, void* stream) {
+    k_peak_iadd<<<(unsigned)grid, (unsigned)threads, 0, (cudaStream_t)stream>>>(mode, iters, sink, cycles_out, 12345u, 1u);
+    return (int)cudaGetLastError();
+}
