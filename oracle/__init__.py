@@ -43,6 +43,7 @@ def _load():
     L.orc_delay_constants.argtypes = [i32, vp, f64, vp]; L.orc_delay_constants.restype = None
     L.orc_dm.argtypes = [f64, f64, i32]; L.orc_dm.restype = f64
     L.orc_delay.argtypes = [f64, f64, i32]; L.orc_delay.restype = i64
+    L.orc_delay_table.argtypes = [vp, i32, f64, f64, i32, i32, i32, vp]; L.orc_delay_table.restype = None
     L.orc_bin.argtypes = [vp, sz, i32, i64, i64, i32, vp]; L.orc_bin.restype = None
     L.orc_dedisperse.argtypes = [vp, i64, i32, vp, f64, f64, i32, i32, i32, i64, vp]; L.orc_dedisperse.restype = None
     L.orc_row_stats.argtypes = [vp, i64, vp, vp, vp]; L.orc_row_stats.restype = i32
@@ -74,6 +75,15 @@ def dm_value(dm_low, dm_step, i) -> float:
 
 def delay(k_c, dm, bin_=1) -> int:
     return int(_load().orc_delay(float(k_c), float(dm), int(bin_)))
+
+
+def delay_table(k: np.ndarray, rng, i0: int = 0, i1: int | None = None) -> np.ndarray:
+    """delay(c, i) in binned samples for rows [i0, i1) of rng = (dm_low, dm_step, ndms, bin): int64 [i1-i0][nchans]."""
+    k = np.ascontiguousarray(k, dtype=np.float64)
+    i1 = rng[2] if i1 is None else i1
+    out = np.empty((i1 - i0, len(k)), dtype=np.int64)
+    _load().orc_delay_table(_p(k), len(k), float(rng[0]), float(rng[1]), int(rng[3]), i0, i1, _p(out))
+    return out
 
 
 def bin_time(x: np.ndarray, start: int, nbinned: int, b: int) -> np.ndarray:

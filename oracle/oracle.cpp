@@ -60,6 +60,16 @@ int64_t orc_delay(double k_c, double dm, int32_t bin) {
     return (int64_t)llround((k_c * dm) / (double)bin);   /* round half away from zero */
 }
 
+/* Table form of orc_delay for one range: out[i][c] = orc_delay(k[c], orc_dm(dm_low, dm_step, i), bin), i in [i0, i1).
+ * A plain loop over the function above (no arithmetic of its own); lets tests build whole delay tables quickly. */
+void orc_delay_table(const double* k, int32_t nchans, double dm_low, double dm_step, int32_t bin, int32_t i0, int32_t i1,
+                     int64_t* out) {
+    for (int32_t i = i0; i < i1; ++i) {
+        const double dm = orc_dm(dm_low, dm_step, i);
+        for (int32_t c = 0; c < nchans; ++c) out[(size_t)(i - i0) * (size_t)nchans + (size_t)c] = orc_delay(k[c], dm, bin);
+    }
+}
+
 /* ---- C4: time binning (reading: SUM of b consecutive samples, no division, held in uint16) -----------
  * out[c][t'] = sum_{j<b} x[c][start + b*t' + j],  t' in [0, nbinned) */
 void orc_bin(const uint8_t* x, size_t row_stride, int32_t nchans, int64_t start, int64_t nbinned, int32_t b,

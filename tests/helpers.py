@@ -64,3 +64,96 @@ def compare_candidates(got: np.ndarray, exp: np.ndarray, threshold: float, snr_r
             assert int(a["width"]) == int(b["width"]) and float(a["dm"]) == float(b["dm"]), (k, a, b)
             n += 1
     return n, len(only_g), len(only_e)
+
+
+def row_moments_from_input(x: np.ndarray, k: np.ndarray, rng, start: int, length: int, T: int, chan_block: int = 64):
+    """SURVEY §8(c) pin (v), an O(C)-per-row route to sum_t D[i][t] and sum_t t*D[i][t] for EVERY row of a range that
+    never forms D: per-channel prefix sums P, Q of the binned input and the oracle's delay table.
+    Returns two int64 arrays [ndms]; arithmetic is modulo 2^64 (numpy int64 wraps), as on the device."""
+    b = rng[3]
+    dl = oracle.delay_table(k, rng)                         # [ndms][C]
+    nd, C = dl.shape
+    m0 = np.zeros(nd, np.int64)
+    m1 = np.zeros(nd, np.int64)
+    nb = length // b
+    tt = np.arange(nb, dtype=np.int64)
+    with np.errstate(over="ignore"):
+        for c0 in range(0, C, chan_block):
+            c1 = min(C, c0 + chan_block)
+            xb = oracle.bin_time(x[c0:c1], start, nb, b).astype(np.int64)
+            P = np.zeros((c1 - c0, nb + 1), np.int64)
+            Q = np.zeros((c1 - c0, nb + 1), np.int64)
+            np.cumsum(xb, axis=1, out=P[:, 1:])
+            np.cumsum(xb * tt, axis=1, out=Q[:, 1:])
+            d = dl[:, c0:c1]                                # [ndms][cb]
+            ch = np.arange(c1 - c0)[None, :]
+            dP = P[ch, d + T] - P[ch, d]
+            dQ = Q[ch, d + T] - Q[ch, d]
+            m0 += dP.sum(axis=1)
+            m1 += (dQ - d * dP).sum(axis=1)
+    return m0, m1
+
+
+class GpuRun:
+    """The CUDA path through the C-ABI binding for one workload (plan -> strategy -> chunk loop)."""
+
+    def __init__(self, w, x, **strategy_kw):
+        import paper_1912_07704_b200 as aa
+        self.aa, self.w, self.x = aa, w, x
+        self.plan = aa.Plan(w.freqs_mhz, w.tsamp_s, w.ranges, w.widths, w.threshold)
+        self.st = aa.Strategy(self.plan, x.shape[1], **strategy_kw)
+        self.h = self.st.handle
+        self.info = self.st.info
+        self.chunks = [aa.aa_strategy_get_chunk(self.h, j) for j in range(self.info["nchunks"])]
+
+    def dedisperse(self):
+        return self.aa.aa_run_dedispersion(self.h, self.x)
+
+    def sps(self):
+        return self.aa.aa_run_sps(self.h)
+
+    def row(self, r, i):
+        return self.aa.aa_get_dedispersed_row(self.h, r, i)
+
+    def stats(self, r, i):
+        return self.aa.aa_get_row_stats(self.h, r, i)
+
+    def moments(self, r):
+        return self.aa.aa_get_row_moments(self.h, r, self.w.ranges[r][2])
+
+    def candidates(self, **kw):
+        return self.aa.aa_get_candidates(self.h, **kw)
+
+    def close(self):
+        self.st.close()
+        self.plan.close()
+
+
+def band_rows(ndms: int, centres, half: int = 2):
+    """Bands [i0, i1) of 2*half+1 adjacent DM rows around each centre, clipped to the range, deduplicated."""
+    out = []
+    for c in centres:
+        i0 = max(0, min(ndms - (2 * half + 1), c - half))
+        i1 = min(ndms, i0 + 2 * half + 1)
+        if (i0, i1) not in out:
+            out.append((i0, i1))
+    return out
+
+
+def check_band(gpu: GpuRun, orc: OracleRun, chunk, r, i0, i1, *, after_sps: bool, cands=None):
+    """Bit-exact D rows [i0,i1) and (after SPS) mu/sigma of the same rows; returns the oracle's candidates in the band's
+    INTERIOR rows (those whose 3x3 neighbourhood lies inside the band or at the range edge)."""
+    res = orc.search(chunk, r, i0, i1, want=("D", "stats"))
+    for i in range(i0, i1):
+        got = gpu.row(r, i)
+        exp = res["D"][i - i0]
+        assert got.shape == exp.shape, (r, i, got.shape, exp.shape)
+        if not np.array_equal(got.astype(np.int64), exp):
+            bad = np.flatnonzero(got.astype(np.int64) != exp)
+            raise AssertionError(f"D mismatch range {r} row {i}: {len(bad)} samples, first at t={bad[:5]}, "
+                                 f"got {got[bad[:5]]}, expected {exp[bad[:5]]}")
+        if after_sps:
+            mu, sg, n, it = gpu.stats(r, i)
+            emu, esg = res["stats"][i - i0]
+            assert mu == emu and sg == esg, (r, i, mu, emu, sg, esg)
+    return res["cands"]
