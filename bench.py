@@ -1,0 +1,312 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the dedispersion + single-pulse-search hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload ska] [--impl ours|reference]
+
+A *step* is one pass of the whole hot path (time binning -> dedispersion of every DM range -> row
+statistics -> boxcar SNR / peaks / candidate compaction) over one chunk of synthetic filterbank data.
+  value  DM-trial x samples / s with the chunk already resident in HBM (CUDA events on the compute stream).
+  e2e    the same metric through aa_run_dedispersion(HOST pointer) ... aa_get_candidates: H2D of the chunk from pinned
+         host memory and D2H of the candidate list inside the timed region.
+  roofline  dominant kernel = K2 (k_dedisperse, one launch per DM range); bound "alu" (integer adds), see DESIGN.md.
+  cpu_baseline  the oracle (oracle/, single-threaded C++) timed on a bounded sample of the same workload on this host.
+N > 1 (torchrun): every rank runs the same step on its own chunk (replicas over time chunks, no collective on the data
+path); value = outputs of all ranks / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "dm_trial_samples_per_s"
+UNIT = "DM-trial*samples/s"
+SM_COUNT = 148
+INT_LANES_PER_SM_CLK = 128      # 64 ALU-pipe (IADD3) + 64 FMA-pipe (IMAD) lanes per SM per clock, DESIGN.md "Roofline"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="ska", help="tiny | mid | ska | lowf (BASELINE.json configs 0..3)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def outputs_of(w, n_out):
+    return sum(r[2] * (n_out // r[3]) for r in w.ranges)
+
+
+# ------------------------------------------------------------------------------------------------ clocks sampler
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML every 100 ms while the timed region runs."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.mhz, self.reasons, self.max_mhz, self.power = index, False, [], set(), None, []
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap", nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        while not self.stop_flag:
+            try:
+                self.mhz.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+                bits = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for b, n in names.items():
+                    if bits & b:
+                        self.reasons.add(n)
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        return {"sm_mhz": float(np.median(self.mhz)) if self.mhz else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "power_w_max": max(self.power) if self.power else None,
+                "samples": len(self.mhz)}
+
+
+# ------------------------------------------------------------------------------------------------ oracle legs (CPU)
+def oracle_sample(w, x, n_out, rows_per_range: int):
+    """The oracle as it stands on a bounded sample: time binning of the whole chunk (step a2, done once per job) plus
+    `rows_per_range` evenly spaced DM rows of every range over the full chunk, each row taken through dedispersion ->
+    statistics -> boxcar SNR -> peaks. Work is exactly linear in the number of rows, so the whole-job time is
+    t_bin + sum_r t_rows(r) * ndms_r / rows_r (SURVEY §8(d) "CPU baseline"). Returns (job outputs, job seconds
+    extrapolated, seconds actually spent, text)."""
+    import oracle
+    k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
+    B = max(r[3] for r in w.ranges)
+    L = (x.shape[1] // B) * B
+    t_start = time.perf_counter()
+    binned = {}
+    for b in sorted({r[3] for r in w.ranges}):
+        binned[b] = oracle.bin_time(x, 0, L // b, b)                # step a2
+    t_job = time.perf_counter() - t_start
+    for r, rng in enumerate(w.ranges):
+        b, T = rng[3], n_out // rng[3]
+        idx = sorted({int(round(q * (rng[2] - 1) / max(1, rows_per_range - 1))) for q in range(rows_per_range)})
+        t0 = time.perf_counter()
+        for i in idx:
+            D = oracle.dedisperse(binned[b], k, rng, i, i + 1, T)
+            mu, sg, *_ = oracle.row_stats(D[0])
+            S, wb = oracle.boxcar_snr(D[0], w.widths, mu, sg, prefix=True)
+            oracle.find_peaks(S[None, :], w.threshold)
+        t_job += (time.perf_counter() - t0) * rng[2] / len(idx)
+    spent = time.perf_counter() - t_start
+    what = (f"binning of the full chunk + {rows_per_range} evenly spaced DM row(s) of each of the {len(w.ranges)} ranges over "
+            f"the full chunk (dedispersion+SPS), extrapolated linearly in rows to all {w.ndms_total} rows")
+    return outputs_of(w, n_out), t_job, spent, what
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle timed on the host cores, same metric/config; each step = a bounded sample."""
+    import datagen
+    import oracle
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    pl, dms, dl = w.pulses()
+    x = datagen.generate(w.seed, w.nchans, w.nsamp, pl, dl)
+    k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
+    g = oracle.chunk_geometry(k, w.ranges, w.nsamp)
+    rows = 1 if w.nchans * w.nsamp > (1 << 28) else 3
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(w, x, g["n_out"], rows)
+    outs, secs, spent, what = 0, 0.0, 0.0, ""
+    for _ in range(args.steps):
+        o, s, sp, what = oracle_sample(w, x, g["n_out"], rows)
+        outs += o
+        secs += s
+        spent += sp
+    v = outs / secs
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int64", "sample_seconds_per_step": spent / args.steps, "data": "synthetic",
+            "config": {"workload": w.name, "nchans": w.nchans, "nsamp": w.nsamp, "ndms": w.ndms_total,
+                       "note": "each step is a bounded sample of the workload: " + what},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------ our arm (GPU)
+def run_ours(args, w):
+    import torch
+    import torch.distributed as dist
+    import datagen
+    import paper_1912_07704_b200 as aa
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    # synthetic chunk of this rank (replicas over time chunks: a different seed per rank), pinned for the e2e leg
+    pl, dms, dl = w.pulses()
+    xh = torch.empty((w.nchans, w.nsamp), dtype=torch.uint8, pin_memory=True)
+    x = xh.numpy()
+    datagen.generate(w.seed + 1000003 * rank, w.nchans, w.nsamp, pl, dl, out=x)
+    xd = xh.cuda(non_blocking=False)
+
+    compute, copy = torch.cuda.Stream(), torch.cuda.Stream()
+    plan = aa.Plan(w.freqs_mhz, w.tsamp_s, w.ranges, w.widths, w.threshold)
+    st = aa.Strategy(plan, w.nsamp, compute_stream=compute, copy_stream=copy, max_candidates=1 << 22)
+    h, info = st.handle, st.info
+    assert info["nchunks"] == 1, "the benchmark workload must fit one chunk"
+    outputs = outputs_of(w, info["n_out"])
+    adds = outputs * w.nchans
+    in_bytes = w.nchans * info["chunk_len"]
+
+    def step_resident():
+        aa.aa_strategy_reset(h)
+        aa.aa_run_dedispersion_device(h, xd, xd.stride(0))
+        aa.aa_run_sps(h)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step_resident()
+    aa.aa_synchronize(h)
+    ncand = len(aa.aa_get_candidates(h, allow_overflow=True))
+
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    k2_ms, parts = [], []
+    launches = 0
+    for a, b in evs:
+        a.record(compute)
+        step_resident()
+        b.record(compute)
+        # per-kernel-class CUDA-event times of this step (recorded by the library on the compute stream); reading them
+        # synchronises, which also separates the steps
+        tm = aa.aa_get_last_timings(h)
+        k2_ms.append(tm["dedisp_ms"])
+        parts.append(tm)
+        launches += aa.aa_get_launch_count(h)
+    barrier()
+    sampler.stop_flag = True
+    sampler.join()
+    total_ms = sum(a.elapsed_time(b) for a, b in evs)
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    value = outputs * world * args.steps / (total_ms * 1e-3)
+
+    # e2e: host pointer in, candidate list out, through the public C-ABI calls
+    e2e = None
+    if not args.no_e2e:
+        def step_e2e():
+            aa.aa_strategy_reset(h)
+            aa.aa_run_dedispersion(h, x, xh.stride(0))
+            aa.aa_run_sps(h)
+            return aa.aa_get_candidates(h, allow_overflow=True)
+        step_e2e()
+        barrier()
+        t0 = time.perf_counter()
+        d2h = 0
+        for _ in range(args.steps):
+            c = step_e2e()
+            d2h += c.nbytes + 8
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e = {"value": outputs * world * args.steps / float(t.item()), "unit": UNIT,
+               "h2d_bytes_per_step": int(in_bytes), "d2h_bytes_per_step": int(d2h // args.steps),
+               "ms_per_step": 1e3 * float(t.item()) / args.steps, "timer": "host wall clock around the C-ABI calls, synchronised"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # roofline of the dominant kernel (K2, all ranges of one step = 5 launches): integer adds, bound "alu"
+    iadd3, mixed, mhz = aa.aa_measure_int_add_peak(compute, 300)
+    k2 = float(np.mean(k2_ms)) * 1e-3
+    peak = SM_COUNT * INT_LANES_PER_SM_CLK * (sampler.max_mhz or 1965) * 1e6
+    t_hbm = (in_bytes + 4 * outputs) / (json.loads((ROOT / "MEASURED_PEAKS.json").read_text())["hbm_gbs"] * 1e9) \
+        if (ROOT / "MEASURED_PEAKS.json").exists() else (in_bytes + 4 * outputs) / 6.65e12
+    roofline = {"bound": "alu", "kernel": "k_dedisperse (K2), the launches of all DM ranges of one step",
+                "achieved": adds / k2 / 1e12, "peak": peak / 1e12, "unit": "Tadd/s (algorithmic 32-bit integer adds)",
+                "frac": adds / k2 / peak, "traffic": None,
+                "peak_how": f"derived: {SM_COUNT} SMs x {INT_LANES_PER_SM_CLK} integer-add lanes/clk (64 IADD3 + 64 IMAD) x max SM clock",
+                "measured_iadd3_only_tadd_s": iadd3 / 1e12, "measured_iadd3_imad_mixed_tadd_s": mixed / 1e12,
+                "frac_of_measured_mixed": adds / k2 / max(mixed, iadd3), "frac_of_measured_iadd3_only": adds / k2 / iadd3,
+                "microbench_sm_mhz": mhz, "k2_ms_per_step": k2 * 1e3, "t_hbm_compulsory_ms": t_hbm * 1e3,
+                "algorithmic_adds_per_step": adds}
+    mean = lambda key: float(np.mean([p[key] for p in parts]))
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "int32", "data": "synthetic",
+            "config": {"workload": w.name, "nchans": w.nchans, "nsamp": w.nsamp, "tsamp_us": w.tsamp_s * 1e6, "ndms": w.ndms_total,
+                       "ranges": [list(r) for r in w.ranges], "widths": list(w.widths), "threshold": w.threshold,
+                       "outputs_per_step": outputs, "l2": "inputs larger than L2 (chunk %.2f GB in, %.2f GB out)" % (in_bytes / 1e9, 4 * outputs / 1e9),
+                       "parallelism": "replicas over time chunks" if world > 1 else "single GPU"},
+            "realtime_factor": (info["n_out"] * w.tsamp_s) / (total_ms * 1e-3 / args.steps),
+            "realtime_factor_e2e": (info["n_out"] * w.tsamp_s) / (e2e["ms_per_step"] * 1e-3) if e2e else None,
+            "breakdown_ms": {"bin_and_shift": mean("bin_ms"), "dedispersion": mean("dedisp_ms"), "row_stats": mean("stats_ms"),
+                             "sps_peaks": mean("peaks_ms")},
+            "candidates_per_step": ncand, "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": int(launches),
+            "roofline": roofline}
+    if not args.no_cpu_baseline and world == 1:
+        rows = 1 if w.nchans * w.nsamp > (1 << 28) else 3
+        o, secs, spent, what = oracle_sample(w, x, info["n_out"], rows)
+        line["cpu_baseline"] = {"value": o / secs, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what,
+                                "sample_seconds": spent, "host_cores_available": os.cpu_count()}
+    print(json.dumps(line), flush=True)
+    st.close()
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    import datagen
+    w = datagen.get_workload(args.workload)
+    if args.impl == "reference":
+        run_reference(args, w)
+    else:
+        run_ours(args, w)
+
+
+if __name__ == "__main__":
+    main()
