@@ -61,7 +61,7 @@ struct Range {
     int32_t* d_etab = nullptr;
     int32_t* d_x0tab = nullptr;
     int32_t* d_D = nullptr;
-    CUtensorMap maps[2][4];       /* [raw buffer parity][copy] */
+    CUtensorMap map;              /* 4-D window map over the range's NCOPY-copy input buffer */
     size_t first_row = 0;         /* index of this range's first row in the row tables */
 };
 
@@ -83,10 +83,12 @@ struct Strategy {
     bool owns_arena = false;
     size_t in_pitch = 0;                     /* bytes per channel row of the uint8 buffers */
     uint8_t* d_raw[2] = {nullptr, nullptr};  /* H2D targets (copy 0 of the uint8 input) */
-    uint8_t* d_shift[3] = {nullptr, nullptr, nullptr};   /* copies 1..3 of the uint8 input */
+    uint8_t* d_x4 = nullptr;                 /* the 4 sample-shifted copies of the uint8 chunk, copy k at k*x4_stride */
+    size_t x4_stride = 0;
     bool need_u8_copies = false;
     size_t xb_pitch[9] = {0};                /* elements, indexed by bin */
-    uint16_t* d_xb[9][2] = {{nullptr}};      /* binned input, copies 0 and 1, indexed by bin */
+    uint16_t* d_xb[9] = {nullptr};           /* binned input indexed by bin: copy 0, then copy 1 at +xb_stride bytes */
+    size_t xb_stride[9] = {0};
     aak_row_desc* d_rows[2] = {nullptr, nullptr};   /* [0] full chunk geometry, [1] last (short) chunk */
     double* d_mu_sigma = nullptr;            /* [nrows][2] */
     int64_t* d_n_iters = nullptr;            /* [nrows][2] */

@@ -19,6 +19,10 @@ extern "C" {
 /* ---- K1: time binning, x_b[c][t'] = sum_{j<b} x[c][b*t'+j]  (uint8 -> uint16) --------------------------------- */
 int aak_bin_time(const uint8_t* x, size_t x_pitch, uint16_t* xb, size_t xb_pitch_elems, int32_t nchans,
                  int64_t nbinned, int32_t bin, void* stream);
+/* ---- K1a: the four sample-shifted copies of the uint8 chunk in one pass: out[k*copy_stride + c*pitch + j] = in[c*pitch + j + k],
+ * k = 0..3, j in [0, row_bytes). row_bytes, pitch, copy_stride multiples of 16; in readable 4 bytes past each row. */
+int aak_make_copies_u8(const uint8_t* in, uint8_t* out, size_t pitch, size_t copy_stride, size_t row_bytes, int32_t nrows,
+                       void* stream);
 /* ---- K1b: shifted copy, out[c][j] = in[c][j + shift_bytes] (1..3) for j in [0, row_bytes), rows `pitch` bytes apart.
  * row_bytes and pitch are multiples of 16; the source must be readable up to row_bytes + 4 past each row start. */
 int aak_shift_copy(const uint8_t* in, uint8_t* out, size_t pitch, size_t row_bytes, int32_t nrows, int32_t shift_bytes,
@@ -27,13 +31,14 @@ int aak_shift_copy(const uint8_t* in, uint8_t* out, size_t pitch, size_t row_byt
 /* ---- K2: dedispersion --------------------------------------------------------------------------------------------
  * Tiled kernel: a CTA owns DM_TILE(=32) DM trials x T_TILE(=1024) output samples; channels stream through shared memory
  * in blocks of `chan_block` via TMA (tensor map `tmap`, 128 opaque bytes, see aa_strategy.cpp), NSTAGE-deep mbarrier ring.
- * The input exists as NCOPY = 4 (uint8) or 2 (uint16) sample-shifted copies in global memory, copy k = x[c][t+k];
- * tmap points at NCOPY consecutive 128-byte CUtensorMaps (HOST memory), one per copy.
+ * The input exists as NCOPY = 4 (uint8) or 2 (uint16) sample-shifted copies in ONE global buffer, copy k = x[c][t+k]
+ * at byte offset k*copy_stride; tmap points at the 128-byte 4-D CUtensorMap over it (HOST memory).
+ * A stage in shared memory is [chan_block][NCOPY][window_bytes] followed by the stage's slice of etab.
  * etab  [ndm_tiles][nstages][chan_block][32] int32 : shared-memory byte offset of (channel, DM) inside a stage
  * x0tab [ndm_tiles][nstages*chan_block]    int32 : 16-byte aligned BYTE offset of the channel window relative to the
  *                                                  tile's first output sample */
 typedef struct {
-    const void* tmap;          /* HOST pointer to NCOPY 128-byte CUtensorMaps (copied into kernel params) */
+    const void* tmap;          /* HOST pointer to the 128-byte CUtensorMap (copied into kernel params) */
     const int32_t* etab;
     const int32_t* x0tab;
     int32_t* D;                /* [ndms][pitch] */
@@ -43,7 +48,6 @@ typedef struct {
     int32_t nchans;
     int32_t chan_block;        /* 8, 4 or 2 */
     int32_t window_bytes;      /* WB: bytes per (copy, channel) window in shared memory, multiple of 256 */
-    int32_t boxes_per_row;     /* 1 (one 3-D box covers the window) or WB/256 (one 2-D box per 256 bytes) */
     int32_t spill_stages;      /* carry the 16-bit lanes every this many stages: (256/bin)/chan_block */
     int32_t in16;              /* 0: uint8 input (bin 1), 1: uint16 input (binned) */
     int32_t variant;           /* uint8 only: 1 = odd-byte lane adds issued as IMAD (FMA pipe), 0 = fused IADD3 */

@@ -51,21 +51,20 @@ aa_status enqueue_dedispersion(Strategy& s, int64_t j, int b) {
     const int32_t C = s.plan.nchans;
     AA_CUDA(cudaEventRecord(s.ev_t[0], s.compute), "cudaEventRecord");
     if (s.need_u8_copies)
-        for (int k = 1; k <= 3; ++k)
-            AA_LAUNCH(aak_shift_copy(s.d_raw[b], s.d_shift[k - 1], s.in_pitch, s.in_pitch, C, k, s.compute), "shift copy (uint8)");
+        AA_LAUNCH(aak_make_copies_u8(s.d_raw[b], s.d_x4, s.in_pitch, s.x4_stride, s.in_pitch, C, s.compute), "shifted copies (uint8)");
     for (int bin = 2; bin <= 8; bin *= 2) {
-        if (!s.d_xb[bin][0]) continue;
+        if (!s.d_xb[bin]) continue;
         const size_t pitch_bytes = s.xb_pitch[bin] * 2;
-        AA_LAUNCH(aak_bin_time(s.d_raw[b], s.in_pitch, s.d_xb[bin][0], s.xb_pitch[bin], C, (int64_t)(c.len / (uint64_t)bin), bin, s.compute), "time binning");
-        AA_LAUNCH(aak_shift_copy((const uint8_t*)s.d_xb[bin][0], (uint8_t*)s.d_xb[bin][1], pitch_bytes, pitch_bytes, C, 2, s.compute), "shift copy (uint16)");
+        AA_LAUNCH(aak_bin_time(s.d_raw[b], s.in_pitch, s.d_xb[bin], s.xb_pitch[bin], C, (int64_t)(c.len / (uint64_t)bin), bin, s.compute), "time binning");
+        AA_LAUNCH(aak_shift_copy((const uint8_t*)s.d_xb[bin], (uint8_t*)s.d_xb[bin] + s.xb_stride[bin], pitch_bytes, pitch_bytes, C, 2, s.compute), "shift copy (uint16)");
     }
     AA_CUDA(cudaEventRecord(s.ev_t[1], s.compute), "cudaEventRecord");
     for (Range& rg : s.ranges) {
         aak_dedisp_args a;
-        a.tmap = &rg.maps[b][0];
+        a.tmap = &rg.map;
         a.etab = rg.d_etab; a.x0tab = rg.d_x0tab; a.D = rg.d_D; a.pitch = rg.pitch;
         a.nt = (int64_t)(c.n_out / (uint64_t)rg.r.bin);
-        a.ndms = rg.r.ndms; a.nchans = C; a.chan_block = rg.chan_block; a.window_bytes = rg.window_bytes; a.boxes_per_row = 1;
+        a.ndms = rg.r.ndms; a.nchans = C; a.chan_block = rg.chan_block; a.window_bytes = rg.window_bytes;
         a.spill_stages = rg.spill_stages; a.in16 = rg.in16; a.variant = 1;
         AA_LAUNCH(aak_dedisperse(&a, s.compute), "dedispersion");
     }

@@ -40,16 +40,18 @@ int64_t delay_of(const Strategy& s, const Range& rg, int32_t chan, int32_t dm_in
     return delay_calc(s.k[(size_t)chan], dm_of(rg.r, dm_index), rg.r.bin);
 }
 
-/* Channel rows seen as overlapping 256-byte segments: a {256, nseg, 1} box lands as one linear window (k_dedisp.cu). */
-static bool make_window_map(CUtensorMap* map, void* base, size_t pitch_bytes, int32_t nchans, int32_t window_bytes) {
+/* Channel rows of the NCOPY shifted copies seen as overlapping 256-byte segments: a {256, nseg, NCOPY, 1} box lands as
+ * NCOPY linear windows of window_bytes each (k_dedisp.cu). */
+static bool make_window_map(CUtensorMap* map, void* base, size_t pitch_bytes, size_t copy_stride, int32_t ncopy, int32_t nchans,
+                            int32_t window_bytes) {
     EncodeTiledFn enc = encode_fn();
     if (!enc) { set_error("aa_strategy_setup: cuTensorMapEncodeTiled is not available from this driver"); return false; }
     const cuuint32_t nseg = (cuuint32_t)(window_bytes / 256);
-    cuuint64_t dims[3] = {(cuuint64_t)pitch_bytes, nseg, (cuuint64_t)nchans};
-    cuuint64_t strides[2] = {256, (cuuint64_t)pitch_bytes};
-    cuuint32_t box[3] = {256, nseg, 1};
-    cuuint32_t es[3] = {1, 1, 1};
-    const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+    cuuint64_t dims[4] = {(cuuint64_t)pitch_bytes, nseg, (cuuint64_t)ncopy, (cuuint64_t)nchans};
+    cuuint64_t strides[3] = {256, (cuuint64_t)copy_stride, (cuuint64_t)pitch_bytes};
+    cuuint32_t box[4] = {256, nseg, (cuuint32_t)ncopy, 1};
+    cuuint32_t es[4] = {1, 1, 1, 1};
+    const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 4, base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { set_error("aa_strategy_setup: cuTensorMapEncodeTiled failed with CUresult %d", (int)r); return false; }
     return true;
@@ -63,13 +65,14 @@ static void carve(Strategy& s, int64_t L, bool two_raw) {
     const size_t raw_bytes = (size_t)s.plan.nchans * s.in_pitch + kSlack;
     s.d_raw[0] = (uint8_t*)a.take(raw_bytes);
     s.d_raw[1] = two_raw ? (uint8_t*)a.take(raw_bytes) : nullptr;
-    for (int k = 0; k < 3; ++k) s.d_shift[k] = s.need_u8_copies ? (uint8_t*)a.take(raw_bytes) : nullptr;
+    s.x4_stride = round_up(raw_bytes, 256);
+    s.d_x4 = s.need_u8_copies ? (uint8_t*)a.take(4 * s.x4_stride) : nullptr;
     for (int b = 2; b <= 8; b *= 2) {
         bool used = false;
         for (const Range& rg : s.ranges) used = used || rg.r.bin == b;
         s.xb_pitch[b] = used ? round_up((size_t)(L / b), 256) : 0;
-        for (int k = 0; k < 2; ++k)
-            s.d_xb[b][k] = used ? (uint16_t*)a.take((size_t)s.plan.nchans * s.xb_pitch[b] * 2 + kSlack) : nullptr;
+        s.xb_stride[b] = round_up((size_t)s.plan.nchans * s.xb_pitch[b] * 2 + kSlack, 256);
+        s.d_xb[b] = used ? (uint16_t*)a.take(2 * s.xb_stride[b]) : nullptr;
     }
     const int64_t n_out = L - s.S;
     for (Range& rg : s.ranges) {
@@ -148,7 +151,7 @@ static bool plan_range(Strategy& s, Range& rg, std::vector<int32_t>& etab, std::
             int32_t* e = etab.data() + ((size_t)t * Cpad + c) * kDmTile;     /* [tile][stage][c_local][m] */
             const int32_t cl = c % CB;
             if (c >= C) {                                                   /* padding channel: TMA zero-fills it */
-                for (int m = 0; m < kDmTile; ++m) e[m] = cl * WB;
+                for (int m = 0; m < kDmTile; ++m) e[m] = cl * rg.ncopy * WB;
                 continue;
             }
             const int64_t d0 = rg.delays[(size_t)i0 * C + c];
@@ -159,7 +162,7 @@ static bool plan_range(Strategy& s, Range& rg, std::vector<int32_t>& etab, std::
                 const int32_t i = std::min(nd - 1, i0 + m);
                 const int64_t o = (int64_t)rg.delays[(size_t)i * C + c] - d0 + res;
                 const int64_t copy = o & (rg.spw - 1);
-                e[m] = (int32_t)((copy * CB + cl) * WB + (o - copy) * rg.esz);
+                e[m] = (int32_t)((cl * rg.ncopy + copy) * WB + (o - copy) * rg.esz);
             }
         }
     }
@@ -328,13 +331,10 @@ extern "C" aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, u
         Range& rg = s.ranges[r];
         if ((e = cudaMemcpyAsync(rg.d_etab, etabs[r].data(), etabs[r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
         if ((e = cudaMemcpyAsync(rg.d_x0tab, x0tabs[r].data(), x0tabs[r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
-        for (int par = 0; par < 2; ++par) {
-            for (int k = 0; k < rg.ncopy; ++k) {
-                void* base; size_t pitch_bytes;
-                if (rg.in16) { base = s.d_xb[rg.r.bin][k]; pitch_bytes = s.xb_pitch[rg.r.bin] * 2; }
-                else { base = k == 0 ? (s.d_raw[par] ? s.d_raw[par] : s.d_raw[0]) : s.d_shift[k - 1]; pitch_bytes = s.in_pitch; }
-                if (!make_window_map(&rg.maps[par][k], base, pitch_bytes, C, rg.window_bytes)) return fail(AA_ERR_CUDA);
-            }
+        if (rg.in16) {
+            if (!make_window_map(&rg.map, s.d_xb[rg.r.bin], s.xb_pitch[rg.r.bin] * 2, s.xb_stride[rg.r.bin], 2, C, rg.window_bytes)) return fail(AA_ERR_CUDA);
+        } else {
+            if (!make_window_map(&rg.map, s.d_x4, s.in_pitch, s.x4_stride, 4, C, rg.window_bytes)) return fail(AA_ERR_CUDA);
         }
         for (int32_t i = 0; i < rg.r.ndms; ++i) {
             const int32_t* base = rg.d_D + (size_t)i * (size_t)rg.pitch;
@@ -420,7 +420,7 @@ extern "C" size_t aa_strategy_describe(const aa_strategy* h, char* buf, size_t b
     o += line;
     snprintf(line, sizeof line, "arena: %zu bytes used of %zu (%s), input pitch %zu, raw buffers %d, uint8 shifted copies %s\n", s.arena.used,
              s.arena.size, s.owns_arena ? "library-owned, one cudaMalloc" : "caller-owned", s.in_pitch, s.d_raw[1] ? 2 : 1,
-             s.need_u8_copies ? "3" : "none");
+             s.need_u8_copies ? "4" : "none");
     o += line;
     for (const Range& rg : s.ranges) {
         snprintf(line, sizeof line,

@@ -11,10 +11,13 @@
  *     2 for uint16), so that ANY sample offset t+delay is a word-aligned, bank-conflict-free LDS.32: copy k holds the
  *     window shifted by k samples. TMA needs 16-byte aligned global coordinates (measured: an unaligned inner
  *     coordinate raises an illegal-instruction fault on sm_100a), so the shifted copies exist in GLOBAL memory
- *     (K1 writes them: x_k[c][t] = x[c][t+k]) and each is fetched by its own tensor map; the window start is aligned
- *     down to 16 bytes and the residue is folded into the host-built offset table.
- *   * One TMA per (copy, channel) moves the whole window: the tensor map views a channel row as OVERLAPPING 256-byte
- *     segments (dims {pitch, nseg, C}, strides {256, pitch}), so a {256, nseg, 1} box lands as one linear run.
+ *     (K1 writes them: x_k[c][t] = x[c][t+k], copy k at byte offset k*copy_stride of one buffer); the window start is
+ *     aligned down to 16 bytes and the residue is folded into the host-built offset table.
+ *   * ONE TMA per channel moves the windows of all copies: the tensor map views the buffer as OVERLAPPING 256-byte
+ *     segments (dims {pitch, nseg, NCOPY, C}, strides {256, copy_stride, pitch}), so a {256, nseg, NCOPY, 1} box lands
+ *     as NCOPY linear windows of WB bytes. A stage is therefore CB tensor copies + one bulk copy of the offset table,
+ *     issued by one elected thread (ncu on the first version, one TMA per (copy, channel) issued from 32 divergent
+ *     lanes, showed the producer warp busy 85 % of the time and the compute warps starved: profiles/r01_*).
  *   * Packed arithmetic (uint8): a loaded word w = (b0,b1,b2,b3) is four consecutive time samples of one channel.
  *         A += w                      (whole word, lanes overlap at 8-bit spacing, wraps mod 2^32)
  *         H += (b1, 0, b3, 0)         (one PRMT; two clean 16-bit lanes)
@@ -44,7 +47,6 @@ constexpr int NSTAGE = 3;
 constexpr int NTHREADS = (NW + 1) * 32;
 constexpr int SMEM_HEADER = 1024;    /* mbarriers live here; keeps the stages 1024-byte aligned */
 
-struct TmapPack { CUtensorMap m[4]; };   /* one per shifted copy */
 
 struct DedispParams {
     const int32_t* etab;
@@ -55,7 +57,6 @@ struct DedispParams {
     int ndms;
     int nstages;
     int window_bytes;
-    int boxes_per_row;
     int spill_stages;
     unsigned one;              /* always 1; a runtime value so that x*one+y stays an IMAD (FMA pipe) */
 };
@@ -83,10 +84,10 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int x, int y, int z, uint32_t bar) {
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map, int x, int y, int z, int w, uint32_t bar) {
     asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(dst),
-        "l"(reinterpret_cast<uint64_t>(map)), "r"(x), "r"(y), "r"(z), "r"(bar)
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(dst),
+        "l"(reinterpret_cast<uint64_t>(map)), "r"(x), "r"(y), "r"(z), "r"(w), "r"(bar)
         : "memory");
 }
 __device__ __forceinline__ void bulk_load_1d(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
@@ -108,7 +109,7 @@ __device__ __forceinline__ uint32_t odd_bytes(uint32_t w) { /* (b1, 0, b3, 0) */
 
 template <int IN16, int CB, int FMA_H>
 __global__ void __launch_bounds__(NTHREADS, 1)
-k_dedisperse(const __grid_constant__ TmapPack maps, const DedispParams p) {
+k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
     constexpr int ESZ = IN16 ? 2 : 1;
     constexpr int SPW = 4 / ESZ;                 /* samples per word */
     constexpr int NCOPY = SPW;                   /* shifted copies */
@@ -139,29 +140,29 @@ k_dedisperse(const __grid_constant__ TmapPack maps, const DedispParams p) {
     __syncthreads();
 
     if (warp == NW) {
-        /* ------------------------------------------------------------------ producer warp */
-        const int32_t* x0row = p.x0tab + (size_t)dt * (size_t)p.nstages * CB;
-        const int32_t* erow = p.etab + (size_t)dt * (size_t)p.nstages * (CB * DM_TILE);
-        const int c_local = lane % CB, copy = lane / CB;
-        const bool active = lane < NCOPY * CB;
-        const int box_bytes = WB / p.boxes_per_row;
-        int slot = 0; uint32_t ph = 0;
-        for (int s = 0; s < p.nstages; ++s) {
-            const int x0 = active ? __ldg(x0row + s * CB + c_local) : 0;
-            mbar_wait(bar_empty + 8 * slot, ph ^ 1u);
-            const uint32_t fb = bar_full + 8 * slot;
-            if (lane == 0) mbar_arrive_expect_tx(fb, (uint32_t)stage_bytes);
-            __syncwarp();
-            const uint32_t sbase = smem_u32(stages + (size_t)slot * stage_bytes);
-            if (active) {
-                const long long xs = t0 * ESZ + x0;                    /* 16-byte aligned byte coordinate of the window */
-                const int xi = xs > 0x7fff0000ll ? 0x7fff0000 : (int)xs; /* far out of bounds is zero-filled anyway */
-                const uint32_t dst = sbase + (uint32_t)((copy * CB + c_local) * WB);
-                for (int b = 0; b < p.boxes_per_row; ++b)
-                    tma_load_3d(dst + b * box_bytes, &maps.m[copy], xi + b * box_bytes, 0, s * CB + c_local, fb);
+        /* ------------------------------------------------------------------ producer: one elected thread */
+        if (lane == 0) {
+            const int32_t* x0row = p.x0tab + (size_t)dt * (size_t)p.nstages * CB;
+            const int32_t* erow = p.etab + (size_t)dt * (size_t)p.nstages * (CB * DM_TILE);
+            const long long tb = t0 * ESZ;
+            int slot = 0; uint32_t ph = 0;
+            for (int s = 0; s < p.nstages; ++s) {
+                int x0[CB];
+#pragma unroll
+                for (int c = 0; c < CB; ++c) x0[c] = __ldg(x0row + s * CB + c);
+                mbar_wait(bar_empty + 8 * slot, ph ^ 1u);
+                const uint32_t fb = bar_full + 8 * slot;
+                mbar_arrive_expect_tx(fb, (uint32_t)stage_bytes);
+                const uint32_t sbase = smem_u32(stages + (size_t)slot * stage_bytes);
+#pragma unroll
+                for (int c = 0; c < CB; ++c) {
+                    const long long xs = tb + x0[c];                         /* 16-byte aligned byte coordinate of the window */
+                    const int xi = xs > 0x7fff0000ll ? 0x7fff0000 : (int)xs;   /* far out of bounds is zero-filled anyway */
+                    tma_load_4d(sbase + (uint32_t)(c * NCOPY * WB), &map, xi, 0, 0, s * CB + c, fb);
+                }
+                bulk_load_1d(sbase + data_bytes, erow + (size_t)s * (CB * DM_TILE), ENT_BYTES, fb);
+                if (++slot == NSTAGE) { slot = 0; ph ^= 1u; }
             }
-            if (lane == 0) bulk_load_1d(sbase + data_bytes, erow + (size_t)s * (CB * DM_TILE), ENT_BYTES, fb);
-            if (++slot == NSTAGE) { slot = 0; ph ^= 1u; }
         }
         return;
     }
@@ -279,16 +280,15 @@ int launch(const aak_dedisp_args* a, cudaStream_t st) {
     DedispParams p;
     p.etab = a->etab; p.x0tab = a->x0tab; p.D = a->D; p.pitch = a->pitch; p.nt = a->nt; p.ndms = a->ndms;
     p.nstages = (a->nchans + CB - 1) / CB;
-    p.window_bytes = a->window_bytes; p.boxes_per_row = a->boxes_per_row; p.spill_stages = a->spill_stages; p.one = 1u;
+    p.window_bytes = a->window_bytes; p.spill_stages = a->spill_stages; p.one = 1u;
     const size_t smem = SMEM_HEADER + (size_t)NSTAGE * ((size_t)NCOPY * CB * a->window_bytes + CB * DM_TILE * 4);
     const long long ndm_tiles = (a->ndms + DM_TILE - 1) / DM_TILE;
     const long long nt_tiles = (a->nt + T_TILE - 1) / T_TILE;
     const long long grid = ndm_tiles * nt_tiles;
     if (grid <= 0 || grid > 0x7fffffffll) return (int)cudaErrorInvalidConfiguration;
-    TmapPack maps;
-    memset(&maps, 0, sizeof(maps));
-    memcpy(&maps, a->tmap, sizeof(CUtensorMap) * NCOPY);
-    k_dedisperse<IN16, CB, FMA_H><<<(unsigned)grid, NTHREADS, smem, st>>>(maps, p);
+    CUtensorMap map;
+    memcpy(&map, a->tmap, sizeof(CUtensorMap));
+    k_dedisperse<IN16, CB, FMA_H><<<(unsigned)grid, NTHREADS, smem, st>>>(map, p);
     return (int)cudaGetLastError();
 }
 

@@ -61,6 +61,26 @@ k_shift_copy(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, size_t p
     *reinterpret_cast<uint4*>(out + (size_t)blockIdx.y * pitch + (size_t)g * 16) = o;
 }
 
+/* ---- K1a: all four sample-shifted uint8 copies in one pass (reads the chunk once, writes 4 x): copy k at out + k*copy_stride */
+__global__ void __launch_bounds__(256)
+k_make_copies_u8(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, size_t pitch, size_t copy_stride, long long ngroups) {
+    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= ngroups) return;
+    const size_t off = (size_t)blockIdx.y * pitch + (size_t)g * 16;
+    const uint4 a = *reinterpret_cast<const uint4*>(in + off);
+    const uint32_t nx = *reinterpret_cast<const uint32_t*>(in + off + 16);
+    *reinterpret_cast<uint4*>(out + off) = a;
+#pragma unroll
+    for (int k = 1; k < 4; ++k) {
+        uint4 o;
+        o.x = __funnelshift_r(a.x, a.y, 8 * k);
+        o.y = __funnelshift_r(a.y, a.z, 8 * k);
+        o.z = __funnelshift_r(a.z, a.w, 8 * k);
+        o.w = __funnelshift_r(a.w, nx, 8 * k);
+        *reinterpret_cast<uint4*>(out + (size_t)k * copy_stride + off) = o;
+    }
+}
+
 /* ---- K5: sum_t D[i][t] and sum_t t*D[i][t] per row, int64 (all-rows checksum against the prefix-sum identity) */
 __global__ void __launch_bounds__(256)
 k_row_moments(const int32_t* __restrict__ D, long long pitch, long long nt, long long* __restrict__ sum_d,
@@ -136,6 +156,15 @@ extern "C" int aak_shift_copy(const uint8_t* in, uint8_t* out, size_t pitch, siz
     const long long ngroups = (long long)(row_bytes / 16);
     dim3 grid((unsigned)((ngroups + 255) / 256), (unsigned)nrows);
     k_shift_copy<<<grid, 256, 0, (cudaStream_t)stream>>>(in, out, pitch, ngroups, shift_bytes);
+    return (int)cudaGetLastError();
+}
+
+extern "C" int aak_make_copies_u8(const uint8_t* in, uint8_t* out, size_t pitch, size_t copy_stride, size_t row_bytes, int32_t nrows,
+                                  void* stream) {
+    if ((row_bytes & 15) || (pitch & 15) || (copy_stride & 15)) return (int)cudaErrorInvalidValue;
+    const long long ngroups = (long long)(row_bytes / 16);
+    dim3 grid((unsigned)((ngroups + 255) / 256), (unsigned)nrows);
+    k_make_copies_u8<<<grid, 256, 0, (cudaStream_t)stream>>>(in, out, pitch, copy_stride, ngroups);
     return (int)cudaGetLastError();
 }
 
