@@ -125,12 +125,27 @@ k_row_stats(const aak_row_desc* __restrict__ rows, double* __restrict__ mu_sigma
     }
 }
 
-/* ------------------------------------------------------------------------------------------------ K4 */
-constexpr int SPS_ROWS = 8;                    /* centre rows per CTA */
-constexpr int SPS_TT = 512;                    /* centre samples per CTA */
-constexpr int SPS_WARPS = SPS_ROWS + 2;        /* one warp per row incl. the two halo rows */
-constexpr int SPS_THREADS = SPS_WARPS * 32;
-constexpr int SPS_Q = SPS_TT + 2;              /* positions per row incl. the two halo columns */
+/* ------------------------------------------------------------------------------------------------ K4
+ * One CTA walks DOWN a band of K4_RB DM rows (plus one halo row above and below, recomputed, not exchanged) for one
+ * strip of TT output samples. Per row step:
+ *   1. the row segment (TT + 5 + wmax samples, loaded as int4 one step ahead into registers) is turned into inclusive
+ *      prefix sums of d = D - pivot: thread-local serial scan of 4V contiguous samples, warp shuffle scan of the thread
+ *      totals, cross-warp carry through shared memory; the prefix row goes into a 3-row ring in shared memory;
+ *   2. INTEGER prefilter: position t can only exceed the threshold if for some width B_w - w p >= bmin_w, where
+ *      bmin_w = floor(a_w + threshold/inv_w) - 2 is computed once per (row, width) in double (2 below the exact bound:
+ *      conservative, the rounding error of the SNR expression is < 2^-20 in these units). That is 3 integer
+ *      instructions per (sample, width) and no double arithmetic on the common path. Flagged positions are appended
+ *      to a per-row list in shared memory (warp-aggregated);
+ *   3. for each flagged position of the PREVIOUS row (whose lower neighbour row is now in the ring) the exact double
+ *      SNR map S is evaluated on demand for the position and its 8 neighbours, in the operation order of reading C7,
+ *      then S > threshold and the 3x3 rule of reading C8 decide; candidates are appended to the global list with one
+ *      atomic per warp (ballot + popc).
+ * Two __syncthreads per row step. The result is the same set the plain definition gives: step 2 never drops a
+ * position whose S exceeds the threshold, and step 3 is the definition itself.
+ */
+constexpr int K4_THREADS = 256;
+constexpr int K4_WARPS = K4_THREADS / 32;
+constexpr int K4_RB = 32;                      /* centre rows per CTA */
 constexpr int SPS_MAXW = 16;
 
 struct SpsParams {
@@ -139,130 +154,245 @@ struct SpsParams {
     const double* mu_sigma;
     u64 chunk_start;
     int widths[SPS_MAXW]; int nwidths; int wmax;
+    int tt;                                    /* centre samples per strip, multiple of 4 */
     double threshold;
     aak_candidate* cands; u64* counter; u64 capacity;
 };
 
-__global__ void __launch_bounds__(SPS_THREADS)
-k_sps_peaks(const SpsParams p) {
-    extern __shared__ __align__(16) uint8_t sm[];
-    const int NE = SPS_Q + p.wmax;                                   /* samples loaded per row */
-    double* S = reinterpret_cast<double*>(sm);                       /* [SPS_WARPS][SPS_Q] */
-    double* cst = S + SPS_WARPS * SPS_Q;                             /* [SPS_WARPS][2*SPS_MAXW]: a_w, inv_w */
-    int* P = reinterpret_cast<int*>(cst + SPS_WARPS * 2 * SPS_MAXW); /* [SPS_WARPS][NE+1] */
-    unsigned short* Wb = reinterpret_cast<unsigned short*>(P + SPS_WARPS * (NE + 1));   /* [SPS_WARPS][SPS_Q] */
+struct K4RowConst {                            /* per ring slot */
+    double a[SPS_MAXW];                        /* w * (mu - p) */
+    double inv[SPS_MAXW];                      /* 1 / (sqrt(w) * sigma) */
+    int bmin[SPS_MAXW];
+    int live;                                  /* row exists and sigma > 0 */
+    int pad[3];
+};
 
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const i64 t0 = (i64)blockIdx.x * SPS_TT;
-    const int i_base = blockIdx.y * SPS_ROWS;
-    const int rr = i_base - 1 + warp;                                /* this warp's DM row */
-    double* Srow = S + warp * SPS_Q;
-    unsigned short* Wrow = Wb + warp * SPS_Q;
-    const double ninf = -CUDART_INF;
+template <int V>
+struct K4Smem {
+    unsigned I[3][1024 * V];                   /* inclusive prefix sums of d, ring of 3 rows */
+    K4RowConst rc[4];
+    unsigned wtot[K4_WARPS];
+    int cnt[2];
+    unsigned short list[2][1024 * V];
+};
 
-    bool live = (rr >= 0 && rr < p.ndms);
-    double sigma = 0.0, mu = 0.0;
-    if (live) { mu = p.mu_sigma[2 * (size_t)rr]; sigma = p.mu_sigma[2 * (size_t)rr + 1]; live = sigma > 0.0; }
-    if (!live) {
-        for (int q = lane; q < SPS_Q; q += 32) { Srow[q] = ninf; Wrow[q] = 0; }
-    } else {
-        const int32_t* Drow = p.D + (size_t)rr * (size_t)p.pitch;
-        const int pv = Drow[0];
-        int* Prow = P + warp * (NE + 1);
-        double* crow = cst + warp * 2 * SPS_MAXW;
-        if (lane < p.nwidths) {
-            const double w = (double)p.widths[lane];
-            crow[lane] = __dmul_rn(w, __dsub_rn(mu, (double)pv));
-            crow[SPS_MAXW + lane] = __ddiv_rn(1.0, __dmul_rn(__dsqrt_rn(w), sigma));
-        }
-        /* prefix sums of d = D - p over [t0-1, t0-1+NE): wrapping int32, differences are exact (plan limit) */
-        int carry = 0;
-        if (lane == 0) Prow[0] = 0;
-        for (int e0 = 0; e0 < NE; e0 += 32) {
-            const int e = e0 + lane;
-            const i64 t = t0 - 1 + e;
-            int d = 0;
-            if (e < NE && t >= 0 && t < p.nt) d = Drow[t] - pv;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int u = __shfl_up_sync(0xffffffffu, d, o);
-                if (lane >= o) d += u;
-            }
-            d += carry;
-            if (e < NE) Prow[e + 1] = d;
-            carry = __shfl_sync(0xffffffffu, d, 31);
-        }
-        __syncwarp();
-        for (int q = lane; q < SPS_Q; q += 32) {
-            const i64 t = t0 - 1 + q;
-            double best = ninf; int bw = 0;
-            if (t >= 0 && t < p.nt) {
-                const int base = Prow[q];
-                for (int iw = 0; iw < p.nwidths; ++iw) {
-                    const int w = p.widths[iw];
-                    if (t + w > p.nt) break;                       /* ascending widths */
-                    const int B = Prow[q + w] - base;
-                    const double snr = __dmul_rn(__dsub_rn(__int2double_rn(B), crow[iw]), crow[SPS_MAXW + iw]);
-                    if (snr > best) { best = snr; bw = w; }
-                }
-            }
-            Srow[q] = best; Wrow[q] = (unsigned short)bw;
-        }
+/* exact S (reading C7) of one position from a prefix row: e = element index of the position, t = its sample index */
+__device__ __forceinline__ double k4_eval(const unsigned* I, const K4RowConst& rc, const SpsParams& p, int e, i64 t, int& bw) {
+    double best = -CUDART_INF; bw = 0;
+    const unsigned base = I[e - 1];
+    for (int iw = 0; iw < p.nwidths; ++iw) {
+        const int w = p.widths[iw];
+        if (t + w > p.nt) break;                                   /* ascending widths */
+        const int B = (int)(I[e + w - 1] - base);
+        const double snr = __dmul_rn(__dsub_rn(__int2double_rn(B), rc.a[iw]), rc.inv[iw]);
+        if (snr > best) { best = snr; bw = w; }
     }
-    __syncthreads();
+    return best;
+}
 
-    /* 3x3 local maxima on the centre rows/columns; warp-aggregated append */
-    constexpr int NPOS = SPS_ROWS * SPS_TT;
-    for (int k = 0; k < (NPOS + SPS_THREADS - 1) / SPS_THREADS; ++k) {      /* uniform trip count: ballots need every lane */
-        const int idx = k * SPS_THREADS + threadIdx.x;
-        bool is = false; int r = 0, q = 0; double s = 0.0;
-        if (idx < NPOS) {
-            r = idx / SPS_TT + 1; q = idx % SPS_TT + 1;
-            const int i = i_base + r - 1; const i64 t = t0 + q - 1;
-            if (i < p.ndms && t < p.nt) {
-                s = S[r * SPS_Q + q];
-                if (s > p.threshold) {
-                    is = true;
+/* integer prefilter of one row: flags positions that may exceed the threshold, appends them to list (shared memory) */
+template <int NW>
+__device__ __forceinline__ void k4_prefilter(const unsigned* __restrict__ I, const K4RowConst& rc, const SpsParams& p, i64 t0,
+                                             unsigned short* list, int* cnt, int tid, int lane) {
+    int bm[NW];
 #pragma unroll
-                    for (int dr = -1; dr <= 1; ++dr)
+    for (int iw = 0; iw < NW; ++iw) bm[iw] = rc.bmin[iw];
+    for (int q0 = 0; q0 < p.tt; q0 += K4_THREADS) {                  /* uniform trip count: ballots need every lane */
+        const int q = q0 + tid;
+        const i64 t = t0 + q;
+        bool f = false;
+        if (q < p.tt && t < p.nt) {
+            const unsigned* Iq = I + q + 3;                          /* B_w(t) = I[e+w-1] - I[e-1], e = q + 4 */
+            const unsigned base = Iq[0];
+            if (t + p.wmax <= p.nt) {
 #pragma unroll
-                        for (int dq = -1; dq <= 1; ++dq) {
-                            if (dr == 0 && dq == 0) continue;
-                            const double v = S[(r + dr) * SPS_Q + (q + dq)];
-                            const bool before = (dr < 0) || (dr == 0 && dq < 0);
-                            if (before ? !(s > v) : !(s >= v)) is = false;
-                        }
-                }
+                for (int iw = 0; iw < NW; ++iw) f |= ((int)(Iq[p.widths[iw]] - base) >= bm[iw]);
+            } else {
+#pragma unroll
+                for (int iw = 0; iw < NW; ++iw)
+                    if (t + p.widths[iw] <= p.nt) f |= ((int)(Iq[p.widths[iw]] - base) >= bm[iw]);
             }
         }
-        const unsigned mask = __ballot_sync(0xffffffffu, is);
+        const unsigned mask = __ballot_sync(0xffffffffu, f);
         if (mask) {
             const int leader = __ffs(mask) - 1;
-            u64 base = 0;
-            if (lane == leader) base = atomicAdd(p.counter, (u64)__popc(mask));
+            int base = 0;
+            if (lane == leader) base = atomicAdd(cnt, __popc(mask));
             base = __shfl_sync(0xffffffffu, base, leader);
-            if (is) {
-                const u64 slot = base + (u64)__popc(mask & ((1u << lane) - 1u));
-                if (slot < p.capacity) {
-                    const int i = i_base + r - 1;
-                    aak_candidate c;
-                    c.sample = p.chunk_start + (u64)p.bin * (u64)(t0 + q - 1);
-                    c.dm = (float)__dadd_rn(p.dm_low, __dmul_rn((double)i, p.dm_step));
-                    c.snr = (float)s;
-                    c.width = (uint32_t)p.bin * (uint32_t)Wb[r * SPS_Q + q];
-                    c.range = (uint32_t)p.range_index;
-                    c.dm_index = (uint32_t)i;
-                    p.cands[slot] = c;
-                }
-            }
+            if (f) list[base + __popc(mask & ((1u << lane) - 1u))] = (unsigned short)q;
         }
     }
 }
 
-size_t sps_smem_bytes(int wmax) {
-    const int NE = SPS_Q + wmax;
-    return (size_t)SPS_WARPS * SPS_Q * 8 + (size_t)SPS_WARPS * 2 * SPS_MAXW * 8 + (size_t)SPS_WARPS * (NE + 1) * 4 +
-           (size_t)SPS_WARPS * SPS_Q * 2 + 16;
+template <int V>
+__global__ void __launch_bounds__(K4_THREADS)
+k_sps_peaks(const SpsParams p) {
+    extern __shared__ __align__(16) uint8_t k4_raw[];
+    K4Smem<V>& sm = *reinterpret_cast<K4Smem<V>*>(k4_raw);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const i64 t0 = (i64)blockIdx.x * p.tt;
+    const i64 tb = t0 - 4;                                           /* sample index of element 0 of the segment */
+    const int i0 = blockIdx.y * K4_RB;
+    const int i1 = min(i0 + K4_RB, p.ndms);
+    const int e0 = tid * 4 * V;                                      /* this thread's 4V contiguous elements */
+    const int ne = p.tt + 4 + p.wmax;                                /* elements the strip needs */
+
+    int4 cur[V], nxt[V];
+    int pv_c = 0, pv_n = 0;
+    double mu_c = 0.0, sg_c = 0.0, mu_n = 0.0, sg_n = 0.0;
+
+    auto load_row = [&](int r, int4 (&buf)[V], int& pv, double& mu, double& sg) {
+        sg = 0.0; mu = 0.0; pv = 0;
+        if (r < 0 || r >= p.ndms) return;
+        const int32_t* row = p.D + (size_t)r * (size_t)p.pitch;
+        pv = __ldg(row);
+        mu = __ldg(p.mu_sigma + 2 * (size_t)r);
+        sg = __ldg(p.mu_sigma + 2 * (size_t)r + 1);
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            const i64 t = tb + e0 + 4 * v;
+            if (t >= 0 && t < p.nt && e0 + 4 * v < ne) buf[v] = __ldg(reinterpret_cast<const int4*>(row + t));
+            else buf[v] = make_int4(0, 0, 0, 0);
+        }
+    };
+
+    load_row(i0 - 1, cur, pv_c, mu_c, sg_c);
+    if (tid < 2) sm.cnt[tid] = 0;
+    __syncthreads();
+
+    int s = 0;
+    for (int r = i0 - 1; r <= i1; ++r, ++s) {
+        const int s3 = s % 3, s4 = s & 3, sl = s & 1;
+        if (r + 1 <= i1) load_row(r + 1, nxt, pv_n, mu_n, sg_n);      /* one row ahead, in registers */
+        const bool live = sg_c > 0.0;                                /* exists and sigma > 0 */
+
+        /* ---- phase 1: per-row constants, thread-local + warp scan */
+        if (tid < SPS_MAXW) {
+            K4RowConst& rc = sm.rc[s4];
+            if (tid == 0) rc.live = live ? 1 : 0;
+            if (live && tid < p.nwidths) {
+                const double w = (double)p.widths[tid];
+                const double a = __dmul_rn(w, __dsub_rn(mu_c, (double)pv_c));
+                const double inv = __ddiv_rn(1.0, __dmul_rn(__dsqrt_rn(w), sg_c));
+                rc.a[tid] = a; rc.inv[tid] = inv;
+                const double x = a + p.threshold / inv;              /* real-valued bound on B_w - w p; margin below */
+                int bm;
+                if (x != x) bm = INT32_MIN;
+                else if (x >= 2147483000.0) bm = INT32_MAX;
+                else if (x <= -2147483000.0) bm = INT32_MIN;
+                else bm = (int)floor(x) - 2;
+                rc.bmin[tid] = bm;
+            }
+        }
+        unsigned loc[V][4];
+        unsigned run = 0;
+        if (live) {
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+                const i64 t = tb + e0 + 4 * v;
+                const int d[4] = {cur[v].x, cur[v].y, cur[v].z, cur[v].w};
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const bool in = (t + k >= 0) && (t + k < p.nt);
+                    run += in ? (unsigned)(d[k] - pv_c) : 0u;
+                    loc[v][k] = run;
+                }
+            }
+        }
+        unsigned incl = run;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned u = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += u;
+        }
+        if (lane == 31) sm.wtot[warp] = incl;
+        __syncthreads();                                             /* (a) */
+
+        /* ---- phase 2: cross-warp carry, prefix row into the ring */
+        if (live) {
+            unsigned carry = incl - run;
+#pragma unroll
+            for (int w = 0; w < K4_WARPS; ++w) carry += (w < warp) ? sm.wtot[w] : 0u;
+            uint4* dst = reinterpret_cast<uint4*>(&sm.I[s3][e0]);
+#pragma unroll
+            for (int v = 0; v < V; ++v) dst[v] = make_uint4(loc[v][0] + carry, loc[v][1] + carry, loc[v][2] + carry, loc[v][3] + carry);
+        }
+        if (tid == 0) sm.cnt[sl] = 0;
+        __syncthreads();                                             /* (b) */
+
+        /* ---- phase 3a: integer prefilter of row r */
+        if (live && r >= i0 && r < i1) {
+            const unsigned* I = sm.I[s3];
+            const K4RowConst& rc = sm.rc[s4];
+            unsigned short* list = sm.list[sl];
+            int* cnt = &sm.cnt[sl];
+            switch (p.nwidths) {
+#define K4_CASE(N) case N: k4_prefilter<N>(I, rc, p, t0, list, cnt, tid, lane); break;
+                K4_CASE(1) K4_CASE(2) K4_CASE(3) K4_CASE(4) K4_CASE(5) K4_CASE(6) K4_CASE(7) K4_CASE(8)
+                K4_CASE(9) K4_CASE(10) K4_CASE(11) K4_CASE(12) K4_CASE(13) K4_CASE(14) K4_CASE(15) K4_CASE(16)
+#undef K4_CASE
+            }
+        }
+
+        /* ---- phase 3b: exact S and the 3x3 rule for the flagged positions of row r-1 */
+        const int rp = r - 1;
+        if (rp >= i0 && rp < i1) {
+            const int n = sm.cnt[sl ^ 1];
+            const unsigned short* list = sm.list[sl ^ 1];
+            const unsigned* Irow[3] = {sm.I[(s + 1) % 3], sm.I[(s + 2) % 3], sm.I[s3]};          /* rows rp-1, rp, rp+1 */
+            const K4RowConst* rcs[3] = {&sm.rc[(s + 2) & 3], &sm.rc[(s + 3) & 3], &sm.rc[s4]};
+            for (int k0 = 0; k0 < n; k0 += K4_THREADS) {
+                const int k = k0 + tid;
+                bool is = false; int q = 0, bw = 0; double sc = 0.0;
+                if (k < n) {
+                    q = list[k];
+                    const i64 t = t0 + q;
+                    const int e = q + 4;
+                    sc = k4_eval(Irow[1], *rcs[1], p, e, t, bw);
+                    if (sc > p.threshold) {
+                        is = true;
+#pragma unroll
+                        for (int dr = -1; dr <= 1; ++dr) {
+                            if (!rcs[dr + 1]->live) continue;
+#pragma unroll
+                            for (int dq = -1; dq <= 1; ++dq) {
+                                if (dr == 0 && dq == 0) continue;
+                                const i64 tn = t + dq;
+                                if (tn < 0 || tn >= p.nt) continue;
+                                int dummy;
+                                const double v = k4_eval(Irow[dr + 1], *rcs[dr + 1], p, e + dq, tn, dummy);
+                                const bool before = (dr < 0) || (dr == 0 && dq < 0);
+                                if (before ? !(sc > v) : !(sc >= v)) is = false;
+                            }
+                        }
+                    }
+                }
+                const unsigned mask = __ballot_sync(0xffffffffu, is);
+                if (mask) {
+                    const int leader = __ffs(mask) - 1;
+                    u64 base = 0;
+                    if (lane == leader) base = atomicAdd(p.counter, (u64)__popc(mask));
+                    base = __shfl_sync(0xffffffffu, base, leader);
+                    if (is) {
+                        const u64 slot = base + (u64)__popc(mask & ((1u << lane) - 1u));
+                        if (slot < p.capacity) {
+                            aak_candidate c;
+                            c.sample = p.chunk_start + (u64)p.bin * (u64)(t0 + q);
+                            c.dm = (float)__dadd_rn(p.dm_low, __dmul_rn((double)rp, p.dm_step));
+                            c.snr = (float)sc;
+                            c.width = (uint32_t)p.bin * (uint32_t)bw;
+                            c.range = (uint32_t)p.range_index;
+                            c.dm_index = (uint32_t)rp;
+                            p.cands[slot] = c;
+                        }
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int v = 0; v < V; ++v) cur[v] = nxt[v];
+        pv_c = pv_n; mu_c = mu_n; sg_c = sg_n;
+    }
 }
 
 }  // namespace
@@ -274,7 +404,11 @@ extern "C" int aak_row_stats(const aak_row_desc* rows, int32_t nrows, double* mu
 }
 
 extern "C" int aak_sps_init(void) {
-    return (int)cudaFuncSetAttribute(k_sps_peaks, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    int e;
+    if ((e = (int)cudaFuncSetAttribute(k_sps_peaks<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(K4Smem<3>)))) return e;
+    if ((e = (int)cudaFuncSetAttribute(k_sps_peaks<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(K4Smem<4>)))) return e;
+    if ((e = (int)cudaFuncSetAttribute(k_sps_peaks<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(K4Smem<8>)))) return e;
+    return 0;
 }
 
 extern "C" int aak_sps_peaks(const aak_sps_args* a, void* stream) {
@@ -285,9 +419,17 @@ extern "C" int aak_sps_peaks(const aak_sps_args* a, void* stream) {
     p.nwidths = a->nwidths; p.wmax = 0;
     for (int k = 0; k < SPS_MAXW; ++k) { p.widths[k] = k < a->nwidths ? a->widths[k] : 0; if (p.widths[k] > p.wmax) p.wmax = p.widths[k]; }
     p.threshold = a->threshold; p.cands = a->cands; p.counter = (u64*)a->counter; p.capacity = a->capacity;
-    const size_t smem = sps_smem_bytes(p.wmax);
-    if (smem > 200 * 1024) return (int)cudaErrorInvalidValue;
-    dim3 grid((unsigned)((a->nt + SPS_TT - 1) / SPS_TT), (unsigned)((a->ndms + SPS_ROWS - 1) / SPS_ROWS));
-    k_sps_peaks<<<grid, SPS_THREADS, smem, (cudaStream_t)stream>>>(p);
+    if (a->nt <= 0 || a->ndms <= 0) return 0;
+    /* segment = tt + 4 + wmax elements <= 1024 V; the strip keeps at least ~2000 centre samples */
+    const int V = p.wmax <= 1024 ? 3 : (p.wmax <= 2048 ? 4 : 8);
+    if (p.wmax > 6000) return (int)cudaErrorInvalidValue;
+    p.tt = (1024 * V - 4 - p.wmax) & ~3;
+    dim3 grid((unsigned)((a->nt + p.tt - 1) / p.tt), (unsigned)((a->ndms + K4_RB - 1) / K4_RB));
+    cudaStream_t st = (cudaStream_t)stream;
+    switch (V) {
+        case 3: k_sps_peaks<3><<<grid, K4_THREADS, sizeof(K4Smem<3>), st>>>(p); break;
+        case 4: k_sps_peaks<4><<<grid, K4_THREADS, sizeof(K4Smem<4>), st>>>(p); break;
+        default: k_sps_peaks<8><<<grid, K4_THREADS, sizeof(K4Smem<8>), st>>>(p); break;
+    }
     return (int)cudaGetLastError();
 }
