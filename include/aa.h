@@ -81,6 +81,7 @@ typedef struct {
     int64_t n_out;             /* L - S: unbinned output span per full chunk */
     int64_t nchunks;
     int64_t next_chunk;        /* chunk cursor: index of the chunk the next aa_run_dedispersion will process */
+    int32_t shard_rank, shard_world;   /* aa_strategy_shard: this strategy owns chunks rank, rank+world, ... (0, 1 by default) */
     size_t arena_bytes_used;   /* bytes carved from the arena */
     size_t arena_bytes_total;
     size_t max_candidates;
@@ -138,8 +139,16 @@ aa_status aa_strategy_get_chunk(const aa_strategy* s, int64_t chunk, uint64_t* s
 aa_status aa_strategy_get_delay(const aa_strategy* s, int32_t range, int32_t dm_index, int32_t chan, int64_t* delay);
 /* Human-readable dump of chunking, tiling and arena layout into buf (HOST); returns bytes needed incl. NUL. */
 size_t aa_strategy_describe(const aa_strategy* s, char* buf, size_t buflen);
-/* Rewind the chunk cursor to 0 and forget all candidates (the configuration itself is immutable). */
+/* Rewind the chunk cursor to the first chunk of this strategy's shard and forget all candidates (the configuration
+ * itself is immutable). */
 aa_status aa_strategy_reset(aa_strategy* s);
+/* Multi-GPU replicas over time chunks ("parallel pipeline ... execution on multiple GPUs"; DESIGN.md
+ * "Multi-GPU"): this strategy processes only chunks rank, rank+world, rank+2*world, ...  Chunks are independent given
+ * the S-sample overlap, so there is no exchange between ranks; every rank holds its own arena and the host
+ * concatenates the candidate lists. Host-only, also valid on a planned (not ready) strategy. Rewinds the cursor like
+ * aa_strategy_reset. A rank with no chunk (rank >= nchunks) is legal: its first aa_run_dedispersion returns
+ * AA_ERR_ORDER ("all chunks are done"). Errors: AA_ERR_INVALID_ARG unless 0 <= rank < world. */
+aa_status aa_strategy_shard(aa_strategy* s, int32_t rank, int32_t world);
 
 /* ------------------------------------------------------------------------------------------------ pipeline
  * PAPER.md:47 step 7. One call = one chunk of one module.

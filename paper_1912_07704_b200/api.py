@@ -19,7 +19,7 @@ __all__ = [
     "CANDIDATE_DTYPE", "lib_path", "load",
     "aa_plan_create", "aa_plan_destroy", "aa_strategy_plan", "aa_strategy_setup", "aa_strategy_destroy", "aa_strategy_get_info",
     "aa_strategy_get_range_info", "aa_strategy_get_chunk", "aa_strategy_get_delay", "aa_strategy_describe",
-    "aa_strategy_reset", "aa_run_dedispersion", "aa_run_dedispersion_device", "aa_run_sps", "aa_get_candidates",
+    "aa_strategy_reset", "aa_strategy_shard", "aa_run_dedispersion", "aa_run_dedispersion_device", "aa_run_sps", "aa_get_candidates",
     "aa_get_dedispersed_row", "aa_get_row_stats", "aa_get_row_moments", "aa_get_dedispersed_device", "aa_synchronize",
     "aa_measure_int_add_peak", "aa_get_last_timings", "aa_get_launch_count", "aa_last_error", "aa_version",
     "Plan", "Strategy",
@@ -52,7 +52,8 @@ class _RangeInfo(ctypes.Structure):
 class _StrategyInfo(ctypes.Structure):
     _fields_ = [("ready", c_int32), ("nchans", c_int32), ("nranges", c_int32), ("nwidths", c_int32), ("max_bin", c_int32),
                 ("nsamp_total", c_int64), ("overlap", c_int64), ("chunk_len", c_int64), ("n_out", c_int64),
-                ("nchunks", c_int64), ("next_chunk", c_int64), ("arena_bytes_used", c_size_t),
+                ("nchunks", c_int64), ("next_chunk", c_int64), ("shard_rank", c_int32), ("shard_world", c_int32),
+                ("arena_bytes_used", c_size_t),
                 ("arena_bytes_total", c_size_t), ("max_candidates", c_size_t), ("owns_arena", c_int32)]
 
 
@@ -90,6 +91,7 @@ def load():
         "aa_strategy_get_delay": (c_int32, [vp, c_int32, c_int32, c_int32, POINTER(c_int64)]),
         "aa_strategy_describe": (c_size_t, [vp, vp, c_size_t]),
         "aa_strategy_reset": (c_int32, [vp]),
+        "aa_strategy_shard": (c_int32, [vp, c_int32, c_int32]),
         "aa_run_dedispersion": (c_int32, [vp, vp, c_size_t]),
         "aa_run_dedispersion_device": (c_int32, [vp, vp, c_size_t]),
         "aa_run_sps": (c_int32, [vp]),
@@ -212,6 +214,10 @@ def aa_strategy_reset(strategy) -> int:
     return _check(load().aa_strategy_reset(strategy))
 
 
+def aa_strategy_shard(strategy, rank: int, world: int) -> int:
+    return _check(load().aa_strategy_shard(strategy, int(rank), int(world)))
+
+
 # ---------------------------------------------------------------------------------------------- pipeline
 def aa_run_dedispersion(strategy, host_input, row_stride_bytes=None) -> int:
     """host_input: uint8 numpy array / pinned torch tensor [nchans][nsamp_total] (or a raw host address)."""
@@ -317,12 +323,20 @@ class Strategy:
         self.ranges = plan.ranges
         self.info = aa_strategy_get_info(self.handle)
 
+    def shard(self, rank: int, world: int) -> None:
+        """Own chunks rank, rank+world, ... only (replicas over time chunks, one strategy per GPU)."""
+        aa_strategy_shard(self.handle, rank, world)
+        self.info = aa_strategy_get_info(self.handle)
+
     def run(self, host_input) -> np.ndarray:
-        """The paper's pipeline loop: dedispersion then SPS per chunk until FINISHED."""
-        while True:
-            aa_run_dedispersion(self.handle, host_input)
-            if aa_run_sps(self.handle) == AA_STATUS_FINISHED:
-                break
+        """The paper's pipeline loop: dedispersion then SPS per chunk of this strategy's shard until
+        FINISHED; returns the candidates of those chunks."""
+        info = aa_strategy_get_info(self.handle)
+        if info["next_chunk"] < info["nchunks"]:
+            while True:
+                aa_run_dedispersion(self.handle, host_input)
+                if aa_run_sps(self.handle) == AA_STATUS_FINISHED:
+                    break
         return aa_get_candidates(self.handle)
 
     def close(self):

@@ -109,6 +109,7 @@ struct Strategy {
 
     /* cursor / state */
     int64_t next_chunk = 0;
+    int32_t shard_rank = 0, shard_world = 1;   /* aa_strategy_shard */
     int64_t current_chunk = -1;        /* chunk whose D is on the device */
     bool pending_sps = false;
     int64_t raw_holds[2] = {-1, -1};   /* which chunk each raw buffer holds (or is receiving) */

@@ -116,7 +116,7 @@ extern "C" aa_status aa_run_dedispersion(aa_strategy* h, const uint8_t* host_inp
     if (s.pending_sps) { set_error("aa_run_dedispersion: chunk %lld is dedispersed but aa_run_sps has not run on it yet", (long long)s.current_chunk); return AA_ERR_ORDER; }
     if (s.next_chunk >= (int64_t)s.chunks.size()) { set_error("aa_run_dedispersion: all %zu chunks are done (aa_strategy_reset rewinds)", s.chunks.size()); return AA_ERR_ORDER; }
     const int64_t j = s.next_chunk;
-    const int b = s.d_raw[1] ? (int)(j & 1) : 0;
+    const int b = s.d_raw[1] ? (int)((j / s.shard_world) & 1) : 0;
     s.h2d_timed = false;
     if (s.raw_holds[b] != j) {
         if ((st = enqueue_h2d(s, j, b, host_input, row_stride_bytes, true)) != AA_OK) return st;
@@ -125,8 +125,9 @@ extern "C" aa_status aa_run_dedispersion(aa_strategy* h, const uint8_t* host_inp
     AA_CUDA(cudaStreamWaitEvent(s.compute, s.ev_copied[b], 0), "cudaStreamWaitEvent");
     if ((st = enqueue_dedispersion(s, j, b)) != AA_OK) return st;
     /* double buffering: start moving chunk j+1 while chunk j computes (north_star "Streaming") */
-    if (s.d_raw[1] && j + 1 < (int64_t)s.chunks.size() && s.raw_holds[b ^ 1] != j + 1)
-        if ((st = enqueue_h2d(s, j + 1, b ^ 1, host_input, row_stride_bytes, false)) != AA_OK) return st;
+    const int64_t jn = j + s.shard_world;           /* the next chunk of this strategy's shard */
+    if (s.d_raw[1] && jn < (int64_t)s.chunks.size() && s.raw_holds[b ^ 1] != jn)
+        if ((st = enqueue_h2d(s, jn, b ^ 1, host_input, row_stride_bytes, false)) != AA_OK) return st;
     return AA_OK;
 }
 
@@ -140,7 +141,7 @@ extern "C" aa_status aa_run_dedispersion_device(aa_strategy* h, const uint8_t* d
     const int64_t j = s.next_chunk;
     const Chunk& c = s.chunks[(size_t)j];
     if (row_stride_bytes < c.len) { set_error("aa_run_dedispersion_device: row_stride_bytes = %zu is shorter than the chunk (%llu)", row_stride_bytes, (unsigned long long)c.len); return AA_ERR_INVALID_ARG; }
-    const int b = s.d_raw[1] ? (int)(j & 1) : 0;
+    const int b = s.d_raw[1] ? (int)((j / s.shard_world) & 1) : 0;
     s.h2d_timed = false;
     AA_CUDA(cudaMemcpy2DAsync(s.d_raw[b], s.in_pitch, device_chunk, row_stride_bytes, (size_t)c.len, (size_t)s.plan.nchans,
                               cudaMemcpyDeviceToDevice, s.compute), "cudaMemcpy2DAsync (D2D chunk)");
@@ -177,7 +178,7 @@ extern "C" aa_status aa_run_sps(aa_strategy* h) {
     AA_CUDA(cudaEventRecord(s.ev_count, s.compute), "cudaEventRecord");
     s.harvest_pending = true; s.harvest_chunk = j; s.stats_timed = true;
     s.pending_sps = false;
-    s.next_chunk = j + 1;
+    s.next_chunk = j + s.shard_world;
     return s.next_chunk >= (int64_t)s.chunks.size() ? AA_STATUS_FINISHED : AA_STATUS_CHUNK_DONE;
 }
 
@@ -199,13 +200,20 @@ extern "C" aa_status aa_get_candidates(aa_strategy* h, const aa_candidate** out,
 extern "C" aa_status aa_strategy_reset(aa_strategy* h) {
     if (!h) { set_error("aa_strategy_reset: strategy is NULL"); return AA_ERR_NOT_READY; }
     Strategy& s = h->s;
-    cudaStreamSynchronize(s.compute);
-    cudaStreamSynchronize(s.copy);
-    s.next_chunk = 0; s.current_chunk = -1; s.pending_sps = false; s.harvest_pending = false;
+    if (s.compute) cudaStreamSynchronize(s.compute);
+    if (s.copy) cudaStreamSynchronize(s.copy);
+    s.next_chunk = s.shard_rank; s.current_chunk = -1; s.pending_sps = false; s.harvest_pending = false;
     s.raw_holds[0] = s.raw_holds[1] = -1;
     s.cands.clear(); s.true_count = 0; s.overflow = false; s.launches = 0; s.timed = false; s.stats_timed = false;
     if (s.sticky != AA_ERR_CUDA) s.sticky = AA_OK;
     return AA_OK;
+}
+
+extern "C" aa_status aa_strategy_shard(aa_strategy* h, int32_t rank, int32_t world) {
+    if (!h) { set_error("aa_strategy_shard: strategy is NULL"); return AA_ERR_NOT_READY; }
+    if (world < 1 || rank < 0 || rank >= world) { set_error("aa_strategy_shard: need 0 <= rank < world, got rank = %d, world = %d", rank, world); return AA_ERR_INVALID_ARG; }
+    h->s.shard_rank = rank; h->s.shard_world = world;
+    return aa_strategy_reset(h);
 }
 
 extern "C" aa_status aa_synchronize(aa_strategy* h) {

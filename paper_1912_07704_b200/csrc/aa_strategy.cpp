@@ -377,6 +377,7 @@ extern "C" aa_status aa_strategy_get_info(const aa_strategy* h, aa_strategy_info
     out->nchans = s.plan.nchans; out->nranges = (int32_t)s.ranges.size(); out->nwidths = (int32_t)s.plan.widths.size();
     out->max_bin = s.B; out->nsamp_total = (int64_t)s.nsamp_total; out->overlap = s.S; out->chunk_len = s.L; out->n_out = s.n_out;
     out->nchunks = (int64_t)s.chunks.size(); out->next_chunk = s.next_chunk;
+    out->shard_rank = s.shard_rank; out->shard_world = s.shard_world;
     out->arena_bytes_used = s.arena.used; out->arena_bytes_total = s.arena.size; out->max_candidates = s.max_candidates;
     out->owns_arena = s.owns_arena ? 1 : 0;
     return AA_OK;
