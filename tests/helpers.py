@@ -94,6 +94,68 @@ def row_moments_from_input(x: np.ndarray, k: np.ndarray, rng, start: int, length
     return m0, m1
 
 
+def row_moments_all_ranges(x: np.ndarray, k: np.ndarray, ranges, start: int, length: int, n_out: int, chan_block: int = 32,
+                           threads: int | None = None):
+    """The same identity as row_moments_from_input for EVERY row of EVERY range of a full-size chunk: the per-channel
+    prefix sums P, Q are formed once per time-binning factor and shared by the ranges that use it; channel blocks run on
+    a thread pool (numpy releases the GIL in cumsum). Returns [(m0, m1)] per range, int64 modulo 2^64."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    C = x.shape[0]
+    by_bin = {}
+    for r, rng in enumerate(ranges):
+        by_bin.setdefault(rng[3], []).append(r)
+    tables = {r: oracle.delay_table(k, rng) for r, rng in enumerate(ranges)}
+    out = {r: [np.zeros(rng[2], np.int64), np.zeros(rng[2], np.int64)] for r, rng in enumerate(ranges)}
+
+    def block(b, c0):
+        c1 = min(C, c0 + chan_block)
+        nb = length // b
+        xb = oracle.bin_time(x[c0:c1], start, nb, b).astype(np.int64)
+        P = np.zeros((c1 - c0, nb + 1), np.int64)
+        Q = np.zeros((c1 - c0, nb + 1), np.int64)
+        np.cumsum(xb, axis=1, out=P[:, 1:])
+        xb *= np.arange(nb, dtype=np.int64)
+        np.cumsum(xb, axis=1, out=Q[:, 1:])
+        ch = np.arange(c1 - c0)[None, :]
+        res = {}
+        with np.errstate(over="ignore"):
+            for r in by_bin[b]:
+                T = n_out // b
+                d = tables[r][:, c0:c1]
+                dP = P[ch, d + T] - P[ch, d]
+                dQ = Q[ch, d + T] - Q[ch, d]
+                res[r] = (dP.sum(axis=1), (dQ - d * dP).sum(axis=1))
+        return res
+
+    jobs = [(b, c0) for b in sorted(by_bin) for c0 in range(0, C, chan_block)]
+    with ThreadPoolExecutor(max_workers=threads or min(16, os.cpu_count() or 1)) as ex:
+        for res in ex.map(lambda j: block(*j), jobs):
+            with np.errstate(over="ignore"):
+                for r, (a0, a1) in res.items():
+                    out[r][0] += a0
+                    out[r][1] += a1
+    return [tuple(out[r]) for r in range(len(ranges))]
+
+
+def sampled_outputs(x: np.ndarray, k: np.ndarray, rng, start: int, T: int, points):
+    """D[i][t'] of single outputs, each computed on its own from the definition (reading C5): the oracle's delay row of
+    DM i, the oracle's binning of just the b input samples each channel contributes, one sum over channels.
+    points: iterable of (i, t'). Returns int64 array."""
+    b = rng[3]
+    C = x.shape[0]
+    ch = np.arange(C)
+    out = []
+    for (i, t) in points:
+        d = oracle.delay_table(k, rng, i, i + 1)[0]                 # [C] binned samples
+        u = start + (t + d) * b                                     # first unbinned sample of each channel's bin
+        acc = 0
+        for j in range(b):
+            acc += int(x[ch, u + j].astype(np.int64).sum())
+        out.append(acc)
+    return np.array(out, np.int64)
+
+
 class GpuRun:
     """The CUDA path through the C-ABI binding for one workload (plan -> strategy -> chunk loop)."""
 

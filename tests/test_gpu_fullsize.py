@@ -1,0 +1,88 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (one chunk, the strategy's own
+tiling): Mid (configs[1]) and SKA-like (configs[2], the headline workload). The full oracle would take an hour here, so
+(SURVEY §8(c) "Verification coverage"):
+  1. EVERY row of every range: sum_t D and sum_t t*D equal the values derived from the input's prefix sums (exact, int64);
+  2. sampled single outputs D[i][t'], each computed on its own from the definition (random points + the corners of
+     every range + tile-boundary columns), bit-exact;
+  3. bands of 5 adjacent DM rows (first / middle / last of each range, plus the rows of injected pulses): bit-exact D,
+     identical mu/sigma, identical candidates.
+"""
+import numpy as np
+import pytest
+
+import datagen
+
+from helpers import (GpuRun, OracleRun, band_rows, check_band, compare_candidates, make_input, row_moments_all_ranges,
+                     sampled_outputs)
+
+pytestmark = pytest.mark.gpu
+
+
+def _points(rng_np, ndms, T, n):
+    pts = [(0, 0), (0, T - 1), (ndms - 1, 0), (ndms - 1, T - 1)]
+    for t in (1023, 1024, 1025, T - 1024, (T // 1024) * 1024 - 1, (T // 1024) * 1024):      # K2 time-tile edges
+        if 0 <= t < T:
+            pts.append((int(rng_np.integers(0, ndms)), int(t)))
+    for i in (31, 32, ndms - 33, (ndms // 32) * 32 - 1, (ndms // 32) * 32):                 # K2 DM-tile edges
+        if 0 <= i < ndms:
+            pts.append((int(i), int(rng_np.integers(0, T))))
+    while len(pts) < n:
+        pts.append((int(rng_np.integers(0, ndms)), int(rng_np.integers(0, T))))
+    return pts
+
+
+def _fullsize(name, points_per_range, pulse_bands):
+    w = datagen.get_workload(name)
+    x, pinned = make_input(w, pinned=True)
+    before = datagen.checksum(x)
+    gpu, orc = GpuRun(w, x, max_candidates=1 << 22), OracleRun(w, x)
+    try:
+        assert gpu.info["nchunks"] == 1
+        chunk = gpu.chunks[0]
+        start, length, n_out = chunk
+        gpu.dedisperse()
+        # 1. every row, two exact moments
+        exp = row_moments_all_ranges(x, orc.k, w.ranges, start, length, n_out)
+        for r, rng in enumerate(w.ranges):
+            m0, m1 = gpu.moments(r)
+            bad = np.flatnonzero((m0 != exp[r][0]) | (m1 != exp[r][1]))
+            assert bad.size == 0, f"{name} range {r}: moment identity fails on rows {bad[:10]} ({bad.size} rows)"
+        # 2. sampled outputs, one by one
+        rs = np.random.default_rng(w.seed)
+        for r, rng in enumerate(w.ranges):
+            T = n_out // rng[3]
+            pts = _points(rs, rng[2], T, points_per_range)
+            want = sampled_outputs(x, orc.k, rng, start, T, pts)
+            rows = {}
+            for (i, t), e in zip(pts, want):
+                if i not in rows:
+                    rows[i] = gpu.row(r, i)
+                assert int(rows[i][t]) == int(e), f"{name} range {r} D[{i}][{t}] = {int(rows[i][t])}, definition gives {int(e)}"
+        # 3. bands with statistics and candidates
+        gpu.sps()
+        got = gpu.candidates(allow_overflow=False)
+        pl, dms, _ = w.pulses()
+        nb = 0
+        for r, rng in enumerate(w.ranges):
+            centres = [0, rng[2] // 2, rng[2] - 1]
+            hi = rng[0] + rng[1] * rng[2]
+            centres += [int(round((d - rng[0]) / rng[1])) for d in dms[:pulse_bands] if rng[0] <= d < hi]
+            for (i0, i1) in band_rows(rng[2], [min(rng[2] - 1, max(0, c)) for c in centres]):
+                e = check_band(gpu, orc, chunk, r, i0, i1, after_sps=True)
+                sel = (got["range"] == r) & (got["dm_index"] >= i0) & (got["dm_index"] < i1)
+                compare_candidates(got[sel], e, w.threshold)
+                nb += 1
+        assert datagen.checksum(x) == before          # the user's input is never written
+        return gpu.info, len(got), nb
+    finally:
+        gpu.close()
+
+
+def test_mid_full_size():
+    info, ncand, nb = _fullsize("mid", points_per_range=400, pulse_bands=6)
+    assert (info["overlap"], info["n_out"]) == (7243, 254901) and nb >= 3 and ncand > 0
+
+
+def test_ska_full_size_headline_workload():
+    info, ncand, nb = _fullsize("ska", points_per_range=200, pulse_bands=4)
+    assert (info["overlap"], info["n_out"], info["max_bin"]) == (32384, 491904, 8) and nb >= 15 and ncand > 0

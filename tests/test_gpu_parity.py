@@ -162,3 +162,37 @@ def test_chunked_run_matches_oracle_per_chunk_and_is_chunk_invariant():
     finally:
         one.close()
         many.close()
+
+
+# ------------------------------------------------------------------------------------------------ replicas over chunks (N > 1 path)
+def test_sharded_strategies_partition_the_chunks_and_reproduce_the_single_run():
+    """rank r of W owns chunks r, r+W, ...; no exchange. Two sharded strategies (run one after
+    the other on this one GPU, each with its own arena, as two ranks would) give together exactly the unsharded list."""
+    from paper_1912_07704_b200 import replicas
+    w = scaled(datagen.get_workload("mid"), nsamp=40_000, name="mid40k", ranges=((0.0, 0.5, 120, 1), (60.0, 1.0, 40, 2)))
+    x, pinned = make_input(w, pinned=True)
+    one = GpuRun(w, x, chunk_len_hint=9_000)
+    try:
+        ref = one.st.run(x)
+        nchunks, n_out = one.info["nchunks"], one.info["n_out"]
+    finally:
+        one.close()
+    assert nchunks >= 4 and len(ref) > 0
+    parts, owned = [], []
+    for rank in range(2):
+        g = GpuRun(w, x, chunk_len_hint=9_000)
+        try:
+            g.st.shard(rank, 2)
+            assert g.st.info["next_chunk"] == rank
+            c = g.st.run(x)
+            mine = replicas.chunks_of_rank(nchunks, rank, 2)
+            assert set((c["sample"] // n_out).tolist()) <= set(mine)
+            parts.append(c)
+            owned += mine
+        finally:
+            g.close()
+    assert sorted(owned) == list(range(nchunks))
+    merged = replicas.canonical_order(np.concatenate(parts), n_out)
+    assert len(merged) == len(ref)
+    for f in ref.dtype.names:
+        assert np.array_equal(merged[f], ref[f]), f
