@@ -40,7 +40,8 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="ska", help="tiny | mid | ska | lowf (BASELINE.json configs 0..3)")
+    ap.add_argument("--workload", default="ska", help="tiny | mid | ska | lowf | stream (BASELINE.json configs 0..4); "
+                    "stream = the 600 s chunked pipeline under a 40 GB budget, a step is the whole stream")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -298,12 +299,104 @@ def run_ours(args, w):
         dist.destroy_process_group()
 
 
+def run_stream(args, w):
+    """BASELINE.json configs[4]: the whole observation stays in pinned HOST memory; the strategy splits it into
+    overlapping chunks under the budget; H2D of chunk n+1 is double-buffered over dedispersion+SPS of chunk n.
+    A step = the whole stream. `value` = units / sum of the per-chunk kernel times (CUDA events, chunk resident);
+    `e2e` = units / wall clock of the overlapped run loop (host pointer in, candidate list out)."""
+    import torch
+    import datagen
+    import paper_1912_07704_b200 as aa
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    assert int(os.environ.get("WORLD_SIZE", "1")) == 1, "the stream workload is a single-GPU configuration (BASELINE.json)"
+    torch.cuda.set_device(0)
+    pl, dms, dl = w.pulses()
+    t0 = time.perf_counter()
+    xh = torch.empty((w.nchans, w.nsamp), dtype=torch.uint8, pin_memory=True)
+    x = xh.numpy()
+    datagen.generate(w.seed, w.nchans, w.nsamp, pl, dl, out=x)
+    gen_s = time.perf_counter() - t0
+    compute, copy = torch.cuda.Stream(), torch.cuda.Stream()
+    plan = aa.Plan(w.freqs_mhz, w.tsamp_s, w.ranges, w.widths, w.threshold)
+    st = aa.Strategy(plan, w.nsamp, budget_bytes=w.budget_bytes, compute_stream=compute, copy_stream=copy, max_candidates=1 << 23)
+    h, info = st.handle, st.info
+    chunks = [aa.aa_strategy_get_chunk(h, j) for j in range(info["nchunks"])]
+    outputs = sum(outputs_of(w, c[2]) for c in chunks)
+
+    def pass_timed():                       # kernels only: reading the timings synchronises after every chunk
+        aa.aa_strategy_reset(h)
+        ms = {"bin_ms": 0.0, "dedisp_ms": 0.0, "stats_ms": 0.0, "peaks_ms": 0.0}
+        n = 0
+        while True:
+            aa.aa_run_dedispersion(h, x, xh.stride(0))
+            status = aa.aa_run_sps(h)
+            tm = aa.aa_get_last_timings(h)
+            for k in ms:
+                ms[k] += tm[k]
+            n = aa.aa_get_launch_count(h)
+            if status == aa.AA_STATUS_FINISHED:
+                return ms, n
+
+    def pass_e2e():
+        aa.aa_strategy_reset(h)
+        t = time.perf_counter()
+        c = st.run(x)
+        torch.cuda.synchronize()
+        return time.perf_counter() - t, c
+
+    for _ in range(min(args.warmup, 1)):
+        pass_e2e()
+    sampler = ClockSampler(0)
+    sampler.start()
+    kern, launches, e2e_s, ncand, d2h = [], 0, [], 0, 0
+    for _ in range(args.steps):
+        ms, n = pass_timed()
+        kern.append(ms)
+        launches += n
+        dt, c = pass_e2e()
+        e2e_s.append(dt)
+        ncand, d2h = len(c), c.nbytes + 8 * len(chunks)
+    sampler.stop_flag = True
+    sampler.join()
+    mean = lambda key: float(np.mean([k[key] for k in kern]))
+    step_ms = mean("bin_ms") + mean("dedisp_ms") + mean("stats_ms") + mean("peaks_ms")
+    adds = outputs * w.nchans
+    k2 = mean("dedisp_ms") * 1e-3
+    peak = SM_COUNT * INT_LANES_PER_SM_CLK * (sampler.max_mhz or 1965) * 1e6
+    e2e_mean = float(np.mean(e2e_s))
+    duration = w.nsamp * w.tsamp_s
+    line = {"metric": METRIC, "value": outputs / (step_ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": min(args.warmup, 1), "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "int32", "data": "synthetic",
+            "config": {"workload": w.name, "nchans": w.nchans, "nsamp": w.nsamp, "tsamp_us": w.tsamp_s * 1e6, "ndms": w.ndms_total,
+                       "budget_bytes": w.budget_bytes, "chunk_len": info["chunk_len"], "overlap": info["overlap"],
+                       "nchunks": info["nchunks"], "arena_bytes": info["arena_bytes_used"], "outputs_per_step": outputs,
+                       "l2": "inputs larger than L2 (each chunk %.2f GB in)" % (w.nchans * info["chunk_len"] / 1e9),
+                       "parallelism": "single GPU, double-buffered H2D", "host_generation_s": gen_s},
+            "realtime_factor": duration / (step_ms * 1e-3), "realtime_factor_e2e": duration / e2e_mean,
+            "breakdown_ms": {"bin_and_shift": mean("bin_ms"), "dedispersion": mean("dedisp_ms"), "row_stats": mean("stats_ms"),
+                             "sps_peaks": mean("peaks_ms")},
+            "candidates_per_step": ncand, "clocks": sampler.summary(),
+            "e2e": {"value": outputs / e2e_mean, "unit": UNIT, "h2d_bytes_per_step": int(sum(w.nchans * c[1] for c in chunks)),
+                    "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * e2e_mean,
+                    "timer": "host wall clock around the run loop (aa_run_dedispersion(host) / aa_run_sps per chunk, aa_get_candidates)"},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "alu", "kernel": "k_dedisperse (K2), all ranges of all chunks", "achieved": adds / k2 / 1e12,
+                         "peak": peak / 1e12, "unit": "Tadd/s (algorithmic 32-bit integer adds)", "frac": adds / k2 / peak,
+                         "traffic": None, "k2_ms_per_step": k2 * 1e3, "algorithmic_adds_per_step": adds}}
+    print(json.dumps(line), flush=True)
+    st.close()
+    plan.close()
+
+
 def main():
     args = parse()
     import datagen
     w = datagen.get_workload(args.workload)
     if args.impl == "reference":
         run_reference(args, w)
+    elif w.budget_bytes:
+        run_stream(args, w)
     else:
         run_ours(args, w)
 

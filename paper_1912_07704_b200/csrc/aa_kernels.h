@@ -51,6 +51,7 @@ typedef struct {
     int32_t spill_stages;      /* carry the 16-bit lanes every this many stages: (256/bin)/chan_block */
     int32_t in16;              /* 0: uint8 input (bin 1), 1: uint16 input (binned) */
     int32_t variant;           /* uint8 only: 1 = odd-byte lane adds issued as IMAD (FMA pipe), 0 = fused IADD3 */
+    int32_t dms_per_warp;      /* 2 or 4 adjacent DM trials per warp (words of equal-delay trials are reused from registers) */
 } aak_dedisp_args;
 int aak_dedisperse(const aak_dedisp_args* a, void* stream);
 size_t aak_dedisperse_smem_bytes(int32_t chan_block, int32_t window_bytes, int32_t in16);

@@ -10,6 +10,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -140,6 +141,12 @@ static bool plan_range(Strategy& s, Range& rg, std::vector<int32_t>& etab, std::
     for (int cb = 8; cb >= 2; cb /= 2)
         if (aak_dedisperse_smem_bytes(cb, rg.window_bytes, rg.in16) <= 227 * 1024) { rg.chan_block = cb; break; }
     if (!rg.chan_block) { set_error("aa_strategy_setup: range %d: channel window of %d bytes does not fit shared memory", rg.index, rg.window_bytes); return false; }
+    rg.dms_per_warp = rg.in16 ? 4 : 2;
+    rg.variant = 1;
+#ifdef AA_TUNING
+    if (const char* ev = getenv(rg.in16 ? "AA_K2_M16" : "AA_K2_M8")) rg.dms_per_warp = atoi(ev) == 4 ? 4 : 2;
+    if (const char* ev = getenv("AA_K2_VARIANT")) rg.variant = atoi(ev);
+#endif
     rg.nstages = (C + rg.chan_block - 1) / rg.chan_block;
     rg.spill_stages = (256 / rg.r.bin) / rg.chan_block;
     const int32_t CB = rg.chan_block, Cpad = rg.nstages * CB, WB = rg.window_bytes;

@@ -40,9 +40,8 @@
 namespace {
 
 constexpr int NW = 16;               /* compute warps */
-constexpr int M = 2;                 /* DM trials per warp */
-constexpr int DM_TILE = NW * M;      /* 32 */
-constexpr int T_TILE = 1024;
+constexpr int DM_TILE = 32;          /* DM trials per CTA */
+constexpr int T_TILE = 1024;         /* output samples per CTA */
 constexpr int NSTAGE = 3;
 constexpr int NTHREADS = (NW + 1) * 32;
 constexpr int SMEM_HEADER = 1024;    /* mbarriers live here; keeps the stages 1024-byte aligned */
@@ -107,14 +106,22 @@ __device__ __forceinline__ uint32_t odd_bytes(uint32_t w) { /* (b1, 0, b3, 0) */
     return d;
 }
 
-template <int IN16, int CB, int FMA_H>
+/* M = adjacent DM trials per warp. The 16 compute warps form 32/M DM groups x NTH = 16*M/32 time parts of the tile.
+ * Adjacent DM trials often have the SAME delay in a channel (the delay grows by less than one sample per DM step over
+ * much of the band): the words loaded for trial m-1 are then exactly the words trial m needs, and are reused from
+ * registers instead of being read from shared memory again (a warp-uniform test of two table entries). */
+template <int IN16, int CB, int FMA_H, int M>
 __global__ void __launch_bounds__(NTHREADS, 1)
 k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
     constexpr int ESZ = IN16 ? 2 : 1;
     constexpr int SPW = 4 / ESZ;                 /* samples per word */
     constexpr int NCOPY = SPW;                   /* shifted copies */
-    constexpr int J = T_TILE / (32 * SPW);       /* words per thread per DM: 8 (u8) or 16 (u16) */
+    constexpr int NG = DM_TILE / M;              /* DM groups */
+    constexpr int NTH = NW / NG;                 /* time parts */
+    constexpr int T_PART = T_TILE / NTH;
+    constexpr int J = T_PART / (32 * SPW);       /* words per thread per DM */
     constexpr int ENT_BYTES = CB * DM_TILE * 4;
+    static_assert(NG * NTH == NW && NTH >= 1 && J >= 1, "warp layout");
 
     extern __shared__ __align__(1024) uint8_t smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -179,32 +186,71 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
             if (!IN16) { H[m][j] = 0; C2[m][j] = 0; }
         }
 
-    const int ent_off = data_bytes + warp * M * 4;
+    const int grp = warp % NG, part = warp / NG;
+    const int ent_off = data_bytes + grp * M * 4;
     int until_spill = p.spill_stages;
     int slot = 0; uint32_t ph = 0;
     for (int s = 0; s < p.nstages; ++s) {
         mbar_wait(bar_full + 8 * slot, ph);
         const uint8_t* sb = stages + (size_t)slot * stage_bytes;
-        const uint8_t* db = sb + lane * 4;
+        const uint8_t* db = sb + lane * 4 + part * (T_PART * ESZ);
+        if (M == 2) {
+            /* two trials per warp: every word is loaded where it is used (no registers to spare for reuse) */
 #pragma unroll
-        for (int cp = 0; cp < CB / 2; ++cp) {
-            const uint2 e1 = *reinterpret_cast<const uint2*>(sb + ent_off + (2 * cp) * (DM_TILE * 4));
-            const uint2 e2 = *reinterpret_cast<const uint2*>(sb + ent_off + (2 * cp + 1) * (DM_TILE * 4));
+            for (int cp = 0; cp < CB / 2; ++cp) {
+                const uint2 e1 = *reinterpret_cast<const uint2*>(sb + ent_off + (2 * cp) * (DM_TILE * 4));
+                const uint2 e2 = *reinterpret_cast<const uint2*>(sb + ent_off + (2 * cp + 1) * (DM_TILE * 4));
 #pragma unroll
-            for (int m = 0; m < M; ++m) {
-                const uint8_t* a1 = db + (m == 0 ? e1.x : e1.y);
-                const uint8_t* a2 = db + (m == 0 ? e2.x : e2.y);
+                for (int m = 0; m < 2; ++m) {
+                    const uint8_t* a1 = db + (m == 0 ? e1.x : e1.y);
+                    const uint8_t* a2 = db + (m == 0 ? e2.x : e2.y);
 #pragma unroll
-                for (int j = 0; j < J; ++j) {
-                    const uint32_t w1 = *reinterpret_cast<const uint32_t*>(a1 + j * 128);
-                    const uint32_t w2 = *reinterpret_cast<const uint32_t*>(a2 + j * 128);
-                    A[m][j] = A[m][j] + w1 + w2;
-                    if (!IN16) {
-                        if (FMA_H) {
-                            H[m][j] = add_fma_pipe(odd_bytes(w1), one, H[m][j]);
-                            H[m][j] = add_fma_pipe(odd_bytes(w2), one, H[m][j]);
-                        } else {
-                            H[m][j] = H[m][j] + odd_bytes(w1) + odd_bytes(w2);
+                    for (int j = 0; j < J; ++j) {
+                        const uint32_t w1 = *reinterpret_cast<const uint32_t*>(a1 + j * 128);
+                        const uint32_t w2 = *reinterpret_cast<const uint32_t*>(a2 + j * 128);
+                        A[m][j] = A[m][j] + w1 + w2;
+                        if (!IN16) {
+                            if (FMA_H) {
+                                H[m][j] = add_fma_pipe(odd_bytes(w1), one, H[m][j]);
+                                H[m][j] = add_fma_pipe(odd_bytes(w2), one, H[m][j]);
+                            } else {
+                                H[m][j] = H[m][j] + odd_bytes(w1) + odd_bytes(w2);
+                            }
+                        }
+                    }
+                }
+            }
+        } else {
+            /* four adjacent trials per warp: the words of trial m-1 are reused when trial m has the same delay */
+#pragma unroll 1
+            for (int cp = 0; cp < CB / 2; ++cp) {
+                const uint4 ea = *reinterpret_cast<const uint4*>(sb + ent_off + (2 * cp) * (DM_TILE * 4));
+                const uint4 eb = *reinterpret_cast<const uint4*>(sb + ent_off + (2 * cp + 1) * (DM_TILE * 4));
+                const uint32_t e1[4] = {ea.x, ea.y, ea.z, ea.w};
+                const uint32_t e2[4] = {eb.x, eb.y, eb.z, eb.w};
+                uint32_t w1[J], w2[J];
+#pragma unroll
+                for (int m = 0; m < M; ++m) {
+                    if (m == 0 || e1[m] != e1[m - 1]) {             /* warp-uniform: one table entry for all lanes */
+                        const uint8_t* a1 = db + e1[m];
+#pragma unroll
+                        for (int j = 0; j < J; ++j) w1[j] = *reinterpret_cast<const uint32_t*>(a1 + j * 128);
+                    }
+                    if (m == 0 || e2[m] != e2[m - 1]) {
+                        const uint8_t* a2 = db + e2[m];
+#pragma unroll
+                        for (int j = 0; j < J; ++j) w2[j] = *reinterpret_cast<const uint32_t*>(a2 + j * 128);
+                    }
+#pragma unroll
+                    for (int j = 0; j < J; ++j) {
+                        A[m][j] = A[m][j] + w1[j] + w2[j];
+                        if (!IN16) {
+                            if (FMA_H) {
+                                H[m][j] = add_fma_pipe(odd_bytes(w1[j]), one, H[m][j]);
+                                H[m][j] = add_fma_pipe(odd_bytes(w2[j]), one, H[m][j]);
+                            } else {
+                                H[m][j] = H[m][j] + odd_bytes(w1[j]) + odd_bytes(w2[j]);
+                            }
                         }
                     }
                 }
@@ -237,12 +283,12 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
     /* ---------------------------------------------------------------------- unpack and store */
 #pragma unroll
     for (int m = 0; m < M; ++m) {
-        const int i = dt * DM_TILE + warp * M + m;
+        const int i = dt * DM_TILE + grp * M + m;
         if (i >= p.ndms) continue;
         int32_t* row = p.D + (size_t)i * (size_t)p.pitch;
 #pragma unroll
         for (int j = 0; j < J; ++j) {
-            const long long t = t0 + (long long)(j * 32 + lane) * SPW;
+            const long long t = t0 + part * T_PART + (long long)(j * 32 + lane) * SPW;
             if (t >= p.nt) continue;
             if (!IN16) {
                 const uint32_t L = A[m][j] - (H[m][j] << 8);
@@ -274,7 +320,7 @@ __global__ void k_dedisperse_naive(const T* __restrict__ x, size_t pitch, const 
     D[(size_t)i * dpitch + t] = acc;
 }
 
-template <int IN16, int CB, int FMA_H>
+template <int IN16, int CB, int FMA_H, int M>
 int launch(const aak_dedisp_args* a, cudaStream_t st) {
     constexpr int NCOPY = IN16 ? 2 : 4;
     DedispParams p;
@@ -288,13 +334,13 @@ int launch(const aak_dedisp_args* a, cudaStream_t st) {
     if (grid <= 0 || grid > 0x7fffffffll) return (int)cudaErrorInvalidConfiguration;
     CUtensorMap map;
     memcpy(&map, a->tmap, sizeof(CUtensorMap));
-    k_dedisperse<IN16, CB, FMA_H><<<(unsigned)grid, NTHREADS, smem, st>>>(map, p);
+    k_dedisperse<IN16, CB, FMA_H, M><<<(unsigned)grid, NTHREADS, smem, st>>>(map, p);
     return (int)cudaGetLastError();
 }
 
-template <int IN16, int CB, int FMA_H>
+template <int IN16, int CB, int FMA_H, int M>
 int set_attr() {
-    return (int)cudaFuncSetAttribute(k_dedisperse<IN16, CB, FMA_H>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    return (int)cudaFuncSetAttribute(k_dedisperse<IN16, CB, FMA_H, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
 }
 
 }  // namespace
@@ -304,35 +350,26 @@ extern "C" size_t aak_dedisperse_smem_bytes(int32_t chan_block, int32_t window_b
     return SMEM_HEADER + (size_t)NSTAGE * (ncopy * chan_block * (size_t)window_bytes + (size_t)chan_block * DM_TILE * 4);
 }
 
+#define AA_FOR_ALL_VARIANTS(X) \
+    X(0, 8, 0, 2) X(0, 4, 0, 2) X(0, 2, 0, 2) X(0, 8, 1, 2) X(0, 4, 1, 2) X(0, 2, 1, 2) X(1, 8, 0, 2) X(1, 4, 0, 2) X(1, 2, 0, 2) \
+    X(0, 8, 0, 4) X(0, 4, 0, 4) X(0, 2, 0, 4) X(0, 8, 1, 4) X(0, 4, 1, 4) X(0, 2, 1, 4) X(1, 8, 0, 4) X(1, 4, 0, 4) X(1, 2, 0, 4)
+
 extern "C" int aak_dedisperse_init(void) {
     int e = 0;
-    if ((e = set_attr<0, 8, 0>())) return e;
-    if ((e = set_attr<0, 4, 0>())) return e;
-    if ((e = set_attr<0, 2, 0>())) return e;
-    if ((e = set_attr<0, 8, 1>())) return e;
-    if ((e = set_attr<0, 4, 1>())) return e;
-    if ((e = set_attr<0, 2, 1>())) return e;
-    if ((e = set_attr<1, 8, 0>())) return e;
-    if ((e = set_attr<1, 4, 0>())) return e;
-    if ((e = set_attr<1, 2, 0>())) return e;
+#define X(I, C, F, MM) if ((e = set_attr<I, C, F, MM>())) return e;
+    AA_FOR_ALL_VARIANTS(X)
+#undef X
     return 0;
 }
 
+/* variant bit 0: H adds on the FMA pipe (uint8 only); dms_per_warp in {2, 4} */
 extern "C" int aak_dedisperse(const aak_dedisp_args* a, void* stream) {
     cudaStream_t st = (cudaStream_t)stream;
-    if (a->in16) {
-        switch (a->chan_block) {
-            case 8: return launch<1, 8, 0>(a, st);
-            case 4: return launch<1, 4, 0>(a, st);
-            case 2: return launch<1, 2, 0>(a, st);
-        }
-    } else {
-        switch (a->chan_block) {
-            case 8: return a->variant ? launch<0, 8, 1>(a, st) : launch<0, 8, 0>(a, st);
-            case 4: return a->variant ? launch<0, 4, 1>(a, st) : launch<0, 4, 0>(a, st);
-            case 2: return a->variant ? launch<0, 2, 1>(a, st) : launch<0, 2, 0>(a, st);
-        }
-    }
+    const int fma = a->in16 ? 0 : (a->variant & 1);
+    const int mm = a->dms_per_warp == 4 ? 4 : 2;
+#define X(I, C, F, MM) if (a->in16 == I && a->chan_block == C && fma == F && mm == MM) return launch<I, C, F, MM>(a, st);
+    AA_FOR_ALL_VARIANTS(X)
+#undef X
     return (int)cudaErrorInvalidValue;
 }
 
