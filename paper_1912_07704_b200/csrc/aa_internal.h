@@ -57,7 +57,7 @@ struct Range {
     int64_t nt_full = 0;          /* T_r of a full chunk */
     int64_t pitch = 0;            /* D row pitch, elements */
     int32_t chan_block = 8, window_bytes = 0, spill_stages = 0, ndm_tiles = 0, nstages = 0;
-    int32_t dms_per_warp = 2, variant = 1;   /* K2 tuning chosen by the strategy */
+    int32_t dms_per_warp = 2, variant = 1, ring_stages = 3;   /* K2 tuning chosen by the strategy */
     std::vector<int32_t> delays;  /* [ndms][nchans], binned samples (host) */
     int32_t* d_etab = nullptr;
     int32_t* d_x0tab = nullptr;

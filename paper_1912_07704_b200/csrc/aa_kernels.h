@@ -50,11 +50,12 @@ typedef struct {
     int32_t window_bytes;      /* WB: bytes per (copy, channel) window in shared memory, multiple of 256 */
     int32_t spill_stages;      /* carry the 16-bit lanes every this many stages: (256/bin)/chan_block */
     int32_t in16;              /* 0: uint8 input (bin 1), 1: uint16 input (binned) */
-    int32_t variant;           /* uint8 only: 1 = odd-byte lane adds issued as IMAD (FMA pipe), 0 = fused IADD3 */
+    int32_t variant;           /* uint8 only: odd-byte lane adds as 0 = IADD3, 1 = IMAD (FMA pipe), 2 = alternating */
+    int32_t ring_stages;       /* depth of the shared-memory stage ring (2..8) */
     int32_t dms_per_warp;      /* 2 or 4 adjacent DM trials per warp (words of equal-delay trials are reused from registers) */
 } aak_dedisp_args;
 int aak_dedisperse(const aak_dedisp_args* a, void* stream);
-size_t aak_dedisperse_smem_bytes(int32_t chan_block, int32_t window_bytes, int32_t in16);
+size_t aak_dedisperse_smem_bytes(int32_t chan_block, int32_t window_bytes, int32_t in16, int32_t ring_stages);
 int aak_dedisperse_init(void);   /* sets the dynamic shared-memory attribute of every instantiation */
 
 /* Reference kernel (one thread per output, global loads): debugging / cross-check only. delays [ndms][nchans] int32. */

@@ -65,7 +65,7 @@ aa_status enqueue_dedispersion(Strategy& s, int64_t j, int b) {
         a.etab = rg.d_etab; a.x0tab = rg.d_x0tab; a.D = rg.d_D; a.pitch = rg.pitch;
         a.nt = (int64_t)(c.n_out / (uint64_t)rg.r.bin);
         a.ndms = rg.r.ndms; a.nchans = C; a.chan_block = rg.chan_block; a.window_bytes = rg.window_bytes;
-        a.spill_stages = rg.spill_stages; a.in16 = rg.in16; a.variant = rg.variant; a.dms_per_warp = rg.dms_per_warp;
+        a.spill_stages = rg.spill_stages; a.in16 = rg.in16; a.variant = rg.variant; a.dms_per_warp = rg.dms_per_warp; a.ring_stages = rg.ring_stages;
         AA_LAUNCH(aak_dedisperse(&a, s.compute), "dedispersion");
     }
     AA_CUDA(cudaEventRecord(s.ev_t[2], s.compute), "cudaEventRecord");

@@ -138,14 +138,23 @@ static bool plan_range(Strategy& s, Range& rg, std::vector<int32_t>& etab, std::
     rg.window_bytes = (int32_t)round_up((size_t)(wsamp * rg.esz), 256);
     if (rg.window_bytes > 65536) { set_error("aa_strategy_setup: range %d needs a %d-byte channel window per DM tile (> 65536): DM step too coarse for this band", rg.index, rg.window_bytes); return false; }
     rg.chan_block = 0;
+    rg.ring_stages = 3;
     for (int cb = 8; cb >= 2; cb /= 2)
-        if (aak_dedisperse_smem_bytes(cb, rg.window_bytes, rg.in16) <= 227 * 1024) { rg.chan_block = cb; break; }
+        if (aak_dedisperse_smem_bytes(cb, rg.window_bytes, rg.in16, rg.ring_stages) <= 227 * 1024) { rg.chan_block = cb; break; }
     if (!rg.chan_block) { set_error("aa_strategy_setup: range %d: channel window of %d bytes does not fit shared memory", rg.index, rg.window_bytes); return false; }
+    if (aak_dedisperse_smem_bytes(rg.chan_block, rg.window_bytes, rg.in16, 4) <= 227 * 1024) rg.ring_stages = 4;
+    /* measured on B200 (profiles/): binned ranges are shared-memory bound and gain 13 % from 4 trials per warp with
+     * register reuse; the uint8 ranges are issue bound and lose 7 % to the extra branches, so they keep 2 trials per warp
+     * with the odd-byte adds on the FMA pipe */
     rg.dms_per_warp = rg.in16 ? 4 : 2;
     rg.variant = 1;
 #ifdef AA_TUNING
     if (const char* ev = getenv(rg.in16 ? "AA_K2_M16" : "AA_K2_M8")) rg.dms_per_warp = atoi(ev) == 4 ? 4 : 2;
     if (const char* ev = getenv("AA_K2_VARIANT")) rg.variant = atoi(ev);
+    if (const char* ev = getenv("AA_K2_RING")) {
+        const int n = atoi(ev);
+        if (n >= 2 && n <= 8 && aak_dedisperse_smem_bytes(rg.chan_block, rg.window_bytes, rg.in16, n) <= 227 * 1024) rg.ring_stages = n;
+    }
 #endif
     rg.nstages = (C + rg.chan_block - 1) / rg.chan_block;
     rg.spill_stages = (256 / rg.r.bin) / rg.chan_block;
@@ -436,7 +445,7 @@ extern "C" size_t aa_strategy_describe(const aa_strategy* h, char* buf, size_t b
                  "dm_tiles=%d spill/%d smem=%zuB\n",
                  rg.index, rg.r.dm_low, rg.r.dm_step, rg.r.ndms, rg.r.bin, (long long)rg.max_delay, (long long)rg.nt_full, (long long)rg.pitch,
                  kDmTile, kTTile, rg.chan_block, rg.window_bytes, rg.nstages, rg.ndm_tiles, rg.spill_stages,
-                 aak_dedisperse_smem_bytes(rg.chan_block, rg.window_bytes, rg.in16));
+                 aak_dedisperse_smem_bytes(rg.chan_block, rg.window_bytes, rg.in16, rg.ring_stages));
         o += line;
     }
     for (size_t j = 0; j < s.chunks.size() && j < 4; ++j) {

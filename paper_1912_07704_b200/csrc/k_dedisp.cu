@@ -42,7 +42,7 @@ namespace {
 constexpr int NW = 16;               /* compute warps */
 constexpr int DM_TILE = 32;          /* DM trials per CTA */
 constexpr int T_TILE = 1024;         /* output samples per CTA */
-constexpr int NSTAGE = 3;
+constexpr int MAX_RING = 8;          /* shared-memory ring depth is a launch parameter (2..MAX_RING) */
 constexpr int NTHREADS = (NW + 1) * 32;
 constexpr int SMEM_HEADER = 1024;    /* mbarriers live here; keeps the stages 1024-byte aligned */
 
@@ -57,6 +57,7 @@ struct DedispParams {
     int nstages;
     int window_bytes;
     int spill_stages;
+    int nring;                 /* ring depth */
     unsigned one;              /* always 1; a runtime value so that x*one+y stays an IMAD (FMA pipe) */
 };
 
@@ -70,11 +71,11 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "{\n"
         ".reg .pred p;\n"
         "AA_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
         "@p bra AA_DONE;\n"
         "bra AA_WAIT;\n"
         "AA_DONE:\n"
-        "}\n" ::"r"(bar), "r"(parity)
+        "}\n" ::"r"(bar), "r"(parity), "r"(0x989680u)   /* suspend-time hint: sleep in hardware until the phase completes */
         : "memory");
 }
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
@@ -132,8 +133,9 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
     const int WB = p.window_bytes;
     const int data_bytes = NCOPY * CB * WB;
     const int stage_bytes = data_bytes + ENT_BYTES;
+    const int NSTAGE = p.nring;
     const uint32_t bar_full = smem_u32(smem);            /* NSTAGE x 8 bytes */
-    const uint32_t bar_empty = bar_full + 8 * NSTAGE;
+    const uint32_t bar_empty = bar_full + 8 * MAX_RING;
     uint8_t* const stages = smem + SMEM_HEADER;
 
     if (threadIdx.x == 0) {
@@ -210,7 +212,7 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
                         const uint32_t w2 = *reinterpret_cast<const uint32_t*>(a2 + j * 128);
                         A[m][j] = A[m][j] + w1 + w2;
                         if (!IN16) {
-                            if (FMA_H) {
+                            if (FMA_H == 1 || (FMA_H == 2 && (j & 1))) {
                                 H[m][j] = add_fma_pipe(odd_bytes(w1), one, H[m][j]);
                                 H[m][j] = add_fma_pipe(odd_bytes(w2), one, H[m][j]);
                             } else {
@@ -245,7 +247,7 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
                     for (int j = 0; j < J; ++j) {
                         A[m][j] = A[m][j] + w1[j] + w2[j];
                         if (!IN16) {
-                            if (FMA_H) {
+                            if (FMA_H == 1 || (FMA_H == 2 && (j & 1))) {
                                 H[m][j] = add_fma_pipe(odd_bytes(w1[j]), one, H[m][j]);
                                 H[m][j] = add_fma_pipe(odd_bytes(w2[j]), one, H[m][j]);
                             } else {
@@ -327,7 +329,9 @@ int launch(const aak_dedisp_args* a, cudaStream_t st) {
     p.etab = a->etab; p.x0tab = a->x0tab; p.D = a->D; p.pitch = a->pitch; p.nt = a->nt; p.ndms = a->ndms;
     p.nstages = (a->nchans + CB - 1) / CB;
     p.window_bytes = a->window_bytes; p.spill_stages = a->spill_stages; p.one = 1u;
-    const size_t smem = SMEM_HEADER + (size_t)NSTAGE * ((size_t)NCOPY * CB * a->window_bytes + CB * DM_TILE * 4);
+    p.nring = a->ring_stages;
+    if (p.nring < 2 || p.nring > MAX_RING) return (int)cudaErrorInvalidValue;
+    const size_t smem = SMEM_HEADER + (size_t)p.nring * ((size_t)NCOPY * CB * a->window_bytes + CB * DM_TILE * 4);
     const long long ndm_tiles = (a->ndms + DM_TILE - 1) / DM_TILE;
     const long long nt_tiles = (a->nt + T_TILE - 1) / T_TILE;
     const long long grid = ndm_tiles * nt_tiles;
@@ -345,14 +349,15 @@ int set_attr() {
 
 }  // namespace
 
-extern "C" size_t aak_dedisperse_smem_bytes(int32_t chan_block, int32_t window_bytes, int32_t in16) {
+extern "C" size_t aak_dedisperse_smem_bytes(int32_t chan_block, int32_t window_bytes, int32_t in16, int32_t ring_stages) {
     const size_t ncopy = in16 ? 2 : 4;
-    return SMEM_HEADER + (size_t)NSTAGE * (ncopy * chan_block * (size_t)window_bytes + (size_t)chan_block * DM_TILE * 4);
+    return SMEM_HEADER + (size_t)ring_stages * (ncopy * chan_block * (size_t)window_bytes + (size_t)chan_block * DM_TILE * 4);
 }
 
 #define AA_FOR_ALL_VARIANTS(X) \
     X(0, 8, 0, 2) X(0, 4, 0, 2) X(0, 2, 0, 2) X(0, 8, 1, 2) X(0, 4, 1, 2) X(0, 2, 1, 2) X(1, 8, 0, 2) X(1, 4, 0, 2) X(1, 2, 0, 2) \
-    X(0, 8, 0, 4) X(0, 4, 0, 4) X(0, 2, 0, 4) X(0, 8, 1, 4) X(0, 4, 1, 4) X(0, 2, 1, 4) X(1, 8, 0, 4) X(1, 4, 0, 4) X(1, 2, 0, 4)
+    X(0, 8, 0, 4) X(0, 4, 0, 4) X(0, 2, 0, 4) X(0, 8, 1, 4) X(0, 4, 1, 4) X(0, 2, 1, 4) X(1, 8, 0, 4) X(1, 4, 0, 4) X(1, 2, 0, 4) \
+    X(0, 8, 2, 2) X(0, 4, 2, 2) X(0, 2, 2, 2)
 
 extern "C" int aak_dedisperse_init(void) {
     int e = 0;
@@ -362,10 +367,10 @@ extern "C" int aak_dedisperse_init(void) {
     return 0;
 }
 
-/* variant bit 0: H adds on the FMA pipe (uint8 only); dms_per_warp in {2, 4} */
+/* variant (uint8 only): 0 = odd-byte adds as IADD3, 1 = as IMAD (FMA pipe), 2 = alternating; dms_per_warp in {2, 4} */
 extern "C" int aak_dedisperse(const aak_dedisp_args* a, void* stream) {
     cudaStream_t st = (cudaStream_t)stream;
-    const int fma = a->in16 ? 0 : (a->variant & 1);
+    const int fma = a->in16 ? 0 : (a->dms_per_warp == 4 ? (a->variant & 1) : a->variant);
     const int mm = a->dms_per_warp == 4 ? 4 : 2;
 #define X(I, C, F, MM) if (a->in16 == I && a->chan_block == C && fma == F && mm == MM) return launch<I, C, F, MM>(a, st);
     AA_FOR_ALL_VARIANTS(X)
