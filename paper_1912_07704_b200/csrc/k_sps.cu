@@ -94,28 +94,183 @@ __device__ __forceinline__ int clamp_i32(double x) {
     return (int)x;                          /* x is integral here */
 }
 
-__global__ void __launch_bounds__(STAT_THREADS)
+/* Single-pass form. The clip iterations only ever move samples in the TAILS of the row's distribution in or out, so the
+ * row is read once: samples inside a provisional CORE interval [clo, chi] (about +-2.75 sigma, estimated from the head
+ * of the row) are reduced to their exact moments straight away, every other sample is kept in a list in shared memory
+ * (0.6 % of a Gaussian row). Each iteration of reading C6 then needs core + (list entries inside its bounds), the same
+ * exact integers the full passes give (integer sums do not depend on the order or grouping). If a bound ever cuts into
+ * the core, or the list overflows, the row falls back to the plain multi-pass loop below - same result, more reads. */
+constexpr int STAT_LIST_CAP = 12288;                 /* int32 entries of shared memory per row (48 KB: 4 CTAs per SM) */
+constexpr double STAT_CORE_Z = 2.75;                 /* core half-width in head sigmas: 0.6 % of a Gaussian row goes to the list */
+constexpr int STAT_HEAD = 8192;                      /* samples used for the provisional core */
+
+struct StatSmem {
+    u64 red[(STAT_THREADS / 32) * 4];
+    int cnt;
+    int overflow;
+    int list[STAT_LIST_CAP];
+};
+
+__device__ Moments list_moments(const int* list, int n_list, int p, int lo, int hi, u64* red) {
+    unsigned n = 0; i64 s1 = 0; u64 s2 = 0;
+    for (int q = threadIdx.x; q < n_list; q += STAT_THREADS) acc_sample(list[q], p, lo, hi, true, n, s1, s2);
+    u64 a = n, b = (u64)s1, c = s2 & 0xFFFFFFFFull, d = s2 >> 32;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_down_sync(0xffffffffu, a, o);
+        b += __shfl_down_sync(0xffffffffu, b, o);
+        c += __shfl_down_sync(0xffffffffu, c, o);
+        d += __shfl_down_sync(0xffffffffu, d, o);
+    }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();
+    if (lane == 0) { red[warp * 4 + 0] = a; red[warp * 4 + 1] = b; red[warp * 4 + 2] = c; red[warp * 4 + 3] = d; }
+    __syncthreads();
+    Moments m; m.n = 0; m.s1 = 0; m.s2lo = 0; m.s2hi = 0;
+    for (int w = 0; w < STAT_THREADS / 32; ++w) {
+        m.n += red[w * 4 + 0]; m.s1 += (i64)red[w * 4 + 1]; m.s2lo += red[w * 4 + 2]; m.s2hi += red[w * 4 + 3];
+    }
+    return m;
+}
+
+__device__ __forceinline__ Moments add_moments(const Moments& a, const Moments& b) {
+    Moments m; m.n = a.n + b.n; m.s1 = a.s1 + b.s1; m.s2lo = a.s2lo + b.s2lo; m.s2hi = a.s2hi + b.s2hi; return m;
+}
+__device__ __forceinline__ bool same_moments(const Moments& a, const Moments& b) {
+    /* s2 is carried as two partial sums whose split depends on the grouping: compare the value s2hi*2^32 + s2lo */
+    const u128 x = ((u128)a.s2hi << 32) + (u128)a.s2lo, y = ((u128)b.s2hi << 32) + (u128)b.s2lo;
+    return a.n == b.n && a.s1 == b.s1 && x == y;
+}
+
+/* one core-vs-list decision per sample; list appends are warp-aggregated */
+__device__ __forceinline__ void split_sample(bool valid, int v, int p, int clo, int chi, unsigned& n, i64& s1, u64& s2,
+                                             StatSmem& sm, int lane) {
+    const bool in_core = valid && v >= clo && v <= chi;
+    if (in_core) { const i64 d = (i64)v - (i64)p; ++n; s1 += d; s2 += (u64)(d * d); }
+    const bool out = valid && !in_core;
+    const unsigned mask = __ballot_sync(0xffffffffu, out);
+    if (mask) {
+        const int leader = __ffs(mask) - 1;
+        int base = 0;
+        if (lane == leader) base = atomicAdd(&sm.cnt, __popc(mask));
+        base = __shfl_sync(0xffffffffu, base, leader);
+        if (out) {
+            const int slot = base + __popc(mask & ((1u << lane) - 1u));
+            if (slot < STAT_LIST_CAP) sm.list[slot] = v; else sm.overflow = 1;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(STAT_THREADS, 2)
 k_row_stats(const aak_row_desc* __restrict__ rows, double* __restrict__ mu_sigma, i64* __restrict__ n_iters) {
-    __shared__ u64 red[(STAT_THREADS / 32) * 4];
+    extern __shared__ __align__(16) uint8_t stat_raw[];
+    StatSmem& sm = *reinterpret_cast<StatSmem*>(stat_raw);
+    u64* red = sm.red;
     const aak_row_desc rd = rows[blockIdx.x];
     const int32_t* D = rd.D;
     const i64 T = rd.nt;
     const int p = D[0];
-    Moments m = block_moments(D, T, p, 0, 0, false, red);
+    const int lane = threadIdx.x & 31;
     double mu, sigma;
-    mu_sigma_of(p, m, mu, sigma);
+    Moments m;
+    bool fast = false;
+    Moments core; core.n = 0; core.s1 = 0; core.s2lo = 0; core.s2hi = 0;
+    int clo = 0, chi = -1, n_list = 0;
+
+    /* ---- provisional core from the head of the row (any interval would be CORRECT; this one makes the list short) */
+    {
+        const i64 Th = T < STAT_HEAD ? T : STAT_HEAD;
+        const Moments h = block_moments(D, Th, p, 0, 0, false, red);
+        double hm, hs;
+        mu_sigma_of(p, h, hm, hs);
+        if (hs > 0.0 && hs < 1.0e8) {
+            clo = clamp_i32(ceil(hm - STAT_CORE_Z * hs));
+            chi = clamp_i32(floor(hm + STAT_CORE_Z * hs));
+        }
+        if (threadIdx.x == 0) { sm.cnt = 0; sm.overflow = 0; }
+        __syncthreads();
+    }
+    if (chi >= clo) {
+        /* ---- the single pass over the row */
+        unsigned n = 0; i64 s1 = 0; u64 s2 = 0;
+        const i64 nvec = T >> 2;
+        const int4* Dv = reinterpret_cast<const int4*>(D);
+        const i64 nvec_pad = (nvec + STAT_THREADS - 1) / STAT_THREADS * STAT_THREADS;     /* uniform trip count for the ballots */
+        constexpr int U = 4;                                                            /* 64 bytes in flight per thread */
+        for (i64 q0 = 0; q0 < nvec_pad; q0 += U * STAT_THREADS) {
+            int4 v[U]; bool ok[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const i64 q = q0 + u * STAT_THREADS + threadIdx.x;
+                ok[u] = q < nvec;
+                v[u] = ok[u] ? __ldg(Dv + q) : make_int4(0, 0, 0, 0);
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                split_sample(ok[u], v[u].x, p, clo, chi, n, s1, s2, sm, lane);
+                split_sample(ok[u], v[u].y, p, clo, chi, n, s1, s2, sm, lane);
+                split_sample(ok[u], v[u].z, p, clo, chi, n, s1, s2, sm, lane);
+                split_sample(ok[u], v[u].w, p, clo, chi, n, s1, s2, sm, lane);
+            }
+        }
+        {
+            const i64 t = (nvec << 2) + threadIdx.x;                                    /* at most 3 tail samples */
+            const bool ok = t < T;
+            split_sample(ok, ok ? D[t] : 0, p, clo, chi, n, s1, s2, sm, lane);
+        }
+        u64 a = n, b = (u64)s1, c = s2 & 0xFFFFFFFFull, d = s2 >> 32;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            a += __shfl_down_sync(0xffffffffu, a, o);
+            b += __shfl_down_sync(0xffffffffu, b, o);
+            c += __shfl_down_sync(0xffffffffu, c, o);
+            d += __shfl_down_sync(0xffffffffu, d, o);
+        }
+        const int warp = threadIdx.x >> 5;
+        __syncthreads();
+        if (lane == 0) { red[warp * 4 + 0] = a; red[warp * 4 + 1] = b; red[warp * 4 + 2] = c; red[warp * 4 + 3] = d; }
+        __syncthreads();
+        for (int w = 0; w < STAT_THREADS / 32; ++w) {
+            core.n += red[w * 4 + 0]; core.s1 += (i64)red[w * 4 + 1]; core.s2lo += red[w * 4 + 2]; core.s2hi += red[w * 4 + 3];
+        }
+        n_list = sm.cnt;
+        fast = (sm.overflow == 0) && n_list <= STAT_LIST_CAP;
+    }
+
     int it = 0;
     bool degenerate = false;
-    for (it = 0; it < 8; ++it) {
-        const double t3 = __dmul_rn(3.0, sigma);
-        const int lo = clamp_i32(ceil(__dsub_rn(mu, t3)));
-        const int hi = clamp_i32(floor(__dadd_rn(mu, t3)));
-        const Moments m2 = block_moments(D, T, p, lo, hi, true, red);
-        if (m2.n == 0) { degenerate = true; ++it; break; }
-        const bool same = (m2.n == m.n && m2.s1 == m.s1 && m2.s2lo == m.s2lo && m2.s2hi == m.s2hi);
-        m = m2;
+    if (fast) {
+        m = add_moments(core, list_moments(sm.list, n_list, p, INT32_MIN, INT32_MAX, red));      /* unclipped row */
         mu_sigma_of(p, m, mu, sigma);
-        if (same) { ++it; break; }
+        for (it = 0; it < 8; ++it) {
+            const double t3 = __dmul_rn(3.0, sigma);
+            const int lo = clamp_i32(ceil(__dsub_rn(mu, t3)));
+            const int hi = clamp_i32(floor(__dadd_rn(mu, t3)));
+            if (lo > clo || hi < chi) { fast = false; break; }       /* a bound cuts into the core: take the plain route */
+            const Moments m2 = add_moments(core, list_moments(sm.list, n_list, p, lo, hi, red));
+            if (m2.n == 0) { degenerate = true; ++it; break; }
+            const bool same = same_moments(m2, m);
+            m = m2;
+            mu_sigma_of(p, m, mu, sigma);
+            if (same) { ++it; break; }
+        }
+    }
+    if (!fast) {
+        /* ---- plain route: one pass over the row per iteration (reading C6 written out) */
+        degenerate = false;
+        m = block_moments(D, T, p, 0, 0, false, red);
+        mu_sigma_of(p, m, mu, sigma);
+        for (it = 0; it < 8; ++it) {
+            const double t3 = __dmul_rn(3.0, sigma);
+            const int lo = clamp_i32(ceil(__dsub_rn(mu, t3)));
+            const int hi = clamp_i32(floor(__dadd_rn(mu, t3)));
+            const Moments m2 = block_moments(D, T, p, lo, hi, true, red);
+            if (m2.n == 0) { degenerate = true; ++it; break; }
+            const bool same = same_moments(m2, m);
+            m = m2;
+            mu_sigma_of(p, m, mu, sigma);
+            if (same) { ++it; break; }
+        }
     }
     if (threadIdx.x == 0) {
         mu_sigma[2 * (size_t)blockIdx.x] = mu;
@@ -399,12 +554,13 @@ k_sps_peaks(const SpsParams p) {
 
 extern "C" int aak_row_stats(const aak_row_desc* rows, int32_t nrows, double* mu_sigma, int64_t* n_iters, void* stream) {
     if (nrows <= 0) return 0;
-    k_row_stats<<<(unsigned)nrows, STAT_THREADS, 0, (cudaStream_t)stream>>>(rows, mu_sigma, (i64*)n_iters);
+    k_row_stats<<<(unsigned)nrows, STAT_THREADS, sizeof(StatSmem), (cudaStream_t)stream>>>(rows, mu_sigma, (i64*)n_iters);
     return (int)cudaGetLastError();
 }
 
 extern "C" int aak_sps_init(void) {
     int e;
+    if ((e = (int)cudaFuncSetAttribute(k_row_stats, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(StatSmem)))) return e;
     if ((e = (int)cudaFuncSetAttribute(k_sps_peaks<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(K4Smem<3>)))) return e;
     if ((e = (int)cudaFuncSetAttribute(k_sps_peaks<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(K4Smem<4>)))) return e;
     if ((e = (int)cudaFuncSetAttribute(k_sps_peaks<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(K4Smem<8>)))) return e;
