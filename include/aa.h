@@ -86,6 +86,7 @@ typedef struct {
     size_t arena_bytes_total;
     size_t max_candidates;
     int32_t owns_arena;        /* 1 if the library made the (single) cudaMalloc */
+    int32_t input_layout;      /* aa_input_layout of the bound plan */
 } aa_strategy_info;
 
 /* ------------------------------------------------------------------------------------------------ plan
@@ -102,6 +103,14 @@ aa_status aa_plan_create(aa_plan** out, int32_t nchans, const double* chan_freq_
                          const aa_dm_range* ranges, int32_t nranges,
                          const int32_t* boxcar_widths, int32_t nwidths, float snr_threshold);
 void aa_plan_destroy(aa_plan* plan);
+
+/* Layout of the input data (metadata of the telescope data, PAPER.md:47 step 1). Default AA_LAYOUT_CHANNEL_MAJOR:
+ * x[c][t], one row per channel. AA_LAYOUT_TIME_MAJOR: x[t][c], one row per time sample, the order telescopes
+ * deliver; each chunk is then one contiguous host block, copied as it is and corner-turned on the device (kernel
+ * K0t) before binning and dedispersion. Must be called before aa_strategy_setup binds the plan (the strategy reserves
+ * the staging buffers). Results are identical in both layouts. Errors: AA_ERR_INVALID_ARG naming `layout`. */
+typedef enum { AA_LAYOUT_CHANNEL_MAJOR = 0, AA_LAYOUT_TIME_MAJOR = 1 } aa_input_layout;
+aa_status aa_plan_set_input_layout(aa_plan* plan, int32_t layout);
 
 /* ------------------------------------------------------------------------------------------------ strategy
  * PAPER.md:47 steps 4-6 ("bind", "the API calculates the optimal strategy", "checks whether all modules are
@@ -157,14 +166,17 @@ aa_status aa_strategy_shard(aa_strategy* s, int32_t rank, int32_t world);
  * into the other input buffer on the copy stream, time binning for ranges with bin > 1, then
  *   D_r[i][t'] = sum_c x_b[c][t' + delay(c,r,i)]   (int32, bit-exact)            [north_star]
  * for every range. Asynchronous: returns after enqueueing.
- *   host_input (HOST, const, user-owned, never written): x[c][t] uint8, channel-major, the WHOLE observation
- *              (nsamp_total samples per channel), row_stride_bytes between channels. Must stay valid until the
+ *   host_input (HOST, const, user-owned, never written): the WHOLE observation, uint8. Channel-major plans:
+ *              x[c][t], nsamp_total samples per channel, row_stride_bytes between channels. Time-major plans
+ *              (aa_plan_set_input_layout): x[t][c], nchans samples per row, row_stride_bytes (>= nchans) between
+ *              consecutive time samples. Must stay valid until the
  *              following aa_run_* call returns (prefetch). Pinned memory is needed for the copy to overlap compute.
  * Returns AA_OK; AA_ERR_NOT_READY; AA_ERR_ORDER if the previous chunk's SPS has not run; AA_ERR_CUDA. */
 aa_status aa_run_dedispersion(aa_strategy* s, const uint8_t* host_input, size_t row_stride_bytes);
 
 /* Same, with the chunk already resident on the DEVICE: device_chunk points at sample `start` of chunk `cursor`
- * (x[c][0..L_j)), row stride in bytes, at least 16-byte aligned rows; the data are copied device-to-device into the
+ * (x[c][0..L_j), or x[0..L_j)[c] for a time-major plan: then 4-byte aligned with a stride that is a multiple of 4 and
+ * >= nchans rounded up to 4), row stride in bytes, at least 16-byte aligned rows; the data are copied device-to-device into the
  * arena's input buffer (so the kernel's over-read slack exists). Used when the producer is another GPU stage. */
 aa_status aa_run_dedispersion_device(aa_strategy* s, const uint8_t* device_chunk, size_t row_stride_bytes);
 

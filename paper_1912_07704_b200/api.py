@@ -17,7 +17,7 @@ __all__ = [
     "AaError", "AA_OK", "AA_STATUS_CHUNK_DONE", "AA_STATUS_FINISHED", "AA_ERR_INVALID_ARG", "AA_ERR_NOT_READY",
     "AA_ERR_BUDGET_TOO_SMALL", "AA_ERR_CUDA", "AA_ERR_CANDIDATE_OVERFLOW", "AA_ERR_ORDER", "AA_ERR_INTERNAL",
     "CANDIDATE_DTYPE", "lib_path", "load",
-    "aa_plan_create", "aa_plan_destroy", "aa_strategy_plan", "aa_strategy_setup", "aa_strategy_destroy", "aa_strategy_get_info",
+    "AA_LAYOUT_CHANNEL_MAJOR", "AA_LAYOUT_TIME_MAJOR", "aa_plan_create", "aa_plan_destroy", "aa_plan_set_input_layout", "aa_strategy_plan", "aa_strategy_setup", "aa_strategy_destroy", "aa_strategy_get_info",
     "aa_strategy_get_range_info", "aa_strategy_get_chunk", "aa_strategy_get_delay", "aa_strategy_describe",
     "aa_strategy_reset", "aa_strategy_shard", "aa_run_dedispersion", "aa_run_dedispersion_device", "aa_run_sps", "aa_get_candidates",
     "aa_get_dedispersed_row", "aa_get_row_stats", "aa_get_row_moments", "aa_get_dedispersed_device", "aa_synchronize",
@@ -28,6 +28,7 @@ __all__ = [
 AA_OK, AA_STATUS_CHUNK_DONE, AA_STATUS_FINISHED = 0, 1, 2
 AA_ERR_INVALID_ARG, AA_ERR_NOT_READY, AA_ERR_BUDGET_TOO_SMALL, AA_ERR_CUDA = -1, -2, -3, -4
 AA_ERR_CANDIDATE_OVERFLOW, AA_ERR_ORDER, AA_ERR_INTERNAL = -5, -6, -7
+AA_LAYOUT_CHANNEL_MAJOR, AA_LAYOUT_TIME_MAJOR = 0, 1
 
 CANDIDATE_DTYPE = np.dtype([("sample", np.uint64), ("dm", np.float32), ("snr", np.float32), ("width", np.uint32),
                             ("range", np.uint32), ("dm_index", np.uint32)], align=True)
@@ -54,7 +55,7 @@ class _StrategyInfo(ctypes.Structure):
                 ("nsamp_total", c_int64), ("overlap", c_int64), ("chunk_len", c_int64), ("n_out", c_int64),
                 ("nchunks", c_int64), ("next_chunk", c_int64), ("shard_rank", c_int32), ("shard_world", c_int32),
                 ("arena_bytes_used", c_size_t),
-                ("arena_bytes_total", c_size_t), ("max_candidates", c_size_t), ("owns_arena", c_int32)]
+                ("arena_bytes_total", c_size_t), ("max_candidates", c_size_t), ("owns_arena", c_int32), ("input_layout", c_int32)]
 
 
 def _struct_dict(s):
@@ -82,6 +83,7 @@ def load():
     sig = {
         "aa_plan_create": (c_int32, [POINTER(vp), c_int32, vp, c_double, vp, c_int32, vp, c_int32, c_float]),
         "aa_plan_destroy": (None, [vp]),
+        "aa_plan_set_input_layout": (c_int32, [vp, c_int32]),
         "aa_strategy_setup": (c_int32, [POINTER(vp), vp, c_uint64, vp, c_size_t, c_size_t, vp, vp, c_size_t, c_uint64]),
         "aa_strategy_plan": (c_int32, [POINTER(vp), vp, c_uint64, c_size_t, c_size_t, c_uint64]),
         "aa_strategy_destroy": (None, [vp]),
@@ -153,6 +155,10 @@ def aa_plan_create(chan_freq_mhz, tsamp_s, ranges, boxcar_widths, snr_threshold)
     _check(load().aa_plan_create(byref(out), len(f), f.ctypes.data, float(tsamp_s), ctypes.addressof(rs), len(ranges),
                                  w.ctypes.data, len(w), float(snr_threshold)))
     return out.value
+
+
+def aa_plan_set_input_layout(plan, layout: int) -> int:
+    return _check(load().aa_plan_set_input_layout(plan, int(layout)))
 
 
 def aa_plan_destroy(plan) -> None:
@@ -299,9 +305,11 @@ def aa_get_launch_count(strategy) -> int:
 class Plan:
     """Owns an aa_plan handle."""
 
-    def __init__(self, chan_freq_mhz, tsamp_s, ranges, boxcar_widths, snr_threshold):
+    def __init__(self, chan_freq_mhz, tsamp_s, ranges, boxcar_widths, snr_threshold, time_major: bool = False):
         self.handle = aa_plan_create(chan_freq_mhz, tsamp_s, ranges, boxcar_widths, snr_threshold)
         self.ranges = [tuple(r) for r in ranges]
+        if time_major:
+            aa_plan_set_input_layout(self.handle, AA_LAYOUT_TIME_MAJOR)
 
     def close(self):
         if getattr(self, "handle", None):

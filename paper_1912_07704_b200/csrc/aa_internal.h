@@ -34,6 +34,7 @@ struct Plan {
     std::vector<aa_dm_range> ranges;
     std::vector<int32_t> widths;
     float threshold = 0.f;
+    int32_t layout = 0;           /* aa_input_layout */
 };
 
 /* Single-allocation bump allocator over caller- or library-owned device memory. */
@@ -84,6 +85,8 @@ struct Strategy {
     bool owns_arena = false;
     size_t in_pitch = 0;                     /* bytes per channel row of the uint8 buffers */
     uint8_t* d_raw[2] = {nullptr, nullptr};  /* H2D targets (copy 0 of the uint8 input) */
+    uint8_t* d_stage[2] = {nullptr, nullptr};   /* time-major plans: H2D targets [L][stage_stride]; d_raw[0] is the corner-turn target */
+    size_t stage_stride = 0;
     uint8_t* d_x4 = nullptr;                 /* the 4 sample-shifted copies of the uint8 chunk, copy k at k*x4_stride */
     size_t x4_stride = 0;
     bool need_u8_copies = false;

@@ -62,6 +62,9 @@ int aak_dedisperse_init(void);   /* sets the dynamic shared-memory attribute of 
 int aak_dedisperse_naive(const void* x, size_t pitch_elems, int32_t in16, const int32_t* delays, int32_t nchans,
                          int32_t ndms, int64_t nt, int32_t* D, int64_t pitch, void* stream);
 
+/* ---- K0t: corner turn of a time-major chunk x_tm[t][c] into channel-major rows x[c][t] (uint8) */
+int aak_corner_turn(const uint8_t* in, size_t in_stride, uint8_t* out, size_t out_pitch, int32_t nchans, int64_t nsamp, void* stream);
+
 /* ---- K3: robust row statistics ---------------------------------------------------------------------------------
  * rows: one entry per DM row of all ranges of the chunk. stats out: per row {mu, sigma} doubles and {n, iters} */
 typedef struct {

@@ -37,19 +37,30 @@ aa_status enqueue_h2d(Strategy& s, int64_t j, int b, const uint8_t* host_input, 
     const Chunk& c = s.chunks[(size_t)j];
     if (s.raw_free_recorded[b]) AA_CUDA(cudaStreamWaitEvent(s.copy, s.ev_raw_free[b], 0), "cudaStreamWaitEvent");
     if (timed) AA_CUDA(cudaEventRecord(s.ev_h2d[0], s.copy), "cudaEventRecord");
-    AA_CUDA(cudaMemcpy2DAsync(s.d_raw[b], s.in_pitch, host_input + c.start, row_stride, (size_t)c.len, (size_t)s.plan.nchans,
-                              cudaMemcpyHostToDevice, s.copy), "cudaMemcpy2DAsync (H2D chunk)");
+    if (s.plan.layout == AA_LAYOUT_TIME_MAJOR)      /* one contiguous block of c.len time rows */
+        AA_CUDA(cudaMemcpy2DAsync(s.d_stage[b], s.stage_stride, host_input + (size_t)c.start * row_stride, row_stride, (size_t)s.plan.nchans,
+                                  (size_t)c.len, cudaMemcpyHostToDevice, s.copy), "cudaMemcpy2DAsync (H2D chunk, time-major)");
+    else
+        AA_CUDA(cudaMemcpy2DAsync(s.d_raw[b], s.in_pitch, host_input + c.start, row_stride, (size_t)c.len, (size_t)s.plan.nchans,
+                                  cudaMemcpyHostToDevice, s.copy), "cudaMemcpy2DAsync (H2D chunk)");
     if (timed) AA_CUDA(cudaEventRecord(s.ev_h2d[1], s.copy), "cudaEventRecord");
     AA_CUDA(cudaEventRecord(s.ev_copied[b], s.copy), "cudaEventRecord");
     s.raw_holds[b] = j;
     return AA_OK;
 }
 
-/* Shifted copies, binning and the dedispersion launches for the chunk resident in raw buffer b. */
-aa_status enqueue_dedispersion(Strategy& s, int64_t j, int b) {
+/* Corner turn (time-major plans), shifted copies, binning and the dedispersion launches for the chunk resident in input
+ * buffer b. tm_src/tm_stride: the time-major source of the corner turn (the staging buffer, or the caller's device chunk). */
+aa_status enqueue_dedispersion(Strategy& s, int64_t j, int b, const uint8_t* tm_src = nullptr, size_t tm_stride = 0) {
     const Chunk& c = s.chunks[(size_t)j];
     const int32_t C = s.plan.nchans;
+    const int slot = b;                               /* the buffer whose reuse the raw_free event guards */
     AA_CUDA(cudaEventRecord(s.ev_t[0], s.compute), "cudaEventRecord");
+    if (s.plan.layout == AA_LAYOUT_TIME_MAJOR) {
+        if (!tm_src) { tm_src = s.d_stage[b]; tm_stride = s.stage_stride; }
+        AA_LAUNCH(aak_corner_turn(tm_src, tm_stride, s.d_raw[0], s.in_pitch, C, (int64_t)c.len, s.compute), "corner turn");
+        b = 0;                                        /* the channel-major copy lives in d_raw[0] */
+    }
     if (s.need_u8_copies)
         AA_LAUNCH(aak_make_copies_u8(s.d_raw[b], s.d_x4, s.in_pitch, s.x4_stride, s.in_pitch, C, s.compute), "shifted copies (uint8)");
     for (int bin = 2; bin <= 8; bin *= 2) {
@@ -69,8 +80,8 @@ aa_status enqueue_dedispersion(Strategy& s, int64_t j, int b) {
         AA_LAUNCH(aak_dedisperse(&a, s.compute), "dedispersion");
     }
     AA_CUDA(cudaEventRecord(s.ev_t[2], s.compute), "cudaEventRecord");
-    AA_CUDA(cudaEventRecord(s.ev_raw_free[b], s.compute), "cudaEventRecord");
-    s.raw_free_recorded[b] = true;
+    AA_CUDA(cudaEventRecord(s.ev_raw_free[slot], s.compute), "cudaEventRecord");
+    s.raw_free_recorded[slot] = true;
     s.timed = true; s.stats_timed = false;
     s.current_chunk = j;
     s.pending_sps = true;
@@ -112,11 +123,14 @@ extern "C" aa_status aa_run_dedispersion(aa_strategy* h, const uint8_t* host_inp
     if (st != AA_OK) return st;
     Strategy& s = h->s;
     if (!host_input) { set_error("aa_run_dedispersion: host_input is NULL"); return AA_ERR_INVALID_ARG; }
-    if (row_stride_bytes < s.nsamp_total) { set_error("aa_run_dedispersion: row_stride_bytes = %zu is shorter than nsamp_total = %llu", row_stride_bytes, (unsigned long long)s.nsamp_total); return AA_ERR_INVALID_ARG; }
+    const bool tmajor = s.plan.layout == AA_LAYOUT_TIME_MAJOR;
+    if (!tmajor && row_stride_bytes < s.nsamp_total) { set_error("aa_run_dedispersion: row_stride_bytes = %zu is shorter than nsamp_total = %llu", row_stride_bytes, (unsigned long long)s.nsamp_total); return AA_ERR_INVALID_ARG; }
+    if (tmajor && row_stride_bytes < (size_t)s.plan.nchans) { set_error("aa_run_dedispersion: row_stride_bytes = %zu is shorter than nchans = %d (time-major plan)", row_stride_bytes, s.plan.nchans); return AA_ERR_INVALID_ARG; }
+    const bool two_buffers = s.d_raw[1] || s.d_stage[1];
     if (s.pending_sps) { set_error("aa_run_dedispersion: chunk %lld is dedispersed but aa_run_sps has not run on it yet", (long long)s.current_chunk); return AA_ERR_ORDER; }
     if (s.next_chunk >= (int64_t)s.chunks.size()) { set_error("aa_run_dedispersion: all %zu chunks are done (aa_strategy_reset rewinds)", s.chunks.size()); return AA_ERR_ORDER; }
     const int64_t j = s.next_chunk;
-    const int b = s.d_raw[1] ? (int)((j / s.shard_world) & 1) : 0;
+    const int b = two_buffers ? (int)((j / s.shard_world) & 1) : 0;
     s.h2d_timed = false;
     if (s.raw_holds[b] != j) {
         if ((st = enqueue_h2d(s, j, b, host_input, row_stride_bytes, true)) != AA_OK) return st;
@@ -126,7 +140,7 @@ extern "C" aa_status aa_run_dedispersion(aa_strategy* h, const uint8_t* host_inp
     if ((st = enqueue_dedispersion(s, j, b)) != AA_OK) return st;
     /* double buffering: start moving chunk j+1 while chunk j computes (north_star "Streaming") */
     const int64_t jn = j + s.shard_world;           /* the next chunk of this strategy's shard */
-    if (s.d_raw[1] && jn < (int64_t)s.chunks.size() && s.raw_holds[b ^ 1] != jn)
+    if (two_buffers && jn < (int64_t)s.chunks.size() && s.raw_holds[b ^ 1] != jn)
         if ((st = enqueue_h2d(s, jn, b ^ 1, host_input, row_stride_bytes, false)) != AA_OK) return st;
     return AA_OK;
 }
@@ -140,9 +154,17 @@ extern "C" aa_status aa_run_dedispersion_device(aa_strategy* h, const uint8_t* d
     if (s.next_chunk >= (int64_t)s.chunks.size()) { set_error("aa_run_dedispersion_device: all %zu chunks are done", s.chunks.size()); return AA_ERR_ORDER; }
     const int64_t j = s.next_chunk;
     const Chunk& c = s.chunks[(size_t)j];
+    s.h2d_timed = false;
+    if (s.plan.layout == AA_LAYOUT_TIME_MAJOR) {
+        if (((uintptr_t)device_chunk & 3) || (row_stride_bytes & 3) || row_stride_bytes < (size_t)((s.plan.nchans + 3) & ~3)) {
+            set_error("aa_run_dedispersion_device: a time-major device chunk must be 4-byte aligned with row_stride_bytes a multiple of 4 and >= nchans rounded up to 4 (got %zu)", row_stride_bytes);
+            return AA_ERR_INVALID_ARG;
+        }
+        s.raw_holds[0] = j;
+        return enqueue_dedispersion(s, j, 0, device_chunk, row_stride_bytes);
+    }
     if (row_stride_bytes < c.len) { set_error("aa_run_dedispersion_device: row_stride_bytes = %zu is shorter than the chunk (%llu)", row_stride_bytes, (unsigned long long)c.len); return AA_ERR_INVALID_ARG; }
     const int b = s.d_raw[1] ? (int)((j / s.shard_world) & 1) : 0;
-    s.h2d_timed = false;
     AA_CUDA(cudaMemcpy2DAsync(s.d_raw[b], s.in_pitch, device_chunk, row_stride_bytes, (size_t)c.len, (size_t)s.plan.nchans,
                               cudaMemcpyDeviceToDevice, s.compute), "cudaMemcpy2DAsync (D2D chunk)");
     s.raw_holds[b] = j;

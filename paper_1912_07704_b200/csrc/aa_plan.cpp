@@ -91,3 +91,13 @@ extern "C" aa_status aa_plan_create(aa_plan** out, int32_t nchans, const double*
 }
 
 extern "C" void aa_plan_destroy(aa_plan* plan) { delete plan; }
+
+extern "C" aa_status aa_plan_set_input_layout(aa_plan* plan, int32_t layout) {
+    if (!plan) { aa::set_error("aa_plan_set_input_layout: plan is NULL"); return AA_ERR_NOT_READY; }
+    if (layout != AA_LAYOUT_CHANNEL_MAJOR && layout != AA_LAYOUT_TIME_MAJOR) {
+        aa::set_error("aa_plan_set_input_layout: layout = %d must be AA_LAYOUT_CHANNEL_MAJOR (0) or AA_LAYOUT_TIME_MAJOR (1)", layout);
+        return AA_ERR_INVALID_ARG;
+    }
+    plan->p.layout = layout;
+    return AA_OK;
+}

@@ -65,7 +65,17 @@ static void carve(Strategy& s, int64_t L, bool two_raw) {
     s.in_pitch = round_up((size_t)L, 256);
     const size_t raw_bytes = (size_t)s.plan.nchans * s.in_pitch + kSlack;
     s.d_raw[0] = (uint8_t*)a.take(raw_bytes);
-    s.d_raw[1] = two_raw ? (uint8_t*)a.take(raw_bytes) : nullptr;
+    s.d_stage[0] = s.d_stage[1] = nullptr;
+    if (s.plan.layout == AA_LAYOUT_TIME_MAJOR) {
+        /* the chunk lands time-major in a staging buffer (two when chunks are double-buffered); one channel-major buffer */
+        s.stage_stride = round_up((size_t)s.plan.nchans, 16);
+        const size_t stage_bytes = (size_t)L * s.stage_stride + kSlack;
+        s.d_stage[0] = (uint8_t*)a.take(stage_bytes);
+        s.d_stage[1] = two_raw ? (uint8_t*)a.take(stage_bytes) : nullptr;
+        s.d_raw[1] = nullptr;
+    } else {
+        s.d_raw[1] = two_raw ? (uint8_t*)a.take(raw_bytes) : nullptr;
+    }
     s.x4_stride = round_up(raw_bytes, 256);
     s.d_x4 = s.need_u8_copies ? (uint8_t*)a.take(4 * s.x4_stride) : nullptr;
     for (int b = 2; b <= 8; b *= 2) {
@@ -396,6 +406,7 @@ extern "C" aa_status aa_strategy_get_info(const aa_strategy* h, aa_strategy_info
     out->shard_rank = s.shard_rank; out->shard_world = s.shard_world;
     out->arena_bytes_used = s.arena.used; out->arena_bytes_total = s.arena.size; out->max_candidates = s.max_candidates;
     out->owns_arena = s.owns_arena ? 1 : 0;
+    out->input_layout = s.plan.layout;
     return AA_OK;
 }
 
@@ -436,7 +447,7 @@ extern "C" size_t aa_strategy_describe(const aa_strategy* h, char* buf, size_t b
              (unsigned long long)s.nsamp_total, s.B, (long long)s.S, (long long)s.L, (long long)s.n_out, s.chunks.size());
     o += line;
     snprintf(line, sizeof line, "arena: %zu bytes used of %zu (%s), input pitch %zu, raw buffers %d, uint8 shifted copies %s\n", s.arena.used,
-             s.arena.size, s.owns_arena ? "library-owned, one cudaMalloc" : "caller-owned", s.in_pitch, s.d_raw[1] ? 2 : 1,
+             s.arena.size, s.owns_arena ? "library-owned, one cudaMalloc" : "caller-owned", s.in_pitch, (s.d_raw[1] || s.d_stage[1]) ? 2 : 1,
              s.need_u8_copies ? "4" : "none");
     o += line;
     for (const Range& rg : s.ranges) {

@@ -81,6 +81,48 @@ k_make_copies_u8(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, size
     }
 }
 
+/* ---- K0t: corner turn. Telescopes deliver TIME-major samples x_tm[t][c] (PAPER.md:47 step 1 "telescope data");
+ * the dedispersion kernels read CHANNEL-major rows x[c][t]. A CTA transposes a 128-channel x 128-sample tile:
+ * each thread loads 4 words = 4 samples x 4 channels, transposes the 4x4 bytes in registers (8 PRMT), and stores four
+ * words (one channel x 4 samples each) into an XOR-swizzled shared-memory tile, so that both the stores and the
+ * row reads that follow are bank-conflict free; a warp then writes one 128-byte channel row segment per instruction. */
+constexpr int CT_TILE = 128;
+__global__ void __launch_bounds__(256)
+k_corner_turn(const uint8_t* __restrict__ in, size_t in_stride, uint8_t* __restrict__ out, size_t out_pitch, int nchans, long long nsamp) {
+    __shared__ uint32_t T[CT_TILE][32];                          /* T[c][(t/4) ^ (c/4)] = 4 consecutive samples of channel c */
+    const int x = threadIdx.x & 31, y = threadIdx.x >> 5;
+    const long long t_tile = (long long)blockIdx.x * CT_TILE;
+    const int c_tile = blockIdx.y * CT_TILE;
+    const int c0 = c_tile + 4 * x;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const int tq = y + 8 * q;                                /* sample quad inside the tile */
+        uint32_t w[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const long long t = t_tile + 4 * tq + k;
+            w[k] = (t < nsamp && c0 < nchans) ? *reinterpret_cast<const uint32_t*>(in + (size_t)t * in_stride + c0) : 0u;
+        }
+        /* 4x4 byte transpose: o[j] = (w0.bj, w1.bj, w2.bj, w3.bj) */
+        const uint32_t a0 = __byte_perm(w[0], w[1], 0x5140), a1 = __byte_perm(w[0], w[1], 0x7362);
+        const uint32_t b0 = __byte_perm(w[2], w[3], 0x5140), b1 = __byte_perm(w[2], w[3], 0x7362);
+        const uint32_t o0 = __byte_perm(a0, b0, 0x5410), o1 = __byte_perm(a0, b0, 0x7632);
+        const uint32_t o2 = __byte_perm(a1, b1, 0x5410), o3 = __byte_perm(a1, b1, 0x7632);
+        T[4 * x + 0][tq ^ x] = o0;
+        T[4 * x + 1][tq ^ x] = o1;
+        T[4 * x + 2][tq ^ x] = o2;
+        T[4 * x + 3][tq ^ x] = o3;
+    }
+    __syncthreads();
+    for (int r = y; r < CT_TILE; r += 8) {
+        const int c = c_tile + r;
+        if (c >= nchans) break;
+        const uint32_t v = T[r][x ^ (r >> 2)];
+        const long long t = t_tile + 4 * x;
+        if (t < nsamp) *reinterpret_cast<uint32_t*>(out + (size_t)c * out_pitch + (size_t)t) = v;   /* rows are padded to 256 bytes */
+    }
+}
+
 /* ---- K5: sum_t D[i][t] and sum_t t*D[i][t] per row, int64 (all-rows checksum against the prefix-sum identity) */
 __global__ void __launch_bounds__(256)
 k_row_moments(const int32_t* __restrict__ D, long long pitch, long long nt, long long* __restrict__ sum_d,
@@ -177,5 +219,16 @@ extern "C" int aak_row_moments(const int32_t* D, int64_t pitch, int64_t nt, int3
 extern "C" int aak_peak_iadd(int32_t mode, int32_t iters, int32_t grid, int32_t threads, uint32_t* sink,
                              unsigned long long* cycles_out, void* stream) {
     k_peak_iadd<<<(unsigned)grid, (unsigned)threads, 0, (cudaStream_t)stream>>>(mode, iters, sink, cycles_out, 12345u, 1u);
+    return (int)cudaGetLastError();
+}
+
+/* in: [nsamp][in_stride] time-major (in_stride >= round_up(nchans, 4), in and in_stride 4-byte aligned);
+ * out: [nchans][out_pitch] channel-major, out_pitch a multiple of 4 with room for round_up(nsamp, 4) bytes per row. */
+extern "C" int aak_corner_turn(const uint8_t* in, size_t in_stride, uint8_t* out, size_t out_pitch, int32_t nchans, int64_t nsamp,
+                               void* stream) {
+    if (((uintptr_t)in & 3) || (in_stride & 3) || (out_pitch & 3) || in_stride < (size_t)((nchans + 3) & ~3)) return (int)cudaErrorInvalidValue;
+    if (nsamp <= 0 || nchans <= 0) return 0;
+    dim3 grid((unsigned)((nsamp + CT_TILE - 1) / CT_TILE), (unsigned)((nchans + CT_TILE - 1) / CT_TILE));
+    k_corner_turn<<<grid, 256, 0, (cudaStream_t)stream>>>(in, in_stride, out, out_pitch, nchans, nsamp);
     return (int)cudaGetLastError();
 }

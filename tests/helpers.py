@@ -159,10 +159,13 @@ def sampled_outputs(x: np.ndarray, k: np.ndarray, rng, start: int, T: int, point
 class GpuRun:
     """The CUDA path through the C-ABI binding for one workload (plan -> strategy -> chunk loop)."""
 
-    def __init__(self, w, x, **strategy_kw):
+    def __init__(self, w, x, time_major: bool = False, **strategy_kw):
+        """x is always the channel-major array [nchans][nsamp] the oracle sees; with time_major=True the library is handed
+        its transpose x_tm[t][c] (the plain definition of the corner turn) through a time-major plan."""
         import paper_1912_07704_b200 as aa
-        self.aa, self.w, self.x = aa, w, x
-        self.plan = aa.Plan(w.freqs_mhz, w.tsamp_s, w.ranges, w.widths, w.threshold)
+        self.aa, self.w = aa, w
+        self.x = np.ascontiguousarray(x.T) if time_major else x
+        self.plan = aa.Plan(w.freqs_mhz, w.tsamp_s, w.ranges, w.widths, w.threshold, time_major=time_major)
         self.st = aa.Strategy(self.plan, x.shape[1], **strategy_kw)
         self.h = self.st.handle
         self.info = self.st.info

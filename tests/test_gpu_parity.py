@@ -196,3 +196,59 @@ def test_sharded_strategies_partition_the_chunks_and_reproduce_the_single_run():
     assert len(merged) == len(ref)
     for f in ref.dtype.names:
         assert np.array_equal(merged[f], ref[f]), f
+
+
+# ------------------------------------------------------------------------------------------------ time-major input (corner turn)
+@pytest.mark.parametrize("nchans,nsamp,ranges,hint", [
+    (64, 8192, ((0.0, 1.0, 101, 1),), 0),                                              # Tiny, one chunk
+    (61, 5003, ((0.0, 1.3, 37, 1), (48.1, 2.6, 5, 2), (226.1, 9.0, 3, 8)), 0),         # nothing a multiple of a tile or of 4
+    (300, 30000, ((0.0, 0.5, 65, 2), (10.0, 0.5, 40, 1)), 8000),                       # several chunks: double-buffered staging
+])
+def test_time_major_input_gives_the_channel_major_result(nchans, nsamp, ranges, hint):
+    """PAPER.md:47 step 1: telescopes deliver x[t][c]. The library corner-turns each chunk on the device; the oracle is
+    handed the transpose (the plain definition). Every D row, every statistic and the candidate list must be identical."""
+    w = Workload("tm", nchans, 1500.0, -100.0 / max(nchans, 2), 256e-6, nsamp, ranges, (1, 2, 4, 8), 5.5,
+                 seed=4242 + nchans, npulses=3, pulse_dm=(5.0, 30.0), pulse_width_max=6, pulse_snr=(10.0, 25.0))
+    x, _ = make_input(w)
+    kw = dict(chunk_len_hint=hint) if hint else {}
+    gpu, orc = GpuRun(w, x, time_major=True, **kw), OracleRun(w, x)
+    try:
+        assert gpu.info["input_layout"] == gpu.aa.AA_LAYOUT_TIME_MAJOR and gpu.x.shape == (nsamp, nchans)
+        before = gpu.x.copy()
+        exp_all = []
+        for chunk in gpu.chunks:
+            gpu.dedisperse()
+            gpu.sps()
+            for r, rng in enumerate(w.ranges):
+                exp_all.append(check_band(gpu, orc, chunk, r, 0, rng[2], after_sps=True))
+        got = gpu.candidates()
+        n, og, oe = compare_candidates(got, np.concatenate(exp_all), w.threshold)
+        assert n + og == len(got) and n + oe == sum(len(e) for e in exp_all)
+        assert np.array_equal(gpu.x, before)
+        if hint:
+            assert gpu.info["nchunks"] >= 3
+    finally:
+        gpu.close()
+
+
+def test_time_major_device_chunk_and_layout_errors():
+    import torch
+    aa = __import__("paper_1912_07704_b200")
+    w = datagen.get_workload("tiny")
+    x, _ = make_input(w)
+    gpu, orc = GpuRun(w, x, time_major=True), OracleRun(w, x)
+    try:
+        xd = torch.from_numpy(gpu.x).cuda()                       # [nsamp][nchans] on the device
+        aa.aa_run_dedispersion_device(gpu.h, xd, xd.stride(0))
+        gpu.sps()
+        exp = check_band(gpu, orc, gpu.chunks[0], 0, 0, w.ranges[0][2], after_sps=True)
+        compare_candidates(gpu.candidates(), exp, w.threshold)
+        aa.aa_strategy_reset(gpu.h)
+        with pytest.raises(aa.AaError) as e:                      # stride shorter than a time row
+            aa.aa_run_dedispersion(gpu.h, gpu.x, w.nchans - 1)
+        assert e.value.status == aa.AA_ERR_INVALID_ARG and "nchans" in e.value.message
+        with pytest.raises(aa.AaError) as e:
+            aa.aa_plan_set_input_layout(gpu.plan.handle, 7)
+        assert e.value.status == aa.AA_ERR_INVALID_ARG and "layout" in e.value.message
+    finally:
+        gpu.close()
