@@ -1,0 +1,154 @@
+"""GPU tests of the boundary behaviour the paper asks of the API and of the rarely taken routes of the kernels:
+memory manager (one allocation, no leak, caller-lent arena: PAPER.md:33), ownership of results, immutable
+strategy, status codes per iteration, candidate overflow, and the fallback route of K3
+(rows whose head is not representative of the row) — all compared with the oracle where there is arithmetic."""
+import numpy as np
+import pytest
+
+import datagen
+from datagen.workloads import Workload, scaled
+
+from helpers import GpuRun, OracleRun, check_band, compare_candidates, make_input
+
+pytestmark = pytest.mark.gpu
+
+
+def _free_bytes():
+    import torch
+    torch.cuda.synchronize()
+    return torch.cuda.mem_get_info()[0]
+
+
+def test_one_allocation_no_leak_and_lent_arena():
+    import torch
+    import paper_1912_07704_b200 as aa
+    torch.cuda.init()
+    torch.zeros(1, device="cuda")
+    w = datagen.get_workload("tiny")
+    x, _ = make_input(w)
+    warm = GpuRun(w, x)                 # first use loads the kernels and creates the context's pools: not part of the check
+    warm.st.run(x)
+    warm.close()
+    before = _free_bytes()
+    g = GpuRun(w, x)
+    try:
+        info = g.info
+        assert info["owns_arena"] == 1 and info["arena_bytes_total"] == info["arena_bytes_used"] > 0
+        during = _free_bytes()
+        assert before - during >= info["arena_bytes_used"]                 # the single cudaMalloc (+ allocator granularity)
+        ref = g.st.run(x)
+        assert _free_bytes() == during                                     # nothing is allocated by aa_run_*
+    finally:
+        g.close()
+    assert _free_bytes() == before                                         # proper de-allocation
+    # caller-lent arena: a torch tensor; the library allocates nothing on the device
+    need = info["arena_bytes_used"]
+    arena = torch.empty(need + 4096, dtype=torch.uint8, device="cuda")
+    base = _free_bytes()
+    g2 = GpuRun(w, x, arena=arena)
+    try:
+        assert g2.info["owns_arena"] == 0 and _free_bytes() == base
+        got = g2.st.run(x)
+        assert _free_bytes() == base
+        assert len(got) == len(ref) and all(np.array_equal(got[f], ref[f]) for f in ref.dtype.names)
+    finally:
+        g2.close()
+    small = torch.empty(need // 2, dtype=torch.uint8, device="cuda")
+    with pytest.raises(aa.AaError) as e:
+        GpuRun(w, x, arena=small)
+    assert e.value.status == aa.AA_ERR_BUDGET_TOO_SMALL and "needs" in e.value.message     # states the bytes required
+
+
+def test_status_codes_order_and_immutable_strategy():
+    import paper_1912_07704_b200 as aa
+    w = scaled(datagen.get_workload("tiny"), nsamp=6000, name="tiny6k")
+    x, _ = make_input(w)
+    g = GpuRun(w, x, chunk_len_hint=2048)
+    try:
+        n = g.info["nchunks"]
+        assert n >= 3
+        desc0 = aa.aa_strategy_describe(g.h)
+        geo0 = [aa.aa_strategy_get_range_info(g.h, r) for r in range(len(w.ranges))]
+        with pytest.raises(aa.AaError) as e:                               # "another module still needs to run"
+            aa.aa_run_sps(g.h)
+        assert e.value.status == aa.AA_ERR_ORDER
+        seen = []
+        for j in range(n):
+            assert aa.aa_run_dedispersion(g.h, x) == aa.AA_OK
+            with pytest.raises(aa.AaError) as e:
+                aa.aa_run_dedispersion(g.h, x)                             # SPS of this chunk has not run yet
+            assert e.value.status == aa.AA_ERR_ORDER and "aa_run_sps" in e.value.message
+            seen.append(aa.aa_run_sps(g.h))
+        assert seen == [aa.AA_STATUS_CHUNK_DONE] * (n - 1) + [aa.AA_STATUS_FINISHED]
+        with pytest.raises(aa.AaError) as e:                               # after FINISHED: an error code, not a crash
+            aa.aa_run_dedispersion(g.h, x)
+        assert e.value.status == aa.AA_ERR_ORDER and "all" in e.value.message
+        c1 = aa.aa_get_candidates(g.h)
+        c2 = aa.aa_get_candidates(g.h)                                     # results stay valid and stable
+        assert len(c1) == len(c2) > 0 and all(np.array_equal(c1[f], c2[f]) for f in c1.dtype.names)
+        # immutable once configured: the description and geometry do not change by running
+        assert aa.aa_strategy_describe(g.h) == desc0
+        assert [aa.aa_strategy_get_range_info(g.h, r) for r in range(len(w.ranges))] == geo0
+        # reset rewinds; a second run gives the same list
+        aa.aa_strategy_reset(g.h)
+        c3 = g.st.run(x)
+        assert len(c3) == len(c1) and all(np.array_equal(c3[f], c1[f]) for f in c1.dtype.names)
+    finally:
+        g.close()
+
+
+def test_candidate_overflow_is_counted_not_crashed():
+    import paper_1912_07704_b200 as aa
+    w = scaled(datagen.get_workload("tiny"), threshold=2.5, name="tiny_low_threshold")   # thousands of noise peaks
+    x, _ = make_input(w)
+    full = GpuRun(w, x, max_candidates=1 << 20)
+    try:
+        ref = full.st.run(x)
+    finally:
+        full.close()
+    assert len(ref) > 500
+    g = GpuRun(w, x, max_candidates=100)
+    try:
+        g.dedisperse()
+        g.sps()
+        with pytest.raises(aa.AaError) as e:
+            aa.aa_get_candidates(g.h)
+        assert e.value.status == aa.AA_ERR_CANDIDATE_OVERFLOW and str(len(ref)) in e.value.message   # the true count
+        part = aa.aa_get_candidates(g.h, allow_overflow=True)
+        assert len(part) == 100
+        keys = set(zip(ref["range"].tolist(), ref["dm_index"].tolist(), ref["sample"].tolist()))
+        assert all(k in keys for k in zip(part["range"].tolist(), part["dm_index"].tolist(), part["sample"].tolist()))
+    finally:
+        g.close()
+
+
+@pytest.mark.parametrize("kind", ["quiet_head", "loud_head", "heavy_tails", "two_level"])
+def test_row_statistics_fallback_routes_match_the_oracle(kind):
+    """K3 reads a row once, using a core interval estimated from the row's first 8192 samples. These inputs break that
+    estimate on purpose (head much quieter / much louder than the row, > 2.4 % outliers, bimodal row), forcing the list
+    overflow and the 'bound cuts into the core' exits into the plain multi-pass route. mu and sigma must still equal the
+    oracle's exactly, and so must the candidates."""
+    rs = np.random.default_rng(99)
+    C, N = 16, 70_000
+    sig = np.full(N, 12.0)
+    if kind == "quiet_head":
+        sig[:12_000] = 0.7
+    elif kind == "loud_head":
+        sig[:12_000] = 60.0
+    v = 127.0 + rs.standard_normal((C, N)) * sig
+    if kind == "heavy_tails":
+        m = rs.random((C, N)) < 0.06
+        v[m] += rs.choice([-90.0, 90.0], size=int(m.sum()))
+    if kind == "two_level":
+        v[:, N // 2:] += 40.0
+    x = np.clip(np.floor(v + 0.5), 0, 255).astype(np.uint8)
+    w = Workload(kind, C, 1500.0, -1.0, 256e-6, N, ((0.0, 2.0, 6, 1), (12.0, 4.0, 5, 2)), (1, 2, 4, 8), 5.0, seed=1, npulses=0,
+                 pulse_dm=(0.0, 0.0), pulse_width_max=1)
+    gpu, orc = GpuRun(w, x), OracleRun(w, x)
+    try:
+        gpu.dedisperse()
+        gpu.sps()
+        exp = [check_band(gpu, orc, gpu.chunks[0], r, 0, rng[2], after_sps=True) for r, rng in enumerate(w.ranges)]
+        compare_candidates(gpu.candidates(allow_overflow=True), np.concatenate(exp), w.threshold)
+    finally:
+        gpu.close()
