@@ -23,6 +23,7 @@ aa_status cuda_fail(cudaError_t e, const char* what);
 
 constexpr int kDmTile = 32;       /* must match k_dedisp.cu */
 constexpr int kTTile = 1024;
+constexpr int kMaxGroups = 4;      /* channel groups of a pipelined (not prefetched) chunk copy */
 constexpr size_t kSlack = 64 * 1024;   /* readable bytes after every input buffer (TMA windows over-read) */
 
 inline size_t round_up(size_t v, size_t m) { return (v + m - 1) / m * m; }
@@ -106,6 +107,7 @@ struct Strategy {
     bool owns_compute = false, owns_copy = false;
     cudaEvent_t ev_copied[2] = {nullptr, nullptr};    /* chunk landed in d_raw[b] (copy stream) */
     cudaEvent_t ev_raw_free[2] = {nullptr, nullptr};  /* last reader of d_raw[b] finished (compute stream) */
+    cudaEvent_t ev_group[kMaxGroups] = {nullptr};     /* channel group g of the current chunk landed (copy stream) */
     cudaEvent_t ev_count = nullptr;                   /* candidate counter copied to the host */
     cudaEvent_t ev_t[6] = {nullptr};                  /* timing marks on the compute stream */
     cudaEvent_t ev_h2d[2] = {nullptr, nullptr};       /* timing marks on the copy stream */

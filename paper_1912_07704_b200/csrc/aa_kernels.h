@@ -52,6 +52,8 @@ typedef struct {
     int32_t in16;              /* 0: uint8 input (bin 1), 1: uint16 input (binned) */
     int32_t variant;           /* uint8 only: odd-byte lane adds as 0 = IADD3, 1 = IMAD (FMA pipe), 2 = alternating */
     int32_t ring_stages;       /* depth of the shared-memory stage ring (2..8) */
+    int32_t chan_begin, chan_end; /* sum channels [chan_begin, chan_end) only (multiples of chan_block; chan_end 0 = nchans) */
+    int32_t accumulate;        /* 1: D += the partial sums (a later channel group of the same chunk), 0: D = */
     int32_t dms_per_warp;      /* 2 or 4 adjacent DM trials per warp (words of equal-delay trials are reused from registers) */
 } aak_dedisp_args;
 int aak_dedisperse(const aak_dedisp_args* a, void* stream);

@@ -49,9 +49,62 @@ aa_status enqueue_h2d(Strategy& s, int64_t j, int b, const uint8_t* host_input, 
     return AA_OK;
 }
 
+/* Channel groups of a chunk whose H2D copy is pipelined with its own dedispersion (boundaries are multiples of 8, the
+ * largest channel block of K2). */
+struct ChannelGroups { int n; int32_t c[kMaxGroups + 1]; };
+
+/* K1 for channel rows [c0, c1) of the chunk in raw buffer b: sample-shifted uint8 copies, binned inputs and their copies. */
+aa_status enqueue_prep(Strategy& s, const Chunk& c, int b, int32_t c0, int32_t c1) {
+    const int32_t n = c1 - c0;
+    const uint8_t* raw = s.d_raw[b] + (size_t)c0 * s.in_pitch;
+    if (s.need_u8_copies)
+        AA_LAUNCH(aak_make_copies_u8(raw, s.d_x4 + (size_t)c0 * s.in_pitch, s.in_pitch, s.x4_stride, s.in_pitch, n, s.compute), "shifted copies (uint8)");
+    for (int bin = 2; bin <= 8; bin *= 2) {
+        if (!s.d_xb[bin]) continue;
+        const size_t pitch_bytes = s.xb_pitch[bin] * 2;
+        uint16_t* xb = s.d_xb[bin] + (size_t)c0 * s.xb_pitch[bin];
+        AA_LAUNCH(aak_bin_time(raw, s.in_pitch, xb, s.xb_pitch[bin], n, (int64_t)(c.len / (uint64_t)bin), bin, s.compute), "time binning");
+        AA_LAUNCH(aak_shift_copy((const uint8_t*)xb, (uint8_t*)xb + s.xb_stride[bin], pitch_bytes, pitch_bytes, n, 2, s.compute), "shift copy (uint16)");
+    }
+    return AA_OK;
+}
+
+/* K2 of every range over channels [c0, c1); accumulate = add to the D already there. */
+aa_status enqueue_k2(Strategy& s, const Chunk& c, int32_t c0, int32_t c1, bool accumulate) {
+    for (Range& rg : s.ranges) {
+        aak_dedisp_args a;
+        a.tmap = &rg.map;
+        a.etab = rg.d_etab; a.x0tab = rg.d_x0tab; a.D = rg.d_D; a.pitch = rg.pitch;
+        a.nt = (int64_t)(c.n_out / (uint64_t)rg.r.bin);
+        a.ndms = rg.r.ndms; a.nchans = s.plan.nchans; a.chan_block = rg.chan_block; a.window_bytes = rg.window_bytes;
+        a.spill_stages = rg.spill_stages; a.in16 = rg.in16; a.variant = rg.variant; a.dms_per_warp = rg.dms_per_warp; a.ring_stages = rg.ring_stages;
+        a.chan_begin = c0; a.chan_end = c1; a.accumulate = accumulate ? 1 : 0;
+        AA_LAUNCH(aak_dedisperse(&a, s.compute), "dedispersion");
+    }
+    return AA_OK;
+}
+
+/* H2D of chunk j into raw buffer b as `groups.n` row blocks, one event per block (channel-major plans). */
+aa_status enqueue_h2d_groups(Strategy& s, int64_t j, int b, const uint8_t* host_input, size_t row_stride, const ChannelGroups& groups) {
+    const Chunk& c = s.chunks[(size_t)j];
+    if (s.raw_free_recorded[b]) AA_CUDA(cudaStreamWaitEvent(s.copy, s.ev_raw_free[b], 0), "cudaStreamWaitEvent");
+    AA_CUDA(cudaEventRecord(s.ev_h2d[0], s.copy), "cudaEventRecord");
+    for (int g = 0; g < groups.n; ++g) {
+        const int32_t c0 = groups.c[g], c1 = groups.c[g + 1];
+        AA_CUDA(cudaMemcpy2DAsync(s.d_raw[b] + (size_t)c0 * s.in_pitch, s.in_pitch, host_input + (size_t)c0 * row_stride + c.start, row_stride,
+                                  (size_t)c.len, (size_t)(c1 - c0), cudaMemcpyHostToDevice, s.copy), "cudaMemcpy2DAsync (H2D channel group)");
+        AA_CUDA(cudaEventRecord(s.ev_group[g], s.copy), "cudaEventRecord");
+    }
+    AA_CUDA(cudaEventRecord(s.ev_h2d[1], s.copy), "cudaEventRecord");
+    AA_CUDA(cudaEventRecord(s.ev_copied[b], s.copy), "cudaEventRecord");
+    s.raw_holds[b] = j;
+    return AA_OK;
+}
+
 /* Corner turn (time-major plans), shifted copies, binning and the dedispersion launches for the chunk resident in input
  * buffer b. tm_src/tm_stride: the time-major source of the corner turn (the staging buffer, or the caller's device chunk). */
-aa_status enqueue_dedispersion(Strategy& s, int64_t j, int b, const uint8_t* tm_src = nullptr, size_t tm_stride = 0) {
+aa_status enqueue_dedispersion(Strategy& s, int64_t j, int b, const uint8_t* tm_src = nullptr, size_t tm_stride = 0,
+                               const ChannelGroups* groups = nullptr) {
     const Chunk& c = s.chunks[(size_t)j];
     const int32_t C = s.plan.nchans;
     const int slot = b;                               /* the buffer whose reuse the raw_free event guards */
@@ -61,23 +114,21 @@ aa_status enqueue_dedispersion(Strategy& s, int64_t j, int b, const uint8_t* tm_
         AA_LAUNCH(aak_corner_turn(tm_src, tm_stride, s.d_raw[0], s.in_pitch, C, (int64_t)c.len, s.compute), "corner turn");
         b = 0;                                        /* the channel-major copy lives in d_raw[0] */
     }
-    if (s.need_u8_copies)
-        AA_LAUNCH(aak_make_copies_u8(s.d_raw[b], s.d_x4, s.in_pitch, s.x4_stride, s.in_pitch, C, s.compute), "shifted copies (uint8)");
-    for (int bin = 2; bin <= 8; bin *= 2) {
-        if (!s.d_xb[bin]) continue;
-        const size_t pitch_bytes = s.xb_pitch[bin] * 2;
-        AA_LAUNCH(aak_bin_time(s.d_raw[b], s.in_pitch, s.d_xb[bin], s.xb_pitch[bin], C, (int64_t)(c.len / (uint64_t)bin), bin, s.compute), "time binning");
-        AA_LAUNCH(aak_shift_copy((const uint8_t*)s.d_xb[bin], (uint8_t*)s.d_xb[bin] + s.xb_stride[bin], pitch_bytes, pitch_bytes, C, 2, s.compute), "shift copy (uint16)");
-    }
-    AA_CUDA(cudaEventRecord(s.ev_t[1], s.compute), "cudaEventRecord");
-    for (Range& rg : s.ranges) {
-        aak_dedisp_args a;
-        a.tmap = &rg.map;
-        a.etab = rg.d_etab; a.x0tab = rg.d_x0tab; a.D = rg.d_D; a.pitch = rg.pitch;
-        a.nt = (int64_t)(c.n_out / (uint64_t)rg.r.bin);
-        a.ndms = rg.r.ndms; a.nchans = C; a.chan_block = rg.chan_block; a.window_bytes = rg.window_bytes;
-        a.spill_stages = rg.spill_stages; a.in16 = rg.in16; a.variant = rg.variant; a.dms_per_warp = rg.dms_per_warp; a.ring_stages = rg.ring_stages;
-        AA_LAUNCH(aak_dedisperse(&a, s.compute), "dedispersion");
+    if (groups) {
+        /* the chunk is still arriving: channel group g is prepared and added to D as soon as its rows have landed, so only
+         * the first group's copy is exposed (D is accumulated over the groups: int32 sums, any grouping gives the same bits) */
+        for (int g = 0; g < groups->n; ++g) {
+            AA_CUDA(cudaStreamWaitEvent(s.compute, s.ev_group[g], 0), "cudaStreamWaitEvent");
+            aa_status st = enqueue_prep(s, c, b, groups->c[g], groups->c[g + 1]);
+            if (st != AA_OK) return st;
+            if (g == 0) AA_CUDA(cudaEventRecord(s.ev_t[1], s.compute), "cudaEventRecord");
+            if ((st = enqueue_k2(s, c, groups->c[g], groups->c[g + 1], g > 0)) != AA_OK) return st;
+        }
+    } else {
+        aa_status st = enqueue_prep(s, c, b, 0, C);
+        if (st != AA_OK) return st;
+        AA_CUDA(cudaEventRecord(s.ev_t[1], s.compute), "cudaEventRecord");
+        if ((st = enqueue_k2(s, c, 0, C, false)) != AA_OK) return st;
     }
     AA_CUDA(cudaEventRecord(s.ev_t[2], s.compute), "cudaEventRecord");
     AA_CUDA(cudaEventRecord(s.ev_raw_free[slot], s.compute), "cudaEventRecord");
@@ -132,12 +183,21 @@ extern "C" aa_status aa_run_dedispersion(aa_strategy* h, const uint8_t* host_inp
     const int64_t j = s.next_chunk;
     const int b = two_buffers ? (int)((j / s.shard_world) & 1) : 0;
     s.h2d_timed = false;
+    ChannelGroups groups; groups.n = 0;
     if (s.raw_holds[b] != j) {
-        if ((st = enqueue_h2d(s, j, b, host_input, row_stride_bytes, true)) != AA_OK) return st;
+        /* not prefetched (first chunk, or a single-chunk observation): pipeline the copy with the compute by channel groups */
+        const int32_t C = s.plan.nchans;
+        if (!tmajor && C >= 64 * kMaxGroups) {
+            groups.n = kMaxGroups;
+            for (int g = 0; g <= groups.n; ++g) groups.c[g] = g == groups.n ? C : (int32_t)(((int64_t)C * g / groups.n) & ~7);
+            if ((st = enqueue_h2d_groups(s, j, b, host_input, row_stride_bytes, groups)) != AA_OK) return st;
+        } else {
+            if ((st = enqueue_h2d(s, j, b, host_input, row_stride_bytes, true)) != AA_OK) return st;
+        }
         s.h2d_timed = true;
     }
-    AA_CUDA(cudaStreamWaitEvent(s.compute, s.ev_copied[b], 0), "cudaStreamWaitEvent");
-    if ((st = enqueue_dedispersion(s, j, b)) != AA_OK) return st;
+    if (!groups.n) AA_CUDA(cudaStreamWaitEvent(s.compute, s.ev_copied[b], 0), "cudaStreamWaitEvent");
+    if ((st = enqueue_dedispersion(s, j, b, nullptr, 0, groups.n ? &groups : nullptr)) != AA_OK) return st;
     /* double buffering: start moving chunk j+1 while chunk j computes (north_star "Streaming") */
     const int64_t jn = j + s.shard_world;           /* the next chunk of this strategy's shard */
     if (two_buffers && jn < (int64_t)s.chunks.size() && s.raw_holds[b ^ 1] != jn)

@@ -343,6 +343,8 @@ extern "C" aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, u
         if ((e = cudaEventCreate(&s.ev_h2d[b])) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
     }
     if ((e = cudaEventCreateWithFlags(&s.ev_count, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
+    for (int g = 0; g < kMaxGroups; ++g)
+        if ((e = cudaEventCreateWithFlags(&s.ev_group[g], cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
     for (int i = 0; i < 6; ++i)
         if ((e = cudaEventCreate(&s.ev_t[i])) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
     if ((e = cudaHostAlloc((void**)&s.h_counter, 64, cudaHostAllocDefault)) != cudaSuccess) return fail(cuda_fail(e, "cudaHostAlloc"));
@@ -388,6 +390,7 @@ extern "C" void aa_strategy_destroy(aa_strategy* h) {
         if (s.ev_h2d[b]) cudaEventDestroy(s.ev_h2d[b]);
     }
     if (s.ev_count) cudaEventDestroy(s.ev_count);
+    for (int g = 0; g < kMaxGroups; ++g) if (s.ev_group[g]) cudaEventDestroy(s.ev_group[g]);
     for (int i = 0; i < 6; ++i) if (s.ev_t[i]) cudaEventDestroy(s.ev_t[i]);
     if (s.owns_compute && s.compute) cudaStreamDestroy(s.compute);
     if (s.owns_copy && s.copy) cudaStreamDestroy(s.copy);

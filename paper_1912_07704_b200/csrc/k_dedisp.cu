@@ -65,6 +65,8 @@ struct DedispParams {
     int window_bytes;
     int spill_stages;
     int nring;                 /* ring depth */
+    int stage_begin, stage_end; /* channel blocks [stage_begin, stage_end) of the nstages are summed by this launch */
+    int accumulate;            /* 1: add to the values already in D (a later channel group of the same chunk) */
     unsigned one;              /* always 1; a runtime value so that x*one+y stays an IMAD (FMA pipe) */
 };
 
@@ -171,7 +173,7 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
             const int32_t* erow = p.etab + (size_t)dt * (size_t)p.nstages * (CB * DM_TILE);
             const long long tb = t0 * ESZ;
             int slot = 0; uint32_t ph = 0;
-            for (int s = 0; s < p.nstages; ++s) {
+            for (int s = p.stage_begin; s < p.stage_end; ++s) {
                 int x0[CB];
 #pragma unroll
                 for (int c = 0; c < CB; ++c) x0[c] = __ldg(x0row + s * CB + c);
@@ -208,7 +210,7 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
     const int ent_off = data_bytes + grp * M * 4;
     int until_spill = p.spill_stages;
     int slot = 0; uint32_t ph = 0;
-    for (int s = 0; s < p.nstages; ++s) {
+    for (int s = p.stage_begin; s < p.stage_end; ++s) {
         mbar_wait<CONSUMER_SLEEP_NS>(bar_full + 8 * slot, ph);
         const uint8_t* sb = stages + (size_t)slot * stage_bytes;
         const uint8_t* db = sb + lane * 4 + part * (T_PART * ESZ);
@@ -315,11 +317,19 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
                 v.y = (int)((H[m][j] & 0xFFFFu) + ((C2[m][j] & 0xFFFFu) << 8));
                 v.z = (int)((L >> 16) + ((C1[m][j] >> 16) << 8));
                 v.w = (int)((H[m][j] >> 16) + ((C2[m][j] >> 16) << 8));
+                if (p.accumulate) {
+                    const int4 o = *reinterpret_cast<const int4*>(row + t);
+                    v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w;
+                }
                 *reinterpret_cast<int4*>(row + t) = v;
             } else {
                 int2 v;
                 v.x = (int)((A[m][j] & 0xFFFFu) + ((C1[m][j] & 0xFFFFu) << 8));
                 v.y = (int)((A[m][j] >> 16) + ((C1[m][j] >> 16) << 8));
+                if (p.accumulate) {
+                    const int2 o = *reinterpret_cast<const int2*>(row + t);
+                    v.x += o.x; v.y += o.y;
+                }
                 *reinterpret_cast<int2*>(row + t) = v;
             }
         }
@@ -344,6 +354,10 @@ int launch(const aak_dedisp_args* a, cudaStream_t st) {
     DedispParams p;
     p.etab = a->etab; p.x0tab = a->x0tab; p.D = a->D; p.pitch = a->pitch; p.nt = a->nt; p.ndms = a->ndms;
     p.nstages = (a->nchans + CB - 1) / CB;
+    /* channel group [chan_begin, chan_end): whole channel blocks (chan_end == 0 means all channels) */
+    const int cend = a->chan_end > 0 ? a->chan_end : a->nchans;
+    if (a->chan_begin % CB || (cend % CB && cend != a->nchans) || a->chan_begin >= cend) return (int)cudaErrorInvalidValue;
+    p.stage_begin = a->chan_begin / CB; p.stage_end = (cend + CB - 1) / CB; p.accumulate = a->accumulate;
     p.window_bytes = a->window_bytes; p.spill_stages = a->spill_stages; p.one = 1u;
     p.nring = a->ring_stages;
     if (p.nring < 2 || p.nring > MAX_RING) return (int)cudaErrorInvalidValue;
