@@ -189,7 +189,11 @@ extern "C" aa_status aa_run_dedispersion(aa_strategy* h, const uint8_t* host_inp
         const int32_t C = s.plan.nchans;
         if (!tmajor && C >= 64 * kMaxGroups) {
             groups.n = kMaxGroups;
-            for (int g = 0; g <= groups.n; ++g) groups.c[g] = g == groups.n ? C : (int32_t)(((int64_t)C * g / groups.n) & ~7);
+            /* the copy is several times faster than the compute, so only the FIRST group's copy is exposed: make it small
+             * (1/16 of the channels) and split the rest evenly */
+            const int32_t first = std::max<int32_t>(8, (C / 16) & ~7);
+            groups.c[0] = 0; groups.c[groups.n] = C;
+            for (int g = 1; g < groups.n; ++g) groups.c[g] = (int32_t)((first + (int64_t)(C - first) * (g - 1) / (groups.n - 1)) & ~7);
             if ((st = enqueue_h2d_groups(s, j, b, host_input, row_stride_bytes, groups)) != AA_OK) return st;
         } else {
             if ((st = enqueue_h2d(s, j, b, host_input, row_stride_bytes, true)) != AA_OK) return st;
