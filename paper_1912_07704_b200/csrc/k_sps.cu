@@ -300,7 +300,7 @@ k_row_stats(const aak_row_desc* __restrict__ rows, double* __restrict__ mu_sigma
  */
 constexpr int K4_THREADS = 256;
 constexpr int K4_WARPS = K4_THREADS / 32;
-constexpr int K4_RB = 32;                      /* centre rows per CTA */
+constexpr int K4_RB = 32;                      /* centre rows per CTA (fewer when the grid would not fill the GPU) */
 constexpr int SPS_MAXW = 16;
 
 struct SpsParams {
@@ -310,6 +310,7 @@ struct SpsParams {
     u64 chunk_start;
     int widths[SPS_MAXW]; int nwidths; int wmax;
     int tt;                                    /* centre samples per strip, multiple of 4 */
+    int rb;                                    /* centre rows per CTA */
     double threshold;
     aak_candidate* cands; u64* counter; u64 capacity;
 };
@@ -387,8 +388,8 @@ k_sps_peaks(const SpsParams p) {
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const i64 t0 = (i64)blockIdx.x * p.tt;
     const i64 tb = t0 - 4;                                           /* sample index of element 0 of the segment */
-    const int i0 = blockIdx.y * K4_RB;
-    const int i1 = min(i0 + K4_RB, p.ndms);
+    const int i0 = blockIdx.y * p.rb;
+    const int i1 = min(i0 + p.rb, p.ndms);
     const int e0 = tid * 4 * V;                                      /* this thread's 4V contiguous elements */
     const int ne = p.tt + 4 + p.wmax;                                /* elements the strip needs */
 
@@ -580,7 +581,11 @@ extern "C" int aak_sps_peaks(const aak_sps_args* a, void* stream) {
     const int V = p.wmax <= 1024 ? 3 : (p.wmax <= 2048 ? 4 : 8);
     if (p.wmax > 6000) return (int)cudaErrorInvalidValue;
     p.tt = (1024 * V - 4 - p.wmax) & ~3;
-    dim3 grid((unsigned)((a->nt + p.tt - 1) / p.tt), (unsigned)((a->ndms + K4_RB - 1) / K4_RB));
+    /* each CTA recomputes 2 halo rows, so tall bands are cheaper; small searches take shorter bands to fill the 148 SMs */
+    const long long strips = (a->nt + p.tt - 1) / p.tt;
+    p.rb = K4_RB;
+    while (p.rb > 2 && strips * ((a->ndms + p.rb - 1) / p.rb) < 2 * 148) p.rb /= 2;
+    dim3 grid((unsigned)strips, (unsigned)((a->ndms + p.rb - 1) / p.rb));
     cudaStream_t st = (cudaStream_t)stream;
     switch (V) {
         case 3: k_sps_peaks<3><<<grid, K4_THREADS, sizeof(K4Smem<3>), st>>>(p); break;
