@@ -23,7 +23,8 @@ aa_status cuda_fail(cudaError_t e, const char* what);
 
 constexpr int kDmTile = 32;       /* must match k_dedisp.cu */
 constexpr int kTTile = 1024;
-constexpr int kMaxGroups = 4;      /* channel groups of a pipelined (not prefetched) chunk copy */
+constexpr int kMaxGroups = 4;
+constexpr unsigned kExcCap = 1u << 20;   /* exception records per (bin, channel group) */      /* channel groups of a pipelined (not prefetched) chunk copy */
 constexpr size_t kSlack = 64 * 1024;   /* readable bytes after every input buffer (TMA windows over-read) */
 
 inline size_t round_up(size_t v, size_t m) { return (v + m - 1) / m * m; }
@@ -51,21 +52,28 @@ struct Arena {
     }
 };
 
-struct Range {
+/* Tiling of K2 for one range in one input format (uint8 samples, or uint16 binned samples). */
+struct K2Plan {
+    int32_t in16 = 0, esz = 1, spw = 4, ncopy = 4;
+    int32_t chan_block = 8, window_bytes = 0, spill_stages = 0, nstages = 0;
+    int32_t dms_per_warp = 2, variant = 1, ring_stages = 3;   /* K2 tuning chosen by the strategy */
+    int32_t* d_etab = nullptr;
+    int32_t* d_x0tab = nullptr;
+    CUtensorMap map;              /* 4-D window map over the NCOPY-copy input buffer of this format */
+};
+
+struct Range : K2Plan {           /* the base is the range's main plan: uint8 for bin 1, uint16 for binned ranges */
     aa_dm_range r;
     int32_t index = 0;
-    int32_t in16 = 0, esz = 1, spw = 4, ncopy = 4;
     int64_t max_delay = 0;        /* binned samples */
     int64_t nt_full = 0;          /* T_r of a full chunk */
     int64_t pitch = 0;            /* D row pitch, elements */
-    int32_t chan_block = 8, window_bytes = 0, spill_stages = 0, ndm_tiles = 0, nstages = 0;
-    int32_t dms_per_warp = 2, variant = 1, ring_stages = 3;   /* K2 tuning chosen by the strategy */
+    int32_t ndm_tiles = 0;
     std::vector<int32_t> delays;  /* [ndms][nchans], binned samples (host) */
-    int32_t* d_etab = nullptr;
-    int32_t* d_x0tab = nullptr;
     int32_t* d_D = nullptr;
-    CUtensorMap map;              /* 4-D window map over the range's NCOPY-copy input buffer */
     size_t first_row = 0;         /* index of this range's first row in the row tables */
+    bool has_lo = false;          /* bin 2 / 4: the offset-uint8 route (k_misc.cu "Offset-uint8 form") with its own tiling */
+    K2Plan lo;
 };
 
 struct Chunk { uint64_t start, len, n_out; };
@@ -94,6 +102,15 @@ struct Strategy {
     size_t xb_pitch[9] = {0};                /* elements, indexed by bin */
     uint16_t* d_xb[9] = {nullptr};           /* binned input indexed by bin: copy 0, then copy 1 at +xb_stride bytes */
     size_t xb_stride[9] = {0};
+    /* offset-uint8 form of the binned inputs (bin 2, 4): 4 shifted byte copies, per-channel offsets, exceptions */
+    uint8_t* d_lo[9] = {nullptr};            /* copy k at + k*lo_stride bytes */
+    size_t lo_pitch[9] = {0}, lo_stride[9] = {0};
+    int32_t* d_off[9] = {nullptr};           /* [nchans] */
+    uint2* d_exc[9] = {nullptr};             /* [kMaxGroups][exc_cap] */
+    unsigned* d_exc_cnt[9] = {nullptr};      /* [kMaxGroups] exception counters, then [kMaxGroups] int32 biases (one memset clears both) */
+    unsigned exc_limit[9] = {0};             /* a group with more exceptions than this takes the uint16 route */
+    double* d_k = nullptr;                   /* delay constants on the device (exception scatter) */
+    bool d_k_needed = false;
     aak_row_desc* d_rows[2] = {nullptr, nullptr};   /* [0] full chunk geometry, [1] last (short) chunk */
     double* d_mu_sigma = nullptr;            /* [nrows][2] */
     int64_t* d_n_iters = nullptr;            /* [nrows][2] */

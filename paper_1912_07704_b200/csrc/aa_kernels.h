@@ -11,14 +11,17 @@
 
 #include <stddef.h>
 #include <stdint.h>
+#include <vector_types.h>
 
 #ifdef __cplusplus
 extern "C" {
 #endif
 
 /* ---- K1: time binning, x_b[c][t'] = sum_{j<b} x[c][b*t'+j]  (uint8 -> uint16) --------------------------------- */
+/* only_if_cnt (may be NULL): the kernel returns at once unless *only_if_cnt > only_if_above (the uint16 route of a
+ * range that also has the offset-uint8 route runs only for chunks with too many exceptions). Same for aak_shift_copy. */
 int aak_bin_time(const uint8_t* x, size_t x_pitch, uint16_t* xb, size_t xb_pitch_elems, int32_t nchans,
-                 int64_t nbinned, int32_t bin, void* stream);
+                 int64_t nbinned, int32_t bin, const unsigned* only_if_cnt, unsigned only_if_above, void* stream);
 /* ---- K1a: the four sample-shifted copies of the uint8 chunk in one pass: out[k*copy_stride + c*pitch + j] = in[c*pitch + j + k],
  * k = 0..3, j in [0, row_bytes). row_bytes, pitch, copy_stride multiples of 16; in readable 4 bytes past each row. */
 int aak_make_copies_u8(const uint8_t* in, uint8_t* out, size_t pitch, size_t copy_stride, size_t row_bytes, int32_t nrows,
@@ -26,7 +29,20 @@ int aak_make_copies_u8(const uint8_t* in, uint8_t* out, size_t pitch, size_t cop
 /* ---- K1b: shifted copy, out[c][j] = in[c][j + shift_bytes] (1..3) for j in [0, row_bytes), rows `pitch` bytes apart.
  * row_bytes and pitch are multiples of 16; the source must be readable up to row_bytes + 4 past each row start. */
 int aak_shift_copy(const uint8_t* in, uint8_t* out, size_t pitch, size_t row_bytes, int32_t nrows, int32_t shift_bytes,
-                   void* stream);
+                   const unsigned* only_if_cnt, unsigned only_if_above, void* stream);
+
+/* ---- K1c: offset-uint8 form of a binned input (bin 2, 4), see k_misc.cu: x_b = lo + off_c + r with lo a byte and r an
+ * exception list. aak_chan_offsets: off_b[c] = clamp(round(b * mean_t x[c][t]) - 128, 0, 255 (b-1)) for rows [0, nrows) and
+ * *bias_b += sum of them (either pair may be NULL). aak_bin_offset: lo[c][t'] (copy 0, bytes) and the exceptions
+ * {c + chan0 | (r + 1024) << 16, t'} appended at exc[atomicAdd(exc_cnt)] while below cap (the counter keeps counting).
+ * aak_scatter_exceptions: D[i][t' - delay(c, i)] += r for every exception and every trial of one range; returns at once
+ * if *exc_cnt > cap. k = the plan's delay constants (device doubles). */
+int aak_chan_offsets(const uint8_t* x, size_t pitch, int64_t len, int32_t nrows, int32_t* off2, int32_t* off4, int32_t* bias2,
+                     int32_t* bias4, void* stream);
+int aak_bin_offset(const uint8_t* x, size_t x_pitch, uint8_t* lo, size_t lo_pitch, const int32_t* off, int32_t nrows, int32_t chan0,
+                   int64_t nbinned, int32_t bin, uint2* exc, unsigned* exc_cnt, unsigned cap, void* stream);
+int aak_scatter_exceptions(const uint2* exc, const unsigned* exc_cnt, unsigned cap, const double* k, double dm_low, double dm_step,
+                           int32_t ndms, int32_t bin, int64_t nt, int32_t* D, int64_t pitch, void* stream);
 
 /* ---- K2: dedispersion --------------------------------------------------------------------------------------------
  * Tiled kernel: a CTA owns DM_TILE(=32) DM trials x T_TILE(=1024) output samples; channels stream through shared memory
@@ -54,6 +70,10 @@ typedef struct {
     int32_t ring_stages;       /* depth of the shared-memory stage ring (2..8) */
     int32_t chan_begin, chan_end; /* sum channels [chan_begin, chan_end) only (multiples of chan_block; chan_end 0 = nchans) */
     int32_t accumulate;        /* 1: D += the partial sums (a later channel group of the same chunk), 0: D = */
+    const unsigned* mode_cnt;  /* may be NULL. Else the launch returns at once unless (*mode_cnt > mode_cap) == mode_dense */
+    unsigned mode_cap;
+    int32_t mode_dense;
+    const int32_t* bias;       /* may be NULL. Else *bias is added to every output (sum of the channel offsets) */
     int32_t dms_per_warp;      /* 2 or 4 adjacent DM trials per warp (words of equal-delay trials are reused from registers) */
 } aak_dedisp_args;
 int aak_dedisperse(const aak_dedisp_args* a, void* stream);

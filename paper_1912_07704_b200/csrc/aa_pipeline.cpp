@@ -53,33 +53,60 @@ aa_status enqueue_h2d(Strategy& s, int64_t j, int b, const uint8_t* host_input, 
  * largest channel block of K2). */
 struct ChannelGroups { int n; int32_t c[kMaxGroups + 1]; };
 
-/* K1 for channel rows [c0, c1) of the chunk in raw buffer b: sample-shifted uint8 copies, binned inputs and their copies. */
-aa_status enqueue_prep(Strategy& s, const Chunk& c, int b, int32_t c0, int32_t c1) {
+/* K1 for channel rows [c0, c1) (= channel group g) of the chunk in raw buffer b: sample-shifted uint8 copies, the
+ * offset-uint8 form of the bin 2 / 4 inputs (per-channel offsets, byte copies, exception list), and the uint16 binned
+ * inputs with their shifted copies (for bin 2 / 4 only when the group has too many exceptions). */
+aa_status enqueue_prep(Strategy& s, const Chunk& c, int b, int32_t c0, int32_t c1, int g) {
     const int32_t n = c1 - c0;
     const uint8_t* raw = s.d_raw[b] + (size_t)c0 * s.in_pitch;
     if (s.need_u8_copies)
         AA_LAUNCH(aak_make_copies_u8(raw, s.d_x4 + (size_t)c0 * s.in_pitch, s.in_pitch, s.x4_stride, s.in_pitch, n, s.compute), "shifted copies (uint8)");
+    if (s.d_lo[2] || s.d_lo[4])
+        AA_LAUNCH(aak_chan_offsets(raw, s.in_pitch, (int64_t)c.len, n, s.d_lo[2] ? s.d_off[2] + c0 : nullptr, s.d_lo[4] ? s.d_off[4] + c0 : nullptr,
+                                   s.d_lo[2] ? (int32_t*)(s.d_exc_cnt[2] + kMaxGroups + g) : nullptr,
+                                   s.d_lo[4] ? (int32_t*)(s.d_exc_cnt[4] + kMaxGroups + g) : nullptr, s.compute), "channel offsets");
     for (int bin = 2; bin <= 8; bin *= 2) {
+        const int64_t nb = (int64_t)(c.len / (uint64_t)bin);
+        const unsigned* cnt = nullptr;
+        if (bin <= 4 && s.d_lo[bin]) {
+            cnt = s.d_exc_cnt[bin] + g;
+            uint8_t* lo = s.d_lo[bin] + (size_t)c0 * s.lo_pitch[bin];
+            AA_LAUNCH(aak_bin_offset(raw, s.in_pitch, lo, s.lo_pitch[bin], s.d_off[bin] + c0, n, c0, nb, bin, s.d_exc[bin] + (size_t)g * kExcCap,
+                                     s.d_exc_cnt[bin] + g, kExcCap, s.compute), "time binning (offset uint8)");
+            AA_LAUNCH(aak_make_copies_u8(lo, lo, s.lo_pitch[bin], s.lo_stride[bin], s.lo_pitch[bin], n, s.compute), "shifted copies (offset uint8)");
+        }
         if (!s.d_xb[bin]) continue;
         const size_t pitch_bytes = s.xb_pitch[bin] * 2;
         uint16_t* xb = s.d_xb[bin] + (size_t)c0 * s.xb_pitch[bin];
-        AA_LAUNCH(aak_bin_time(raw, s.in_pitch, xb, s.xb_pitch[bin], n, (int64_t)(c.len / (uint64_t)bin), bin, s.compute), "time binning");
-        AA_LAUNCH(aak_shift_copy((const uint8_t*)xb, (uint8_t*)xb + s.xb_stride[bin], pitch_bytes, pitch_bytes, n, 2, s.compute), "shift copy (uint16)");
+        AA_LAUNCH(aak_bin_time(raw, s.in_pitch, xb, s.xb_pitch[bin], n, nb, bin, cnt, s.exc_limit[bin], s.compute), "time binning");
+        AA_LAUNCH(aak_shift_copy((const uint8_t*)xb, (uint8_t*)xb + s.xb_stride[bin], pitch_bytes, pitch_bytes, n, 2, cnt, s.exc_limit[bin], s.compute), "shift copy (uint16)");
     }
     return AA_OK;
 }
 
-/* K2 of every range over channels [c0, c1); accumulate = add to the D already there. */
-aa_status enqueue_k2(Strategy& s, const Chunk& c, int32_t c0, int32_t c1, bool accumulate) {
+/* K2 of every range over channels [c0, c1) (channel group g); accumulate = add to the D already there. A bin 2 / 4 range
+ * launches both of its routes; each tests the group's exception counter and only one of them runs. */
+aa_status enqueue_k2(Strategy& s, const Chunk& c, int32_t c0, int32_t c1, bool accumulate, int g) {
     for (Range& rg : s.ranges) {
+        const int bin = rg.r.bin;
         aak_dedisp_args a;
-        a.tmap = &rg.map;
-        a.etab = rg.d_etab; a.x0tab = rg.d_x0tab; a.D = rg.d_D; a.pitch = rg.pitch;
-        a.nt = (int64_t)(c.n_out / (uint64_t)rg.r.bin);
-        a.ndms = rg.r.ndms; a.nchans = s.plan.nchans; a.chan_block = rg.chan_block; a.window_bytes = rg.window_bytes;
-        a.spill_stages = rg.spill_stages; a.in16 = rg.in16; a.variant = rg.variant; a.dms_per_warp = rg.dms_per_warp; a.ring_stages = rg.ring_stages;
+        a.D = rg.d_D; a.pitch = rg.pitch;
+        a.nt = (int64_t)(c.n_out / (uint64_t)bin);
+        a.ndms = rg.r.ndms; a.nchans = s.plan.nchans;
         a.chan_begin = c0; a.chan_end = c1; a.accumulate = accumulate ? 1 : 0;
-        AA_LAUNCH(aak_dedisperse(&a, s.compute), "dedispersion");
+        for (int route = rg.has_lo ? 0 : 1; route < 2; ++route) {
+            const K2Plan& p = route == 0 ? rg.lo : static_cast<const K2Plan&>(rg);
+            a.tmap = &p.map; a.etab = p.d_etab; a.x0tab = p.d_x0tab;
+            a.chan_block = p.chan_block; a.window_bytes = p.window_bytes; a.spill_stages = p.spill_stages; a.in16 = p.in16;
+            a.variant = p.variant; a.dms_per_warp = p.dms_per_warp; a.ring_stages = p.ring_stages;
+            a.mode_cnt = rg.has_lo ? s.d_exc_cnt[bin] + g : nullptr;
+            a.mode_cap = s.exc_limit[bin]; a.mode_dense = route;
+            a.bias = route == 0 ? (const int32_t*)(s.d_exc_cnt[bin] + kMaxGroups + g) : nullptr;
+            AA_LAUNCH(aak_dedisperse(&a, s.compute), "dedispersion");
+        }
+        if (rg.has_lo)
+            AA_LAUNCH(aak_scatter_exceptions(s.d_exc[bin] + (size_t)g * kExcCap, s.d_exc_cnt[bin] + g, s.exc_limit[bin], s.d_k, rg.r.dm_low, rg.r.dm_step,
+                                             rg.r.ndms, bin, a.nt, rg.d_D, rg.pitch, s.compute), "exception scatter");
     }
     return AA_OK;
 }
@@ -114,21 +141,23 @@ aa_status enqueue_dedispersion(Strategy& s, int64_t j, int b, const uint8_t* tm_
         AA_LAUNCH(aak_corner_turn(tm_src, tm_stride, s.d_raw[0], s.in_pitch, C, (int64_t)c.len, s.compute), "corner turn");
         b = 0;                                        /* the channel-major copy lives in d_raw[0] */
     }
+    for (int bn = 2; bn <= 4; bn *= 2)             /* exception counters and biases of this chunk's channel groups */
+        if (s.d_exc_cnt[bn]) AA_CUDA(cudaMemsetAsync(s.d_exc_cnt[bn], 0, 2 * kMaxGroups * 4, s.compute), "cudaMemsetAsync");
     if (groups) {
         /* the chunk is still arriving: channel group g is prepared and added to D as soon as its rows have landed, so only
          * the first group's copy is exposed (D is accumulated over the groups: int32 sums, any grouping gives the same bits) */
         for (int g = 0; g < groups->n; ++g) {
             AA_CUDA(cudaStreamWaitEvent(s.compute, s.ev_group[g], 0), "cudaStreamWaitEvent");
-            aa_status st = enqueue_prep(s, c, b, groups->c[g], groups->c[g + 1]);
+            aa_status st = enqueue_prep(s, c, b, groups->c[g], groups->c[g + 1], g);
             if (st != AA_OK) return st;
             if (g == 0) AA_CUDA(cudaEventRecord(s.ev_t[1], s.compute), "cudaEventRecord");
-            if ((st = enqueue_k2(s, c, groups->c[g], groups->c[g + 1], g > 0)) != AA_OK) return st;
+            if ((st = enqueue_k2(s, c, groups->c[g], groups->c[g + 1], g > 0, g)) != AA_OK) return st;
         }
     } else {
-        aa_status st = enqueue_prep(s, c, b, 0, C);
+        aa_status st = enqueue_prep(s, c, b, 0, C, 0);
         if (st != AA_OK) return st;
         AA_CUDA(cudaEventRecord(s.ev_t[1], s.compute), "cudaEventRecord");
-        if ((st = enqueue_k2(s, c, 0, C, false)) != AA_OK) return st;
+        if ((st = enqueue_k2(s, c, 0, C, false, 0)) != AA_OK) return st;
     }
     AA_CUDA(cudaEventRecord(s.ev_t[2], s.compute), "cudaEventRecord");
     AA_CUDA(cudaEventRecord(s.ev_raw_free[slot], s.compute), "cudaEventRecord");

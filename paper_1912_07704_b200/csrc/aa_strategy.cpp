@@ -85,6 +85,21 @@ static void carve(Strategy& s, int64_t L, bool two_raw) {
         s.xb_stride[b] = round_up((size_t)s.plan.nchans * s.xb_pitch[b] * 2 + kSlack, 256);
         s.d_xb[b] = used ? (uint16_t*)a.take(2 * s.xb_stride[b]) : nullptr;
     }
+    for (int bn = 2; bn <= 4; bn *= 2) {
+        bool used = false;
+        int64_t nd = 0;
+        for (const Range& rg : s.ranges) if (rg.r.bin == bn && rg.has_lo) { used = true; nd += rg.r.ndms; }
+        s.lo_pitch[bn] = used ? round_up((size_t)(L / bn), 256) : 0;
+        s.lo_stride[bn] = round_up((size_t)s.plan.nchans * s.lo_pitch[bn] + kSlack, 256);
+        s.d_lo[bn] = used ? (uint8_t*)a.take(4 * s.lo_stride[bn]) : nullptr;
+        s.d_off[bn] = used ? (int32_t*)a.take((size_t)s.plan.nchans * 4) : nullptr;
+        s.d_exc[bn] = used ? (uint2*)a.take((size_t)kMaxGroups * kExcCap * sizeof(uint2)) : nullptr;
+        s.d_exc_cnt[bn] = used ? (unsigned*)a.take(2 * kMaxGroups * 4) : nullptr;
+        /* the scatter costs one atomic per (exception, trial): beyond ~1e8 of them per group the uint16 route is cheaper */
+        s.exc_limit[bn] = used ? (unsigned)std::min<int64_t>((int64_t)kExcCap, std::max<int64_t>(1, 100000000 / std::max<int64_t>(1, nd))) : 0;
+        if (used && !s.d_k_needed) s.d_k_needed = true;
+    }
+    s.d_k = s.d_k_needed ? (double*)a.take((size_t)s.plan.nchans * 8) : nullptr;
     const int64_t n_out = L - s.S;
     for (Range& rg : s.ranges) {
         rg.nt_full = n_out / rg.r.bin;
@@ -92,6 +107,10 @@ static void carve(Strategy& s, int64_t L, bool two_raw) {
         rg.d_D = (int32_t*)a.take((size_t)rg.r.ndms * (size_t)rg.pitch * 4);
         rg.d_etab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * kDmTile * 4);
         rg.d_x0tab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * 4);
+        if (rg.has_lo) {
+            rg.lo.d_etab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.lo.nstages * rg.lo.chan_block * kDmTile * 4);
+            rg.lo.d_x0tab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.lo.nstages * rg.lo.chan_block * 4);
+        }
     }
     s.d_rows[0] = (aak_row_desc*)a.take(s.nrows * sizeof(aak_row_desc));
     s.d_rows[1] = (aak_row_desc*)a.take(s.nrows * sizeof(aak_row_desc));
@@ -120,10 +139,74 @@ static std::vector<Chunk> make_chunks(uint64_t nsamp, int64_t B, int64_t S, int6
     return v;
 }
 
-/* Kernel tiling and offset tables of one range (host side). Returns false with the error set. */
-static bool plan_range(Strategy& s, Range& rg, std::vector<int32_t>& etab, std::vector<int32_t>& x0tab) {
+/* Tiling and offset tables of K2 for one range in one input format (in16: uint16 binned samples, else bytes). */
+static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16, std::vector<int32_t>& etab, std::vector<int32_t>& x0tab) {
     const int32_t C = s.plan.nchans, nd = rg.r.ndms;
-    rg.in16 = rg.r.bin > 1; rg.esz = rg.in16 ? 2 : 1; rg.spw = 4 / rg.esz; rg.ncopy = rg.spw;
+    p.in16 = in16; p.esz = in16 ? 2 : 1; p.spw = 4 / p.esz; p.ncopy = p.spw;
+    /* widest window: T_TILE + largest in-tile delay spread + alignment residue (< 16 bytes) */
+    int64_t omax = 0;
+    for (int32_t t = 0; t < rg.ndm_tiles; ++t) {
+        const int32_t i0 = t * kDmTile, i1 = std::min(nd - 1, i0 + kDmTile - 1);
+        const int32_t* a = rg.delays.data() + (size_t)i0 * C;
+        const int32_t* b = rg.delays.data() + (size_t)i1 * C;
+        for (int32_t c = 0; c < C; ++c) omax = std::max<int64_t>(omax, (int64_t)b[c] - a[c]);
+    }
+    const int64_t wsamp = kTTile + omax + 16 / p.esz;
+    p.window_bytes = (int32_t)round_up((size_t)(wsamp * p.esz), 256);
+    if (p.window_bytes > 65536) { set_error("aa_strategy_setup: range %d needs a %d-byte channel window per DM tile (> 65536): DM step too coarse for this band", rg.index, p.window_bytes); return false; }
+    p.chan_block = 0;
+    p.ring_stages = 3;
+    for (int cb = 8; cb >= 2; cb /= 2)
+        if (aak_dedisperse_smem_bytes(cb, p.window_bytes, p.in16, p.ring_stages) <= 227 * 1024) { p.chan_block = cb; break; }
+    if (!p.chan_block) { set_error("aa_strategy_setup: range %d: channel window of %d bytes does not fit shared memory", rg.index, p.window_bytes); return false; }
+    if (aak_dedisperse_smem_bytes(p.chan_block, p.window_bytes, p.in16, 4) <= 227 * 1024) p.ring_stages = 4;
+    /* measured on B200 (profiles/): binned ranges are shared-memory bound and gain 13 % from 4 trials per warp with
+     * register reuse; the uint8 ranges are issue bound and lose 7 % to the extra branches, so they keep 2 trials per warp
+     * with the odd-byte adds on the FMA pipe */
+    p.dms_per_warp = p.in16 ? 4 : 2;
+    p.variant = 1;
+#ifdef AA_TUNING
+    if (const char* ev = getenv(p.in16 ? "AA_K2_M16" : "AA_K2_M8")) p.dms_per_warp = atoi(ev) == 4 ? 4 : 2;
+    if (const char* ev = getenv("AA_K2_VARIANT")) p.variant = atoi(ev);
+    if (const char* ev = getenv("AA_K2_RING")) {
+        const int n = atoi(ev);
+        if (n >= 2 && n <= 8 && aak_dedisperse_smem_bytes(p.chan_block, p.window_bytes, p.in16, n) <= 227 * 1024) p.ring_stages = n;
+    }
+#endif
+    p.nstages = (C + p.chan_block - 1) / p.chan_block;
+    /* 16-bit lanes are carried every 65536 / (largest sample value + 1) channels: bytes 256, uint16 sums of b bytes 256/b */
+    p.spill_stages = (in16 ? 256 / rg.r.bin : 256) / p.chan_block;
+    const int32_t CB = p.chan_block, Cpad = p.nstages * CB, WB = p.window_bytes;
+    etab.assign((size_t)rg.ndm_tiles * Cpad * kDmTile, 0);
+    x0tab.assign((size_t)rg.ndm_tiles * Cpad, 0);
+    for (int32_t t = 0; t < rg.ndm_tiles; ++t) {
+        const int32_t i0 = t * kDmTile;
+        for (int32_t c = 0; c < Cpad; ++c) {
+            int32_t* e = etab.data() + ((size_t)t * Cpad + c) * kDmTile;     /* [tile][stage][c_local][m] */
+            const int32_t cl = c % CB;
+            if (c >= C) {                                                   /* padding channel: TMA zero-fills it */
+                for (int m = 0; m < kDmTile; ++m) e[m] = cl * p.ncopy * WB;
+                continue;
+            }
+            const int64_t d0 = rg.delays[(size_t)i0 * C + c];
+            const int64_t xs = d0 * p.esz, xa = xs & ~(int64_t)15;
+            const int64_t res = (xs - xa) / p.esz;                          /* samples folded into the offsets */
+            x0tab[(size_t)t * Cpad + c] = (int32_t)xa;
+            for (int m = 0; m < kDmTile; ++m) {
+                const int32_t i = std::min(nd - 1, i0 + m);
+                const int64_t o = (int64_t)rg.delays[(size_t)i * C + c] - d0 + res;
+                const int64_t copy = o & (p.spw - 1);
+                e[m] = (int32_t)((cl * p.ncopy + copy) * WB + (o - copy) * p.esz);
+            }
+        }
+    }
+    return true;
+}
+
+/* Delays and the K2 plan(s) of one range (host side). Returns false with the error set. */
+static bool plan_range(Strategy& s, Range& rg, std::vector<int32_t>& etab, std::vector<int32_t>& x0tab,
+                       std::vector<int32_t>& etab_lo, std::vector<int32_t>& x0tab_lo) {
+    const int32_t C = s.plan.nchans, nd = rg.r.ndms;
     rg.delays.resize((size_t)nd * C);
     for (int32_t i = 0; i < nd; ++i) {
         const double dm = dm_of(rg.r, i);
@@ -136,62 +219,14 @@ static bool plan_range(Strategy& s, Range& rg, std::vector<int32_t>& etab, std::
     }
     rg.max_delay = rg.delays[(size_t)(nd - 1) * C + (C - 1)];
     rg.ndm_tiles = (nd + kDmTile - 1) / kDmTile;
-    /* widest window: T_TILE + largest in-tile delay spread + alignment residue (< 16 bytes) */
-    int64_t omax = 0;
-    for (int32_t t = 0; t < rg.ndm_tiles; ++t) {
-        const int32_t i0 = t * kDmTile, i1 = std::min(nd - 1, i0 + kDmTile - 1);
-        const int32_t* a = rg.delays.data() + (size_t)i0 * C;
-        const int32_t* b = rg.delays.data() + (size_t)i1 * C;
-        for (int32_t c = 0; c < C; ++c) omax = std::max<int64_t>(omax, (int64_t)b[c] - a[c]);
-    }
-    const int64_t wsamp = kTTile + omax + 16 / rg.esz;
-    rg.window_bytes = (int32_t)round_up((size_t)(wsamp * rg.esz), 256);
-    if (rg.window_bytes > 65536) { set_error("aa_strategy_setup: range %d needs a %d-byte channel window per DM tile (> 65536): DM step too coarse for this band", rg.index, rg.window_bytes); return false; }
-    rg.chan_block = 0;
-    rg.ring_stages = 3;
-    for (int cb = 8; cb >= 2; cb /= 2)
-        if (aak_dedisperse_smem_bytes(cb, rg.window_bytes, rg.in16, rg.ring_stages) <= 227 * 1024) { rg.chan_block = cb; break; }
-    if (!rg.chan_block) { set_error("aa_strategy_setup: range %d: channel window of %d bytes does not fit shared memory", rg.index, rg.window_bytes); return false; }
-    if (aak_dedisperse_smem_bytes(rg.chan_block, rg.window_bytes, rg.in16, 4) <= 227 * 1024) rg.ring_stages = 4;
-    /* measured on B200 (profiles/): binned ranges are shared-memory bound and gain 13 % from 4 trials per warp with
-     * register reuse; the uint8 ranges are issue bound and lose 7 % to the extra branches, so they keep 2 trials per warp
-     * with the odd-byte adds on the FMA pipe */
-    rg.dms_per_warp = rg.in16 ? 4 : 2;
-    rg.variant = 1;
+    if (!plan_format(s, rg, rg, rg.r.bin > 1, etab, x0tab)) return false;
+    /* bin 2 and 4 also get the offset-uint8 route (half the shared-memory bytes per add); the uint16 plan above stays as
+     * the route for chunks with too many exceptions. C < 65536 so a channel index fits the exception record. */
+    rg.has_lo = (rg.r.bin == 2 || rg.r.bin == 4) && C < 65536;
 #ifdef AA_TUNING
-    if (const char* ev = getenv(rg.in16 ? "AA_K2_M16" : "AA_K2_M8")) rg.dms_per_warp = atoi(ev) == 4 ? 4 : 2;
-    if (const char* ev = getenv("AA_K2_VARIANT")) rg.variant = atoi(ev);
-    if (const char* ev = getenv("AA_K2_RING")) {
-        const int n = atoi(ev);
-        if (n >= 2 && n <= 8 && aak_dedisperse_smem_bytes(rg.chan_block, rg.window_bytes, rg.in16, n) <= 227 * 1024) rg.ring_stages = n;
-    }
+    if (const char* ev = getenv("AA_K2_LO")) rg.has_lo = rg.has_lo && atoi(ev) != 0;
 #endif
-    rg.nstages = (C + rg.chan_block - 1) / rg.chan_block;
-    rg.spill_stages = (256 / rg.r.bin) / rg.chan_block;
-    const int32_t CB = rg.chan_block, Cpad = rg.nstages * CB, WB = rg.window_bytes;
-    etab.assign((size_t)rg.ndm_tiles * Cpad * kDmTile, 0);
-    x0tab.assign((size_t)rg.ndm_tiles * Cpad, 0);
-    for (int32_t t = 0; t < rg.ndm_tiles; ++t) {
-        const int32_t i0 = t * kDmTile;
-        for (int32_t c = 0; c < Cpad; ++c) {
-            int32_t* e = etab.data() + ((size_t)t * Cpad + c) * kDmTile;     /* [tile][stage][c_local][m] */
-            const int32_t cl = c % CB;
-            if (c >= C) {                                                   /* padding channel: TMA zero-fills it */
-                for (int m = 0; m < kDmTile; ++m) e[m] = cl * rg.ncopy * WB;
-                continue;
-            }
-            const int64_t d0 = rg.delays[(size_t)i0 * C + c];
-            const int64_t xs = d0 * rg.esz, xa = xs & ~(int64_t)15;
-            const int64_t res = (xs - xa) / rg.esz;                         /* samples folded into the offsets */
-            x0tab[(size_t)t * Cpad + c] = (int32_t)xa;
-            for (int m = 0; m < kDmTile; ++m) {
-                const int32_t i = std::min(nd - 1, i0 + m);
-                const int64_t o = (int64_t)rg.delays[(size_t)i * C + c] - d0 + res;
-                const int64_t copy = o & (rg.spw - 1);
-                e[m] = (int32_t)((cl * rg.ncopy + copy) * WB + (o - copy) * rg.esz);
-            }
-        }
-    }
+    if (rg.has_lo && !plan_format(s, rg, rg.lo, 0, etab_lo, x0tab_lo)) return false;
     return true;
 }
 
@@ -215,14 +250,14 @@ static aa_status plan_host(aa_strategy* h, const aa_plan* plan, uint64_t nsamp_t
     s.B = 1;
     for (const aa_dm_range& r : s.plan.ranges) s.B = std::max(s.B, r.bin);
     s.ranges.resize(s.plan.ranges.size());
-    etabs.resize(s.ranges.size()); x0tabs.resize(s.ranges.size());
+    etabs.resize(2 * s.ranges.size()); x0tabs.resize(2 * s.ranges.size());      /* [r]: main plan, [nranges + r]: offset-uint8 plan */
     int64_t smax = 0;
     s.nrows = 0;
     for (size_t r = 0; r < s.ranges.size(); ++r) {
         Range& rg = s.ranges[r];
         rg.r = s.plan.ranges[r];
         rg.index = (int32_t)r;
-        if (!plan_range(s, rg, etabs[r], x0tabs[r])) return AA_ERR_INVALID_ARG;
+        if (!plan_range(s, rg, etabs[r], x0tabs[r], etabs[s.ranges.size() + r], x0tabs[s.ranges.size() + r])) return AA_ERR_INVALID_ARG;
         smax = std::max<int64_t>(smax, rg.max_delay * rg.r.bin);
         rg.first_row = s.nrows;
         s.nrows += (size_t)rg.r.ndms;
@@ -359,6 +394,12 @@ extern "C" aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, u
         Range& rg = s.ranges[r];
         if ((e = cudaMemcpyAsync(rg.d_etab, etabs[r].data(), etabs[r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
         if ((e = cudaMemcpyAsync(rg.d_x0tab, x0tabs[r].data(), x0tabs[r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
+        if (rg.has_lo) {
+            const size_t n = s.ranges.size();
+            if ((e = cudaMemcpyAsync(rg.lo.d_etab, etabs[n + r].data(), etabs[n + r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
+            if ((e = cudaMemcpyAsync(rg.lo.d_x0tab, x0tabs[n + r].data(), x0tabs[n + r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
+            if (!make_window_map(&rg.lo.map, s.d_lo[rg.r.bin], s.lo_pitch[rg.r.bin], s.lo_stride[rg.r.bin], 4, C, rg.lo.window_bytes)) return fail(AA_ERR_CUDA);
+        }
         if (rg.in16) {
             if (!make_window_map(&rg.map, s.d_xb[rg.r.bin], s.xb_pitch[rg.r.bin] * 2, s.xb_stride[rg.r.bin], 2, C, rg.window_bytes)) return fail(AA_ERR_CUDA);
         } else {
@@ -373,6 +414,7 @@ extern "C" aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, u
     if ((e = cudaMemcpyAsync(s.d_rows[0], rows_full.data(), s.nrows * sizeof(aak_row_desc), cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "row table upload"));
     if ((e = cudaMemcpyAsync(s.d_rows[1], rows_last.data(), s.nrows * sizeof(aak_row_desc), cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "row table upload"));
     if ((e = cudaMemsetAsync(s.d_counter, 0, 256, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "cudaMemsetAsync"));
+    if (s.d_k && (e = cudaMemcpyAsync(s.d_k, s.k.data(), (size_t)C * 8, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "delay constants upload"));
     if ((e = cudaStreamSynchronize(s.compute)) != cudaSuccess) return fail(cuda_fail(e, "strategy upload"));   /* host tables go out of scope */
     s.ready = true;
     *out = h;
@@ -461,6 +503,11 @@ extern "C" size_t aa_strategy_describe(const aa_strategy* h, char* buf, size_t b
                  kDmTile, kTTile, rg.chan_block, rg.window_bytes, rg.nstages, rg.ndm_tiles, rg.spill_stages,
                  aak_dedisperse_smem_bytes(rg.chan_block, rg.window_bytes, rg.in16, rg.ring_stages));
         o += line;
+        if (rg.has_lo) {
+            snprintf(line, sizeof line, "         offset-uint8 route: chan_block=%d window=%dB stages=%d ring=%d exception limit %u per channel group\n",
+                     rg.lo.chan_block, rg.lo.window_bytes, rg.lo.nstages, rg.lo.ring_stages, s.exc_limit[rg.r.bin]);
+            o += line;
+        }
     }
     for (size_t j = 0; j < s.chunks.size() && j < 4; ++j) {
         snprintf(line, sizeof line, "chunk %zu: start=%llu len=%llu n_out=%llu\n", j, (unsigned long long)s.chunks[j].start,

@@ -67,6 +67,10 @@ struct DedispParams {
     int nring;                 /* ring depth */
     int stage_begin, stage_end; /* channel blocks [stage_begin, stage_end) of the nstages are summed by this launch */
     int accumulate;            /* 1: add to the values already in D (a later channel group of the same chunk) */
+    const unsigned* mode_cnt;  /* NULL, or: run only if (*mode_cnt > mode_cap) == mode_dense */
+    unsigned mode_cap;
+    int mode_dense;
+    const int* bias;           /* NULL, or a constant added to every output */
     unsigned one;              /* always 1; a runtime value so that x*one+y stays an IMAD (FMA pipe) */
 };
 
@@ -142,6 +146,7 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
     constexpr int ENT_BYTES = CB * DM_TILE * 4;
     static_assert(NG * NTH == NW && NTH >= 1 && J >= 1, "warp layout");
 
+    if (p.mode_cnt && ((*p.mode_cnt > p.mode_cap) ? 1 : 0) != p.mode_dense) return;     /* the other input format handles this chunk */
     extern __shared__ __align__(1024) uint8_t smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int ndm_tiles = (p.ndms + DM_TILE - 1) / DM_TILE;
@@ -301,6 +306,7 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
     }
 
     /* ---------------------------------------------------------------------- unpack and store */
+    const int bias = p.bias ? *p.bias : 0;
 #pragma unroll
     for (int m = 0; m < M; ++m) {
         const int i = dt * DM_TILE + grp * M + m;
@@ -313,10 +319,10 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
             if (!IN16) {
                 const uint32_t L = A[m][j] - (H[m][j] << 8);
                 int4 v;
-                v.x = (int)((L & 0xFFFFu) + ((C1[m][j] & 0xFFFFu) << 8));
-                v.y = (int)((H[m][j] & 0xFFFFu) + ((C2[m][j] & 0xFFFFu) << 8));
-                v.z = (int)((L >> 16) + ((C1[m][j] >> 16) << 8));
-                v.w = (int)((H[m][j] >> 16) + ((C2[m][j] >> 16) << 8));
+                v.x = bias + (int)((L & 0xFFFFu) + ((C1[m][j] & 0xFFFFu) << 8));
+                v.y = bias + (int)((H[m][j] & 0xFFFFu) + ((C2[m][j] & 0xFFFFu) << 8));
+                v.z = bias + (int)((L >> 16) + ((C1[m][j] >> 16) << 8));
+                v.w = bias + (int)((H[m][j] >> 16) + ((C2[m][j] >> 16) << 8));
                 if (p.accumulate) {
                     const int4 o = *reinterpret_cast<const int4*>(row + t);
                     v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w;
@@ -358,6 +364,7 @@ int launch(const aak_dedisp_args* a, cudaStream_t st) {
     const int cend = a->chan_end > 0 ? a->chan_end : a->nchans;
     if (a->chan_begin % CB || (cend % CB && cend != a->nchans) || a->chan_begin >= cend) return (int)cudaErrorInvalidValue;
     p.stage_begin = a->chan_begin / CB; p.stage_end = (cend + CB - 1) / CB; p.accumulate = a->accumulate;
+    p.mode_cnt = a->mode_cnt; p.mode_cap = a->mode_cap; p.mode_dense = a->mode_dense; p.bias = a->bias;
     p.window_bytes = a->window_bytes; p.spill_stages = a->spill_stages; p.one = 1u;
     p.nring = a->ring_stages;
     if (p.nring < 2 || p.nring > MAX_RING) return (int)cudaErrorInvalidValue;

@@ -11,7 +11,9 @@ namespace {
  * DESIGN.md reading C4: binning is a SUM held in uint16). One thread turns 16 input bytes into 16/b outputs. */
 template <int B>
 __global__ void __launch_bounds__(256)
-k_bin_time(const uint8_t* __restrict__ x, size_t x_pitch, uint16_t* __restrict__ xb, size_t xb_pitch, long long ngroups) {
+k_bin_time(const uint8_t* __restrict__ x, size_t x_pitch, uint16_t* __restrict__ xb, size_t xb_pitch, long long ngroups,
+           const unsigned* __restrict__ only_if_cnt, unsigned only_if_above) {
+    if (only_if_cnt && *only_if_cnt <= only_if_above) return;      /* the offset-uint8 route handles this chunk */
     const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= ngroups) return;
     const int c = blockIdx.y;
@@ -46,7 +48,9 @@ k_bin_time(const uint8_t* __restrict__ x, size_t x_pitch, uint16_t* __restrict__
 /* ---- K1b: out[c][j] = in[c][j + shift] (shift = 1, 2 or 3 bytes): the sample-shifted copies K2's TMA loads need
  * (TMA wants 16-byte aligned global coordinates, so a window at an odd sample offset is read from a shifted copy). */
 __global__ void __launch_bounds__(256)
-k_shift_copy(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, size_t pitch, long long ngroups, int shift) {
+k_shift_copy(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, size_t pitch, long long ngroups, int shift,
+             const unsigned* __restrict__ only_if_cnt, unsigned only_if_above) {
+    if (only_if_cnt && *only_if_cnt <= only_if_above) return;
     const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= ngroups) return;
     const uint8_t* src = in + (size_t)blockIdx.y * pitch + (size_t)g * 16;
@@ -123,6 +127,94 @@ k_corner_turn(const uint8_t* __restrict__ in, size_t in_stride, uint8_t* __restr
     }
 }
 
+/* ---- Offset-uint8 form of a binned input (ranges with bin 2 and 4). A binned sample x_b <= 255*b needs 9-10 bits, and as
+ * uint16 it costs K2 two shared-memory bytes per add - the crossbar is what limits K2. Radio data are noise around a
+ * per-channel mean, so x_b - off_c (off_c = the channel's mean binned value - 128) fits a byte almost always:
+ *     x_b[c][t] = lo[c][t] + off_c + r[c][t],   lo = clamp(x_b - off_c, 0, 255),   r = 0 except for rare outliers.
+ * K2 then runs its 1-byte path on lo (half the shared-memory traffic), adds sum_c off_c to every output, and the few
+ * (c, t, r != 0) EXCEPTIONS are scattered into D exactly by k_scatter_exceptions. Nothing is approximated: if a chunk has
+ * too many exceptions (counter above `cap`), the uint16 kernels run instead (every kernel of both routes tests the same
+ * counter and returns at once when it is not its turn). */
+__global__ void __launch_bounds__(256)
+k_chan_offsets(const uint8_t* __restrict__ x, size_t pitch, long long len, int32_t* __restrict__ off2, int32_t* __restrict__ off4,
+               int32_t* __restrict__ bias2, int32_t* __restrict__ bias4) {
+    __shared__ unsigned long long red[8];
+    const uint8_t* row = x + (size_t)blockIdx.x * pitch;
+    unsigned long long s = 0;
+    const long long nvec = len >> 4;
+    for (long long q = threadIdx.x; q < nvec; q += 256) {
+        const uint4 v = *reinterpret_cast<const uint4*>(row + q * 16);
+        s += __dp4a(v.x, 0x01010101u, 0u) + __dp4a(v.y, 0x01010101u, 0u) + __dp4a(v.z, 0x01010101u, 0u) + __dp4a(v.w, 0x01010101u, 0u);
+    }
+    for (long long t = (nvec << 4) + threadIdx.x; t < len; t += 256) s += row[t];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned long long tot = 0;
+        for (int w = 0; w < 8; ++w) tot += red[w];
+        const long long n = len > 0 ? len : 1;
+        /* any offset is CORRECT; this one centres the channel's noise on 128 */
+        if (off2) { long long o = (long long)((2 * tot + n / 2) / n) - 128; o = o < 0 ? 0 : (o > 255 ? 255 : o); off2[blockIdx.x] = (int32_t)o; atomicAdd(bias2, (int32_t)o); }
+        if (off4) { long long o = (long long)((4 * tot + n / 2) / n) - 128; o = o < 0 ? 0 : (o > 765 ? 765 : o); off4[blockIdx.x] = (int32_t)o; atomicAdd(bias4, (int32_t)o); }
+    }
+}
+
+template <int B>
+__global__ void __launch_bounds__(256)
+k_bin_offset(const uint8_t* __restrict__ x, size_t x_pitch, uint8_t* __restrict__ lo, size_t lo_pitch, const int32_t* __restrict__ off,
+             long long ngroups, long long nbinned, int chan0, uint2* __restrict__ exc, unsigned* __restrict__ exc_cnt, unsigned cap) {
+    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= ngroups) return;
+    const int c = blockIdx.y;
+    const int oc = off[c];
+    const uint4 v = *reinterpret_cast<const uint4*>(x + (size_t)c * x_pitch + (size_t)g * 16);
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+    uint32_t packed[2] = {0u, 0u};
+#pragma unroll
+    for (int k = 0; k < 16 / B; ++k) {
+        int s = 0;
+#pragma unroll
+        for (int j = 0; j < B; ++j) {
+            const int byte = k * B + j;
+            s += (int)((w[byte >> 2] >> (8 * (byte & 3))) & 0xFFu);
+        }
+        const int y = s - oc;
+        const int l = y < 0 ? 0 : (y > 255 ? 255 : y);
+        packed[k >> 2] |= (uint32_t)l << (8 * (k & 3));
+        const long long t = g * (16 / B) + k;
+        if (y != l && t < nbinned) {                                   /* rare: one atomic per exception */
+            const unsigned idx = atomicAdd(exc_cnt, 1u);
+            if (idx < cap) exc[idx] = make_uint2((uint32_t)(chan0 + c) | ((uint32_t)(y - l + 1024) << 16), (uint32_t)t);
+        }
+    }
+    uint8_t* dst = lo + (size_t)c * lo_pitch + (size_t)g * (16 / B);
+    if (B == 2) *reinterpret_cast<uint2*>(dst) = make_uint2(packed[0], packed[1]);
+    else *reinterpret_cast<uint32_t*>(dst) = packed[0];
+}
+
+/* D[i][t - delay(c, i)] += r for every exception (c, t, r) and every DM trial i of one range. The delay is reading C2
+ * evaluated in IEEE double with explicit round-to-nearest operations, the same operation order as the host tables. */
+__global__ void __launch_bounds__(256)
+k_scatter_exceptions(const uint2* __restrict__ exc, const unsigned* __restrict__ exc_cnt, unsigned cap, const double* __restrict__ k,
+                     double dm_low, double dm_step, int ndms, int bin, long long nt, int32_t* __restrict__ D, long long pitch) {
+    const unsigned n = *exc_cnt;
+    if (n > cap) return;                                               /* dense chunk: the uint16 route produced D */
+    const unsigned long long total = (unsigned long long)n * (unsigned)ndms;
+    for (unsigned long long q = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (unsigned long long)gridDim.x * blockDim.x) {
+        const unsigned e = (unsigned)(q / (unsigned)ndms);
+        const int i = (int)(q - (unsigned long long)e * (unsigned)ndms);
+        const uint2 rec = exc[e];
+        const int c = (int)(rec.x & 0xFFFFu);
+        const int r = (int)(rec.x >> 16) - 1024;
+        const double dm = __dadd_rn(dm_low, __dmul_rn((double)i, dm_step));
+        const long long delay = llround(__ddiv_rn(__dmul_rn(k[c], dm), (double)bin));
+        const long long t = (long long)rec.y - delay;
+        if (t >= 0 && t < nt) atomicAdd(D + (size_t)i * (size_t)pitch + (size_t)t, r);
+    }
+}
+
 /* ---- K5: sum_t D[i][t] and sum_t t*D[i][t] per row, int64 (all-rows checksum against the prefix-sum identity) */
 __global__ void __launch_bounds__(256)
 k_row_moments(const int32_t* __restrict__ D, long long pitch, long long nt, long long* __restrict__ sum_d,
@@ -179,25 +271,25 @@ k_peak_iadd(int mode, int iters, uint32_t* __restrict__ sink, unsigned long long
 }  // namespace
 
 extern "C" int aak_bin_time(const uint8_t* x, size_t x_pitch, uint16_t* xb, size_t xb_pitch_elems, int32_t nchans,
-                            int64_t nbinned, int32_t bin, void* stream) {
+                            int64_t nbinned, int32_t bin, const unsigned* only_if_cnt, unsigned only_if_above, void* stream) {
     cudaStream_t st = (cudaStream_t)stream;
     const long long ngroups = (nbinned * bin + 15) / 16;
     dim3 grid((unsigned)((ngroups + 255) / 256), (unsigned)nchans);
     switch (bin) {
-        case 2: k_bin_time<2><<<grid, 256, 0, st>>>(x, x_pitch, xb, xb_pitch_elems, ngroups); break;
-        case 4: k_bin_time<4><<<grid, 256, 0, st>>>(x, x_pitch, xb, xb_pitch_elems, ngroups); break;
-        case 8: k_bin_time<8><<<grid, 256, 0, st>>>(x, x_pitch, xb, xb_pitch_elems, ngroups); break;
+        case 2: k_bin_time<2><<<grid, 256, 0, st>>>(x, x_pitch, xb, xb_pitch_elems, ngroups, only_if_cnt, only_if_above); break;
+        case 4: k_bin_time<4><<<grid, 256, 0, st>>>(x, x_pitch, xb, xb_pitch_elems, ngroups, only_if_cnt, only_if_above); break;
+        case 8: k_bin_time<8><<<grid, 256, 0, st>>>(x, x_pitch, xb, xb_pitch_elems, ngroups, only_if_cnt, only_if_above); break;
         default: return (int)cudaErrorInvalidValue;
     }
     return (int)cudaGetLastError();
 }
 
 extern "C" int aak_shift_copy(const uint8_t* in, uint8_t* out, size_t pitch, size_t row_bytes, int32_t nrows, int32_t shift_bytes,
-                              void* stream) {
+                              const unsigned* only_if_cnt, unsigned only_if_above, void* stream) {
     if (shift_bytes < 1 || shift_bytes > 3 || (row_bytes & 15) || (pitch & 15)) return (int)cudaErrorInvalidValue;
     const long long ngroups = (long long)(row_bytes / 16);
     dim3 grid((unsigned)((ngroups + 255) / 256), (unsigned)nrows);
-    k_shift_copy<<<grid, 256, 0, (cudaStream_t)stream>>>(in, out, pitch, ngroups, shift_bytes);
+    k_shift_copy<<<grid, 256, 0, (cudaStream_t)stream>>>(in, out, pitch, ngroups, shift_bytes, only_if_cnt, only_if_above);
     return (int)cudaGetLastError();
 }
 
@@ -230,5 +322,29 @@ extern "C" int aak_corner_turn(const uint8_t* in, size_t in_stride, uint8_t* out
     if (nsamp <= 0 || nchans <= 0) return 0;
     dim3 grid((unsigned)((nsamp + CT_TILE - 1) / CT_TILE), (unsigned)((nchans + CT_TILE - 1) / CT_TILE));
     k_corner_turn<<<grid, 256, 0, (cudaStream_t)stream>>>(in, in_stride, out, out_pitch, nchans, nsamp);
+    return (int)cudaGetLastError();
+}
+
+extern "C" int aak_chan_offsets(const uint8_t* x, size_t pitch, int64_t len, int32_t nrows, int32_t* off2, int32_t* off4,
+                                int32_t* bias2, int32_t* bias4, void* stream) {
+    if (nrows <= 0) return 0;
+    k_chan_offsets<<<(unsigned)nrows, 256, 0, (cudaStream_t)stream>>>(x, pitch, len, off2, off4, bias2, bias4);
+    return (int)cudaGetLastError();
+}
+
+extern "C" int aak_bin_offset(const uint8_t* x, size_t x_pitch, uint8_t* lo, size_t lo_pitch, const int32_t* off, int32_t nrows,
+                              int32_t chan0, int64_t nbinned, int32_t bin, uint2* exc, unsigned* exc_cnt, unsigned cap, void* stream) {
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long ngroups = (nbinned * bin + 15) / 16;
+    dim3 grid((unsigned)((ngroups + 255) / 256), (unsigned)nrows);
+    if (bin == 2) k_bin_offset<2><<<grid, 256, 0, st>>>(x, x_pitch, lo, lo_pitch, off, ngroups, nbinned, chan0, exc, exc_cnt, cap);
+    else if (bin == 4) k_bin_offset<4><<<grid, 256, 0, st>>>(x, x_pitch, lo, lo_pitch, off, ngroups, nbinned, chan0, exc, exc_cnt, cap);
+    else return (int)cudaErrorInvalidValue;
+    return (int)cudaGetLastError();
+}
+
+extern "C" int aak_scatter_exceptions(const uint2* exc, const unsigned* exc_cnt, unsigned cap, const double* k, double dm_low,
+                                      double dm_step, int32_t ndms, int32_t bin, int64_t nt, int32_t* D, int64_t pitch, void* stream) {
+    k_scatter_exceptions<<<148 * 4, 256, 0, (cudaStream_t)stream>>>(exc, exc_cnt, cap, k, dm_low, dm_step, ndms, bin, nt, D, pitch);
     return (int)cudaGetLastError();
 }

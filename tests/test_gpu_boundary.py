@@ -152,3 +152,36 @@ def test_row_statistics_fallback_routes_match_the_oracle(kind):
         compare_candidates(gpu.candidates(allow_overflow=True), np.concatenate(exp), w.threshold)
     finally:
         gpu.close()
+
+
+@pytest.mark.parametrize("kind", ["gaussian_sparse", "uniform_dense", "mixed_groups"])
+def test_offset_uint8_route_and_its_uint16_fallback_are_bit_exact(kind):
+    """Binned ranges with bin 2 / 4 run K2 on bytes lo = clamp(x_b - off_c, 0, 255) plus an exactly scattered exception
+    list; a channel group with too many exceptions takes the uint16 route instead (each kernel of both routes tests the
+    same device counter). Inputs: Gaussian noise (few exceptions), uniform random bytes (about half the binned samples are
+    exceptions: dense route), and channels 0..255 Gaussian / the rest uniform with >= 256 channels so that the channel
+    groups of the pipelined copy choose DIFFERENT routes for the same chunk. Every row must equal the oracle's."""
+    rs = np.random.default_rng(2024)
+    C, N = (320, 12_000) if kind == "mixed_groups" else (24, 40_000)
+    gauss = np.clip(np.floor(127.0 + 16.0 * rs.standard_normal((C, N)) + 0.5), 0, 255).astype(np.uint8)
+    unif = rs.integers(0, 256, size=(C, N), dtype=np.uint8)
+    if kind == "gaussian_sparse":
+        x = gauss
+    elif kind == "uniform_dense":
+        x = unif
+    else:
+        x = np.where((np.arange(C) < 256)[:, None], gauss, unif).astype(np.uint8)
+    nd = 2100 if kind != "mixed_groups" else 600            # many trials: a low exception limit (1e8 / ndms per group)
+    w = Workload(kind, C, 1500.0, -0.5, 256e-6, N, ((0.0, 0.01, nd, 2), (30.0, 0.02, nd, 4)), (1, 2, 4), 6.0, seed=1, npulses=0,
+                 pulse_dm=(0.0, 0.0), pulse_width_max=1)
+    gpu, orc = GpuRun(w, x), OracleRun(w, x)
+    try:
+        assert "offset-uint8 route" in gpu.aa.aa_strategy_describe(gpu.h)
+        gpu.dedisperse()
+        chunk = gpu.chunks[0]
+        for r, rng in enumerate(w.ranges):
+            for (i0, i1) in ((0, 3), (nd // 2, nd // 2 + 3), (nd - 3, nd)):
+                check_band(gpu, orc, chunk, r, i0, i1, after_sps=False)
+        gpu.sps()
+    finally:
+        gpu.close()
