@@ -7,6 +7,8 @@
 
 namespace {
 
+constexpr int K1_GROUPS_PER_THREAD = 8;   /* 16-byte groups per thread of the binning / shifted-copy kernels */
+
 /* ---- K1: x_b[c][t'] = sum_{j<b} x[c][b*t'+j] (north_star "DM ranges that decimate in time by 1/2/4/8";
  * DESIGN.md reading C4: binning is a SUM held in uint16). One thread turns 16 input bytes into 16/b outputs. */
 template <int B>
@@ -14,9 +16,11 @@ __global__ void __launch_bounds__(256)
 k_bin_time(const uint8_t* __restrict__ x, size_t x_pitch, uint16_t* __restrict__ xb, size_t xb_pitch, long long ngroups,
            const unsigned* __restrict__ only_if_cnt, unsigned only_if_above) {
     if (only_if_cnt && *only_if_cnt <= only_if_above) return;      /* the offset-uint8 route handles this chunk */
-    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= ngroups) return;
     const int c = blockIdx.y;
+#pragma unroll 1
+    for (int it = 0; it < K1_GROUPS_PER_THREAD; ++it) {            /* few, fat CTAs: a skipped launch costs microseconds */
+    const long long g = ((long long)blockIdx.x * K1_GROUPS_PER_THREAD + it) * blockDim.x + threadIdx.x;
+    if (g >= ngroups) return;
     const uint4 v = *reinterpret_cast<const uint4*>(x + (size_t)c * x_pitch + (size_t)g * 16);
     const uint32_t w[4] = {v.x, v.y, v.z, v.w};
     uint16_t o[16 / B];
@@ -43,6 +47,7 @@ k_bin_time(const uint8_t* __restrict__ x, size_t x_pitch, uint16_t* __restrict__
     } else {
         *reinterpret_cast<uint32_t*>(dst) = o[0] | ((uint32_t)o[1] << 16);
     }
+    }
 }
 
 /* ---- K1b: out[c][j] = in[c][j + shift] (shift = 1, 2 or 3 bytes): the sample-shifted copies K2's TMA loads need
@@ -51,7 +56,9 @@ __global__ void __launch_bounds__(256)
 k_shift_copy(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, size_t pitch, long long ngroups, int shift,
              const unsigned* __restrict__ only_if_cnt, unsigned only_if_above) {
     if (only_if_cnt && *only_if_cnt <= only_if_above) return;
-    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+#pragma unroll 1
+    for (int it = 0; it < K1_GROUPS_PER_THREAD; ++it) {
+    const long long g = ((long long)blockIdx.x * K1_GROUPS_PER_THREAD + it) * blockDim.x + threadIdx.x;
     if (g >= ngroups) return;
     const uint8_t* src = in + (size_t)blockIdx.y * pitch + (size_t)g * 16;
     const uint4 a = *reinterpret_cast<const uint4*>(src);
@@ -63,6 +70,7 @@ k_shift_copy(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, size_t p
     o.z = __funnelshift_r(a.z, a.w, bs);
     o.w = __funnelshift_r(a.w, nx, bs);
     *reinterpret_cast<uint4*>(out + (size_t)blockIdx.y * pitch + (size_t)g * 16) = o;
+    }
 }
 
 /* ---- K1a: all four sample-shifted uint8 copies in one pass (reads the chunk once, writes 4 x): copy k at out + k*copy_stride */
@@ -274,7 +282,7 @@ extern "C" int aak_bin_time(const uint8_t* x, size_t x_pitch, uint16_t* xb, size
                             int64_t nbinned, int32_t bin, const unsigned* only_if_cnt, unsigned only_if_above, void* stream) {
     cudaStream_t st = (cudaStream_t)stream;
     const long long ngroups = (nbinned * bin + 15) / 16;
-    dim3 grid((unsigned)((ngroups + 255) / 256), (unsigned)nchans);
+    dim3 grid((unsigned)((ngroups + 256 * K1_GROUPS_PER_THREAD - 1) / (256 * K1_GROUPS_PER_THREAD)), (unsigned)nchans);
     switch (bin) {
         case 2: k_bin_time<2><<<grid, 256, 0, st>>>(x, x_pitch, xb, xb_pitch_elems, ngroups, only_if_cnt, only_if_above); break;
         case 4: k_bin_time<4><<<grid, 256, 0, st>>>(x, x_pitch, xb, xb_pitch_elems, ngroups, only_if_cnt, only_if_above); break;
@@ -288,7 +296,7 @@ extern "C" int aak_shift_copy(const uint8_t* in, uint8_t* out, size_t pitch, siz
                               const unsigned* only_if_cnt, unsigned only_if_above, void* stream) {
     if (shift_bytes < 1 || shift_bytes > 3 || (row_bytes & 15) || (pitch & 15)) return (int)cudaErrorInvalidValue;
     const long long ngroups = (long long)(row_bytes / 16);
-    dim3 grid((unsigned)((ngroups + 255) / 256), (unsigned)nrows);
+    dim3 grid((unsigned)((ngroups + 256 * K1_GROUPS_PER_THREAD - 1) / (256 * K1_GROUPS_PER_THREAD)), (unsigned)nrows);
     k_shift_copy<<<grid, 256, 0, (cudaStream_t)stream>>>(in, out, pitch, ngroups, shift_bytes, only_if_cnt, only_if_above);
     return (int)cudaGetLastError();
 }
