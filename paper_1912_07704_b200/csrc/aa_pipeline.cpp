@@ -53,6 +53,12 @@ aa_status enqueue_h2d(Strategy& s, int64_t j, int b, const uint8_t* host_input, 
  * largest channel block of K2). */
 struct ChannelGroups { int n; int32_t c[kMaxGroups + 1]; };
 
+/* Exception budget of a channel group: the chunk's budget in proportion to the group's channels. */
+static unsigned group_limit(const Strategy& s, int bin, int32_t c0, int32_t c1) {
+    const uint64_t v = (uint64_t)s.exc_limit[bin] * (uint64_t)(c1 - c0) / (uint64_t)s.plan.nchans;
+    return (unsigned)std::max<uint64_t>(1, std::min<uint64_t>(v, kExcCap));
+}
+
 /* K1 for channel rows [c0, c1) (= channel group g) of the chunk in raw buffer b: sample-shifted uint8 copies, the
  * offset-uint8 form of the bin 2 / 4 inputs (per-channel offsets, byte copies, exception list), and the uint16 binned
  * inputs with their shifted copies (for bin 2 / 4 only when the group has too many exceptions). */
@@ -78,8 +84,8 @@ aa_status enqueue_prep(Strategy& s, const Chunk& c, int b, int32_t c0, int32_t c
         if (!s.d_xb[bin]) continue;
         const size_t pitch_bytes = s.xb_pitch[bin] * 2;
         uint16_t* xb = s.d_xb[bin] + (size_t)c0 * s.xb_pitch[bin];
-        AA_LAUNCH(aak_bin_time(raw, s.in_pitch, xb, s.xb_pitch[bin], n, nb, bin, cnt, s.exc_limit[bin], s.compute), "time binning");
-        AA_LAUNCH(aak_shift_copy((const uint8_t*)xb, (uint8_t*)xb + s.xb_stride[bin], pitch_bytes, pitch_bytes, n, 2, cnt, s.exc_limit[bin], s.compute), "shift copy (uint16)");
+        AA_LAUNCH(aak_bin_time(raw, s.in_pitch, xb, s.xb_pitch[bin], n, nb, bin, cnt, cnt ? group_limit(s, bin, c0, c1) : 0u, s.compute), "time binning");
+        AA_LAUNCH(aak_shift_copy((const uint8_t*)xb, (uint8_t*)xb + s.xb_stride[bin], pitch_bytes, pitch_bytes, n, 2, cnt, cnt ? group_limit(s, bin, c0, c1) : 0u, s.compute), "shift copy (uint16)");
     }
     return AA_OK;
 }
@@ -100,12 +106,12 @@ aa_status enqueue_k2(Strategy& s, const Chunk& c, int32_t c0, int32_t c1, bool a
             a.chan_block = p.chan_block; a.window_bytes = p.window_bytes; a.spill_stages = p.spill_stages; a.in16 = p.in16;
             a.variant = p.variant; a.dms_per_warp = p.dms_per_warp; a.ring_stages = p.ring_stages;
             a.mode_cnt = rg.has_lo ? s.d_exc_cnt[bin] + g : nullptr;
-            a.mode_cap = s.exc_limit[bin]; a.mode_dense = route;
+            a.mode_cap = rg.has_lo ? group_limit(s, bin, c0, c1) : 0u; a.mode_dense = route;
             a.bias = route == 0 ? (const int32_t*)(s.d_exc_cnt[bin] + kMaxGroups + g) : nullptr;
             AA_LAUNCH(aak_dedisperse(&a, s.compute), "dedispersion");
         }
         if (rg.has_lo)
-            AA_LAUNCH(aak_scatter_exceptions(s.d_exc[bin] + (size_t)g * kExcCap, s.d_exc_cnt[bin] + g, s.exc_limit[bin], s.d_k, rg.r.dm_low, rg.r.dm_step,
+            AA_LAUNCH(aak_scatter_exceptions(s.d_exc[bin] + (size_t)g * kExcCap, s.d_exc_cnt[bin] + g, group_limit(s, bin, c0, c1), s.d_k, rg.r.dm_low, rg.r.dm_step,
                                              rg.r.ndms, bin, a.nt, rg.d_D, rg.pitch, s.compute), "exception scatter");
     }
     return AA_OK;

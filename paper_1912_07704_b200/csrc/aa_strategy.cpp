@@ -95,8 +95,9 @@ static void carve(Strategy& s, int64_t L, bool two_raw) {
         s.d_off[bn] = used ? (int32_t*)a.take((size_t)s.plan.nchans * 4) : nullptr;
         s.d_exc[bn] = used ? (uint2*)a.take((size_t)kMaxGroups * kExcCap * sizeof(uint2)) : nullptr;
         s.d_exc_cnt[bn] = used ? (unsigned*)a.take(2 * kMaxGroups * 4) : nullptr;
-        /* the scatter costs one atomic per (exception, trial): beyond ~1e8 of them per group the uint16 route is cheaper */
-        s.exc_limit[bn] = used ? (unsigned)std::min<int64_t>((int64_t)kExcCap, std::max<int64_t>(1, 100000000 / std::max<int64_t>(1, nd))) : 0;
+        /* the scatter costs one atomic per (exception, trial), measured 2.7e10 atomics/s: beyond ~1e8 of them per chunk the
+         * uint16 route is cheaper (a channel group gets the share of its channels) */
+        s.exc_limit[bn] = used ? (unsigned)std::min<int64_t>((int64_t)kMaxGroups * kExcCap, std::max<int64_t>(1, 100000000 / std::max<int64_t>(1, nd))) : 0;
         if (used && !s.d_k_needed) s.d_k_needed = true;
     }
     s.d_k = s.d_k_needed ? (double*)a.take((size_t)s.plan.nchans * 8) : nullptr;
@@ -504,7 +505,7 @@ extern "C" size_t aa_strategy_describe(const aa_strategy* h, char* buf, size_t b
                  aak_dedisperse_smem_bytes(rg.chan_block, rg.window_bytes, rg.in16, rg.ring_stages));
         o += line;
         if (rg.has_lo) {
-            snprintf(line, sizeof line, "         offset-uint8 route: chan_block=%d window=%dB stages=%d ring=%d exception limit %u per channel group\n",
+            snprintf(line, sizeof line, "         offset-uint8 route: chan_block=%d window=%dB stages=%d ring=%d exception limit %u per chunk\n",
                      rg.lo.chan_block, rg.lo.window_bytes, rg.lo.nstages, rg.lo.ring_stages, s.exc_limit[rg.r.bin]);
             o += line;
         }
