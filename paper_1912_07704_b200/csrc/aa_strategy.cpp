@@ -155,12 +155,15 @@ static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16,
     const int64_t wsamp = kTTile + omax + 16 / p.esz;
     p.window_bytes = (int32_t)round_up((size_t)(wsamp * p.esz), 256);
     if (p.window_bytes > 65536) { set_error("aa_strategy_setup: range %d needs a %d-byte channel window per DM tile (> 65536): DM step too coarse for this band", rg.index, p.window_bytes); return false; }
+    /* the largest channel block that still leaves a 2-deep ring, then the deepest ring (<= 4) that fits: measured on the
+     * low-frequency config (wide windows), 8 channels x 2 stages beats 4 x 4 by 6 %; ring depth alone moves < 1 % */
     p.chan_block = 0;
-    p.ring_stages = 3;
+    p.ring_stages = 2;
     for (int cb = 8; cb >= 2; cb /= 2)
-        if (aak_dedisperse_smem_bytes(cb, p.window_bytes, p.in16, p.ring_stages) <= 227 * 1024) { p.chan_block = cb; break; }
+        if (aak_dedisperse_smem_bytes(cb, p.window_bytes, p.in16, 2) <= 227 * 1024) { p.chan_block = cb; break; }
     if (!p.chan_block) { set_error("aa_strategy_setup: range %d: channel window of %d bytes does not fit shared memory", rg.index, p.window_bytes); return false; }
-    if (aak_dedisperse_smem_bytes(p.chan_block, p.window_bytes, p.in16, 4) <= 227 * 1024) p.ring_stages = 4;
+    for (int n = 3; n <= 4; ++n)
+        if (aak_dedisperse_smem_bytes(p.chan_block, p.window_bytes, p.in16, n) <= 227 * 1024) p.ring_stages = n;
     /* measured on B200 (profiles/): binned ranges are shared-memory bound and gain 13 % from 4 trials per warp with
      * register reuse; the uint8 ranges are issue bound and lose 7 % to the extra branches, so they keep 2 trials per warp
      * with the odd-byte adds on the FMA pipe */
@@ -169,6 +172,14 @@ static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16,
 #ifdef AA_TUNING
     if (const char* ev = getenv(p.in16 ? "AA_K2_M16" : "AA_K2_M8")) p.dms_per_warp = atoi(ev) == 4 ? 4 : 2;
     if (const char* ev = getenv("AA_K2_VARIANT")) p.variant = atoi(ev);
+    if (const char* ev = getenv("AA_K2_CB")) {
+        const int cb = atoi(ev);
+        if ((cb == 2 || cb == 4 || cb == 8) && aak_dedisperse_smem_bytes(cb, p.window_bytes, p.in16, 2) <= 227 * 1024) {
+            p.chan_block = cb;
+            p.ring_stages = 2;
+            for (int n = 3; n <= 4; ++n) if (aak_dedisperse_smem_bytes(cb, p.window_bytes, p.in16, n) <= 227 * 1024) p.ring_stages = n;
+        }
+    }
     if (const char* ev = getenv("AA_K2_RING")) {
         const int n = atoi(ev);
         if (n >= 2 && n <= 8 && aak_dedisperse_smem_bytes(p.chan_block, p.window_bytes, p.in16, n) <= 227 * 1024) p.ring_stages = n;
