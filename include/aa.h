@@ -185,6 +185,12 @@ aa_status aa_run_dedispersion_device(aa_strategy* s, const uint8_t* device_chunk
  * Returns AA_STATUS_CHUNK_DONE or AA_STATUS_FINISHED; AA_ERR_ORDER if no dedispersed chunk is pending. */
 aa_status aa_run_sps(aa_strategy* s);
 
+/* aa_run_pipeline: the whole chunk loop in one call (PAPER.md:47 step 7 "run the pipeline"): aa_run_dedispersion then
+ * aa_run_sps for every remaining chunk of this strategy's shard. Returns AA_STATUS_FINISHED, or the first error. The
+ * per-iteration status codes remain available to callers that drive the loop themselves; a test compares this C loop
+ * with the Python loop over the same calls (the front-end adds no appreciable run time). */
+aa_status aa_run_pipeline(aa_strategy* s, const uint8_t* host_input, size_t row_stride_bytes);
+
 /* aa_get_candidates: synchronises, copies the device records to library-owned HOST memory, and returns ALL candidates
  * of the chunks processed so far in canonical order (chunk, range, dm_index, sample). *out stays valid until the next
  * aa_run_*, aa_strategy_reset or aa_strategy_destroy. Returns AA_OK, or AA_ERR_CANDIDATE_OVERFLOW when more

@@ -19,7 +19,7 @@ __all__ = [
     "CANDIDATE_DTYPE", "lib_path", "load",
     "AA_LAYOUT_CHANNEL_MAJOR", "AA_LAYOUT_TIME_MAJOR", "aa_plan_create", "aa_plan_destroy", "aa_plan_set_input_layout", "aa_strategy_plan", "aa_strategy_setup", "aa_strategy_destroy", "aa_strategy_get_info",
     "aa_strategy_get_range_info", "aa_strategy_get_chunk", "aa_strategy_get_delay", "aa_strategy_describe",
-    "aa_strategy_reset", "aa_strategy_shard", "aa_run_dedispersion", "aa_run_dedispersion_device", "aa_run_sps", "aa_get_candidates",
+    "aa_strategy_reset", "aa_strategy_shard", "aa_run_dedispersion", "aa_run_dedispersion_device", "aa_run_sps", "aa_run_pipeline", "aa_get_candidates",
     "aa_get_dedispersed_row", "aa_get_row_stats", "aa_get_row_moments", "aa_get_dedispersed_device", "aa_synchronize",
     "aa_measure_int_add_peak", "aa_get_last_timings", "aa_get_launch_count", "aa_last_error", "aa_version",
     "Plan", "Strategy",
@@ -97,6 +97,7 @@ def load():
         "aa_run_dedispersion": (c_int32, [vp, vp, c_size_t]),
         "aa_run_dedispersion_device": (c_int32, [vp, vp, c_size_t]),
         "aa_run_sps": (c_int32, [vp]),
+        "aa_run_pipeline": (c_int32, [vp, vp, c_size_t]),
         "aa_get_candidates": (c_int32, [vp, POINTER(vp), POINTER(c_size_t)]),
         "aa_get_dedispersed_row": (c_int32, [vp, c_int32, c_int32, POINTER(vp), POINTER(c_size_t)]),
         "aa_get_row_stats": (c_int32, [vp, c_int32, c_int32, POINTER(c_double), POINTER(c_double), POINTER(c_int64), POINTER(c_int32)]),
@@ -240,6 +241,13 @@ def aa_run_dedispersion_device(strategy, device_chunk, row_stride_bytes=None) ->
 
 def aa_run_sps(strategy) -> int:
     return _check(load().aa_run_sps(strategy))
+
+
+def aa_run_pipeline(strategy, host_input, row_stride_bytes=None) -> int:
+    """The chunk loop inside the library (one call)."""
+    if row_stride_bytes is None:
+        row_stride_bytes = host_input.strides[0] if isinstance(host_input, np.ndarray) else host_input.stride(0)
+    return _check(load().aa_run_pipeline(strategy, _ptr(host_input), int(row_stride_bytes)))
 
 
 def aa_get_candidates(strategy, allow_overflow: bool = False) -> np.ndarray:

@@ -303,6 +303,17 @@ extern "C" aa_status aa_run_sps(aa_strategy* h) {
     return s.next_chunk >= (int64_t)s.chunks.size() ? AA_STATUS_FINISHED : AA_STATUS_CHUNK_DONE;
 }
 
+extern "C" aa_status aa_run_pipeline(aa_strategy* h, const uint8_t* host_input, size_t row_stride_bytes) {
+    aa_status st = check_ready(h, "aa_run_pipeline");
+    if (st != AA_OK) return st;
+    if (h->s.pending_sps && (st = aa_run_sps(h)) < 0) return st;
+    while (h->s.next_chunk < (int64_t)h->s.chunks.size()) {
+        if ((st = aa_run_dedispersion(h, host_input, row_stride_bytes)) < 0) return st;
+        if ((st = aa_run_sps(h)) < 0) return st;
+    }
+    return AA_STATUS_FINISHED;
+}
+
 extern "C" aa_status aa_get_candidates(aa_strategy* h, const aa_candidate** out, size_t* n) {
     aa_status st = check_ready(h, "aa_get_candidates");
     if (st != AA_OK) return st;

@@ -185,3 +185,45 @@ def test_offset_uint8_route_and_its_uint16_fallback_are_bit_exact(kind):
         gpu.sps()
     finally:
         gpu.close()
+
+
+def test_python_front_end_adds_no_appreciable_run_time():
+    """PAPER.md:67 (§4): the Python front-end "did not show an appreciable runtime impact". The chunk loop driven from Python
+    (two ctypes calls per chunk) against the same loop inside the library (aa_run_pipeline, one call): same candidates,
+    and the wall-clock difference stays within a few per cent of a run that takes tens of milliseconds."""
+    import time
+    import torch
+    import paper_1912_07704_b200 as aa
+    w = scaled(datagen.get_workload("mid"), nsamp=1 << 16, name="mid64k")
+    x, pinned = make_input(w, pinned=True)
+    g = GpuRun(w, x, chunk_len_hint=16384)
+    try:
+        assert g.info["nchunks"] >= 5
+
+        def python_loop():
+            aa.aa_strategy_reset(g.h)
+            return g.st.run(x)
+
+        def c_loop():
+            aa.aa_strategy_reset(g.h)
+            assert aa.aa_run_pipeline(g.h, x) == aa.AA_STATUS_FINISHED
+            return aa.aa_get_candidates(g.h)
+
+        def best(f, n=7):
+            ts = []
+            for _ in range(n):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                c = f()
+                torch.cuda.synchronize()
+                ts.append(time.perf_counter() - t0)
+            return min(ts), c
+
+        python_loop(); c_loop()
+        tp, cp = best(python_loop)
+        tc, cc = best(c_loop)
+        assert len(cp) == len(cc) > 0 and all(np.array_equal(cp[f], cc[f]) for f in cp.dtype.names)
+        print(f"python loop {tp * 1e3:.3f} ms, C loop {tc * 1e3:.3f} ms, difference {100 * (tp - tc) / tc:+.2f} %")
+        assert tp <= tc * 1.05 + 0.5e-3
+    finally:
+        g.close()
