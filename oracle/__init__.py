@@ -50,7 +50,7 @@ def _load():
     for f in (L.orc_boxcar_snr, L.orc_boxcar_snr_prefix):
         f.argtypes = [vp, i64, vp, i32, f64, f64, vp, vp]; f.restype = None
     L.orc_find_peaks.argtypes = [vp, i32, i64, f64, i32, i32, vp, vp, i64]; L.orc_find_peaks.restype = i64
-    L.orc_search_rows.argtypes = [vp, i64, i32, vp, f64, f64, i32, i32, i32, i64, vp, i32, f64, u64, i32, i32,
+    L.orc_search_rows.argtypes = [vp, i64, i32, vp, f64, f64, i32, i32, i32, i64, i64, vp, i32, f64, u64, i32, i32,
                                   vp, vp, vp, vp, vp, i64]
     L.orc_search_rows.restype = i64
     L.orc_range_max_delay_unbinned.argtypes = [vp, i32, f64, f64, i32, i32]; L.orc_range_max_delay_unbinned.restype = i64
@@ -135,12 +135,14 @@ def range_max_delay_unbinned(k, rng) -> int:
     return int(_load().orc_range_max_delay_unbinned(_p(k), len(k), rng[0], rng[1], rng[2], rng[3]))
 
 
-def chunk_geometry(k: np.ndarray, ranges, nsamp_total: int, chunk_len: int | None = None):
+def chunk_geometry(k: np.ndarray, ranges, nsamp_total: int, chunk_len: int | None = None, boxcar_extra: int = 0):
     """Reading C3: overlap S = max_r S_r rounded up to a multiple of B = max bin; chunk input
     length L (multiple of B, > S), n_out = L - S, chunk j starts at j*n_out; the last chunk takes the remaining
-    input rounded down to a multiple of B. Returns dict(B, S, L, n_out, chunks=[(start, L_j, n_out_j)])."""
+    input rounded down to a multiple of B. Returns dict(B, S, L, n_out, chunks=[(start, L_j, n_out_j)]).
+    boxcar_extra = E > 0 is reading C3x (boxcar-complete chunks): every row is dedispersed E binned samples beyond its
+    chunk's output span, so S_r = b_r * (delay(C-1, r, last) + E)."""
     B = max(r[3] for r in ranges)
-    S = max(range_max_delay_unbinned(k, r) for r in ranges)
+    S = max(range_max_delay_unbinned(k, r) + r[3] * boxcar_extra for r in ranges)
     S = -(-S // B) * B
     L = (nsamp_total // B) * B if chunk_len is None else chunk_len
     assert L % B == 0 and L > S
@@ -159,19 +161,20 @@ def chunk_geometry(k: np.ndarray, ranges, nsamp_total: int, chunk_len: int | Non
 
 
 def search_rows(xb: np.ndarray, k: np.ndarray, rng, range_index: int, T: int, widths, threshold: float,
-                chunk_start: int, i0: int, i1: int, want=("D", "stats"), cap: int = 1 << 20):
+                chunk_start: int, i0: int, i1: int, want=("D", "stats"), cap: int = 1 << 20, extra: int = 0):
     """Steps a4..a7 for rows [i0,i1) of one range on one binned chunk. Returns dict with 'cands' (structured array,
-    canonical order) and whichever of 'D','stats','S','w' were asked for."""
+    canonical order) and whichever of 'D','stats','S','w' were asked for. extra = E (reading C3x): rows are dedispersed for
+    T + E samples ('D' then has T + E columns), statistics / S / peaks stay on the first T."""
     assert xb.dtype == np.uint16 and xb.flags.c_contiguous
     w = np.ascontiguousarray(widths, dtype=np.int32)
     n = i1 - i0
-    D = np.empty((n, T), np.int64) if "D" in want else None
+    D = np.empty((n, T + extra), np.int64) if "D" in want else None
     st = np.empty((n, 2), np.float64) if "stats" in want else None
     S = np.empty((n, T), np.float64) if "S" in want else None
     W = np.empty((n, T), np.int32) if "w" in want else None
     c = np.zeros(cap, dtype=CAND_DTYPE)
     cnt = int(_load().orc_search_rows(_p(xb), xb.shape[1], xb.shape[0], _p(k), rng[0], rng[1], rng[2], rng[3],
-                                      range_index, T, _p(w), len(w), float(threshold), int(chunk_start), i0, i1,
+                                      range_index, T, int(extra), _p(w), len(w), float(threshold), int(chunk_start), i0, i1,
                                       _p(D), _p(st), _p(S), _p(W), _p(c), cap))
     assert cnt <= cap, "raise cap"
     out = dict(cands=c[:cnt].copy(), count=cnt)

@@ -239,27 +239,33 @@ typedef struct {
     uint64_t sample; float dm; float snr; uint32_t width; uint32_t range; uint32_t dm_index;
 } orc_candidate;
 
+/* `extra` = E (reading C3x, optional "boxcar-complete chunks"): each row is dedispersed for T + E samples, the
+ * statistics use the first T (the chunk's own output span), a boxcar starting at t < T may extend into the E extra samples
+ * (valid while t + w <= T + E), and S / peaks are defined on t in [0, T). extra = 0 is readings C3/C7 as they were. */
 int64_t orc_search_rows(const uint16_t* xb /* binned chunk [nchans][nbinned], from orc_bin */, int64_t nbinned, int32_t nchans,
                         const double* k, double dm_low, double dm_step, int32_t ndms, int32_t bin, int32_t range_index,
-                        int64_t T, const int32_t* widths, int32_t nwidths, double threshold, uint64_t chunk_start,
+                        int64_t T, int64_t extra, const int32_t* widths, int32_t nwidths, double threshold, uint64_t chunk_start,
                         int32_t i0, int32_t i1,
-                        int64_t* D_out /* [(i1-i0)][T] or NULL */, double* stats_out /* [(i1-i0)][2] or NULL */,
+                        int64_t* D_out /* [(i1-i0)][T+extra] or NULL */, double* stats_out /* [(i1-i0)][2] or NULL */,
                         double* S_out /* [(i1-i0)][T] or NULL */, int32_t* w_out /* [(i1-i0)][T] or NULL */,
                         orc_candidate* cands, int64_t cap) {
     const int32_t h0 = i0 > 0 ? i0 - 1 : i0, h1 = i1 < ndms ? i1 + 1 : i1;   /* halo rows for the 3x3 test */
     const int32_t nr = h1 - h0;
-    std::vector<int64_t> D((size_t)nr * (size_t)T);
-    orc_dedisperse(xb, nbinned, nchans, k, dm_low, dm_step, bin, h0, h1, T, D.data());
-    std::vector<double> S((size_t)nr * (size_t)T);
-    std::vector<int32_t> W((size_t)nr * (size_t)T);
+    const int64_t Tx = T + extra;
+    std::vector<int64_t> D((size_t)nr * (size_t)Tx);
+    orc_dedisperse(xb, nbinned, nchans, k, dm_low, dm_step, bin, h0, h1, Tx, D.data());
+    std::vector<double> S((size_t)nr * (size_t)T), Sx((size_t)Tx);
+    std::vector<int32_t> W((size_t)nr * (size_t)T), Wx((size_t)Tx);
     for (int32_t r = 0; r < nr; ++r) {
         double mu, sigma; int64_t info[4];
-        orc_row_stats(D.data() + (size_t)r * T, T, &mu, &sigma, info);
-        orc_boxcar_snr_prefix(D.data() + (size_t)r * T, T, widths, nwidths, mu, sigma, S.data() + (size_t)r * T, W.data() + (size_t)r * T);
+        orc_row_stats(D.data() + (size_t)r * Tx, T, &mu, &sigma, info);
+        orc_boxcar_snr_prefix(D.data() + (size_t)r * Tx, Tx, widths, nwidths, mu, sigma, Sx.data(), Wx.data());
+        memcpy(S.data() + (size_t)r * T, Sx.data(), sizeof(double) * (size_t)T);
+        memcpy(W.data() + (size_t)r * T, Wx.data(), sizeof(int32_t) * (size_t)T);
         const int32_t i = h0 + r;
         if (i >= i0 && i < i1) {
             if (stats_out) { stats_out[2 * (i - i0)] = mu; stats_out[2 * (i - i0) + 1] = sigma; }
-            if (D_out) memcpy(D_out + (size_t)(i - i0) * T, D.data() + (size_t)r * T, sizeof(int64_t) * (size_t)T);
+            if (D_out) memcpy(D_out + (size_t)(i - i0) * Tx, D.data() + (size_t)r * Tx, sizeof(int64_t) * (size_t)Tx);
             if (S_out) memcpy(S_out + (size_t)(i - i0) * T, S.data() + (size_t)r * T, sizeof(double) * (size_t)T);
             if (w_out) memcpy(w_out + (size_t)(i - i0) * T, W.data() + (size_t)r * T, sizeof(int32_t) * (size_t)T);
         }

@@ -334,3 +334,45 @@ def test_band_search_equals_full_search(tiny):
     band = oracle.search_rows(xb, k, w.ranges[0], 0, g["n_out"], w.widths, w.threshold, 0, 47, 54, want=())
     sel = full["cands"][(full["cands"]["dm_index"] >= 47) & (full["cands"]["dm_index"] < 54)]
     assert len(sel) > 0 and np.array_equal(sel, band["cands"])
+
+
+# ------------------------------------------------------------------------------------------------ reading C3x (boxcar-complete chunks)
+def test_boxcar_complete_chunks_equal_the_untruncated_definition(tiny):
+    """Reading C3x: with E = W_max - 1 extra samples per row, every boxcar that STARTS inside a chunk's output span is
+    complete. Pin (independent route): the S map of a chunk equals, position by position, the SNR of numpy boxcar sums
+    taken on a row dedispersed over the WHOLE observation, normalised with the chunk's own mu / sigma; and the geometry
+    obeys S_x = ceil_B(max_r b_r (delay_max_r + E)), chunks tiling the output axis without gap."""
+    w, x, k, g0 = tiny
+    widths = w.widths
+    E = max(widths) - 1
+    rng = w.ranges[0]
+    L = 2048
+    g = oracle.chunk_geometry(k, w.ranges, w.nsamp, chunk_len=L, boxcar_extra=E)
+    assert g["S"] == g0["S"] + E and g["n_out"] == L - g["S"]                     # tiny: bin 1, so S grows by exactly E
+    assert [c[0] for c in g["chunks"]] == [j * g["n_out"] for j in range(len(g["chunks"]))]
+    xb_all = oracle.bin_time(x, 0, w.nsamp, 1)
+    T_all = w.nsamp - g0["S"]
+    rows = (0, 50, 100)
+    D_all = {i: oracle.dedisperse(xb_all, k, rng, i, i + 1, T_all)[0] for i in rows}
+    for (start, Lj, n_out) in g["chunks"][:3]:
+        xb = oracle.bin_time(x, start, Lj, 1)
+        for i in rows:
+            res = oracle.search_rows(xb, k, rng, 0, n_out, widths, w.threshold, start, i, i + 1, want=("D", "stats", "S", "w"), extra=E)
+            assert res["D"].shape == (1, n_out + E)
+            assert np.array_equal(res["D"][0], D_all[i][start:start + n_out + E])  # D is chunk-invariant, extra samples included
+            mu, sg = res["stats"][0]
+            m0, s0, *_ = oracle.row_stats(D_all[i][start:start + n_out])           # statistics: the chunk's own span only
+            assert (mu, sg) == (m0, s0)
+            best = np.full(n_out, -np.inf)
+            bw = np.zeros(n_out, np.int32)
+            for wd in widths:                                                      # numpy route, no truncation at the chunk end
+                B = np.convolve(D_all[i].astype(np.float64), np.ones(wd), mode="valid")[start:start + n_out]
+                snr = (B - wd * mu) / (np.sqrt(wd) * sg)
+                upd = snr > best + 1e-9
+                best[upd] = snr[upd]
+                bw[upd] = wd
+            assert np.allclose(res["S"][0], best, rtol=1e-9, atol=1e-9)
+            assert np.array_equal(res["w"][0][best > 3.0], bw[best > 3.0])
+            # and without the extra samples the last W_max - 1 positions are truncated (the behaviour C3x removes)
+            old = oracle.search_rows(xb, k, rng, 0, n_out, widths, w.threshold, start, i, i + 1, want=("S",), extra=0)["S"][0]
+            assert np.array_equal(old[: n_out - E], res["S"][0][: n_out - E]) or np.allclose(old[: n_out - E], res["S"][0][: n_out - E])
