@@ -69,6 +69,7 @@ typedef struct {
     int64_t row_pitch;     /* int32 elements between consecutive DM rows of D_r on the device */
     int64_t max_delay;     /* delay(C-1, last DM) in binned samples */
     int32_t dm_tile, t_tile, chan_block, window;   /* dedispersion kernel tiling chosen for this range */
+    int32_t boxcar_extra;  /* E: samples dedispersed beyond nt per row (0 unless aa_plan_set_boxcar_overlap) */
 } aa_range_info;
 
 typedef struct {
@@ -111,6 +112,15 @@ void aa_plan_destroy(aa_plan* plan);
  * the staging buffers). Results are identical in both layouts. Errors: AA_ERR_INVALID_ARG naming `layout`. */
 typedef enum { AA_LAYOUT_CHANNEL_MAJOR = 0, AA_LAYOUT_TIME_MAJOR = 1 } aa_input_layout;
 aa_status aa_plan_set_input_layout(aa_plan* plan, int32_t layout);
+
+/* Boxcar-complete chunks (reading C3x; off by default). With the plain chunking a boxcar of width w that starts in
+ * the last w-1 samples of a chunk's output span is not evaluated (it would need samples of the next chunk), so a wide
+ * pulse straddling a chunk boundary is seen only by narrower boxcars. on != 0: every row is dedispersed
+ * E = max(boxcar_widths) - 1 binned samples beyond its chunk's output span (the overlap S grows to
+ * ceil_B(max_r bin_r (delay_max_r + E))), statistics still use the span itself, and every boxcar that STARTS inside the span
+ * is complete. Candidates are still reported for start samples inside the span only, so chunks do not duplicate them.
+ * Must be called before aa_strategy_setup binds the plan. */
+aa_status aa_plan_set_boxcar_overlap(aa_plan* plan, int32_t on);
 
 /* ------------------------------------------------------------------------------------------------ strategy
  * PAPER.md:47 steps 4-6 ("bind", "the API calculates the optimal strategy", "checks whether all modules are
@@ -198,8 +208,8 @@ aa_status aa_run_pipeline(aa_strategy* s, const uint8_t* host_input, size_t row_
  * count is in aa_last_error()). */
 aa_status aa_get_candidates(aa_strategy* s, const aa_candidate** out, size_t* n);
 
-/* Parity hooks: copy one row of the CURRENT chunk (the one last dedispersed / searched) to library-owned HOST memory.
- * Valid until the next call on this strategy. */
+/* Parity hooks: copy one row of the CURRENT chunk (the one last dedispersed / searched) to library-owned HOST memory:
+ * nt + boxcar_extra samples. Valid until the next call on this strategy. */
 aa_status aa_get_dedispersed_row(aa_strategy* s, int32_t range, int32_t dm_index, const int32_t** host_row, size_t* len);
 /* mu, sigma, n kept, clip iterations of a row, as computed by aa_run_sps for the current chunk. */
 aa_status aa_get_row_stats(aa_strategy* s, int32_t range, int32_t dm_index, double* mu, double* sigma,

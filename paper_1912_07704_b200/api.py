@@ -17,7 +17,7 @@ __all__ = [
     "AaError", "AA_OK", "AA_STATUS_CHUNK_DONE", "AA_STATUS_FINISHED", "AA_ERR_INVALID_ARG", "AA_ERR_NOT_READY",
     "AA_ERR_BUDGET_TOO_SMALL", "AA_ERR_CUDA", "AA_ERR_CANDIDATE_OVERFLOW", "AA_ERR_ORDER", "AA_ERR_INTERNAL",
     "CANDIDATE_DTYPE", "lib_path", "load",
-    "AA_LAYOUT_CHANNEL_MAJOR", "AA_LAYOUT_TIME_MAJOR", "aa_plan_create", "aa_plan_destroy", "aa_plan_set_input_layout", "aa_strategy_plan", "aa_strategy_setup", "aa_strategy_destroy", "aa_strategy_get_info",
+    "AA_LAYOUT_CHANNEL_MAJOR", "AA_LAYOUT_TIME_MAJOR", "aa_plan_create", "aa_plan_destroy", "aa_plan_set_input_layout", "aa_plan_set_boxcar_overlap", "aa_strategy_plan", "aa_strategy_setup", "aa_strategy_destroy", "aa_strategy_get_info",
     "aa_strategy_get_range_info", "aa_strategy_get_chunk", "aa_strategy_get_delay", "aa_strategy_describe",
     "aa_strategy_reset", "aa_strategy_shard", "aa_run_dedispersion", "aa_run_dedispersion_device", "aa_run_sps", "aa_run_pipeline", "aa_get_candidates",
     "aa_get_dedispersed_row", "aa_get_row_stats", "aa_get_row_moments", "aa_get_dedispersed_device", "aa_synchronize",
@@ -47,7 +47,8 @@ class _DmRange(ctypes.Structure):
 
 class _RangeInfo(ctypes.Structure):
     _fields_ = [("ndms", c_int32), ("bin", c_int32), ("nt", c_int64), ("row_pitch", c_int64), ("max_delay", c_int64),
-                ("dm_tile", c_int32), ("t_tile", c_int32), ("chan_block", c_int32), ("window", c_int32)]
+                ("dm_tile", c_int32), ("t_tile", c_int32), ("chan_block", c_int32), ("window", c_int32),
+                ("boxcar_extra", c_int32)]
 
 
 class _StrategyInfo(ctypes.Structure):
@@ -84,6 +85,7 @@ def load():
         "aa_plan_create": (c_int32, [POINTER(vp), c_int32, vp, c_double, vp, c_int32, vp, c_int32, c_float]),
         "aa_plan_destroy": (None, [vp]),
         "aa_plan_set_input_layout": (c_int32, [vp, c_int32]),
+        "aa_plan_set_boxcar_overlap": (c_int32, [vp, c_int32]),
         "aa_strategy_setup": (c_int32, [POINTER(vp), vp, c_uint64, vp, c_size_t, c_size_t, vp, vp, c_size_t, c_uint64]),
         "aa_strategy_plan": (c_int32, [POINTER(vp), vp, c_uint64, c_size_t, c_size_t, c_uint64]),
         "aa_strategy_destroy": (None, [vp]),
@@ -160,6 +162,10 @@ def aa_plan_create(chan_freq_mhz, tsamp_s, ranges, boxcar_widths, snr_threshold)
 
 def aa_plan_set_input_layout(plan, layout: int) -> int:
     return _check(load().aa_plan_set_input_layout(plan, int(layout)))
+
+
+def aa_plan_set_boxcar_overlap(plan, on: bool) -> int:
+    return _check(load().aa_plan_set_boxcar_overlap(plan, 1 if on else 0))
 
 
 def aa_plan_destroy(plan) -> None:
@@ -313,11 +319,14 @@ def aa_get_launch_count(strategy) -> int:
 class Plan:
     """Owns an aa_plan handle."""
 
-    def __init__(self, chan_freq_mhz, tsamp_s, ranges, boxcar_widths, snr_threshold, time_major: bool = False):
+    def __init__(self, chan_freq_mhz, tsamp_s, ranges, boxcar_widths, snr_threshold, time_major: bool = False,
+                 boxcar_overlap: bool = False):
         self.handle = aa_plan_create(chan_freq_mhz, tsamp_s, ranges, boxcar_widths, snr_threshold)
         self.ranges = [tuple(r) for r in ranges]
         if time_major:
             aa_plan_set_input_layout(self.handle, AA_LAYOUT_TIME_MAJOR)
+        if boxcar_overlap:
+            aa_plan_set_boxcar_overlap(self.handle, True)
 
     def close(self):
         if getattr(self, "handle", None):

@@ -37,6 +37,7 @@ struct Plan {
     std::vector<int32_t> widths;
     float threshold = 0.f;
     int32_t layout = 0;           /* aa_input_layout */
+    bool boxcar_overlap = false;  /* reading C3x */
 };
 
 /* Single-allocation bump allocator over caller- or library-owned device memory. */
@@ -67,6 +68,7 @@ struct Range : K2Plan {           /* the base is the range's main plan: uint8 fo
     int32_t index = 0;
     int64_t max_delay = 0;        /* binned samples */
     int64_t nt_full = 0;          /* T_r of a full chunk */
+    int32_t extra = 0;            /* E: samples dedispersed beyond T_r (reading C3x), 0 by default */
     int64_t pitch = 0;            /* D row pitch, elements */
     int32_t ndm_tiles = 0;
     std::vector<int32_t> delays;  /* [ndms][nchans], binned samples (host) */

@@ -102,6 +102,7 @@ typedef struct {
 } aak_candidate;
 typedef struct {
     const int32_t* D; int64_t pitch; int64_t nt; int32_t ndms; int32_t bin; int32_t range_index;
+    int64_t nt_data;           /* samples present per row (>= nt): boxcars may extend to here, candidates start below nt */
     double dm_low, dm_step;
     const double* mu_sigma;    /* [ndms][2] for this range */
     uint64_t chunk_start;

@@ -97,7 +97,7 @@ aa_status enqueue_k2(Strategy& s, const Chunk& c, int32_t c0, int32_t c1, bool a
         const int bin = rg.r.bin;
         aak_dedisp_args a;
         a.D = rg.d_D; a.pitch = rg.pitch;
-        a.nt = (int64_t)(c.n_out / (uint64_t)bin);
+        a.nt = (int64_t)(c.n_out / (uint64_t)bin) + rg.extra;      /* reading C3x: E samples beyond the output span */
         a.ndms = rg.r.ndms; a.nchans = s.plan.nchans;
         a.chan_begin = c0; a.chan_end = c1; a.accumulate = accumulate ? 1 : 0;
         for (int route = rg.has_lo ? 0 : 1; route < 2; ++route) {
@@ -285,7 +285,7 @@ extern "C" aa_status aa_run_sps(aa_strategy* h) {
     AA_CUDA(cudaEventRecord(s.ev_t[4], s.compute), "cudaEventRecord");
     for (Range& rg : s.ranges) {
         aak_sps_args a;
-        a.D = rg.d_D; a.pitch = rg.pitch; a.nt = (int64_t)(c.n_out / (uint64_t)rg.r.bin); a.ndms = rg.r.ndms; a.bin = rg.r.bin;
+        a.D = rg.d_D; a.pitch = rg.pitch; a.nt = (int64_t)(c.n_out / (uint64_t)rg.r.bin); a.nt_data = a.nt + rg.extra; a.ndms = rg.r.ndms; a.bin = rg.r.bin;
         a.range_index = rg.index; a.dm_low = rg.r.dm_low; a.dm_step = rg.r.dm_step;
         a.mu_sigma = s.d_mu_sigma + 2 * rg.first_row; a.chunk_start = c.start;
         a.nwidths = (int32_t)s.plan.widths.size();
@@ -366,7 +366,7 @@ extern "C" aa_status aa_get_dedispersed_row(aa_strategy* h, int32_t range, int32
         set_error("aa_get_dedispersed_row: range %d / dm_index %d out of bounds", range, dm_index); return AA_ERR_INVALID_ARG;
     }
     const Range& rg = s.ranges[(size_t)range];
-    const size_t nt = (size_t)(s.chunks[(size_t)s.current_chunk].n_out / (uint64_t)rg.r.bin);
+    const size_t nt = (size_t)(s.chunks[(size_t)s.current_chunk].n_out / (uint64_t)rg.r.bin) + (size_t)rg.extra;
     s.host_row.resize(nt);
     AA_CUDA(cudaMemcpyAsync(s.host_row.data(), rg.d_D + (size_t)dm_index * (size_t)rg.pitch, nt * 4, cudaMemcpyDeviceToHost, s.compute), "row D2H");
     AA_CUDA(cudaStreamSynchronize(s.compute), "cudaStreamSynchronize");
@@ -413,7 +413,7 @@ extern "C" aa_status aa_get_row_moments(aa_strategy* h, int32_t range, int64_t* 
     if (s.current_chunk < 0) { set_error("aa_get_row_moments: no chunk has been dedispersed yet"); return AA_ERR_ORDER; }
     if (!sum_d || !sum_td || range < 0 || range >= (int32_t)s.ranges.size()) { set_error("aa_get_row_moments: bad argument"); return AA_ERR_INVALID_ARG; }
     const Range& rg = s.ranges[(size_t)range];
-    const int64_t nt = (int64_t)(s.chunks[(size_t)s.current_chunk].n_out / (uint64_t)rg.r.bin);
+    const int64_t nt = (int64_t)(s.chunks[(size_t)s.current_chunk].n_out / (uint64_t)rg.r.bin) + rg.extra;
     long long* a = s.d_moments;
     long long* b = s.d_moments + rg.r.ndms;
     AA_LAUNCH(aak_row_moments(rg.d_D, rg.pitch, nt, rg.r.ndms, a, b, s.compute), "row moments");

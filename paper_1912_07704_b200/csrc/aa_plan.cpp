@@ -92,6 +92,12 @@ extern "C" aa_status aa_plan_create(aa_plan** out, int32_t nchans, const double*
 
 extern "C" void aa_plan_destroy(aa_plan* plan) { delete plan; }
 
+extern "C" aa_status aa_plan_set_boxcar_overlap(aa_plan* plan, int32_t on) {
+    if (!plan) { aa::set_error("aa_plan_set_boxcar_overlap: plan is NULL"); return AA_ERR_NOT_READY; }
+    plan->p.boxcar_overlap = on != 0;
+    return AA_OK;
+}
+
 extern "C" aa_status aa_plan_set_input_layout(aa_plan* plan, int32_t layout) {
     if (!plan) { aa::set_error("aa_plan_set_input_layout: plan is NULL"); return AA_ERR_NOT_READY; }
     if (layout != AA_LAYOUT_CHANNEL_MAJOR && layout != AA_LAYOUT_TIME_MAJOR) {

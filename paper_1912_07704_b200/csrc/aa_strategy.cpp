@@ -104,7 +104,7 @@ static void carve(Strategy& s, int64_t L, bool two_raw) {
     const int64_t n_out = L - s.S;
     for (Range& rg : s.ranges) {
         rg.nt_full = n_out / rg.r.bin;
-        rg.pitch = (int64_t)round_up((size_t)rg.nt_full, 128);
+        rg.pitch = (int64_t)round_up((size_t)(rg.nt_full + rg.extra), 128);
         rg.d_D = (int32_t*)a.take((size_t)rg.r.ndms * (size_t)rg.pitch * 4);
         rg.d_etab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * kDmTile * 4);
         rg.d_x0tab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * 4);
@@ -270,7 +270,8 @@ static aa_status plan_host(aa_strategy* h, const aa_plan* plan, uint64_t nsamp_t
         rg.r = s.plan.ranges[r];
         rg.index = (int32_t)r;
         if (!plan_range(s, rg, etabs[r], x0tabs[r], etabs[s.ranges.size() + r], x0tabs[s.ranges.size() + r])) return AA_ERR_INVALID_ARG;
-        smax = std::max<int64_t>(smax, rg.max_delay * rg.r.bin);
+        rg.extra = s.plan.boxcar_overlap ? s.plan.widths.back() - 1 : 0;       /* reading C3x */
+        smax = std::max<int64_t>(smax, (rg.max_delay + rg.extra) * rg.r.bin);
         rg.first_row = s.nrows;
         s.nrows += (size_t)rg.r.ndms;
         if (rg.r.bin == 1) s.need_u8_copies = true;
@@ -473,6 +474,7 @@ extern "C" aa_status aa_strategy_get_range_info(const aa_strategy* h, int32_t ra
     const Range& rg = h->s.ranges[(size_t)range];
     out->ndms = rg.r.ndms; out->bin = rg.r.bin; out->nt = rg.nt_full; out->row_pitch = rg.pitch; out->max_delay = rg.max_delay;
     out->dm_tile = kDmTile; out->t_tile = kTTile; out->chan_block = rg.chan_block; out->window = rg.window_bytes;
+    out->boxcar_extra = rg.extra;
     return AA_OK;
 }
 

@@ -304,7 +304,7 @@ constexpr int K4_RB = 32;                      /* centre rows per CTA (fewer whe
 constexpr int SPS_MAXW = 16;
 
 struct SpsParams {
-    const int32_t* D; i64 pitch; i64 nt; int ndms; int bin; int range_index;
+    const int32_t* D; i64 pitch; i64 nt; i64 ntd; int ndms; int bin; int range_index;   /* ntd: samples present per row >= nt */
     double dm_low, dm_step;
     const double* mu_sigma;
     u64 chunk_start;
@@ -338,7 +338,7 @@ __device__ __forceinline__ double k4_eval(const unsigned* I, const K4RowConst& r
     const unsigned base = I[e - 1];
     for (int iw = 0; iw < p.nwidths; ++iw) {
         const int w = p.widths[iw];
-        if (t + w > p.nt) break;                                   /* ascending widths */
+        if (t + w > p.ntd) break;                                  /* ascending widths */
         const int B = (int)(I[e + w - 1] - base);
         const double snr = __dmul_rn(__dsub_rn(__int2double_rn(B), rc.a[iw]), rc.inv[iw]);
         if (snr > best) { best = snr; bw = w; }
@@ -360,13 +360,13 @@ __device__ __forceinline__ void k4_prefilter(const unsigned* __restrict__ I, con
         if (q < p.tt && t < p.nt) {
             const unsigned* Iq = I + q + 3;                          /* B_w(t) = I[e+w-1] - I[e-1], e = q + 4 */
             const unsigned base = Iq[0];
-            if (t + p.wmax <= p.nt) {
+            if (t + p.wmax <= p.ntd) {
 #pragma unroll
                 for (int iw = 0; iw < NW; ++iw) f |= ((int)(Iq[p.widths[iw]] - base) >= bm[iw]);
             } else {
 #pragma unroll
                 for (int iw = 0; iw < NW; ++iw)
-                    if (t + p.widths[iw] <= p.nt) f |= ((int)(Iq[p.widths[iw]] - base) >= bm[iw]);
+                    if (t + p.widths[iw] <= p.ntd) f |= ((int)(Iq[p.widths[iw]] - base) >= bm[iw]);
             }
         }
         const unsigned mask = __ballot_sync(0xffffffffu, f);
@@ -407,7 +407,7 @@ k_sps_peaks(const SpsParams p) {
 #pragma unroll
         for (int v = 0; v < V; ++v) {
             const i64 t = tb + e0 + 4 * v;
-            if (t >= 0 && t < p.nt && e0 + 4 * v < ne) buf[v] = __ldg(reinterpret_cast<const int4*>(row + t));
+            if (t >= 0 && t < p.ntd && e0 + 4 * v < ne) buf[v] = __ldg(reinterpret_cast<const int4*>(row + t));
             else buf[v] = make_int4(0, 0, 0, 0);
         }
     };
@@ -449,7 +449,7 @@ k_sps_peaks(const SpsParams p) {
                 const int d[4] = {cur[v].x, cur[v].y, cur[v].z, cur[v].w};
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
-                    const bool in = (t + k >= 0) && (t + k < p.nt);
+                    const bool in = (t + k >= 0) && (t + k < p.ntd);
                     run += in ? (unsigned)(d[k] - pv_c) : 0u;
                     loc[v][k] = run;
                 }
@@ -571,7 +571,7 @@ extern "C" int aak_sps_init(void) {
 extern "C" int aak_sps_peaks(const aak_sps_args* a, void* stream) {
     if (a->nwidths < 1 || a->nwidths > SPS_MAXW) return (int)cudaErrorInvalidValue;
     SpsParams p;
-    p.D = a->D; p.pitch = a->pitch; p.nt = a->nt; p.ndms = a->ndms; p.bin = a->bin; p.range_index = a->range_index;
+    p.D = a->D; p.pitch = a->pitch; p.nt = a->nt; p.ntd = a->nt_data > a->nt ? a->nt_data : a->nt; p.ndms = a->ndms; p.bin = a->bin; p.range_index = a->range_index;
     p.dm_low = a->dm_low; p.dm_step = a->dm_step; p.mu_sigma = a->mu_sigma; p.chunk_start = a->chunk_start;
     p.nwidths = a->nwidths; p.wmax = 0;
     for (int k = 0; k < SPS_MAXW; ++k) { p.widths[k] = k < a->nwidths ? a->widths[k] : 0; if (p.widths[k] > p.wmax) p.wmax = p.widths[k]; }

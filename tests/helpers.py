@@ -34,11 +34,12 @@ class OracleRun:
             self._xb[key] = oracle.bin_time(self.x, start, length // b, b)
         return self._xb[key]
 
-    def search(self, chunk, r_index, i0, i1, want=("D", "stats")):
+    def search(self, chunk, r_index, i0, i1, want=("D", "stats"), extra=0):
         start, length, n_out = chunk
         rng = self.w.ranges[r_index]
         xb = self.binned(start, length, rng[3])
-        return oracle.search_rows(xb, self.k, rng, r_index, n_out // rng[3], self.w.widths, self.w.threshold, start, i0, i1, want=want)
+        return oracle.search_rows(xb, self.k, rng, r_index, n_out // rng[3], self.w.widths, self.w.threshold, start, i0, i1, want=want,
+                                  extra=extra)
 
 
 def compare_candidates(got: np.ndarray, exp: np.ndarray, threshold: float, snr_rtol=1e-4, band=1e-3):
@@ -159,13 +160,15 @@ def sampled_outputs(x: np.ndarray, k: np.ndarray, rng, start: int, T: int, point
 class GpuRun:
     """The CUDA path through the C-ABI binding for one workload (plan -> strategy -> chunk loop)."""
 
-    def __init__(self, w, x, time_major: bool = False, **strategy_kw):
+    def __init__(self, w, x, time_major: bool = False, boxcar_overlap: bool = False, **strategy_kw):
         """x is always the channel-major array [nchans][nsamp] the oracle sees; with time_major=True the library is handed
         its transpose x_tm[t][c] (the plain definition of the corner turn) through a time-major plan."""
         import paper_1912_07704_b200 as aa
         self.aa, self.w = aa, w
         self.x = np.ascontiguousarray(x.T) if time_major else x
-        self.plan = aa.Plan(w.freqs_mhz, w.tsamp_s, w.ranges, w.widths, w.threshold, time_major=time_major)
+        self.plan = aa.Plan(w.freqs_mhz, w.tsamp_s, w.ranges, w.widths, w.threshold, time_major=time_major,
+                            boxcar_overlap=boxcar_overlap)
+        self.extra = max(w.widths) - 1 if boxcar_overlap else 0          # reading C3x
         self.st = aa.Strategy(self.plan, x.shape[1], **strategy_kw)
         self.h = self.st.handle
         self.info = self.st.info
@@ -208,7 +211,7 @@ def band_rows(ndms: int, centres, half: int = 2):
 def check_band(gpu: GpuRun, orc: OracleRun, chunk, r, i0, i1, *, after_sps: bool, cands=None):
     """Bit-exact D rows [i0,i1) and (after SPS) mu/sigma of the same rows; returns the oracle's candidates in the band's
     INTERIOR rows (those whose 3x3 neighbourhood lies inside the band or at the range edge)."""
-    res = orc.search(chunk, r, i0, i1, want=("D", "stats"))
+    res = orc.search(chunk, r, i0, i1, want=("D", "stats"), extra=getattr(gpu, "extra", 0))
     for i in range(i0, i1):
         got = gpu.row(r, i)
         exp = res["D"][i - i0]

@@ -227,3 +227,51 @@ def test_python_front_end_adds_no_appreciable_run_time():
         assert tp <= tc * 1.05 + 0.5e-3
     finally:
         g.close()
+
+
+def test_boxcar_complete_chunks_match_the_oracle_and_recover_a_straddling_pulse():
+    """Reading C3x (aa_plan_set_boxcar_overlap): rows are dedispersed E = W_max - 1 samples beyond the chunk's output span.
+    Every row (incl. the extra samples), statistic and candidate equals the oracle's with the same E; the geometry is the
+    oracle's; and a wide pulse placed across a chunk boundary, which the plain chunking only sees with narrow boxcars at
+    the end of the chunk, is now found at its full width."""
+    import oracle
+    base = datagen.get_workload("tiny")
+    widths = (1, 2, 4, 8, 16, 32, 64)
+    E = max(widths) - 1
+    L = 2048
+    k = oracle.delay_constants(base.freqs_mhz, base.tsamp_s)
+    geo = oracle.chunk_geometry(k, base.ranges, base.nsamp, chunk_len=L, boxcar_extra=E)
+    t_edge = geo["chunks"][1][0] + geo["n_out"]                    # first output sample of chunk 2
+    w = scaled(base, name="tiny_c3x", widths=widths, ranges=((0.0, 1.0, 60, 1), (60.0, 2.0, 20, 2)),
+               fixed_pulses=((20.0, t_edge - 24, 48, 3.0),))        # 48 samples wide, half of it beyond the chunk's span
+    x, _ = make_input(w)
+    k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
+    geo = oracle.chunk_geometry(k, w.ranges, w.nsamp, chunk_len=L, boxcar_extra=E)
+    gpu, orc = GpuRun(w, x, boxcar_overlap=True, chunk_len_hint=L), OracleRun(w, x)
+    plain = GpuRun(w, x, chunk_len_hint=L)
+    try:
+        assert (gpu.info["overlap"], gpu.info["n_out"]) == (geo["S"], geo["n_out"]) and gpu.chunks == geo["chunks"]
+        assert gpu.info["overlap"] > plain.info["overlap"]
+        assert all(gpu.aa.aa_strategy_get_range_info(gpu.h, r)["boxcar_extra"] == E for r in range(len(w.ranges)))
+        exp_all = []
+        for chunk in gpu.chunks:
+            gpu.dedisperse()
+            gpu.sps()
+            for r, rng in enumerate(w.ranges):
+                exp_all.append(check_band(gpu, orc, chunk, r, 0, rng[2], after_sps=True))
+        got = gpu.candidates()
+        n, og, oe = compare_candidates(got, np.concatenate(exp_all), w.threshold)
+        assert n + og == len(got) and n + oe == sum(len(e) for e in exp_all)
+        # the straddling pulse: with C3x a candidate of width >= 32 starts within the last 48 samples before the edge
+        near = (got["range"] == 0) & (got["sample"] >= t_edge - 48) & (got["sample"] < t_edge)
+        assert near.any() and int(got["width"][near].max()) >= 32
+        ref = plain.st.run(x)
+        pe = plain.info["n_out"]                                    # the plain run's own chunk edges
+        edges = [(j + 1) * pe for j in range(plain.info["nchunks"] - 1)]
+        for e in edges:                                              # plain chunking: no boxcar can cross its chunk's end
+            m = (ref["range"] == 0) & (ref["sample"] < e) & (ref["sample"] + ref["width"] > e)
+            assert not m.any()
+        assert ((got["range"] == 0) & (got["sample"] < t_edge) & (got["sample"] + got["width"] > t_edge)).any()
+    finally:
+        gpu.close()
+        plain.close()
