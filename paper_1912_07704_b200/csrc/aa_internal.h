@@ -123,6 +123,9 @@ struct Strategy {
 
     /* streams / events */
     cudaStream_t compute = nullptr, copy = nullptr;
+    cudaStream_t aux = nullptr;                       /* library-owned: every other DM range's K2 runs here, so that the tail
+                                                         wave of one range overlaps the first wave of the next */
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     bool owns_compute = false, owns_copy = false;
     cudaEvent_t ev_copied[2] = {nullptr, nullptr};    /* chunk landed in d_raw[b] (copy stream) */
     cudaEvent_t ev_raw_free[2] = {nullptr, nullptr};  /* last reader of d_raw[b] finished (compute stream) */

@@ -93,7 +93,15 @@ aa_status enqueue_prep(Strategy& s, const Chunk& c, int b, int32_t c0, int32_t c
 /* K2 of every range over channels [c0, c1) (channel group g); accumulate = add to the D already there. A bin 2 / 4 range
  * launches both of its routes; each tests the group's exception counter and only one of them runs. */
 aa_status enqueue_k2(Strategy& s, const Chunk& c, int32_t c0, int32_t c1, bool accumulate, int g) {
+    /* ranges are independent: odd ranges go to the auxiliary stream so the last, partly filled wave of one range's K2
+     * overlaps the first wave of the next one (fork after the prep kernels, join before anything reads D) */
+    const bool two = s.ranges.size() > 1 && s.aux;
+    if (two) {
+        AA_CUDA(cudaEventRecord(s.ev_fork, s.compute), "cudaEventRecord");
+        AA_CUDA(cudaStreamWaitEvent(s.aux, s.ev_fork, 0), "cudaStreamWaitEvent");
+    }
     for (Range& rg : s.ranges) {
+        cudaStream_t st = (two && (rg.index & 1)) ? s.aux : s.compute;
         const int bin = rg.r.bin;
         aak_dedisp_args a;
         a.D = rg.d_D; a.pitch = rg.pitch;
@@ -108,11 +116,15 @@ aa_status enqueue_k2(Strategy& s, const Chunk& c, int32_t c0, int32_t c1, bool a
             a.mode_cnt = rg.has_lo ? s.d_exc_cnt[bin] + g : nullptr;
             a.mode_cap = rg.has_lo ? group_limit(s, bin, c0, c1) : 0u; a.mode_dense = route;
             a.bias = route == 0 ? (const int32_t*)(s.d_exc_cnt[bin] + kMaxGroups + g) : nullptr;
-            AA_LAUNCH(aak_dedisperse(&a, s.compute), "dedispersion");
+            AA_LAUNCH(aak_dedisperse(&a, st), "dedispersion");
         }
         if (rg.has_lo)
             AA_LAUNCH(aak_scatter_exceptions(s.d_exc[bin] + (size_t)g * kExcCap, s.d_exc_cnt[bin] + g, group_limit(s, bin, c0, c1), s.d_k, rg.r.dm_low, rg.r.dm_step,
-                                             rg.r.ndms, bin, a.nt, rg.d_D, rg.pitch, s.compute), "exception scatter");
+                                             rg.r.ndms, bin, a.nt, rg.d_D, rg.pitch, st), "exception scatter");
+    }
+    if (two) {
+        AA_CUDA(cudaEventRecord(s.ev_join, s.aux), "cudaEventRecord");
+        AA_CUDA(cudaStreamWaitEvent(s.compute, s.ev_join, 0), "cudaStreamWaitEvent");
     }
     return AA_OK;
 }

@@ -391,6 +391,9 @@ extern "C" aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, u
         if ((e = cudaEventCreate(&s.ev_h2d[b])) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
     }
     if ((e = cudaEventCreateWithFlags(&s.ev_count, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
+    if ((e = cudaStreamCreateWithFlags(&s.aux, cudaStreamNonBlocking)) != cudaSuccess) return fail(cuda_fail(e, "cudaStreamCreate"));
+    if ((e = cudaEventCreateWithFlags(&s.ev_fork, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
+    if ((e = cudaEventCreateWithFlags(&s.ev_join, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
     for (int g = 0; g < kMaxGroups; ++g)
         if ((e = cudaEventCreateWithFlags(&s.ev_group[g], cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
     for (int i = 0; i < 6; ++i)
@@ -444,6 +447,9 @@ extern "C" void aa_strategy_destroy(aa_strategy* h) {
         if (s.ev_raw_free[b]) cudaEventDestroy(s.ev_raw_free[b]);
         if (s.ev_h2d[b]) cudaEventDestroy(s.ev_h2d[b]);
     }
+    if (s.aux) { cudaStreamSynchronize(s.aux); cudaStreamDestroy(s.aux); }
+    if (s.ev_fork) cudaEventDestroy(s.ev_fork);
+    if (s.ev_join) cudaEventDestroy(s.ev_join);
     if (s.ev_count) cudaEventDestroy(s.ev_count);
     for (int g = 0; g < kMaxGroups; ++g) if (s.ev_group[g]) cudaEventDestroy(s.ev_group[g]);
     for (int i = 0; i < 6; ++i) if (s.ev_t[i]) cudaEventDestroy(s.ev_t[i]);
