@@ -262,7 +262,7 @@ def run_ours(args, w):
         return
 
     # roofline of the dominant kernel (K2, all ranges of one step = 5 launches): integer adds, bound "alu"
-    iadd3, mixed, mhz = aa.aa_measure_int_add_peak(compute, 300)
+    iadd3, mixed, imad, mhz = aa.aa_measure_int_add_peak3(compute, 300)
     k2 = float(np.mean(k2_ms)) * 1e-3
     peak = SM_COUNT * INT_LANES_PER_SM_CLK * (sampler.max_mhz or 1965) * 1e6
     t_hbm = (in_bytes + 4 * outputs) / (json.loads((ROOT / "MEASURED_PEAKS.json").read_text())["hbm_gbs"] * 1e9) \
@@ -273,7 +273,7 @@ def run_ours(args, w):
                 "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of the K2 launches of one step (9 launches on ska), one "
                                 "ncu capture: profiles/r01c_dram_per_launch.csv; compulsory bytes are input once + D once",
                 "peak_how": f"derived: {SM_COUNT} SMs x {INT_LANES_PER_SM_CLK} integer-add lanes/clk (64 IADD3 + 64 IMAD) x max SM clock",
-                "measured_iadd3_only_tadd_s": iadd3 / 1e12, "measured_iadd3_imad_mixed_tadd_s": mixed / 1e12,
+                "measured_iadd3_only_tadd_s": iadd3 / 1e12, "measured_iadd3_imad_mixed_tadd_s": mixed / 1e12, "measured_imad_only_tadd_s": imad / 1e12,
                 "frac_of_measured_mixed": adds / k2 / max(mixed, iadd3), "frac_of_measured_iadd3_only": adds / k2 / iadd3,
                 "microbench_sm_mhz": mhz, "k2_ms_per_step": k2 * 1e3, "t_hbm_compulsory_ms": t_hbm * 1e3,
                 "algorithmic_adds_per_step": adds}

@@ -229,6 +229,9 @@ aa_status aa_synchronize(aa_strategy* s);
  * IADD3-only chains, with IADD3+IMAD mixed chains (both integer pipes), and the SM clock (MHz) observed via the cycle
  * counter. */
 aa_status aa_measure_int_add_peak(void* stream, int32_t millis, double* iadd3_per_s, double* mixed_per_s, double* sm_mhz);
+/* Same, plus the rate of IMAD-only chains (x*1+y on the FMA pipe alone). Any output pointer may be NULL. */
+aa_status aa_measure_int_add_peak3(void* stream, int32_t millis, double* iadd3_per_s, double* mixed_per_s, double* imad_per_s,
+                                   double* sm_mhz);
 
 /* CUDA-event time (ms) of the kernel classes of the last chunk: [0] binning, [1] dedispersion (all ranges),
  * [2] SPS statistics, [3] SPS boxcar/peaks, [4] H2D of the chunk (0 if prefetched/overlapped). Synchronises. */

@@ -21,7 +21,7 @@ __all__ = [
     "aa_strategy_get_range_info", "aa_strategy_get_chunk", "aa_strategy_get_delay", "aa_strategy_describe",
     "aa_strategy_reset", "aa_strategy_shard", "aa_run_dedispersion", "aa_run_dedispersion_device", "aa_run_sps", "aa_run_pipeline", "aa_get_candidates",
     "aa_get_dedispersed_row", "aa_get_row_stats", "aa_get_row_moments", "aa_get_dedispersed_device", "aa_synchronize",
-    "aa_measure_int_add_peak", "aa_get_last_timings", "aa_get_launch_count", "aa_last_error", "aa_version",
+    "aa_measure_int_add_peak", "aa_measure_int_add_peak3", "aa_get_last_timings", "aa_get_launch_count", "aa_last_error", "aa_version",
     "Plan", "Strategy",
 ]
 
@@ -107,6 +107,7 @@ def load():
         "aa_get_dedispersed_device": (c_int32, [vp, c_int32, POINTER(vp), POINTER(c_int64)]),
         "aa_synchronize": (c_int32, [vp]),
         "aa_measure_int_add_peak": (c_int32, [vp, c_int32, POINTER(c_double), POINTER(c_double), POINTER(c_double)]),
+        "aa_measure_int_add_peak3": (c_int32, [vp, c_int32, POINTER(c_double), POINTER(c_double), POINTER(c_double), POINTER(c_double)]),
         "aa_get_last_timings": (c_int32, [vp, POINTER(c_float * 5)]),
         "aa_get_launch_count": (c_int32, [vp, POINTER(c_uint64)]),
         "aa_last_error": (c_char_p, []),
@@ -301,6 +302,13 @@ def aa_measure_int_add_peak(stream=None, millis: int = 200):
     a, b, c = c_double(), c_double(), c_double()
     _check(load().aa_measure_int_add_peak(_ptr(stream), int(millis), byref(a), byref(b), byref(c)))
     return a.value, b.value, c.value
+
+
+def aa_measure_int_add_peak3(stream=None, millis: int = 200):
+    """(IADD3-only, IADD3+IMAD mixed, IMAD-only) lane-adds per second and the SM clock in MHz."""
+    a, b, c, d = c_double(), c_double(), c_double(), c_double()
+    _check(load().aa_measure_int_add_peak3(_ptr(stream), int(millis), byref(a), byref(b), byref(c), byref(d)))
+    return a.value, b.value, c.value, d.value
 
 
 def aa_get_last_timings(strategy) -> dict:

@@ -463,6 +463,10 @@ extern "C" aa_status aa_get_launch_count(const aa_strategy* h, uint64_t* launche
 }
 
 extern "C" aa_status aa_measure_int_add_peak(void* stream, int32_t millis, double* iadd3_per_s, double* mixed_per_s, double* sm_mhz) {
+    return aa_measure_int_add_peak3(stream, millis, iadd3_per_s, mixed_per_s, nullptr, sm_mhz);
+}
+
+extern "C" aa_status aa_measure_int_add_peak3(void* stream, int32_t millis, double* iadd3_per_s, double* mixed_per_s, double* imad_per_s, double* sm_mhz) {
     cudaStream_t st = (cudaStream_t)stream;
     int dev = 0, nsm = 0;
     cudaError_t e;
@@ -475,10 +479,10 @@ extern "C" aa_status aa_measure_int_add_peak(void* stream, int32_t millis, doubl
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0); cudaEventCreate(&e1);
     std::vector<unsigned long long> hc((size_t)grid);
-    double rate[2] = {0, 0}, mhz = 0;
+    double rate[3] = {0, 0, 0}, mhz = 0;
     aa_status ret = AA_OK;
     if (millis < 1) millis = 1;
-    for (int mode = 0; mode < 2 && ret == AA_OK; ++mode) {
+    for (int mode = 0; mode < 3 && ret == AA_OK; ++mode) {
         int iters = 4096;
         for (int pass = 0; pass < 2; ++pass) {       /* pass 0 calibrates the iteration count */
             cudaEventRecord(e0, st);
@@ -504,6 +508,7 @@ extern "C" aa_status aa_measure_int_add_peak(void* stream, int32_t millis, doubl
     if (ret != AA_OK) return ret;
     if (iadd3_per_s) *iadd3_per_s = rate[0];
     if (mixed_per_s) *mixed_per_s = rate[1];
+    if (imad_per_s) *imad_per_s = rate[2];
     if (sm_mhz) *sm_mhz = mhz;
     return AA_OK;
 }

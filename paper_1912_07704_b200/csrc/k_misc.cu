@@ -259,6 +259,12 @@ k_peak_iadd(int mode, int iters, uint32_t* __restrict__ sink, unsigned long long
             for (int i = 0; i < AAK_PEAK_ADDS_PER_THREAD_ITER; ++i)
                 asm volatile("{.reg .u32 t; add.u32 t, %0, %1; add.u32 %0, t, %2;}" : "+r"(a[i]) : "r"(b), "r"(m));   /* one IADD3 */
         }
+    } else if (mode == 2) {                                       /* every step an IMAD (FMA pipe only) */
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int i = 0; i < AAK_PEAK_ADDS_PER_THREAD_ITER; ++i)
+                asm volatile("mad.lo.u32 %0, %1, %2, %0;" : "+r"(a[i]) : "r"(b), "r"(m));
+        }
     } else {
         for (int it = 0; it < iters; ++it) {
 #pragma unroll
