@@ -36,7 +36,7 @@ extern "C" aa_status aa_plan_create(aa_plan** out, int32_t nchans, const double*
     using aa::set_error;
     if (!out) { set_error("aa_plan_create: out is NULL"); return AA_ERR_INVALID_ARG; }
     *out = nullptr;
-    if (nchans < 1) { set_error("aa_plan_create: nchans = %d must be >= 1", nchans); return AA_ERR_INVALID_ARG; }
+    if (nchans < 1 || nchans > 65535) { set_error("aa_plan_create: nchans = %d must be in 1..65535", nchans); return AA_ERR_INVALID_ARG; }
     if (!chan_freq_mhz) { set_error("aa_plan_create: chan_freq_mhz is NULL"); return AA_ERR_INVALID_ARG; }
     for (int32_t c = 0; c < nchans; ++c) {
         if (!(chan_freq_mhz[c] > 0.0) || !std::isfinite(chan_freq_mhz[c])) {
