@@ -305,6 +305,10 @@ static aa_status plan_host(aa_strategy* h, const aa_plan* plan, uint64_t nsamp_t
         }
         while (p2 * 2 < usable && need(p2 * 2) <= limit) p2 *= 2;
         L = p2;
+        /* then grow in eighths of that power of two while the arena still fits: every chunk recomputes S samples of
+         * overlap, so longer chunks waste less (600 s stream under 40 GB: L = 2^19 -> 9 * 2^16, 19 -> 17 chunks) */
+        const int64_t step = (int64_t)round_up((size_t)std::max<int64_t>(p2 / 8, s.B), (size_t)s.B);
+        while (L + step < usable && need(L + step) <= limit) L += step;
     }
     s.L = L;
     s.n_out = L - s.S;
