@@ -22,10 +22,6 @@ extern "C" {
  * range that also has the offset-uint8 route runs only for chunks with too many exceptions). Same for aak_shift_copy. */
 int aak_bin_time(const uint8_t* x, size_t x_pitch, uint16_t* xb, size_t xb_pitch_elems, int32_t nchans,
                  int64_t nbinned, int32_t bin, const unsigned* only_if_cnt, unsigned only_if_above, void* stream);
-/* ---- K1a: the four sample-shifted copies of the uint8 chunk in one pass: out[k*copy_stride + c*pitch + j] = in[c*pitch + j + k],
- * k = 0..3, j in [0, row_bytes). row_bytes, pitch, copy_stride multiples of 16; in readable 4 bytes past each row. */
-int aak_make_copies_u8(const uint8_t* in, uint8_t* out, size_t pitch, size_t copy_stride, size_t row_bytes, int32_t nrows,
-                       void* stream);
 /* ---- K1b: shifted copy, out[c][j] = in[c][j + shift_bytes] (1..3) for j in [0, row_bytes), rows `pitch` bytes apart.
  * row_bytes and pitch are multiples of 16; the source must be readable up to row_bytes + 4 past each row start. */
 int aak_shift_copy(const uint8_t* in, uint8_t* out, size_t pitch, size_t row_bytes, int32_t nrows, int32_t shift_bytes,
@@ -33,16 +29,27 @@ int aak_shift_copy(const uint8_t* in, uint8_t* out, size_t pitch, size_t row_byt
 
 /* ---- K1c: offset-uint8 form of a binned input (bin 2, 4), see k_misc.cu: x_b = lo + off_c + r with lo a byte and r an
  * exception list. aak_chan_offsets: off_b[c] = clamp(round(b * mean_t x[c][t]) - 128, 0, 255 (b-1)) for rows [0, nrows) and
- * *bias_b += sum of them (either pair may be NULL). aak_bin_offset: lo[c][t'] (copy 0, bytes) and the exceptions
- * {c + chan0 | (r + 1024) << 16, t'} appended at exc[atomicAdd(exc_cnt)] while below cap (the counter keeps counting).
+ * *bias_b += sum of them (either pair may be NULL). aak_prep_fused (below) writes lo[c][t'] and appends the exceptions
+ * {c + chan0 | (r + 1024) << 16, t'} at exc[atomicAdd(exc_cnt)] while below cap (the counter keeps counting).
  * aak_scatter_exceptions: D[i][t' - delay(c, i)] += r for every exception and every trial of one range; returns at once
  * if *exc_cnt > cap. k = the plan's delay constants (device doubles). */
 int aak_chan_offsets(const uint8_t* x, size_t pitch, int64_t len, int32_t nrows, int32_t* off2, int32_t* off4, int32_t* bias2,
                      int32_t* bias4, void* stream);
-int aak_bin_offset(const uint8_t* x, size_t x_pitch, uint8_t* lo, size_t lo_pitch, const int32_t* off, int32_t nrows, int32_t chan0,
-                   int64_t nbinned, int32_t bin, uint2* exc, unsigned* exc_cnt, unsigned cap, void* stream);
 int aak_scatter_exceptions(const uint2* exc, const unsigned* exc_cnt, unsigned cap, const double* k, double dm_low, double dm_step,
                            int32_t ndms, int32_t bin, int64_t nt, int32_t* D, int64_t pitch, void* stream);
+
+/* ---- K1 fused: one read of raw rows [0, nrows) (pointers already offset to the first row; chan0 = its channel index)
+ * writes the 4 uint8 copies (x4, may be NULL), the offset-uint8 forms lo2 / lo4 with their 4 copies and exceptions (may be
+ * NULL; off2/off4 offset to the first row; nb = valid binned samples) and the 2 copies of the uint16 bin-8 input (xb8,
+ * may be NULL; xb8_pitch in elements, xb8_stride in bytes). ngroups = 16-byte groups per row. */
+typedef struct {
+    const uint8_t* raw; size_t pitch; int64_t ngroups; int32_t chan0; unsigned cap;
+    uint8_t* x4; size_t x4_stride;
+    uint8_t* lo2; size_t lo2_pitch, lo2_stride; const int32_t* off2; uint2* exc2; unsigned* cnt2; int64_t nb2;
+    uint8_t* lo4; size_t lo4_pitch, lo4_stride; const int32_t* off4; uint2* exc4; unsigned* cnt4; int64_t nb4;
+    uint16_t* xb8; size_t xb8_pitch, xb8_stride;
+} aak_prep_args;
+int aak_prep_fused(const aak_prep_args* a, int32_t nrows, void* stream);
 
 /* ---- K2: dedispersion --------------------------------------------------------------------------------------------
  * Tiled kernel: a CTA owns DM_TILE(=32) DM trials x T_TILE(=1024) output samples; channels stream through shared memory

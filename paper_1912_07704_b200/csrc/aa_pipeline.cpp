@@ -65,27 +65,33 @@ static unsigned group_limit(const Strategy& s, int bin, int32_t c0, int32_t c1) 
 aa_status enqueue_prep(Strategy& s, const Chunk& c, int b, int32_t c0, int32_t c1, int g) {
     const int32_t n = c1 - c0;
     const uint8_t* raw = s.d_raw[b] + (size_t)c0 * s.in_pitch;
-    if (s.need_u8_copies)
-        AA_LAUNCH(aak_make_copies_u8(raw, s.d_x4 + (size_t)c0 * s.in_pitch, s.in_pitch, s.x4_stride, s.in_pitch, n, s.compute), "shifted copies (uint8)");
     if (s.d_lo[2] || s.d_lo[4])
         AA_LAUNCH(aak_chan_offsets(raw, s.in_pitch, (int64_t)c.len, n, s.d_lo[2] ? s.d_off[2] + c0 : nullptr, s.d_lo[4] ? s.d_off[4] + c0 : nullptr,
                                    s.d_lo[2] ? (int32_t*)(s.d_exc_cnt[2] + kMaxGroups + g) : nullptr,
                                    s.d_lo[4] ? (int32_t*)(s.d_exc_cnt[4] + kMaxGroups + g) : nullptr, s.compute), "channel offsets");
-    for (int bin = 2; bin <= 8; bin *= 2) {
-        const int64_t nb = (int64_t)(c.len / (uint64_t)bin);
-        const unsigned* cnt = nullptr;
-        if (bin <= 4 && s.d_lo[bin]) {
-            cnt = s.d_exc_cnt[bin] + g;
-            uint8_t* lo = s.d_lo[bin] + (size_t)c0 * s.lo_pitch[bin];
-            AA_LAUNCH(aak_bin_offset(raw, s.in_pitch, lo, s.lo_pitch[bin], s.d_off[bin] + c0, n, c0, nb, bin, s.d_exc[bin] + (size_t)g * kExcCap,
-                                     s.d_exc_cnt[bin] + g, kExcCap, s.compute), "time binning (offset uint8)");
-            AA_LAUNCH(aak_make_copies_u8(lo, lo, s.lo_pitch[bin], s.lo_stride[bin], s.lo_pitch[bin], n, s.compute), "shifted copies (offset uint8)");
-        }
+    /* one read of the raw rows writes every input form K2 may read, except the uint16 forms of bin 2 / 4 */
+    aak_prep_args a;
+    memset(&a, 0, sizeof a);
+    a.raw = raw; a.pitch = s.in_pitch; a.ngroups = (int64_t)(s.in_pitch / 16); a.chan0 = c0; a.cap = kExcCap;
+    if (s.need_u8_copies) { a.x4 = s.d_x4 + (size_t)c0 * s.in_pitch; a.x4_stride = s.x4_stride; }
+    if (s.d_lo[2]) {
+        a.lo2 = s.d_lo[2] + (size_t)c0 * s.lo_pitch[2]; a.lo2_pitch = s.lo_pitch[2]; a.lo2_stride = s.lo_stride[2]; a.off2 = s.d_off[2] + c0;
+        a.exc2 = s.d_exc[2] + (size_t)g * kExcCap; a.cnt2 = s.d_exc_cnt[2] + g; a.nb2 = (int64_t)(c.len / 2);
+    }
+    if (s.d_lo[4]) {
+        a.lo4 = s.d_lo[4] + (size_t)c0 * s.lo_pitch[4]; a.lo4_pitch = s.lo_pitch[4]; a.lo4_stride = s.lo_stride[4]; a.off4 = s.d_off[4] + c0;
+        a.exc4 = s.d_exc[4] + (size_t)g * kExcCap; a.cnt4 = s.d_exc_cnt[4] + g; a.nb4 = (int64_t)(c.len / 4);
+    }
+    if (s.d_xb[8]) { a.xb8 = s.d_xb[8] + (size_t)c0 * s.xb_pitch[8]; a.xb8_pitch = s.xb_pitch[8]; a.xb8_stride = s.xb_stride[8]; }
+    AA_LAUNCH(aak_prep_fused(&a, n, s.compute), "input forms (fused)");
+    for (int bin = 2; bin <= 4; bin *= 2) {
         if (!s.d_xb[bin]) continue;
+        const unsigned* cnt = s.d_lo[bin] ? s.d_exc_cnt[bin] + g : nullptr;      /* NULL: the range has no offset-uint8 route */
+        const unsigned lim = cnt ? group_limit(s, bin, c0, c1) : 0u;
         const size_t pitch_bytes = s.xb_pitch[bin] * 2;
         uint16_t* xb = s.d_xb[bin] + (size_t)c0 * s.xb_pitch[bin];
-        AA_LAUNCH(aak_bin_time(raw, s.in_pitch, xb, s.xb_pitch[bin], n, nb, bin, cnt, cnt ? group_limit(s, bin, c0, c1) : 0u, s.compute), "time binning");
-        AA_LAUNCH(aak_shift_copy((const uint8_t*)xb, (uint8_t*)xb + s.xb_stride[bin], pitch_bytes, pitch_bytes, n, 2, cnt, cnt ? group_limit(s, bin, c0, c1) : 0u, s.compute), "shift copy (uint16)");
+        AA_LAUNCH(aak_bin_time(raw, s.in_pitch, xb, s.xb_pitch[bin], n, (int64_t)(c.len / (uint64_t)bin), bin, cnt, lim, s.compute), "time binning");
+        AA_LAUNCH(aak_shift_copy((const uint8_t*)xb, (uint8_t*)xb + s.xb_stride[bin], pitch_bytes, pitch_bytes, n, 2, cnt, lim, s.compute), "shift copy (uint16)");
     }
     return AA_OK;
 }

@@ -73,26 +73,6 @@ k_shift_copy(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, size_t p
     }
 }
 
-/* ---- K1a: all four sample-shifted uint8 copies in one pass (reads the chunk once, writes 4 x): copy k at out + k*copy_stride */
-__global__ void __launch_bounds__(256)
-k_make_copies_u8(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, size_t pitch, size_t copy_stride, long long ngroups) {
-    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= ngroups) return;
-    const size_t off = (size_t)blockIdx.y * pitch + (size_t)g * 16;
-    const uint4 a = *reinterpret_cast<const uint4*>(in + off);
-    const uint32_t nx = *reinterpret_cast<const uint32_t*>(in + off + 16);
-    *reinterpret_cast<uint4*>(out + off) = a;
-#pragma unroll
-    for (int k = 1; k < 4; ++k) {
-        uint4 o;
-        o.x = __funnelshift_r(a.x, a.y, 8 * k);
-        o.y = __funnelshift_r(a.y, a.z, 8 * k);
-        o.z = __funnelshift_r(a.z, a.w, 8 * k);
-        o.w = __funnelshift_r(a.w, nx, 8 * k);
-        *reinterpret_cast<uint4*>(out + (size_t)k * copy_stride + off) = o;
-    }
-}
-
 /* ---- K0t: corner turn. Telescopes deliver TIME-major samples x_tm[t][c] (PAPER.md:47 step 1 "telescope data");
  * the dedispersion kernels read CHANNEL-major rows x[c][t]. A CTA transposes a 128-channel x 128-sample tile:
  * each thread loads 4 words = 4 samples x 4 channels, transposes the 4x4 bytes in registers (8 PRMT), and stores four
@@ -169,39 +149,6 @@ k_chan_offsets(const uint8_t* __restrict__ x, size_t pitch, long long len, int32
     }
 }
 
-template <int B>
-__global__ void __launch_bounds__(256)
-k_bin_offset(const uint8_t* __restrict__ x, size_t x_pitch, uint8_t* __restrict__ lo, size_t lo_pitch, const int32_t* __restrict__ off,
-             long long ngroups, long long nbinned, int chan0, uint2* __restrict__ exc, unsigned* __restrict__ exc_cnt, unsigned cap) {
-    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= ngroups) return;
-    const int c = blockIdx.y;
-    const int oc = off[c];
-    const uint4 v = *reinterpret_cast<const uint4*>(x + (size_t)c * x_pitch + (size_t)g * 16);
-    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
-    uint32_t packed[2] = {0u, 0u};
-#pragma unroll
-    for (int k = 0; k < 16 / B; ++k) {
-        int s = 0;
-#pragma unroll
-        for (int j = 0; j < B; ++j) {
-            const int byte = k * B + j;
-            s += (int)((w[byte >> 2] >> (8 * (byte & 3))) & 0xFFu);
-        }
-        const int y = s - oc;
-        const int l = y < 0 ? 0 : (y > 255 ? 255 : y);
-        packed[k >> 2] |= (uint32_t)l << (8 * (k & 3));
-        const long long t = g * (16 / B) + k;
-        if (y != l && t < nbinned) {                                   /* rare: one atomic per exception */
-            const unsigned idx = atomicAdd(exc_cnt, 1u);
-            if (idx < cap) exc[idx] = make_uint2((uint32_t)(chan0 + c) | ((uint32_t)(y - l + 1024) << 16), (uint32_t)t);
-        }
-    }
-    uint8_t* dst = lo + (size_t)c * lo_pitch + (size_t)g * (16 / B);
-    if (B == 2) *reinterpret_cast<uint2*>(dst) = make_uint2(packed[0], packed[1]);
-    else *reinterpret_cast<uint32_t*>(dst) = packed[0];
-}
-
 /* D[i][t - delay(c, i)] += r for every exception (c, t, r) and every DM trial i of one range. The delay is reading C2
  * evaluated in IEEE double with explicit round-to-nearest operations, the same operation order as the host tables. */
 __global__ void __launch_bounds__(256)
@@ -220,6 +167,95 @@ k_scatter_exceptions(const uint2* __restrict__ exc, const unsigned* __restrict__
         const long long delay = llround(__ddiv_rn(__dmul_rn(k[c], dm), (double)bin));
         const long long t = (long long)rec.y - delay;
         if (t >= 0 && t < nt) atomicAdd(D + (size_t)i * (size_t)pitch + (size_t)t, r);
+    }
+}
+
+/* ---- K1 fused: ONE read of the raw chunk produces everything K2's TMA windows need: the 4 sample-shifted uint8 copies,
+ * the offset-uint8 forms of the bin-2 and bin-4 inputs (4 shifted byte copies each, exceptions appended), and the two
+ * copies of the uint16 bin-8 input. A thread owns 16 raw samples and looks 16 samples ahead for the shifted copies.
+ * (The uint16 forms of bin 2 / 4 are written by k_bin_time / k_shift_copy, only for exception-heavy chunks.) */
+struct PrepFused {
+    const uint8_t* raw; size_t pitch; long long ngroups; int chan0; unsigned cap;
+    uint8_t* x4; size_t x4_stride;
+    uint8_t* lo2; size_t lo2_pitch, lo2_stride; const int32_t* off2; uint2* exc2; unsigned* cnt2; long long nb2;
+    uint8_t* lo4; size_t lo4_pitch, lo4_stride; const int32_t* off4; uint2* exc4; unsigned* cnt4; long long nb4;
+    uint16_t* xb8; size_t xb8_pitch, xb8_stride;
+};
+
+__device__ __forceinline__ uint32_t byte_of(const uint32_t (&w)[8], int i) { return (w[i >> 2] >> (8 * (i & 3))) & 0xFFu; }
+
+__global__ void __launch_bounds__(256)
+k_prep_fused(const PrepFused p) {
+    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= p.ngroups) return;
+    const int c = blockIdx.y;
+    const uint8_t* src = p.raw + (size_t)c * p.pitch + (size_t)g * 16;
+    const uint4 a = *reinterpret_cast<const uint4*>(src);
+    const uint4 n = *reinterpret_cast<const uint4*>(src + 16);          /* rows are padded: readable past the chunk */
+    const uint32_t w[8] = {a.x, a.y, a.z, a.w, n.x, n.y, n.z, n.w};
+    if (p.x4) {
+        const size_t off = (size_t)c * p.pitch + (size_t)g * 16;
+        *reinterpret_cast<uint4*>(p.x4 + off) = a;
+#pragma unroll
+        for (int k = 1; k < 4; ++k) {
+            uint4 o;
+            o.x = __funnelshift_r(a.x, a.y, 8 * k); o.y = __funnelshift_r(a.y, a.z, 8 * k);
+            o.z = __funnelshift_r(a.z, a.w, 8 * k); o.w = __funnelshift_r(a.w, n.x, 8 * k);
+            *reinterpret_cast<uint4*>(p.x4 + (size_t)k * p.x4_stride + off) = o;
+        }
+    }
+    if (p.lo2) {
+        const int oc = p.off2[c];
+        uint32_t l[11];
+#pragma unroll
+        for (int k = 0; k < 11; ++k) {
+            const int y = (int)(byte_of(w, 2 * k) + byte_of(w, 2 * k + 1)) - oc;
+            const int v = y < 0 ? 0 : (y > 255 ? 255 : y);
+            l[k] = (uint32_t)v;
+            const long long t = g * 8 + k;
+            if (k < 8 && y != v && t < p.nb2) {
+                const unsigned idx = atomicAdd(p.cnt2, 1u);
+                if (idx < p.cap) p.exc2[idx] = make_uint2((uint32_t)(p.chan0 + c) | ((uint32_t)(y - v + 1024) << 16), (uint32_t)t);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t lo = l[j] | (l[j + 1] << 8) | (l[j + 2] << 16) | (l[j + 3] << 24);
+            const uint32_t hi = l[j + 4] | (l[j + 5] << 8) | (l[j + 6] << 16) | (l[j + 7] << 24);
+            *reinterpret_cast<uint2*>(p.lo2 + (size_t)j * p.lo2_stride + (size_t)c * p.lo2_pitch + (size_t)g * 8) = make_uint2(lo, hi);
+        }
+    }
+    if (p.lo4) {
+        const int oc = p.off4[c];
+        uint32_t l[7];
+#pragma unroll
+        for (int k = 0; k < 7; ++k) {
+            const int y = (int)(byte_of(w, 4 * k) + byte_of(w, 4 * k + 1) + byte_of(w, 4 * k + 2) + byte_of(w, 4 * k + 3)) - oc;
+            const int v = y < 0 ? 0 : (y > 255 ? 255 : y);
+            l[k] = (uint32_t)v;
+            const long long t = g * 4 + k;
+            if (k < 4 && y != v && t < p.nb4) {
+                const unsigned idx = atomicAdd(p.cnt4, 1u);
+                if (idx < p.cap) p.exc4[idx] = make_uint2((uint32_t)(p.chan0 + c) | ((uint32_t)(y - v + 1024) << 16), (uint32_t)t);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            *reinterpret_cast<uint32_t*>(p.lo4 + (size_t)j * p.lo4_stride + (size_t)c * p.lo4_pitch + (size_t)g * 4) =
+                l[j] | (l[j + 1] << 8) | (l[j + 2] << 16) | (l[j + 3] << 24);
+    }
+    if (p.xb8) {
+        uint32_t s8[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            uint32_t t = 0;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) t += byte_of(w, 8 * k + j);
+            s8[k] = t;
+        }
+        uint8_t* d0 = reinterpret_cast<uint8_t*>(p.xb8 + (size_t)c * p.xb8_pitch + (size_t)g * 2);
+        *reinterpret_cast<uint32_t*>(d0) = s8[0] | (s8[1] << 16);
+        *reinterpret_cast<uint32_t*>(d0 + p.xb8_stride) = s8[1] | (s8[2] << 16);
     }
 }
 
@@ -307,15 +343,6 @@ extern "C" int aak_shift_copy(const uint8_t* in, uint8_t* out, size_t pitch, siz
     return (int)cudaGetLastError();
 }
 
-extern "C" int aak_make_copies_u8(const uint8_t* in, uint8_t* out, size_t pitch, size_t copy_stride, size_t row_bytes, int32_t nrows,
-                                  void* stream) {
-    if ((row_bytes & 15) || (pitch & 15) || (copy_stride & 15)) return (int)cudaErrorInvalidValue;
-    const long long ngroups = (long long)(row_bytes / 16);
-    dim3 grid((unsigned)((ngroups + 255) / 256), (unsigned)nrows);
-    k_make_copies_u8<<<grid, 256, 0, (cudaStream_t)stream>>>(in, out, pitch, copy_stride, ngroups);
-    return (int)cudaGetLastError();
-}
-
 extern "C" int aak_row_moments(const int32_t* D, int64_t pitch, int64_t nt, int32_t ndms, long long* sum_d, long long* sum_td,
                                void* stream) {
     k_row_moments<<<(unsigned)ndms, 256, 0, (cudaStream_t)stream>>>(D, pitch, nt, sum_d, sum_td);
@@ -346,19 +373,21 @@ extern "C" int aak_chan_offsets(const uint8_t* x, size_t pitch, int64_t len, int
     return (int)cudaGetLastError();
 }
 
-extern "C" int aak_bin_offset(const uint8_t* x, size_t x_pitch, uint8_t* lo, size_t lo_pitch, const int32_t* off, int32_t nrows,
-                              int32_t chan0, int64_t nbinned, int32_t bin, uint2* exc, unsigned* exc_cnt, unsigned cap, void* stream) {
-    cudaStream_t st = (cudaStream_t)stream;
-    const long long ngroups = (nbinned * bin + 15) / 16;
-    dim3 grid((unsigned)((ngroups + 255) / 256), (unsigned)nrows);
-    if (bin == 2) k_bin_offset<2><<<grid, 256, 0, st>>>(x, x_pitch, lo, lo_pitch, off, ngroups, nbinned, chan0, exc, exc_cnt, cap);
-    else if (bin == 4) k_bin_offset<4><<<grid, 256, 0, st>>>(x, x_pitch, lo, lo_pitch, off, ngroups, nbinned, chan0, exc, exc_cnt, cap);
-    else return (int)cudaErrorInvalidValue;
-    return (int)cudaGetLastError();
-}
-
 extern "C" int aak_scatter_exceptions(const uint2* exc, const unsigned* exc_cnt, unsigned cap, const double* k, double dm_low,
                                       double dm_step, int32_t ndms, int32_t bin, int64_t nt, int32_t* D, int64_t pitch, void* stream) {
     k_scatter_exceptions<<<148 * 4, 256, 0, (cudaStream_t)stream>>>(exc, exc_cnt, cap, k, dm_low, dm_step, ndms, bin, nt, D, pitch);
+    return (int)cudaGetLastError();
+}
+
+extern "C" int aak_prep_fused(const aak_prep_args* a, int32_t nrows, void* stream) {
+    if (nrows <= 0 || a->ngroups <= 0) return 0;
+    PrepFused p;
+    p.raw = a->raw; p.pitch = a->pitch; p.ngroups = a->ngroups; p.chan0 = a->chan0; p.cap = a->cap;
+    p.x4 = a->x4; p.x4_stride = a->x4_stride;
+    p.lo2 = a->lo2; p.lo2_pitch = a->lo2_pitch; p.lo2_stride = a->lo2_stride; p.off2 = a->off2; p.exc2 = a->exc2; p.cnt2 = a->cnt2; p.nb2 = a->nb2;
+    p.lo4 = a->lo4; p.lo4_pitch = a->lo4_pitch; p.lo4_stride = a->lo4_stride; p.off4 = a->off4; p.exc4 = a->exc4; p.cnt4 = a->cnt4; p.nb4 = a->nb4;
+    p.xb8 = a->xb8; p.xb8_pitch = a->xb8_pitch; p.xb8_stride = a->xb8_stride;
+    dim3 grid((unsigned)((a->ngroups + 255) / 256), (unsigned)nrows);
+    k_prep_fused<<<grid, 256, 0, (cudaStream_t)stream>>>(p);
     return (int)cudaGetLastError();
 }
