@@ -197,3 +197,43 @@ def test_null_arguments_are_rejected():
     assert aa.aa_last_error() != ""
     lib.aa_plan_destroy(None)          # destroying NULL is a no-op (graceful exit)
     lib.aa_strategy_destroy(None)
+
+
+def test_header_is_plain_c_and_links_from_c(tmp_path):
+    """The boundary is a C ABI (no C++ in the header): a C99 translation unit that includes include/aa.h compiles with
+    -Wall -Werror -pedantic, links against libaa.so and gets the documented error feedback without touching a GPU."""
+    import subprocess
+    src = tmp_path / "use_aa.c"
+    src.write_text(r'''
+#include <stdio.h>
+#include <string.h>
+#include "aa.h"
+int main(void) {
+    aa_plan* plan = NULL;
+    double f[3] = {1500.0, 1499.0, 1498.0};
+    aa_dm_range r = {0.0, 1.0, 4, 2};
+    int32_t w[2] = {1, 2};
+    if (aa_plan_create(&plan, 3, f, 64e-6, &r, 1, w, 2, 6.0f) != AA_OK) return 1;
+    if (aa_plan_set_input_layout(plan, AA_LAYOUT_TIME_MAJOR) != AA_OK) return 2;
+    if (aa_plan_set_input_layout(plan, 5) != AA_ERR_INVALID_ARG || !strstr(aa_last_error(), "layout")) return 3;
+    aa_strategy* st = NULL;
+    if (aa_strategy_plan(&st, plan, 4096, 0, 16, 0) != AA_OK) return 4;
+    aa_strategy_info info;
+    if (aa_strategy_get_info(st, &info) != AA_OK || info.ready != 0 || info.max_bin != 2 || info.input_layout != AA_LAYOUT_TIME_MAJOR) return 5;
+    if (aa_run_sps(st) != AA_ERR_NOT_READY) return 6;
+    r.bin = 3;
+    aa_plan* bad = NULL;
+    if (aa_plan_create(&bad, 3, f, 64e-6, &r, 1, w, 2, 6.0f) != AA_ERR_INVALID_ARG || !strstr(aa_last_error(), "bin")) return 7;
+    aa_strategy_destroy(st);
+    aa_plan_destroy(plan);
+    printf("%s\n", aa_version());
+    return 0;
+}
+''')
+    exe = tmp_path / "use_aa"
+    libdir = aa.lib_path().parent
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-pedantic", f"-I{ROOT / 'include'}", str(src), "-o", str(exe),
+                           f"-L{libdir}", "-l:libaa.so", f"-Wl,-rpath,{libdir}"])
+    out = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert out.returncode == 0, (out.returncode, out.stdout, out.stderr)
+    assert "sm_100a" in out.stdout
