@@ -211,6 +211,26 @@ aa_status aa_run_pipeline(aa_strategy* s, const uint8_t* host_input, size_t row_
  * count is in aa_last_error()). */
 aa_status aa_get_candidates(aa_strategy* s, const aa_candidate** out, size_t* n);
 
+/* Candidate clustering (reading C10): one bright pulse yields many candidates (neighbouring DM
+ * trials, widths, DM ranges, chunk edges). Two candidates are LINKED iff |dm_a - dm_b| <= dm_tol and their boxcars,
+ * [sample, sample + width), are at most `gap` samples apart (sample_a <= sample_b + width_b + gap and vice versa);
+ * clusters are the connected components of that relation over ALL candidates gathered so far (any range, any chunk).
+ * Each cluster is reported by its member of highest SNR (first by (range, dm_index, sample) on ties) plus its extent.
+ * Host-side, on the library-owned list; *out stays valid until the next aa_run_*, aa_get_clusters, reset or destroy.
+ * Clusters are ordered by (range, dm_index, sample) of their representatives. Errors: as aa_get_candidates, and
+ * AA_ERR_INVALID_ARG for a negative or non-finite dm_tol. */
+typedef struct {
+    aa_candidate best;          /* the member with the highest SNR */
+    uint32_t members;           /* number of candidates in the cluster */
+    float dm_min, dm_max;       /* extent over the members */
+    uint64_t sample_min;        /* earliest boxcar start */
+    uint64_t sample_end;        /* latest boxcar end (sample + width), exclusive */
+} aa_cluster;
+aa_status aa_get_clusters(aa_strategy* s, double dm_tol, uint64_t gap, const aa_cluster** out, size_t* n);
+/* The same relation on a caller-supplied list (HOST, any order); results land in caller memory `out` of capacity >= n.
+ * Returns the number of clusters through *nout. Needs no strategy and no GPU. */
+aa_status aa_cluster_candidates(const aa_candidate* in, size_t n, double dm_tol, uint64_t gap, aa_cluster* out, size_t* nout);
+
 /* Parity hooks: copy one row of the CURRENT chunk (the one last dedispersed / searched) to library-owned HOST memory:
  * nt + boxcar_extra samples. Valid until the next call on this strategy. */
 aa_status aa_get_dedispersed_row(aa_strategy* s, int32_t range, int32_t dm_index, const int32_t** host_row, size_t* len);

@@ -183,3 +183,37 @@ def search_rows(xb: np.ndarray, k: np.ndarray, rng, range_index: int, T: int, wi
     if S is not None: out["S"] = S
     if W is not None: out["w"] = W
     return out
+
+
+def cluster_candidates(cands: np.ndarray, dm_tol: float, gap: int):
+    """Reading C10, the definition written out in O(n^2): candidates a, b are linked iff |dm_a - dm_b| <= dm_tol
+    and sample_a <= sample_b + width_b + gap and sample_b <= sample_a + width_a + gap; clusters are the connected
+    components. Returns a list of clusters, each a sorted list of member indices, plus the representative index of each
+    (highest snr; first by (range, dm_index, sample) on ties). Pure Python: small lists only."""
+    n = len(cands)
+    s = [int(v) for v in cands["sample"]]
+    w = [int(v) for v in cands["width"]]
+    dm = [float(v) for v in cands["dm"]]
+    adj = [[] for _ in range(n)]
+    for a in range(n):
+        for b in range(a + 1, n):
+            if abs(dm[a] - dm[b]) <= dm_tol and s[a] <= s[b] + w[b] + gap and s[b] <= s[a] + w[a] + gap:
+                adj[a].append(b)
+                adj[b].append(a)
+    seen, clusters = [False] * n, []
+    for a in range(n):
+        if seen[a]:
+            continue
+        comp, stack = [], [a]
+        seen[a] = True
+        while stack:
+            u = stack.pop()
+            comp.append(u)
+            for v in adj[u]:
+                if not seen[v]:
+                    seen[v] = True
+                    stack.append(v)
+        clusters.append(sorted(comp))
+    key = lambda i: (-float(cands["snr"][i]), int(cands["range"][i]), int(cands["dm_index"][i]), int(cands["sample"][i]))
+    reps = [min(c, key=key) for c in clusters]
+    return clusters, reps

@@ -19,7 +19,7 @@ __all__ = [
     "CANDIDATE_DTYPE", "lib_path", "load",
     "AA_LAYOUT_CHANNEL_MAJOR", "AA_LAYOUT_TIME_MAJOR", "aa_plan_create", "aa_plan_destroy", "aa_plan_set_input_layout", "aa_plan_set_boxcar_overlap", "aa_strategy_plan", "aa_strategy_setup", "aa_strategy_destroy", "aa_strategy_get_info",
     "aa_strategy_get_range_info", "aa_strategy_get_chunk", "aa_strategy_get_delay", "aa_strategy_describe",
-    "aa_strategy_reset", "aa_strategy_shard", "aa_run_dedispersion", "aa_run_dedispersion_device", "aa_run_sps", "aa_run_pipeline", "aa_get_candidates",
+    "aa_strategy_reset", "aa_strategy_shard", "aa_run_dedispersion", "aa_run_dedispersion_device", "aa_run_sps", "aa_run_pipeline", "aa_get_candidates", "aa_get_clusters", "aa_cluster_candidates", "CLUSTER_DTYPE",
     "aa_get_dedispersed_row", "aa_get_row_stats", "aa_get_row_moments", "aa_get_dedispersed_device", "aa_synchronize",
     "aa_measure_int_add_peak", "aa_measure_int_add_peak3", "aa_get_last_timings", "aa_get_launch_count", "aa_last_error", "aa_version",
     "Plan", "Strategy",
@@ -30,8 +30,13 @@ AA_ERR_INVALID_ARG, AA_ERR_NOT_READY, AA_ERR_BUDGET_TOO_SMALL, AA_ERR_CUDA = -1,
 AA_ERR_CANDIDATE_OVERFLOW, AA_ERR_ORDER, AA_ERR_INTERNAL = -5, -6, -7
 AA_LAYOUT_CHANNEL_MAJOR, AA_LAYOUT_TIME_MAJOR = 0, 1
 
+CLUSTER_DTYPE = None  # defined below CANDIDATE_DTYPE
 CANDIDATE_DTYPE = np.dtype([("sample", np.uint64), ("dm", np.float32), ("snr", np.float32), ("width", np.uint32),
                             ("range", np.uint32), ("dm_index", np.uint32)], align=True)
+
+
+CLUSTER_DTYPE = np.dtype([("best", CANDIDATE_DTYPE), ("members", np.uint32), ("dm_min", np.float32), ("dm_max", np.float32),
+                          ("sample_min", np.uint64), ("sample_end", np.uint64)], align=True)
 
 
 class AaError(RuntimeError):
@@ -101,6 +106,8 @@ def load():
         "aa_run_sps": (c_int32, [vp]),
         "aa_run_pipeline": (c_int32, [vp, vp, c_size_t]),
         "aa_get_candidates": (c_int32, [vp, POINTER(vp), POINTER(c_size_t)]),
+        "aa_get_clusters": (c_int32, [vp, c_double, c_uint64, POINTER(vp), POINTER(c_size_t)]),
+        "aa_cluster_candidates": (c_int32, [vp, c_size_t, c_double, c_uint64, vp, POINTER(c_size_t)]),
         "aa_get_dedispersed_row": (c_int32, [vp, c_int32, c_int32, POINTER(vp), POINTER(c_size_t)]),
         "aa_get_row_stats": (c_int32, [vp, c_int32, c_int32, POINTER(c_double), POINTER(c_double), POINTER(c_int64), POINTER(c_int32)]),
         "aa_get_row_moments": (c_int32, [vp, c_int32, vp, vp]),
@@ -265,6 +272,27 @@ def aa_get_candidates(strategy, allow_overflow: bool = False) -> np.ndarray:
         return np.zeros(0, dtype=CANDIDATE_DTYPE)
     buf = (ctypes.c_char * (n.value * CANDIDATE_DTYPE.itemsize)).from_address(p.value)
     return np.frombuffer(buf, dtype=CANDIDATE_DTYPE).copy()
+
+
+def aa_get_clusters(strategy, dm_tol: float, gap: int, allow_overflow: bool = False) -> np.ndarray:
+    """Clusters of all candidates gathered so far (a copy), see include/aa.h."""
+    p, n = c_void_p(), c_size_t()
+    _check(load().aa_get_clusters(strategy, float(dm_tol), int(gap), byref(p), byref(n)),
+           allow=(AA_ERR_CANDIDATE_OVERFLOW,) if allow_overflow else ())
+    if n.value == 0:
+        return np.zeros(0, dtype=CLUSTER_DTYPE)
+    buf = (ctypes.c_char * (n.value * CLUSTER_DTYPE.itemsize)).from_address(p.value)
+    return np.frombuffer(buf, dtype=CLUSTER_DTYPE).copy()
+
+
+def aa_cluster_candidates(cands: np.ndarray, dm_tol: float, gap: int) -> np.ndarray:
+    """The same clustering on any candidate array (host only, no strategy, no GPU)."""
+    c = np.ascontiguousarray(cands, dtype=CANDIDATE_DTYPE)
+    out = np.zeros(len(c), dtype=CLUSTER_DTYPE)
+    n = c_size_t()
+    _check(load().aa_cluster_candidates(c.ctypes.data if len(c) else None, len(c), float(dm_tol), int(gap),
+                                        out.ctypes.data if len(c) else None, byref(n)))
+    return out[:n.value].copy()
 
 
 def aa_get_dedispersed_row(strategy, rng: int, dm_index: int) -> np.ndarray:

@@ -151,6 +151,7 @@ struct Strategy {
     /* host results */
     unsigned long long* h_counter = nullptr;    /* pinned */
     std::vector<aa_candidate> cands;
+    std::vector<aa_cluster> clusters;
     uint64_t true_count = 0;
     bool overflow = false;
     std::vector<int32_t> host_row;

@@ -275,3 +275,24 @@ def test_boxcar_complete_chunks_match_the_oracle_and_recover_a_straddling_pulse(
     finally:
         gpu.close()
         plain.close()
+
+
+def test_clusters_of_the_tiny_pulse():
+    """Reading C10 on real output: the injected pulse of the Tiny config produces ~20 candidates along its bow-tie in the
+    (DM, time) plane; linked with a 2-DM-step / 8-sample tolerance the ones around the pulse merge into a cluster whose representative is
+    the pulse itself, and the library's clusters equal the oracle's written-out definition on the same list."""
+    import oracle
+    w = datagen.get_workload("tiny")
+    x, _ = make_input(w)
+    g = GpuRun(w, x)
+    try:
+        cands = g.st.run(x)
+        cl = g.aa.aa_get_clusters(g.h, 2.0, 8)
+        clusters, reps = oracle.cluster_candidates(cands, 2.0, 8)
+        assert len(cl) == len(clusters) and int(cl["members"].sum()) == len(cands)
+        top = cl[np.argmax(cl["best"]["snr"])]
+        assert int(top["members"]) >= 2 and len(cl) < len(cands)
+        assert abs(int(top["best"]["dm_index"]) - 50) <= 1 and abs(int(top["best"]["sample"]) - 3000) <= 1 and int(top["best"]["width"]) == 4
+        assert sorted(int(cands["sample"][r]) for r in reps) == sorted(int(s) for s in cl["best"]["sample"])
+    finally:
+        g.close()
