@@ -21,7 +21,7 @@ namespace aa {
 void set_error(const char* fmt, ...);
 aa_status cuda_fail(cudaError_t e, const char* what);
 
-constexpr int kDmTile = 32;       /* must match k_dedisp.cu */
+constexpr int kDmTile = 32;       /* row length of K2's offset table = the largest DM tile (must match k_dedisp.cu) */
 constexpr int kTTile = 1024;
 constexpr int kMaxGroups = 4;
 constexpr unsigned kExcCap = 1u << 20;   /* exception records per (bin, channel group) */      /* channel groups of a pipelined (not prefetched) chunk copy */
@@ -57,6 +57,7 @@ struct Arena {
 struct K2Plan {
     int32_t in16 = 0, esz = 1, spw = 4, ncopy = 4;
     int32_t chan_block = 8, window_bytes = 0, spill_stages = 0, nstages = 0;
+    int32_t dm_tile = 32, ndm_tiles = 0;                      /* DM trials per CTA (32 or 30) and the number of DM tiles */
     int32_t dms_per_warp = 2, variant = 1, ring_stages = 3;   /* K2 tuning chosen by the strategy */
     int32_t* d_etab = nullptr;
     int32_t* d_x0tab = nullptr;
@@ -70,7 +71,6 @@ struct Range : K2Plan {           /* the base is the range's main plan: uint8 fo
     int64_t nt_full = 0;          /* T_r of a full chunk */
     int32_t extra = 0;            /* E: samples dedispersed beyond T_r (reading C3x), 0 by default */
     int64_t pitch = 0;            /* D row pitch, elements */
-    int32_t ndm_tiles = 0;
     std::vector<int32_t> delays;  /* [ndms][nchans], binned samples (host) */
     int32_t* d_D = nullptr;
     size_t first_row = 0;         /* index of this range's first row in the row tables */

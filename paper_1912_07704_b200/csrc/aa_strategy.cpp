@@ -106,11 +106,11 @@ static void carve(Strategy& s, int64_t L, bool two_raw) {
         rg.nt_full = n_out / rg.r.bin;
         rg.pitch = (int64_t)round_up((size_t)(rg.nt_full + rg.extra), 128);
         rg.d_D = (int32_t*)a.take((size_t)rg.r.ndms * (size_t)rg.pitch * 4);
-        rg.d_etab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * kDmTile * 4);
+        rg.d_etab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * kDmTile * 4);   /* rg. = the main plan */
         rg.d_x0tab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * 4);
         if (rg.has_lo) {
-            rg.lo.d_etab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.lo.nstages * rg.lo.chan_block * kDmTile * 4);
-            rg.lo.d_x0tab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.lo.nstages * rg.lo.chan_block * 4);
+            rg.lo.d_etab = (int32_t*)a.take((size_t)rg.lo.ndm_tiles * rg.lo.nstages * rg.lo.chan_block * kDmTile * 4);
+            rg.lo.d_x0tab = (int32_t*)a.take((size_t)rg.lo.ndm_tiles * rg.lo.nstages * rg.lo.chan_block * 4);
         }
     }
     s.d_rows[0] = (aak_row_desc*)a.take(s.nrows * sizeof(aak_row_desc));
@@ -144,10 +144,18 @@ static std::vector<Chunk> make_chunks(uint64_t nsamp, int64_t B, int64_t S, int6
 static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16, std::vector<int32_t>& etab, std::vector<int32_t>& x0tab) {
     const int32_t C = s.plan.nchans, nd = rg.r.ndms;
     p.in16 = in16; p.esz = in16 ? 2 : 1; p.spw = 4 / p.esz; p.ncopy = p.spw;
+    /* uint8 samples: 15 compute warps x 2 trials (+ the producer = 16 warps, 128 registers per thread, 30 trials per CTA):
+     * measured 216.6 -> 204.9 ms on SKA-like against 16 + 1 warps at 96 registers (11 or 7 warps are slower again);
+     * binned uint16 samples: 16 warps x (4 adjacent trials, half the tile), 32 trials per CTA */
+    p.dm_tile = in16 ? kDmTile : 30;
+#ifdef AA_TUNING
+    if (!in16) if (const char* ev = getenv("AA_K2_W15")) p.dm_tile = atoi(ev) ? 30 : kDmTile;
+#endif
+    p.ndm_tiles = (nd + p.dm_tile - 1) / p.dm_tile;
     /* widest window: T_TILE + largest in-tile delay spread + alignment residue (< 16 bytes) */
     int64_t omax = 0;
-    for (int32_t t = 0; t < rg.ndm_tiles; ++t) {
-        const int32_t i0 = t * kDmTile, i1 = std::min(nd - 1, i0 + kDmTile - 1);
+    for (int32_t t = 0; t < p.ndm_tiles; ++t) {
+        const int32_t i0 = t * p.dm_tile, i1 = std::min(nd - 1, i0 + p.dm_tile - 1);
         const int32_t* a = rg.delays.data() + (size_t)i0 * C;
         const int32_t* b = rg.delays.data() + (size_t)i1 * C;
         for (int32_t c = 0; c < C; ++c) omax = std::max<int64_t>(omax, (int64_t)b[c] - a[c]);
@@ -189,10 +197,10 @@ static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16,
     /* 16-bit lanes are carried every 65536 / (largest sample value + 1) channels: bytes 256, uint16 sums of b bytes 256/b */
     p.spill_stages = (in16 ? 256 / rg.r.bin : 256) / p.chan_block;
     const int32_t CB = p.chan_block, Cpad = p.nstages * CB, WB = p.window_bytes;
-    etab.assign((size_t)rg.ndm_tiles * Cpad * kDmTile, 0);
-    x0tab.assign((size_t)rg.ndm_tiles * Cpad, 0);
-    for (int32_t t = 0; t < rg.ndm_tiles; ++t) {
-        const int32_t i0 = t * kDmTile;
+    etab.assign((size_t)p.ndm_tiles * Cpad * kDmTile, 0);
+    x0tab.assign((size_t)p.ndm_tiles * Cpad, 0);
+    for (int32_t t = 0; t < p.ndm_tiles; ++t) {
+        const int32_t i0 = t * p.dm_tile;
         for (int32_t c = 0; c < Cpad; ++c) {
             int32_t* e = etab.data() + ((size_t)t * Cpad + c) * kDmTile;     /* [tile][stage][c_local][m] */
             const int32_t cl = c % CB;
@@ -230,7 +238,6 @@ static bool plan_range(Strategy& s, Range& rg, std::vector<int32_t>& etab, std::
         }
     }
     rg.max_delay = rg.delays[(size_t)(nd - 1) * C + (C - 1)];
-    rg.ndm_tiles = (nd + kDmTile - 1) / kDmTile;
     if (!plan_format(s, rg, rg, rg.r.bin > 1, etab, x0tab)) return false;
     /* bin 2 and 4 also get the offset-uint8 route (half the shared-memory bytes per add); the uint16 plan above stays as
      * the route for chunks with too many exceptions. C < 65536 so a channel index fits the exception record. */
@@ -483,7 +490,7 @@ extern "C" aa_status aa_strategy_get_range_info(const aa_strategy* h, int32_t ra
     if (!out || range < 0 || range >= (int32_t)h->s.ranges.size()) { set_error("aa_strategy_get_range_info: range %d out of bounds", range); return AA_ERR_INVALID_ARG; }
     const Range& rg = h->s.ranges[(size_t)range];
     out->ndms = rg.r.ndms; out->bin = rg.r.bin; out->nt = rg.nt_full; out->row_pitch = rg.pitch; out->max_delay = rg.max_delay;
-    out->dm_tile = kDmTile; out->t_tile = kTTile; out->chan_block = rg.chan_block; out->window = rg.window_bytes;
+    out->dm_tile = rg.dm_tile; out->t_tile = kTTile; out->chan_block = rg.chan_block; out->window = rg.window_bytes;
     out->boxcar_extra = rg.extra;
     return AA_OK;
 }
@@ -524,7 +531,7 @@ extern "C" size_t aa_strategy_describe(const aa_strategy* h, char* buf, size_t b
                  "range %d: dm_low=%g step=%g ndms=%d bin=%d max_delay=%lld T=%lld pitch=%lld | tile %dx%d chan_block=%d window=%dB stages=%d "
                  "dm_tiles=%d spill/%d smem=%zuB\n",
                  rg.index, rg.r.dm_low, rg.r.dm_step, rg.r.ndms, rg.r.bin, (long long)rg.max_delay, (long long)rg.nt_full, (long long)rg.pitch,
-                 kDmTile, kTTile, rg.chan_block, rg.window_bytes, rg.nstages, rg.ndm_tiles, rg.spill_stages,
+                 rg.dm_tile, kTTile, rg.chan_block, rg.window_bytes, rg.nstages, rg.ndm_tiles, rg.spill_stages,
                  aak_dedisperse_smem_bytes(rg.chan_block, rg.window_bytes, rg.in16, rg.ring_stages));
         o += line;
         if (rg.has_lo) {

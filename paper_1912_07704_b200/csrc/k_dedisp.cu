@@ -4,8 +4,11 @@
  *   D[i][t] = sum_{c<C} x_b[c][t + delay(c,i)]          (BASELINE.json north_star; every term is added individually)
  *
  * Design:
- *   * A CTA owns DM_TILE = 32 DM trials x T_TILE = 1024 output samples. 16 compute warps each hold 2 DMs x 1024 samples
- *     in registers; a 17th warp is the TMA producer. Channels stream through shared memory in blocks of CB channels,
+ *   * A CTA owns 30 or 32 DM trials x T_TILE = 1024 output samples, held in registers by its compute warps; one more
+ *     warp is the TMA producer. uint8 input: 15 compute warps x (2 DMs x 1024 samples) + producer = 16 warps, so a thread
+ *     may use 128 registers (measured 5 % faster than 16 + 1 warps at 96 registers: ptxas keeps more shared-memory loads
+ *     in flight). Binned uint16 input: 16 compute warps x (4 adjacent DMs x 512 samples) + producer.
+ *     Channels stream through shared memory in blocks of CB channels,
  *     NSTAGE-deep ring, full/empty mbarriers (no __syncthreads in the main loop).
  *   * Shared memory holds SPW sample-shifted copies of every channel window (SPW = samples per 32-bit word: 4 for uint8,
  *     2 for uint16), so that ANY sample offset t+delay is a word-aligned, bank-conflict-free LDS.32: copy k holds the
@@ -39,8 +42,7 @@
 
 namespace {
 
-constexpr int NW = 16;               /* compute warps */
-constexpr int DM_TILE = 32;          /* DM trials per CTA */
+constexpr int DM_TILE = 32;          /* row length of the offset table: at most this many DM trials per CTA */
 constexpr int T_TILE = 1024;         /* output samples per CTA */
 #ifndef AA_PRODUCER_SLEEP_NS
 #define AA_PRODUCER_SLEEP_NS 400
@@ -50,7 +52,6 @@ constexpr int T_TILE = 1024;         /* output samples per CTA */
 #endif
 constexpr int PRODUCER_SLEEP_NS = AA_PRODUCER_SLEEP_NS, CONSUMER_SLEEP_NS = AA_CONSUMER_SLEEP_NS;
 constexpr int MAX_RING = 8;          /* shared-memory ring depth is a launch parameter (2..MAX_RING) */
-constexpr int NTHREADS = (NW + 1) * 32;
 constexpr int SMEM_HEADER = 1024;    /* mbarriers live here; keeps the stages 1024-byte aligned */
 
 
@@ -133,14 +134,18 @@ __device__ __forceinline__ uint32_t odd_bytes(uint32_t w) { /* (b1, 0, b3, 0) */
  * Adjacent DM trials often have the SAME delay in a channel (the delay grows by less than one sample per DM step over
  * much of the band): the words loaded for trial m-1 are then exactly the words trial m needs, and are reused from
  * registers instead of being read from shared memory again (a warp-uniform test of two table entries). */
-template <int IN16, int CB, int FMA_H, int M>
-__global__ void __launch_bounds__(NTHREADS, 1)
+/* NWC = compute warps: 16 (+1 producer = 17 warps, 96 registers per thread) or 15 (+1 = 16 warps, 128 registers per
+ * thread, 30 trials per CTA: the extra registers let ptxas keep more shared-memory loads in flight). */
+template <int IN16, int CB, int FMA_H, int M, int NWC>
+__global__ void __launch_bounds__((NWC + 1) * 32, 1)
 k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
     constexpr int ESZ = IN16 ? 2 : 1;
     constexpr int SPW = 4 / ESZ;                 /* samples per word */
     constexpr int NCOPY = SPW;                   /* shifted copies */
-    constexpr int NG = DM_TILE / M;              /* DM groups */
+    constexpr int NW = NWC;
+    constexpr int NG = (M == 2) ? NWC : DM_TILE / M;   /* DM groups */
     constexpr int NTH = NW / NG;                 /* time parts */
+    constexpr int DMT = NG * M;                  /* DM trials per CTA: 32 or 30 */
     constexpr int T_PART = T_TILE / NTH;
     constexpr int J = T_PART / (32 * SPW);       /* words per thread per DM */
     constexpr int ENT_BYTES = CB * DM_TILE * 4;
@@ -149,7 +154,7 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
     if (p.mode_cnt && ((*p.mode_cnt > p.mode_cap) ? 1 : 0) != p.mode_dense) return;     /* the other input format handles this chunk */
     extern __shared__ __align__(1024) uint8_t smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int ndm_tiles = (p.ndms + DM_TILE - 1) / DM_TILE;
+    const int ndm_tiles = (p.ndms + DMT - 1) / DMT;
     const int dt = blockIdx.x % ndm_tiles;       /* DM tile fastest: concurrent CTAs share the same input windows in L2 */
     const int tt = blockIdx.x / ndm_tiles;
     const long long t0 = (long long)tt * T_TILE;
@@ -309,7 +314,7 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
     const int bias = p.bias ? *p.bias : 0;
 #pragma unroll
     for (int m = 0; m < M; ++m) {
-        const int i = dt * DM_TILE + grp * M + m;
+        const int i = dt * DMT + grp * M + m;
         if (i >= p.ndms) continue;
         int32_t* row = p.D + (size_t)i * (size_t)p.pitch;
 #pragma unroll
@@ -354,7 +359,7 @@ __global__ void k_dedisperse_naive(const T* __restrict__ x, size_t pitch, const 
     D[(size_t)i * dpitch + t] = acc;
 }
 
-template <int IN16, int CB, int FMA_H, int M>
+template <int IN16, int CB, int FMA_H, int M, int NWC>
 int launch(const aak_dedisp_args* a, cudaStream_t st) {
     constexpr int NCOPY = IN16 ? 2 : 4;
     DedispParams p;
@@ -369,19 +374,21 @@ int launch(const aak_dedisp_args* a, cudaStream_t st) {
     p.nring = a->ring_stages;
     if (p.nring < 2 || p.nring > MAX_RING) return (int)cudaErrorInvalidValue;
     const size_t smem = SMEM_HEADER + (size_t)p.nring * ((size_t)NCOPY * CB * a->window_bytes + CB * DM_TILE * 4);
-    const long long ndm_tiles = (a->ndms + DM_TILE - 1) / DM_TILE;
+    constexpr int DMT = (M == 2) ? 2 * NWC : DM_TILE;
+    if (a->dm_tile != DMT) return (int)cudaErrorInvalidValue;
+    const long long ndm_tiles = (a->ndms + DMT - 1) / DMT;
     const long long nt_tiles = (a->nt + T_TILE - 1) / T_TILE;
     const long long grid = ndm_tiles * nt_tiles;
     if (grid <= 0 || grid > 0x7fffffffll) return (int)cudaErrorInvalidConfiguration;
     CUtensorMap map;
     memcpy(&map, a->tmap, sizeof(CUtensorMap));
-    k_dedisperse<IN16, CB, FMA_H, M><<<(unsigned)grid, NTHREADS, smem, st>>>(map, p);
+    k_dedisperse<IN16, CB, FMA_H, M, NWC><<<(unsigned)grid, (NWC + 1) * 32, smem, st>>>(map, p);
     return (int)cudaGetLastError();
 }
 
-template <int IN16, int CB, int FMA_H, int M>
+template <int IN16, int CB, int FMA_H, int M, int NWC>
 int set_attr() {
-    return (int)cudaFuncSetAttribute(k_dedisperse<IN16, CB, FMA_H, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    return (int)cudaFuncSetAttribute(k_dedisperse<IN16, CB, FMA_H, M, NWC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
 }
 
 }  // namespace
@@ -392,13 +399,16 @@ extern "C" size_t aak_dedisperse_smem_bytes(int32_t chan_block, int32_t window_b
 }
 
 #define AA_FOR_ALL_VARIANTS(X) \
-    X(0, 8, 0, 2) X(0, 4, 0, 2) X(0, 2, 0, 2) X(0, 8, 1, 2) X(0, 4, 1, 2) X(0, 2, 1, 2) X(1, 8, 0, 2) X(1, 4, 0, 2) X(1, 2, 0, 2) \
-    X(0, 8, 0, 4) X(0, 4, 0, 4) X(0, 2, 0, 4) X(0, 8, 1, 4) X(0, 4, 1, 4) X(0, 2, 1, 4) X(1, 8, 0, 4) X(1, 4, 0, 4) X(1, 2, 0, 4) \
-    X(0, 8, 2, 2) X(0, 4, 2, 2) X(0, 2, 2, 2)
+    X(0, 8, 0, 2, 16) X(0, 4, 0, 2, 16) X(0, 2, 0, 2, 16) X(0, 8, 1, 2, 16) X(0, 4, 1, 2, 16) X(0, 2, 1, 2, 16) \
+    X(1, 8, 0, 2, 16) X(1, 4, 0, 2, 16) X(1, 2, 0, 2, 16) \
+    X(0, 8, 0, 4, 16) X(0, 4, 0, 4, 16) X(0, 2, 0, 4, 16) X(0, 8, 1, 4, 16) X(0, 4, 1, 4, 16) X(0, 2, 1, 4, 16) \
+    X(1, 8, 0, 4, 16) X(1, 4, 0, 4, 16) X(1, 2, 0, 4, 16) \
+    X(0, 8, 2, 2, 16) X(0, 4, 2, 2, 16) X(0, 2, 2, 2, 16) \
+    X(0, 8, 1, 2, 15) X(0, 4, 1, 2, 15) X(0, 2, 1, 2, 15) X(0, 8, 0, 2, 15) X(0, 4, 0, 2, 15) X(0, 2, 0, 2, 15)
 
 extern "C" int aak_dedisperse_init(void) {
     int e = 0;
-#define X(I, C, F, MM) if ((e = set_attr<I, C, F, MM>())) return e;
+#define X(I, C, F, MM, W) if ((e = set_attr<I, C, F, MM, W>())) return e;
     AA_FOR_ALL_VARIANTS(X)
 #undef X
     return 0;
@@ -409,7 +419,8 @@ extern "C" int aak_dedisperse(const aak_dedisp_args* a, void* stream) {
     cudaStream_t st = (cudaStream_t)stream;
     const int fma = a->in16 ? 0 : (a->dms_per_warp == 4 ? (a->variant & 1) : a->variant);
     const int mm = a->dms_per_warp == 4 ? 4 : 2;
-#define X(I, C, F, MM) if (a->in16 == I && a->chan_block == C && fma == F && mm == MM) return launch<I, C, F, MM>(a, st);
+    const int nwc = (mm == 2 && !a->in16) ? a->dm_tile / 2 : 16;
+#define X(I, C, F, MM, W) if (a->in16 == I && a->chan_block == C && fma == F && mm == MM && nwc == W) return launch<I, C, F, MM, W>(a, st);
     AA_FOR_ALL_VARIANTS(X)
 #undef X
     return (int)cudaErrorInvalidValue;
