@@ -145,7 +145,8 @@ static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16,
     const int32_t C = s.plan.nchans, nd = rg.r.ndms;
     p.in16 = in16; p.esz = in16 ? 2 : 1; p.spw = 4 / p.esz; p.ncopy = p.spw;
     /* uint8 samples: 15 compute warps x 2 trials (+ the producer = 16 warps, 128 registers per thread, 30 trials per CTA):
-     * measured 216.6 -> 204.9 ms on SKA-like against 16 + 1 warps at 96 registers (11 or 7 warps are slower again);
+     * measured 216.6 -> 204.9 ms on SKA-like against 16 + 1 warps at 96 registers (11 or 7 warps are slower again, and
+     * 14 + 1 warps change nothing for the uint16 kernel, which is bound by shared-memory bytes, not by loads in flight);
      * binned uint16 samples: 16 warps x (4 adjacent trials, half the tile), 32 trials per CTA */
     p.dm_tile = in16 ? kDmTile : 30;
 #ifdef AA_TUNING

@@ -143,13 +143,13 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
     constexpr int SPW = 4 / ESZ;                 /* samples per word */
     constexpr int NCOPY = SPW;                   /* shifted copies */
     constexpr int NW = NWC;
-    constexpr int NG = (M == 2) ? NWC : DM_TILE / M;   /* DM groups */
-    constexpr int NTH = NW / NG;                 /* time parts */
+    constexpr int NTH = (M == 2) ? 1 : 2;        /* time parts of the tile */
+    constexpr int NG = NWC / NTH;                /* DM groups */
     constexpr int DMT = NG * M;                  /* DM trials per CTA: 32 or 30 */
     constexpr int T_PART = T_TILE / NTH;
     constexpr int J = T_PART / (32 * SPW);       /* words per thread per DM */
     constexpr int ENT_BYTES = CB * DM_TILE * 4;
-    static_assert(NG * NTH == NW && NTH >= 1 && J >= 1, "warp layout");
+    static_assert(NG * NTH == NW && NTH >= 1 && J >= 1 && DMT <= DM_TILE, "warp layout");
 
     if (p.mode_cnt && ((*p.mode_cnt > p.mode_cap) ? 1 : 0) != p.mode_dense) return;     /* the other input format handles this chunk */
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -374,7 +374,7 @@ int launch(const aak_dedisp_args* a, cudaStream_t st) {
     p.nring = a->ring_stages;
     if (p.nring < 2 || p.nring > MAX_RING) return (int)cudaErrorInvalidValue;
     const size_t smem = SMEM_HEADER + (size_t)p.nring * ((size_t)NCOPY * CB * a->window_bytes + CB * DM_TILE * 4);
-    constexpr int DMT = (M == 2) ? 2 * NWC : DM_TILE;
+    constexpr int DMT = 2 * NWC;                 /* M = 2: NWC groups of 2; M = 4: NWC / 2 groups of 4 */
     if (a->dm_tile != DMT) return (int)cudaErrorInvalidValue;
     const long long ndm_tiles = (a->ndms + DMT - 1) / DMT;
     const long long nt_tiles = (a->nt + T_TILE - 1) / T_TILE;
@@ -419,7 +419,7 @@ extern "C" int aak_dedisperse(const aak_dedisp_args* a, void* stream) {
     cudaStream_t st = (cudaStream_t)stream;
     const int fma = a->in16 ? 0 : (a->dms_per_warp == 4 ? (a->variant & 1) : a->variant);
     const int mm = a->dms_per_warp == 4 ? 4 : 2;
-    const int nwc = (mm == 2 && !a->in16) ? a->dm_tile / 2 : 16;
+    const int nwc = a->dm_tile / 2;
 #define X(I, C, F, MM, W) if (a->in16 == I && a->chan_block == C && fma == F && mm == MM && nwc == W) return launch<I, C, F, MM, W>(a, st);
     AA_FOR_ALL_VARIANTS(X)
 #undef X
