@@ -32,8 +32,8 @@ if str(ROOT) not in sys.path:
 METRIC = "dm_trial_samples_per_s"
 UNIT = "DM-trial*samples/s"
 SM_COUNT = 148
-# ncu, profiles/r01c_dram_per_launch.csv: bytes read + written by the K2 launches (k_dedisperse + k_scatter_exceptions) of one SKA-like step
-K2_DRAM_BYTES_PER_STEP = {"ska": 39117169408 + 6902735872}
+# ncu, profiles/r01f_dram_per_launch.csv: bytes read + written by the K2 launches (k_dedisperse + k_scatter_exceptions) of one SKA-like step
+K2_DRAM_BYTES_PER_STEP = {"ska": 38461107200 + 6906948352}
 INT_LANES_PER_SM_CLK = 128      # 64 ALU-pipe (IADD3) + 64 FMA-pipe (IMAD) lanes per SM per clock, DESIGN.md "Roofline"
 
 
@@ -271,7 +271,7 @@ def run_ours(args, w):
                 "achieved": adds / k2 / 1e12, "peak": peak / 1e12, "unit": "Tadd/s (algorithmic 32-bit integer adds)",
                 "frac": adds / k2 / peak, "traffic": K2_DRAM_BYTES_PER_STEP.get(w.name),
                 "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of the K2 launches of one step (9 launches on ska), one "
-                                "ncu capture: profiles/r01c_dram_per_launch.csv; compulsory bytes are input once + D once",
+                                "ncu capture: profiles/r01f_dram_per_launch.csv; compulsory bytes are input once + D once",
                 "peak_how": f"derived: {SM_COUNT} SMs x {INT_LANES_PER_SM_CLK} integer-add lanes/clk (64 IADD3 + 64 IMAD) x max SM clock",
                 "measured_iadd3_only_tadd_s": iadd3 / 1e12, "measured_iadd3_imad_mixed_tadd_s": mixed / 1e12, "measured_imad_only_tadd_s": imad / 1e12,
                 "frac_of_measured_mixed": adds / k2 / max(mixed, iadd3), "frac_of_measured_iadd3_only": adds / k2 / iadd3,
