@@ -57,6 +57,7 @@ struct Arena {
 struct K2Plan {
     int32_t in16 = 0, esz = 1, spw = 4, ncopy = 4;
     int32_t chan_block = 8, window_bytes = 0, spill_stages = 0, nstages = 0;
+    int32_t skew_q16 = 0;                                     /* CTA rasterisation skew (time tiles per DM tile, 16.16) */
     int32_t dm_tile = 32, ndm_tiles = 0;                      /* DM trials per CTA (32 or 30) and the number of DM tiles */
     int32_t dms_per_warp = 2, variant = 1, ring_stages = 3;   /* K2 tuning chosen by the strategy */
     int32_t* d_etab = nullptr;

@@ -75,6 +75,7 @@ typedef struct {
     int32_t in16;              /* 0: uint8 input (bin 1), 1: uint16 input (binned) */
     int32_t variant;           /* uint8 only: odd-byte lane adds as 0 = IADD3, 1 = IMAD (FMA pipe), 2 = alternating */
     int32_t ring_stages;       /* depth of the shared-memory stage ring (2..8) */
+    int32_t skew_q16;          /* CTA order: time tiles skewed by skew_q16 / 65536 per DM tile (0 = plain order) */
     int32_t dm_tile;           /* DM trials per CTA: 32, or 30 (uint8, 2 trials per warp: 15 compute warps with 128 registers) */
     int32_t chan_begin, chan_end; /* sum channels [chan_begin, chan_end) only (multiples of chan_block; chan_end 0 = nchans) */
     int32_t accumulate;        /* 1: D += the partial sums (a later channel group of the same chunk), 0: D = */

@@ -118,7 +118,7 @@ aa_status enqueue_k2(Strategy& s, const Chunk& c, int32_t c0, int32_t c1, bool a
             const K2Plan& p = route == 0 ? rg.lo : static_cast<const K2Plan&>(rg);
             a.tmap = &p.map; a.etab = p.d_etab; a.x0tab = p.d_x0tab;
             a.chan_block = p.chan_block; a.window_bytes = p.window_bytes; a.spill_stages = p.spill_stages; a.in16 = p.in16;
-            a.variant = p.variant; a.dms_per_warp = p.dms_per_warp; a.ring_stages = p.ring_stages; a.dm_tile = p.dm_tile;
+            a.variant = p.variant; a.dms_per_warp = p.dms_per_warp; a.ring_stages = p.ring_stages; a.dm_tile = p.dm_tile; a.skew_q16 = p.skew_q16;
             a.mode_cnt = rg.has_lo ? s.d_exc_cnt[bin] + g : nullptr;
             a.mode_cap = rg.has_lo ? group_limit(s, bin, c0, c1) : 0u; a.mode_dense = route;
             a.bias = route == 0 ? (const int32_t*)(s.d_exc_cnt[bin] + kMaxGroups + g) : nullptr;

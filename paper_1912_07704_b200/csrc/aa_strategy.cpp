@@ -194,6 +194,17 @@ static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16,
         if (n >= 2 && n <= 8 && aak_dedisperse_smem_bytes(p.chan_block, p.window_bytes, p.in16, n) <= 227 * 1024) p.ring_stages = n;
     }
 #endif
+    /* rasterisation skew = the channel-averaged delay growth per DM tile, in time tiles (only worth it above ~1/4 tile) */
+    {
+        double sum = 0.0;
+        const int32_t* last = rg.delays.data() + (size_t)(nd - 1) * C;
+        for (int32_t c = 0; c < C; ++c) sum += (double)last[c];
+        const double per_tile = (sum / C) / std::max(1, p.ndm_tiles - 1) / (double)kTTile;
+        p.skew_q16 = per_tile >= 0.25 ? (int32_t)std::min(per_tile * 65536.0, 2.0e9) : 0;
+#ifdef AA_TUNING
+        if (const char* ev = getenv("AA_K2_SKEW")) p.skew_q16 = (int32_t)(atof(ev) * per_tile * 65536.0);
+#endif
+    }
     p.nstages = (C + p.chan_block - 1) / p.chan_block;
     /* 16-bit lanes are carried every 65536 / (largest sample value + 1) channels: bytes 256, uint16 sums of b bytes 256/b */
     p.spill_stages = (in16 ? 256 / rg.r.bin : 256) / p.chan_block;

@@ -72,6 +72,8 @@ struct DedispParams {
     unsigned mode_cap;
     int mode_dense;
     const int* bias;           /* NULL, or a constant added to every output */
+    int skew_q16;              /* CTA order: time tile = blockIdx / ndm_tiles - (skew_q16 * dm_tile >> 16), see launch() */
+    int nt_tiles;
     unsigned one;              /* always 1; a runtime value so that x*one+y stays an IMAD (FMA pipe) */
 };
 
@@ -155,8 +157,12 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
     extern __shared__ __align__(1024) uint8_t smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int ndm_tiles = (p.ndms + DMT - 1) / DMT;
-    const int dt = blockIdx.x % ndm_tiles;       /* DM tile fastest: concurrent CTAs share the same input windows in L2 */
-    const int tt = blockIdx.x / ndm_tiles;
+    /* DM tile fastest, and the time tile skewed by the average delay of the DM tile: CTAs that run together then read the
+     * same stretch of the INPUT (t + delay), so the windows of neighbouring DM tiles are L2 hits also where the delay grows
+     * by more than a tile per DM tile (low-frequency bands). skew 0 = plain (DM tile, time tile) order. */
+    const int dt = blockIdx.x % ndm_tiles;
+    const int tt = blockIdx.x / ndm_tiles - (int)(((long long)p.skew_q16 * dt) >> 16);
+    if (tt < 0 || tt >= p.nt_tiles) return;
     const long long t0 = (long long)tt * T_TILE;
     const int WB = p.window_bytes;
     const int data_bytes = NCOPY * CB * WB;
@@ -378,7 +384,9 @@ int launch(const aak_dedisp_args* a, cudaStream_t st) {
     if (a->dm_tile != DMT) return (int)cudaErrorInvalidValue;
     const long long ndm_tiles = (a->ndms + DMT - 1) / DMT;
     const long long nt_tiles = (a->nt + T_TILE - 1) / T_TILE;
-    const long long grid = ndm_tiles * nt_tiles;
+    p.skew_q16 = a->skew_q16 > 0 ? a->skew_q16 : 0; p.nt_tiles = (int)nt_tiles;
+    const long long extra_rows = ((long long)p.skew_q16 * (ndm_tiles - 1)) >> 16;     /* diagonals that start before time tile 0 */
+    const long long grid = ndm_tiles * (nt_tiles + extra_rows);
     if (grid <= 0 || grid > 0x7fffffffll) return (int)cudaErrorInvalidConfiguration;
     CUtensorMap map;
     memcpy(&map, a->tmap, sizeof(CUtensorMap));
