@@ -181,8 +181,8 @@ aa_status aa_strategy_shard(aa_strategy* s, int32_t rank, int32_t world);
  *              (aa_plan_set_input_layout): x[t][c], nchans samples per row, row_stride_bytes (>= nchans) between
  *              consecutive time samples. Must stay valid until the
  *              following aa_run_* call returns (prefetch). Pinned memory is needed for the copy to overlap compute.
- * A chunk that was not prefetched (the first chunk; a single-chunk observation) is copied in four channel groups and each
- * group is binned and added into D as soon as it has landed, so only the first group's copy (1/16 of the channels) is
+ * A chunk that was not prefetched (the first chunk; a single-chunk observation) is copied in three channel groups (1/16, 5/16, 10/16 of the channels) and each
+ * group is binned and added into D as soon as it has landed, so only the first group's copy is
  * exposed; the sums are int32, any grouping gives the same bits.
  * Returns AA_OK; AA_ERR_NOT_READY; AA_ERR_ORDER if the previous chunk's SPS has not run; AA_ERR_CUDA. */
 aa_status aa_run_dedispersion(aa_strategy* s, const uint8_t* host_input, size_t row_stride_bytes);
