@@ -308,7 +308,7 @@ struct SpsParams {
     double dm_low, dm_step;
     const double* mu_sigma;
     u64 chunk_start;
-    int widths[SPS_MAXW]; int nwidths; int wmax;
+    int widths[SPS_MAXW]; int nwidths; int wmax; int pow2;      /* pow2: widths[i] == 1 << i */
     int tt;                                    /* centre samples per strip, multiple of 4 */
     int rb;                                    /* centre rows per CTA */
     double threshold;
@@ -346,27 +346,30 @@ __device__ __forceinline__ double k4_eval(const unsigned* I, const K4RowConst& r
     return best;
 }
 
-/* integer prefilter of one row: flags positions that may exceed the threshold, appends them to list (shared memory) */
-template <int NW>
-__device__ __forceinline__ void k4_prefilter(const unsigned* __restrict__ I, const K4RowConst& rc, const SpsParams& p, i64 t0,
-                                             unsigned short* list, int* cnt, int tid, int lane) {
-    int bm[NW];
+/* integer prefilter of one row: flags positions that may exceed the threshold, appends them to list (shared memory).
+ * qmax = centre positions of this strip that exist (t < nt); qfull = those for which every width fits (t + wmax <= ntd);
+ * nloc = ntd - t0 (samples of the row from the strip's first centre sample on), all as 32-bit strip-local numbers. */
+template <int NW, bool POW2>
+__device__ __forceinline__ void k4_prefilter(const unsigned* __restrict__ I, const K4RowConst& rc, const SpsParams& p, int qmax, int qfull,
+                                             int nloc, unsigned short* list, int* cnt, int tid, int lane) {
+    /* POW2: the plan's widths are 1, 2, 4, ... (every BASELINE.json config): the prefix offsets are then immediates of the
+     * shared-memory loads instead of values re-read from the parameter bank and added per sample */
+    int bm[NW], wd[NW];
 #pragma unroll
-    for (int iw = 0; iw < NW; ++iw) bm[iw] = rc.bmin[iw];
+    for (int iw = 0; iw < NW; ++iw) { bm[iw] = rc.bmin[iw]; wd[iw] = POW2 ? (1 << iw) : p.widths[iw]; }
     for (int q0 = 0; q0 < p.tt; q0 += K4_THREADS) {                  /* uniform trip count: ballots need every lane */
         const int q = q0 + tid;
-        const i64 t = t0 + q;
         bool f = false;
-        if (q < p.tt && t < p.nt) {
+        if (q < qmax) {
             const unsigned* Iq = I + q + 3;                          /* B_w(t) = I[e+w-1] - I[e-1], e = q + 4 */
             const unsigned base = Iq[0];
-            if (t + p.wmax <= p.ntd) {
+            if (q < qfull) {
 #pragma unroll
-                for (int iw = 0; iw < NW; ++iw) f |= ((int)(Iq[p.widths[iw]] - base) >= bm[iw]);
+                for (int iw = 0; iw < NW; ++iw) f |= ((int)(Iq[wd[iw]] - base) >= bm[iw]);
             } else {
 #pragma unroll
                 for (int iw = 0; iw < NW; ++iw)
-                    if (t + p.widths[iw] <= p.ntd) f |= ((int)(Iq[p.widths[iw]] - base) >= bm[iw]);
+                    if (q + wd[iw] <= nloc) f |= ((int)(Iq[wd[iw]] - base) >= bm[iw]);
             }
         }
         const unsigned mask = __ballot_sync(0xffffffffu, f);
@@ -392,6 +395,16 @@ k_sps_peaks(const SpsParams p) {
     const int i1 = min(i0 + p.rb, p.ndms);
     const int e0 = tid * 4 * V;                                      /* this thread's 4V contiguous elements */
     const int ne = p.tt + 4 + p.wmax;                                /* elements the strip needs */
+    /* 32-bit strip-local bounds (the 64-bit sample indices stay out of the per-sample code) */
+    const i64 nd_loc = p.ntd - tb;                                   /* elements of the segment that exist: e < nd_loc */
+    const int e_hi = (int)(nd_loc < (i64)ne ? (nd_loc < 0 ? 0 : nd_loc) : (i64)ne);
+    const int e_lo = tb < 0 ? (int)(-tb) : 0;                        /* first element with a sample (t >= 0) */
+    const i64 c_loc = p.nt - t0;
+    const int qmax = (int)(c_loc < (i64)p.tt ? (c_loc < 0 ? 0 : c_loc) : (i64)p.tt);
+    const i64 f_loc = p.ntd - t0 - p.wmax + 1;
+    const int qfull = (int)(f_loc < (i64)qmax ? (f_loc < 0 ? 0 : f_loc) : (i64)qmax);
+    const i64 n_loc64 = p.ntd - t0;
+    const int nloc = (int)(n_loc64 > 0x3fffffff ? 0x3fffffff : (n_loc64 < 0 ? 0 : n_loc64));
 
     int4 cur[V], nxt[V];
     int pv_c = 0, pv_n = 0;
@@ -406,8 +419,8 @@ k_sps_peaks(const SpsParams p) {
         sg = __ldg(p.mu_sigma + 2 * (size_t)r + 1);
 #pragma unroll
         for (int v = 0; v < V; ++v) {
-            const i64 t = tb + e0 + 4 * v;
-            if (t >= 0 && t < p.ntd && e0 + 4 * v < ne) buf[v] = __ldg(reinterpret_cast<const int4*>(row + t));
+            const int e = e0 + 4 * v;                                /* tb and nt are multiples of 4 or the row is padded to 128 */
+            if (e >= e_lo && e < e_hi) buf[v] = __ldg(reinterpret_cast<const int4*>(row + (tb + e)));
             else buf[v] = make_int4(0, 0, 0, 0);
         }
     };
@@ -445,11 +458,11 @@ k_sps_peaks(const SpsParams p) {
         if (live) {
 #pragma unroll
             for (int v = 0; v < V; ++v) {
-                const i64 t = tb + e0 + 4 * v;
+                const int e = e0 + 4 * v;
                 const int d[4] = {cur[v].x, cur[v].y, cur[v].z, cur[v].w};
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
-                    const bool in = (t + k >= 0) && (t + k < p.ntd);
+                    const bool in = (e + k >= e_lo) && (e + k < e_hi);
                     run += in ? (unsigned)(d[k] - pv_c) : 0u;
                     loc[v][k] = run;
                 }
@@ -483,7 +496,8 @@ k_sps_peaks(const SpsParams p) {
             unsigned short* list = sm.list[sl];
             int* cnt = &sm.cnt[sl];
             switch (p.nwidths) {
-#define K4_CASE(N) case N: k4_prefilter<N>(I, rc, p, t0, list, cnt, tid, lane); break;
+#define K4_CASE(N) case N: if (p.pow2) k4_prefilter<N, true>(I, rc, p, qmax, qfull, nloc, list, cnt, tid, lane); \
+                           else k4_prefilter<N, false>(I, rc, p, qmax, qfull, nloc, list, cnt, tid, lane); break;
                 K4_CASE(1) K4_CASE(2) K4_CASE(3) K4_CASE(4) K4_CASE(5) K4_CASE(6) K4_CASE(7) K4_CASE(8)
                 K4_CASE(9) K4_CASE(10) K4_CASE(11) K4_CASE(12) K4_CASE(13) K4_CASE(14) K4_CASE(15) K4_CASE(16)
 #undef K4_CASE
@@ -573,7 +587,8 @@ extern "C" int aak_sps_peaks(const aak_sps_args* a, void* stream) {
     SpsParams p;
     p.D = a->D; p.pitch = a->pitch; p.nt = a->nt; p.ntd = a->nt_data > a->nt ? a->nt_data : a->nt; p.ndms = a->ndms; p.bin = a->bin; p.range_index = a->range_index;
     p.dm_low = a->dm_low; p.dm_step = a->dm_step; p.mu_sigma = a->mu_sigma; p.chunk_start = a->chunk_start;
-    p.nwidths = a->nwidths; p.wmax = 0;
+    p.nwidths = a->nwidths; p.wmax = 0; p.pow2 = 1;
+    for (int k = 0; k < a->nwidths; ++k) if (a->widths[k] != (1 << k)) p.pow2 = 0;
     for (int k = 0; k < SPS_MAXW; ++k) { p.widths[k] = k < a->nwidths ? a->widths[k] : 0; if (p.widths[k] > p.wmax) p.wmax = p.widths[k]; }
     p.threshold = a->threshold; p.cands = a->cands; p.counter = (u64*)a->counter; p.capacity = a->capacity;
     if (a->nt <= 0 || a->ndms <= 0) return 0;
