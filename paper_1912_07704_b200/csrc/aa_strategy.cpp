@@ -164,14 +164,14 @@ static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16,
     const int64_t wsamp = kTTile + omax + 16 / p.esz;
     p.window_bytes = (int32_t)round_up((size_t)(wsamp * p.esz), 256);
     if (p.window_bytes > 65536) { set_error("aa_strategy_setup: range %d needs a %d-byte channel window per DM tile (> 65536): DM step too coarse for this band", rg.index, p.window_bytes); return false; }
-    /* the largest channel block that still leaves a 2-deep ring, then the deepest ring (<= 4) that fits: measured on the
+    /* the largest channel block that still leaves a 2-deep ring, then the deepest ring (<= 5) that fits: measured on the
      * low-frequency config (wide windows), 8 channels x 2 stages beats 4 x 4 by 6 %; ring depth alone moves < 1 % */
     p.chan_block = 0;
     p.ring_stages = 2;
     for (int cb = 8; cb >= 2; cb /= 2)
         if (aak_dedisperse_smem_bytes(cb, p.window_bytes, p.in16, 2) <= 227 * 1024) { p.chan_block = cb; break; }
     if (!p.chan_block) { set_error("aa_strategy_setup: range %d: channel window of %d bytes does not fit shared memory", rg.index, p.window_bytes); return false; }
-    for (int n = 3; n <= 4; ++n)
+    for (int n = 3; n <= 5; ++n)
         if (aak_dedisperse_smem_bytes(p.chan_block, p.window_bytes, p.in16, n) <= 227 * 1024) p.ring_stages = n;
     /* measured on B200 (profiles/): binned ranges are shared-memory bound and gain 13 % from 4 trials per warp with
      * register reuse; the uint8 ranges are issue bound and lose 7 % to the extra branches, so they keep 2 trials per warp
