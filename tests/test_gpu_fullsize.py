@@ -7,6 +7,8 @@ tiling): Mid (configs[1]) and SKA-like (configs[2], the headline workload). The 
   3. bands of 5 adjacent DM rows (first / middle / last of each range, plus the rows of injected pulses): bit-exact D,
      identical mu/sigma, identical candidates.
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -86,3 +88,59 @@ def test_mid_full_size():
 def test_ska_full_size_headline_workload():
     info, ncand, nb = _fullsize("ska", points_per_range=200, pulse_bands=4)
     assert (info["overlap"], info["n_out"], info["max_bin"]) == (32384, 491904, 8) and nb >= 15 and ncand > 0
+
+
+@pytest.mark.slow
+@pytest.mark.skipif(not os.environ.get("AA_TEST_LOWF_FULL"), reason="8.6 GB input, about 6 minutes: set AA_TEST_LOWF_FULL=1 (run once per round, result in profiles/)")
+def test_lowf_full_size():
+    """BASELINE.json configs[3] at full size (4096 channels x 2^21 samples, 6000 DM trials, delays up to 545 316 samples):
+    all-row moments, sampled outputs and bands, as for the SKA-like config."""
+    info, ncand, nb = _fullsize("lowf", points_per_range=120, pulse_bands=2)
+    assert (info["overlap"], info["n_out"], info["max_bin"]) == (545316, 1551836, 4) and nb >= 9 and ncand > 0
+
+
+@pytest.mark.slow
+@pytest.mark.skipif(not os.environ.get("AA_TEST_STREAM_FULL"), reason="38.4 GB of pinned host input, about 10 minutes: set AA_TEST_STREAM_FULL=1")
+def test_stream_full_size_selected_chunks():
+    """BASELINE.json configs[4] at full size (600 s, 40 GB budget, double-buffered H2D): the whole chunk loop runs; the first,
+    a middle and the last (short) chunk get the all-row moment identity, sampled outputs and one band per range, and the
+    candidate lists of those bands are compared; status codes are checked on every chunk."""
+    w = datagen.get_workload("stream")
+    x, pinned = make_input(w, pinned=True)
+    gpu, orc = GpuRun(w, x, budget_bytes=w.budget_bytes, max_candidates=1 << 23), OracleRun(w, x)
+    try:
+        n = gpu.info["nchunks"]
+        assert n >= 10 and gpu.info["arena_bytes_used"] <= w.budget_bytes
+        check = {0, n // 2, n - 1}
+        rs = np.random.default_rng(w.seed)
+        exp_bands = []
+        for j, chunk in enumerate(gpu.chunks):
+            start, length, n_out = chunk
+            gpu.dedisperse()
+            if j in check:
+                exp = row_moments_all_ranges(x[:, start:start + length], orc.k, w.ranges, 0, length, n_out)
+                for r, rng in enumerate(w.ranges):
+                    m0, m1 = gpu.moments(r)
+                    assert np.array_equal(m0, exp[r][0]) and np.array_equal(m1, exp[r][1]), (j, r)
+                    T = n_out // rng[3]
+                    pts = _points(rs, rng[2], T, 40)
+                    want = sampled_outputs(x, orc.k, rng, start, T, pts)
+                    rows = {}
+                    for (i, t), e in zip(pts, want):
+                        if i not in rows:
+                            rows[i] = gpu.row(r, i)
+                        assert int(rows[i][t]) == int(e), (j, r, i, t)
+            status = gpu.sps()
+            assert status == (gpu.aa.AA_STATUS_FINISHED if j == n - 1 else gpu.aa.AA_STATUS_CHUNK_DONE)
+            if j in check:
+                for r, rng in enumerate(w.ranges):
+                    i0, i1 = band_rows(rng[2], [rng[2] // 2])[0]
+                    e = check_band(gpu, orc, chunk, r, i0, i1, after_sps=True)
+                    exp_bands.append((r, i0, i1, start, n_out, e))
+        got = gpu.candidates()
+        for (r, i0, i1, start, n_out, e) in exp_bands:
+            sel = (got["range"] == r) & (got["dm_index"] >= i0) & (got["dm_index"] < i1) & (got["sample"] >= start) & (got["sample"] < start + n_out)
+            compare_candidates(got[sel], e, w.threshold)
+        assert len(got) > 0
+    finally:
+        gpu.close()
