@@ -139,7 +139,7 @@ def run_reference(args, w):
     x = datagen.generate(w.seed, w.nchans, w.nsamp, pl, dl)
     k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
     g = oracle.chunk_geometry(k, w.ranges, w.nsamp)
-    rows = 1 if w.nchans * w.nsamp > (1 << 28) else 3
+    rows = 2 if w.nchans * w.nsamp > (1 << 28) else 3
     for _ in range(min(args.warmup, 1)):
         oracle_sample(w, x, g["n_out"], rows)
     outs, secs, spent, what = 0, 0.0, 0.0, ""
@@ -292,7 +292,7 @@ def run_ours(args, w):
             "candidates_per_step": ncand, "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline}
     if not args.no_cpu_baseline and world == 1:
-        rows = 1 if w.nchans * w.nsamp > (1 << 28) else 3
+        rows = 2 if w.nchans * w.nsamp > (1 << 28) else 3
         o, secs, spent, what = oracle_sample(w, x, info["n_out"], rows)
         line["cpu_baseline"] = {"value": o / secs, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what,
                                 "sample_seconds": spent, "host_cores_available": os.cpu_count()}
