@@ -139,7 +139,7 @@ def run_reference(args, w):
     x = datagen.generate(w.seed, w.nchans, w.nsamp, pl, dl)
     k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
     g = oracle.chunk_geometry(k, w.ranges, w.nsamp)
-    rows = 2 if w.nchans * w.nsamp > (1 << 28) else 3
+    rows = 1 if w.nchans * w.nsamp > (1 << 28) else 3
     for _ in range(min(args.warmup, 1)):
         oracle_sample(w, x, g["n_out"], rows)
     outs, secs, spent, what = 0, 0.0, 0.0, ""
