@@ -52,12 +52,14 @@ typedef struct {
 int aak_prep_fused(const aak_prep_args* a, int32_t nrows, void* stream);
 
 /* ---- K2: dedispersion --------------------------------------------------------------------------------------------
- * Tiled kernel: a CTA owns DM_TILE(=32) DM trials x T_TILE(=1024) output samples; channels stream through shared memory
- * in blocks of `chan_block` via TMA (tensor map `tmap`, 128 opaque bytes, see aa_strategy.cpp), NSTAGE-deep mbarrier ring.
+ * Tiled kernel: a CTA owns `dm_tile` (30 or 32) DM trials x T_TILE(=1024) output samples; channels stream through shared
+ * memory in blocks of `chan_block` via TMA (tensor map `tmap`, 128 opaque bytes, see aa_strategy.cpp), `ring_stages`-deep
+ * mbarrier ring.
  * The input exists as NCOPY = 4 (uint8) or 2 (uint16) sample-shifted copies in ONE global buffer, copy k = x[c][t+k]
  * at byte offset k*copy_stride; tmap points at the 128-byte 4-D CUtensorMap over it (HOST memory).
  * A stage in shared memory is [chan_block][NCOPY][window_bytes] followed by the stage's slice of etab.
- * etab  [ndm_tiles][nstages][chan_block][32] int32 : shared-memory byte offset of (channel, DM) inside a stage
+ * etab  [ndm_tiles][nstages][chan_block][32] int32 : shared-memory byte offset of (channel, DM) inside a stage (rows of 32
+ *                                                  entries, the first dm_tile are used; ndm_tiles = ceil(ndms / dm_tile))
  * x0tab [ndm_tiles][nstages*chan_block]    int32 : 16-byte aligned BYTE offset of the channel window relative to the
  *                                                  tile's first output sample */
 typedef struct {
@@ -71,8 +73,8 @@ typedef struct {
     int32_t nchans;
     int32_t chan_block;        /* 8, 4 or 2 */
     int32_t window_bytes;      /* WB: bytes per (copy, channel) window in shared memory, multiple of 256 */
-    int32_t spill_stages;      /* carry the 16-bit lanes every this many stages: (256/bin)/chan_block */
-    int32_t in16;              /* 0: uint8 input (bin 1), 1: uint16 input (binned) */
+    int32_t spill_stages;      /* carry the 16-bit lanes every this many stages: 256/chan_block (bytes), (256/bin)/chan_block (uint16) */
+    int32_t in16;              /* 0: byte input (bin 1, or the offset-uint8 form of a binned input), 1: uint16 binned input */
     int32_t variant;           /* uint8 only: odd-byte lane adds as 0 = IADD3, 1 = IMAD (FMA pipe), 2 = alternating */
     int32_t ring_stages;       /* depth of the shared-memory stage ring (2..8) */
     int32_t skew_q16;          /* CTA order: time tiles skewed by skew_q16 / 65536 per DM tile (0 = plain order) */
