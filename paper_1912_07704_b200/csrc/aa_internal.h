@@ -75,6 +75,8 @@ struct Range : K2Plan {           /* the base is the range's main plan: uint8 fo
     std::vector<int32_t> delays;  /* [ndms][nchans], binned samples (host) */
     int32_t* d_D = nullptr;
     size_t first_row = 0;         /* index of this range's first row in the row tables */
+    bool naive = false;           /* the tile window does not fit shared memory: one-thread-per-output kernel on a delay table */
+    int32_t* d_delays = nullptr;  /* [ndms][nchans] (naive route only) */
     bool has_lo = false;          /* bin 2 / 4: the offset-uint8 route (k_misc.cu "Offset-uint8 form") with its own tiling */
     K2Plan lo;
 };

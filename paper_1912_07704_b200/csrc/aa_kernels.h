@@ -91,9 +91,11 @@ int aak_dedisperse(const aak_dedisp_args* a, void* stream);
 size_t aak_dedisperse_smem_bytes(int32_t chan_block, int32_t window_bytes, int32_t in16, int32_t ring_stages);
 int aak_dedisperse_init(void);   /* sets the dynamic shared-memory attribute of every instantiation */
 
-/* Reference kernel (one thread per output, global loads): debugging / cross-check only. delays [ndms][nchans] int32. */
-int aak_dedisperse_naive(const void* x, size_t pitch_elems, int32_t in16, const int32_t* delays, int32_t nchans,
-                         int32_t ndms, int64_t nt, int32_t* D, int64_t pitch, void* stream);
+/* One thread per output, global loads (copy 0 of the input, pitch in elements): the route for ranges whose channel window
+ * does not fit shared memory, and a cross-check. delays [ndms][nchans] int32; sums channels [chan_begin, chan_end),
+ * accumulate as in aak_dedisperse. */
+int aak_dedisperse_naive(const void* x, size_t pitch_elems, int32_t in16, const int32_t* delays, int32_t nchans, int32_t chan_begin,
+                         int32_t chan_end, int32_t ndms, int64_t nt, int32_t* D, int64_t pitch, int32_t accumulate, void* stream);
 
 /* ---- K0t: corner turn of a time-major chunk x_tm[t][c] into channel-major rows x[c][t] (uint8) */
 int aak_corner_turn(const uint8_t* in, size_t in_stride, uint8_t* out, size_t out_pitch, int32_t nchans, int64_t nsamp, void* stream);

@@ -114,6 +114,13 @@ aa_status enqueue_k2(Strategy& s, const Chunk& c, int32_t c0, int32_t c1, bool a
         a.nt = (int64_t)(c.n_out / (uint64_t)bin) + rg.extra;      /* reading C3x: E samples beyond the output span */
         a.ndms = rg.r.ndms; a.nchans = s.plan.nchans;
         a.chan_begin = c0; a.chan_end = c1; a.accumulate = accumulate ? 1 : 0;
+        if (rg.naive) {
+            const void* x0 = bin == 1 ? (const void*)s.d_x4 : (const void*)s.d_xb[bin];        /* copy 0 of the range's input form */
+            const size_t pitch_elems = bin == 1 ? s.in_pitch : s.xb_pitch[bin];
+            AA_LAUNCH(aak_dedisperse_naive(x0, pitch_elems, bin > 1, rg.d_delays, s.plan.nchans, c0, c1, rg.r.ndms, a.nt, rg.d_D, rg.pitch,
+                                           accumulate ? 1 : 0, st), "dedispersion (global-memory route)");
+            continue;
+        }
         for (int route = rg.has_lo ? 0 : 1; route < 2; ++route) {
             const K2Plan& p = route == 0 ? rg.lo : static_cast<const K2Plan&>(rg);
             a.tmap = &p.map; a.etab = p.d_etab; a.x0tab = p.d_x0tab;

@@ -106,6 +106,7 @@ static void carve(Strategy& s, int64_t L, bool two_raw) {
         rg.nt_full = n_out / rg.r.bin;
         rg.pitch = (int64_t)round_up((size_t)(rg.nt_full + rg.extra), 128);
         rg.d_D = (int32_t*)a.take((size_t)rg.r.ndms * (size_t)rg.pitch * 4);
+        rg.d_delays = rg.naive ? (int32_t*)a.take((size_t)rg.r.ndms * s.plan.nchans * 4) : nullptr;
         rg.d_etab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * kDmTile * 4);   /* rg. = the main plan */
         rg.d_x0tab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * 4);
         if (rg.has_lo) {
@@ -163,14 +164,14 @@ static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16,
     }
     const int64_t wsamp = kTTile + omax + 16 / p.esz;
     p.window_bytes = (int32_t)round_up((size_t)(wsamp * p.esz), 256);
-    if (p.window_bytes > 65536) { set_error("aa_strategy_setup: range %d needs a %d-byte channel window per DM tile (> 65536): DM step too coarse for this band", rg.index, p.window_bytes); return false; }
+    if (p.window_bytes > 65536) return false;
     /* the largest channel block that still leaves a 2-deep ring, then the deepest ring (<= 5) that fits: measured on the
      * low-frequency config (wide windows), 8 channels x 2 stages beats 4 x 4 by 6 %; ring depth alone moves < 1 % */
     p.chan_block = 0;
     p.ring_stages = 2;
     for (int cb = 8; cb >= 2; cb /= 2)
         if (aak_dedisperse_smem_bytes(cb, p.window_bytes, p.in16, 2) <= 227 * 1024) { p.chan_block = cb; break; }
-    if (!p.chan_block) { set_error("aa_strategy_setup: range %d: channel window of %d bytes does not fit shared memory", rg.index, p.window_bytes); return false; }
+    if (!p.chan_block) return false;
     for (int n = 3; n <= 5; ++n)
         if (aak_dedisperse_smem_bytes(p.chan_block, p.window_bytes, p.in16, n) <= 227 * 1024) p.ring_stages = n;
     /* measured on B200 (profiles/): binned ranges are shared-memory bound and gain 13 % from 4 trials per warp with
@@ -250,14 +251,23 @@ static bool plan_range(Strategy& s, Range& rg, std::vector<int32_t>& etab, std::
         }
     }
     rg.max_delay = rg.delays[(size_t)(nd - 1) * C + (C - 1)];
-    if (!plan_format(s, rg, rg, rg.r.bin > 1, etab, x0tab)) return false;
+    if (!plan_format(s, rg, rg, rg.r.bin > 1, etab, x0tab)) {
+        /* a window that does not fit shared memory is not an error of the plan: such a range (DM step very coarse for the
+         * band) takes the one-thread-per-output kernel on a device delay table; everything else about it stays the same */
+        rg.naive = true;
+        rg.in16 = rg.r.bin > 1; rg.esz = rg.in16 ? 2 : 1; rg.spw = 4 / rg.esz; rg.ncopy = rg.spw;
+        rg.dm_tile = kDmTile; rg.ndm_tiles = 0; rg.nstages = 0; rg.chan_block = 8; rg.window_bytes = 0;
+        etab.clear(); x0tab.clear();
+        rg.has_lo = false;
+        return true;
+    }
     /* bin 2 and 4 also get the offset-uint8 route (half the shared-memory bytes per add); the uint16 plan above stays as
      * the route for chunks with too many exceptions. C < 65536 so a channel index fits the exception record. */
     rg.has_lo = (rg.r.bin == 2 || rg.r.bin == 4) && C < 65536;
 #ifdef AA_TUNING
     if (const char* ev = getenv("AA_K2_LO")) rg.has_lo = rg.has_lo && atoi(ev) != 0;
 #endif
-    if (rg.has_lo && !plan_format(s, rg, rg.lo, 0, etab_lo, x0tab_lo)) return false;
+    if (rg.has_lo && !plan_format(s, rg, rg.lo, 0, etab_lo, x0tab_lo)) rg.has_lo = false;
     return true;
 }
 
@@ -295,6 +305,9 @@ static aa_status plan_host(aa_strategy* h, const aa_plan* plan, uint64_t nsamp_t
         s.nrows += (size_t)rg.r.ndms;
         if (rg.r.bin == 1) s.need_u8_copies = true;
     }
+    /* a naive range reads the uint16 form of its bin on every chunk, so that bin keeps no offset-uint8 route */
+    for (const Range& nv : s.ranges)
+        if (nv.naive) for (Range& rg : s.ranges) if (rg.r.bin == nv.r.bin) rg.has_lo = false;
     s.S = (int64_t)round_up((size_t)smax, (size_t)s.B);
     const int64_t usable = (int64_t)(nsamp_total / (uint64_t)s.B) * s.B;
     if (usable <= s.S) {
@@ -431,6 +444,8 @@ extern "C" aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, u
     const Chunk& last = s.chunks.back();
     for (size_t r = 0; r < s.ranges.size(); ++r) {
         Range& rg = s.ranges[r];
+        if (rg.naive && (e = cudaMemcpyAsync(rg.d_delays, rg.delays.data(), rg.delays.size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "delay table upload"));
+        if (rg.naive) { for (int32_t i = 0; i < rg.r.ndms; ++i) { const int32_t* base = rg.d_D + (size_t)i * (size_t)rg.pitch; rows_full[rg.first_row + i] = aak_row_desc{base, rg.nt_full}; rows_last[rg.first_row + i] = aak_row_desc{base, (int64_t)(last.n_out / (uint64_t)rg.r.bin)}; } continue; }
         if ((e = cudaMemcpyAsync(rg.d_etab, etabs[r].data(), etabs[r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
         if ((e = cudaMemcpyAsync(rg.d_x0tab, x0tabs[r].data(), x0tabs[r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
         if (rg.has_lo) {
@@ -546,6 +561,7 @@ extern "C" size_t aa_strategy_describe(const aa_strategy* h, char* buf, size_t b
                  rg.dm_tile, kTTile, rg.chan_block, rg.window_bytes, rg.nstages, rg.ndm_tiles, rg.spill_stages,
                  aak_dedisperse_smem_bytes(rg.chan_block, rg.window_bytes, rg.in16, rg.ring_stages));
         o += line;
+        if (rg.naive) o += "         tile window does not fit shared memory: one-thread-per-output kernel on a device delay table\n";
         if (rg.has_lo) {
             snprintf(line, sizeof line, "         offset-uint8 route: chan_block=%d window=%dB stages=%d ring=%d exception limit %u per chunk\n",
                      rg.lo.chan_block, rg.lo.window_bytes, rg.lo.nstages, rg.lo.ring_stages, s.exc_limit[rg.r.bin]);

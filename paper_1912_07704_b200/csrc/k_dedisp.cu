@@ -353,15 +353,17 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
     }
 }
 
+/* One thread per output, global loads: the route for ranges whose per-tile channel window does not fit shared memory (a DM
+ * step so coarse for the band that 30 trials spread over more than ~14 000 samples), and a cross-check. */
 template <typename T>
-__global__ void k_dedisperse_naive(const T* __restrict__ x, size_t pitch, const int32_t* __restrict__ delays, int nchans,
-                                   int ndms, long long nt, int32_t* __restrict__ D, long long dpitch) {
+__global__ void k_dedisperse_naive(const T* __restrict__ x, size_t pitch, const int32_t* __restrict__ delays, int nchans, int c0, int c1,
+                                   int ndms, long long nt, int32_t* __restrict__ D, long long dpitch, int accumulate) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int i = blockIdx.y;
     if (t >= nt || i >= ndms) return;
     const int32_t* dl = delays + (size_t)i * nchans;
-    int acc = 0;
-    for (int c = 0; c < nchans; ++c) acc += (int)x[(size_t)c * pitch + (size_t)(t + dl[c])];
+    int acc = accumulate ? D[(size_t)i * dpitch + t] : 0;
+    for (int c = c0; c < c1; ++c) acc += (int)x[(size_t)c * pitch + (size_t)(t + dl[c])];
     D[(size_t)i * dpitch + t] = acc;
 }
 
@@ -435,12 +437,15 @@ extern "C" int aak_dedisperse(const aak_dedisp_args* a, void* stream) {
 }
 
 extern "C" int aak_dedisperse_naive(const void* x, size_t pitch_elems, int32_t in16, const int32_t* delays, int32_t nchans,
-                                    int32_t ndms, int64_t nt, int32_t* D, int64_t pitch, void* stream) {
+                                    int32_t chan_begin, int32_t chan_end, int32_t ndms, int64_t nt, int32_t* D, int64_t pitch,
+                                    int32_t accumulate, void* stream) {
     cudaStream_t st = (cudaStream_t)stream;
+    if (ndms <= 0 || nt <= 0) return 0;
+    if (ndms > 65535) return (int)cudaErrorInvalidConfiguration;
     dim3 grid((unsigned)((nt + 255) / 256), (unsigned)ndms);
     if (in16)
-        k_dedisperse_naive<uint16_t><<<grid, 256, 0, st>>>((const uint16_t*)x, pitch_elems, delays, nchans, ndms, nt, D, pitch);
+        k_dedisperse_naive<uint16_t><<<grid, 256, 0, st>>>((const uint16_t*)x, pitch_elems, delays, nchans, chan_begin, chan_end, ndms, nt, D, pitch, accumulate);
     else
-        k_dedisperse_naive<uint8_t><<<grid, 256, 0, st>>>((const uint8_t*)x, pitch_elems, delays, nchans, ndms, nt, D, pitch);
+        k_dedisperse_naive<uint8_t><<<grid, 256, 0, st>>>((const uint8_t*)x, pitch_elems, delays, nchans, chan_begin, chan_end, ndms, nt, D, pitch, accumulate);
     return (int)cudaGetLastError();
 }

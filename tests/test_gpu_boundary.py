@@ -296,3 +296,81 @@ def test_clusters_of_the_tiny_pulse():
         assert sorted(int(cands["sample"][r]) for r in reps) == sorted(int(s) for s in cl["best"]["sample"])
     finally:
         g.close()
+
+
+@pytest.mark.parametrize("seed", range(int(__import__("os").environ.get("AA_TEST_FUZZ", "6"))))
+def test_random_small_configurations_match_the_oracle(seed):
+    """Randomised shapes and options (channel counts around the tile and group sizes, 1-3 DM ranges with random binning,
+    arbitrary width lists, chunking, time-major input, boxcar-complete chunks, uniform or Gaussian samples): every row,
+    statistic and candidate equals the oracle's. AA_TEST_FUZZ=N runs N seeds (default 6)."""
+    rs = np.random.default_rng(1000 + seed)
+    C = int(rs.choice([1, 3, 7, 8, 9, 31, 64, 100, 255, 256, 257, 300, 520]))
+    nr = int(rs.integers(1, 4))
+    ranges, dm = [], 0.0
+    for _ in range(nr):
+        b = int(rs.choice([1, 2, 4, 8]))
+        nd = int(rs.choice([1, 2, 29, 30, 31, 32, 33, 61, 64]))
+        step = float(rs.choice([0.25, 0.5, 1.0, 3.0]))
+        ranges.append((dm, step, nd, b))
+        dm += step * nd
+    widths = tuple(sorted(set(int(v) for v in rs.choice([1, 2, 3, 4, 5, 8, 16, 21, 32], size=int(rs.integers(1, 6)), replace=False))))
+    tsamp = float(rs.choice([64e-6, 256e-6, 1024e-6]))
+    f_top, bw = float(rs.choice([1500.0, 800.0, 420.0])), float(rs.choice([50.0, 100.0, 200.0]))
+    B = max(r[3] for r in ranges)
+    wtmp = Workload("fz", C, f_top, -bw / max(C, 2), tsamp, 1 << 20, tuple(ranges), widths, 5.0, seed=seed, npulses=0, pulse_dm=(0.0, 0.0), pulse_width_max=1)
+    import oracle
+    k = oracle.delay_constants(wtmp.freqs_mhz, tsamp)
+    boxcar = bool(rs.integers(0, 2))
+    E = (max(widths) - 1) if boxcar else 0
+    S = oracle.chunk_geometry(k, ranges, 1 << 20, boxcar_extra=E)["S"]
+    n_out_target = int(rs.choice([700, 2000, 5000])) * B
+    nsamp = int(S + n_out_target * float(rs.choice([1.0, 2.6])) + int(rs.integers(0, 17)))
+    if S > 300_000 or nsamp * C > 60_000_000:
+        pytest.skip("delay span too large for a quick case")
+    hint = 0
+    if rs.integers(0, 2):
+        hint = int(-(-(S + n_out_target) // B) * B)
+        if hint >= (nsamp // B) * B:
+            hint = 0
+    w = Workload("fz", C, f_top, -bw / max(C, 2), tsamp, nsamp, tuple(ranges), widths, 5.0, seed=seed, npulses=2, pulse_dm=(0.0, max(dm, 1.0)),
+                 pulse_width_max=max(widths), pulse_snr=(9.0, 20.0))
+    x, _ = make_input(w)
+    if rs.integers(0, 3) == 0:
+        x = rs.integers(0, 256, size=x.shape, dtype=np.uint8)             # dense exceptions: uint16 route for bin 2 / 4
+    tm = bool(rs.integers(0, 2))
+    kw = dict(chunk_len_hint=hint) if hint else {}
+    gpu, orc = GpuRun(w, x, time_major=tm, boxcar_overlap=boxcar, **kw), OracleRun(w, x)
+    try:
+        exp_all = []
+        for j, chunk in enumerate(gpu.chunks):
+            gpu.dedisperse()
+            gpu.sps()
+            for r, rng in enumerate(w.ranges):
+                exp_all.append(check_band(gpu, orc, chunk, r, 0, rng[2], after_sps=True))
+        got = gpu.candidates(allow_overflow=True)
+        exp = np.concatenate(exp_all)
+        if len(exp) < (1 << 20):
+            n, og, oe = compare_candidates(got, exp, w.threshold)
+            assert n + og == len(got) and n + oe == len(exp)
+    finally:
+        gpu.close()
+
+
+def test_range_whose_tile_window_exceeds_shared_memory_takes_the_global_memory_route():
+    """A DM step so coarse for the band that the 30 trials of a tile spread over more samples than shared memory holds is
+    not a configuration error: the range runs the one-thread-per-output kernel on a device delay table (also in channel
+    groups and next to ordinary ranges), with the same results as the oracle."""
+    w = Workload("coarse", 272, 420.0, -200.0 / 272, 64e-6, 420_000, ((0.0, 40.0, 9, 1), (0.0, 0.05, 35, 2), (360.0, 20.0, 3, 8)),
+                 (1, 2, 4, 8), 5.5, seed=12, npulses=2, pulse_dm=(0.0, 300.0), pulse_width_max=8, pulse_snr=(10.0, 20.0))
+    x, _ = make_input(w)
+    gpu, orc = GpuRun(w, x), OracleRun(w, x)
+    try:
+        assert "one-thread-per-output" in gpu.aa.aa_strategy_describe(gpu.h)
+        gpu.dedisperse()
+        gpu.sps()
+        exp = [check_band(gpu, orc, gpu.chunks[0], r, 0, rng[2], after_sps=True) for r, rng in enumerate(w.ranges)]
+        got = gpu.candidates()
+        n, og, oe = compare_candidates(got, np.concatenate(exp), w.threshold)
+        assert n + og == len(got) and n + oe == sum(len(e) for e in exp)
+    finally:
+        gpu.close()
