@@ -190,7 +190,7 @@ k_row_stats(const aak_row_desc* __restrict__ rows, double* __restrict__ mu_sigma
         const i64 nvec = T >> 2;
         const int4* Dv = reinterpret_cast<const int4*>(D);
         const i64 nvec_pad = (nvec + STAT_THREADS - 1) / STAT_THREADS * STAT_THREADS;     /* uniform trip count for the ballots */
-        constexpr int U = 4;                                                            /* 64 bytes in flight per thread */
+        constexpr int U = 8;                                                            /* 128 bytes in flight per thread */
         for (i64 q0 = 0; q0 < nvec_pad; q0 += U * STAT_THREADS) {
             int4 v[U]; bool ok[U];
 #pragma unroll
