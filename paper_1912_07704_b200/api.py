@@ -400,6 +400,10 @@ class Strategy:
                     break
         return aa_get_candidates(self.handle)
 
+    def clusters(self, dm_tol: float, gap: int) -> np.ndarray:
+        """Friends-of-friends clusters of the candidates gathered so far (include/aa.h, aa_get_clusters)."""
+        return aa_get_clusters(self.handle, dm_tol, gap)
+
     def close(self):
         if getattr(self, "handle", None):
             aa_strategy_destroy(self.handle)
