@@ -47,6 +47,9 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--nsamp", type=int, default=0, help="shorten (or lengthen) the workload's observation to this many samples: "
+                    "same band, DM plan and tiling, used for profiler captures of the large configurations; the line then "
+                    "names the workload '<name>@<nsamp>' and is not a BASELINE.json configuration")
     return ap.parse_args()
 
 
@@ -397,6 +400,8 @@ def main():
     args = parse()
     import datagen
     w = datagen.get_workload(args.workload)
+    if args.nsamp:
+        w = datagen.scaled(w, nsamp=args.nsamp, name=f"{w.name}@{args.nsamp}")
     if args.impl == "reference":
         run_reference(args, w)
     elif w.budget_bytes:

@@ -6,4 +6,4 @@ five BASELINE.json configurations (frequencies, DM plans, widths, thresholds, pu
 signal model used to sweep an injected pulse across the band.
 """
 from .generator import build, generate, checksum, lib_path  # noqa: F401
-from .workloads import WORKLOADS, Workload, get_workload, pulse_sweep  # noqa: F401
+from .workloads import WORKLOADS, Workload, get_workload, pulse_sweep, scaled  # noqa: F401

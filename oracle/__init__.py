@@ -50,8 +50,9 @@ def _load():
     for f in (L.orc_boxcar_snr, L.orc_boxcar_snr_prefix):
         f.argtypes = [vp, i64, vp, i32, f64, f64, vp, vp]; f.restype = None
     L.orc_find_peaks.argtypes = [vp, i32, i64, f64, i32, i32, vp, vp, i64]; L.orc_find_peaks.restype = i64
-    L.orc_search_rows.argtypes = [vp, i64, i32, vp, f64, f64, i32, i32, i32, i64, i64, vp, i32, f64, u64, i32, i32,
+    L.orc_search_rows.argtypes = [vp, i64, i32, vp, f64, f64, i32, i32, i32, i64, i64, vp, i32, f64, u64, i32, i32, i32,
                                   vp, vp, vp, vp, vp, i64]
+    L.orc_boxcar_snr_perwidth.argtypes = [vp, i64, i64, vp, i32, vp, vp, vp]; L.orc_boxcar_snr_perwidth.restype = None
     L.orc_search_rows.restype = i64
     L.orc_range_max_delay_unbinned.argtypes = [vp, i32, f64, f64, i32, i32]; L.orc_range_max_delay_unbinned.restype = i64
     _lib = L
@@ -86,10 +87,12 @@ def delay_table(k: np.ndarray, rng, i0: int = 0, i1: int | None = None) -> np.nd
     return out
 
 
-def bin_time(x: np.ndarray, start: int, nbinned: int, b: int) -> np.ndarray:
+def bin_time(x: np.ndarray, start: int, nbinned: int, b: int, out: np.ndarray | None = None) -> np.ndarray:
     assert x.dtype == np.uint8 and x.ndim == 2 and x.strides[1] == 1
     assert start + nbinned * b <= x.shape[1]
-    out = np.empty((x.shape[0], nbinned), dtype=np.uint16)
+    if out is None:
+        out = np.empty((x.shape[0], nbinned), dtype=np.uint16)
+    assert out.dtype == np.uint16 and out.shape == (x.shape[0], nbinned) and out.flags.c_contiguous
     _load().orc_bin(_p(x), x.strides[0], x.shape[0], start, nbinned, b, _p(out))
     return out
 
@@ -119,6 +122,18 @@ def boxcar_snr(row: np.ndarray, widths, mu: float, sigma: float, prefix: bool = 
     fn = _load().orc_boxcar_snr_prefix if prefix else _load().orc_boxcar_snr
     fn(_p(row), len(row), _p(w), len(w), float(mu), float(sigma), _p(S), _p(wb))
     return S, wb
+
+
+def boxcar_snr_perwidth(row: np.ndarray, T: int, widths):
+    """Reading C7m: per-width measured statistics. row holds Tx >= T samples (Tx - T = E of reading C3x). Returns
+    (S[T], wbest[T], wstats[nwidths][3] = mu_w, sigma_w, p_w)."""
+    row = np.ascontiguousarray(row, dtype=np.int64)
+    w = np.ascontiguousarray(widths, dtype=np.int32)
+    S = np.empty(T, dtype=np.float64)
+    wb = np.empty(T, dtype=np.int32)
+    ws = np.zeros((len(w), 3), dtype=np.float64)
+    _load().orc_boxcar_snr_perwidth(_p(row), int(T), len(row), _p(w), len(w), _p(S), _p(wb), _p(ws))
+    return S, wb, ws
 
 
 def find_peaks(S: np.ndarray, threshold: float, r0: int = 0, r1: int | None = None, cap: int = 1 << 20):
@@ -161,10 +176,12 @@ def chunk_geometry(k: np.ndarray, ranges, nsamp_total: int, chunk_len: int | Non
 
 
 def search_rows(xb: np.ndarray, k: np.ndarray, rng, range_index: int, T: int, widths, threshold: float,
-                chunk_start: int, i0: int, i1: int, want=("D", "stats"), cap: int = 1 << 20, extra: int = 0):
+                chunk_start: int, i0: int, i1: int, want=("D", "stats"), cap: int = 1 << 20, extra: int = 0,
+                per_width: bool = False):
     """Steps a4..a7 for rows [i0,i1) of one range on one binned chunk. Returns dict with 'cands' (structured array,
     canonical order) and whichever of 'D','stats','S','w' were asked for. extra = E (reading C3x): rows are dedispersed for
-    T + E samples ('D' then has T + E columns), statistics / S / peaks stay on the first T."""
+    T + E samples ('D' then has T + E columns), statistics / S / peaks stay on the first T. per_width: reading C7m
+    (each width normalised by the measured statistics of its own boxcar series) instead of C7."""
     assert xb.dtype == np.uint16 and xb.flags.c_contiguous
     w = np.ascontiguousarray(widths, dtype=np.int32)
     n = i1 - i0
@@ -175,7 +192,7 @@ def search_rows(xb: np.ndarray, k: np.ndarray, rng, range_index: int, T: int, wi
     c = np.zeros(cap, dtype=CAND_DTYPE)
     cnt = int(_load().orc_search_rows(_p(xb), xb.shape[1], xb.shape[0], _p(k), rng[0], rng[1], rng[2], rng[3],
                                       range_index, T, int(extra), _p(w), len(w), float(threshold), int(chunk_start), i0, i1,
-                                      _p(D), _p(st), _p(S), _p(W), _p(c), cap))
+                                      1 if per_width else 0, _p(D), _p(st), _p(S), _p(W), _p(c), cap))
     assert cnt <= cap, "raise cap"
     out = dict(cands=c[:cnt].copy(), count=cnt)
     if D is not None: out["D"] = D

@@ -29,6 +29,11 @@
  *   boxcar / SNR      pinned: direct summation, hand-worked rational example, injected-pulse SNR closed form
  *   peaks             pinned on hand-built maps; the plateau tie rule and strict '>' at the threshold are
  *                             conventions: "parity unpinned" beyond self-consistency
+ *   delay table       pinned: entry by entry against orc_delay and the golden delays (test_delay_table_*)
+ *   candidate record  pinned: pulses injected at known unbinned samples in a bin-4 range and in later chunks
+ *   per-width stats   pinned: w = 1 equals C7 bit for bit, hand-worked rational example, white-noise closed form
+ *                             sigma_w = 0.98485 sigma sqrt(w), AR(1) closed form where sqrt(w) scaling is wrong by 2x,
+ *                             invariance under a constant shift of D
  */
 #include <cmath>
 #include <cstdint>
@@ -199,6 +204,48 @@ void orc_boxcar_snr_prefix(const int64_t* D, int64_t T, const int32_t* widths, i
     }
 }
 
+/* ---- C7m: per-width MEASURED statistics (reading C7m; SURVEY §8(f3) "per-width measured sigma instead of
+ * sqrt(w) scaling"; "boxcar filters ... to maximise signal-to-noise"). Optional, off by default.
+ * For each plan width w the series of boxcar sums of the row
+ *     B_w[t] = sum_{j<w} D[t+j],   t in [0, n_w),   n_w = min(T, Tx - w + 1)      (T: the chunk's output span, Tx = T + E
+ *                                                                                   samples present; E = 0 unless C3x)
+ * is itself given reading C6 (orc_row_stats on the integer series B_w: pivot p_w = B_w[0], exact integer moments,
+ * iterated 3-sigma clip, at most 8 clips) -> mu_w, sigma_w, and
+ *     SNR_w[t] = ( (double)(B_w[t] - p_w) - (mu_w - (double)p_w) ) * (1.0 / sigma_w)
+ * replaces the white-noise scaling w*mu, sqrt(w)*sigma of C7. A width with n_w < 1, or sigma_w == 0 (or a degenerate
+ * clip) gives no SNR in this row. S = max over the remaining widths, smallest width on ties; S = -inf if none.
+ * For w = 1 this is C7 exactly (B_1 = D). wstats_out (may be NULL): [nwidths][3] = mu_w, sigma_w, (double)p_w. */
+void orc_boxcar_snr_perwidth(const int64_t* D, int64_t T, int64_t Tx, const int32_t* widths, int32_t nwidths,
+                             double* S, int32_t* wbest, double* wstats_out) {
+    const double ninf = -INFINITY;
+    for (int64_t t = 0; t < T; ++t) { S[t] = ninf; wbest[t] = 0; }
+    std::vector<int64_t> B;
+    for (int32_t iw = 0; iw < nwidths; ++iw) {
+        const int64_t w = widths[iw];
+        if (wstats_out) { wstats_out[3 * iw] = 0.0; wstats_out[3 * iw + 1] = 0.0; wstats_out[3 * iw + 2] = 0.0; }
+        int64_t nw = Tx - w + 1;
+        if (nw > T) nw = T;
+        if (nw < 1) continue;
+        B.assign((size_t)nw, 0);
+        for (int64_t t = 0; t < nw; ++t) {
+            int64_t b = 0;
+            for (int64_t j = 0; j < w; ++j) b += D[t + j];
+            B[(size_t)t] = b;
+        }
+        double mu, sigma; int64_t info[4];
+        const int32_t degenerate = orc_row_stats(B.data(), nw, &mu, &sigma, info);
+        const int64_t pw = B[0];
+        if (wstats_out) { wstats_out[3 * iw] = mu; wstats_out[3 * iw + 1] = degenerate ? 0.0 : sigma; wstats_out[3 * iw + 2] = (double)pw; }
+        if (degenerate || !(sigma > 0.0)) continue;
+        const double mrel = mu - (double)pw;
+        const double inv = 1.0 / sigma;
+        for (int64_t t = 0; t < nw; ++t) {
+            const double snr = ((double)(B[(size_t)t] - pw) - mrel) * inv;
+            if (snr > S[t]) { S[t] = snr; wbest[t] = (int32_t)w; }
+        }
+    }
+}
+
 /* ---- C8: peak finding ("peak-finding"; north_star "finds local peaks above a threshold") ---
  * On the map S[row][t] of ONE range in ONE chunk: (row, t) is a candidate iff S > threshold (strict) and, for
  * each of the 8 neighbours that exist (rows inside [0,nrows), t inside [0,T)):  S > neighbour when the neighbour
@@ -245,7 +292,7 @@ typedef struct {
 int64_t orc_search_rows(const uint16_t* xb /* binned chunk [nchans][nbinned], from orc_bin */, int64_t nbinned, int32_t nchans,
                         const double* k, double dm_low, double dm_step, int32_t ndms, int32_t bin, int32_t range_index,
                         int64_t T, int64_t extra, const int32_t* widths, int32_t nwidths, double threshold, uint64_t chunk_start,
-                        int32_t i0, int32_t i1,
+                        int32_t i0, int32_t i1, int32_t per_width /* 0: reading C7; 1: reading C7m */,
                         int64_t* D_out /* [(i1-i0)][T+extra] or NULL */, double* stats_out /* [(i1-i0)][2] or NULL */,
                         double* S_out /* [(i1-i0)][T] or NULL */, int32_t* w_out /* [(i1-i0)][T] or NULL */,
                         orc_candidate* cands, int64_t cap) {
@@ -259,7 +306,8 @@ int64_t orc_search_rows(const uint16_t* xb /* binned chunk [nchans][nbinned], fr
     for (int32_t r = 0; r < nr; ++r) {
         double mu, sigma; int64_t info[4];
         orc_row_stats(D.data() + (size_t)r * Tx, T, &mu, &sigma, info);
-        orc_boxcar_snr_prefix(D.data() + (size_t)r * Tx, Tx, widths, nwidths, mu, sigma, Sx.data(), Wx.data());
+        if (per_width) orc_boxcar_snr_perwidth(D.data() + (size_t)r * Tx, T, Tx, widths, nwidths, Sx.data(), Wx.data(), nullptr);
+        else orc_boxcar_snr_prefix(D.data() + (size_t)r * Tx, Tx, widths, nwidths, mu, sigma, Sx.data(), Wx.data());
         memcpy(S.data() + (size_t)r * T, Sx.data(), sizeof(double) * (size_t)T);
         memcpy(W.data() + (size_t)r * T, Wx.data(), sizeof(int32_t) * (size_t)T);
         const int32_t i = h0 + r;

@@ -22,8 +22,6 @@ CU_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-
             "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 CXX_FLAGS = ["-O2", "-std=c++17", "-fPIC", "-ffp-contract=off", "-Wall", "-Wno-unused-function",
              f"-I{CUDA_HOME / 'include'}"]
-if os.environ.get("AA_TUNING"):            # development builds only: lets environment variables override the K2 tiling
-    CXX_FLAGS.append("-DAA_TUNING")
 
 
 def _sources():

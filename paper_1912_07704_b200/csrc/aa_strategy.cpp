@@ -150,9 +150,6 @@ static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16,
      * 14 + 1 warps change nothing for the uint16 kernel, which is bound by shared-memory bytes, not by loads in flight);
      * binned uint16 samples: 16 warps x (4 adjacent trials, half the tile), 32 trials per CTA */
     p.dm_tile = in16 ? kDmTile : 30;
-#ifdef AA_TUNING
-    if (!in16) if (const char* ev = getenv("AA_K2_W15")) p.dm_tile = atoi(ev) ? 30 : kDmTile;
-#endif
     p.ndm_tiles = (nd + p.dm_tile - 1) / p.dm_tile;
     /* widest window: T_TILE + largest in-tile delay spread + alignment residue (< 16 bytes) */
     int64_t omax = 0;
@@ -179,22 +176,6 @@ static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16,
      * with the odd-byte adds on the FMA pipe */
     p.dms_per_warp = p.in16 ? 4 : 2;
     p.variant = 1;
-#ifdef AA_TUNING
-    if (const char* ev = getenv(p.in16 ? "AA_K2_M16" : "AA_K2_M8")) p.dms_per_warp = atoi(ev) == 4 ? 4 : 2;
-    if (const char* ev = getenv("AA_K2_VARIANT")) p.variant = atoi(ev);
-    if (const char* ev = getenv("AA_K2_CB")) {
-        const int cb = atoi(ev);
-        if ((cb == 2 || cb == 4 || cb == 8) && aak_dedisperse_smem_bytes(cb, p.window_bytes, p.in16, 2) <= 227 * 1024) {
-            p.chan_block = cb;
-            p.ring_stages = 2;
-            for (int n = 3; n <= 4; ++n) if (aak_dedisperse_smem_bytes(cb, p.window_bytes, p.in16, n) <= 227 * 1024) p.ring_stages = n;
-        }
-    }
-    if (const char* ev = getenv("AA_K2_RING")) {
-        const int n = atoi(ev);
-        if (n >= 2 && n <= 8 && aak_dedisperse_smem_bytes(p.chan_block, p.window_bytes, p.in16, n) <= 227 * 1024) p.ring_stages = n;
-    }
-#endif
     /* rasterisation skew = the channel-averaged delay growth per DM tile, in time tiles (only worth it above ~1/4 tile) */
     {
         double sum = 0.0;
@@ -202,9 +183,6 @@ static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16,
         for (int32_t c = 0; c < C; ++c) sum += (double)last[c];
         const double per_tile = (sum / C) / std::max(1, p.ndm_tiles - 1) / (double)kTTile;
         p.skew_q16 = per_tile >= 0.25 ? (int32_t)std::min(per_tile * 65536.0, 2.0e9) : 0;
-#ifdef AA_TUNING
-        if (const char* ev = getenv("AA_K2_SKEW")) p.skew_q16 = (int32_t)(atof(ev) * per_tile * 65536.0);
-#endif
     }
     p.nstages = (C + p.chan_block - 1) / p.chan_block;
     /* 16-bit lanes are carried every 65536 / (largest sample value + 1) channels: bytes 256, uint16 sums of b bytes 256/b */
@@ -264,9 +242,6 @@ static bool plan_range(Strategy& s, Range& rg, std::vector<int32_t>& etab, std::
     /* bin 2 and 4 also get the offset-uint8 route (half the shared-memory bytes per add); the uint16 plan above stays as
      * the route for chunks with too many exceptions. C < 65536 so a channel index fits the exception record. */
     rg.has_lo = (rg.r.bin == 2 || rg.r.bin == 4) && C < 65536;
-#ifdef AA_TUNING
-    if (const char* ev = getenv("AA_K2_LO")) rg.has_lo = rg.has_lo && atoi(ev) != 0;
-#endif
     if (rg.has_lo && !plan_format(s, rg, rg.lo, 0, etab_lo, x0tab_lo)) rg.has_lo = false;
     return true;
 }

@@ -408,13 +408,12 @@ extern "C" size_t aak_dedisperse_smem_bytes(int32_t chan_block, int32_t window_b
     return SMEM_HEADER + (size_t)ring_stages * (ncopy * chan_block * (size_t)window_bytes + (size_t)chan_block * DM_TILE * 4);
 }
 
+/* The instantiations the strategy can select (aa_strategy.cpp plan_format): bytes (uint8 input and the offset-uint8 form) =
+ * 15 compute warps x 2 trials, odd-byte adds on the FMA pipe; binned uint16 = 16 compute warps x 4 adjacent trials with
+ * equal-delay reuse; channel block 8, 4 or 2 by window size. The variants measured and rejected are in profiles/r01c_profiles.md. */
 #define AA_FOR_ALL_VARIANTS(X) \
-    X(0, 8, 0, 2, 16) X(0, 4, 0, 2, 16) X(0, 2, 0, 2, 16) X(0, 8, 1, 2, 16) X(0, 4, 1, 2, 16) X(0, 2, 1, 2, 16) \
-    X(1, 8, 0, 2, 16) X(1, 4, 0, 2, 16) X(1, 2, 0, 2, 16) \
-    X(0, 8, 0, 4, 16) X(0, 4, 0, 4, 16) X(0, 2, 0, 4, 16) X(0, 8, 1, 4, 16) X(0, 4, 1, 4, 16) X(0, 2, 1, 4, 16) \
-    X(1, 8, 0, 4, 16) X(1, 4, 0, 4, 16) X(1, 2, 0, 4, 16) \
-    X(0, 8, 2, 2, 16) X(0, 4, 2, 2, 16) X(0, 2, 2, 2, 16) \
-    X(0, 8, 1, 2, 15) X(0, 4, 1, 2, 15) X(0, 2, 1, 2, 15) X(0, 8, 0, 2, 15) X(0, 4, 0, 2, 15) X(0, 2, 0, 2, 15)
+    X(0, 8, 1, 2, 15) X(0, 4, 1, 2, 15) X(0, 2, 1, 2, 15) \
+    X(1, 8, 0, 4, 16) X(1, 4, 0, 4, 16) X(1, 2, 0, 4, 16)
 
 extern "C" int aak_dedisperse_init(void) {
     int e = 0;

@@ -38,8 +38,9 @@ class OracleRun:
         start, length, n_out = chunk
         rng = self.w.ranges[r_index]
         xb = self.binned(start, length, rng[3])
-        return oracle.search_rows(xb, self.k, rng, r_index, n_out // rng[3], self.w.widths, self.w.threshold, start, i0, i1, want=want,
-                                  extra=extra)
+        # the C ABI takes the threshold as float and widens it (include/aa.h): the oracle is handed the same double
+        return oracle.search_rows(xb, self.k, rng, r_index, n_out // rng[3], self.w.widths, float(np.float32(self.w.threshold)), start,
+                                  i0, i1, want=want, extra=extra)
 
 
 def compare_candidates(got: np.ndarray, exp: np.ndarray, threshold: float, snr_rtol=1e-4, band=1e-3):
@@ -155,6 +156,90 @@ def sampled_outputs(x: np.ndarray, k: np.ndarray, rng, start: int, T: int, point
             acc += int(x[ch, u + j].astype(np.int64).sum())
         out.append(acc)
     return np.array(out, np.int64)
+
+
+# ---------------------------------------------------------------------------------------- the whole oracle, in parallel
+# SURVEY §8(c) "Verification coverage": "run the single-threaded oracle as independent processes over DM slices with one
+# halo row each side". The oracle itself is untouched (orc_search_rows adds the halo rows on its own); this only hands
+# disjoint row slices [i0, i1) of one chunk to a pool of processes and gathers what they return. The binned chunk
+# (oracle.bin_time, once per binning factor) lives in shared memory so that every process reads the same arrays.
+_POOL_XB = {}
+
+
+def _pool_init(spec):
+    from multiprocessing import shared_memory
+    for b, (name, shape) in spec.items():
+        shm = shared_memory.SharedMemory(name=name)
+        _POOL_XB[b] = (shm, np.ndarray(shape, dtype=np.uint16, buffer=shm.buf))
+
+
+def _pool_slice(task):
+    """One slice: rows [i0, i1) of range r. Returns the statistics, a 128-bit hash of every D row (as int32 bytes: D < 2^23)
+    and the slice's candidates."""
+    import hashlib
+    (k, rng, r, T, widths, threshold, chunk_start, i0, i1, extra) = task
+    xb = _POOL_XB[rng[3]][1]
+    res = oracle.search_rows(xb, k, rng, r, T, widths, threshold, chunk_start, i0, i1, want=("D", "stats"), extra=extra)
+    hashes = [hashlib.blake2b(np.ascontiguousarray(res["D"][q], dtype=np.int32).tobytes(), digest_size=16).digest()
+              for q in range(i1 - i0)]
+    return r, i0, i1, res["stats"], hashes, res["cands"]
+
+
+def row_hash(row: np.ndarray) -> bytes:
+    import hashlib
+    return hashlib.blake2b(np.ascontiguousarray(row, dtype=np.int32).tobytes(), digest_size=16).digest()
+
+
+def oracle_slices(ranges, rows_per_unit_cost: int = 16, keep_every: int = 1):
+    """Disjoint DM slices covering every row of every range; a binned range's rows are cheaper, so its slices are taller.
+    keep_every = n keeps every n-th slice (a bounded sample of the same partition)."""
+    out = []
+    for r, rng in enumerate(ranges):
+        step = rows_per_unit_cost * rng[3]
+        for q, i0 in enumerate(range(0, rng[2], step)):
+            if q % keep_every == 0:
+                out.append((r, i0, min(rng[2], i0 + step)))
+    return out
+
+
+def run_oracle_slices(w, x, chunk, slices, processes: int | None = None, extra: int = 0, on_idle=None):
+    """Runs oracle.search_rows for every (r, i0, i1) of `slices` on `chunk` = (start, length, n_out) in a pool of
+    single-threaded processes. Returns {(r, i0, i1): (stats [n][2], hashes [n], cands)}. `on_idle` (if given) is called in
+    the parent between results, so GPU-side work can proceed while the pool computes."""
+    import multiprocessing as mp
+    import os
+    from multiprocessing import shared_memory
+    start, length, n_out = chunk
+    k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
+    shms, spec = [], {}
+    try:
+        for b in sorted({w.ranges[r][3] for (r, _, _) in slices}):
+            shape = (x.shape[0], length // b)
+            shm = shared_memory.SharedMemory(create=True, size=int(np.prod(shape)) * 2)
+            shms.append(shm)
+            oracle.bin_time(x, start, length // b, b, out=np.ndarray(shape, dtype=np.uint16, buffer=shm.buf))
+            spec[b] = (shm.name, shape)
+        thr = float(np.float32(w.threshold))
+        tasks = [(k, w.ranges[r], r, n_out // w.ranges[r][3], tuple(w.widths), thr, start, i0, i1, extra) for (r, i0, i1) in slices]
+        tasks.sort(key=lambda t: -(t[8] - t[7]) / t[1][3])           # longest first
+        out = {}
+        ctx = mp.get_context("spawn")                                # fresh interpreters: no CUDA state is inherited
+        with ctx.Pool(processes or os.cpu_count() or 1, initializer=_pool_init, initargs=(spec,)) as pool:
+            it = pool.imap_unordered(_pool_slice, tasks)
+            pending = len(tasks)
+            while pending:
+                try:
+                    r, i0, i1, st, hs, c = it.next(timeout=0.05 if on_idle else None)
+                except mp.TimeoutError:
+                    on_idle()
+                    continue
+                out[(r, i0, i1)] = (st, hs, c)
+                pending -= 1
+        return out
+    finally:
+        for shm in shms:
+            shm.close()
+            shm.unlink()
 
 
 class GpuRun:

@@ -165,9 +165,11 @@ def test_chunked_run_matches_oracle_per_chunk_and_is_chunk_invariant():
 
 
 # ------------------------------------------------------------------------------------------------ replicas over chunks (N > 1 path)
-def test_sharded_strategies_partition_the_chunks_and_reproduce_the_single_run():
+def test_sharded_strategies_match_the_oracle_per_shard_and_reproduce_the_single_run():
     """rank r of W owns chunks r, r+W, ...; no exchange. Two sharded strategies (run one after
-    the other on this one GPU, each with its own arena, as two ranks would) give together exactly the unsharded list."""
+    the other on this one GPU, each with its own arena, as two ranks would): every chunk a shard owns is compared with the
+    ORACLE (every D row bit-exact, every mu/sigma, the shard's candidate list), which also exercises the shard's
+    double-buffer parity ((j / world) & 1); together the shards give exactly the unsharded list."""
     from paper_1912_07704_b200 import replicas
     w = scaled(datagen.get_workload("mid"), nsamp=40_000, name="mid40k", ranges=((0.0, 0.5, 120, 1), (60.0, 1.0, 40, 2)))
     x, pinned = make_input(w, pinned=True)
@@ -178,15 +180,30 @@ def test_sharded_strategies_partition_the_chunks_and_reproduce_the_single_run():
     finally:
         one.close()
     assert nchunks >= 4 and len(ref) > 0
+    orc = OracleRun(w, x)
     parts, owned = [], []
     for rank in range(2):
         g = GpuRun(w, x, chunk_len_hint=9_000)
         try:
             g.st.shard(rank, 2)
             assert g.st.info["next_chunk"] == rank
-            c = g.st.run(x)
             mine = replicas.chunks_of_rank(nchunks, rank, 2)
+            exp_all = []
+            for n, j in enumerate(mine):
+                assert g.st.info["next_chunk"] == j
+                g.dedisperse()                                   # the shard's cursor: chunks rank, rank + 2, ...
+                status = g.sps()
+                assert status == (g.aa.AA_STATUS_FINISHED if n == len(mine) - 1 else g.aa.AA_STATUS_CHUNK_DONE)
+                for r, rng in enumerate(w.ranges):
+                    exp_all.append(check_band(g, orc, g.chunks[j], r, 0, rng[2], after_sps=True))
+            c = g.candidates()
+            nm, og, oe = compare_candidates(c, np.concatenate(exp_all), w.threshold)
+            assert nm + og == len(c) and nm + oe == sum(len(e) for e in exp_all)
             assert set((c["sample"] // n_out).tolist()) <= set(mine)
+            # and the one-call loop of the same shard gives the same list
+            g.st.shard(rank, 2)
+            c2 = g.st.run(x)
+            assert np.array_equal(c2, c)
             parts.append(c)
             owned += mine
         finally:
@@ -196,6 +213,36 @@ def test_sharded_strategies_partition_the_chunks_and_reproduce_the_single_run():
     assert len(merged) == len(ref)
     for f in ref.dtype.names:
         assert np.array_equal(merged[f], ref[f]), f
+
+
+# ------------------------------------------------------------------------------------------------ reading C9 on the GPU
+def test_candidate_record_in_binned_ranges_and_later_chunks_gpu():
+    """GPU twin of tests/test_oracle_pins.py::test_candidate_record_in_binned_ranges_and_later_chunks: pulses injected at
+    known UNBINNED samples in a bin-4 range and in chunks 1 and 2 come back at those coordinates through the C ABI
+    (sample = chunk_start + bin*t', width = bin*w*), and the whole run equals the oracle."""
+    base = datagen.get_workload("tiny")
+    w = scaled(base, name="tiny_c9", nsamp=16384, ranges=((0.0, 1.0, 40, 1), (40.0, 2.0, 30, 4)), widths=(1, 2, 4, 8, 16),
+               fixed_pulses=((20.0, 5000, 4, 14.0), (70.0, 9000, 16, 8.0)))
+    x, _ = make_input(w)
+    info, got, exp, (nmatch, og, oe) = _full_parity(w, x, chunk_len_hint=4096)
+    assert info["nchunks"] >= 4 and nmatch + og == len(got) and nmatch + oe == len(exp)
+    for (r_index, t0, width, dm_index) in ((0, 5000, 4, 20), (1, 9000, 16, 15)):
+        b = w.ranges[r_index][3]
+        j = t0 // info["n_out"]
+        sel = got[(got["range"] == r_index) & (got["sample"] // info["n_out"] == j)]
+        top = sel[np.argmax(sel["snr"])]
+        assert abs(int(top["dm_index"]) - dm_index) <= 1 and abs(int(top["sample"]) - t0) <= b
+        assert int(top["width"]) % b == 0 and width // 2 <= int(top["width"]) <= 2 * width
+
+
+def test_threshold_that_is_not_float_exact():
+    """The library takes the threshold as float and widens it; the oracle is handed the same double (helpers.OracleRun).
+    6.1 is not representable: with thousands of noise peaks near it, a double-vs-float mix-up would show as unmatched
+    candidates outside the 1e-3 band only by luck, so the lists are also required to agree in LENGTH."""
+    w = scaled(datagen.get_workload("tiny"), name="tiny_thr", threshold=6.1, widths=(1, 2, 4, 8, 16))
+    x, _ = make_input(w)
+    info, got, exp, (nmatch, og, oe) = _full_parity(w, x)
+    assert len(got) == len(exp) and nmatch == len(exp) and len(got) > 0
 
 
 # ------------------------------------------------------------------------------------------------ time-major input (corner turn, SURVEY §8(f1))

@@ -376,3 +376,211 @@ def test_boxcar_complete_chunks_equal_the_untruncated_definition(tiny):
             # and without the extra samples the last W_max - 1 positions are truncated (the behaviour C3x removes)
             old = oracle.search_rows(xb, k, rng, 0, n_out, widths, w.threshold, start, i, i + 1, want=("S",), extra=0)["S"][0]
             assert np.array_equal(old[: n_out - E], res["S"][0][: n_out - E]) or np.allclose(old[: n_out - E], res["S"][0][: n_out - E])
+
+
+# ------------------------------------------------------------------------------------------------ delay table (helper of the full-size checks)
+@pytest.mark.parametrize("wl", ["tiny", "mid", "ska", "lowf"])
+def test_delay_table_equals_delay(wl):
+    """orc_delay_table is what the all-rows moment identity and the sampled outputs of the full-size GPU tests are built
+    from. Pin: its [i][c] entry is orc_delay(k[c], DM_i, bin) on a scatter of (range, i, c) that includes the corners, and
+    an (i, c) transposition or a dropped `bin` cannot pass (the scatter has i != c and binned ranges)."""
+    w = datagen.get_workload(wl)
+    k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
+    rs = np.random.default_rng(17)
+    for r in w.ranges:
+        i0 = int(rs.integers(0, max(1, r[2] - 40)))
+        i1 = min(r[2], i0 + 40)
+        tab = oracle.delay_table(k, r, i0, i1)
+        assert tab.shape == (i1 - i0, w.nchans) and tab.dtype == np.int64
+        cs = np.concatenate([[0, 1, w.nchans - 1], rs.integers(0, w.nchans, 50)])
+        js = np.concatenate([[i0, i1 - 1, i0], rs.integers(i0, i1, 50)])
+        for c, i in zip(cs, js):
+            assert tab[int(i) - i0, int(c)] == oracle.delay(k[int(c)], oracle.dm_value(r[0], r[1], int(i)), r[3]), (wl, r, i, c)
+        # whole-table form (i0 = 0, i1 = ndms) agrees with the slice form
+        if r[2] <= 2500:
+            assert np.array_equal(oracle.delay_table(k, r)[i0:i1], tab)
+
+
+def test_delay_table_reproduces_the_golden_delays():
+    """The 25 closed-form rows of tests/golden/delays.txt (SURVEY §8(c) 'C2 delays'), read through the table form: the DM of
+    each golden row is located in the workload's DM plan and the entry [i][c] must be the golden value."""
+    n = 0
+    for wl, c, dm, b, exp in _rows("delays.txt"):
+        w = datagen.get_workload(wl)
+        k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
+        for r in w.ranges:
+            if r[3] != int(b):
+                continue
+            i = int(round((float(dm) - r[0]) / r[1]))
+            if 0 <= i < r[2] and oracle.dm_value(r[0], r[1], i) == float(dm):
+                assert oracle.delay_table(k, r, i, i + 1)[0, int(c)] == int(exp), (wl, c, dm, b)
+                n += 1
+    assert n >= 15          # most golden rows lie on a DM trial of their workload's plan
+
+
+# ------------------------------------------------------------------------------------------------ C9 record
+def _c9_workload():
+    """Tiny's band with a bin-1 and a bin-4 range, 4 chunks of 4096 samples, two bright pulses whose place is fixed by the
+    INJECTION (datagen), not by the oracle: pulse A at DM 20 (range 0, bin 1), t0 = 5000, 4 samples wide -> chunk 1;
+    pulse B at DM 70 (range 1, bin 4, dm_index 15), t0 = 9000, 16 samples wide -> chunk 2."""
+    base = datagen.get_workload("tiny")
+    return datagen.scaled(base, name="tiny_c9", nsamp=16384, ranges=((0.0, 1.0, 40, 1), (40.0, 2.0, 30, 4)), widths=(1, 2, 4, 8, 16),
+                          fixed_pulses=((20.0, 5000, 4, 14.0), (70.0, 9000, 16, 8.0)))
+
+
+def test_candidate_record_in_binned_ranges_and_later_chunks():
+    """Reading C9: sample = chunk_start + bin*t', width = bin*w*. Pin: pulses injected at known UNBINNED samples, widths and
+    DMs in a bin-4 range and in chunks 1 and 2 of a chunked geometry must come back at those unbinned coordinates (a
+    dropped `bin` factor would report sample ~ 8064 + 234 and width 4; a dropped chunk_start would report sample < 4096)."""
+    w = _c9_workload()
+    pl, dms, dl = w.pulses()
+    x = datagen.generate(w.seed, w.nchans, w.nsamp, pl, dl)
+    k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
+    g = oracle.chunk_geometry(k, w.ranges, w.nsamp, chunk_len=4096)
+    assert g["B"] == 4 and g["S"] % 4 == 0 and len(g["chunks"]) >= 4
+    found = {}
+    for (r_index, t0, width, dm_index) in ((0, 5000, 4, 20), (1, 9000, 16, 15)):
+        rng = w.ranges[r_index]
+        b = rng[3]
+        j = t0 // g["n_out"]
+        start, Lj, n_out = g["chunks"][j]
+        assert start == j * g["n_out"] and start <= t0 < start + n_out and j >= 1
+        xb = oracle.bin_time(x, start, Lj // b, b)
+        res = oracle.search_rows(xb, k, rng, r_index, n_out // b, w.widths, w.threshold, start, 0, rng[2], want=())
+        c = res["cands"]
+        assert len(c) > 0
+        top = c[np.argmax(c["snr"])]
+        found[r_index] = top
+        assert int(top["range"]) == r_index and abs(int(top["dm_index"]) - dm_index) <= 1
+        assert abs(int(top["sample"]) - t0) <= b, (int(top["sample"]), t0)                  # unbinned, absolute
+        assert int(top["sample"]) >= start and (int(top["sample"]) - start) % b == 0
+        assert int(top["width"]) % b == 0 and width // 2 <= int(top["width"]) <= 2 * width, int(top["width"])
+        assert float(top["dm"]) == np.float32(oracle.dm_value(rng[0], rng[1], int(top["dm_index"])))
+        assert np.all(c["sample"] >= start) and np.all(c["sample"] < start + n_out)          # every record is inside its chunk
+    assert float(found[0]["snr"]) > 10 and float(found[1]["snr"]) > 10
+
+
+def test_threshold_is_compared_as_a_float32_value():
+    """The C ABI takes the threshold as float (include/aa.h) and widens it; the tests hand the oracle np.float32(threshold)
+    so both sides compare against the same double. 6.1 is not float-exact: the two doubles differ, and a row built to sit
+    between them shows which one is in force."""
+    t32, t64 = float(np.float32(6.1)), 6.1
+    assert t32 != t64 and t32 < t64
+    S = np.full((1, 5), -np.inf)
+    S[0, 2] = (t32 + t64) / 2                       # above float32(6.1), below the double 6.1
+    assert len(oracle.find_peaks(S, t32)[0]) == 1 and len(oracle.find_peaks(S, t64)[0]) == 0
+
+
+# ------------------------------------------------------------------------------------------------ the parallel harness of the full-size check
+def test_sliced_parallel_oracle_equals_the_single_call(tiny):
+    """tests/helpers.run_oracle_slices (DM slices in a process pool, the route of the SKA-like full-oracle GPU test) returns,
+    slice by slice, exactly what ONE oracle.search_rows call over the whole range returns: statistics, D (through the
+    row hashes) and candidates. Pins the slicing, the halo handling and the gathering, not the oracle."""
+    from helpers import oracle_slices, row_hash, run_oracle_slices
+    w, x, k, g = tiny
+    chunk = g["chunks"][0]
+    full = oracle.search_rows(oracle.bin_time(x, 0, g["L"], 1), k, w.ranges[0], 0, g["n_out"], w.widths,
+                              float(np.float32(w.threshold)), 0, 0, w.ranges[0][2], want=("D", "stats"))
+    slices = oracle_slices(w.ranges, rows_per_unit_cost=16)
+    assert [s[1] for s in slices] == list(range(0, 101, 16)) and slices[-1][2] == 101
+    res = run_oracle_slices(w, x, chunk, slices, processes=2)
+    cands = []
+    for (r, i0, i1) in slices:
+        st, hs, c = res[(r, i0, i1)]
+        assert np.array_equal(st, full["stats"][i0:i1])
+        assert hs == [row_hash(full["D"][i]) for i in range(i0, i1)]
+        cands.append(c)
+    assert np.array_equal(np.concatenate(cands), full["cands"])
+    assert row_hash(full["D"][3]) != row_hash(full["D"][4])
+
+
+# ------------------------------------------------------------------------------------------------ reading C7m (per-width measured statistics)
+def test_per_width_stats_width_one_is_reading_c7_bit_for_bit():
+    rng = np.random.default_rng(21)
+    row = np.round(rng.normal(52000.0, 410.0, 6000)).astype(np.int64)
+    row[1000:1004] += 3000
+    mu, sg, *_ = oracle.row_stats(row)
+    S1, w1 = oracle.boxcar_snr(row, [1], mu, sg)
+    Sm, wm, ws = oracle.boxcar_snr_perwidth(row, len(row), [1])
+    assert np.array_equal(S1, Sm) and np.array_equal(w1, wm) and (ws[0, 0], ws[0, 1], ws[0, 2]) == (mu, sg, float(row[0]))
+    # in a longer width list the width-1 statistics are unchanged and each width's p_w is its first boxcar sum
+    _, _, ws = oracle.boxcar_snr_perwidth(row, len(row), [1, 2, 5, 32])
+    assert (ws[0, 0], ws[0, 1]) == (mu, sg)
+    assert [ws[i, 2] for i in range(4)] == [float(row[:w].sum()) for w in (1, 2, 5, 32)]
+
+
+def test_per_width_stats_hand_worked():
+    # w = 2 sums are constant -> sigma_2 = 0 -> width 2 is skipped; width 1: mean 2, sigma 1
+    S, wb, ws = oracle.boxcar_snr_perwidth(np.array([1, 3] * 4), 8, [1, 2])
+    assert ws[1, 1] == 0.0 and np.all(wb == 1) and np.array_equal(S, np.array([-1.0, 1.0] * 4))
+    # row 0 0 4 0 0 0 4 0 0: B_2 = 0 4 4 0 0 4 4 0 -> mean 2, sigma 2 exactly; B_1: mean 8/9, var 224/81
+    row = np.array([0, 0, 4, 0, 0, 0, 4, 0, 0])
+    S, wb, ws = oracle.boxcar_snr_perwidth(row, 9, [1, 2])
+    assert (ws[1, 0], ws[1, 1], ws[1, 2]) == (2.0, 2.0, 0.0)
+    assert abs(ws[0, 0] - 8 / 9) < 1e-15 and abs(ws[0, 1] - np.sqrt(224.0) / 9) < 1e-15
+    s1 = (4 - 8 / 9) / (np.sqrt(224.0) / 9)                # 1.871 > 1: width 1 wins on the spikes
+    s0 = (0 - 8 / 9) / (np.sqrt(224.0) / 9)                # -0.534: beats SNR_2 = -1 where B_2 = 0, loses to SNR_2 = +1 where B_2 = 4
+    assert wb.tolist() == [1, 2, 1, 1, 1, 2, 1, 1, 1]      # SNR_2 = -1 1 1 -1 -1 1 1 -1; the last position has only w = 1
+    assert abs(S[2] - s1) < 1e-14 and S[1] == 1.0 and S[5] == 1.0 and abs(S[0] - s0) < 1e-14 and abs(S[8] - s0) < 1e-14
+    # with E extra samples present (reading C3x) every start position t < T has a complete boxcar: n_w = T
+    S2, wb2, ws2 = oracle.boxcar_snr_perwidth(np.array([0, 0, 4, 0, 0, 0, 4, 0, 0, 0]), 9, [1, 2])
+    assert len(S2) == 9 and abs(ws2[1, 0] - 16 / 9) < 1e-15            # B_2 = 0 4 4 0 0 4 4 0 0: nine sums, mean 16/9
+    assert (ws2[0, 0], ws2[0, 1]) == (ws[0, 0], ws[0, 1])              # width-1 statistics still use the first T samples only
+
+
+def test_per_width_stats_white_noise_closed_form():
+    """White Gaussian rows: sigma_w -> 0.98485 * sigma * sqrt(w), mu_w -> w * mu (SURVEY §8(c) C6 fixed point applied to B_w),
+    i.e. C7m reduces to C7 where C7's assumption holds; the estimate's scatter grows with w (n/w independent sums)."""
+    rng = np.random.default_rng(22)
+    n, sig = 400_000, 700.0
+    row = np.round(rng.normal(3.0e6, sig, n)).astype(np.int64)
+    widths = [1, 2, 4, 16, 64]
+    S, wb, ws = oracle.boxcar_snr_perwidth(row, n, widths)
+    for iw, w in enumerate(widths):
+        assert abs(ws[iw, 1] / (0.98485 * sig * np.sqrt(w)) - 1.0) < 5.0 * np.sqrt(w / (2.0 * n)) + 2e-3, (w, ws[iw])
+        assert abs(ws[iw, 0] - w * 3.0e6) < 6.0 * sig * w / np.sqrt(n)
+
+
+def test_per_width_stats_red_noise_where_sqrt_w_scaling_is_wrong():
+    """AR(1) noise x_t = rho x_(t-1) + e_t: Var(sum of w samples) = s^2 [w + 2 sum_{k=1}^{w-1} (w-k) rho^k] (textbook
+    autocovariance s^2 rho^k). The measured sigma_w follows it; the sqrt(w) scaling of the width-1 sigma (reading C7) is
+    low by more than a factor 2 at w = 16, rho = 0.9 - the case C7m exists for."""
+    rng = np.random.default_rng(23)
+    n, rho, s_e = 600_000, 0.9, 200.0
+    e = rng.normal(0.0, s_e, n)
+    x = np.empty(n)
+    acc = 0.0
+    for t in range(n):
+        acc = rho * acc + e[t]
+        x[t] = acc
+    row = np.round(x + 1.0e6).astype(np.int64)
+    s_x = s_e / np.sqrt(1 - rho * rho)
+    widths = [1, 4, 16]
+    _, _, ws = oracle.boxcar_snr_perwidth(row, n, widths)
+    for iw, w in enumerate(widths):
+        var_w = s_x ** 2 * (w + 2.0 * sum((w - k) * rho ** k for k in range(1, w)))
+        assert abs(ws[iw, 1] / (0.98485 * np.sqrt(var_w)) - 1.0) < 0.04, (w, ws[iw, 1], np.sqrt(var_w))
+    assert ws[2, 1] > 2.0 * np.sqrt(16.0) * ws[0, 1]          # sqrt(w) scaling underestimates sigma_16 by > 2x
+
+
+def test_per_width_stats_invariant_under_a_constant_shift():
+    """All arithmetic is about the pivots p_w, so adding a constant to D changes the SNR only through the rounding of
+    mu_w = p_w + S1/n (about 1e-10 relative here) and never the chosen width or the integer statistics."""
+    rng = np.random.default_rng(24)
+    row = np.round(rng.normal(0.0, 90.0, 5000)).astype(np.int64)
+    row[2000:2010] += 700
+    a = oracle.boxcar_snr_perwidth(row + 4096, len(row), [1, 2, 8, 32])
+    b = oracle.boxcar_snr_perwidth(row + 8_000_000, len(row), [1, 2, 8, 32])
+    assert np.allclose(a[0], b[0], rtol=1e-8, atol=1e-8) and np.array_equal(a[1], b[1]) and np.array_equal(a[2][:, 1], b[2][:, 1])
+    assert np.array_equal(a[2][:, 2] - np.array([1, 2, 8, 32]) * 4096.0, b[2][:, 2] - np.array([1, 2, 8, 32]) * 8.0e6)   # p_w shifts by w * c
+    assert a[1][2000] in (8, 32) and a[0][2000] > 10
+
+
+def test_per_width_stats_end_to_end_recovers_the_injected_pulse(tiny):
+    w, x, k, g = tiny
+    xb = oracle.bin_time(x, 0, g["L"], 1)
+    a = oracle.search_rows(xb, k, w.ranges[0], 0, g["n_out"], w.widths, w.threshold, 0, 0, 101, want=())["cands"]
+    b = oracle.search_rows(xb, k, w.ranges[0], 0, g["n_out"], w.widths, w.threshold, 0, 0, 101, want=(), per_width=True)["cands"]
+    ta, tb = a[np.argmax(a["snr"])], b[np.argmax(b["snr"])]
+    assert (int(tb["dm_index"]), int(tb["sample"]), int(tb["width"])) == (int(ta["dm_index"]), int(ta["sample"]), int(ta["width"]))
+    assert abs(float(tb["snr"]) / float(ta["snr"]) - 1.0) < 0.05          # white noise: the two readings nearly agree
