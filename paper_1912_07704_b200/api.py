@@ -240,16 +240,38 @@ def aa_strategy_shard(strategy, rank: int, world: int) -> int:
 
 
 # ---------------------------------------------------------------------------------------------- pipeline
+def _host_input(strategy, host_input, row_stride_bytes):
+    """Marshalling checks of a host array handed to aa_run_*: the C side reads raw bytes through the pointer, so a wrong
+    dtype, a transposed view or a short array would be read without any error there. Raw addresses (int) pass unchecked."""
+    if isinstance(host_input, np.ndarray):
+        info = aa_strategy_get_info(strategy)
+        item = 2 if info.get("input_bits", 8) > 8 else 1
+        want = np.uint16 if item == 2 else np.uint8
+        if host_input.dtype != want:
+            raise TypeError(f"host_input must be {np.dtype(want).name} (the plan's sample type), got {host_input.dtype}")
+        if host_input.ndim != 2 or host_input.strides[1] != item:
+            raise ValueError("host_input must be 2-D with unit stride along its rows")
+        rows, cols = ((info["nsamp_total"], info["nchans"]) if info["input_layout"] == AA_LAYOUT_TIME_MAJOR
+                      else (info["nchans"], info["nsamp_total"]))
+        if host_input.shape[0] < rows or host_input.shape[1] < cols:
+            raise ValueError(f"host_input has shape {host_input.shape}, the plan's layout needs at least ({rows}, {cols})")
+        if row_stride_bytes is None:
+            row_stride_bytes = host_input.strides[0]
+    elif row_stride_bytes is None:
+        row_stride_bytes = host_input.stride(0) * host_input.element_size()
+    return _ptr(host_input), int(row_stride_bytes)
+
+
 def aa_run_dedispersion(strategy, host_input, row_stride_bytes=None) -> int:
-    """host_input: uint8 numpy array / pinned torch tensor [nchans][nsamp_total] (or a raw host address)."""
-    if row_stride_bytes is None:
-        row_stride_bytes = host_input.strides[0] if isinstance(host_input, np.ndarray) else host_input.stride(0)
-    return _check(load().aa_run_dedispersion(strategy, _ptr(host_input), int(row_stride_bytes)))
+    """host_input: numpy array / pinned torch tensor [nchans][nsamp_total] of the plan's sample type (or a raw host
+    address together with row_stride_bytes)."""
+    ptr, stride = _host_input(strategy, host_input, row_stride_bytes)
+    return _check(load().aa_run_dedispersion(strategy, ptr, stride))
 
 
 def aa_run_dedispersion_device(strategy, device_chunk, row_stride_bytes=None) -> int:
     if row_stride_bytes is None:
-        row_stride_bytes = device_chunk.stride(0)
+        row_stride_bytes = device_chunk.stride(0) * device_chunk.element_size()
     return _check(load().aa_run_dedispersion_device(strategy, _ptr(device_chunk), int(row_stride_bytes)))
 
 
@@ -259,9 +281,8 @@ def aa_run_sps(strategy) -> int:
 
 def aa_run_pipeline(strategy, host_input, row_stride_bytes=None) -> int:
     """The chunk loop inside the library (one call)."""
-    if row_stride_bytes is None:
-        row_stride_bytes = host_input.strides[0] if isinstance(host_input, np.ndarray) else host_input.stride(0)
-    return _check(load().aa_run_pipeline(strategy, _ptr(host_input), int(row_stride_bytes)))
+    ptr, stride = _host_input(strategy, host_input, row_stride_bytes)
+    return _check(load().aa_run_pipeline(strategy, ptr, stride))
 
 
 def aa_get_candidates(strategy, allow_overflow: bool = False) -> np.ndarray:
@@ -308,7 +329,13 @@ def aa_get_row_stats(strategy, rng: int, dm_index: int):
     return mu.value, sg.value, n.value, it.value
 
 
-def aa_get_row_moments(strategy, rng: int, ndms: int):
+def aa_get_row_moments(strategy, rng: int, ndms: int | None = None):
+    """sum_t D and sum_t t*D of every row of a range. The arrays are sized from the strategy's own range info (the C side
+    writes ndms values whatever the caller believes); `ndms`, if given, is only checked against it."""
+    n = aa_strategy_get_range_info(strategy, rng)["ndms"]
+    if ndms is not None and int(ndms) != n:
+        raise ValueError(f"range {rng} has {n} DM trials, not {ndms}")
+    ndms = n
     a = np.zeros(ndms, dtype=np.int64)
     b = np.zeros(ndms, dtype=np.int64)
     _check(load().aa_get_row_moments(strategy, rng, a.ctypes.data, b.ctypes.data))

@@ -98,18 +98,23 @@ struct Strategy {
     Arena arena;
     bool owns_arena = false;
     size_t in_pitch = 0;                     /* bytes per channel row of the uint8 buffers */
-    uint8_t* d_raw[2] = {nullptr, nullptr};  /* H2D targets (copy 0 of the uint8 input) */
+    uint8_t* d_raw[2] = {nullptr, nullptr};  /* [0]: the H2D target of a channel-major plan / the corner-turn target; [1] is unused: K2 never
+                                                reads the raw chunk (K1 does), so the next chunk's copy may start as soon as K1 is done */
     uint8_t* d_stage[2] = {nullptr, nullptr};   /* time-major plans: H2D targets [L][stage_stride]; d_raw[0] is the corner-turn target */
     size_t stage_stride = 0;
-    uint8_t* d_x4 = nullptr;                 /* the 4 sample-shifted copies of the uint8 chunk, copy k at k*x4_stride */
-    size_t x4_stride = 0;
+    /* Input forms of K2. Every form of a time-binning factor lives in ONE buffer of nchans rows of 4P bytes (P = samples per
+     * row rounded up to 256): a byte form is 4 sample-shifted copies of P bytes (copy k at + k P), a uint16 form 2 copies of
+     * 2P bytes (copy k at + 2 k P). The offset-uint8 form of bin 2 / 4 and their uint16 form (the route of exception-heavy
+     * chunks) share the rows: a channel group takes one route or the other, never both. */
+    uint8_t* d_x4 = nullptr;                 /* bin 1: the 4 sample-shifted copies of the uint8 chunk */
+    size_t x4_pitch = 0, x4_stride = 0;      /* bytes between channel rows (4P) and between copies (P) */
     bool need_u8_copies = false;
-    size_t xb_pitch[9] = {0};                /* elements, indexed by bin */
-    uint16_t* d_xb[9] = {nullptr};           /* binned input indexed by bin: copy 0, then copy 1 at +xb_stride bytes */
+    size_t xb_pitch[9] = {0};                /* uint16 ELEMENTS between channel rows (2P), indexed by bin */
+    uint16_t* d_xb[9] = {nullptr};           /* binned input indexed by bin: copy 0, then copy 1 at +xb_stride bytes (2P) */
     size_t xb_stride[9] = {0};
     /* offset-uint8 form of the binned inputs (bin 2, 4): 4 shifted byte copies, per-channel offsets, exceptions */
-    uint8_t* d_lo[9] = {nullptr};            /* copy k at + k*lo_stride bytes */
-    size_t lo_pitch[9] = {0}, lo_stride[9] = {0};
+    uint8_t* d_lo[9] = {nullptr};            /* copy k at + k*lo_stride bytes (P); the same memory as d_xb of the bin */
+    size_t lo_pitch[9] = {0}, lo_stride[9] = {0};   /* bytes between channel rows (4P) and between copies (P) */
     int32_t* d_off[9] = {nullptr};           /* [nchans] */
     uint2* d_exc[9] = {nullptr};             /* [kMaxGroups][exc_cap] */
     unsigned* d_exc_cnt[9] = {nullptr};      /* [kMaxGroups] exception counters, then [kMaxGroups] int32 biases (one memset clears both) */
@@ -128,6 +133,7 @@ struct Strategy {
     cudaStream_t compute = nullptr, copy = nullptr;
     cudaStream_t aux = nullptr;                       /* library-owned: every other DM range's K2 runs here, so that the tail
                                                          wave of one range overlaps the first wave of the next */
+    cudaStream_t d2h = nullptr;                       /* library-owned: candidate records leave the device here */
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     bool owns_compute = false, owns_copy = false;
     cudaEvent_t ev_copied[2] = {nullptr, nullptr};    /* chunk landed in d_raw[b] (copy stream) */

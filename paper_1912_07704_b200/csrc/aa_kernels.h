@@ -39,12 +39,12 @@ int aak_scatter_exceptions(const uint2* exc, const unsigned* exc_cnt, unsigned c
                            int32_t ndms, int32_t bin, int64_t nt, int32_t* D, int64_t pitch, void* stream);
 
 /* ---- K1 fused: one read of raw rows [0, nrows) (pointers already offset to the first row; chan0 = its channel index)
- * writes the 4 uint8 copies (x4, may be NULL), the offset-uint8 forms lo2 / lo4 with their 4 copies and exceptions (may be
+ * writes the 4 uint8 copies (x4, may be NULL; rows x4_pitch bytes apart, copy k at + k x4_stride), the offset-uint8 forms lo2 / lo4 with their 4 copies and exceptions (may be
  * NULL; off2/off4 offset to the first row; nb = valid binned samples) and the 2 copies of the uint16 bin-8 input (xb8,
  * may be NULL; xb8_pitch in elements, xb8_stride in bytes). ngroups = 16-byte groups per row. */
 typedef struct {
     const uint8_t* raw; size_t pitch; int64_t ngroups; int32_t chan0; unsigned cap;
-    uint8_t* x4; size_t x4_stride;
+    uint8_t* x4; size_t x4_pitch, x4_stride;
     uint8_t* lo2; size_t lo2_pitch, lo2_stride; const int32_t* off2; uint2* exc2; unsigned* cnt2; int64_t nb2;
     uint8_t* lo4; size_t lo4_pitch, lo4_stride; const int32_t* off4; uint2* exc4; unsigned* cnt4; int64_t nb4;
     uint16_t* xb8; size_t xb8_pitch, xb8_stride;

@@ -73,7 +73,7 @@ aa_status enqueue_prep(Strategy& s, const Chunk& c, int b, int32_t c0, int32_t c
     aak_prep_args a;
     memset(&a, 0, sizeof a);
     a.raw = raw; a.pitch = s.in_pitch; a.ngroups = (int64_t)(s.in_pitch / 16); a.chan0 = c0; a.cap = kExcCap;
-    if (s.need_u8_copies) { a.x4 = s.d_x4 + (size_t)c0 * s.in_pitch; a.x4_stride = s.x4_stride; }
+    if (s.need_u8_copies) { a.x4 = s.d_x4 + (size_t)c0 * s.x4_pitch; a.x4_pitch = s.x4_pitch; a.x4_stride = s.x4_stride; }
     if (s.d_lo[2]) {
         a.lo2 = s.d_lo[2] + (size_t)c0 * s.lo_pitch[2]; a.lo2_pitch = s.lo_pitch[2]; a.lo2_stride = s.lo_stride[2]; a.off2 = s.d_off[2] + c0;
         a.exc2 = s.d_exc[2] + (size_t)g * kExcCap; a.cnt2 = s.d_exc_cnt[2] + g; a.nb2 = (int64_t)(c.len / 2);
@@ -88,10 +88,10 @@ aa_status enqueue_prep(Strategy& s, const Chunk& c, int b, int32_t c0, int32_t c
         if (!s.d_xb[bin]) continue;
         const unsigned* cnt = s.d_lo[bin] ? s.d_exc_cnt[bin] + g : nullptr;      /* NULL: the range has no offset-uint8 route */
         const unsigned lim = cnt ? group_limit(s, bin, c0, c1) : 0u;
-        const size_t pitch_bytes = s.xb_pitch[bin] * 2;
+        const size_t pitch_bytes = s.xb_pitch[bin] * 2;           /* a row = 2 copies of xb_stride bytes */
         uint16_t* xb = s.d_xb[bin] + (size_t)c0 * s.xb_pitch[bin];
         AA_LAUNCH(aak_bin_time(raw, s.in_pitch, xb, s.xb_pitch[bin], n, (int64_t)(c.len / (uint64_t)bin), bin, cnt, lim, s.compute), "time binning");
-        AA_LAUNCH(aak_shift_copy((const uint8_t*)xb, (uint8_t*)xb + s.xb_stride[bin], pitch_bytes, pitch_bytes, n, 2, cnt, lim, s.compute), "shift copy (uint16)");
+        AA_LAUNCH(aak_shift_copy((const uint8_t*)xb, (uint8_t*)xb + s.xb_stride[bin], pitch_bytes, s.xb_stride[bin], n, 2, cnt, lim, s.compute), "shift copy (uint16)");
     }
     return AA_OK;
 }
@@ -116,7 +116,7 @@ aa_status enqueue_k2(Strategy& s, const Chunk& c, int32_t c0, int32_t c1, bool a
         a.chan_begin = c0; a.chan_end = c1; a.accumulate = accumulate ? 1 : 0;
         if (rg.naive) {
             const void* x0 = bin == 1 ? (const void*)s.d_x4 : (const void*)s.d_xb[bin];        /* copy 0 of the range's input form */
-            const size_t pitch_elems = bin == 1 ? s.in_pitch : s.xb_pitch[bin];
+            const size_t pitch_elems = bin == 1 ? s.x4_pitch : s.xb_pitch[bin];
             AA_LAUNCH(aak_dedisperse_naive(x0, pitch_elems, bin > 1, rg.d_delays, s.plan.nchans, c0, c1, rg.r.ndms, a.nt, rg.d_D, rg.pitch,
                                            accumulate ? 1 : 0, st), "dedispersion (global-memory route)");
             continue;
@@ -182,17 +182,19 @@ aa_status enqueue_dedispersion(Strategy& s, int64_t j, int b, const uint8_t* tm_
             aa_status st = enqueue_prep(s, c, b, groups->c[g], groups->c[g + 1], g);
             if (st != AA_OK) return st;
             if (g == 0) AA_CUDA(cudaEventRecord(s.ev_t[1], s.compute), "cudaEventRecord");
+            if (g == groups->n - 1) { AA_CUDA(cudaEventRecord(s.ev_raw_free[slot], s.compute), "cudaEventRecord"); s.raw_free_recorded[slot] = true; }
             if ((st = enqueue_k2(s, c, groups->c[g], groups->c[g + 1], g > 0, g)) != AA_OK) return st;
         }
     } else {
         aa_status st = enqueue_prep(s, c, b, 0, C, 0);
         if (st != AA_OK) return st;
         AA_CUDA(cudaEventRecord(s.ev_t[1], s.compute), "cudaEventRecord");
+        /* K1 was the last reader of the H2D buffer (K2 reads the input forms K1 wrote): the next chunk's copy may start now */
+        AA_CUDA(cudaEventRecord(s.ev_raw_free[slot], s.compute), "cudaEventRecord");
+        s.raw_free_recorded[slot] = true;
         if ((st = enqueue_k2(s, c, 0, C, false, 0)) != AA_OK) return st;
     }
     AA_CUDA(cudaEventRecord(s.ev_t[2], s.compute), "cudaEventRecord");
-    AA_CUDA(cudaEventRecord(s.ev_raw_free[slot], s.compute), "cudaEventRecord");
-    s.raw_free_recorded[slot] = true;
     s.timed = true; s.stats_timed = false;
     s.current_chunk = j;
     s.pending_sps = true;
@@ -219,8 +221,10 @@ aa_status harvest(Strategy& s) {
         const size_t old = s.cands.size();
         s.cands.resize(old + (size_t)take);
         static_assert(sizeof(aa_candidate) == sizeof(aak_candidate), "candidate layouts must match");
-        AA_CUDA(cudaMemcpyAsync(s.cands.data() + old, s.d_cands, (size_t)take * sizeof(aa_candidate), cudaMemcpyDeviceToHost, s.compute), "candidate D2H");
-        AA_CUDA(cudaStreamSynchronize(s.compute), "cudaStreamSynchronize");
+        /* on the library's own stream: the compute stream may already hold the next chunk's K2 (200 ms), and ev_count says the
+         * records are complete; the next K4 is enqueued only after this returns */
+        AA_CUDA(cudaMemcpyAsync(s.cands.data() + old, s.d_cands, (size_t)take * sizeof(aa_candidate), cudaMemcpyDeviceToHost, s.d2h), "candidate D2H");
+        AA_CUDA(cudaStreamSynchronize(s.d2h), "cudaStreamSynchronize");
         std::sort(s.cands.begin() + (ptrdiff_t)old, s.cands.end(), cand_less);   /* chunks arrive in order: canonical */
     }
     s.harvest_pending = false;
@@ -237,7 +241,8 @@ extern "C" aa_status aa_run_dedispersion(aa_strategy* h, const uint8_t* host_inp
     const bool tmajor = s.plan.layout == AA_LAYOUT_TIME_MAJOR;
     if (!tmajor && row_stride_bytes < s.nsamp_total) { set_error("aa_run_dedispersion: row_stride_bytes = %zu is shorter than nsamp_total = %llu", row_stride_bytes, (unsigned long long)s.nsamp_total); return AA_ERR_INVALID_ARG; }
     if (tmajor && row_stride_bytes < (size_t)s.plan.nchans) { set_error("aa_run_dedispersion: row_stride_bytes = %zu is shorter than nchans = %d (time-major plan)", row_stride_bytes, s.plan.nchans); return AA_ERR_INVALID_ARG; }
-    const bool two_buffers = s.d_raw[1] || s.d_stage[1];
+    const bool two_buffers = s.d_stage[1] != nullptr;      /* time-major staging; a channel-major plan has ONE H2D buffer */
+    const bool prefetch = s.chunks.size() > 1;
     if (s.pending_sps) { set_error("aa_run_dedispersion: chunk %lld is dedispersed but aa_run_sps has not run on it yet", (long long)s.current_chunk); return AA_ERR_ORDER; }
     if (s.next_chunk >= (int64_t)s.chunks.size()) { set_error("aa_run_dedispersion: all %zu chunks are done (aa_strategy_reset rewinds)", s.chunks.size()); return AA_ERR_ORDER; }
     const int64_t j = s.next_chunk;
@@ -266,8 +271,9 @@ extern "C" aa_status aa_run_dedispersion(aa_strategy* h, const uint8_t* host_inp
     if ((st = enqueue_dedispersion(s, j, b, nullptr, 0, groups.n ? &groups : nullptr)) != AA_OK) return st;
     /* double buffering: start moving chunk j+1 while chunk j computes (north_star "Streaming") */
     const int64_t jn = j + s.shard_world;           /* the next chunk of this strategy's shard */
-    if (two_buffers && jn < (int64_t)s.chunks.size() && s.raw_holds[b ^ 1] != jn)
-        if ((st = enqueue_h2d(s, jn, b ^ 1, host_input, row_stride_bytes, false)) != AA_OK) return st;
+    const int bn = two_buffers ? (b ^ 1) : 0;       /* the single buffer is free again once K1 of chunk j has run (ev_raw_free) */
+    if (prefetch && jn < (int64_t)s.chunks.size() && s.raw_holds[bn] != jn)
+        if ((st = enqueue_h2d(s, jn, bn, host_input, row_stride_bytes, false)) != AA_OK) return st;
     return AA_OK;
 }
 
@@ -286,11 +292,13 @@ extern "C" aa_status aa_run_dedispersion_device(aa_strategy* h, const uint8_t* d
             set_error("aa_run_dedispersion_device: a time-major device chunk must be 4-byte aligned with row_stride_bytes a multiple of 4 and >= nchans rounded up to 4 (got %zu)", row_stride_bytes);
             return AA_ERR_INVALID_ARG;
         }
-        s.raw_holds[0] = j;
+        /* the corner turn writes d_raw[0]; nothing else is in flight into it (host prefetches of a time-major plan go to d_stage) */
         return enqueue_dedispersion(s, j, 0, device_chunk, row_stride_bytes);
     }
     if (row_stride_bytes < c.len) { set_error("aa_run_dedispersion_device: row_stride_bytes = %zu is shorter than the chunk (%llu)", row_stride_bytes, (unsigned long long)c.len); return AA_ERR_INVALID_ARG; }
-    const int b = s.d_raw[1] ? (int)((j / s.shard_world) & 1) : 0;
+    const int b = 0;
+    /* a host prefetch of an earlier aa_run_dedispersion(host) may still be writing this buffer on the copy stream */
+    if (s.raw_holds[b] >= 0) AA_CUDA(cudaStreamWaitEvent(s.compute, s.ev_copied[b], 0), "cudaStreamWaitEvent");
     AA_CUDA(cudaMemcpy2DAsync(s.d_raw[b], s.in_pitch, device_chunk, row_stride_bytes, (size_t)c.len, (size_t)s.plan.nchans,
                               cudaMemcpyDeviceToDevice, s.compute), "cudaMemcpy2DAsync (D2D chunk)");
     s.raw_holds[b] = j;

@@ -42,13 +42,13 @@ int64_t delay_of(const Strategy& s, const Range& rg, int32_t chan, int32_t dm_in
 }
 
 /* Channel rows of the NCOPY shifted copies seen as overlapping 256-byte segments: a {256, nseg, NCOPY, 1} box lands as
- * NCOPY linear windows of window_bytes each (k_dedisp.cu). */
-static bool make_window_map(CUtensorMap* map, void* base, size_t pitch_bytes, size_t copy_stride, int32_t ncopy, int32_t nchans,
-                            int32_t window_bytes) {
+ * NCOPY linear windows of window_bytes each (k_dedisp.cu). Rows are pitch_bytes apart, the copies of a row copy_stride. */
+static bool make_window_map(CUtensorMap* map, void* base, size_t row_bytes, size_t pitch_bytes, size_t copy_stride, int32_t ncopy,
+                            int32_t nchans, int32_t window_bytes) {
     EncodeTiledFn enc = encode_fn();
     if (!enc) { set_error("aa_strategy_setup: cuTensorMapEncodeTiled is not available from this driver"); return false; }
     const cuuint32_t nseg = (cuuint32_t)(window_bytes / 256);
-    cuuint64_t dims[4] = {(cuuint64_t)pitch_bytes, nseg, (cuuint64_t)ncopy, (cuuint64_t)nchans};
+    cuuint64_t dims[4] = {(cuuint64_t)row_bytes, nseg, (cuuint64_t)ncopy, (cuuint64_t)nchans};   /* row_bytes: one copy of one channel */
     cuuint64_t strides[3] = {256, (cuuint64_t)copy_stride, (cuuint64_t)pitch_bytes};
     cuuint32_t box[4] = {256, nseg, (cuuint32_t)ncopy, 1};
     cuuint32_t es[4] = {1, 1, 1, 1};
@@ -59,46 +59,49 @@ static bool make_window_map(CUtensorMap* map, void* base, size_t pitch_bytes, si
 }
 
 /* Everything that depends on the chunk length L. Carves (or, on a dry arena, only measures) the device buffers. */
-static void carve(Strategy& s, int64_t L, bool two_raw) {
+static void carve(Strategy& s, int64_t L, bool two_stage) {
     Arena& a = s.arena;
     a.used = 0;
     s.in_pitch = round_up((size_t)L, 256);
     const size_t raw_bytes = (size_t)s.plan.nchans * s.in_pitch + kSlack;
+    /* ONE raw buffer also when chunks are double-buffered: only K1 reads it (3 ms of a 200 ms step), so the copy of the next
+     * chunk starts when K1 of this one is done and still overlaps the whole of K2 */
     s.d_raw[0] = (uint8_t*)a.take(raw_bytes);
+    s.d_raw[1] = nullptr;
     s.d_stage[0] = s.d_stage[1] = nullptr;
     if (s.plan.layout == AA_LAYOUT_TIME_MAJOR) {
         /* the chunk lands time-major in a staging buffer (two when chunks are double-buffered); one channel-major buffer */
         s.stage_stride = round_up((size_t)s.plan.nchans, 16);
         const size_t stage_bytes = (size_t)L * s.stage_stride + kSlack;
         s.d_stage[0] = (uint8_t*)a.take(stage_bytes);
-        s.d_stage[1] = two_raw ? (uint8_t*)a.take(stage_bytes) : nullptr;
-        s.d_raw[1] = nullptr;
-    } else {
-        s.d_raw[1] = two_raw ? (uint8_t*)a.take(raw_bytes) : nullptr;
+        s.d_stage[1] = two_stage ? (uint8_t*)a.take(stage_bytes) : nullptr;
     }
-    s.x4_stride = round_up(raw_bytes, 256);
-    s.d_x4 = s.need_u8_copies ? (uint8_t*)a.take(4 * s.x4_stride) : nullptr;
+    /* input forms: nchans rows of 4P bytes per binning factor (aa_internal.h), kSlack readable bytes after the last row */
+    s.x4_stride = s.in_pitch;
+    s.x4_pitch = 4 * s.in_pitch;
+    s.d_x4 = s.need_u8_copies ? (uint8_t*)a.take((size_t)s.plan.nchans * s.x4_pitch + kSlack) : nullptr;
     for (int b = 2; b <= 8; b *= 2) {
-        bool used = false;
-        for (const Range& rg : s.ranges) used = used || rg.r.bin == b;
-        s.xb_pitch[b] = used ? round_up((size_t)(L / b), 256) : 0;
-        s.xb_stride[b] = round_up((size_t)s.plan.nchans * s.xb_pitch[b] * 2 + kSlack, 256);
-        s.d_xb[b] = used ? (uint16_t*)a.take(2 * s.xb_stride[b]) : nullptr;
-    }
-    for (int bn = 2; bn <= 4; bn *= 2) {
-        bool used = false;
+        bool used = false, lo = false;
         int64_t nd = 0;
-        for (const Range& rg : s.ranges) if (rg.r.bin == bn && rg.has_lo) { used = true; nd += rg.r.ndms; }
-        s.lo_pitch[bn] = used ? round_up((size_t)(L / bn), 256) : 0;
-        s.lo_stride[bn] = round_up((size_t)s.plan.nchans * s.lo_pitch[bn] + kSlack, 256);
-        s.d_lo[bn] = used ? (uint8_t*)a.take(4 * s.lo_stride[bn]) : nullptr;
-        s.d_off[bn] = used ? (int32_t*)a.take((size_t)s.plan.nchans * 4) : nullptr;
-        s.d_exc[bn] = used ? (uint2*)a.take((size_t)kMaxGroups * kExcCap * sizeof(uint2)) : nullptr;
-        s.d_exc_cnt[bn] = used ? (unsigned*)a.take(2 * kMaxGroups * 4) : nullptr;
+        for (const Range& rg : s.ranges) {
+            used = used || rg.r.bin == b;
+            if (rg.r.bin == b && rg.has_lo) { lo = true; nd += rg.r.ndms; }
+        }
+        const size_t P = used ? round_up((size_t)(L / b), 256) : 0;
+        uint8_t* base = used ? (uint8_t*)a.take((size_t)s.plan.nchans * 4 * P + kSlack) : nullptr;
+        s.d_xb[b] = (uint16_t*)base;
+        s.xb_pitch[b] = 2 * P;                     /* elements: a row is 2 copies of 2P bytes */
+        s.xb_stride[b] = 2 * P;                    /* bytes */
+        s.d_lo[b] = lo ? base : nullptr;           /* the same rows as 4 copies of P bytes */
+        s.lo_pitch[b] = lo ? 4 * P : 0;
+        s.lo_stride[b] = lo ? P : 0;
+        s.d_off[b] = lo ? (int32_t*)a.take((size_t)s.plan.nchans * 4) : nullptr;
+        s.d_exc[b] = lo ? (uint2*)a.take((size_t)kMaxGroups * kExcCap * sizeof(uint2)) : nullptr;
+        s.d_exc_cnt[b] = lo ? (unsigned*)a.take(2 * kMaxGroups * 4) : nullptr;
         /* the scatter costs one atomic per (exception, trial), measured 2.7e10 atomics/s: beyond ~1e8 of them per chunk the
          * uint16 route is cheaper (a channel group gets the share of its channels) */
-        s.exc_limit[bn] = used ? (unsigned)std::min<int64_t>((int64_t)kMaxGroups * kExcCap, std::max<int64_t>(1, 100000000 / std::max<int64_t>(1, nd))) : 0;
-        if (used && !s.d_k_needed) s.d_k_needed = true;
+        s.exc_limit[b] = lo ? (unsigned)std::min<int64_t>((int64_t)kMaxGroups * kExcCap, std::max<int64_t>(1, 100000000 / std::max<int64_t>(1, nd))) : 0;
+        if (lo && !s.d_k_needed) s.d_k_needed = true;
     }
     s.d_k = s.d_k_needed ? (double*)a.take((size_t)s.plan.nchans * 8) : nullptr;
     const int64_t n_out = L - s.S;
@@ -283,6 +286,11 @@ static aa_status plan_host(aa_strategy* h, const aa_plan* plan, uint64_t nsamp_t
     /* a naive range reads the uint16 form of its bin on every chunk, so that bin keeps no offset-uint8 route */
     for (const Range& nv : s.ranges)
         if (nv.naive) for (Range& rg : s.ranges) if (rg.r.bin == nv.r.bin) rg.has_lo = false;
+    /* the uint16 input of a bin is written per BIN (only for exception-heavy chunks once the bin has an offset-uint8 buffer),
+     * while its ranges pick their route per RANGE: a range without the offset-uint8 plan (its byte window did not fit) would
+     * then read a uint16 buffer that a sparse chunk never filled. So a bin keeps the route only if all its ranges have it. */
+    for (const Range& nl : s.ranges)
+        if (!nl.has_lo) for (Range& rg : s.ranges) if (rg.r.bin == nl.r.bin) rg.has_lo = false;
     s.S = (int64_t)round_up((size_t)smax, (size_t)s.B);
     const int64_t usable = (int64_t)(nsamp_total / (uint64_t)s.B) * s.B;
     if (usable <= s.S) {
@@ -292,7 +300,7 @@ static aa_status plan_host(aa_strategy* h, const aa_plan* plan, uint64_t nsamp_t
 
     /* chunk length under the budget (reading C3): whole observation if it fits, else the largest power of two */
     s.arena.dry = true; s.arena.base = nullptr; s.arena.size = 0;
-    auto need = [&](int64_t L) { const bool two = (L < usable); carve(s, L, two); return s.arena.used; };
+    auto need = [&](int64_t L) { const bool two = (L < usable); carve(s, L, two); return s.arena.used; };   /* two: double-buffered staging */
     int64_t L = 0;
     if (chunk_len_hint) {
         L = (int64_t)chunk_len_hint;
@@ -375,7 +383,7 @@ extern "C" aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, u
     }
     const int32_t C = s.plan.nchans;
     const int64_t L = s.L;
-    const bool two_raw = s.chunks.size() > 1;
+    const bool two_stage = s.chunks.size() > 1;
 
     /* the single allocation (north_star "one allocation per run") */
     if (device_arena) {
@@ -388,7 +396,7 @@ extern "C" aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, u
         s.arena.base = (uint8_t*)p; s.arena.size = bytes_needed; s.owns_arena = true;
     }
     s.arena.dry = false;
-    carve(s, L, two_raw);
+    carve(s, L, two_stage);
 
     /* streams, events, pinned counter */
     cudaError_t e;
@@ -403,6 +411,7 @@ extern "C" aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, u
     }
     if ((e = cudaEventCreateWithFlags(&s.ev_count, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
     if ((e = cudaStreamCreateWithFlags(&s.aux, cudaStreamNonBlocking)) != cudaSuccess) return fail(cuda_fail(e, "cudaStreamCreate"));
+    if ((e = cudaStreamCreateWithFlags(&s.d2h, cudaStreamNonBlocking)) != cudaSuccess) return fail(cuda_fail(e, "cudaStreamCreate"));
     if ((e = cudaEventCreateWithFlags(&s.ev_fork, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
     if ((e = cudaEventCreateWithFlags(&s.ev_join, cudaEventDisableTiming)) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
     for (int g = 0; g < kMaxGroups; ++g)
@@ -427,12 +436,12 @@ extern "C" aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, u
             const size_t n = s.ranges.size();
             if ((e = cudaMemcpyAsync(rg.lo.d_etab, etabs[n + r].data(), etabs[n + r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
             if ((e = cudaMemcpyAsync(rg.lo.d_x0tab, x0tabs[n + r].data(), x0tabs[n + r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
-            if (!make_window_map(&rg.lo.map, s.d_lo[rg.r.bin], s.lo_pitch[rg.r.bin], s.lo_stride[rg.r.bin], 4, C, rg.lo.window_bytes)) return fail(AA_ERR_CUDA);
+            if (!make_window_map(&rg.lo.map, s.d_lo[rg.r.bin], s.lo_stride[rg.r.bin], s.lo_pitch[rg.r.bin], s.lo_stride[rg.r.bin], 4, C, rg.lo.window_bytes)) return fail(AA_ERR_CUDA);
         }
         if (rg.in16) {
-            if (!make_window_map(&rg.map, s.d_xb[rg.r.bin], s.xb_pitch[rg.r.bin] * 2, s.xb_stride[rg.r.bin], 2, C, rg.window_bytes)) return fail(AA_ERR_CUDA);
+            if (!make_window_map(&rg.map, s.d_xb[rg.r.bin], s.xb_stride[rg.r.bin], s.xb_pitch[rg.r.bin] * 2, s.xb_stride[rg.r.bin], 2, C, rg.window_bytes)) return fail(AA_ERR_CUDA);
         } else {
-            if (!make_window_map(&rg.map, s.d_x4, s.in_pitch, s.x4_stride, 4, C, rg.window_bytes)) return fail(AA_ERR_CUDA);
+            if (!make_window_map(&rg.map, s.d_x4, s.x4_stride, s.x4_pitch, s.x4_stride, 4, C, rg.window_bytes)) return fail(AA_ERR_CUDA);
         }
         for (int32_t i = 0; i < rg.r.ndms; ++i) {
             const int32_t* base = rg.d_D + (size_t)i * (size_t)rg.pitch;
@@ -461,6 +470,7 @@ extern "C" void aa_strategy_destroy(aa_strategy* h) {
         if (s.ev_h2d[b]) cudaEventDestroy(s.ev_h2d[b]);
     }
     if (s.aux) { cudaStreamSynchronize(s.aux); cudaStreamDestroy(s.aux); }
+    if (s.d2h) { cudaStreamSynchronize(s.d2h); cudaStreamDestroy(s.d2h); }
     if (s.ev_fork) cudaEventDestroy(s.ev_fork);
     if (s.ev_join) cudaEventDestroy(s.ev_join);
     if (s.ev_count) cudaEventDestroy(s.ev_count);
@@ -524,8 +534,8 @@ extern "C" size_t aa_strategy_describe(const aa_strategy* h, char* buf, size_t b
     snprintf(line, sizeof line, "strategy: nchans=%d nsamp=%llu B=%d overlap S=%lld chunk L=%lld n_out=%lld nchunks=%zu\n", s.plan.nchans,
              (unsigned long long)s.nsamp_total, s.B, (long long)s.S, (long long)s.L, (long long)s.n_out, s.chunks.size());
     o += line;
-    snprintf(line, sizeof line, "arena: %zu bytes used of %zu (%s), input pitch %zu, raw buffers %d, uint8 shifted copies %s\n", s.arena.used,
-             s.arena.size, s.owns_arena ? "library-owned, one cudaMalloc" : "caller-owned", s.in_pitch, (s.d_raw[1] || s.d_stage[1]) ? 2 : 1,
+    snprintf(line, sizeof line, "arena: %zu bytes used of %zu (%s), input pitch %zu, H2D buffers %d, uint8 shifted copies %s\n", s.arena.used,
+             s.arena.size, s.owns_arena ? "library-owned, one cudaMalloc" : "caller-owned", s.in_pitch, s.d_stage[0] ? (s.d_stage[1] ? 2 : 1) : 1,
              s.need_u8_copies ? "4" : "none");
     o += line;
     for (const Range& rg : s.ranges) {

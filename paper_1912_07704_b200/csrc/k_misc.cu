@@ -176,13 +176,28 @@ k_scatter_exceptions(const uint2* __restrict__ exc, const unsigned* __restrict__
  * (The uint16 forms of bin 2 / 4 are written by k_bin_time / k_shift_copy, only for exception-heavy chunks.) */
 struct PrepFused {
     const uint8_t* raw; size_t pitch; long long ngroups; int chan0; unsigned cap;
-    uint8_t* x4; size_t x4_stride;
+    uint8_t* x4; size_t x4_pitch, x4_stride;
     uint8_t* lo2; size_t lo2_pitch, lo2_stride; const int32_t* off2; uint2* exc2; unsigned* cnt2; long long nb2;
     uint8_t* lo4; size_t lo4_pitch, lo4_stride; const int32_t* off4; uint2* exc4; unsigned* cnt4; long long nb4;
     uint16_t* xb8; size_t xb8_pitch, xb8_stride;
 };
 
 __device__ __forceinline__ uint32_t byte_of(const uint32_t (&w)[8], int i) { return (w[i >> 2] >> (8 * (i & 3))) & 0xFFu; }
+
+/* Append one exception record. The lanes of a warp that arrive together share ONE atomic on the counter; once the counter
+ * has passed `cap` the chunk is bound for the other route anyway (every route test is `counter > limit`, limit <= cap, and
+ * the counter never decreases), so nothing more is counted or recorded: a dense input costs one L2 read per exception
+ * instead of one same-address atomic. */
+__device__ __forceinline__ void append_exception(uint2* __restrict__ exc, unsigned* __restrict__ cnt, unsigned cap, uint2 rec) {
+    if (*reinterpret_cast<volatile unsigned*>(cnt) > cap) return;
+    const unsigned m = __activemask();
+    const int lane = threadIdx.x & 31, leader = __ffs(m) - 1;
+    unsigned base = 0;
+    if (lane == leader) base = atomicAdd(cnt, (unsigned)__popc(m));
+    base = __shfl_sync(m, base, leader);
+    const unsigned idx = base + (unsigned)__popc(m & ((1u << lane) - 1u));
+    if (idx < cap) exc[idx] = rec;
+}
 
 __global__ void __launch_bounds__(256)
 k_prep_fused(const PrepFused p) {
@@ -194,7 +209,7 @@ k_prep_fused(const PrepFused p) {
     const uint4 n = *reinterpret_cast<const uint4*>(src + 16);          /* rows are padded: readable past the chunk */
     const uint32_t w[8] = {a.x, a.y, a.z, a.w, n.x, n.y, n.z, n.w};
     if (p.x4) {
-        const size_t off = (size_t)c * p.pitch + (size_t)g * 16;
+        const size_t off = (size_t)c * p.x4_pitch + (size_t)g * 16;
         *reinterpret_cast<uint4*>(p.x4 + off) = a;
 #pragma unroll
         for (int k = 1; k < 4; ++k) {
@@ -213,10 +228,8 @@ k_prep_fused(const PrepFused p) {
             const int v = y < 0 ? 0 : (y > 255 ? 255 : y);
             l[k] = (uint32_t)v;
             const long long t = g * 8 + k;
-            if (k < 8 && y != v && t < p.nb2) {
-                const unsigned idx = atomicAdd(p.cnt2, 1u);
-                if (idx < p.cap) p.exc2[idx] = make_uint2((uint32_t)(p.chan0 + c) | ((uint32_t)(y - v + 1024) << 16), (uint32_t)t);
-            }
+            if (k < 8 && y != v && t < p.nb2)
+                append_exception(p.exc2, p.cnt2, p.cap, make_uint2((uint32_t)(p.chan0 + c) | ((uint32_t)(y - v + 1024) << 16), (uint32_t)t));
         }
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
@@ -234,10 +247,8 @@ k_prep_fused(const PrepFused p) {
             const int v = y < 0 ? 0 : (y > 255 ? 255 : y);
             l[k] = (uint32_t)v;
             const long long t = g * 4 + k;
-            if (k < 4 && y != v && t < p.nb4) {
-                const unsigned idx = atomicAdd(p.cnt4, 1u);
-                if (idx < p.cap) p.exc4[idx] = make_uint2((uint32_t)(p.chan0 + c) | ((uint32_t)(y - v + 1024) << 16), (uint32_t)t);
-            }
+            if (k < 4 && y != v && t < p.nb4)
+                append_exception(p.exc4, p.cnt4, p.cap, make_uint2((uint32_t)(p.chan0 + c) | ((uint32_t)(y - v + 1024) << 16), (uint32_t)t));
         }
 #pragma unroll
         for (int j = 0; j < 4; ++j)
@@ -375,7 +386,12 @@ extern "C" int aak_chan_offsets(const uint8_t* x, size_t pitch, int64_t len, int
 
 extern "C" int aak_scatter_exceptions(const uint2* exc, const unsigned* exc_cnt, unsigned cap, const double* k, double dm_low,
                                       double dm_step, int32_t ndms, int32_t bin, int64_t nt, int32_t* D, int64_t pitch, void* stream) {
-    k_scatter_exceptions<<<148 * 4, 256, 0, (cudaStream_t)stream>>>(exc, exc_cnt, cap, k, dm_low, dm_step, ndms, bin, nt, D, pitch);
+    static int nsm = 0;
+    if (!nsm) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) nsm = 148;
+    }
+    k_scatter_exceptions<<<nsm * 4, 256, 0, (cudaStream_t)stream>>>(exc, exc_cnt, cap, k, dm_low, dm_step, ndms, bin, nt, D, pitch);
     return (int)cudaGetLastError();
 }
 
@@ -383,7 +399,7 @@ extern "C" int aak_prep_fused(const aak_prep_args* a, int32_t nrows, void* strea
     if (nrows <= 0 || a->ngroups <= 0) return 0;
     PrepFused p;
     p.raw = a->raw; p.pitch = a->pitch; p.ngroups = a->ngroups; p.chan0 = a->chan0; p.cap = a->cap;
-    p.x4 = a->x4; p.x4_stride = a->x4_stride;
+    p.x4 = a->x4; p.x4_pitch = a->x4_pitch; p.x4_stride = a->x4_stride;
     p.lo2 = a->lo2; p.lo2_pitch = a->lo2_pitch; p.lo2_stride = a->lo2_stride; p.off2 = a->off2; p.exc2 = a->exc2; p.cnt2 = a->cnt2; p.nb2 = a->nb2;
     p.lo4 = a->lo4; p.lo4_pitch = a->lo4_pitch; p.lo4_stride = a->lo4_stride; p.off4 = a->off4; p.exc4 = a->exc4; p.cnt4 = a->cnt4; p.nb4 = a->nb4;
     p.xb8 = a->xb8; p.xb8_pitch = a->xb8_pitch; p.xb8_stride = a->xb8_stride;

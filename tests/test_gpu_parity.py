@@ -190,7 +190,7 @@ def test_sharded_strategies_match_the_oracle_per_shard_and_reproduce_the_single_
             mine = replicas.chunks_of_rank(nchunks, rank, 2)
             exp_all = []
             for n, j in enumerate(mine):
-                assert g.st.info["next_chunk"] == j
+                assert g.aa.aa_strategy_get_info(g.h)["next_chunk"] == j
                 g.dedisperse()                                   # the shard's cursor: chunks rank, rank + 2, ...
                 status = g.sps()
                 assert status == (g.aa.AA_STATUS_FINISHED if n == len(mine) - 1 else g.aa.AA_STATUS_CHUNK_DONE)
