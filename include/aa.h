@@ -122,6 +122,16 @@ aa_status aa_plan_set_input_layout(aa_plan* plan, int32_t layout);
  * Must be called before aa_strategy_setup binds the plan. */
 aa_status aa_plan_set_boxcar_overlap(aa_plan* plan, int32_t on);
 
+/* Per-width measured statistics (reading C7m; off by default; §1 "boxcar filters and peak-finding to
+ * maximise signal-to-noise"). By default a boxcar of width w is normalised with the width-1 statistics of its row scaled for
+ * white noise (w mu, sqrt(w) sigma). on != 0: for every row and every plan width w the series B_w[t] = sum_{j<w} D[t+j],
+ * t in [0, n_w), n_w = min(T_r, samples present - w + 1), gets its OWN robust statistics (the same iterated 3-sigma clip on
+ * exact integer moments, pivot p_w = B_w[0]) and SNR_w[t] = ((double)(B_w[t] - p_w) - (mu_w - p_w)) * (1 / sigma_w). A width
+ * whose series is constant or clips to nothing gives no SNR in that row. For w = 1 this is the default exactly; for red
+ * (correlated) noise the sqrt(w) scaling overstates the SNR of wide boxcars and this option does not. Costs one more kernel
+ * (K3w) that reads D once per clip iteration. Must be called before aa_strategy_setup binds the plan. */
+aa_status aa_plan_set_per_width_stats(aa_plan* plan, int32_t on);
+
 /* ------------------------------------------------------------------------------------------------ strategy
  * PAPER.md:47 steps 4-6 ("bind", "the API calculates the optimal strategy", "checks whether all modules are
  * configured"). Host-side planning plus ONE device allocation (or none if the caller lends an arena):
@@ -237,6 +247,11 @@ aa_status aa_get_dedispersed_row(aa_strategy* s, int32_t range, int32_t dm_index
 /* mu, sigma, n kept, clip iterations of a row, as computed by aa_run_sps for the current chunk. */
 aa_status aa_get_row_stats(aa_strategy* s, int32_t range, int32_t dm_index, double* mu, double* sigma,
                            int64_t* n_kept, int32_t* iterations);
+/* Reading C7m only (aa_plan_set_per_width_stats): mu_w, sigma_w (0 = this width gives no SNR in this row) and the pivot
+ * p_w = B_w[0] of plan width `width_index` in a row, as computed by aa_run_sps for the current chunk.
+ * AA_ERR_ORDER if the option is off or aa_run_sps has not run. */
+aa_status aa_get_row_width_stats(aa_strategy* s, int32_t range, int32_t dm_index, int32_t width_index, double* mu, double* sigma,
+                                 int64_t* pivot);
 /* Per-row moments sum_t D and sum_t t*D (int64) of every row of a range, computed on the device (test hook for the
  * all-rows checksum). out arrays are HOST, length ndms. */
 aa_status aa_get_row_moments(aa_strategy* s, int32_t range, int64_t* sum_d, int64_t* sum_td);

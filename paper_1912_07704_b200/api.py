@@ -17,7 +17,7 @@ __all__ = [
     "AaError", "AA_OK", "AA_STATUS_CHUNK_DONE", "AA_STATUS_FINISHED", "AA_ERR_INVALID_ARG", "AA_ERR_NOT_READY",
     "AA_ERR_BUDGET_TOO_SMALL", "AA_ERR_CUDA", "AA_ERR_CANDIDATE_OVERFLOW", "AA_ERR_ORDER", "AA_ERR_INTERNAL",
     "CANDIDATE_DTYPE", "lib_path", "load",
-    "AA_LAYOUT_CHANNEL_MAJOR", "AA_LAYOUT_TIME_MAJOR", "aa_plan_create", "aa_plan_destroy", "aa_plan_set_input_layout", "aa_plan_set_boxcar_overlap", "aa_strategy_plan", "aa_strategy_setup", "aa_strategy_destroy", "aa_strategy_get_info",
+    "AA_LAYOUT_CHANNEL_MAJOR", "AA_LAYOUT_TIME_MAJOR", "aa_plan_create", "aa_plan_destroy", "aa_plan_set_input_layout", "aa_plan_set_boxcar_overlap", "aa_plan_set_per_width_stats", "aa_get_row_width_stats", "aa_strategy_plan", "aa_strategy_setup", "aa_strategy_destroy", "aa_strategy_get_info",
     "aa_strategy_get_range_info", "aa_strategy_get_chunk", "aa_strategy_get_delay", "aa_strategy_describe",
     "aa_strategy_reset", "aa_strategy_shard", "aa_run_dedispersion", "aa_run_dedispersion_device", "aa_run_sps", "aa_run_pipeline", "aa_get_candidates", "aa_get_clusters", "aa_cluster_candidates", "CLUSTER_DTYPE",
     "aa_get_dedispersed_row", "aa_get_row_stats", "aa_get_row_moments", "aa_get_dedispersed_device", "aa_synchronize",
@@ -91,6 +91,8 @@ def load():
         "aa_plan_destroy": (None, [vp]),
         "aa_plan_set_input_layout": (c_int32, [vp, c_int32]),
         "aa_plan_set_boxcar_overlap": (c_int32, [vp, c_int32]),
+        "aa_plan_set_per_width_stats": (c_int32, [vp, c_int32]),
+        "aa_get_row_width_stats": (c_int32, [vp, c_int32, c_int32, c_int32, POINTER(c_double), POINTER(c_double), POINTER(c_int64)]),
         "aa_strategy_setup": (c_int32, [POINTER(vp), vp, c_uint64, vp, c_size_t, c_size_t, vp, vp, c_size_t, c_uint64]),
         "aa_strategy_plan": (c_int32, [POINTER(vp), vp, c_uint64, c_size_t, c_size_t, c_uint64]),
         "aa_strategy_destroy": (None, [vp]),
@@ -174,6 +176,10 @@ def aa_plan_set_input_layout(plan, layout: int) -> int:
 
 def aa_plan_set_boxcar_overlap(plan, on: bool) -> int:
     return _check(load().aa_plan_set_boxcar_overlap(plan, 1 if on else 0))
+
+
+def aa_plan_set_per_width_stats(plan, on: bool) -> int:
+    return _check(load().aa_plan_set_per_width_stats(plan, 1 if on else 0))
 
 
 def aa_plan_destroy(plan) -> None:
@@ -329,6 +335,13 @@ def aa_get_row_stats(strategy, rng: int, dm_index: int):
     return mu.value, sg.value, n.value, it.value
 
 
+def aa_get_row_width_stats(strategy, rng: int, dm_index: int, width_index: int):
+    """(mu_w, sigma_w, p_w) of one plan width in one row (reading C7m plans only)."""
+    mu, sg, pv = c_double(), c_double(), c_int64()
+    _check(load().aa_get_row_width_stats(strategy, rng, dm_index, width_index, byref(mu), byref(sg), byref(pv)))
+    return mu.value, sg.value, pv.value
+
+
 def aa_get_row_moments(strategy, rng: int, ndms: int | None = None):
     """sum_t D and sum_t t*D of every row of a range. The arrays are sized from the strategy's own range info (the C side
     writes ndms values whatever the caller believes); `ndms`, if given, is only checked against it."""
@@ -383,13 +396,15 @@ class Plan:
     """Owns an aa_plan handle."""
 
     def __init__(self, chan_freq_mhz, tsamp_s, ranges, boxcar_widths, snr_threshold, time_major: bool = False,
-                 boxcar_overlap: bool = False):
+                 boxcar_overlap: bool = False, per_width_stats: bool = False):
         self.handle = aa_plan_create(chan_freq_mhz, tsamp_s, ranges, boxcar_widths, snr_threshold)
         self.ranges = [tuple(r) for r in ranges]
         if time_major:
             aa_plan_set_input_layout(self.handle, AA_LAYOUT_TIME_MAJOR)
         if boxcar_overlap:
             aa_plan_set_boxcar_overlap(self.handle, True)
+        if per_width_stats:
+            aa_plan_set_per_width_stats(self.handle, True)
 
     def close(self):
         if getattr(self, "handle", None):

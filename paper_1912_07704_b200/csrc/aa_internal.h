@@ -38,6 +38,7 @@ struct Plan {
     float threshold = 0.f;
     int32_t layout = 0;           /* aa_input_layout */
     bool boxcar_overlap = false;  /* reading C3x */
+    bool per_width = false;       /* reading C7m */
 };
 
 /* Single-allocation bump allocator over caller- or library-owned device memory. */
@@ -124,6 +125,9 @@ struct Strategy {
     aak_row_desc* d_rows[2] = {nullptr, nullptr};   /* [0] full chunk geometry, [1] last (short) chunk */
     double* d_mu_sigma = nullptr;            /* [nrows][2] */
     int64_t* d_n_iters = nullptr;            /* [nrows][2] */
+    double* d_wstats = nullptr;              /* reading C7m: [nrows][nwidths][2] = mu_w, sigma_w */
+    int64_t* d_wpivot = nullptr;             /* [nrows][nwidths] p_w */
+    int32_t* d_wlive = nullptr;              /* [nrows] */
     aak_candidate* d_cands = nullptr;
     unsigned long long* d_counter = nullptr;
     long long* d_moments = nullptr;          /* [2][max ndms] */

@@ -109,6 +109,20 @@ typedef struct {
 int aak_row_stats(const aak_row_desc* rows, int32_t nrows, double* mu_sigma /* [nrows][2] */,
                   int64_t* n_iters /* [nrows][2] */, void* stream);
 
+/* ---- K3w: per-width measured statistics (reading C7m): for every row of one range and every plan width w, the series
+ * B_w[t] = sum_{j<w} D[t+j], t in [0, n_w), n_w = min(nt, nt_data - w + 1), is given reading C6 about the pivot p_w = B_w[0]
+ * (exact integer moments, iterated 3-sigma clip, at most 8 clips). Outputs per (row, width): wstats = {mu_w, sigma_w} with
+ * sigma_w = 0 when the width yields no SNR in this row (n_w < 1, constant series, degenerate clip); wpivot = p_w;
+ * wlive[row] = 1 if any width of the row has sigma_w > 0. */
+typedef struct {
+    const int32_t* D; int64_t pitch; int64_t nt; int64_t nt_data; int32_t ndms;
+    int32_t widths[16]; int32_t nwidths;
+    double* wstats;       /* [ndms][nwidths][2] */
+    int64_t* wpivot;      /* [ndms][nwidths] */
+    int32_t* wlive;       /* [ndms] */
+} aak_wstats_args;
+int aak_row_width_stats(const aak_wstats_args* a, void* stream);
+
 /* ---- K4: boxcar SNR + 3x3 peaks + candidate append ---------------------------------------------------------------- */
 typedef struct {
     uint64_t sample; float dm; float snr; uint32_t width; uint32_t range; uint32_t dm_index;
@@ -122,6 +136,8 @@ typedef struct {
     int32_t widths[16]; int32_t nwidths;
     double threshold;
     aak_candidate* cands; unsigned long long* counter; unsigned long long capacity;
+    /* reading C7m (per-width measured statistics), all NULL for reading C7: the outputs of aak_row_width_stats for this range */
+    const double* wstats; const int64_t* wpivot; const int32_t* wlive;
 } aak_sps_args;
 int aak_sps_peaks(const aak_sps_args* a, void* stream);
 int aak_sps_init(void);

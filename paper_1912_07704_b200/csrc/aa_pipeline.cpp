@@ -317,6 +317,17 @@ extern "C" aa_status aa_run_sps(aa_strategy* h) {
     AA_CUDA(cudaMemsetAsync(s.d_counter, 0, sizeof(unsigned long long), s.compute), "cudaMemsetAsync");
     AA_CUDA(cudaEventRecord(s.ev_t[3], s.compute), "cudaEventRecord");
     AA_LAUNCH(aak_row_stats(s.d_rows[is_short ? 1 : 0], (int32_t)s.nrows, s.d_mu_sigma, s.d_n_iters, s.compute), "row statistics");
+    const size_t nwd = s.plan.widths.size();
+    if (s.plan.per_width) {                        /* reading C7m: every width's own statistics, range by range (K3w) */
+        for (Range& rg : s.ranges) {
+            aak_wstats_args a;
+            a.D = rg.d_D; a.pitch = rg.pitch; a.nt = (int64_t)(c.n_out / (uint64_t)rg.r.bin); a.nt_data = a.nt + rg.extra; a.ndms = rg.r.ndms;
+            a.nwidths = (int32_t)nwd;
+            for (int k = 0; k < 16; ++k) a.widths[k] = k < a.nwidths ? s.plan.widths[(size_t)k] : 0;
+            a.wstats = s.d_wstats + 2 * nwd * rg.first_row; a.wpivot = s.d_wpivot + nwd * rg.first_row; a.wlive = s.d_wlive + rg.first_row;
+            AA_LAUNCH(aak_row_width_stats(&a, s.compute), "per-width row statistics");
+        }
+    }
     AA_CUDA(cudaEventRecord(s.ev_t[4], s.compute), "cudaEventRecord");
     for (Range& rg : s.ranges) {
         aak_sps_args a;
@@ -327,6 +338,9 @@ extern "C" aa_status aa_run_sps(aa_strategy* h) {
         for (int k = 0; k < 16; ++k) a.widths[k] = k < a.nwidths ? s.plan.widths[(size_t)k] : 0;
         a.threshold = (double)s.plan.threshold;
         a.cands = s.d_cands; a.counter = s.d_counter; a.capacity = s.max_candidates;
+        a.wstats = s.plan.per_width ? s.d_wstats + 2 * nwd * rg.first_row : nullptr;
+        a.wpivot = s.plan.per_width ? s.d_wpivot + nwd * rg.first_row : nullptr;
+        a.wlive = s.plan.per_width ? s.d_wlive + rg.first_row : nullptr;
         AA_LAUNCH(aak_sps_peaks(&a, s.compute), "sps peaks");
     }
     AA_CUDA(cudaEventRecord(s.ev_t[5], s.compute), "cudaEventRecord");
@@ -438,6 +452,29 @@ extern "C" aa_status aa_get_row_stats(aa_strategy* h, int32_t range, int32_t dm_
     if (sigma) *sigma = ms[1];
     if (n_kept) *n_kept = ni[0];
     if (iterations) *iterations = (int32_t)ni[1];
+    return AA_OK;
+}
+
+extern "C" aa_status aa_get_row_width_stats(aa_strategy* h, int32_t range, int32_t dm_index, int32_t width_index, double* mu, double* sigma,
+                                            int64_t* pivot) {
+    aa_status st = check_ready(h, "aa_get_row_width_stats");
+    if (st != AA_OK) return st;
+    Strategy& s = h->s;
+    if (!s.plan.per_width) { set_error("aa_get_row_width_stats: the plan does not ask for per-width statistics (aa_plan_set_per_width_stats)"); return AA_ERR_ORDER; }
+    if (!s.stats_timed) { set_error("aa_get_row_width_stats: aa_run_sps has not run on the current chunk"); return AA_ERR_ORDER; }
+    const size_t nwd = s.plan.widths.size();
+    if (range < 0 || range >= (int32_t)s.ranges.size() || dm_index < 0 || dm_index >= s.ranges[(size_t)range].r.ndms || width_index < 0 ||
+        width_index >= (int32_t)nwd) {
+        set_error("aa_get_row_width_stats: range %d / dm_index %d / width_index %d out of bounds", range, dm_index, width_index); return AA_ERR_INVALID_ARG;
+    }
+    const size_t o = (s.ranges[(size_t)range].first_row + (size_t)dm_index) * nwd + (size_t)width_index;
+    double ms[2]; int64_t pv;
+    AA_CUDA(cudaMemcpyAsync(ms, s.d_wstats + 2 * o, sizeof ms, cudaMemcpyDeviceToHost, s.compute), "width stats D2H");
+    AA_CUDA(cudaMemcpyAsync(&pv, s.d_wpivot + o, sizeof pv, cudaMemcpyDeviceToHost, s.compute), "width stats D2H");
+    AA_CUDA(cudaStreamSynchronize(s.compute), "cudaStreamSynchronize");
+    if (mu) *mu = ms[0];
+    if (sigma) *sigma = ms[1];
+    if (pivot) *pivot = pv;
     return AA_OK;
 }
 

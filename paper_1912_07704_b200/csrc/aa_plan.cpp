@@ -98,6 +98,12 @@ extern "C" aa_status aa_plan_set_boxcar_overlap(aa_plan* plan, int32_t on) {
     return AA_OK;
 }
 
+extern "C" aa_status aa_plan_set_per_width_stats(aa_plan* plan, int32_t on) {
+    if (!plan) { aa::set_error("aa_plan_set_per_width_stats: plan is NULL"); return AA_ERR_NOT_READY; }
+    plan->p.per_width = on != 0;
+    return AA_OK;
+}
+
 extern "C" aa_status aa_plan_set_input_layout(aa_plan* plan, int32_t layout) {
     if (!plan) { aa::set_error("aa_plan_set_input_layout: plan is NULL"); return AA_ERR_NOT_READY; }
     if (layout != AA_LAYOUT_CHANNEL_MAJOR && layout != AA_LAYOUT_TIME_MAJOR) {

@@ -121,6 +121,10 @@ static void carve(Strategy& s, int64_t L, bool two_stage) {
     s.d_rows[1] = (aak_row_desc*)a.take(s.nrows * sizeof(aak_row_desc));
     s.d_mu_sigma = (double*)a.take(s.nrows * 2 * sizeof(double));
     s.d_n_iters = (int64_t*)a.take(s.nrows * 2 * sizeof(int64_t));
+    const size_t nwd = s.plan.widths.size();
+    s.d_wstats = s.plan.per_width ? (double*)a.take(s.nrows * nwd * 2 * sizeof(double)) : nullptr;
+    s.d_wpivot = s.plan.per_width ? (int64_t*)a.take(s.nrows * nwd * sizeof(int64_t)) : nullptr;
+    s.d_wlive = s.plan.per_width ? (int32_t*)a.take(s.nrows * sizeof(int32_t)) : nullptr;
     s.d_cands = (aak_candidate*)a.take(s.max_candidates * sizeof(aak_candidate));
     s.d_counter = (unsigned long long*)a.take(256);
     int32_t maxnd = 0;

@@ -28,6 +28,7 @@ typedef unsigned __int128 u128;
 
 /* ------------------------------------------------------------------------------------------------ K3 */
 constexpr int STAT_THREADS = 512;
+constexpr int SPS_MAXW = 16;                 /* aa_plan_create: at most 16 boxcar widths */
 
 __device__ __forceinline__ double u128_to_double_rn(u128 v) {
     const u64 hi = (u64)(v >> 64);
@@ -274,6 +275,194 @@ k_row_stats(const aak_row_desc* __restrict__ rows, double* __restrict__ mu_sigma
     }
 }
 
+
+/* ------------------------------------------------------------------------------------------------ K3w
+ * Per-width measured statistics (reading C7m; SURVEY §8(f3) "per-width measured sigma instead of sqrt(w)
+ * scaling"). One CTA per DM row. The row is walked in tiles: exclusive prefix sums of d = D - D[0] in shared memory (thread
+ * scan + warp shuffle scan + cross-warp carry), then e = B_w[t] - w D[0] = I[t+w] - I[t] for every width that is still
+ * iterating, and the exact integer moments (n, sum e, sum e^2) of the kept samples. One pass over the row per clip iteration
+ * (pass 0 unclipped, then at most 8 clips), all widths in the same pass. The moments are taken about w D[0] (e fits int32 by
+ * the plan's boxcar limit; sum e^2 is carried to 96 bits) and moved to the definition's pivot p_w = B_w[0] exactly in
+ * 128-bit integers before the double arithmetic, which follows reading C6 operation by operation. */
+constexpr int PW_THREADS = 512;
+constexpr int PW_TILE = 4096;                 /* series samples per tile */
+constexpr int PW_MAXW = 2048;                 /* aa_plan_create: boxcar widths <= 2048 */
+constexpr int PW_EPT = (PW_TILE + PW_MAXW) / PW_THREADS;     /* 12 contiguous elements per thread */
+static_assert(PW_EPT * PW_THREADS == PW_TILE + PW_MAXW && PW_EPT % 4 == 0, "prefix tile layout");
+
+struct PwParams {
+    const int32_t* D; i64 pitch; i64 nt; i64 ntd; int widths[SPS_MAXW]; int nwidths; int wmax;
+    double* wstats; i64* wpivot; int* wlive;
+};
+
+struct PwSmem {
+    unsigned I[PW_TILE + PW_MAXW + 8];        /* I[e] = sum_{j<e} d[t0+j] (mod 2^32) */
+    unsigned wtot[PW_THREADS / 32];
+    u64 red[SPS_MAXW][PW_THREADS / 32][6];    /* per width and warp: n, sum e, and sum e^2 as four 32-bit limbs */
+    i64 nw[SPS_MAXW];                         /* series length n_w */
+    int q[SPS_MAXW];                          /* B_w[0] - w p */
+    int lo[SPS_MAXW], hi[SPS_MAXW];           /* clip bounds on e, clamped to int32 (lo > hi: nothing is kept) */
+    int active[SPS_MAXW];                     /* still iterating */
+    u64 pn[SPS_MAXW]; i64 ps1[SPS_MAXW]; u64 ps2lo[SPS_MAXW], ps2hi[SPS_MAXW];      /* previous keep set */
+    double mu[SPS_MAXW], sigma[SPS_MAXW];
+    int nactive;
+};
+
+__device__ __forceinline__ i64 clamp_i64(double x) {
+    if (!(x > -9.0e18)) return (i64)(-9000000000000000000ll);
+    if (!(x < 9.0e18)) return (i64)(9000000000000000000ll);
+    return (i64)x;                            /* x is integral here */
+}
+
+template <int NWT>
+__global__ void __launch_bounds__(PW_THREADS, 1)
+k_row_width_stats(const PwParams p) {
+    __shared__ PwSmem sm;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int32_t* D = p.D + (size_t)blockIdx.x * (size_t)p.pitch;
+    const int pv = D[0];
+    const i64 T = p.nt, Tx = p.ntd;
+    if (tid < SPS_MAXW) {
+        i64 n = 0;
+        if (tid < p.nwidths) { n = Tx - p.widths[tid] + 1; if (n > T) n = T; if (n < 0) n = 0; }
+        sm.nw[tid] = n; sm.active[tid] = n >= 1 ? 1 : 0; sm.q[tid] = 0; sm.lo[tid] = INT32_MIN; sm.hi[tid] = INT32_MAX;
+        sm.mu[tid] = 0.0; sm.sigma[tid] = 0.0;
+    }
+    if (tid == 0) sm.nactive = 1;
+    __syncthreads();
+
+    for (int pass = 0; pass <= 8 && sm.nactive > 0; ++pass) {
+        unsigned an[NWT], ahi[NWT]; i64 as1[NWT]; u64 alo[NWT];
+#pragma unroll
+        for (int iw = 0; iw < NWT; ++iw) { an[iw] = 0; ahi[iw] = 0; as1[iw] = 0; alo[iw] = 0; }
+        for (i64 t0 = 0; t0 < T; t0 += PW_TILE) {
+            /* ---- exclusive prefix sums of the segment [t0, t0 + PW_TILE + wmax) that exists */
+            const i64 avail = Tx - t0;
+            const int ne = (int)(avail < (i64)(PW_TILE + p.wmax) ? avail : (i64)(PW_TILE + p.wmax));
+            const int e0 = tid * PW_EPT;
+            unsigned loc[PW_EPT];
+            unsigned run = 0;
+#pragma unroll
+            for (int v = 0; v < PW_EPT / 4; ++v) {
+                const int e = e0 + 4 * v;
+                int4 x = make_int4(pv, pv, pv, pv);
+                if (e < ne) x = __ldg(reinterpret_cast<const int4*>(D + t0 + e));      /* rows are padded to 128 elements */
+                loc[4 * v + 0] = run; run += (unsigned)(x.x - pv);
+                loc[4 * v + 1] = run; run += (unsigned)(x.y - pv);
+                loc[4 * v + 2] = run; run += (unsigned)(x.z - pv);
+                loc[4 * v + 3] = run; run += (unsigned)(x.w - pv);
+            }
+            unsigned incl = run;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const unsigned u = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += u;
+            }
+            if (lane == 31) sm.wtot[warp] = incl;
+            __syncthreads();
+            unsigned carry = incl - run;
+#pragma unroll
+            for (int w = 0; w < PW_THREADS / 32; ++w) carry += (w < warp) ? sm.wtot[w] : 0u;
+#pragma unroll
+            for (int v = 0; v < PW_EPT / 4; ++v)
+                *reinterpret_cast<uint4*>(&sm.I[e0 + 4 * v]) = make_uint4(loc[4 * v] + carry, loc[4 * v + 1] + carry, loc[4 * v + 2] + carry, loc[4 * v + 3] + carry);
+            if (tid == PW_THREADS - 1) sm.I[PW_TILE + PW_MAXW] = run + carry;
+            __syncthreads();
+            if (pass == 0 && t0 == 0 && tid < p.nwidths && sm.nw[tid] >= 1) sm.q[tid] = (int)sm.I[p.widths[tid]];   /* B_w[0] - w p */
+
+            /* ---- moments of the kept samples of every width that is still iterating */
+            int klim[NWT], lo[NWT], hi[NWT];                          /* samples of this tile that belong to the width's series */
+            int kmax = 0;
+#pragma unroll
+            for (int iw = 0; iw < NWT; ++iw) {
+                const i64 left = sm.nw[iw] - t0;
+                klim[iw] = sm.active[iw] ? (int)(left < 0 ? 0 : (left > (i64)PW_TILE ? (i64)PW_TILE : left)) : 0;
+                lo[iw] = sm.lo[iw]; hi[iw] = sm.hi[iw];
+                kmax = klim[iw] > kmax ? klim[iw] : kmax;
+            }
+#pragma unroll 2
+            for (int k = tid; k < kmax; k += PW_THREADS) {
+                const unsigned base = sm.I[k];
+#pragma unroll
+                for (int iw = 0; iw < NWT; ++iw) {
+                    if (k >= klim[iw]) continue;
+                    const int e = (int)(sm.I[k + p.widths[iw]] - base);
+                    if (e < lo[iw] || e > hi[iw]) continue;
+                    const u64 e2 = (u64)((i64)e * (i64)e);
+                    ++an[iw]; as1[iw] += e;
+                    alo[iw] += e2; ahi[iw] += (alo[iw] < e2) ? 1u : 0u;
+                }
+            }
+            __syncthreads();
+        }
+        /* ---- block totals per width */
+#pragma unroll
+        for (int iw = 0; iw < NWT; ++iw) {
+            if (!sm.active[iw]) continue;                             /* block-uniform */
+            u64 v[6] = {(u64)an[iw], (u64)as1[iw], alo[iw] & 0xFFFFFFFFull, alo[iw] >> 32, (u64)ahi[iw], 0ull};
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+                for (int j = 0; j < 5; ++j) v[j] += __shfl_down_sync(0xffffffffu, v[j], o);
+            }
+            if (lane == 0) {
+#pragma unroll
+                for (int j = 0; j < 5; ++j) sm.red[iw][warp][j] = v[j];
+            }
+        }
+        __syncthreads();
+        if (tid < p.nwidths && sm.active[tid]) {
+            const int iw = tid;
+            u64 n2 = 0; i64 s1e = 0; u128 s2e = 0;
+            for (int w = 0; w < PW_THREADS / 32; ++w) {
+                n2 += sm.red[iw][w][0]; s1e += (i64)sm.red[iw][w][1];
+                s2e += (u128)sm.red[iw][w][2] + ((u128)sm.red[iw][w][3] << 32) + ((u128)sm.red[iw][w][4] << 64);
+            }
+            bool done = false;
+            if (pass > 0 && n2 == 0) {                                /* degenerate clip: the width yields no SNR in this row */
+                sm.sigma[iw] = 0.0; done = true;
+            } else {
+                const bool same = pass > 0 && n2 == sm.pn[iw] && s1e == sm.ps1[iw] && (u64)s2e == sm.ps2lo[iw] && (u64)(s2e >> 64) == sm.ps2hi[iw];
+                sm.pn[iw] = n2; sm.ps1[iw] = s1e; sm.ps2lo[iw] = (u64)s2e; sm.ps2hi[iw] = (u64)(s2e >> 64);
+                /* to the pivot of the definition, p_w = B_w[0] = w p + q: d = e - q */
+                const i64 q = sm.q[iw];
+                const __int128 S1 = (__int128)s1e - (__int128)n2 * q;
+                const __int128 S2 = (__int128)s2e - 2 * (__int128)q * (__int128)s1e + (__int128)n2 * ((__int128)q * q);
+                const u128 num = (u128)((__int128)n2 * S2 - S1 * S1);           /* n^2 * variance, exact, >= 0 */
+                const i64 pw = (i64)p.widths[iw] * (i64)pv + q;
+                const double nd = __ull2double_rn(n2);
+                const double mu = __dadd_rn(__ll2double_rn(pw), __ddiv_rn(__ll2double_rn((i64)S1), nd));
+                const double sigma = __dsqrt_rn(__ddiv_rn(u128_to_double_rn(num), __dmul_rn(nd, nd)));
+                sm.mu[iw] = mu; sm.sigma[iw] = sigma;
+                if (same || pass == 8) done = true;
+                else {
+                    const double t3 = __dmul_rn(3.0, sigma);
+                    const i64 shift = (i64)p.widths[iw] * (i64)pv;            /* bounds on B_w -> bounds on e = B_w - w p */
+                    const i64 l = clamp_i64(ceil(__dsub_rn(mu, t3))) - shift, h = clamp_i64(floor(__dadd_rn(mu, t3))) - shift;
+                    if (l > (i64)INT32_MAX || h < (i64)INT32_MIN || l > h) { sm.lo[iw] = 1; sm.hi[iw] = 0; }
+                    else { sm.lo[iw] = l < (i64)INT32_MIN ? INT32_MIN : (int)l; sm.hi[iw] = h > (i64)INT32_MAX ? INT32_MAX : (int)h; }
+                }
+            }
+            if (done) sm.active[iw] = 0;
+        }
+        __syncthreads();
+        if (tid == 0) { int n = 0; for (int iw = 0; iw < p.nwidths; ++iw) n += sm.active[iw]; sm.nactive = n; }
+        __syncthreads();
+    }
+    if (tid < p.nwidths) {
+        const size_t o = (size_t)blockIdx.x * (size_t)p.nwidths + (size_t)tid;
+        const bool has = sm.nw[tid] >= 1;
+        p.wstats[2 * o] = has ? sm.mu[tid] : 0.0;
+        p.wstats[2 * o + 1] = has ? sm.sigma[tid] : 0.0;
+        p.wpivot[o] = has ? (i64)p.widths[tid] * (i64)pv + (i64)sm.q[tid] : 0;
+    }
+    if (tid == 0) {
+        int live = 0;
+        for (int iw = 0; iw < p.nwidths; ++iw) live |= (sm.nw[iw] >= 1 && sm.sigma[iw] > 0.0) ? 1 : 0;
+        p.wlive[blockIdx.x] = live;
+    }
+}
+
 /* ------------------------------------------------------------------------------------------------ K4
  * One CTA walks DOWN a band of K4_RB DM rows (plus one halo row above and below, recomputed, not exchanged) for one
  * strip of TT output samples. Per row step:
@@ -295,7 +484,6 @@ k_row_stats(const aak_row_desc* __restrict__ rows, double* __restrict__ mu_sigma
 constexpr int K4_THREADS = 256;
 constexpr int K4_WARPS = K4_THREADS / 32;
 constexpr int K4_RB = 32;                      /* centre rows per CTA (fewer when the grid would not fill the GPU) */
-constexpr int SPS_MAXW = 16;
 
 struct SpsParams {
     const int32_t* D; i64 pitch; i64 nt; i64 ntd; int ndms; int bin; int range_index;   /* ntd: samples present per row >= nt */
@@ -307,13 +495,15 @@ struct SpsParams {
     int rb;                                    /* centre rows per CTA */
     double threshold;
     aak_candidate* cands; u64* counter; u64 capacity;
+    const double* wstats; const i64* wpivot; const int* wlive;     /* reading C7m (NULL: reading C7) */
 };
 
 struct K4RowConst {                            /* per ring slot */
-    double a[SPS_MAXW];                        /* w * (mu - p) */
-    double inv[SPS_MAXW];                      /* 1 / (sqrt(w) * sigma) */
+    double a[SPS_MAXW];                        /* C7: w * (mu - p);          C7m: mu_w - p_w */
+    double inv[SPS_MAXW];                      /* C7: 1 / (sqrt(w) * sigma); C7m: 1 / sigma_w, or 0 = this width gives no SNR in this row */
     int bmin[SPS_MAXW];
-    int live;                                  /* row exists and sigma > 0 */
+    int q[SPS_MAXW];                           /* C7m: p_w - w p = B_w[0] - w p (0 for C7) */
+    int live;                                  /* row exists and has a positive sigma */
     int pad[3];
 };
 
@@ -327,14 +517,22 @@ struct K4Smem {
 };
 
 /* exact S (reading C7) of one position from a prefix row: e = element index of the position, t = its sample index */
+template <bool PW>
 __device__ __forceinline__ double k4_eval(const unsigned* I, const K4RowConst& rc, const SpsParams& p, int e, i64 t, int& bw) {
     double best = -CUDART_INF; bw = 0;
     const unsigned base = I[e - 1];
+    constexpr bool pw = PW;
     for (int iw = 0; iw < p.nwidths; ++iw) {
         const int w = p.widths[iw];
         if (t + w > p.ntd) break;                                  /* ascending widths */
         const int B = (int)(I[e + w - 1] - base);
-        const double snr = __dmul_rn(__dsub_rn(__int2double_rn(B), rc.a[iw]), rc.inv[iw]);
+        double snr;
+        if (pw) {                                                  /* reading C7m: ((double)(B_w - p_w) - (mu_w - p_w)) * (1 / sigma_w) */
+            if (!(rc.inv[iw] > 0.0)) continue;
+            snr = __dmul_rn(__dsub_rn(__ll2double_rn((i64)B - (i64)rc.q[iw]), rc.a[iw]), rc.inv[iw]);
+        } else {
+            snr = __dmul_rn(__dsub_rn(__int2double_rn(B), rc.a[iw]), rc.inv[iw]);
+        }
         if (snr > best) { best = snr; bw = w; }
     }
     return best;
@@ -377,7 +575,7 @@ __device__ __forceinline__ void k4_prefilter(const unsigned* __restrict__ I, con
     }
 }
 
-template <int V>
+template <int V, bool PW>
 __global__ void __launch_bounds__(K4_THREADS)
 k_sps_peaks(const SpsParams p) {
     extern __shared__ __align__(16) uint8_t k4_raw[];
@@ -411,6 +609,7 @@ k_sps_peaks(const SpsParams p) {
         pv = __ldg(row);
         mu = __ldg(p.mu_sigma + 2 * (size_t)r);
         sg = __ldg(p.mu_sigma + 2 * (size_t)r + 1);
+        if (PW) sg = __ldg(p.wlive + r) ? 1.0 : 0.0;            /* reading C7m: the row is live if any width has a sigma_w > 0 */
 #pragma unroll
         for (int v = 0; v < V; ++v) {
             const int e = e0 + 4 * v;                                /* tb and nt are multiples of 4 or the row is padded to 128 */
@@ -434,13 +633,26 @@ k_sps_peaks(const SpsParams p) {
             K4RowConst& rc = sm.rc[s4];
             if (tid == 0) rc.live = live ? 1 : 0;
             if (live && tid < p.nwidths) {
-                const double w = (double)p.widths[tid];
-                const double a = __dmul_rn(w, __dsub_rn(mu_c, (double)pv_c));
-                const double inv = __ddiv_rn(1.0, __dmul_rn(__dsqrt_rn(w), sg_c));
-                rc.a[tid] = a; rc.inv[tid] = inv;
-                const double x = a + p.threshold / inv;              /* real-valued bound on B_w - w p; margin below */
+                double a, inv, qd = 0.0;
+                int q = 0;
+                if (PW) {                                            /* reading C7m: this row's own statistics of B_w */
+                    const size_t o = (size_t)r * (size_t)p.nwidths + (size_t)tid;
+                    const double mu_w = __ldg(p.wstats + 2 * o), sg_w = __ldg(p.wstats + 2 * o + 1);
+                    const i64 pw = __ldg(p.wpivot + o);
+                    q = (int)(pw - (i64)p.widths[tid] * (i64)pv_c);
+                    qd = (double)q;
+                    a = __dsub_rn(mu_w, __ll2double_rn(pw));
+                    inv = sg_w > 0.0 ? __ddiv_rn(1.0, sg_w) : 0.0;
+                } else {
+                    const double w = (double)p.widths[tid];
+                    a = __dmul_rn(w, __dsub_rn(mu_c, (double)pv_c));
+                    inv = __ddiv_rn(1.0, __dmul_rn(__dsqrt_rn(w), sg_c));
+                }
+                rc.a[tid] = a; rc.inv[tid] = inv; if (PW) rc.q[tid] = q;
+                const double x = qd + a + p.threshold / inv;         /* real-valued bound on B_w - w p; margin below */
                 int bm;
-                if (x != x) bm = INT32_MIN;
+                if (!(inv > 0.0)) bm = INT32_MAX;                    /* no SNR from this width: never flagged */
+                else if (x != x) bm = INT32_MIN;
                 else if (x >= 2147483000.0) bm = INT32_MAX;
                 else if (x <= -2147483000.0) bm = INT32_MIN;
                 else bm = (int)floor(x) - 2;
@@ -512,7 +724,7 @@ k_sps_peaks(const SpsParams p) {
                     q = list[k];
                     const i64 t = t0 + q;
                     const int e = q + 4;
-                    sc = k4_eval(Irow[1], *rcs[1], p, e, t, bw);
+                    sc = k4_eval<PW>(Irow[1], *rcs[1], p, e, t, bw);
                     if (sc > p.threshold) {
                         is = true;
 #pragma unroll
@@ -524,7 +736,7 @@ k_sps_peaks(const SpsParams p) {
                                 const i64 tn = t + dq;
                                 if (tn < 0 || tn >= p.nt) continue;
                                 int dummy;
-                                const double v = k4_eval(Irow[dr + 1], *rcs[dr + 1], p, e + dq, tn, dummy);
+                                const double v = k4_eval<PW>(Irow[dr + 1], *rcs[dr + 1], p, e + dq, tn, dummy);
                                 const bool before = (dr < 0) || (dr == 0 && dq < 0);
                                 if (before ? !(sc > v) : !(sc >= v)) is = false;
                             }
@@ -567,12 +779,31 @@ extern "C" int aak_row_stats(const aak_row_desc* rows, int32_t nrows, double* mu
     return (int)cudaGetLastError();
 }
 
+extern "C" int aak_row_width_stats(const aak_wstats_args* a, void* stream) {
+    if (a->nwidths < 1 || a->nwidths > SPS_MAXW) return (int)cudaErrorInvalidValue;
+    if (a->nt <= 0 || a->ndms <= 0) return 0;
+    PwParams p;
+    p.D = a->D; p.pitch = a->pitch; p.nt = a->nt; p.ntd = a->nt_data > a->nt ? a->nt_data : a->nt; p.nwidths = a->nwidths; p.wmax = 0;
+    for (int k = 0; k < SPS_MAXW; ++k) { p.widths[k] = k < a->nwidths ? a->widths[k] : 0; if (p.widths[k] > p.wmax) p.wmax = p.widths[k]; }
+    if (p.wmax > PW_MAXW) return (int)cudaErrorInvalidValue;
+    p.wstats = a->wstats; p.wpivot = (i64*)a->wpivot; p.wlive = a->wlive;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (a->nwidths <= 4) k_row_width_stats<4><<<(unsigned)a->ndms, PW_THREADS, 0, st>>>(p);
+    else if (a->nwidths <= 8) k_row_width_stats<8><<<(unsigned)a->ndms, PW_THREADS, 0, st>>>(p);
+    else if (a->nwidths <= 12) k_row_width_stats<12><<<(unsigned)a->ndms, PW_THREADS, 0, st>>>(p);
+    else k_row_width_stats<16><<<(unsigned)a->ndms, PW_THREADS, 0, st>>>(p);
+    return (int)cudaGetLastError();
+}
+
 extern "C" int aak_sps_init(void) {
     int e;
     if ((e = (int)cudaFuncSetAttribute(k_row_stats, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(StatSmem)))) return e;
-    if ((e = (int)cudaFuncSetAttribute(k_sps_peaks<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(K4Smem<3>)))) return e;
-    if ((e = (int)cudaFuncSetAttribute(k_sps_peaks<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(K4Smem<4>)))) return e;
-    if ((e = (int)cudaFuncSetAttribute(k_sps_peaks<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(K4Smem<8>)))) return e;
+    if ((e = (int)cudaFuncSetAttribute(k_sps_peaks<3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(K4Smem<3>)))) return e;
+    if ((e = (int)cudaFuncSetAttribute(k_sps_peaks<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(K4Smem<4>)))) return e;
+    if ((e = (int)cudaFuncSetAttribute(k_sps_peaks<8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(K4Smem<8>)))) return e;
+    if ((e = (int)cudaFuncSetAttribute(k_sps_peaks<3, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(K4Smem<3>)))) return e;
+    if ((e = (int)cudaFuncSetAttribute(k_sps_peaks<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(K4Smem<4>)))) return e;
+    if ((e = (int)cudaFuncSetAttribute(k_sps_peaks<8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(K4Smem<8>)))) return e;
     return 0;
 }
 
@@ -585,6 +816,7 @@ extern "C" int aak_sps_peaks(const aak_sps_args* a, void* stream) {
     for (int k = 0; k < a->nwidths; ++k) if (a->widths[k] != (1 << k)) p.pow2 = 0;
     for (int k = 0; k < SPS_MAXW; ++k) { p.widths[k] = k < a->nwidths ? a->widths[k] : 0; if (p.widths[k] > p.wmax) p.wmax = p.widths[k]; }
     p.threshold = a->threshold; p.cands = a->cands; p.counter = (u64*)a->counter; p.capacity = a->capacity;
+    p.wstats = a->wstats; p.wpivot = (const i64*)a->wpivot; p.wlive = a->wlive;
     if (a->nt <= 0 || a->ndms <= 0) return 0;
     /* segment = tt + 4 + wmax elements <= 1024 V; the strip keeps at least ~2000 centre samples */
     const int V = p.wmax <= 1024 ? 3 : (p.wmax <= 2048 ? 4 : 8);
@@ -596,10 +828,11 @@ extern "C" int aak_sps_peaks(const aak_sps_args* a, void* stream) {
     while (p.rb > 2 && strips * ((a->ndms + p.rb - 1) / p.rb) < 2 * 148) p.rb /= 2;
     dim3 grid((unsigned)strips, (unsigned)((a->ndms + p.rb - 1) / p.rb));
     cudaStream_t st = (cudaStream_t)stream;
+    const bool pw = p.wstats != nullptr;
     switch (V) {
-        case 3: k_sps_peaks<3><<<grid, K4_THREADS, sizeof(K4Smem<3>), st>>>(p); break;
-        case 4: k_sps_peaks<4><<<grid, K4_THREADS, sizeof(K4Smem<4>), st>>>(p); break;
-        default: k_sps_peaks<8><<<grid, K4_THREADS, sizeof(K4Smem<8>), st>>>(p); break;
+        case 3: if (pw) k_sps_peaks<3, true><<<grid, K4_THREADS, sizeof(K4Smem<3>), st>>>(p); else k_sps_peaks<3, false><<<grid, K4_THREADS, sizeof(K4Smem<3>), st>>>(p); break;
+        case 4: if (pw) k_sps_peaks<4, true><<<grid, K4_THREADS, sizeof(K4Smem<4>), st>>>(p); else k_sps_peaks<4, false><<<grid, K4_THREADS, sizeof(K4Smem<4>), st>>>(p); break;
+        default: if (pw) k_sps_peaks<8, true><<<grid, K4_THREADS, sizeof(K4Smem<8>), st>>>(p); else k_sps_peaks<8, false><<<grid, K4_THREADS, sizeof(K4Smem<8>), st>>>(p); break;
     }
     return (int)cudaGetLastError();
 }

@@ -22,8 +22,8 @@ def make_input(w, pinned: bool = False):
 class OracleRun:
     """Oracle-side view of one workload: delay constants and binned chunks (cached per (chunk, bin))."""
 
-    def __init__(self, w, x):
-        self.w, self.x = w, x
+    def __init__(self, w, x, per_width: bool = False):
+        self.w, self.x, self.per_width = w, x, per_width
         self.k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
         self._xb = {}
 
@@ -40,7 +40,7 @@ class OracleRun:
         xb = self.binned(start, length, rng[3])
         # the C ABI takes the threshold as float and widens it (include/aa.h): the oracle is handed the same double
         return oracle.search_rows(xb, self.k, rng, r_index, n_out // rng[3], self.w.widths, float(np.float32(self.w.threshold)), start,
-                                  i0, i1, want=want, extra=extra)
+                                  i0, i1, want=want, extra=extra, per_width=self.per_width)
 
 
 def compare_candidates(got: np.ndarray, exp: np.ndarray, threshold: float, snr_rtol=1e-4, band=1e-3):
@@ -245,14 +245,14 @@ def run_oracle_slices(w, x, chunk, slices, processes: int | None = None, extra: 
 class GpuRun:
     """The CUDA path through the C-ABI binding for one workload (plan -> strategy -> chunk loop)."""
 
-    def __init__(self, w, x, time_major: bool = False, boxcar_overlap: bool = False, **strategy_kw):
+    def __init__(self, w, x, time_major: bool = False, boxcar_overlap: bool = False, per_width: bool = False, **strategy_kw):
         """x is always the channel-major array [nchans][nsamp] the oracle sees; with time_major=True the library is handed
         its transpose x_tm[t][c] (the plain definition of the corner turn) through a time-major plan."""
         import paper_1912_07704_b200 as aa
         self.aa, self.w = aa, w
         self.x = np.ascontiguousarray(x.T) if time_major else x
         self.plan = aa.Plan(w.freqs_mhz, w.tsamp_s, w.ranges, w.widths, w.threshold, time_major=time_major,
-                            boxcar_overlap=boxcar_overlap)
+                            boxcar_overlap=boxcar_overlap, per_width_stats=per_width)
         self.extra = max(w.widths) - 1 if boxcar_overlap else 0          # reading C3x
         self.st = aa.Strategy(self.plan, x.shape[1], **strategy_kw)
         self.h = self.st.handle
@@ -270,6 +270,9 @@ class GpuRun:
 
     def stats(self, r, i):
         return self.aa.aa_get_row_stats(self.h, r, i)
+
+    def width_stats(self, r, i, iw):
+        return self.aa.aa_get_row_width_stats(self.h, r, i, iw)
 
     def moments(self, r):
         return self.aa.aa_get_row_moments(self.h, r, self.w.ranges[r][2])

@@ -20,7 +20,7 @@ pytestmark = pytest.mark.gpu
 
 def _full_parity(w, x, **kw):
     """Every row of every range of every chunk: D, statistics, candidates."""
-    gpu, orc = GpuRun(w, x, **kw), OracleRun(w, x)
+    gpu, orc = GpuRun(w, x, **kw), OracleRun(w, x, per_width=kw.get("per_width", False))
     try:
         exp_all = []
         for j, chunk in enumerate(gpu.chunks):
@@ -299,3 +299,84 @@ def test_time_major_device_chunk_and_layout_errors():
         assert e.value.status == aa.AA_ERR_INVALID_ARG and "layout" in e.value.message
     finally:
         gpu.close()
+
+
+# ------------------------------------------------------------------------------------------------ reading C7m (per-width measured statistics)
+def _width_stats_parity(w, x, rows_per_range=6, **kw):
+    """mu_w, sigma_w, p_w of every plan width on sampled rows, == the oracle's (reading C7m), on the current chunk(s)."""
+    import oracle
+    gpu, orc = GpuRun(w, x, per_width=True, **kw), OracleRun(w, x, per_width=True)
+    n = 0
+    try:
+        for chunk in gpu.chunks:
+            gpu.dedisperse()
+            gpu.sps()
+            start, length, n_out = chunk
+            for r, rng in enumerate(w.ranges):
+                T = n_out // rng[3]
+                for i in sorted({int(q) for q in np.linspace(0, rng[2] - 1, rows_per_range)}):
+                    row = gpu.row(r, i).astype(np.int64)                      # T + E samples (already checked bit-exact elsewhere)
+                    _, _, ws = oracle.boxcar_snr_perwidth(row, T, w.widths)
+                    for iw in range(len(w.widths)):
+                        mu, sg, pv = gpu.width_stats(r, i, iw)
+                        assert (mu, sg, float(pv)) == (ws[iw][0], ws[iw][1], ws[iw][2]), (r, i, iw, (mu, sg, pv), tuple(ws[iw]))
+                        n += 1
+        return n
+    finally:
+        gpu.close()
+
+
+@pytest.mark.parametrize("kw", [{}, {"chunk_len_hint": 4096}, {"boxcar_overlap": True, "chunk_len_hint": 4096}])
+def test_per_width_statistics_every_row_matches_the_oracle(kw):
+    """SURVEY §8(f3) / DESIGN.md reading C7m with the option on: every row's D, every candidate (whole list) and the
+    per-width statistics equal the oracle's, on a plan with binned ranges, widths that are not powers of two, several chunks
+    and (third case) boxcars that cross the chunk end (reading C3x), where n_w differs per width."""
+    w = scaled(datagen.get_workload("tiny"), name="tiny_pw", nsamp=16384, ranges=((0.0, 1.0, 40, 1), (40.0, 2.0, 30, 4), (100.0, 4.0, 9, 8)),
+               widths=(1, 2, 3, 8, 21, 64), fixed_pulses=((20.0, 5000, 4, 14.0), (70.0, 9000, 16, 8.0)), threshold=5.5)
+    x, _ = make_input(w)
+    info, got, exp, (nmatch, og, oe) = _full_parity(w, x, per_width=True, **kw)
+    assert nmatch + og == len(got) and nmatch + oe == len(exp) and len(got) > 10
+    assert _width_stats_parity(w, x, **kw) > 0
+
+
+def test_per_width_statistics_on_red_noise_differ_from_sqrt_w_scaling_and_match_the_oracle():
+    """A slow baseline wander common to all channels makes every dedispersed row RED: sigma of a wide boxcar is then far
+    above sqrt(w) sigma_1, reading C7 reports inflated SNRs for wide boxcars and reading C7m does not. Both runs must equal
+    the oracle in their own reading; the C7m run must find fewer wide candidates than the C7 run on the same bytes."""
+    base = scaled(datagen.get_workload("tiny"), name="tiny_red", nsamp=32768, ranges=((0.0, 1.0, 48, 1), (48.0, 2.0, 16, 2)),
+                  widths=(1, 2, 4, 8, 16, 32, 64), fixed_pulses=((30.0, 9000, 8, 12.0),), threshold=6.0)
+    x, _ = make_input(base)
+    rs = np.random.default_rng(5)
+    wander = np.cumsum(rs.normal(0.0, 0.35, base.nsamp))
+    wander -= np.convolve(wander, np.ones(2048) / 2048, mode="same")            # keep it inside the byte range
+    x = np.clip(np.round(x.astype(np.float64) + wander[None, :]), 0, 255).astype(np.uint8)
+    _, got_w, exp_w, (nm_w, og_w, oe_w) = _full_parity(base, x, per_width=True)
+    _, got_c, exp_c, (nm_c, og_c, oe_c) = _full_parity(base, x)
+    assert nm_w + og_w == len(got_w) and nm_w + oe_w == len(exp_w)
+    assert nm_c + og_c == len(got_c) and nm_c + oe_c == len(exp_c)
+    wide_c = int(np.sum(got_c["width"] >= 32)); wide_w = int(np.sum(got_w["width"] >= 32))
+    assert wide_c > 4 * max(1, wide_w), (wide_c, wide_w)
+    assert _width_stats_parity(base, x, rows_per_range=4) > 0
+
+
+def test_per_width_statistics_full_length_rows_and_degenerate_widths():
+    """Rows of the Mid shape (T ~ 58 000: many tiles of K3w, ragged tail) with widths up to 512; a constant input gives
+    sigma_w = 0 for every width (no SNR, no candidates) on both sides; the hook refuses plans without the option."""
+    import paper_1912_07704_b200 as aa
+    w = scaled(datagen.get_workload("mid"), name="mid_pw", nsamp=65_536, nchans=256, ranges=((0.0, 0.5, 24, 1), (12.0, 1.0, 10, 2)),
+               widths=(1, 2, 4, 8, 16, 32, 64, 128, 256, 512), npulses=4, pulse_dm=(2.0, 20.0))
+    x, _ = make_input(w)
+    info, got, exp, (nmatch, og, oe) = _full_parity(w, x, per_width=True)
+    assert nmatch + og == len(got) and nmatch + oe == len(exp)
+    assert _width_stats_parity(w, x, rows_per_range=3) > 0
+    flat = np.full_like(x, 100)
+    info, got, exp, _ = _full_parity(w, flat, per_width=True)
+    assert len(got) == 0 and len(exp) == 0
+    g = GpuRun(w, x)
+    try:
+        g.dedisperse(); g.sps()
+        with pytest.raises(aa.AaError) as e:
+            g.width_stats(0, 0, 0)
+        assert e.value.status == aa.AA_ERR_ORDER
+    finally:
+        g.close()
