@@ -91,6 +91,47 @@ void dg_fill(uint8_t* out, size_t row_stride, int32_t nchans, int64_t t_begin, i
     }
 }
 
+/* The same recipe for 16-bit samples: x = clip(floor(v + 0.5), 0, max_value), max_value <= 65535 (the stated bit
+ * depth, e.g. 4095). out rows are row_stride BYTES apart. */
+void dg_fill16(uint16_t* out, size_t row_stride, int32_t nchans, int64_t t_begin, int64_t nsamp,
+               uint64_t seed, double mean, double sigma, double max_value,
+               int32_t npulses, const dg_pulse* pulses, const int64_t* pulse_delays)
+{
+    #pragma omp parallel for schedule(dynamic, 4)
+    for (int32_t c = 0; c < nchans; ++c) {
+        uint16_t* row = (uint16_t*)((uint8_t*)out + (size_t)c * row_stride);
+        int64_t t_end = t_begin + nsamp;
+        int64_t tp0 = t_begin >> 1, tp1 = (t_end + 1) >> 1;
+        for (int64_t tp = tp0; tp < tp1; ++tp) {
+            double g[2];
+            dg_normal_pair(dg_hash(seed, (uint64_t)c, (uint64_t)tp), &g[0], &g[1]);
+            for (int k = 0; k < 2; ++k) {
+                int64_t t = 2 * tp + k;
+                if (t < t_begin || t >= t_end) continue;
+                double q = floor(mean + sigma * g[k] + 0.5);
+                row[t - t_begin] = (uint16_t)(q < 0.0 ? 0.0 : (q > max_value ? max_value : q));
+            }
+        }
+        for (int32_t p = 0; p < npulses; ++p) {
+            int64_t a = pulses[p].t0 + pulse_delays[(size_t)p * nchans + c];
+            int64_t b = a + pulses[p].width;
+            if (a < t_begin) a = t_begin;
+            if (b > t_end) b = t_end;
+            for (int64_t t = a; t < b; ++t) {
+                double g[2];
+                dg_normal_pair(dg_hash(seed, (uint64_t)c, (uint64_t)(t >> 1)), &g[0], &g[1]);
+                double v = mean + sigma * g[t & 1];
+                for (int32_t q = 0; q < npulses; ++q) {
+                    int64_t qa = pulses[q].t0 + pulse_delays[(size_t)q * nchans + c];
+                    if (t >= qa && t < qa + pulses[q].width) v += pulses[q].amp;
+                }
+                double r = floor(v + 0.5);
+                row[t - t_begin] = (uint16_t)(r < 0.0 ? 0.0 : (r > max_value ? max_value : r));
+            }
+        }
+    }
+}
+
 /* 64-bit FNV-1a over a strided 2-D byte array; lets tests assert that host input is untouched. */
 uint64_t dg_checksum(const uint8_t* x, size_t row_stride, int32_t nchans, int64_t nsamp) {
     uint64_t h = 0xCBF29CE484222325ull;

@@ -40,6 +40,10 @@ def _load():
         lib.dg_fill.argtypes = [ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64,
                                 ctypes.c_uint64, ctypes.c_double, ctypes.c_double, ctypes.c_int32,
                                 ctypes.c_void_p, ctypes.c_void_p]
+        lib.dg_fill16.restype = None
+        lib.dg_fill16.argtypes = [ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64,
+                                  ctypes.c_uint64, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int32,
+                                  ctypes.c_void_p, ctypes.c_void_p]
         lib.dg_checksum.restype = ctypes.c_uint64
         lib.dg_checksum.argtypes = [ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int32, ctypes.c_int64]
         _lib = lib
@@ -47,8 +51,10 @@ def _load():
 
 
 def generate(seed: int, nchans: int, nsamp: int, pulses=(), pulse_delays=None, *, t_begin: int = 0,
-             mean: float = 127.0, sigma: float = 16.0, out: np.ndarray | None = None) -> np.ndarray:
-    """Return x[nchans][nsamp] uint8 for absolute samples [t_begin, t_begin+nsamp).
+             mean: float = 127.0, sigma: float = 16.0, out: np.ndarray | None = None, bits: int = 8,
+             max_value: int | None = None) -> np.ndarray:
+    """Return x[nchans][nsamp] for absolute samples [t_begin, t_begin+nsamp): uint8 (bits = 8), or uint16 clipped to
+    [0, max_value] (bits = 16; max_value = the stated bit depth, default 65535).
 
     ``pulses`` is a sequence of (t0, width, amp); ``pulse_delays`` an int64 array [npulses][nchans] of the
     per-channel arrival offsets in samples (computed by the caller, e.g. ``workloads.pulse_sweep``).
@@ -56,9 +62,11 @@ def generate(seed: int, nchans: int, nsamp: int, pulses=(), pulse_delays=None, *
     [nchans][>=nsamp]; its row stride is honoured.
     """
     lib = _load()
+    dt = np.uint16 if bits == 16 else np.uint8
+    assert bits in (8, 16)
     if out is None:
-        out = np.empty((nchans, nsamp), dtype=np.uint8)
-    assert out.dtype == np.uint8 and out.shape[0] == nchans and out.shape[1] >= nsamp and out.strides[1] == 1
+        out = np.empty((nchans, nsamp), dtype=dt)
+    assert out.dtype == dt and out.shape[0] == nchans and out.shape[1] >= nsamp and out.strides[1] == out.itemsize
     npulses = len(pulses)
     if npulses:
         parr = (_Pulse * npulses)(*[_Pulse(int(p[0]), int(p[1]), float(p[2])) for p in pulses])
@@ -67,10 +75,14 @@ def generate(seed: int, nchans: int, nsamp: int, pulses=(), pulse_delays=None, *
         pptr, dptr = ctypes.addressof(parr), pd.ctypes.data
     else:
         pptr, dptr = None, None
-    lib.dg_fill(out.ctypes.data, out.strides[0], nchans, t_begin, nsamp, seed, mean, sigma, npulses, pptr, dptr)
+    if bits == 16:
+        lib.dg_fill16(out.ctypes.data, out.strides[0], nchans, t_begin, nsamp, seed, mean, sigma,
+                      float(65535 if max_value is None else max_value), npulses, pptr, dptr)
+    else:
+        lib.dg_fill(out.ctypes.data, out.strides[0], nchans, t_begin, nsamp, seed, mean, sigma, npulses, pptr, dptr)
     return out
 
 
 def checksum(x: np.ndarray) -> int:
-    assert x.dtype == np.uint8 and x.ndim == 2 and x.strides[1] == 1
-    return int(_load().dg_checksum(x.ctypes.data, x.strides[0], x.shape[0], x.shape[1]))
+    assert x.dtype in (np.uint8, np.uint16) and x.ndim == 2 and x.strides[1] == x.itemsize
+    return int(_load().dg_checksum(x.ctypes.data, x.strides[0], x.shape[0], x.shape[1] * x.itemsize))

@@ -38,6 +38,17 @@ class Workload:
     budget_bytes: int = 0     # 0 = no budget stated (single chunk)
     noise_mean: float = 127.0
     noise_sigma: float = 16.0
+    input_bits: int = 8       # 8: uint8 samples; 16: uint16 samples clipped to [0, max_value]
+    max_value: int = 255      # the largest sample value the telescope delivers (the stated bit depth)
+
+    @property
+    def dtype(self):
+        return np.uint16 if self.input_bits == 16 else np.uint8
+
+    @property
+    def gen_kw(self) -> dict:
+        """Keyword arguments of datagen.generate that this workload fixes (noise level, sample type)."""
+        return dict(mean=self.noise_mean, sigma=self.noise_sigma, bits=self.input_bits, max_value=self.max_value)
 
     @property
     def freqs_mhz(self) -> np.ndarray:
@@ -95,6 +106,9 @@ WORKLOADS = {
     "lowf": Workload("lowf", 4096, 350.0, -150.0 / 4096, 64e-6, 1 << 21,
                      ((0.0, 0.05, 2000, 1), (100.0, 0.1, 1500, 2), (250.0, 0.1, 2500, 4)), _pow2(512), 7.0,
                      3500200, 100, (5.0, 500.0), 512),
+    # the SKA-like configuration delivered as 16-bit samples of 12-bit depth (noise N(1800, 16), pulses as in ska)
+    "ska16": Workload("ska16", 4096, 1500.0, -300.0 / 4096, 64e-6, 1 << 19, _SKA_RANGES, _pow2(256), 7.0,
+                      20191207, 50, (0.0, 2000.0), 256, noise_mean=1800.0, input_bits=16, max_value=4095),
     "stream": Workload("stream", 4096, 1500.0, -300.0 / 4096, 64e-6, 9_375_000, _SKA_RANGES, _pow2(256), 7.0,
                        600, 300, (0.0, 2000.0), 256, budget_bytes=40 * 10**9),
 }

@@ -45,6 +45,7 @@ def _load():
     L.orc_delay.argtypes = [f64, f64, i32]; L.orc_delay.restype = i64
     L.orc_delay_table.argtypes = [vp, i32, f64, f64, i32, i32, i32, vp]; L.orc_delay_table.restype = None
     L.orc_bin.argtypes = [vp, sz, i32, i64, i64, i32, vp]; L.orc_bin.restype = None
+    L.orc_bin16.argtypes = [vp, sz, i32, i64, i64, i32, vp]; L.orc_bin16.restype = None
     L.orc_dedisperse.argtypes = [vp, i64, i32, vp, f64, f64, i32, i32, i32, i64, vp]; L.orc_dedisperse.restype = None
     L.orc_row_stats.argtypes = [vp, i64, vp, vp, vp]; L.orc_row_stats.restype = i32
     for f in (L.orc_boxcar_snr, L.orc_boxcar_snr_prefix):
@@ -88,12 +89,18 @@ def delay_table(k: np.ndarray, rng, i0: int = 0, i1: int | None = None) -> np.nd
 
 
 def bin_time(x: np.ndarray, start: int, nbinned: int, b: int, out: np.ndarray | None = None) -> np.ndarray:
-    assert x.dtype == np.uint8 and x.ndim == 2 and x.strides[1] == 1
+    """x: uint8 or uint16 samples [nchans][nsamp] (16-bit input: b * max(x) must fit uint16, checked here)."""
+    assert x.dtype in (np.uint8, np.uint16) and x.ndim == 2 and x.strides[1] == x.itemsize
     assert start + nbinned * b <= x.shape[1]
     if out is None:
         out = np.empty((x.shape[0], nbinned), dtype=np.uint16)
     assert out.dtype == np.uint16 and out.shape == (x.shape[0], nbinned) and out.flags.c_contiguous
-    _load().orc_bin(_p(x), x.strides[0], x.shape[0], start, nbinned, b, _p(out))
+    if x.dtype == np.uint16:
+        if x.size:
+            assert int(x[:, start:start + nbinned * b].max()) * b <= 65535, "binned 16-bit samples must fit uint16"
+        _load().orc_bin16(_p(x), x.strides[0], x.shape[0], start, nbinned, b, _p(out))
+    else:
+        _load().orc_bin(_p(x), x.strides[0], x.shape[0], start, nbinned, b, _p(out))
     return out
 
 

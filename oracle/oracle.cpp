@@ -20,7 +20,8 @@
  *
  * Pin status (tests/test_oracle_pins.py, -m "not gpu"):
  *   delays            pinned: 60-digit decimal evaluation of the north_star formula + SURVEY §8(c) values
- *   binning           pinned: constant input, sum conservation
+ *   binning           pinned: constant input, sum conservation (8- and 16-bit input; the 16-bit entry also against numpy
+ *                             reshape-sums and, through dedispersion, the pure-Python brute force and DM 0 = channel sum)
  *   dedispersion      pinned: DM=0 = channel sum, pure-Python brute force, constant input, impulse response,
  *                             all-rows moment identity, injected-pulse recovery
  *   row statistics    pinned for the definition of (n, S1, S2) -> (mu, sigma) (exact rational checks, Gaussian
@@ -81,6 +82,22 @@ void orc_bin(const uint8_t* x, size_t row_stride, int32_t nchans, int64_t start,
              uint16_t* out) {
     for (int32_t c = 0; c < nchans; ++c) {
         const uint8_t* row = x + (size_t)c * row_stride + start;
+        uint16_t* o = out + (size_t)c * (size_t)nbinned;
+        for (int64_t t = 0; t < nbinned; ++t) {
+            uint32_t s = 0;
+            for (int32_t j = 0; j < b; ++j) s += row[(int64_t)b * t + j];
+            o[t] = (uint16_t)s;
+        }
+    }
+}
+
+/* The same sum for 16-bit input samples (PAPER.md:47 step 1 "telescope data, metadata": back-ends deliver 8- or
+ * 16-bit samples). row_stride in BYTES. The caller guarantees b * max(x) <= 65535 so that a sum fits the uint16 it is held in
+ * (reading C4w: the plan states the largest sample value; the Python wrapper checks the data). */
+void orc_bin16(const uint16_t* x, size_t row_stride_bytes, int32_t nchans, int64_t start, int64_t nbinned, int32_t b,
+               uint16_t* out) {
+    for (int32_t c = 0; c < nchans; ++c) {
+        const uint16_t* row = (const uint16_t*)((const uint8_t*)x + (size_t)c * row_stride_bytes) + start;
         uint16_t* o = out + (size_t)c * (size_t)nbinned;
         for (int64_t t = 0; t < nbinned; ++t) {
             uint32_t s = 0;

@@ -12,11 +12,11 @@ def make_input(w, pinned: bool = False):
     pl, dms, dl = w.pulses()
     if pinned:
         import torch
-        t = torch.empty((w.nchans, w.nsamp), dtype=torch.uint8, pin_memory=True)
+        t = torch.empty((w.nchans, w.nsamp), dtype=torch.uint16 if w.input_bits == 16 else torch.uint8, pin_memory=True)
         x = t.numpy()
-        datagen.generate(w.seed, w.nchans, w.nsamp, pl, dl, out=x)
+        datagen.generate(w.seed, w.nchans, w.nsamp, pl, dl, out=x, **w.gen_kw)
         return x, t
-    return datagen.generate(w.seed, w.nchans, w.nsamp, pl, dl), None
+    return datagen.generate(w.seed, w.nchans, w.nsamp, pl, dl, **w.gen_kw), None
 
 
 class OracleRun:

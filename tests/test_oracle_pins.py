@@ -584,3 +584,63 @@ def test_per_width_stats_end_to_end_recovers_the_injected_pulse(tiny):
     ta, tb = a[np.argmax(a["snr"])], b[np.argmax(b["snr"])]
     assert (int(tb["dm_index"]), int(tb["sample"]), int(tb["width"])) == (int(ta["dm_index"]), int(ta["sample"]), int(ta["width"]))
     assert abs(float(tb["snr"]) / float(ta["snr"]) - 1.0) < 0.05          # white noise: the two readings nearly agree
+
+
+# ------------------------------------------------------------------------------------------------ 16-bit input samples
+def test_bin16_constant_conservation_and_numpy_reshape_sum():
+    """orc_bin16 (uint16 input): constant input v gives b*v; the sum over t' equals the sum over t; and every binned value
+    equals numpy's reshape-sum of the same samples, for every b, on values that need all 12 bits and a strided view."""
+    rs = np.random.default_rng(16)
+    big = rs.integers(0, 4096, size=(7, 1000), dtype=np.uint16)
+    x = big[:, 3:963]                                                   # rows are not contiguous with each other
+    for b in (1, 2, 4, 8):
+        nb = 900 // b
+        got = oracle.bin_time(x, 40, nb, b)
+        exp = x[:, 40:40 + nb * b].astype(np.int64).reshape(7, nb, b).sum(axis=2)
+        assert got.dtype == np.uint16 and np.array_equal(got.astype(np.int64), exp)
+        assert int(got.astype(np.int64).sum()) == int(x[:, 40:40 + nb * b].astype(np.int64).sum())
+        const = np.full((3, 64), 4095, np.uint16)
+        assert np.all(oracle.bin_time(const, 0, 64 // b, b) == 4095 * b)
+    with pytest.raises(AssertionError):                                  # 8 * 9000 does not fit the uint16 a sum is held in
+        oracle.bin_time(np.full((2, 64), 9000, np.uint16), 0, 8, 8)
+
+
+def test_dedispersion_of_16bit_input_brute_force_and_dm0_channel_sum():
+    """The whole chain on a 16-bit array: D of every row equals a pure-Python triple loop written from the north_star
+    formula (bin 1 and bin 2), and the DM = 0 row is the channel sum."""
+    rs = np.random.default_rng(1616)
+    C, N = 6, 400
+    x = rs.integers(0, 4096, size=(C, N), dtype=np.uint16)
+    freqs = 1400.0 - 25.0 * np.arange(C)
+    tsamp = 1e-3
+    k = oracle.delay_constants(freqs, tsamp)
+    for b, rng in ((1, (0.0, 3.0, 9, 1)), (2, (5.0, 4.0, 6, 2))):
+        nb = N // b
+        xb = oracle.bin_time(x, 0, nb, b)
+        dmax = oracle.delay(k[-1], oracle.dm_value(rng[0], rng[1], rng[2] - 1), b)
+        T = nb - dmax
+        D = oracle.dedisperse(xb, k, rng, 0, rng[2], T)
+        for i in range(rng[2]):
+            dm = rng[0] + i * rng[1]
+            for t in range(0, T, 7):
+                acc = 0
+                for c in range(C):
+                    d = int(np.floor(4.148808e3 * dm * (freqs[c] ** -2 - freqs[0] ** -2) / tsamp / b + 0.5))
+                    for j in range(b):
+                        acc += int(x[c, b * (t + d) + j])
+                assert int(D[i, t]) == acc, (b, i, t)
+    xb = oracle.bin_time(x, 0, N, 1)
+    D0 = oracle.dedisperse(xb, k, (0.0, 1.0, 1, 1), 0, 1, N)
+    assert np.array_equal(D0[0], x.astype(np.int64).sum(axis=0))
+
+
+def test_generator_16bit_matches_its_recipe():
+    """datagen 16-bit mode: same Gaussian draws as the 8-bit recipe (same seed => (x16 - mean16) == (x8 - mean8) wherever
+    neither clips), clipped to the stated bit depth."""
+    a = datagen.generate(77, 5, 4096, mean=127.0, sigma=16.0)
+    b = datagen.generate(77, 5, 4096, mean=1800.0, sigma=16.0, bits=16, max_value=4095)
+    assert b.dtype == np.uint16 and int(b.max()) <= 4095
+    ok = (a > 0) & (a < 255)
+    assert np.array_equal(a[ok].astype(np.int64) - 127, b[ok].astype(np.int64) - 1800)
+    c = datagen.generate(77, 5, 4096, mean=4090.0, sigma=16.0, bits=16, max_value=4095)
+    assert int(c.max()) == 4095 and np.mean(c == 4095) > 0.3
