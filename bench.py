@@ -42,7 +42,7 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="ska", help="tiny | mid | ska | lowf | stream (BASELINE.json configs 0..4); "
+    ap.add_argument("--workload", default="ska", help="tiny | mid | ska | lowf | stream (BASELINE.json configs 0..4), ska16 (ska as 16-bit samples); "
                     "stream = the 600 s chunked pipeline under a 40 GB budget, a step is the whole stream")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -139,7 +139,7 @@ def run_reference(args, w):
     if rank != 0:
         return
     pl, dms, dl = w.pulses()
-    x = datagen.generate(w.seed, w.nchans, w.nsamp, pl, dl)
+    x = datagen.generate(w.seed, w.nchans, w.nsamp, pl, dl, **w.gen_kw)
     k = oracle.delay_constants(w.freqs_mhz, w.tsamp_s)
     g = oracle.chunk_geometry(k, w.ranges, w.nsamp)
     rows = 1 if w.nchans * w.nsamp > (1 << 28) else 3
@@ -179,23 +179,25 @@ def run_ours(args, w):
 
     # synthetic chunk of this rank (replicas over time chunks: a different seed per rank), pinned for the e2e leg
     pl, dms, dl = w.pulses()
-    xh = torch.empty((w.nchans, w.nsamp), dtype=torch.uint8, pin_memory=True)
+    esz = 2 if w.input_bits == 16 else 1
+    xh = torch.empty((w.nchans, w.nsamp), dtype=torch.uint16 if esz == 2 else torch.uint8, pin_memory=True)
     x = xh.numpy()
-    datagen.generate(w.seed + 1000003 * rank, w.nchans, w.nsamp, pl, dl, out=x)
+    datagen.generate(w.seed + 1000003 * rank, w.nchans, w.nsamp, pl, dl, out=x, **w.gen_kw)
     xd = xh.cuda(non_blocking=False)
 
     compute, copy = torch.cuda.Stream(), torch.cuda.Stream()
-    plan = aa.Plan(w.freqs_mhz, w.tsamp_s, w.ranges, w.widths, w.threshold)
+    plan = aa.Plan(w.freqs_mhz, w.tsamp_s, w.ranges, w.widths, w.threshold, input_bits=w.input_bits,
+                   input_max=w.max_value if esz == 2 else 0)
     st = aa.Strategy(plan, w.nsamp, compute_stream=compute, copy_stream=copy, max_candidates=1 << 22)
     h, info = st.handle, st.info
     assert info["nchunks"] == 1, "the benchmark workload must fit one chunk"
     outputs = outputs_of(w, info["n_out"])
     adds = outputs * w.nchans
-    in_bytes = w.nchans * info["chunk_len"]
+    in_bytes = w.nchans * info["chunk_len"] * esz
 
     def step_resident():
         aa.aa_strategy_reset(h)
-        aa.aa_run_dedispersion_device(h, xd, xd.stride(0))
+        aa.aa_run_dedispersion_device(h, xd, xd.stride(0) * esz)
         aa.aa_run_sps(h)
 
     def barrier():
@@ -240,7 +242,7 @@ def run_ours(args, w):
     if not args.no_e2e:
         def step_e2e():
             aa.aa_strategy_reset(h)
-            aa.aa_run_dedispersion(h, x, xh.stride(0))
+            aa.aa_run_dedispersion(h, x, xh.stride(0) * esz)
             aa.aa_run_sps(h)
             return aa.aa_get_candidates(h, allow_overflow=True)
         step_e2e()
@@ -285,6 +287,7 @@ def run_ours(args, w):
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "int32", "data": "synthetic",
             "config": {"workload": w.name, "nchans": w.nchans, "nsamp": w.nsamp, "tsamp_us": w.tsamp_s * 1e6, "ndms": w.ndms_total,
+                       "input_bits": w.input_bits, "input_max": w.max_value,
                        "ranges": [list(r) for r in w.ranges], "widths": list(w.widths), "threshold": w.threshold,
                        "outputs_per_step": outputs, "l2": "inputs larger than L2 (chunk %.2f GB in, %.2f GB out)" % (in_bytes / 1e9, 4 * outputs / 1e9),
                        "parallelism": "replicas over time chunks" if world > 1 else "single GPU"},

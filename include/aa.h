@@ -41,7 +41,8 @@ typedef enum {
     AA_ERR_CUDA = -4,
     AA_ERR_CANDIDATE_OVERFLOW = -5,  /* records beyond capacity were dropped, the count is still exact */
     AA_ERR_ORDER = -6,               /* "another module still needs to run" */
-    AA_ERR_INTERNAL = -7
+    AA_ERR_INTERNAL = -7,
+    AA_ERR_RANGE = -8                /* 16-bit plans only: the data made a boxcar sum leave int32 (see aa_plan_set_input_bits) */
 } aa_status;
 
 /* One DM range: DM_i = dm_low + i*dm_step for i in [0, ndms); the range is searched on data decimated in time by
@@ -88,6 +89,8 @@ typedef struct {
     size_t max_candidates;
     int32_t owns_arena;        /* 1 if the library made the (single) cudaMalloc */
     int32_t input_layout;      /* aa_input_layout of the bound plan */
+    int32_t input_bits;        /* 8 or 16 (aa_plan_set_input_bits) */
+    uint32_t input_max;        /* the plan's largest sample value */
 } aa_strategy_info;
 
 /* ------------------------------------------------------------------------------------------------ plan
@@ -112,6 +115,23 @@ void aa_plan_destroy(aa_plan* plan);
  * the staging buffers). Results are identical in both layouts. Errors: AA_ERR_INVALID_ARG naming `layout`. */
 typedef enum { AA_LAYOUT_CHANNEL_MAJOR = 0, AA_LAYOUT_TIME_MAJOR = 1 } aa_input_layout;
 aa_status aa_plan_set_input_layout(aa_plan* plan, int32_t layout);
+
+/* Sample type of the input (metadata of the telescope data, PAPER.md:47 step 1; the user directs the library at
+ * telescope data, which back-ends deliver as 8- or 16-bit samples). Default: bits = 8, uint8 samples.
+ * bits = 16: every sample is a uint16 in host byte order and at most max_value (the telescope's stated bit depth, e.g. 4095;
+ * 0 means 65535). host_input of aa_run_* then points at uint16 samples (row strides stay in BYTES), and a time-major
+ * device chunk needs rows that are 4-byte aligned. Results are exact for ANY input within max_value (binning, dedispersion
+ * and everything after are the same definitions; reading C4w).
+ * Limits checked here (AA_ERR_INVALID_ARG naming the field): max_value * max(bin) <= 65535 (a binned sample is held in 16
+ * bits) and nchans * max_value * max(bin) < 2^31 (int32 sums). The 8-bit plan's worst-case bound on boxcar sums cannot be
+ * given at plan time for 16-bit samples (256 * 4096 * 4095 * 8 is far beyond int32 although real boxcar sums of (D - D[0])
+ * are tiny), so it is checked on the DATA instead: if width_max * max|D - D[0]| of a row reaches 2^31, aa_run_sps /
+ * aa_get_candidates return AA_ERR_RANGE (sticky) rather than a wrong candidate.
+ * Speed: noise around a per-channel mean rides the 1-byte dedispersion path whatever the sample type (per-channel offset +
+ * exception list); a chunk whose channels spread over more than about +-128 (bin 1, 2, 4) or +-512 (bin 8)
+ * around their mean in too many samples falls back to a slow global-memory kernel - still exact.
+ * Must be called before aa_strategy_setup binds the plan. */
+aa_status aa_plan_set_input_bits(aa_plan* plan, int32_t bits, uint32_t max_value);
 
 /* Boxcar-complete chunks (reading C3x; off by default). With the plain chunking a boxcar of width w that starts in
  * the last w-1 samples of a chunk's output span is not evaluated (it would need samples of the next chunk), so a wide
@@ -195,7 +215,7 @@ aa_status aa_strategy_shard(aa_strategy* s, int32_t rank, int32_t world);
  * group is binned and added into D as soon as it has landed, so only the first group's copy is
  * exposed; the sums are int32, any grouping gives the same bits.
  * Returns AA_OK; AA_ERR_NOT_READY; AA_ERR_ORDER if the previous chunk's SPS has not run; AA_ERR_CUDA. */
-aa_status aa_run_dedispersion(aa_strategy* s, const uint8_t* host_input, size_t row_stride_bytes);
+aa_status aa_run_dedispersion(aa_strategy* s, const uint8_t* host_input /* uint16 samples for a 16-bit plan */, size_t row_stride_bytes);
 
 /* Same, with the chunk already resident on the DEVICE: device_chunk points at sample `start` of chunk `cursor`
  * (x[c][0..L_j), or x[0..L_j)[c] for a time-major plan: then 4-byte aligned with a stride that is a multiple of 4 and

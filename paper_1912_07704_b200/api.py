@@ -15,7 +15,8 @@ import numpy as np
 
 __all__ = [
     "AaError", "AA_OK", "AA_STATUS_CHUNK_DONE", "AA_STATUS_FINISHED", "AA_ERR_INVALID_ARG", "AA_ERR_NOT_READY",
-    "AA_ERR_BUDGET_TOO_SMALL", "AA_ERR_CUDA", "AA_ERR_CANDIDATE_OVERFLOW", "AA_ERR_ORDER", "AA_ERR_INTERNAL",
+    "AA_ERR_BUDGET_TOO_SMALL", "AA_ERR_CUDA", "AA_ERR_CANDIDATE_OVERFLOW", "AA_ERR_ORDER", "AA_ERR_INTERNAL", "AA_ERR_RANGE",
+    "aa_plan_set_input_bits",
     "CANDIDATE_DTYPE", "lib_path", "load",
     "AA_LAYOUT_CHANNEL_MAJOR", "AA_LAYOUT_TIME_MAJOR", "aa_plan_create", "aa_plan_destroy", "aa_plan_set_input_layout", "aa_plan_set_boxcar_overlap", "aa_plan_set_per_width_stats", "aa_get_row_width_stats", "aa_strategy_plan", "aa_strategy_setup", "aa_strategy_destroy", "aa_strategy_get_info",
     "aa_strategy_get_range_info", "aa_strategy_get_chunk", "aa_strategy_get_delay", "aa_strategy_describe",
@@ -27,7 +28,7 @@ __all__ = [
 
 AA_OK, AA_STATUS_CHUNK_DONE, AA_STATUS_FINISHED = 0, 1, 2
 AA_ERR_INVALID_ARG, AA_ERR_NOT_READY, AA_ERR_BUDGET_TOO_SMALL, AA_ERR_CUDA = -1, -2, -3, -4
-AA_ERR_CANDIDATE_OVERFLOW, AA_ERR_ORDER, AA_ERR_INTERNAL = -5, -6, -7
+AA_ERR_CANDIDATE_OVERFLOW, AA_ERR_ORDER, AA_ERR_INTERNAL, AA_ERR_RANGE = -5, -6, -7, -8
 AA_LAYOUT_CHANNEL_MAJOR, AA_LAYOUT_TIME_MAJOR = 0, 1
 
 CLUSTER_DTYPE = None  # defined below CANDIDATE_DTYPE
@@ -61,7 +62,8 @@ class _StrategyInfo(ctypes.Structure):
                 ("nsamp_total", c_int64), ("overlap", c_int64), ("chunk_len", c_int64), ("n_out", c_int64),
                 ("nchunks", c_int64), ("next_chunk", c_int64), ("shard_rank", c_int32), ("shard_world", c_int32),
                 ("arena_bytes_used", c_size_t),
-                ("arena_bytes_total", c_size_t), ("max_candidates", c_size_t), ("owns_arena", c_int32), ("input_layout", c_int32)]
+                ("arena_bytes_total", c_size_t), ("max_candidates", c_size_t), ("owns_arena", c_int32), ("input_layout", c_int32),
+                ("input_bits", c_int32), ("input_max", c_uint32)]
 
 
 def _struct_dict(s):
@@ -92,6 +94,7 @@ def load():
         "aa_plan_set_input_layout": (c_int32, [vp, c_int32]),
         "aa_plan_set_boxcar_overlap": (c_int32, [vp, c_int32]),
         "aa_plan_set_per_width_stats": (c_int32, [vp, c_int32]),
+        "aa_plan_set_input_bits": (c_int32, [vp, c_int32, c_uint32]),
         "aa_get_row_width_stats": (c_int32, [vp, c_int32, c_int32, c_int32, POINTER(c_double), POINTER(c_double), POINTER(c_int64)]),
         "aa_strategy_setup": (c_int32, [POINTER(vp), vp, c_uint64, vp, c_size_t, c_size_t, vp, vp, c_size_t, c_uint64]),
         "aa_strategy_plan": (c_int32, [POINTER(vp), vp, c_uint64, c_size_t, c_size_t, c_uint64]),
@@ -176,6 +179,10 @@ def aa_plan_set_input_layout(plan, layout: int) -> int:
 
 def aa_plan_set_boxcar_overlap(plan, on: bool) -> int:
     return _check(load().aa_plan_set_boxcar_overlap(plan, 1 if on else 0))
+
+
+def aa_plan_set_input_bits(plan, bits: int, max_value: int = 0) -> int:
+    return _check(load().aa_plan_set_input_bits(plan, int(bits), int(max_value)))
 
 
 def aa_plan_set_per_width_stats(plan, on: bool) -> int:
@@ -396,7 +403,7 @@ class Plan:
     """Owns an aa_plan handle."""
 
     def __init__(self, chan_freq_mhz, tsamp_s, ranges, boxcar_widths, snr_threshold, time_major: bool = False,
-                 boxcar_overlap: bool = False, per_width_stats: bool = False):
+                 boxcar_overlap: bool = False, per_width_stats: bool = False, input_bits: int = 8, input_max: int = 0):
         self.handle = aa_plan_create(chan_freq_mhz, tsamp_s, ranges, boxcar_widths, snr_threshold)
         self.ranges = [tuple(r) for r in ranges]
         if time_major:
@@ -405,6 +412,8 @@ class Plan:
             aa_plan_set_boxcar_overlap(self.handle, True)
         if per_width_stats:
             aa_plan_set_per_width_stats(self.handle, True)
+        if input_bits != 8:
+            aa_plan_set_input_bits(self.handle, input_bits, input_max)
 
     def close(self):
         if getattr(self, "handle", None):

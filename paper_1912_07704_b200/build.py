@@ -29,7 +29,7 @@ def _sources():
 
 
 def _newest_header() -> float:
-    hs = list(CSRC.glob("*.h")) + [HERE.parent / "include" / "aa.h"]
+    hs = list(CSRC.glob("*.h")) + list(CSRC.glob("*.cuh")) + [HERE.parent / "include" / "aa.h"]
     return max(h.stat().st_mtime for h in hs)
 
 

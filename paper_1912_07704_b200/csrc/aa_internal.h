@@ -39,6 +39,8 @@ struct Plan {
     int32_t layout = 0;           /* aa_input_layout */
     bool boxcar_overlap = false;  /* reading C3x */
     bool per_width = false;       /* reading C7m */
+    int32_t input_bits = 8;       /* 8: uint8 samples, 16: uint16 samples <= input_max */
+    uint32_t input_max = 255;
 };
 
 /* Single-allocation bump allocator over caller- or library-owned device memory. */
@@ -78,8 +80,11 @@ struct Range : K2Plan {           /* the base is the range's main plan: uint8 fo
     size_t first_row = 0;         /* index of this range's first row in the row tables */
     bool naive = false;           /* the tile window does not fit shared memory: one-thread-per-output kernel on a delay table */
     int32_t* d_delays = nullptr;  /* [ndms][nchans] (naive route only) */
-    bool has_lo = false;          /* bin 2 / 4: the offset-uint8 route (k_misc.cu "Offset-uint8 form") with its own tiling */
+    bool has_lo = false;          /* the offset-uint8 route (k_misc.cu "Offset-uint8 form") with its own tiling: bin 2 / 4 of an 8-bit
+                                     plan, bin 1 / 2 / 4 of a 16-bit plan */
     K2Plan lo;
+    bool main_exc = false;        /* 16-bit plan, bin 8: the main (uint16) plan reads the offset-uint16 form (offsets + exceptions) */
+    bool dense_naive = false;     /* 16-bit plan: exception-heavy chunks take the global-memory kernel on the plain binned samples */
 };
 
 struct Chunk { uint64_t start, len, n_out; };
@@ -98,7 +103,9 @@ struct Strategy {
     /* device memory */
     Arena arena;
     bool owns_arena = false;
-    size_t in_pitch = 0;                     /* bytes per channel row of the uint8 buffers */
+    int32_t esz_in = 1;                      /* bytes per input sample */
+    int32_t lo16_max = 1023;                 /* window of the offset-uint16 form */
+    size_t in_pitch = 0;                     /* bytes per channel row of the raw chunk */
     uint8_t* d_raw[2] = {nullptr, nullptr};  /* [0]: the H2D target of a channel-major plan / the corner-turn target; [1] is unused: K2 never
                                                 reads the raw chunk (K1 does), so the next chunk's copy may start as soon as K1 is done */
     uint8_t* d_stage[2] = {nullptr, nullptr};   /* time-major plans: H2D targets [L][stage_stride]; d_raw[0] is the corner-turn target */

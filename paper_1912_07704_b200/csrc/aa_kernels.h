@@ -51,6 +51,26 @@ typedef struct {
 } aak_prep_args;
 int aak_prep_fused(const aak_prep_args* a, int32_t nrows, void* stream);
 
+/* ---- K1 for 16-bit input samples (k_input16.cu): the offset forms x_b = lo + off_b[c] + r of a uint16 chunk.
+ * aak_chan_offsets16: off[k][c] = clamp(round(b mean_t x[c][t]) - centre[k], 0, ..) and *bias[k] += off[k][c], k = 0..3 <-> b = 1, 2, 4, 8
+ * (NULL entries are skipped; pointers already offset to the first row).
+ * aak_prep16: one read of raw rows writes the byte forms of bin 1, 2, 4 (lo[k], 4 copies, window [0, 255]) and the uint16 form
+ * of bin 8 (lo8, 2 copies, window [0, hi8]) with their exception lists; ngroups = 32-byte groups (16 samples) per row.
+ * aak_bin_time16: plain x_b as uint16, one copy (the input of the global-memory route); bin in {1, 2, 4, 8}; conditional like
+ * aak_bin_time. aak_corner_turn16: x[c][t] = x_tm[t][c] for uint16 samples. */
+int aak_chan_offsets16(const uint16_t* x, size_t pitch_bytes, int64_t len, int32_t nrows, int32_t* const off[4], int32_t* const bias[4],
+                       const int32_t centre[4], void* stream);
+typedef struct {
+    const uint16_t* raw; size_t pitch_bytes; int64_t ngroups; int32_t chan0; unsigned cap;
+    uint8_t* lo[3]; size_t pitch[3], stride[3]; const int32_t* off[3]; uint2* exc[3]; unsigned* cnt[3]; int64_t nb[3];
+    uint16_t* lo8; size_t pitch8, stride8; const int32_t* off8; uint2* exc8; unsigned* cnt8; int64_t nb8; int32_t hi8;
+} aak_prep16_args;
+int aak_prep16(const aak_prep16_args* a, int32_t nrows, void* stream);
+int aak_bin_time16(const uint16_t* x, size_t x_pitch_bytes, uint16_t* xb, size_t xb_pitch_bytes, int32_t nchans, int64_t nbinned,
+                   int32_t bin, const unsigned* only_if_cnt, unsigned only_if_above, void* stream);
+int aak_corner_turn16(const uint16_t* in, size_t in_stride_bytes, uint16_t* out, size_t out_pitch_bytes, int32_t nchans, int64_t nsamp,
+                      void* stream);
+
 /* ---- K2: dedispersion --------------------------------------------------------------------------------------------
  * Tiled kernel: a CTA owns `dm_tile` (30 or 32) DM trials x T_TILE(=1024) output samples; channels stream through shared
  * memory in blocks of `chan_block` via TMA (tensor map `tmap`, 128 opaque bytes, see aa_strategy.cpp), `ring_stages`-deep
@@ -95,7 +115,8 @@ int aak_dedisperse_init(void);   /* sets the dynamic shared-memory attribute of 
  * does not fit shared memory, and a cross-check. delays [ndms][nchans] int32; sums channels [chan_begin, chan_end),
  * accumulate as in aak_dedisperse. */
 int aak_dedisperse_naive(const void* x, size_t pitch_elems, int32_t in16, const int32_t* delays, int32_t nchans, int32_t chan_begin,
-                         int32_t chan_end, int32_t ndms, int64_t nt, int32_t* D, int64_t pitch, int32_t accumulate, void* stream);
+                         int32_t chan_end, int32_t ndms, int64_t nt, int32_t* D, int64_t pitch, int32_t accumulate,
+                         const unsigned* mode_cnt /* may be NULL; else runs only if *mode_cnt > mode_cap */, unsigned mode_cap, void* stream);
 
 /* ---- K0t: corner turn of a time-major chunk x_tm[t][c] into channel-major rows x[c][t] (uint8) */
 int aak_corner_turn(const uint8_t* in, size_t in_stride, uint8_t* out, size_t out_pitch, int32_t nchans, int64_t nsamp, void* stream);
@@ -136,6 +157,8 @@ typedef struct {
     int32_t widths[16]; int32_t nwidths;
     double threshold;
     aak_candidate* cands; unsigned long long* counter; unsigned long long capacity;
+    unsigned* range_flag;      /* may be NULL. Else bit 0 is set if wmax * max|D - D[0]| of a row reaches 2^31: the int32 boxcar sums are
+                                  then not trustworthy (plans whose sample maximum is too large for a plan-time guarantee) */
     /* reading C7m (per-width measured statistics), all NULL for reading C7: the outputs of aak_row_width_stats for this range */
     const double* wstats; const int64_t* wpivot; const int32_t* wlive;
 } aak_sps_args;

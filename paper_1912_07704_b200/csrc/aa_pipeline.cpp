@@ -37,11 +37,12 @@ aa_status enqueue_h2d(Strategy& s, int64_t j, int b, const uint8_t* host_input, 
     const Chunk& c = s.chunks[(size_t)j];
     if (s.raw_free_recorded[b]) AA_CUDA(cudaStreamWaitEvent(s.copy, s.ev_raw_free[b], 0), "cudaStreamWaitEvent");
     if (timed) AA_CUDA(cudaEventRecord(s.ev_h2d[0], s.copy), "cudaEventRecord");
+    const size_t esz = (size_t)s.esz_in;
     if (s.plan.layout == AA_LAYOUT_TIME_MAJOR)      /* one contiguous block of c.len time rows */
-        AA_CUDA(cudaMemcpy2DAsync(s.d_stage[b], s.stage_stride, host_input + (size_t)c.start * row_stride, row_stride, (size_t)s.plan.nchans,
+        AA_CUDA(cudaMemcpy2DAsync(s.d_stage[b], s.stage_stride, host_input + (size_t)c.start * row_stride, row_stride, (size_t)s.plan.nchans * esz,
                                   (size_t)c.len, cudaMemcpyHostToDevice, s.copy), "cudaMemcpy2DAsync (H2D chunk, time-major)");
     else
-        AA_CUDA(cudaMemcpy2DAsync(s.d_raw[b], s.in_pitch, host_input + c.start, row_stride, (size_t)c.len, (size_t)s.plan.nchans,
+        AA_CUDA(cudaMemcpy2DAsync(s.d_raw[b], s.in_pitch, host_input + c.start * esz, row_stride, (size_t)c.len * esz, (size_t)s.plan.nchans,
                                   cudaMemcpyHostToDevice, s.copy), "cudaMemcpy2DAsync (H2D chunk)");
     if (timed) AA_CUDA(cudaEventRecord(s.ev_h2d[1], s.copy), "cudaEventRecord");
     AA_CUDA(cudaEventRecord(s.ev_copied[b], s.copy), "cudaEventRecord");
@@ -62,7 +63,50 @@ static unsigned group_limit(const Strategy& s, int bin, int32_t c0, int32_t c1) 
 /* K1 for channel rows [c0, c1) (= channel group g) of the chunk in raw buffer b: sample-shifted uint8 copies, the
  * offset-uint8 form of the bin 2 / 4 inputs (per-channel offsets, byte copies, exception list), and the uint16 binned
  * inputs with their shifted copies (for bin 2 / 4 only when the group has too many exceptions). */
+/* K1 of a 16-bit plan (k_input16.cu): per-channel offsets, the offset forms of every bin with their exception lists, and the
+ * plain binned samples for the groups / bins that take the global-memory route. */
+aa_status enqueue_prep16(Strategy& s, const Chunk& c, int b, int32_t c0, int32_t c1, int g) {
+    const int32_t n = c1 - c0;
+    const uint16_t* raw = (const uint16_t*)(s.d_raw[b] + (size_t)c0 * s.in_pitch);
+    int32_t* off[4]; int32_t* bias[4]; int32_t centre[4];
+    bool any = false;
+    for (int k = 0; k < 4; ++k) {
+        const int bin = 1 << k;
+        const bool sparse = s.d_exc_cnt[bin] != nullptr;
+        off[k] = sparse ? s.d_off[bin] + c0 : nullptr;
+        bias[k] = sparse ? (int32_t*)(s.d_exc_cnt[bin] + kMaxGroups + g) : nullptr;
+        centre[k] = bin == 8 ? (s.lo16_max + 1) / 2 : 128;
+        any = any || sparse;
+    }
+    if (any) {
+        AA_LAUNCH(aak_chan_offsets16(raw, s.in_pitch, (int64_t)c.len, n, off, bias, centre, s.compute), "channel offsets (16-bit)");
+        aak_prep16_args a;
+        memset(&a, 0, sizeof a);
+        a.raw = raw; a.pitch_bytes = s.in_pitch; a.ngroups = (int64_t)(s.in_pitch / 32); a.chan0 = c0; a.cap = kExcCap;
+        for (int k = 0; k < 3; ++k) {
+            const int bin = 1 << k;
+            if (!s.d_lo[bin] || !s.d_exc_cnt[bin]) continue;
+            a.lo[k] = s.d_lo[bin] + (size_t)c0 * s.lo_pitch[bin]; a.pitch[k] = s.lo_pitch[bin]; a.stride[k] = s.lo_stride[bin]; a.off[k] = s.d_off[bin] + c0;
+            a.exc[k] = s.d_exc[bin] + (size_t)g * kExcCap; a.cnt[k] = s.d_exc_cnt[bin] + g; a.nb[k] = (int64_t)(c.len / (uint64_t)bin);
+        }
+        if (s.d_xb[8] && s.d_exc_cnt[8]) {
+            a.lo8 = s.d_xb[8] + (size_t)c0 * s.xb_pitch[8]; a.pitch8 = s.xb_pitch[8] * 2; a.stride8 = s.xb_stride[8]; a.off8 = s.d_off[8] + c0;
+            a.exc8 = s.d_exc[8] + (size_t)g * kExcCap; a.cnt8 = s.d_exc_cnt[8] + g; a.nb8 = (int64_t)(c.len / 8); a.hi8 = s.lo16_max;
+        }
+        AA_LAUNCH(aak_prep16(&a, n, s.compute), "input forms (16-bit)");
+    }
+    for (int bin = 1; bin <= 8; bin *= 2) {
+        if (!s.d_xb[bin]) continue;
+        const unsigned* cnt = s.d_exc_cnt[bin] ? s.d_exc_cnt[bin] + g : nullptr;     /* NULL: the bin has only the global-memory route */
+        const unsigned lim = cnt ? group_limit(s, bin, c0, c1) : 0u;
+        AA_LAUNCH(aak_bin_time16(raw, s.in_pitch, s.d_xb[bin] + (size_t)c0 * s.xb_pitch[bin], s.xb_pitch[bin] * 2, n, (int64_t)(c.len / (uint64_t)bin), bin, cnt,
+                                 lim, s.compute), "time binning (16-bit)");
+    }
+    return AA_OK;
+}
+
 aa_status enqueue_prep(Strategy& s, const Chunk& c, int b, int32_t c0, int32_t c1, int g) {
+    if (s.plan.input_bits == 16) return enqueue_prep16(s, c, b, c0, c1, g);
     const int32_t n = c1 - c0;
     const uint8_t* raw = s.d_raw[b] + (size_t)c0 * s.in_pitch;
     if (s.d_lo[2] || s.d_lo[4])
@@ -114,26 +158,39 @@ aa_status enqueue_k2(Strategy& s, const Chunk& c, int32_t c0, int32_t c1, bool a
         a.nt = (int64_t)(c.n_out / (uint64_t)bin) + rg.extra;      /* reading C3x: E samples beyond the output span */
         a.ndms = rg.r.ndms; a.nchans = s.plan.nchans;
         a.chan_begin = c0; a.chan_end = c1; a.accumulate = accumulate ? 1 : 0;
+        const bool plain_u8 = bin == 1 && s.plan.input_bits == 8;
+        const void* x0 = plain_u8 ? (const void*)s.d_x4 : (const void*)s.d_xb[bin];            /* copy 0 of the range's plain input form */
+        const size_t pitch_elems = plain_u8 ? s.x4_pitch : s.xb_pitch[bin];
         if (rg.naive) {
-            const void* x0 = bin == 1 ? (const void*)s.d_x4 : (const void*)s.d_xb[bin];        /* copy 0 of the range's input form */
-            const size_t pitch_elems = bin == 1 ? s.x4_pitch : s.xb_pitch[bin];
-            AA_LAUNCH(aak_dedisperse_naive(x0, pitch_elems, bin > 1, rg.d_delays, s.plan.nchans, c0, c1, rg.r.ndms, a.nt, rg.d_D, rg.pitch,
-                                           accumulate ? 1 : 0, st), "dedispersion (global-memory route)");
+            AA_LAUNCH(aak_dedisperse_naive(x0, pitch_elems, !plain_u8, rg.d_delays, s.plan.nchans, c0, c1, rg.r.ndms, a.nt, rg.d_D, rg.pitch,
+                                           accumulate ? 1 : 0, nullptr, 0u, st), "dedispersion (global-memory route)");
             continue;
         }
-        for (int route = rg.has_lo ? 0 : 1; route < 2; ++route) {
+        /* routes: [offset-uint8 plan] [main plan: plain input, or the offset-uint16 form] [global-memory kernel]. Where a range
+         * has a sparse route (offsets + exceptions) and a dense one, both are launched; each tests the group's exception
+         * counter and only one of them runs. */
+        const bool sparse = rg.has_lo || rg.main_exc;
+        const bool has_main = rg.ndm_tiles > 0;
+        const unsigned* cnt = sparse ? s.d_exc_cnt[bin] + g : nullptr;
+        const unsigned lim = sparse ? group_limit(s, bin, c0, c1) : 0u;
+        for (int route = 0; route < 2; ++route) {
+            if (route == 0 && !rg.has_lo) continue;
+            if (route == 1 && !has_main) continue;
             const K2Plan& p = route == 0 ? rg.lo : static_cast<const K2Plan&>(rg);
+            const bool route_sparse = route == 0 || rg.main_exc;
             a.tmap = &p.map; a.etab = p.d_etab; a.x0tab = p.d_x0tab;
             a.chan_block = p.chan_block; a.window_bytes = p.window_bytes; a.spill_stages = p.spill_stages; a.in16 = p.in16;
             a.variant = p.variant; a.dms_per_warp = p.dms_per_warp; a.ring_stages = p.ring_stages; a.dm_tile = p.dm_tile; a.skew_q16 = p.skew_q16;
-            a.mode_cnt = rg.has_lo ? s.d_exc_cnt[bin] + g : nullptr;
-            a.mode_cap = rg.has_lo ? group_limit(s, bin, c0, c1) : 0u; a.mode_dense = route;
-            a.bias = route == 0 ? (const int32_t*)(s.d_exc_cnt[bin] + kMaxGroups + g) : nullptr;
+            a.mode_cnt = cnt; a.mode_cap = lim; a.mode_dense = route_sparse ? 0 : 1;
+            a.bias = route_sparse ? (const int32_t*)(s.d_exc_cnt[bin] + kMaxGroups + g) : nullptr;
             AA_LAUNCH(aak_dedisperse(&a, st), "dedispersion");
         }
-        if (rg.has_lo)
-            AA_LAUNCH(aak_scatter_exceptions(s.d_exc[bin] + (size_t)g * kExcCap, s.d_exc_cnt[bin] + g, group_limit(s, bin, c0, c1), s.d_k, rg.r.dm_low, rg.r.dm_step,
+        if (sparse)
+            AA_LAUNCH(aak_scatter_exceptions(s.d_exc[bin] + (size_t)g * kExcCap, s.d_exc_cnt[bin] + g, lim, s.d_k, rg.r.dm_low, rg.r.dm_step,
                                              rg.r.ndms, bin, a.nt, rg.d_D, rg.pitch, st), "exception scatter");
+        if (rg.dense_naive)
+            AA_LAUNCH(aak_dedisperse_naive(x0, pitch_elems, 1, rg.d_delays, s.plan.nchans, c0, c1, rg.r.ndms, a.nt, rg.d_D, rg.pitch,
+                                           accumulate ? 1 : 0, cnt, lim, st), "dedispersion (global-memory route of an exception-heavy chunk)");
     }
     if (two) {
         AA_CUDA(cudaEventRecord(s.ev_join, s.aux), "cudaEventRecord");
@@ -149,8 +206,8 @@ aa_status enqueue_h2d_groups(Strategy& s, int64_t j, int b, const uint8_t* host_
     AA_CUDA(cudaEventRecord(s.ev_h2d[0], s.copy), "cudaEventRecord");
     for (int g = 0; g < groups.n; ++g) {
         const int32_t c0 = groups.c[g], c1 = groups.c[g + 1];
-        AA_CUDA(cudaMemcpy2DAsync(s.d_raw[b] + (size_t)c0 * s.in_pitch, s.in_pitch, host_input + (size_t)c0 * row_stride + c.start, row_stride,
-                                  (size_t)c.len, (size_t)(c1 - c0), cudaMemcpyHostToDevice, s.copy), "cudaMemcpy2DAsync (H2D channel group)");
+        AA_CUDA(cudaMemcpy2DAsync(s.d_raw[b] + (size_t)c0 * s.in_pitch, s.in_pitch, host_input + (size_t)c0 * row_stride + c.start * (size_t)s.esz_in, row_stride,
+                                  (size_t)c.len * (size_t)s.esz_in, (size_t)(c1 - c0), cudaMemcpyHostToDevice, s.copy), "cudaMemcpy2DAsync (H2D channel group)");
         AA_CUDA(cudaEventRecord(s.ev_group[g], s.copy), "cudaEventRecord");
     }
     AA_CUDA(cudaEventRecord(s.ev_h2d[1], s.copy), "cudaEventRecord");
@@ -169,10 +226,13 @@ aa_status enqueue_dedispersion(Strategy& s, int64_t j, int b, const uint8_t* tm_
     AA_CUDA(cudaEventRecord(s.ev_t[0], s.compute), "cudaEventRecord");
     if (s.plan.layout == AA_LAYOUT_TIME_MAJOR) {
         if (!tm_src) { tm_src = s.d_stage[b]; tm_stride = s.stage_stride; }
-        AA_LAUNCH(aak_corner_turn(tm_src, tm_stride, s.d_raw[0], s.in_pitch, C, (int64_t)c.len, s.compute), "corner turn");
+        if (s.plan.input_bits == 16)
+            AA_LAUNCH(aak_corner_turn16((const uint16_t*)tm_src, tm_stride, (uint16_t*)s.d_raw[0], s.in_pitch, C, (int64_t)c.len, s.compute), "corner turn (16-bit)");
+        else
+            AA_LAUNCH(aak_corner_turn(tm_src, tm_stride, s.d_raw[0], s.in_pitch, C, (int64_t)c.len, s.compute), "corner turn");
         b = 0;                                        /* the channel-major copy lives in d_raw[0] */
     }
-    for (int bn = 2; bn <= 4; bn *= 2)             /* exception counters and biases of this chunk's channel groups */
+    for (int bn = 1; bn <= 8; bn *= 2)             /* exception counters and biases of this chunk's channel groups */
         if (s.d_exc_cnt[bn]) AA_CUDA(cudaMemsetAsync(s.d_exc_cnt[bn], 0, 2 * kMaxGroups * 4, s.compute), "cudaMemsetAsync");
     if (groups) {
         /* the chunk is still arriving: channel group g is prepared and added to D as soon as its rows have landed, so only
@@ -211,7 +271,14 @@ bool cand_less(const aa_candidate& a, const aa_candidate& b) {
 aa_status harvest(Strategy& s) {
     if (!s.harvest_pending) return AA_OK;
     AA_CUDA(cudaEventSynchronize(s.ev_count), "cudaEventSynchronize");
-    const unsigned long long found = *s.h_counter;
+    const unsigned long long found = s.h_counter[0];
+    if (s.h_counter[1] & 1ull) {
+        s.harvest_pending = false;
+        set_error("aa_run_sps: in chunk %lld the widest boxcar times the largest |D - D[0]| of a row reaches 2^31: the int32 boxcar sums cannot be "
+                  "trusted for this data (16-bit plan; narrow the widths or the sample maximum)", (long long)s.harvest_chunk);
+        s.sticky = AA_ERR_RANGE;
+        return s.sticky;
+    }
     s.true_count += found;
     unsigned long long take = std::min<unsigned long long>(found, s.max_candidates);
     const size_t room = s.max_candidates - std::min(s.max_candidates, s.cands.size());
@@ -239,8 +306,10 @@ extern "C" aa_status aa_run_dedispersion(aa_strategy* h, const uint8_t* host_inp
     Strategy& s = h->s;
     if (!host_input) { set_error("aa_run_dedispersion: host_input is NULL"); return AA_ERR_INVALID_ARG; }
     const bool tmajor = s.plan.layout == AA_LAYOUT_TIME_MAJOR;
-    if (!tmajor && row_stride_bytes < s.nsamp_total) { set_error("aa_run_dedispersion: row_stride_bytes = %zu is shorter than nsamp_total = %llu", row_stride_bytes, (unsigned long long)s.nsamp_total); return AA_ERR_INVALID_ARG; }
-    if (tmajor && row_stride_bytes < (size_t)s.plan.nchans) { set_error("aa_run_dedispersion: row_stride_bytes = %zu is shorter than nchans = %d (time-major plan)", row_stride_bytes, s.plan.nchans); return AA_ERR_INVALID_ARG; }
+    const size_t esz = (size_t)s.esz_in;
+    if (!tmajor && row_stride_bytes < s.nsamp_total * esz) { set_error("aa_run_dedispersion: row_stride_bytes = %zu is shorter than nsamp_total = %llu samples of %zu byte(s)", row_stride_bytes, (unsigned long long)s.nsamp_total, esz); return AA_ERR_INVALID_ARG; }
+    if (tmajor && row_stride_bytes < (size_t)s.plan.nchans * esz) { set_error("aa_run_dedispersion: row_stride_bytes = %zu is shorter than nchans = %d samples of %zu byte(s) (time-major plan)", row_stride_bytes, s.plan.nchans, esz); return AA_ERR_INVALID_ARG; }
+    if (esz == 2 && (((uintptr_t)host_input | row_stride_bytes) & 1)) { set_error("aa_run_dedispersion: a 16-bit plan needs host_input and row_stride_bytes = %zu aligned to 2 bytes", row_stride_bytes); return AA_ERR_INVALID_ARG; }
     const bool two_buffers = s.d_stage[1] != nullptr;      /* time-major staging; a channel-major plan has ONE H2D buffer */
     const bool prefetch = s.chunks.size() > 1;
     if (s.pending_sps) { set_error("aa_run_dedispersion: chunk %lld is dedispersed but aa_run_sps has not run on it yet", (long long)s.current_chunk); return AA_ERR_ORDER; }
@@ -288,18 +357,18 @@ extern "C" aa_status aa_run_dedispersion_device(aa_strategy* h, const uint8_t* d
     const Chunk& c = s.chunks[(size_t)j];
     s.h2d_timed = false;
     if (s.plan.layout == AA_LAYOUT_TIME_MAJOR) {
-        if (((uintptr_t)device_chunk & 3) || (row_stride_bytes & 3) || row_stride_bytes < (size_t)((s.plan.nchans + 3) & ~3)) {
+        if (((uintptr_t)device_chunk & 3) || (row_stride_bytes & 3) || row_stride_bytes < (size_t)((s.plan.nchans * s.esz_in + 3) & ~3)) {
             set_error("aa_run_dedispersion_device: a time-major device chunk must be 4-byte aligned with row_stride_bytes a multiple of 4 and >= nchans rounded up to 4 (got %zu)", row_stride_bytes);
             return AA_ERR_INVALID_ARG;
         }
         /* the corner turn writes d_raw[0]; nothing else is in flight into it (host prefetches of a time-major plan go to d_stage) */
         return enqueue_dedispersion(s, j, 0, device_chunk, row_stride_bytes);
     }
-    if (row_stride_bytes < c.len) { set_error("aa_run_dedispersion_device: row_stride_bytes = %zu is shorter than the chunk (%llu)", row_stride_bytes, (unsigned long long)c.len); return AA_ERR_INVALID_ARG; }
+    if (row_stride_bytes < c.len * (size_t)s.esz_in) { set_error("aa_run_dedispersion_device: row_stride_bytes = %zu is shorter than the chunk (%llu samples)", row_stride_bytes, (unsigned long long)c.len); return AA_ERR_INVALID_ARG; }
     const int b = 0;
     /* a host prefetch of an earlier aa_run_dedispersion(host) may still be writing this buffer on the copy stream */
     if (s.raw_holds[b] >= 0) AA_CUDA(cudaStreamWaitEvent(s.compute, s.ev_copied[b], 0), "cudaStreamWaitEvent");
-    AA_CUDA(cudaMemcpy2DAsync(s.d_raw[b], s.in_pitch, device_chunk, row_stride_bytes, (size_t)c.len, (size_t)s.plan.nchans,
+    AA_CUDA(cudaMemcpy2DAsync(s.d_raw[b], s.in_pitch, device_chunk, row_stride_bytes, (size_t)c.len * (size_t)s.esz_in, (size_t)s.plan.nchans,
                               cudaMemcpyDeviceToDevice, s.compute), "cudaMemcpy2DAsync (D2D chunk)");
     s.raw_holds[b] = j;
     return enqueue_dedispersion(s, j, b);
@@ -314,7 +383,7 @@ extern "C" aa_status aa_run_sps(aa_strategy* h) {
     const int64_t j = s.current_chunk;
     const Chunk& c = s.chunks[(size_t)j];
     const bool is_short = c.len != (uint64_t)s.L;
-    AA_CUDA(cudaMemsetAsync(s.d_counter, 0, sizeof(unsigned long long), s.compute), "cudaMemsetAsync");
+    AA_CUDA(cudaMemsetAsync(s.d_counter, 0, 2 * sizeof(unsigned long long), s.compute), "cudaMemsetAsync");   /* [0] candidates, [1] range flag */
     AA_CUDA(cudaEventRecord(s.ev_t[3], s.compute), "cudaEventRecord");
     AA_LAUNCH(aak_row_stats(s.d_rows[is_short ? 1 : 0], (int32_t)s.nrows, s.d_mu_sigma, s.d_n_iters, s.compute), "row statistics");
     const size_t nwd = s.plan.widths.size();
@@ -338,13 +407,14 @@ extern "C" aa_status aa_run_sps(aa_strategy* h) {
         for (int k = 0; k < 16; ++k) a.widths[k] = k < a.nwidths ? s.plan.widths[(size_t)k] : 0;
         a.threshold = (double)s.plan.threshold;
         a.cands = s.d_cands; a.counter = s.d_counter; a.capacity = s.max_candidates;
+        a.range_flag = s.plan.input_bits == 16 ? (unsigned*)(s.d_counter + 1) : nullptr;      /* no plan-time bound on boxcar sums */
         a.wstats = s.plan.per_width ? s.d_wstats + 2 * nwd * rg.first_row : nullptr;
         a.wpivot = s.plan.per_width ? s.d_wpivot + nwd * rg.first_row : nullptr;
         a.wlive = s.plan.per_width ? s.d_wlive + rg.first_row : nullptr;
         AA_LAUNCH(aak_sps_peaks(&a, s.compute), "sps peaks");
     }
     AA_CUDA(cudaEventRecord(s.ev_t[5], s.compute), "cudaEventRecord");
-    AA_CUDA(cudaMemcpyAsync(s.h_counter, s.d_counter, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s.compute), "counter D2H");
+    AA_CUDA(cudaMemcpyAsync(s.h_counter, s.d_counter, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s.compute), "counter D2H");
     AA_CUDA(cudaEventRecord(s.ev_count, s.compute), "cudaEventRecord");
     s.harvest_pending = true; s.harvest_chunk = j; s.stats_timed = true;
     s.pending_sps = false;

@@ -98,6 +98,28 @@ extern "C" aa_status aa_plan_set_boxcar_overlap(aa_plan* plan, int32_t on) {
     return AA_OK;
 }
 
+extern "C" aa_status aa_plan_set_input_bits(aa_plan* plan, int32_t bits, uint32_t max_value) {
+    using aa::set_error;
+    if (!plan) { set_error("aa_plan_set_input_bits: plan is NULL"); return AA_ERR_NOT_READY; }
+    if (bits != 8 && bits != 16) { set_error("aa_plan_set_input_bits: bits = %d must be 8 or 16", bits); return AA_ERR_INVALID_ARG; }
+    if (bits == 8) { plan->p.input_bits = 8; plan->p.input_max = 255; return AA_OK; }
+    if (max_value == 0) max_value = 65535;
+    if (max_value > 65535) { set_error("aa_plan_set_input_bits: max_value = %u does not fit 16 bits", max_value); return AA_ERR_INVALID_ARG; }
+    int64_t max_bin = 1;
+    for (const aa_dm_range& g : plan->p.ranges) max_bin = g.bin > max_bin ? g.bin : max_bin;
+    if ((int64_t)max_value * max_bin > 65535) {
+        set_error("aa_plan_set_input_bits: max_value * max bin = %lld exceeds 65535 (a binned sample is held in 16 bits)", (long long)max_value * max_bin);
+        return AA_ERR_INVALID_ARG;
+    }
+    if ((int64_t)plan->p.nchans * max_value * max_bin >= (int64_t)1 << 31) {
+        set_error("aa_plan_set_input_bits: nchans * max_value * max bin = %lld does not fit the int32 dedispersed sums",
+                  (long long)plan->p.nchans * max_value * max_bin);
+        return AA_ERR_INVALID_ARG;
+    }
+    plan->p.input_bits = 16; plan->p.input_max = max_value;
+    return AA_OK;
+}
+
 extern "C" aa_status aa_plan_set_per_width_stats(aa_plan* plan, int32_t on) {
     if (!plan) { aa::set_error("aa_plan_set_per_width_stats: plan is NULL"); return AA_ERR_NOT_READY; }
     plan->p.per_width = on != 0;

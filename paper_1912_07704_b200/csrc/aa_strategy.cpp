@@ -62,7 +62,8 @@ static bool make_window_map(CUtensorMap* map, void* base, size_t row_bytes, size
 static void carve(Strategy& s, int64_t L, bool two_stage) {
     Arena& a = s.arena;
     a.used = 0;
-    s.in_pitch = round_up((size_t)L, 256);
+    const size_t esz = (size_t)s.esz_in;
+    s.in_pitch = round_up((size_t)L * esz, 256);
     const size_t raw_bytes = (size_t)s.plan.nchans * s.in_pitch + kSlack;
     /* ONE raw buffer also when chunks are double-buffered: only K1 reads it (3 ms of a 200 ms step), so the copy of the next
      * chunk starts when K1 of this one is done and still overlaps the whole of K2 */
@@ -71,37 +72,42 @@ static void carve(Strategy& s, int64_t L, bool two_stage) {
     s.d_stage[0] = s.d_stage[1] = nullptr;
     if (s.plan.layout == AA_LAYOUT_TIME_MAJOR) {
         /* the chunk lands time-major in a staging buffer (two when chunks are double-buffered); one channel-major buffer */
-        s.stage_stride = round_up((size_t)s.plan.nchans, 16);
+        s.stage_stride = round_up((size_t)s.plan.nchans * esz, 16);
         const size_t stage_bytes = (size_t)L * s.stage_stride + kSlack;
         s.d_stage[0] = (uint8_t*)a.take(stage_bytes);
         s.d_stage[1] = two_stage ? (uint8_t*)a.take(stage_bytes) : nullptr;
     }
     /* input forms: nchans rows of 4P bytes per binning factor (aa_internal.h), kSlack readable bytes after the last row */
-    s.x4_stride = s.in_pitch;
-    s.x4_pitch = 4 * s.in_pitch;
-    s.d_x4 = s.need_u8_copies ? (uint8_t*)a.take((size_t)s.plan.nchans * s.x4_pitch + kSlack) : nullptr;
-    for (int b = 2; b <= 8; b *= 2) {
-        bool used = false, lo = false;
+    s.d_x4 = nullptr; s.x4_stride = s.x4_pitch = 0;
+    for (int b = 1; b <= 8; b *= 2) {
+        bool used = false, lo = false, sparse = false;
         int64_t nd = 0;
         for (const Range& rg : s.ranges) {
-            used = used || rg.r.bin == b;
-            if (rg.r.bin == b && rg.has_lo) { lo = true; nd += rg.r.ndms; }
+            if (rg.r.bin != b) continue;
+            used = true;
+            lo = lo || rg.has_lo;
+            if (rg.has_lo || rg.main_exc) { sparse = true; nd += rg.r.ndms; }
         }
         const size_t P = used ? round_up((size_t)(L / b), 256) : 0;
         uint8_t* base = used ? (uint8_t*)a.take((size_t)s.plan.nchans * 4 * P + kSlack) : nullptr;
+        if (b == 1 && s.plan.input_bits == 8) {       /* plain bytes: the 4 sample-shifted copies of the chunk itself */
+            s.d_x4 = base; s.x4_pitch = 4 * P; s.x4_stride = P;
+            s.d_xb[b] = nullptr; s.d_lo[b] = nullptr;
+            continue;
+        }
         s.d_xb[b] = (uint16_t*)base;
         s.xb_pitch[b] = 2 * P;                     /* elements: a row is 2 copies of 2P bytes */
         s.xb_stride[b] = 2 * P;                    /* bytes */
         s.d_lo[b] = lo ? base : nullptr;           /* the same rows as 4 copies of P bytes */
         s.lo_pitch[b] = lo ? 4 * P : 0;
         s.lo_stride[b] = lo ? P : 0;
-        s.d_off[b] = lo ? (int32_t*)a.take((size_t)s.plan.nchans * 4) : nullptr;
-        s.d_exc[b] = lo ? (uint2*)a.take((size_t)kMaxGroups * kExcCap * sizeof(uint2)) : nullptr;
-        s.d_exc_cnt[b] = lo ? (unsigned*)a.take(2 * kMaxGroups * 4) : nullptr;
+        s.d_off[b] = sparse ? (int32_t*)a.take((size_t)s.plan.nchans * 4) : nullptr;
+        s.d_exc[b] = sparse ? (uint2*)a.take((size_t)kMaxGroups * kExcCap * sizeof(uint2)) : nullptr;
+        s.d_exc_cnt[b] = sparse ? (unsigned*)a.take(2 * kMaxGroups * 4) : nullptr;
         /* the scatter costs one atomic per (exception, trial), measured 2.7e10 atomics/s: beyond ~1e8 of them per chunk the
-         * uint16 route is cheaper (a channel group gets the share of its channels) */
-        s.exc_limit[b] = lo ? (unsigned)std::min<int64_t>((int64_t)kMaxGroups * kExcCap, std::max<int64_t>(1, 100000000 / std::max<int64_t>(1, nd))) : 0;
-        if (lo && !s.d_k_needed) s.d_k_needed = true;
+         * dense route is cheaper (a channel group gets the share of its channels) */
+        s.exc_limit[b] = sparse ? (unsigned)std::min<int64_t>((int64_t)kMaxGroups * kExcCap, std::max<int64_t>(1, 100000000 / std::max<int64_t>(1, nd))) : 0;
+        if (sparse && !s.d_k_needed) s.d_k_needed = true;
     }
     s.d_k = s.d_k_needed ? (double*)a.take((size_t)s.plan.nchans * 8) : nullptr;
     const int64_t n_out = L - s.S;
@@ -109,7 +115,7 @@ static void carve(Strategy& s, int64_t L, bool two_stage) {
         rg.nt_full = n_out / rg.r.bin;
         rg.pitch = (int64_t)round_up((size_t)(rg.nt_full + rg.extra), 128);
         rg.d_D = (int32_t*)a.take((size_t)rg.r.ndms * (size_t)rg.pitch * 4);
-        rg.d_delays = rg.naive ? (int32_t*)a.take((size_t)rg.r.ndms * s.plan.nchans * 4) : nullptr;
+        rg.d_delays = (rg.naive || rg.dense_naive) ? (int32_t*)a.take((size_t)rg.r.ndms * s.plan.nchans * 4) : nullptr;
         rg.d_etab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * kDmTile * 4);   /* rg. = the main plan */
         rg.d_x0tab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * 4);
         if (rg.has_lo) {
@@ -149,7 +155,8 @@ static std::vector<Chunk> make_chunks(uint64_t nsamp, int64_t B, int64_t S, int6
 }
 
 /* Tiling and offset tables of K2 for one range in one input format (in16: uint16 binned samples, else bytes). */
-static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16, std::vector<int32_t>& etab, std::vector<int32_t>& x0tab) {
+static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16, int carry_channels, std::vector<int32_t>& etab,
+                        std::vector<int32_t>& x0tab) {
     const int32_t C = s.plan.nchans, nd = rg.r.ndms;
     p.in16 = in16; p.esz = in16 ? 2 : 1; p.spw = 4 / p.esz; p.ncopy = p.spw;
     /* uint8 samples: 15 compute warps x 2 trials (+ the producer = 16 warps, 128 registers per thread, 30 trials per CTA):
@@ -192,8 +199,10 @@ static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16,
         p.skew_q16 = per_tile >= 0.25 ? (int32_t)std::min(per_tile * 65536.0, 2.0e9) : 0;
     }
     p.nstages = (C + p.chan_block - 1) / p.chan_block;
-    /* 16-bit lanes are carried every 65536 / (largest sample value + 1) channels: bytes 256, uint16 sums of b bytes 256/b */
-    p.spill_stages = (in16 ? 256 / rg.r.bin : 256) / p.chan_block;
+    /* 16-bit lanes are carried every 65536 / (largest sample value + 1) channels: bytes 256, uint16 sums of b bytes 256/b,
+     * the offset-uint16 form 65536 / (lo16_max + 1) */
+    p.spill_stages = carry_channels / p.chan_block;
+    if (p.spill_stages < 1) return false;
     const int32_t CB = p.chan_block, Cpad = p.nstages * CB, WB = p.window_bytes;
     etab.assign((size_t)p.ndm_tiles * Cpad * kDmTile, 0);
     x0tab.assign((size_t)p.ndm_tiles * Cpad, 0);
@@ -236,20 +245,38 @@ static bool plan_range(Strategy& s, Range& rg, std::vector<int32_t>& etab, std::
         }
     }
     rg.max_delay = rg.delays[(size_t)(nd - 1) * C + (C - 1)];
-    if (!plan_format(s, rg, rg, rg.r.bin > 1, etab, x0tab)) {
-        /* a window that does not fit shared memory is not an error of the plan: such a range (DM step very coarse for the
-         * band) takes the one-thread-per-output kernel on a device delay table; everything else about it stays the same */
-        rg.naive = true;
-        rg.in16 = rg.r.bin > 1; rg.esz = rg.in16 ? 2 : 1; rg.spw = 4 / rg.esz; rg.ncopy = rg.spw;
+    auto no_main = [&]() {                 /* no tiled plan on the main input form */
+        rg.in16 = (rg.r.bin > 1 || s.plan.input_bits == 16); rg.esz = rg.in16 ? 2 : 1; rg.spw = 4 / rg.esz; rg.ncopy = rg.spw;
         rg.dm_tile = kDmTile; rg.ndm_tiles = 0; rg.nstages = 0; rg.chan_block = 8; rg.window_bytes = 0;
         etab.clear(); x0tab.clear();
-        rg.has_lo = false;
+    };
+    rg.naive = false; rg.has_lo = false; rg.main_exc = false; rg.dense_naive = false;
+    if (s.plan.input_bits == 16) {
+        /* 16-bit samples (k_input16.cu): bin 1 / 2 / 4 ride the byte path on the offset-uint8 form, bin 8 the uint16 path on the
+         * offset-uint16 form; a chunk with too many exceptions, or a range whose window does not fit, takes the global-memory
+         * kernel on the plain binned samples */
+        rg.dense_naive = true;
+        if (rg.r.bin <= 4) {
+            no_main();
+            rg.has_lo = plan_format(s, rg, rg.lo, 0, 256, etab_lo, x0tab_lo);
+            if (!rg.has_lo) { rg.naive = true; rg.dense_naive = false; }
+        } else {
+            if (plan_format(s, rg, rg, 1, 65536 / (s.lo16_max + 1), etab, x0tab)) rg.main_exc = true;
+            else { no_main(); rg.naive = true; rg.dense_naive = false; }
+        }
+        return true;
+    }
+    if (!plan_format(s, rg, rg, rg.r.bin > 1, rg.r.bin > 1 ? 256 / rg.r.bin : 256, etab, x0tab)) {
+        /* a window that does not fit shared memory is not an error of the plan: such a range (DM step very coarse for the
+         * band) takes the one-thread-per-output kernel on a device delay table; everything else about it stays the same */
+        no_main();
+        rg.naive = true;
         return true;
     }
     /* bin 2 and 4 also get the offset-uint8 route (half the shared-memory bytes per add); the uint16 plan above stays as
-     * the route for chunks with too many exceptions. C < 65536 so a channel index fits the exception record. */
-    rg.has_lo = (rg.r.bin == 2 || rg.r.bin == 4) && C < 65536;
-    if (rg.has_lo && !plan_format(s, rg, rg.lo, 0, etab_lo, x0tab_lo)) rg.has_lo = false;
+     * the route for chunks with too many exceptions. */
+    rg.has_lo = (rg.r.bin == 2 || rg.r.bin == 4);
+    if (rg.has_lo && !plan_format(s, rg, rg.lo, 0, 256, etab_lo, x0tab_lo)) rg.has_lo = false;
     return true;
 }
 
@@ -272,6 +299,8 @@ static aa_status plan_host(aa_strategy* h, const aa_plan* plan, uint64_t nsamp_t
     }
     s.B = 1;
     for (const aa_dm_range& r : s.plan.ranges) s.B = std::max(s.B, r.bin);
+    s.esz_in = s.plan.input_bits == 16 ? 2 : 1;
+    s.lo16_max = C <= 16384 ? 1023 : 255;      /* nchans * lo16_max < 2^24: the packed accumulators of the uint16 kernel */
     s.ranges.resize(s.plan.ranges.size());
     etabs.resize(2 * s.ranges.size()); x0tabs.resize(2 * s.ranges.size());      /* [r]: main plan, [nranges + r]: offset-uint8 plan */
     int64_t smax = 0;
@@ -285,7 +314,7 @@ static aa_status plan_host(aa_strategy* h, const aa_plan* plan, uint64_t nsamp_t
         smax = std::max<int64_t>(smax, (rg.max_delay + rg.extra) * rg.r.bin);
         rg.first_row = s.nrows;
         s.nrows += (size_t)rg.r.ndms;
-        if (rg.r.bin == 1) s.need_u8_copies = true;
+        if (rg.r.bin == 1 && s.plan.input_bits == 8) s.need_u8_copies = true;
     }
     /* a naive range reads the uint16 form of its bin on every chunk, so that bin keeps no offset-uint8 route */
     for (const Range& nv : s.ranges)
@@ -295,6 +324,16 @@ static aa_status plan_host(aa_strategy* h, const aa_plan* plan, uint64_t nsamp_t
      * then read a uint16 buffer that a sparse chunk never filled. So a bin keeps the route only if all its ranges have it. */
     for (const Range& nl : s.ranges)
         if (!nl.has_lo) for (Range& rg : s.ranges) if (rg.r.bin == nl.r.bin) rg.has_lo = false;
+    /* 16-bit plans: a bin's rows hold EITHER its offset form (with the plain samples written only for exception-heavy chunks) OR,
+     * if one of its ranges has only the global-memory route, the plain samples always: then every range of the bin takes it */
+    if (s.plan.input_bits == 16)
+        for (const Range& nv : s.ranges)
+            if (nv.naive)
+                for (Range& rg : s.ranges)
+                    if (rg.r.bin == nv.r.bin && !rg.naive) {
+                        rg.naive = true; rg.dense_naive = false; rg.has_lo = false; rg.main_exc = false;
+                        rg.ndm_tiles = 0; rg.nstages = 0; etabs[(size_t)rg.index].clear(); x0tabs[(size_t)rg.index].clear();
+                    }
     s.S = (int64_t)round_up((size_t)smax, (size_t)s.B);
     const int64_t usable = (int64_t)(nsamp_total / (uint64_t)s.B) * s.B;
     if (usable <= s.S) {
@@ -432,17 +471,19 @@ extern "C" aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, u
     const Chunk& last = s.chunks.back();
     for (size_t r = 0; r < s.ranges.size(); ++r) {
         Range& rg = s.ranges[r];
-        if (rg.naive && (e = cudaMemcpyAsync(rg.d_delays, rg.delays.data(), rg.delays.size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "delay table upload"));
+        if ((rg.naive || rg.dense_naive) && (e = cudaMemcpyAsync(rg.d_delays, rg.delays.data(), rg.delays.size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "delay table upload"));
         if (rg.naive) { for (int32_t i = 0; i < rg.r.ndms; ++i) { const int32_t* base = rg.d_D + (size_t)i * (size_t)rg.pitch; rows_full[rg.first_row + i] = aak_row_desc{base, rg.nt_full}; rows_last[rg.first_row + i] = aak_row_desc{base, (int64_t)(last.n_out / (uint64_t)rg.r.bin)}; } continue; }
-        if ((e = cudaMemcpyAsync(rg.d_etab, etabs[r].data(), etabs[r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
-        if ((e = cudaMemcpyAsync(rg.d_x0tab, x0tabs[r].data(), x0tabs[r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
+        const bool has_main = rg.ndm_tiles > 0;
+        if (has_main && (e = cudaMemcpyAsync(rg.d_etab, etabs[r].data(), etabs[r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
+        if (has_main && (e = cudaMemcpyAsync(rg.d_x0tab, x0tabs[r].data(), x0tabs[r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
         if (rg.has_lo) {
             const size_t n = s.ranges.size();
             if ((e = cudaMemcpyAsync(rg.lo.d_etab, etabs[n + r].data(), etabs[n + r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
             if ((e = cudaMemcpyAsync(rg.lo.d_x0tab, x0tabs[n + r].data(), x0tabs[n + r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
             if (!make_window_map(&rg.lo.map, s.d_lo[rg.r.bin], s.lo_stride[rg.r.bin], s.lo_pitch[rg.r.bin], s.lo_stride[rg.r.bin], 4, C, rg.lo.window_bytes)) return fail(AA_ERR_CUDA);
         }
-        if (rg.in16) {
+        if (!has_main) {
+        } else if (rg.in16) {
             if (!make_window_map(&rg.map, s.d_xb[rg.r.bin], s.xb_stride[rg.r.bin], s.xb_pitch[rg.r.bin] * 2, s.xb_stride[rg.r.bin], 2, C, rg.window_bytes)) return fail(AA_ERR_CUDA);
         } else {
             if (!make_window_map(&rg.map, s.d_x4, s.x4_stride, s.x4_pitch, s.x4_stride, 4, C, rg.window_bytes)) return fail(AA_ERR_CUDA);
@@ -498,6 +539,7 @@ extern "C" aa_status aa_strategy_get_info(const aa_strategy* h, aa_strategy_info
     out->arena_bytes_used = s.arena.used; out->arena_bytes_total = s.arena.size; out->max_candidates = s.max_candidates;
     out->owns_arena = s.owns_arena ? 1 : 0;
     out->input_layout = s.plan.layout;
+    out->input_bits = s.plan.input_bits; out->input_max = s.plan.input_max;
     return AA_OK;
 }
 
@@ -506,7 +548,8 @@ extern "C" aa_status aa_strategy_get_range_info(const aa_strategy* h, int32_t ra
     if (!out || range < 0 || range >= (int32_t)h->s.ranges.size()) { set_error("aa_strategy_get_range_info: range %d out of bounds", range); return AA_ERR_INVALID_ARG; }
     const Range& rg = h->s.ranges[(size_t)range];
     out->ndms = rg.r.ndms; out->bin = rg.r.bin; out->nt = rg.nt_full; out->row_pitch = rg.pitch; out->max_delay = rg.max_delay;
-    out->dm_tile = rg.dm_tile; out->t_tile = kTTile; out->chan_block = rg.chan_block; out->window = rg.window_bytes;
+    const K2Plan& kp = (rg.ndm_tiles > 0 || !rg.has_lo) ? static_cast<const K2Plan&>(rg) : rg.lo;     /* the tiled plan that exists */
+    out->dm_tile = kp.dm_tile; out->t_tile = kTTile; out->chan_block = kp.chan_block; out->window = kp.window_bytes;
     out->boxcar_extra = rg.extra;
     return AA_OK;
 }
@@ -551,6 +594,8 @@ extern "C" size_t aa_strategy_describe(const aa_strategy* h, char* buf, size_t b
                  aak_dedisperse_smem_bytes(rg.chan_block, rg.window_bytes, rg.in16, rg.ring_stages));
         o += line;
         if (rg.naive) o += "         tile window does not fit shared memory: one-thread-per-output kernel on a device delay table\n";
+        if (rg.main_exc) o += "         the uint16 plan reads the offset-uint16 form (per-channel offsets + exceptions)\n";
+        if (rg.dense_naive) o += "         exception-heavy chunks take the one-thread-per-output kernel on the plain binned samples\n";
         if (rg.has_lo) {
             snprintf(line, sizeof line, "         offset-uint8 route: chan_block=%d window=%dB stages=%d ring=%d exception limit %u per chunk\n",
                      rg.lo.chan_block, rg.lo.window_bytes, rg.lo.nstages, rg.lo.ring_stages, s.exc_limit[rg.r.bin]);

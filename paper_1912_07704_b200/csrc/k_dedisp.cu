@@ -341,8 +341,8 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
                 *reinterpret_cast<int4*>(row + t) = v;
             } else {
                 int2 v;
-                v.x = (int)((A[m][j] & 0xFFFFu) + ((C1[m][j] & 0xFFFFu) << 8));
-                v.y = (int)((A[m][j] >> 16) + ((C1[m][j] >> 16) << 8));
+                v.x = bias + (int)((A[m][j] & 0xFFFFu) + ((C1[m][j] & 0xFFFFu) << 8));
+                v.y = bias + (int)((A[m][j] >> 16) + ((C1[m][j] >> 16) << 8));
                 if (p.accumulate) {
                     const int2 o = *reinterpret_cast<const int2*>(row + t);
                     v.x += o.x; v.y += o.y;
@@ -357,7 +357,9 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
  * step so coarse for the band that 30 trials spread over more than ~14 000 samples), and a cross-check. */
 template <typename T>
 __global__ void k_dedisperse_naive(const T* __restrict__ x, size_t pitch, const int32_t* __restrict__ delays, int nchans, int c0, int c1,
-                                   int ndms, long long nt, int32_t* __restrict__ D, long long dpitch, int accumulate) {
+                                   int ndms, long long nt, int32_t* __restrict__ D, long long dpitch, int accumulate,
+                                   const unsigned* __restrict__ mode_cnt, unsigned mode_cap) {
+    if (mode_cnt && *mode_cnt <= mode_cap) return;                   /* the offset form handles this chunk */
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int i = blockIdx.y;
     if (t >= nt || i >= ndms) return;
@@ -437,14 +439,14 @@ extern "C" int aak_dedisperse(const aak_dedisp_args* a, void* stream) {
 
 extern "C" int aak_dedisperse_naive(const void* x, size_t pitch_elems, int32_t in16, const int32_t* delays, int32_t nchans,
                                     int32_t chan_begin, int32_t chan_end, int32_t ndms, int64_t nt, int32_t* D, int64_t pitch,
-                                    int32_t accumulate, void* stream) {
+                                    int32_t accumulate, const unsigned* mode_cnt, unsigned mode_cap, void* stream) {
     cudaStream_t st = (cudaStream_t)stream;
     if (ndms <= 0 || nt <= 0) return 0;
     if (ndms > 65535) return (int)cudaErrorInvalidConfiguration;
     dim3 grid((unsigned)((nt + 255) / 256), (unsigned)ndms);
     if (in16)
-        k_dedisperse_naive<uint16_t><<<grid, 256, 0, st>>>((const uint16_t*)x, pitch_elems, delays, nchans, chan_begin, chan_end, ndms, nt, D, pitch, accumulate);
+        k_dedisperse_naive<uint16_t><<<grid, 256, 0, st>>>((const uint16_t*)x, pitch_elems, delays, nchans, chan_begin, chan_end, ndms, nt, D, pitch, accumulate, mode_cnt, mode_cap);
     else
-        k_dedisperse_naive<uint8_t><<<grid, 256, 0, st>>>((const uint8_t*)x, pitch_elems, delays, nchans, chan_begin, chan_end, ndms, nt, D, pitch, accumulate);
+        k_dedisperse_naive<uint8_t><<<grid, 256, 0, st>>>((const uint8_t*)x, pitch_elems, delays, nchans, chan_begin, chan_end, ndms, nt, D, pitch, accumulate, mode_cnt, mode_cap);
     return (int)cudaGetLastError();
 }

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include "aa_kernels.h"
+#include "k_common.cuh"
 
 namespace {
 
@@ -162,10 +163,10 @@ k_scatter_exceptions(const uint2* __restrict__ exc, const unsigned* __restrict__
         const int i = (int)(q - (unsigned long long)e * (unsigned)ndms);
         const uint2 rec = exc[e];
         const int c = (int)(rec.x & 0xFFFFu);
-        const int r = (int)(rec.x >> 16) - 1024;
+        const int r = ((int)(((rec.x >> 16) | ((rec.y >> 28) << 16)) << 12)) >> 12;          /* sign-extend 20 bits */
         const double dm = __dadd_rn(dm_low, __dmul_rn((double)i, dm_step));
         const long long delay = llround(__ddiv_rn(__dmul_rn(k[c], dm), (double)bin));
-        const long long t = (long long)rec.y - delay;
+        const long long t = (long long)(rec.y & 0x0FFFFFFFu) - delay;
         if (t >= 0 && t < nt) atomicAdd(D + (size_t)i * (size_t)pitch + (size_t)t, r);
     }
 }
@@ -184,20 +185,6 @@ struct PrepFused {
 
 __device__ __forceinline__ uint32_t byte_of(const uint32_t (&w)[8], int i) { return (w[i >> 2] >> (8 * (i & 3))) & 0xFFu; }
 
-/* Append one exception record. The lanes of a warp that arrive together share ONE atomic on the counter; once the counter
- * has passed `cap` the chunk is bound for the other route anyway (every route test is `counter > limit`, limit <= cap, and
- * the counter never decreases), so nothing more is counted or recorded: a dense input costs one L2 read per exception
- * instead of one same-address atomic. */
-__device__ __forceinline__ void append_exception(uint2* __restrict__ exc, unsigned* __restrict__ cnt, unsigned cap, uint2 rec) {
-    if (*reinterpret_cast<volatile unsigned*>(cnt) > cap) return;
-    const unsigned m = __activemask();
-    const int lane = threadIdx.x & 31, leader = __ffs(m) - 1;
-    unsigned base = 0;
-    if (lane == leader) base = atomicAdd(cnt, (unsigned)__popc(m));
-    base = __shfl_sync(m, base, leader);
-    const unsigned idx = base + (unsigned)__popc(m & ((1u << lane) - 1u));
-    if (idx < cap) exc[idx] = rec;
-}
 
 __global__ void __launch_bounds__(256)
 k_prep_fused(const PrepFused p) {
@@ -229,7 +216,7 @@ k_prep_fused(const PrepFused p) {
             l[k] = (uint32_t)v;
             const long long t = g * 8 + k;
             if (k < 8 && y != v && t < p.nb2)
-                append_exception(p.exc2, p.cnt2, p.cap, make_uint2((uint32_t)(p.chan0 + c) | ((uint32_t)(y - v + 1024) << 16), (uint32_t)t));
+                append_exception(p.exc2, p.cnt2, p.cap, make_exception(p.chan0 + c, t, y - v));
         }
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
@@ -248,7 +235,7 @@ k_prep_fused(const PrepFused p) {
             l[k] = (uint32_t)v;
             const long long t = g * 4 + k;
             if (k < 4 && y != v && t < p.nb4)
-                append_exception(p.exc4, p.cnt4, p.cap, make_uint2((uint32_t)(p.chan0 + c) | ((uint32_t)(y - v + 1024) << 16), (uint32_t)t));
+                append_exception(p.exc4, p.cnt4, p.cap, make_exception(p.chan0 + c, t, y - v));
         }
 #pragma unroll
         for (int j = 0; j < 4; ++j)

@@ -496,6 +496,7 @@ struct SpsParams {
     double threshold;
     aak_candidate* cands; u64* counter; u64 capacity;
     const double* wstats; const i64* wpivot; const int* wlive;     /* reading C7m (NULL: reading C7) */
+    unsigned* range_flag;                                          /* NULL, or: bit 0 set when wmax * max|d| of a row reaches 2^31 */
 };
 
 struct K4RowConst {                            /* per ring slot */
@@ -673,6 +674,20 @@ k_sps_peaks(const SpsParams p) {
                     loc[v][k] = run;
                 }
             }
+            if (p.range_flag) {                                      /* block-uniform; plans without a plan-time bound only */
+                long long mx = 0;
+#pragma unroll
+                for (int v = 0; v < V; ++v) {
+                    const int e = e0 + 4 * v;
+                    const int d[4] = {cur[v].x, cur[v].y, cur[v].z, cur[v].w};
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const long long a = (long long)d[k] - (long long)pv_c;
+                        if ((e + k >= e_lo) && (e + k < e_hi)) mx = max(mx, a < 0 ? -a : a);
+                    }
+                }
+                if (mx * (long long)p.wmax >= (1ll << 31)) atomicOr(p.range_flag, 1u);
+            }
         }
         unsigned incl = run;
 #pragma unroll
@@ -816,7 +831,7 @@ extern "C" int aak_sps_peaks(const aak_sps_args* a, void* stream) {
     for (int k = 0; k < a->nwidths; ++k) if (a->widths[k] != (1 << k)) p.pow2 = 0;
     for (int k = 0; k < SPS_MAXW; ++k) { p.widths[k] = k < a->nwidths ? a->widths[k] : 0; if (p.widths[k] > p.wmax) p.wmax = p.widths[k]; }
     p.threshold = a->threshold; p.cands = a->cands; p.counter = (u64*)a->counter; p.capacity = a->capacity;
-    p.wstats = a->wstats; p.wpivot = (const i64*)a->wpivot; p.wlive = a->wlive;
+    p.wstats = a->wstats; p.wpivot = (const i64*)a->wpivot; p.wlive = a->wlive; p.range_flag = a->range_flag;
     if (a->nt <= 0 || a->ndms <= 0) return 0;
     /* segment = tt + 4 + wmax elements <= 1024 V; the strip keeps at least ~2000 centre samples */
     const int V = p.wmax <= 1024 ? 3 : (p.wmax <= 2048 ? 4 : 8);

@@ -252,7 +252,8 @@ class GpuRun:
         self.aa, self.w = aa, w
         self.x = np.ascontiguousarray(x.T) if time_major else x
         self.plan = aa.Plan(w.freqs_mhz, w.tsamp_s, w.ranges, w.widths, w.threshold, time_major=time_major,
-                            boxcar_overlap=boxcar_overlap, per_width_stats=per_width)
+                            boxcar_overlap=boxcar_overlap, per_width_stats=per_width, input_bits=w.input_bits,
+                            input_max=w.max_value if w.input_bits == 16 else 0)
         self.extra = max(w.widths) - 1 if boxcar_overlap else 0          # reading C3x
         self.st = aa.Strategy(self.plan, x.shape[1], **strategy_kw)
         self.h = self.st.handle

@@ -301,7 +301,7 @@ def test_clusters_of_the_tiny_pulse():
 @pytest.mark.parametrize("seed", range(int(__import__("os").environ.get("AA_TEST_FUZZ", "6"))))
 def test_random_small_configurations_match_the_oracle(seed):
     """Randomised shapes and options (channel counts around the tile and group sizes, 1-3 DM ranges with random binning,
-    arbitrary width lists, chunking, time-major input, boxcar-complete chunks, uniform or Gaussian samples): every row,
+    arbitrary width lists, chunking, time-major input, boxcar-complete chunks, uniform or Gaussian samples, 8- or 16-bit input): every row,
     statistic and candidate equals the oracle's. AA_TEST_FUZZ=N runs N seeds (default 6)."""
     rs = np.random.default_rng(1000 + seed)
     C = int(rs.choice([1, 3, 7, 8, 9, 31, 64, 100, 255, 256, 257, 300, 520]))
@@ -332,11 +332,14 @@ def test_random_small_configurations_match_the_oracle(seed):
         hint = int(-(-(S + n_out_target) // B) * B)
         if hint >= (nsamp // B) * B:
             hint = 0
+    bits16 = bool(rs.integers(0, 3) == 0)                                 # a third of the cases: 16-bit input samples
+    depth = int(rs.choice([1023, 4095, 8191])) if bits16 else 255
     w = Workload("fz", C, f_top, -bw / max(C, 2), tsamp, nsamp, tuple(ranges), widths, 5.0, seed=seed, npulses=2, pulse_dm=(0.0, max(dm, 1.0)),
-                 pulse_width_max=max(widths), pulse_snr=(9.0, 20.0))
+                 pulse_width_max=max(widths), pulse_snr=(9.0, 20.0), noise_mean=float(depth // 2) if bits16 else 127.0,
+                 input_bits=16 if bits16 else 8, max_value=depth)
     x, _ = make_input(w)
     if rs.integers(0, 3) == 0:
-        x = rs.integers(0, 256, size=x.shape, dtype=np.uint8)             # dense exceptions: uint16 route for bin 2 / 4
+        x = rs.integers(0, depth + 1, size=x.shape, dtype=x.dtype)        # dense exceptions: the dense route of every offset form
     tm = bool(rs.integers(0, 2))
     kw = dict(chunk_len_hint=hint) if hint else {}
     gpu, orc = GpuRun(w, x, time_major=tm, boxcar_overlap=boxcar, **kw), OracleRun(w, x)

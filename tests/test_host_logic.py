@@ -237,3 +237,45 @@ int main(void) {
     out = subprocess.run([str(exe)], capture_output=True, text=True)
     assert out.returncode == 0, (out.returncode, out.stdout, out.stderr)
     assert "sm_100a" in out.stdout
+
+
+# ------------------------------------------------------------------------------------------------ 16-bit plans
+def test_input_bits_validation_names_the_limit_and_the_strategy_plans_the_offset_forms():
+    """aa_plan_set_input_bits: the stated limits are checked with a message naming them; a 16-bit SKA-like plan has the same
+    geometry as the 8-bit one (the sample type changes nothing in C2/C3), one more raw byte per sample in the arena, and
+    every range on an offset form with the global-memory kernel behind it."""
+    w = datagen.get_workload("ska16")
+    plan = _plan(w)
+    try:
+        for bits, mx, word in ((12, 4095, "bits"), (16, 70000, "16 bits"), (16, 8192, "binned sample"), (16, 65535, "binned sample")):
+            with pytest.raises(aa.AaError) as e:
+                aa.aa_plan_set_input_bits(plan, bits, mx)
+            assert e.value.status == aa.AA_ERR_INVALID_ARG and word in e.value.message, e.value.message
+        aa.aa_plan_set_input_bits(plan, 16, w.max_value)
+        st = aa.aa_strategy_plan(plan, w.nsamp)
+        try:
+            info = aa.aa_strategy_get_info(st)
+            assert (info["input_bits"], info["input_max"], info["overlap"], info["n_out"], info["nchunks"]) == (16, 4095, 32384, 491904, 1)
+            desc = aa.aa_strategy_describe(st)
+            assert desc.count("offset-uint8 route") == 4 and "offset-uint16 form" in desc and desc.count("plain binned samples") == 5
+            p8 = _plan(datagen.get_workload("ska"))
+            s8 = aa.aa_strategy_plan(p8, w.nsamp)
+            i8 = aa.aa_strategy_get_info(s8)
+            aa.aa_strategy_destroy(s8); aa.aa_plan_destroy(p8)
+            grow = info["arena_bytes_used"] - i8["arena_bytes_used"]
+            assert 0.9 * w.nchans * w.nsamp < grow < 1.3 * w.nchans * w.nsamp      # the raw chunk is twice as large; delay tables
+        finally:
+            aa.aa_strategy_destroy(st)
+    finally:
+        aa.aa_plan_destroy(plan)
+    # nchans * max_value * max bin must fit int32
+    big = aa.aa_plan_create(1500.0 - 0.01 * np.arange(40000), 64e-6, ((0.0, 1.0, 4, 1),), (1,), 6.0)
+    try:
+        with pytest.raises(aa.AaError) as e:
+            aa.aa_plan_set_input_bits(big, 16, 65535)                      # 40000 * 65535 > 2^31
+        assert "int32" in e.value.message
+        # still fine with a smaller maximum
+        aa.aa_plan_set_input_bits(big, 16, 1023)
+        aa.aa_plan_set_input_bits(big, 8, 0)
+    finally:
+        aa.aa_plan_destroy(big)
