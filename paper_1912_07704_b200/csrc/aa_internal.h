@@ -65,8 +65,16 @@ struct K2Plan {
     int32_t dms_per_warp = 2, variant = 1, ring_stages = 3;   /* K2 tuning chosen by the strategy */
     int32_t* d_etab = nullptr;
     int32_t* d_x0tab = nullptr;
-    CUtensorMap map;              /* 4-D window map over the NCOPY-copy input buffer of this format */
+    /* Window classes: a channel block (stage) loads a window only as wide as ITS channels' delay spread inside a DM tile needs
+     * (the spread grows down the band), rounded up to 256 bytes; window_bytes is the widest (it sizes the shared-memory ring).
+     * One tensor map per distinct width (at most kMaxWinClasses; widths in between are rounded up to the next class). */
+    int32_t nclass = 1;
+    int32_t class_wb[8] = {0};
+    std::vector<int32_t> wcls;    /* [nstages] class of each stage (host copy) */
+    int32_t* d_wcls = nullptr;
+    CUtensorMap maps[8];          /* 4-D window maps over the NCOPY-copy input buffer of this format, one per class */
 };
+constexpr int kMaxWinClasses = 8;
 
 struct Range : K2Plan {           /* the base is the range's main plan: uint8 for bin 1, uint16 for binned ranges */
     aa_dm_range r;

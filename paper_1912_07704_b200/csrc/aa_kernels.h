@@ -77,13 +77,18 @@ int aak_corner_turn16(const uint16_t* in, size_t in_stride_bytes, uint16_t* out,
  * mbarrier ring.
  * The input exists as NCOPY = 4 (uint8) or 2 (uint16) sample-shifted copies in ONE global buffer, copy k = x[c][t+k]
  * at byte offset k*copy_stride; tmap points at the 128-byte 4-D CUtensorMap over it (HOST memory).
- * A stage in shared memory is [chan_block][NCOPY][window_bytes] followed by the stage's slice of etab.
+ * A stage in shared memory is [chan_block][NCOPY][class_wb[wcls[stage]]], and at byte chan_block*NCOPY*window_bytes the stage's
+ * slice of etab.
  * etab  [ndm_tiles][nstages][chan_block][32] int32 : shared-memory byte offset of (channel, DM) inside a stage (rows of 32
  *                                                  entries, the first dm_tile are used; ndm_tiles = ceil(ndms / dm_tile))
  * x0tab [ndm_tiles][nstages*chan_block]    int32 : 16-byte aligned BYTE offset of the channel window relative to the
  *                                                  tile's first output sample */
 typedef struct {
-    const void* tmap;          /* HOST pointer to the 128-byte CUtensorMap (copied into kernel params) */
+    const void* tmap;          /* HOST pointer to nclass consecutive 128-byte CUtensorMaps (copied into kernel params): map k loads
+                                  windows of class_wb[k] bytes */
+    int32_t nclass;            /* 1..8 window classes */
+    int32_t class_wb[8];       /* window bytes of each class (multiples of 256, <= window_bytes) */
+    const int32_t* wcls;       /* [nstages] class of each stage (channel block) */
     const int32_t* etab;
     const int32_t* x0tab;
     int32_t* D;                /* [ndms][pitch] */
@@ -92,7 +97,7 @@ typedef struct {
     int32_t ndms;
     int32_t nchans;
     int32_t chan_block;        /* 8, 4 or 2 */
-    int32_t window_bytes;      /* WB: bytes per (copy, channel) window in shared memory, multiple of 256 */
+    int32_t window_bytes;      /* WB: the WIDEST (copy, channel) window in shared memory, multiple of 256; sizes the ring slots */
     int32_t spill_stages;      /* carry the 16-bit lanes every this many stages: 256/chan_block (bytes), (256/bin)/chan_block (uint16) */
     int32_t in16;              /* 0: byte input (bin 1, or the offset-uint8 form of a binned input), 1: uint16 binned input */
     int32_t variant;           /* uint8 only: odd-byte lane adds as 0 = IADD3, 1 = IMAD (FMA pipe), 2 = alternating */

@@ -178,7 +178,9 @@ aa_status enqueue_k2(Strategy& s, const Chunk& c, int32_t c0, int32_t c1, bool a
             if (route == 1 && !has_main) continue;
             const K2Plan& p = route == 0 ? rg.lo : static_cast<const K2Plan&>(rg);
             const bool route_sparse = route == 0 || rg.main_exc;
-            a.tmap = &p.map; a.etab = p.d_etab; a.x0tab = p.d_x0tab;
+            a.tmap = p.maps; a.etab = p.d_etab; a.x0tab = p.d_x0tab;
+            a.nclass = p.nclass; a.wcls = p.d_wcls;
+            for (int k = 0; k < 8; ++k) a.class_wb[k] = p.class_wb[k];
             a.chan_block = p.chan_block; a.window_bytes = p.window_bytes; a.spill_stages = p.spill_stages; a.in16 = p.in16;
             a.variant = p.variant; a.dms_per_warp = p.dms_per_warp; a.ring_stages = p.ring_stages; a.dm_tile = p.dm_tile; a.skew_q16 = p.skew_q16;
             a.mode_cnt = cnt; a.mode_cap = lim; a.mode_dense = route_sparse ? 0 : 1;

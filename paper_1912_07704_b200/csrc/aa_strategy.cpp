@@ -43,8 +43,8 @@ int64_t delay_of(const Strategy& s, const Range& rg, int32_t chan, int32_t dm_in
 
 /* Channel rows of the NCOPY shifted copies seen as overlapping 256-byte segments: a {256, nseg, NCOPY, 1} box lands as
  * NCOPY linear windows of window_bytes each (k_dedisp.cu). Rows are pitch_bytes apart, the copies of a row copy_stride. */
-static bool make_window_map(CUtensorMap* map, void* base, size_t row_bytes, size_t pitch_bytes, size_t copy_stride, int32_t ncopy,
-                            int32_t nchans, int32_t window_bytes) {
+static bool make_window_map1(CUtensorMap* map, void* base, size_t row_bytes, size_t pitch_bytes, size_t copy_stride, int32_t ncopy,
+                             int32_t nchans, int32_t window_bytes) {
     EncodeTiledFn enc = encode_fn();
     if (!enc) { set_error("aa_strategy_setup: cuTensorMapEncodeTiled is not available from this driver"); return false; }
     const cuuint32_t nseg = (cuuint32_t)(window_bytes / 256);
@@ -55,6 +55,13 @@ static bool make_window_map(CUtensorMap* map, void* base, size_t row_bytes, size
     const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 4, base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { set_error("aa_strategy_setup: cuTensorMapEncodeTiled failed with CUresult %d", (int)r); return false; }
+    return true;
+}
+
+/* The maps of all window classes of one K2 plan. */
+static bool make_window_maps(K2Plan& p, void* base, size_t row_bytes, size_t pitch_bytes, size_t copy_stride, int32_t ncopy, int32_t nchans) {
+    for (int k = 0; k < p.nclass; ++k)
+        if (!make_window_map1(&p.maps[k], base, row_bytes, pitch_bytes, copy_stride, ncopy, nchans, p.class_wb[k])) return false;
     return true;
 }
 
@@ -104,9 +111,13 @@ static void carve(Strategy& s, int64_t L, bool two_stage) {
         s.d_off[b] = sparse ? (int32_t*)a.take((size_t)s.plan.nchans * 4) : nullptr;
         s.d_exc[b] = sparse ? (uint2*)a.take((size_t)kMaxGroups * kExcCap * sizeof(uint2)) : nullptr;
         s.d_exc_cnt[b] = sparse ? (unsigned*)a.take(2 * kMaxGroups * 4) : nullptr;
-        /* the scatter costs one atomic per (exception, trial), measured 2.7e10 atomics/s: beyond ~1e8 of them per chunk the
-         * dense route is cheaper (a channel group gets the share of its channels) */
-        s.exc_limit[b] = sparse ? (unsigned)std::min<int64_t>((int64_t)kMaxGroups * kExcCap, std::max<int64_t>(1, 100000000 / std::max<int64_t>(1, nd))) : 0;
+        /* Route test = an exception RATE. The scatter costs one atomic per (exception, trial) at a measured 2.7e10 atomics/s; the
+         * dense route costs the range about 2.9e-14 s more per add (16 against 30 Tadd/s measured). Both grow with the number of
+         * trials, so the break-even is a fraction of the bin's samples, 2.9e-14 x 2.7e10 = 8e-4; half of it is allowed (Gaussian
+         * noise: 2e-8 at bin 2, 6e-5 at bin 4, 5e-3 at bin 8). The earlier absolute budget of 1e8 atomics sent the bin-4 range of
+         * the low-frequency configuration (1.3e5 exceptions x 2500 trials) down the uint16 route: 257 ms instead of ~150. */
+        (void)nd;
+        s.exc_limit[b] = sparse ? (unsigned)std::min<double>((double)kMaxGroups * kExcCap, std::max(1.0, 4.0e-4 * (double)s.plan.nchans * (double)(L / b))) : 0;
         if (sparse && !s.d_k_needed) s.d_k_needed = true;
     }
     s.d_k = s.d_k_needed ? (double*)a.take((size_t)s.plan.nchans * 8) : nullptr;
@@ -118,9 +129,11 @@ static void carve(Strategy& s, int64_t L, bool two_stage) {
         rg.d_delays = (rg.naive || rg.dense_naive) ? (int32_t*)a.take((size_t)rg.r.ndms * s.plan.nchans * 4) : nullptr;
         rg.d_etab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * kDmTile * 4);   /* rg. = the main plan */
         rg.d_x0tab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * 4);
+        rg.d_wcls = (int32_t*)a.take((size_t)rg.nstages * 4);
         if (rg.has_lo) {
             rg.lo.d_etab = (int32_t*)a.take((size_t)rg.lo.ndm_tiles * rg.lo.nstages * rg.lo.chan_block * kDmTile * 4);
             rg.lo.d_x0tab = (int32_t*)a.take((size_t)rg.lo.ndm_tiles * rg.lo.nstages * rg.lo.chan_block * 4);
+            rg.lo.d_wcls = (int32_t*)a.take((size_t)rg.lo.nstages * 4);
         }
     }
     s.d_rows[0] = (aak_row_desc*)a.take(s.nrows * sizeof(aak_row_desc));
@@ -165,14 +178,18 @@ static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16,
      * binned uint16 samples: 16 warps x (4 adjacent trials, half the tile), 32 trials per CTA */
     p.dm_tile = in16 ? kDmTile : 30;
     p.ndm_tiles = (nd + p.dm_tile - 1) / p.dm_tile;
-    /* widest window: T_TILE + largest in-tile delay spread + alignment residue (< 16 bytes) */
+    /* in-tile delay spread of every channel (largest over the DM tiles); the widest window: T_TILE + spread + alignment
+     * residue (< 16 bytes) */
+    std::vector<int64_t> spread((size_t)C, 0);
     int64_t omax = 0;
     for (int32_t t = 0; t < p.ndm_tiles; ++t) {
         const int32_t i0 = t * p.dm_tile, i1 = std::min(nd - 1, i0 + p.dm_tile - 1);
         const int32_t* a = rg.delays.data() + (size_t)i0 * C;
         const int32_t* b = rg.delays.data() + (size_t)i1 * C;
-        for (int32_t c = 0; c < C; ++c) omax = std::max<int64_t>(omax, (int64_t)b[c] - a[c]);
+        for (int32_t c = 0; c < C; ++c) spread[(size_t)c] = std::max<int64_t>(spread[(size_t)c], (int64_t)b[c] - a[c]);
     }
+    for (int32_t c = 0; c < C; ++c) omax = std::max(omax, spread[(size_t)c]);
+    auto window_of = [&](int64_t o) { return (int32_t)round_up((size_t)((kTTile + o + 16 / p.esz) * p.esz), 256); };
     const int64_t wsamp = kTTile + omax + 16 / p.esz;
     p.window_bytes = (int32_t)round_up((size_t)(wsamp * p.esz), 256);
     if (p.window_bytes > 65536) return false;
@@ -203,7 +220,35 @@ static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16,
      * the offset-uint16 form 65536 / (lo16_max + 1) */
     p.spill_stages = carry_channels / p.chan_block;
     if (p.spill_stages < 1) return false;
-    const int32_t CB = p.chan_block, Cpad = p.nstages * CB, WB = p.window_bytes;
+    const int32_t CB = p.chan_block, Cpad = p.nstages * CB;
+    /* window classes: the width each channel block needs, at most kMaxWinClasses distinct values (rounded up to the next kept one) */
+    std::vector<int32_t> need((size_t)p.nstages, 256);
+    for (int32_t st = 0; st < p.nstages; ++st) {
+        int64_t o = 0;
+        for (int32_t c = st * CB; c < std::min(C, (st + 1) * CB); ++c) o = std::max(o, spread[(size_t)c]);
+        need[(size_t)st] = window_of(o);
+    }
+    {
+        std::vector<int32_t> vals(need);
+        std::sort(vals.begin(), vals.end());
+        vals.erase(std::unique(vals.begin(), vals.end()), vals.end());
+        while ((int)vals.size() > kMaxWinClasses) {                 /* drop the value whose removal rounds the fewest bytes up */
+            size_t best = 0; int64_t cost = -1;
+            for (size_t k = 0; k + 1 < vals.size(); ++k) {
+                int64_t n = 0;
+                for (int32_t v : need) if (v == vals[k]) ++n;
+                const int64_t cst = n * (int64_t)(vals[k + 1] - vals[k]);
+                if (cost < 0 || cst < cost) { cost = cst; best = k; }
+            }
+            for (int32_t& v : need) if (v == vals[best]) v = vals[best + 1];
+            vals.erase(vals.begin() + (ptrdiff_t)best);
+        }
+        p.nclass = (int32_t)vals.size();
+        for (int k = 0; k < 8; ++k) p.class_wb[k] = k < p.nclass ? vals[(size_t)k] : 0;
+        p.wcls.assign((size_t)p.nstages, 0);
+        for (int32_t st = 0; st < p.nstages; ++st)
+            p.wcls[(size_t)st] = (int32_t)(std::lower_bound(vals.begin(), vals.end(), need[(size_t)st]) - vals.begin());
+    }
     etab.assign((size_t)p.ndm_tiles * Cpad * kDmTile, 0);
     x0tab.assign((size_t)p.ndm_tiles * Cpad, 0);
     for (int32_t t = 0; t < p.ndm_tiles; ++t) {
@@ -211,6 +256,7 @@ static bool plan_format(const Strategy& s, const Range& rg, K2Plan& p, int in16,
         for (int32_t c = 0; c < Cpad; ++c) {
             int32_t* e = etab.data() + ((size_t)t * Cpad + c) * kDmTile;     /* [tile][stage][c_local][m] */
             const int32_t cl = c % CB;
+            const int32_t WB = need[(size_t)(c / CB)];                         /* this channel block's window */
             if (c >= C) {                                                   /* padding channel: TMA zero-fills it */
                 for (int m = 0; m < kDmTile; ++m) e[m] = cl * p.ncopy * WB;
                 continue;
@@ -476,17 +522,19 @@ extern "C" aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, u
         const bool has_main = rg.ndm_tiles > 0;
         if (has_main && (e = cudaMemcpyAsync(rg.d_etab, etabs[r].data(), etabs[r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
         if (has_main && (e = cudaMemcpyAsync(rg.d_x0tab, x0tabs[r].data(), x0tabs[r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
+        if (has_main && (e = cudaMemcpyAsync(rg.d_wcls, rg.wcls.data(), rg.wcls.size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
         if (rg.has_lo) {
             const size_t n = s.ranges.size();
             if ((e = cudaMemcpyAsync(rg.lo.d_etab, etabs[n + r].data(), etabs[n + r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
             if ((e = cudaMemcpyAsync(rg.lo.d_x0tab, x0tabs[n + r].data(), x0tabs[n + r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
-            if (!make_window_map(&rg.lo.map, s.d_lo[rg.r.bin], s.lo_stride[rg.r.bin], s.lo_pitch[rg.r.bin], s.lo_stride[rg.r.bin], 4, C, rg.lo.window_bytes)) return fail(AA_ERR_CUDA);
+            if ((e = cudaMemcpyAsync(rg.lo.d_wcls, rg.lo.wcls.data(), rg.lo.wcls.size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
+            if (!make_window_maps(rg.lo, s.d_lo[rg.r.bin], s.lo_stride[rg.r.bin], s.lo_pitch[rg.r.bin], s.lo_stride[rg.r.bin], 4, C)) return fail(AA_ERR_CUDA);
         }
         if (!has_main) {
         } else if (rg.in16) {
-            if (!make_window_map(&rg.map, s.d_xb[rg.r.bin], s.xb_stride[rg.r.bin], s.xb_pitch[rg.r.bin] * 2, s.xb_stride[rg.r.bin], 2, C, rg.window_bytes)) return fail(AA_ERR_CUDA);
+            if (!make_window_maps(rg, s.d_xb[rg.r.bin], s.xb_stride[rg.r.bin], s.xb_pitch[rg.r.bin] * 2, s.xb_stride[rg.r.bin], 2, C)) return fail(AA_ERR_CUDA);
         } else {
-            if (!make_window_map(&rg.map, s.d_x4, s.x4_stride, s.x4_pitch, s.x4_stride, 4, C, rg.window_bytes)) return fail(AA_ERR_CUDA);
+            if (!make_window_maps(rg, s.d_x4, s.x4_stride, s.x4_pitch, s.x4_stride, 4, C)) return fail(AA_ERR_CUDA);
         }
         for (int32_t i = 0; i < rg.r.ndms; ++i) {
             const int32_t* base = rg.d_D + (size_t)i * (size_t)rg.pitch;
@@ -593,6 +641,16 @@ extern "C" size_t aa_strategy_describe(const aa_strategy* h, char* buf, size_t b
                  rg.dm_tile, kTTile, rg.chan_block, rg.window_bytes, rg.nstages, rg.ndm_tiles, rg.spill_stages,
                  aak_dedisperse_smem_bytes(rg.chan_block, rg.window_bytes, rg.in16, rg.ring_stages));
         o += line;
+        {
+            const K2Plan& kp = (rg.ndm_tiles > 0 || !rg.has_lo) ? static_cast<const K2Plan&>(rg) : rg.lo;
+            if (kp.nclass > 1 && !kp.wcls.empty()) {
+                double sum = 0.0;
+                for (int32_t c : kp.wcls) sum += kp.class_wb[c];
+                snprintf(line, sizeof line, "         %d window classes, %d..%d bytes, %.0f on average over the channel blocks\n", kp.nclass, kp.class_wb[0],
+                         kp.class_wb[kp.nclass - 1], sum / (double)kp.wcls.size());
+                o += line;
+            }
+        }
         if (rg.naive) o += "         tile window does not fit shared memory: one-thread-per-output kernel on a device delay table\n";
         if (rg.main_exc) o += "         the uint16 plan reads the offset-uint16 form (per-channel offsets + exceptions)\n";
         if (rg.dense_naive) o += "         exception-heavy chunks take the one-thread-per-output kernel on the plain binned samples\n";

@@ -16,6 +16,10 @@
  *     coordinate raises an illegal-instruction fault on sm_100a), so the shifted copies exist in GLOBAL memory
  *     (K1 writes them: x_k[c][t] = x[c][t+k], copy k at byte offset k*copy_stride of one buffer); the window start is
  *     aligned down to 16 bytes and the residue is folded into the host-built offset table.
+ *   * The window of a channel block is only as wide as its channels' delay spread inside a DM tile needs (window classes, one
+ *     tensor map each): with the low-frequency configuration's spreads (up to 1600 samples per tile at the bottom of the band,
+ *     none at the top) a uniform window made the L2 -> shared-memory fill (4 copies x 2816 bytes x 8 channels per 1920 clocks of
+ *     adds = 47 B/clk/SM, the chip-wide TMA rate) the limiter of K2; per-block windows cut it by a third.
  *   * ONE TMA per channel moves the windows of all copies: the tensor map views the buffer as OVERLAPPING 256-byte
  *     segments (dims {pitch, nseg, NCOPY, C}, strides {256, copy_stride, pitch}), so a {256, nseg, NCOPY, 1} box lands
  *     as NCOPY linear windows of WB bytes. A stage is therefore CB tensor copies + one bulk copy of the offset table,
@@ -55,26 +59,39 @@ constexpr int MAX_RING = 8;          /* shared-memory ring depth is a launch par
 constexpr int SMEM_HEADER = 1024;    /* mbarriers live here; keeps the stages 1024-byte aligned */
 
 
-struct DedispParams {
-    const int32_t* etab;
-    const int32_t* x0tab;
-    int32_t* D;
-    long long pitch;
-    long long nt;
-    int ndms;
-    int nstages;
-    int window_bytes;
-    int spill_stages;
-    int nring;                 /* ring depth */
-    int stage_begin, stage_end; /* channel blocks [stage_begin, stage_end) of the nstages are summed by this launch */
-    int accumulate;            /* 1: add to the values already in D (a later channel group of the same chunk) */
-    const unsigned* mode_cnt;  /* NULL, or: run only if (*mode_cnt > mode_cap) == mode_dense */
-    unsigned mode_cap;
-    int mode_dense;
+/* one tensor map per window class (boxes of 256 x nseg bytes, nseg = class_wb / 256) */
+template <int N> struct WindowMaps { CUtensorMap m[N]; };
+
+/* Kernel parameters. VW (plans with several window classes) adds the class table; plans with one class keep the parameter
+ * block of the first version of this kernel byte for byte: ptxas schedules the main loop differently when the block grows,
+ * and the schedule it picks for the original block is 0.5 % faster (measured, identical opcode mix). */
+#define AA_DEDISP_PARAMS_HEAD \
+    const int32_t* etab; \
+    const int32_t* x0tab; \
+    int32_t* D; \
+    long long pitch; \
+    long long nt; \
+    int ndms; \
+    int nstages; \
+    int window_bytes; \
+    int spill_stages; \
+    int nring;                 /* ring depth */ \
+    int stage_begin, stage_end; /* channel blocks [stage_begin, stage_end) of the nstages are summed by this launch */ \
+    int accumulate;            /* 1: add to the values already in D (a later channel group of the same chunk) */ \
+    const unsigned* mode_cnt;  /* NULL, or: run only if (*mode_cnt > mode_cap) == mode_dense */ \
+    unsigned mode_cap; \
+    int mode_dense; \
     const int* bias;           /* NULL, or a constant added to every output */
-    int skew_q16;              /* CTA order: time tile = blockIdx / ndm_tiles - (skew_q16 * dm_tile >> 16), see launch() */
-    int nt_tiles;
+#define AA_DEDISP_PARAMS_TAIL \
+    int skew_q16;              /* CTA order: time tile = blockIdx / ndm_tiles - (skew_q16 * dm_tile >> 16), see launch() */ \
+    int nt_tiles; \
     unsigned one;              /* always 1; a runtime value so that x*one+y stays an IMAD (FMA pipe) */
+template <bool VW> struct DedispParamsT { AA_DEDISP_PARAMS_HEAD AA_DEDISP_PARAMS_TAIL };
+template <> struct DedispParamsT<true> {
+    AA_DEDISP_PARAMS_HEAD
+    const int* wcls;           /* [nstages] window class of each stage */
+    int class_wb[8];           /* window bytes per class */
+    AA_DEDISP_PARAMS_TAIL
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -138,9 +155,11 @@ __device__ __forceinline__ uint32_t odd_bytes(uint32_t w) { /* (b1, 0, b3, 0) */
  * registers instead of being read from shared memory again (a warp-uniform test of two table entries). */
 /* NWC = compute warps: 16 (+1 producer = 17 warps, 96 registers per thread) or 15 (+1 = 16 warps, 128 registers per
  * thread, 30 trials per CTA: the extra registers let ptxas keep more shared-memory loads in flight). */
-template <int IN16, int CB, int FMA_H, int M, int NWC>
+/* VW: the plan has more than one window class (the producer looks the class of every channel block up); plans with ONE class
+ * keep the constant map and window of the first version of this kernel (measured: the look-up costs the byte kernel 2 %). */
+template <int IN16, int CB, int FMA_H, int M, int NWC, bool VW>
 __global__ void __launch_bounds__((NWC + 1) * 32, 1)
-k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
+k_dedisperse(const __grid_constant__ WindowMaps<VW ? 8 : 1> maps, const DedispParamsT<VW> p) {
     constexpr int ESZ = IN16 ? 2 : 1;
     constexpr int SPW = 4 / ESZ;                 /* samples per word */
     constexpr int NCOPY = SPW;                   /* shifted copies */
@@ -193,17 +212,34 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
                 int x0[CB];
 #pragma unroll
                 for (int c = 0; c < CB; ++c) x0[c] = __ldg(x0row + s * CB + c);
-                mbar_wait<PRODUCER_SLEEP_NS>(bar_empty + 8 * slot, ph ^ 1u);
-                const uint32_t fb = bar_full + 8 * slot;
-                mbar_arrive_expect_tx(fb, (uint32_t)stage_bytes);
-                const uint32_t sbase = smem_u32(stages + (size_t)slot * stage_bytes);
+                if constexpr (VW) {
+                    const int cls = __ldg(p.wcls + s);
+                    const int WBs = p.class_wb[cls];                         /* this channel block's window (<= WB) */
+                    const CUtensorMap* map = &maps.m[cls];
+                    mbar_wait<PRODUCER_SLEEP_NS>(bar_empty + 8 * slot, ph ^ 1u);
+                    const uint32_t fb = bar_full + 8 * slot;
+                    mbar_arrive_expect_tx(fb, (uint32_t)(NCOPY * CB * WBs + ENT_BYTES));
+                    const uint32_t sbase = smem_u32(stages + (size_t)slot * stage_bytes);
 #pragma unroll
-                for (int c = 0; c < CB; ++c) {
-                    const long long xs = tb + x0[c];                         /* 16-byte aligned byte coordinate of the window */
-                    const int xi = xs > 0x7fff0000ll ? 0x7fff0000 : (int)xs;   /* far out of bounds is zero-filled anyway */
-                    tma_load_4d(sbase + (uint32_t)(c * NCOPY * WB), &map, xi, 0, 0, s * CB + c, fb);
+                    for (int c = 0; c < CB; ++c) {
+                        const long long xs = tb + x0[c];                     /* 16-byte aligned byte coordinate of the window */
+                        const int xi = xs > 0x7fff0000ll ? 0x7fff0000 : (int)xs;   /* far out of bounds is zero-filled anyway */
+                        tma_load_4d(sbase + (uint32_t)(c * NCOPY * WBs), map, xi, 0, 0, s * CB + c, fb);
+                    }
+                    bulk_load_1d(sbase + data_bytes, erow + (size_t)s * (CB * DM_TILE), ENT_BYTES, fb);
+                } else {
+                    mbar_wait<PRODUCER_SLEEP_NS>(bar_empty + 8 * slot, ph ^ 1u);
+                    const uint32_t fb = bar_full + 8 * slot;
+                    mbar_arrive_expect_tx(fb, (uint32_t)stage_bytes);
+                    const uint32_t sbase = smem_u32(stages + (size_t)slot * stage_bytes);
+#pragma unroll
+                    for (int c = 0; c < CB; ++c) {
+                        const long long xs = tb + x0[c];                     /* 16-byte aligned byte coordinate of the window */
+                        const int xi = xs > 0x7fff0000ll ? 0x7fff0000 : (int)xs;   /* far out of bounds is zero-filled anyway */
+                        tma_load_4d(sbase + (uint32_t)(c * NCOPY * WB), &maps.m[0], xi, 0, 0, s * CB + c, fb);
+                    }
+                    bulk_load_1d(sbase + data_bytes, erow + (size_t)s * (CB * DM_TILE), ENT_BYTES, fb);
                 }
-                bulk_load_1d(sbase + data_bytes, erow + (size_t)s * (CB * DM_TILE), ENT_BYTES, fb);
                 if (++slot == NSTAGE) { slot = 0; ph ^= 1u; }
             }
         }
@@ -341,8 +377,9 @@ k_dedisperse(const __grid_constant__ CUtensorMap map, const DedispParams p) {
                 *reinterpret_cast<int4*>(row + t) = v;
             } else {
                 int2 v;
-                v.x = bias + (int)((A[m][j] & 0xFFFFu) + ((C1[m][j] & 0xFFFFu) << 8));
-                v.y = bias + (int)((A[m][j] >> 16) + ((C1[m][j] >> 16) << 8));
+                v.x = (int)((A[m][j] & 0xFFFFu) + ((C1[m][j] & 0xFFFFu) << 8));
+                v.y = (int)((A[m][j] >> 16) + ((C1[m][j] >> 16) << 8));
+                if (FMA_H) { v.x += bias; v.y += bias; }         /* uint16 kernels: FMA_H = 1 marks the offset-uint16 form (16-bit plans) */
                 if (p.accumulate) {
                     const int2 o = *reinterpret_cast<const int2*>(row + t);
                     v.x += o.x; v.y += o.y;
@@ -369,10 +406,10 @@ __global__ void k_dedisperse_naive(const T* __restrict__ x, size_t pitch, const 
     D[(size_t)i * dpitch + t] = acc;
 }
 
-template <int IN16, int CB, int FMA_H, int M, int NWC>
-int launch(const aak_dedisp_args* a, cudaStream_t st) {
+template <int IN16, int CB, int FMA_H, int M, int NWC, bool VW>
+int launch_vw(const aak_dedisp_args* a, cudaStream_t st) {
     constexpr int NCOPY = IN16 ? 2 : 4;
-    DedispParams p;
+    DedispParamsT<VW> p;
     p.etab = a->etab; p.x0tab = a->x0tab; p.D = a->D; p.pitch = a->pitch; p.nt = a->nt; p.ndms = a->ndms;
     p.nstages = (a->nchans + CB - 1) / CB;
     /* channel group [chan_begin, chan_end): whole channel blocks (chan_end == 0 means all channels) */
@@ -381,6 +418,11 @@ int launch(const aak_dedisp_args* a, cudaStream_t st) {
     p.stage_begin = a->chan_begin / CB; p.stage_end = (cend + CB - 1) / CB; p.accumulate = a->accumulate;
     p.mode_cnt = a->mode_cnt; p.mode_cap = a->mode_cap; p.mode_dense = a->mode_dense; p.bias = a->bias;
     p.window_bytes = a->window_bytes; p.spill_stages = a->spill_stages; p.one = 1u;
+    if (a->nclass < 1 || a->nclass > 8 || !a->wcls) return (int)cudaErrorInvalidValue;
+    if constexpr (VW) {
+        p.wcls = a->wcls;
+        for (int k = 0; k < 8; ++k) p.class_wb[k] = k < a->nclass ? a->class_wb[k] : 0;
+    }
     p.nring = a->ring_stages;
     if (p.nring < 2 || p.nring > MAX_RING) return (int)cudaErrorInvalidValue;
     const size_t smem = SMEM_HEADER + (size_t)p.nring * ((size_t)NCOPY * CB * a->window_bytes + CB * DM_TILE * 4);
@@ -392,15 +434,23 @@ int launch(const aak_dedisp_args* a, cudaStream_t st) {
     const long long extra_rows = ((long long)p.skew_q16 * (ndm_tiles - 1)) >> 16;     /* diagonals that start before time tile 0 */
     const long long grid = ndm_tiles * (nt_tiles + extra_rows);
     if (grid <= 0 || grid > 0x7fffffffll) return (int)cudaErrorInvalidConfiguration;
-    CUtensorMap map;
-    memcpy(&map, a->tmap, sizeof(CUtensorMap));
-    k_dedisperse<IN16, CB, FMA_H, M, NWC><<<(unsigned)grid, (NWC + 1) * 32, smem, st>>>(map, p);
+    WindowMaps<VW ? 8 : 1> maps;
+    memset(&maps, 0, sizeof maps);
+    memcpy(maps.m, a->tmap, sizeof(CUtensorMap) * (size_t)(VW ? a->nclass : 1));
+    k_dedisperse<IN16, CB, FMA_H, M, NWC, VW><<<(unsigned)grid, (NWC + 1) * 32, smem, st>>>(maps, p);
     return (int)cudaGetLastError();
 }
 
 template <int IN16, int CB, int FMA_H, int M, int NWC>
+int launch(const aak_dedisp_args* a, cudaStream_t st) {
+    return a->nclass > 1 ? launch_vw<IN16, CB, FMA_H, M, NWC, true>(a, st) : launch_vw<IN16, CB, FMA_H, M, NWC, false>(a, st);
+}
+
+template <int IN16, int CB, int FMA_H, int M, int NWC>
 int set_attr() {
-    return (int)cudaFuncSetAttribute(k_dedisperse<IN16, CB, FMA_H, M, NWC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    int e = (int)cudaFuncSetAttribute(k_dedisperse<IN16, CB, FMA_H, M, NWC, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e) return e;
+    return (int)cudaFuncSetAttribute(k_dedisperse<IN16, CB, FMA_H, M, NWC, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
 }
 
 }  // namespace
@@ -412,10 +462,13 @@ extern "C" size_t aak_dedisperse_smem_bytes(int32_t chan_block, int32_t window_b
 
 /* The instantiations the strategy can select (aa_strategy.cpp plan_format): bytes (uint8 input and the offset-uint8 form) =
  * 15 compute warps x 2 trials, odd-byte adds on the FMA pipe; binned uint16 = 16 compute warps x 4 adjacent trials with
- * equal-delay reuse; channel block 8, 4 or 2 by window size. The variants measured and rejected are in profiles/r01c_profiles.md. */
+ * equal-delay reuse (third parameter 1: the offset-uint16 form of a 16-bit plan, which adds the sum of the channel offsets -
+ * kept apart because the plain uint16 kernel, at 96 registers with spills, loses 8 % to any change of its epilogue);
+ * channel block 8, 4 or 2 by window size. The variants measured and rejected are in profiles/r01c_profiles.md. */
 #define AA_FOR_ALL_VARIANTS(X) \
     X(0, 8, 1, 2, 15) X(0, 4, 1, 2, 15) X(0, 2, 1, 2, 15) \
-    X(1, 8, 0, 4, 16) X(1, 4, 0, 4, 16) X(1, 2, 0, 4, 16)
+    X(1, 8, 0, 4, 16) X(1, 4, 0, 4, 16) X(1, 2, 0, 4, 16) \
+    X(1, 8, 1, 4, 16) X(1, 4, 1, 4, 16) X(1, 2, 1, 4, 16)
 
 extern "C" int aak_dedisperse_init(void) {
     int e = 0;
@@ -428,7 +481,7 @@ extern "C" int aak_dedisperse_init(void) {
 /* variant (uint8 only): 0 = odd-byte adds as IADD3, 1 = as IMAD (FMA pipe), 2 = alternating; dms_per_warp in {2, 4} */
 extern "C" int aak_dedisperse(const aak_dedisp_args* a, void* stream) {
     cudaStream_t st = (cudaStream_t)stream;
-    const int fma = a->in16 ? 0 : (a->dms_per_warp == 4 ? (a->variant & 1) : a->variant);
+    const int fma = a->in16 ? (a->bias ? 1 : 0) : (a->dms_per_warp == 4 ? (a->variant & 1) : a->variant);
     const int mm = a->dms_per_warp == 4 ? 4 : 2;
     const int nwc = a->dm_tile / 2;
 #define X(I, C, F, MM, W) if (a->in16 == I && a->chan_block == C && fma == F && mm == MM && nwc == W) return launch<I, C, F, MM, W>(a, st);
