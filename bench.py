@@ -32,8 +32,18 @@ if str(ROOT) not in sys.path:
 METRIC = "dm_trial_samples_per_s"
 UNIT = "DM-trial*samples/s"
 SM_COUNT = 148
-# ncu, profiles/r01f_dram_per_launch.csv: bytes read + written by the K2 launches (k_dedisperse + k_scatter_exceptions) of one SKA-like step
-K2_DRAM_BYTES_PER_STEP = {"ska": 38461107200 + 6906948352}
+
+
+def k2_dram_traffic(workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the K2 launches of one step, from the tracked ncu capture
+    profiles/k2_dram_traffic.json (which names the commit and the command it was captured with); None if the workload has none."""
+    f = ROOT / "profiles" / "k2_dram_traffic.json"
+    if not f.exists():
+        return None, None
+    rec = json.loads(f.read_text())
+    e = rec.get("workloads", {}).get(workload)
+    return (e["bytes_per_step"], f"profiles/k2_dram_traffic.json (commit {rec.get('commit')}, {e.get('launches')} launches)") if e else (None, None)
+
 INT_LANES_PER_SM_CLK = 128      # 64 ALU-pipe (IADD3) + 64 FMA-pipe (IMAD) lanes per SM per clock, DESIGN.md "Roofline"
 
 
@@ -274,9 +284,9 @@ def run_ours(args, w):
         if (ROOT / "MEASURED_PEAKS.json").exists() else (in_bytes + 4 * outputs) / 6.65e12
     roofline = {"bound": "alu", "kernel": "k_dedisperse + k_scatter_exceptions (K2), the launches of all DM ranges of one step",
                 "achieved": adds / k2 / 1e12, "peak": peak / 1e12, "unit": "Tadd/s (algorithmic 32-bit integer adds)",
-                "frac": adds / k2 / peak, "traffic": K2_DRAM_BYTES_PER_STEP.get(w.name),
-                "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of the K2 launches of one step (9 launches on ska), one "
-                                "ncu capture: profiles/r01f_dram_per_launch.csv; compulsory bytes are input once + D once",
+                "frac": adds / k2 / peak, "traffic": k2_dram_traffic(w.name)[0],
+                "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of the K2 launches of one step, one ncu capture: "
+                                + str(k2_dram_traffic(w.name)[1]) + "; compulsory bytes are input once + D once",
                 "peak_how": f"derived: {SM_COUNT} SMs x {INT_LANES_PER_SM_CLK} integer-add lanes/clk (64 IADD3 + 64 IMAD) x max SM clock",
                 "measured_iadd3_only_tadd_s": iadd3 / 1e12, "measured_iadd3_imad_mixed_tadd_s": mixed / 1e12, "measured_imad_only_tadd_s": imad / 1e12,
                 "frac_of_measured_mixed": adds / k2 / max(mixed, iadd3), "frac_of_measured_iadd3_only": adds / k2 / iadd3,
@@ -298,7 +308,7 @@ def run_ours(args, w):
             "candidates_per_step": ncand, "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline}
     if not args.no_cpu_baseline and world == 1:
-        rows = 2 if w.nchans * w.nsamp > (1 << 28) else 3
+        rows = 3                              # first, middle and last DM row of every range
         o, secs, spent, what = oracle_sample(w, x, info["n_out"], rows)
         line["cpu_baseline"] = {"value": o / secs, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what,
                                 "sample_seconds": spent, "host_cores_available": os.cpu_count()}

@@ -91,6 +91,9 @@ struct Range : K2Plan {           /* the base is the range's main plan: uint8 fo
     bool has_lo = false;          /* the offset-uint8 route (k_misc.cu "Offset-uint8 form") with its own tiling: bin 2 / 4 of an 8-bit
                                      plan, bin 1 / 2 / 4 of a 16-bit plan */
     K2Plan lo;
+    bool half = false;            /* 8-bit plan, bin 8: the offset-uint8 plan reads the HALF-BYTE form (k_bits.cu): sums are doubled and
+                                     the dropped low bits are dedispersed as a bit plane */
+    int32_t bits_ww = 0;          /* window words of the bit-plane kernel */
     bool main_exc = false;        /* 16-bit plan, bin 8: the main (uint16) plan reads the offset-uint16 form (offsets + exceptions) */
     bool dense_naive = false;     /* 16-bit plan: exception-heavy chunks take the global-memory kernel on the plain binned samples */
 };
@@ -135,6 +138,8 @@ struct Strategy {
     uint2* d_exc[9] = {nullptr};             /* [kMaxGroups][exc_cap] */
     unsigned* d_exc_cnt[9] = {nullptr};      /* [kMaxGroups] exception counters, then [kMaxGroups] int32 biases (one memset clears both) */
     unsigned exc_limit[9] = {0};             /* a group with more exceptions than this takes the uint16 route */
+    uint32_t* d_bits[9] = {nullptr};         /* bit plane of the half-byte form (bin 8): [nchans][bits_pitch] words */
+    size_t bits_pitch[9] = {0};
     double* d_k = nullptr;                   /* delay constants on the device (exception scatter) */
     bool d_k_needed = false;
     aak_row_desc* d_rows[2] = {nullptr, nullptr};   /* [0] full chunk geometry, [1] last (short) chunk */

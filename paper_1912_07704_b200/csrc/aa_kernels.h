@@ -33,8 +33,8 @@ int aak_shift_copy(const uint8_t* in, uint8_t* out, size_t pitch, size_t row_byt
  * {c + chan0 | (r + 1024) << 16, t'} at exc[atomicAdd(exc_cnt)] while below cap (the counter keeps counting).
  * aak_scatter_exceptions: D[i][t' - delay(c, i)] += r for every exception and every trial of one range; returns at once
  * if *exc_cnt > cap. k = the plan's delay constants (device doubles). */
-int aak_chan_offsets(const uint8_t* x, size_t pitch, int64_t len, int32_t nrows, int32_t* off2, int32_t* off4, int32_t* bias2,
-                     int32_t* bias4, void* stream);
+int aak_chan_offsets(const uint8_t* x, size_t pitch, int64_t len, int32_t nrows, int32_t* off2, int32_t* off4, int32_t* off8, int32_t* bias2,
+                     int32_t* bias4, int32_t* bias8, void* stream);
 int aak_scatter_exceptions(const uint2* exc, const unsigned* exc_cnt, unsigned cap, const double* k, double dm_low, double dm_step,
                            int32_t ndms, int32_t bin, int64_t nt, int32_t* D, int64_t pitch, void* stream);
 
@@ -48,6 +48,12 @@ typedef struct {
     uint8_t* lo2; size_t lo2_pitch, lo2_stride; const int32_t* off2; uint2* exc2; unsigned* cnt2; int64_t nb2;
     uint8_t* lo4; size_t lo4_pitch, lo4_stride; const int32_t* off4; uint2* exc4; unsigned* cnt4; int64_t nb4;
     uint16_t* xb8; size_t xb8_pitch, xb8_stride;
+    /* half-byte form of bin 8 (NULL: not used): x_8 = 2 y + bit + off8[c] + r with y a byte (4 shifted copies in hb8), bit the
+     * dropped low bit (bits8: one bit per sample, rows of bits8_pitch 32-bit words) and r an exception list; off8[c] =
+     * clamp(round(8 mean) - 256, 0, ..) from aak_chan_offsets. K2 sums y with its byte path and doubles the sums,
+     * aak_dedisperse_bits adds the dedispersed bit plane, aak_scatter_exceptions the r. */
+    uint8_t* hb8; size_t hb8_pitch, hb8_stride; const int32_t* off8; uint2* exc8; unsigned* cnt8; int64_t nb8;
+    uint32_t* bits8; size_t bits8_pitch;
 } aak_prep_args;
 int aak_prep_fused(const aak_prep_args* a, int32_t nrows, void* stream);
 
@@ -115,6 +121,17 @@ typedef struct {
 int aak_dedisperse(const aak_dedisp_args* a, void* stream);
 size_t aak_dedisperse_smem_bytes(int32_t chan_block, int32_t window_bytes, int32_t in16, int32_t ring_stages);
 int aak_dedisperse_init(void);   /* sets the dynamic shared-memory attribute of every instantiation */
+
+/* ---- K2b: dedispersion of a BIT plane (the low bits the half-byte form of bin 8 drops):
+ *   D[i][t] += sum_{c in [chan_begin, chan_end)} bit[c][t + delay(c, i)]
+ * bits [nchans][pitch_words] uint32 (bit k of word w = sample 32 w + k; readable up to (nt + max delay) / 32 + window_words + 2
+ * words per row), delays [ndms][nchans] int32 (binned samples), window_words = 34 + ceil(largest delay spread inside a tile of
+ * 32 trials / 32) <= 256. A CTA owns 32 trials x 1024 samples; channel blocks go through shared memory, every thread extracts its 32
+ * samples of a channel with one funnel shift and adds them to bit-sliced (vertical) counters with carry-save adders: about
+ * 0.3 instructions per add. Runs only if *mode_cnt <= mode_cap (NULL: always). */
+int aak_dedisperse_bits(const uint32_t* bits, size_t pitch_words, const int32_t* delays, int32_t nchans, int32_t chan_begin, int32_t chan_end,
+                        int32_t ndms, int64_t nt, int32_t window_words, int32_t* D, int64_t pitch, const unsigned* mode_cnt, unsigned mode_cap,
+                        void* stream);
 
 /* One thread per output, global loads (copy 0 of the input, pitch in elements): the route for ranges whose channel window
  * does not fit shared memory, and a cross-check. delays [ndms][nchans] int32; sums channels [chan_begin, chan_end),

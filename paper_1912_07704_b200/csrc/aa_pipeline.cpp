@@ -109,10 +109,12 @@ aa_status enqueue_prep(Strategy& s, const Chunk& c, int b, int32_t c0, int32_t c
     if (s.plan.input_bits == 16) return enqueue_prep16(s, c, b, c0, c1, g);
     const int32_t n = c1 - c0;
     const uint8_t* raw = s.d_raw[b] + (size_t)c0 * s.in_pitch;
-    if (s.d_lo[2] || s.d_lo[4])
+    if (s.d_lo[2] || s.d_lo[4] || s.d_lo[8])
         AA_LAUNCH(aak_chan_offsets(raw, s.in_pitch, (int64_t)c.len, n, s.d_lo[2] ? s.d_off[2] + c0 : nullptr, s.d_lo[4] ? s.d_off[4] + c0 : nullptr,
+                                   s.d_lo[8] ? s.d_off[8] + c0 : nullptr,
                                    s.d_lo[2] ? (int32_t*)(s.d_exc_cnt[2] + kMaxGroups + g) : nullptr,
-                                   s.d_lo[4] ? (int32_t*)(s.d_exc_cnt[4] + kMaxGroups + g) : nullptr, s.compute), "channel offsets");
+                                   s.d_lo[4] ? (int32_t*)(s.d_exc_cnt[4] + kMaxGroups + g) : nullptr,
+                                   s.d_lo[8] ? (int32_t*)(s.d_exc_cnt[8] + kMaxGroups + g) : nullptr, s.compute), "channel offsets");
     /* one read of the raw rows writes every input form K2 may read, except the uint16 forms of bin 2 / 4 */
     aak_prep_args a;
     memset(&a, 0, sizeof a);
@@ -126,9 +128,14 @@ aa_status enqueue_prep(Strategy& s, const Chunk& c, int b, int32_t c0, int32_t c
         a.lo4 = s.d_lo[4] + (size_t)c0 * s.lo_pitch[4]; a.lo4_pitch = s.lo_pitch[4]; a.lo4_stride = s.lo_stride[4]; a.off4 = s.d_off[4] + c0;
         a.exc4 = s.d_exc[4] + (size_t)g * kExcCap; a.cnt4 = s.d_exc_cnt[4] + g; a.nb4 = (int64_t)(c.len / 4);
     }
-    if (s.d_xb[8]) { a.xb8 = s.d_xb[8] + (size_t)c0 * s.xb_pitch[8]; a.xb8_pitch = s.xb_pitch[8]; a.xb8_stride = s.xb_stride[8]; }
+    if (s.d_lo[8]) {                                 /* the half-byte form and its bit plane; the uint16 form only for exception-heavy chunks */
+        a.hb8 = s.d_lo[8] + (size_t)c0 * s.lo_pitch[8]; a.hb8_pitch = s.lo_pitch[8]; a.hb8_stride = s.lo_stride[8]; a.off8 = s.d_off[8] + c0;
+        a.exc8 = s.d_exc[8] + (size_t)g * kExcCap; a.cnt8 = s.d_exc_cnt[8] + g; a.nb8 = (int64_t)(c.len / 8);
+        a.bits8 = s.d_bits[8] + (size_t)c0 * s.bits_pitch[8]; a.bits8_pitch = s.bits_pitch[8];
+    } else if (s.d_xb[8]) { a.xb8 = s.d_xb[8] + (size_t)c0 * s.xb_pitch[8]; a.xb8_pitch = s.xb_pitch[8]; a.xb8_stride = s.xb_stride[8]; }
     AA_LAUNCH(aak_prep_fused(&a, n, s.compute), "input forms (fused)");
-    for (int bin = 2; bin <= 4; bin *= 2) {
+    for (int bin = 2; bin <= 8; bin *= 2) {
+        if (bin == 8 && !s.d_lo[8]) continue;         /* bin 8 without the half-byte route: the fused kernel wrote its uint16 form */
         if (!s.d_xb[bin]) continue;
         const unsigned* cnt = s.d_lo[bin] ? s.d_exc_cnt[bin] + g : nullptr;      /* NULL: the range has no offset-uint8 route */
         const unsigned lim = cnt ? group_limit(s, bin, c0, c1) : 0u;
@@ -187,6 +194,9 @@ aa_status enqueue_k2(Strategy& s, const Chunk& c, int32_t c0, int32_t c1, bool a
             a.bias = route_sparse ? (const int32_t*)(s.d_exc_cnt[bin] + kMaxGroups + g) : nullptr;
             AA_LAUNCH(aak_dedisperse(&a, st), "dedispersion");
         }
+        if (rg.half)                                  /* the low bits the half-byte form dropped */
+            AA_LAUNCH(aak_dedisperse_bits(s.d_bits[bin], s.bits_pitch[bin], rg.d_delays, s.plan.nchans, c0, c1, rg.r.ndms, a.nt, rg.bits_ww, rg.d_D,
+                                          rg.pitch, cnt, lim, st), "bit-plane dedispersion");
         if (sparse)
             AA_LAUNCH(aak_scatter_exceptions(s.d_exc[bin] + (size_t)g * kExcCap, s.d_exc_cnt[bin] + g, lim, s.d_k, rg.r.dm_low, rg.r.dm_step,
                                              rg.r.ndms, bin, a.nt, rg.d_D, rg.pitch, st), "exception scatter");

@@ -119,6 +119,10 @@ static void carve(Strategy& s, int64_t L, bool two_stage) {
         (void)nd;
         s.exc_limit[b] = sparse ? (unsigned)std::min<double>((double)kMaxGroups * kExcCap, std::max(1.0, 4.0e-4 * (double)s.plan.nchans * (double)(L / b))) : 0;
         if (sparse && !s.d_k_needed) s.d_k_needed = true;
+        bool half = false;
+        for (const Range& rg : s.ranges) half = half || (rg.r.bin == b && rg.half);
+        s.bits_pitch[b] = half ? round_up(P / 32 + 1024 + 64, 64) : 0;        /* + the widest window the bit-plane kernel may read */
+        s.d_bits[b] = half ? (uint32_t*)a.take((size_t)s.plan.nchans * s.bits_pitch[b] * 4) : nullptr;
     }
     s.d_k = s.d_k_needed ? (double*)a.take((size_t)s.plan.nchans * 8) : nullptr;
     const int64_t n_out = L - s.S;
@@ -126,7 +130,7 @@ static void carve(Strategy& s, int64_t L, bool two_stage) {
         rg.nt_full = n_out / rg.r.bin;
         rg.pitch = (int64_t)round_up((size_t)(rg.nt_full + rg.extra), 128);
         rg.d_D = (int32_t*)a.take((size_t)rg.r.ndms * (size_t)rg.pitch * 4);
-        rg.d_delays = (rg.naive || rg.dense_naive) ? (int32_t*)a.take((size_t)rg.r.ndms * s.plan.nchans * 4) : nullptr;
+        rg.d_delays = (rg.naive || rg.dense_naive || rg.half) ? (int32_t*)a.take((size_t)rg.r.ndms * s.plan.nchans * 4) : nullptr;
         rg.d_etab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * kDmTile * 4);   /* rg. = the main plan */
         rg.d_x0tab = (int32_t*)a.take((size_t)rg.ndm_tiles * rg.nstages * rg.chan_block * 4);
         rg.d_wcls = (int32_t*)a.take((size_t)rg.nstages * 4);
@@ -296,7 +300,7 @@ static bool plan_range(Strategy& s, Range& rg, std::vector<int32_t>& etab, std::
         rg.dm_tile = kDmTile; rg.ndm_tiles = 0; rg.nstages = 0; rg.chan_block = 8; rg.window_bytes = 0;
         etab.clear(); x0tab.clear();
     };
-    rg.naive = false; rg.has_lo = false; rg.main_exc = false; rg.dense_naive = false;
+    rg.naive = false; rg.has_lo = false; rg.main_exc = false; rg.dense_naive = false; rg.half = false;
     if (s.plan.input_bits == 16) {
         /* 16-bit samples (k_input16.cu): bin 1 / 2 / 4 ride the byte path on the offset-uint8 form, bin 8 the uint16 path on the
          * offset-uint16 form; a chunk with too many exceptions, or a range whose window does not fit, takes the global-memory
@@ -321,8 +325,20 @@ static bool plan_range(Strategy& s, Range& rg, std::vector<int32_t>& etab, std::
     }
     /* bin 2 and 4 also get the offset-uint8 route (half the shared-memory bytes per add); the uint16 plan above stays as
      * the route for chunks with too many exceptions. */
-    rg.has_lo = (rg.r.bin == 2 || rg.r.bin == 4);
+    rg.has_lo = (rg.r.bin == 2 || rg.r.bin == 4 || rg.r.bin == 8);
     if (rg.has_lo && !plan_format(s, rg, rg.lo, 0, 256, etab_lo, x0tab_lo)) rg.has_lo = false;
+    if (rg.has_lo && rg.r.bin == 8) {
+        /* bin 8: the byte plan reads the half-byte form, its low bits go through the bit-plane kernel (k_bits.cu): tiles of 32
+         * trials, window = 34 words + the largest delay spread inside such a tile */
+        int64_t sp = 0;
+        for (int32_t i0 = 0; i0 < nd; i0 += 32) {
+            const int32_t i1 = std::min(nd - 1, i0 + 31);
+            for (int32_t c = 0; c < C; ++c) sp = std::max<int64_t>(sp, (int64_t)rg.delays[(size_t)i1 * C + c] - rg.delays[(size_t)i0 * C + c]);
+        }
+        rg.bits_ww = (int32_t)(34 + (sp + 31) / 32);
+        if (rg.bits_ww > 256) rg.has_lo = false;
+        else { rg.half = true; rg.lo.variant = 3; }
+    }
     return true;
 }
 
@@ -370,6 +386,7 @@ static aa_status plan_host(aa_strategy* h, const aa_plan* plan, uint64_t nsamp_t
      * then read a uint16 buffer that a sparse chunk never filled. So a bin keeps the route only if all its ranges have it. */
     for (const Range& nl : s.ranges)
         if (!nl.has_lo) for (Range& rg : s.ranges) if (rg.r.bin == nl.r.bin) rg.has_lo = false;
+    for (Range& rg : s.ranges) if (!rg.has_lo) rg.half = false;
     /* 16-bit plans: a bin's rows hold EITHER its offset form (with the plain samples written only for exception-heavy chunks) OR,
      * if one of its ranges has only the global-memory route, the plain samples always: then every range of the bin takes it */
     if (s.plan.input_bits == 16)
@@ -517,7 +534,7 @@ extern "C" aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, u
     const Chunk& last = s.chunks.back();
     for (size_t r = 0; r < s.ranges.size(); ++r) {
         Range& rg = s.ranges[r];
-        if ((rg.naive || rg.dense_naive) && (e = cudaMemcpyAsync(rg.d_delays, rg.delays.data(), rg.delays.size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "delay table upload"));
+        if ((rg.naive || rg.dense_naive || rg.half) && (e = cudaMemcpyAsync(rg.d_delays, rg.delays.data(), rg.delays.size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "delay table upload"));
         if (rg.naive) { for (int32_t i = 0; i < rg.r.ndms; ++i) { const int32_t* base = rg.d_D + (size_t)i * (size_t)rg.pitch; rows_full[rg.first_row + i] = aak_row_desc{base, rg.nt_full}; rows_last[rg.first_row + i] = aak_row_desc{base, (int64_t)(last.n_out / (uint64_t)rg.r.bin)}; } continue; }
         const bool has_main = rg.ndm_tiles > 0;
         if (has_main && (e = cudaMemcpyAsync(rg.d_etab, etabs[r].data(), etabs[r].size() * 4, cudaMemcpyHostToDevice, s.compute)) != cudaSuccess) return fail(cuda_fail(e, "table upload"));
@@ -652,6 +669,7 @@ extern "C" size_t aa_strategy_describe(const aa_strategy* h, char* buf, size_t b
             }
         }
         if (rg.naive) o += "         tile window does not fit shared memory: one-thread-per-output kernel on a device delay table\n";
+        if (rg.half) o += "         the offset-uint8 route reads the half-byte form; the dropped low bits are dedispersed as a bit plane\n";
         if (rg.main_exc) o += "         the uint16 plan reads the offset-uint16 form (per-channel offsets + exceptions)\n";
         if (rg.dense_naive) o += "         exception-heavy chunks take the one-thread-per-output kernel on the plain binned samples\n";
         if (rg.has_lo) {

@@ -282,7 +282,7 @@ k_dedisperse(const __grid_constant__ WindowMaps<VW ? 8 : 1> maps, const DedispPa
                         const uint32_t w2 = *reinterpret_cast<const uint32_t*>(a2 + j * 128);
                         A[m][j] = A[m][j] + w1 + w2;
                         if (!IN16) {
-                            if (FMA_H == 1 || (FMA_H == 2 && (j & 1))) {
+                            if ((FMA_H & 1) || (FMA_H == 2 && (j & 1))) {
                                 H[m][j] = add_fma_pipe(odd_bytes(w1), one, H[m][j]);
                                 H[m][j] = add_fma_pipe(odd_bytes(w2), one, H[m][j]);
                             } else {
@@ -317,7 +317,7 @@ k_dedisperse(const __grid_constant__ WindowMaps<VW ? 8 : 1> maps, const DedispPa
                     for (int j = 0; j < J; ++j) {
                         A[m][j] = A[m][j] + w1[j] + w2[j];
                         if (!IN16) {
-                            if (FMA_H == 1 || (FMA_H == 2 && (j & 1))) {
+                            if ((FMA_H & 1) || (FMA_H == 2 && (j & 1))) {
                                 H[m][j] = add_fma_pipe(odd_bytes(w1[j]), one, H[m][j]);
                                 H[m][j] = add_fma_pipe(odd_bytes(w2[j]), one, H[m][j]);
                             } else {
@@ -366,10 +366,11 @@ k_dedisperse(const __grid_constant__ WindowMaps<VW ? 8 : 1> maps, const DedispPa
             if (!IN16) {
                 const uint32_t L = A[m][j] - (H[m][j] << 8);
                 int4 v;
-                v.x = bias + (int)((L & 0xFFFFu) + ((C1[m][j] & 0xFFFFu) << 8));
-                v.y = bias + (int)((H[m][j] & 0xFFFFu) + ((C2[m][j] & 0xFFFFu) << 8));
-                v.z = bias + (int)((L >> 16) + ((C1[m][j] >> 16) << 8));
-                v.w = bias + (int)((H[m][j] >> 16) + ((C2[m][j] >> 16) << 8));
+                constexpr int SH = (FMA_H == 3) ? 1 : 0;             /* half-byte form of bin 8: the sums of y count twice */
+                v.x = bias + (int)(((L & 0xFFFFu) + ((C1[m][j] & 0xFFFFu) << 8)) << SH);
+                v.y = bias + (int)(((H[m][j] & 0xFFFFu) + ((C2[m][j] & 0xFFFFu) << 8)) << SH);
+                v.z = bias + (int)(((L >> 16) + ((C1[m][j] >> 16) << 8)) << SH);
+                v.w = bias + (int)(((H[m][j] >> 16) + ((C2[m][j] >> 16) << 8)) << SH);
                 if (p.accumulate) {
                     const int4 o = *reinterpret_cast<const int4*>(row + t);
                     v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w;
@@ -467,6 +468,7 @@ extern "C" size_t aak_dedisperse_smem_bytes(int32_t chan_block, int32_t window_b
  * channel block 8, 4 or 2 by window size. The variants measured and rejected are in profiles/r01c_profiles.md. */
 #define AA_FOR_ALL_VARIANTS(X) \
     X(0, 8, 1, 2, 15) X(0, 4, 1, 2, 15) X(0, 2, 1, 2, 15) \
+    X(0, 8, 3, 2, 15) X(0, 4, 3, 2, 15) X(0, 2, 3, 2, 15) \
     X(1, 8, 0, 4, 16) X(1, 4, 0, 4, 16) X(1, 2, 0, 4, 16) \
     X(1, 8, 1, 4, 16) X(1, 4, 1, 4, 16) X(1, 2, 1, 4, 16)
 

@@ -126,7 +126,7 @@ k_corner_turn(const uint8_t* __restrict__ in, size_t in_stride, uint8_t* __restr
  * counter and returns at once when it is not its turn). */
 __global__ void __launch_bounds__(256)
 k_chan_offsets(const uint8_t* __restrict__ x, size_t pitch, long long len, int32_t* __restrict__ off2, int32_t* __restrict__ off4,
-               int32_t* __restrict__ bias2, int32_t* __restrict__ bias4) {
+               int32_t* __restrict__ off8, int32_t* __restrict__ bias2, int32_t* __restrict__ bias4, int32_t* __restrict__ bias8) {
     __shared__ unsigned long long red[8];
     const uint8_t* row = x + (size_t)blockIdx.x * pitch;
     unsigned long long s = 0;
@@ -147,6 +147,8 @@ k_chan_offsets(const uint8_t* __restrict__ x, size_t pitch, long long len, int32
         /* any offset is CORRECT; this one centres the channel's noise on 128 */
         if (off2) { long long o = (long long)((2 * tot + n / 2) / n) - 128; o = o < 0 ? 0 : (o > 255 ? 255 : o); off2[blockIdx.x] = (int32_t)o; atomicAdd(bias2, (int32_t)o); }
         if (off4) { long long o = (long long)((4 * tot + n / 2) / n) - 128; o = o < 0 ? 0 : (o > 765 ? 765 : o); off4[blockIdx.x] = (int32_t)o; atomicAdd(bias4, (int32_t)o); }
+        /* bin 8, half-byte form: (x_8 - off) >> 1 is centred on 128 */
+        if (off8) { long long o = (long long)((8 * tot + n / 2) / n) - 256; o = o < 0 ? 0 : (o > 1785 ? 1785 : o); off8[blockIdx.x] = (int32_t)o; atomicAdd(bias8, (int32_t)o); }
     }
 }
 
@@ -181,7 +183,16 @@ struct PrepFused {
     uint8_t* lo2; size_t lo2_pitch, lo2_stride; const int32_t* off2; uint2* exc2; unsigned* cnt2; long long nb2;
     uint8_t* lo4; size_t lo4_pitch, lo4_stride; const int32_t* off4; uint2* exc4; unsigned* cnt4; long long nb4;
     uint16_t* xb8; size_t xb8_pitch, xb8_stride;
+    /* half-byte form of bin 8: hb8 = 4 byte copies of y = clamp((x_8 - off8) >> 1, 0, 255), bits8 = the dropped low bits, one
+     * bit per sample (bit k of word w of a row = sample 32 w + k), exceptions r = x_8 - off8 - 2 y - bit */
+    uint8_t* hb8; size_t hb8_pitch, hb8_stride; const int32_t* off8; uint2* exc8; unsigned* cnt8; long long nb8;
+    uint32_t* bits8; size_t bits8_pitch;
 };
+
+__device__ __forceinline__ uint32_t spread16(uint32_t x) {             /* bit k of the low half -> bit 2k */
+    x = (x | (x << 8)) & 0x00FF00FFu; x = (x | (x << 4)) & 0x0F0F0F0Fu; x = (x | (x << 2)) & 0x33333333u; x = (x | (x << 1)) & 0x55555555u;
+    return x;
+}
 
 __device__ __forceinline__ uint32_t byte_of(const uint32_t (&w)[8], int i) { return (w[i >> 2] >> (8 * (i & 3))) & 0xFFu; }
 
@@ -189,7 +200,7 @@ __device__ __forceinline__ uint32_t byte_of(const uint32_t (&w)[8], int i) { ret
 __global__ void __launch_bounds__(256)
 k_prep_fused(const PrepFused p) {
     const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= p.ngroups) return;
+    if (g >= p.ngroups) return;                                         /* ngroups is a multiple of 16: whole half-warps leave */
     const int c = blockIdx.y;
     const uint8_t* src = p.raw + (size_t)c * p.pitch + (size_t)g * 16;
     const uint4 a = *reinterpret_cast<const uint4*>(src);
@@ -241,6 +252,41 @@ k_prep_fused(const PrepFused p) {
         for (int j = 0; j < 4; ++j)
             *reinterpret_cast<uint32_t*>(p.lo4 + (size_t)j * p.lo4_stride + (size_t)c * p.lo4_pitch + (size_t)g * 4) =
                 l[j] | (l[j + 1] << 8) | (l[j + 2] << 16) | (l[j + 3] << 24);
+    }
+    if (p.hb8) {
+        /* 2 own samples of bin 8 and 3 ahead (the 4 shifted copies): 40 raw samples */
+        const uint2 n2 = *reinterpret_cast<const uint2*>(src + 32);
+        const int oc = p.off8[c];
+        uint32_t y[5], bit[2] = {0u, 0u};
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            int z = -oc;
+            if (k < 4) {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) z += (int)byte_of(w, 8 * k + j);
+            } else {
+                z += (int)__dp4a(n2.x, 0x01010101u, 0u) + (int)__dp4a(n2.y, 0x01010101u, 0u);
+            }
+            const int h = z >> 1;                                       /* arithmetic: floor(z / 2), z = 2 h + (z & 1) */
+            const int v = h < 0 ? 0 : (h > 255 ? 255 : h);
+            y[k] = (uint32_t)v;
+            const long long t = g * 2 + k;
+            if (k < 2) {
+                bit[k] = (uint32_t)(z & 1);
+                if (h != v && t < p.nb8) append_exception(p.exc8, p.cnt8, p.cap, make_exception(p.chan0 + c, t, z - 2 * v - (z & 1)));
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            *reinterpret_cast<uint16_t*>(p.hb8 + (size_t)j * p.hb8_stride + (size_t)c * p.hb8_pitch + (size_t)g * 2) = (uint16_t)(y[j] | (y[j + 1] << 8));
+        /* the bit plane: lane L of the warp holds samples 2L, 2L+1 of a 64-sample run */
+        const int lane = threadIdx.x & 31;
+        const unsigned am = (g - lane + 16 < p.ngroups) ? 0xffffffffu : 0x0000ffffu;   /* the lanes that did not leave at the top */
+        const uint32_t m0 = __ballot_sync(am, bit[0]), m1 = __ballot_sync(am, bit[1]);
+        if ((lane & 15) == 0) {
+            const uint32_t h0 = lane ? (m0 >> 16) : (m0 & 0xFFFFu), h1 = lane ? (m1 >> 16) : (m1 & 0xFFFFu);
+            p.bits8[(size_t)c * p.bits8_pitch + (size_t)(g >> 4)] = spread16(h0) | (spread16(h1) << 1);
+        }
     }
     if (p.xb8) {
         uint32_t s8[3];
@@ -364,10 +410,10 @@ extern "C" int aak_corner_turn(const uint8_t* in, size_t in_stride, uint8_t* out
     return (int)cudaGetLastError();
 }
 
-extern "C" int aak_chan_offsets(const uint8_t* x, size_t pitch, int64_t len, int32_t nrows, int32_t* off2, int32_t* off4,
-                                int32_t* bias2, int32_t* bias4, void* stream) {
+extern "C" int aak_chan_offsets(const uint8_t* x, size_t pitch, int64_t len, int32_t nrows, int32_t* off2, int32_t* off4, int32_t* off8,
+                                int32_t* bias2, int32_t* bias4, int32_t* bias8, void* stream) {
     if (nrows <= 0) return 0;
-    k_chan_offsets<<<(unsigned)nrows, 256, 0, (cudaStream_t)stream>>>(x, pitch, len, off2, off4, bias2, bias4);
+    k_chan_offsets<<<(unsigned)nrows, 256, 0, (cudaStream_t)stream>>>(x, pitch, len, off2, off4, off8, bias2, bias4, bias8);
     return (int)cudaGetLastError();
 }
 
@@ -390,6 +436,8 @@ extern "C" int aak_prep_fused(const aak_prep_args* a, int32_t nrows, void* strea
     p.lo2 = a->lo2; p.lo2_pitch = a->lo2_pitch; p.lo2_stride = a->lo2_stride; p.off2 = a->off2; p.exc2 = a->exc2; p.cnt2 = a->cnt2; p.nb2 = a->nb2;
     p.lo4 = a->lo4; p.lo4_pitch = a->lo4_pitch; p.lo4_stride = a->lo4_stride; p.off4 = a->off4; p.exc4 = a->exc4; p.cnt4 = a->cnt4; p.nb4 = a->nb4;
     p.xb8 = a->xb8; p.xb8_pitch = a->xb8_pitch; p.xb8_stride = a->xb8_stride;
+    p.hb8 = a->hb8; p.hb8_pitch = a->hb8_pitch; p.hb8_stride = a->hb8_stride; p.off8 = a->off8; p.exc8 = a->exc8; p.cnt8 = a->cnt8; p.nb8 = a->nb8;
+    p.bits8 = a->bits8; p.bits8_pitch = a->bits8_pitch;
     dim3 grid((unsigned)((a->ngroups + 255) / 256), (unsigned)nrows);
     k_prep_fused<<<grid, 256, 0, (cudaStream_t)stream>>>(p);
     return (int)cudaGetLastError();

@@ -314,3 +314,33 @@ def check_band(gpu: GpuRun, orc: OracleRun, chunk, r, i0, i1, *, after_sps: bool
             emu, esg = res["stats"][i - i0]
             assert mu == emu and sg == esg, (r, i, mu, emu, sg, esg)
     return res["cands"]
+
+
+def check_bands(gpu: GpuRun, orc: OracleRun, chunk, bands, *, after_sps: bool, threads: int | None = None):
+    """check_band for a list of bands [(r, i0, i1)] of one chunk. The oracle side (single-threaded C per call; ctypes releases the
+    GIL) runs the bands on a thread pool over the host cores, the comparison with the CUDA path stays on the calling thread.
+    Returns the oracle's candidates per band, in the order of `bands`."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    start, length, n_out = chunk
+    for b in sorted({orc.w.ranges[r][3] for (r, _, _) in bands}):
+        orc.binned(start, length, b)                       # bin once, on this thread (the cache is not thread-safe)
+    extra = getattr(gpu, "extra", 0)
+    with ThreadPoolExecutor(max_workers=threads or min(16, os.cpu_count() or 1)) as ex:
+        results = list(ex.map(lambda bd: orc.search(chunk, bd[0], bd[1], bd[2], want=("D", "stats"), extra=extra), bands))
+    out = []
+    for (r, i0, i1), res in zip(bands, results):
+        for i in range(i0, i1):
+            got = gpu.row(r, i)
+            exp = res["D"][i - i0]
+            assert got.shape == exp.shape, (r, i, got.shape, exp.shape)
+            if not np.array_equal(got.astype(np.int64), exp):
+                bad = np.flatnonzero(got.astype(np.int64) != exp)
+                raise AssertionError(f"D mismatch range {r} row {i}: {len(bad)} samples, first at t={bad[:5]}, "
+                                     f"got {got[bad[:5]]}, expected {exp[bad[:5]]}")
+            if after_sps:
+                mu, sg, n, it = gpu.stats(r, i)
+                emu, esg = res["stats"][i - i0]
+                assert mu == emu and sg == esg, (r, i, mu, emu, sg, esg)
+        out.append(res["cands"])
+    return out

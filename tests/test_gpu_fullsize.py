@@ -15,7 +15,7 @@ import pytest
 
 import datagen
 
-from helpers import (GpuRun, OracleRun, band_rows, check_band, compare_candidates, make_input, row_moments_all_ranges,
+from helpers import (GpuRun, OracleRun, band_rows, check_band, check_bands, compare_candidates, make_input, row_moments_all_ranges,
                      sampled_outputs)
 
 pytestmark = pytest.mark.gpu
@@ -65,16 +65,16 @@ def _fullsize(name, points_per_range, pulse_bands):
         gpu.sps()
         got = gpu.candidates(allow_overflow=False)
         pl, dms, _ = w.pulses()
-        nb = 0
+        bands = []
         for r, rng in enumerate(w.ranges):
             centres = [0, rng[2] // 2, rng[2] - 1]
             hi = rng[0] + rng[1] * rng[2]
             centres += [int(round((d - rng[0]) / rng[1])) for d in dms[:pulse_bands] if rng[0] <= d < hi]
-            for (i0, i1) in band_rows(rng[2], [min(rng[2] - 1, max(0, c)) for c in centres]):
-                e = check_band(gpu, orc, chunk, r, i0, i1, after_sps=True)
-                sel = (got["range"] == r) & (got["dm_index"] >= i0) & (got["dm_index"] < i1)
-                compare_candidates(got[sel], e, w.threshold)
-                nb += 1
+            bands += [(r, i0, i1) for (i0, i1) in band_rows(rng[2], [min(rng[2] - 1, max(0, c)) for c in centres])]
+        for (r, i0, i1), e in zip(bands, check_bands(gpu, orc, chunk, bands, after_sps=True)):     # the oracle's bands run in parallel
+            sel = (got["range"] == r) & (got["dm_index"] >= i0) & (got["dm_index"] < i1)
+            compare_candidates(got[sel], e, w.threshold)
+        nb = len(bands)
         assert datagen.checksum(x) == before          # the user's input is never written
         return gpu.info, len(got), nb
     finally:
@@ -190,9 +190,8 @@ def test_stream_full_size_selected_chunks():
             status = gpu.sps()
             assert status == (gpu.aa.AA_STATUS_FINISHED if j == n - 1 else gpu.aa.AA_STATUS_CHUNK_DONE)
             if j in check:
-                for r, rng in enumerate(w.ranges):
-                    i0, i1 = band_rows(rng[2], [rng[2] // 2])[0]
-                    e = check_band(gpu, orc, chunk, r, i0, i1, after_sps=True)
+                bands = [(r,) + band_rows(rng[2], [rng[2] // 2])[0] for r, rng in enumerate(w.ranges)]
+                for (r, i0, i1), e in zip(bands, check_bands(gpu, orc, chunk, bands, after_sps=True)):
                     exp_bands.append((r, i0, i1, start, n_out, e))
         got = gpu.candidates()
         for (r, i0, i1, start, n_out, e) in exp_bands:

@@ -13,7 +13,7 @@ import pytest
 import datagen
 from datagen.workloads import Workload, scaled
 
-from helpers import GpuRun, OracleRun, band_rows, check_band, compare_candidates, make_input, row_moments_from_input
+from helpers import GpuRun, OracleRun, band_rows, check_band, check_bands, compare_candidates, make_input, row_moments_from_input
 
 pytestmark = pytest.mark.gpu
 
@@ -52,13 +52,13 @@ def _band_parity(w, x, centres_per_range, **kw):
                 assert bad.size == 0, f"chunk {j} range {r}: moment identity fails on rows {bad[:10]} ({bad.size} rows)"
             gpu.sps()
             got = gpu.candidates()
-            for r, rng in enumerate(w.ranges):
-                for (i0, i1) in band_rows(rng[2], centres_per_range.get(r, [0, rng[2] // 2, rng[2] - 1])):
-                    exp = check_band(gpu, orc, chunk, r, i0, i1, after_sps=True)
-                    sel = (got["range"] == r) & (got["dm_index"] >= i0) & (got["dm_index"] < i1) & \
-                          (got["sample"] >= start) & (got["sample"] < start + n_out)
-                    compare_candidates(got[sel], exp, w.threshold)
-                    ncheck += 1
+            bands = [(r, i0, i1) for r, rng in enumerate(w.ranges)
+                     for (i0, i1) in band_rows(rng[2], centres_per_range.get(r, [0, rng[2] // 2, rng[2] - 1]))]
+            for (r, i0, i1), exp in zip(bands, check_bands(gpu, orc, chunk, bands, after_sps=True)):
+                sel = (got["range"] == r) & (got["dm_index"] >= i0) & (got["dm_index"] < i1) & \
+                      (got["sample"] >= start) & (got["sample"] < start + n_out)
+                compare_candidates(got[sel], exp, w.threshold)
+                ncheck += 1
         return gpu.info, ncheck
     finally:
         gpu.close()
