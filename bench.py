@@ -55,6 +55,9 @@ def parse():
     ap.add_argument("--workload", default="ska", help="tiny | mid | ska | lowf | stream (BASELINE.json configs 0..4), ska16 (ska as 16-bit samples); "
                     "stream = the 600 s chunked pipeline under a 40 GB budget, a step is the whole stream")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--input", default="noise", choices=["noise", "uniform"], help="noise: the workload's recipe (Gaussian noise + pulses); "
+                    "uniform: uniform random samples over the whole range - every offset form is exception-heavy, so the line records the "
+                    "cost of the dense routes (uint16 kernels / global-memory kernel); not a BASELINE.json configuration")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--nsamp", type=int, default=0, help="shorten (or lengthen) the workload's observation to this many samples: "
@@ -162,9 +165,11 @@ def run_reference(args, w):
         secs += s
         spent += sp
     v = outs / secs
+    # ms_per_step is what a step (= one bounded sample) really took, so that steps x ms_per_step is this run's wall time; value is the
+    # whole-job throughput the sample extrapolates to (work is exactly linear in DM rows), job_ms_extrapolated the job time behind it
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "int64", "sample_seconds_per_step": spent / args.steps, "data": "synthetic",
+            "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * spent / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int64", "job_ms_extrapolated": 1e3 * secs / args.steps, "data": "synthetic",
             "config": {"workload": w.name, "nchans": w.nchans, "nsamp": w.nsamp, "ndms": w.ndms_total,
                        "note": "each step is a bounded sample of the workload: " + what},
             "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what},
@@ -193,6 +198,10 @@ def run_ours(args, w):
     xh = torch.empty((w.nchans, w.nsamp), dtype=torch.uint16 if esz == 2 else torch.uint8, pin_memory=True)
     x = xh.numpy()
     datagen.generate(w.seed + 1000003 * rank, w.nchans, w.nsamp, pl, dl, out=x, **w.gen_kw)
+    if args.input == "uniform":
+        rs = np.random.default_rng(w.seed + rank)
+        for c0 in range(0, w.nchans, 256):
+            x[c0:c0 + 256] = rs.integers(0, w.max_value + 1, size=x[c0:c0 + 256].shape, dtype=x.dtype)
     xd = xh.cuda(non_blocking=False)
 
     compute, copy = torch.cuda.Stream(), torch.cuda.Stream()
@@ -296,8 +305,8 @@ def run_ours(args, w):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "int32", "data": "synthetic",
-            "config": {"workload": w.name, "nchans": w.nchans, "nsamp": w.nsamp, "tsamp_us": w.tsamp_s * 1e6, "ndms": w.ndms_total,
-                       "input_bits": w.input_bits, "input_max": w.max_value,
+            "config": {"workload": w.name if args.input == "noise" else w.name + "+uniform-input", "nchans": w.nchans, "nsamp": w.nsamp,
+                       "tsamp_us": w.tsamp_s * 1e6, "ndms": w.ndms_total, "input_bits": w.input_bits, "input_max": w.max_value,
                        "ranges": [list(r) for r in w.ranges], "widths": list(w.widths), "threshold": w.threshold,
                        "outputs_per_step": outputs, "l2": "inputs larger than L2 (chunk %.2f GB in, %.2f GB out)" % (in_bytes / 1e9, 4 * outputs / 1e9),
                        "parallelism": "replicas over time chunks" if world > 1 else "single GPU"},
