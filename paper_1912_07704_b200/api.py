@@ -262,7 +262,7 @@ def _host_input(strategy, host_input, row_stride_bytes):
         want = np.uint16 if item == 2 else np.uint8
         if host_input.dtype != want:
             raise TypeError(f"host_input must be {np.dtype(want).name} (the plan's sample type), got {host_input.dtype}")
-        if host_input.ndim != 2 or host_input.strides[1] != item:
+        if host_input.ndim != 2 or (host_input.shape[1] > 1 and host_input.strides[1] != item):
             raise ValueError("host_input must be 2-D with unit stride along its rows")
         rows, cols = ((info["nsamp_total"], info["nchans"]) if info["input_layout"] == AA_LAYOUT_TIME_MAJOR
                       else (info["nchans"], info["nsamp_total"]))

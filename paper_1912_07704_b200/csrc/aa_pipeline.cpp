@@ -410,6 +410,13 @@ extern "C" aa_status aa_run_sps(aa_strategy* h) {
         }
     }
     AA_CUDA(cudaEventRecord(s.ev_t[4], s.compute), "cudaEventRecord");
+    /* the ranges' K4 launches are independent (one atomic counter): odd ranges go to the auxiliary stream, as for K2, so that the
+     * short launches of the binned ranges run beside the others instead of each ending in its own partly filled wave */
+    const bool two = s.ranges.size() > 1 && s.aux;
+    if (two) {
+        AA_CUDA(cudaEventRecord(s.ev_fork, s.compute), "cudaEventRecord");
+        AA_CUDA(cudaStreamWaitEvent(s.aux, s.ev_fork, 0), "cudaStreamWaitEvent");
+    }
     for (Range& rg : s.ranges) {
         aak_sps_args a;
         a.D = rg.d_D; a.pitch = rg.pitch; a.nt = (int64_t)(c.n_out / (uint64_t)rg.r.bin); a.nt_data = a.nt + rg.extra; a.ndms = rg.r.ndms; a.bin = rg.r.bin;
@@ -423,7 +430,11 @@ extern "C" aa_status aa_run_sps(aa_strategy* h) {
         a.wstats = s.plan.per_width ? s.d_wstats + 2 * nwd * rg.first_row : nullptr;
         a.wpivot = s.plan.per_width ? s.d_wpivot + nwd * rg.first_row : nullptr;
         a.wlive = s.plan.per_width ? s.d_wlive + rg.first_row : nullptr;
-        AA_LAUNCH(aak_sps_peaks(&a, s.compute), "sps peaks");
+        AA_LAUNCH(aak_sps_peaks(&a, (two && (rg.index & 1)) ? s.aux : s.compute), "sps peaks");
+    }
+    if (two) {
+        AA_CUDA(cudaEventRecord(s.ev_join, s.aux), "cudaEventRecord");
+        AA_CUDA(cudaStreamWaitEvent(s.compute, s.ev_join, 0), "cudaStreamWaitEvent");
     }
     AA_CUDA(cudaEventRecord(s.ev_t[5], s.compute), "cudaEventRecord");
     AA_CUDA(cudaMemcpyAsync(s.h_counter, s.d_counter, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s.compute), "counter D2H");

@@ -42,20 +42,20 @@ struct BitsParams {
 /* the words of NM adjacent trials of one channel: trial m reuses the pair loaded for trial m - 1 when it starts in the same word
  * (a warp-uniform test of two table entries; the first version loaded two words per trial and was bound by the shared-memory
  * load path: ncu l1tex 89 %, mio_throttle the top stall) */
-__device__ __forceinline__ void bk_words(const uint8_t* Sb, const uint2* e, uint32_t (&x)[BK_NM]) {
+__device__ __forceinline__ void bk_words(const uint8_t* Sb, const uint32_t* e, uint32_t (&x)[BK_NM]) {
     uint32_t lo = 0, hi = 0, off = 0xffffffffu;
-    static_assert(BK_NM == 4, "two 16-byte loads fetch the four entries");
-    const uint4 e01 = *reinterpret_cast<const uint4*>(e), e23 = *reinterpret_cast<const uint4*>(e + 2);
-    const uint2 ev[4] = {make_uint2(e01.x, e01.y), make_uint2(e01.z, e01.w), make_uint2(e23.x, e23.y), make_uint2(e23.z, e23.w)};
+    static_assert(BK_NM == 4, "one 16-byte load fetches the four entries");
+    const uint4 e4 = *reinterpret_cast<const uint4*>(e);
+    const uint32_t ev[4] = {e4.x, e4.y, e4.z, e4.w};
 #pragma unroll
     for (int m = 0; m < BK_NM; ++m) {
-        const uint2 em = ev[m];
-        if (em.x != off) {
-            off = em.x;
+        const uint32_t o = ev[m] & 0x00FFFFFFu;
+        if (o != off) {
+            off = o;
             lo = *reinterpret_cast<const uint32_t*>(Sb + off);
             hi = *reinterpret_cast<const uint32_t*>(Sb + off + 4);
         }
-        x[m] = __funnelshift_r(lo, hi, em.y);
+        x[m] = __funnelshift_r(lo, hi, ev[m] >> 24);
     }
 }
 
@@ -64,7 +64,7 @@ k_dedisperse_bits(const BitsParams p) {
     if (p.mode_cnt && *p.mode_cnt > p.mode_cap) return;               /* exception-heavy chunk: the uint16 route produced D */
     extern __shared__ __align__(16) uint32_t bk_smem[];
     uint32_t* S = bk_smem;                                           /* [BK_CB][ww] window words of the block's channels */
-    uint2* ent = reinterpret_cast<uint2*>(S + (size_t)BK_CB * p.ww); /* [BK_CB][BK_DMS]: {byte offset of the first word, shift} */
+    uint32_t* ent = S + (size_t)BK_CB * p.ww;                        /* [BK_CB][BK_DMS]: byte offset of the first word | shift << 24 */
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const long long t0 = (long long)blockIdx.x * BK_T;
     const int i0 = blockIdx.y * BK_DMS;
@@ -98,7 +98,7 @@ k_dedisperse_bits(const BitsParams p) {
                 wv[k][0] = (live && lane < p.ww) ? __ldg(src + lane) : 0u;
                 wv[k][1] = (live && lane + 32 < p.ww) ? __ldg(src + lane + 32) : 0u;
                 const int o = (int)(t0 + d[k] - (w0 << 5));           /* bit offset inside the window, >= 0 */
-                ent[cl * BK_DMS + lane] = make_uint2((uint32_t)((cl * p.ww + (o >> 5)) * 4), (uint32_t)(o & 31));
+                ent[cl * BK_DMS + lane] = (uint32_t)((cl * p.ww + (o >> 5)) * 4) | ((uint32_t)(o & 31) << 24);
             }
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
@@ -116,7 +116,7 @@ k_dedisperse_bits(const BitsParams p) {
         /* ---- every thread: its word of every channel for each of its trials; 32 channels per carry-save tree, the four weight-32
          * carries of the block through a second tree, one ripple into the high planes per block */
         const uint8_t* Sb = reinterpret_cast<const uint8_t*>(S) + lane * 4;
-        const uint2* eb = ent + BK_NM * warp;
+        const uint32_t* eb = ent + BK_NM * warp;
         uint32_t c32v[BK_NM][BK_CB / 32];
 #pragma unroll
         for (int c32 = 0; c32 < BK_CB; c32 += 32) {
@@ -197,7 +197,7 @@ extern "C" int aak_dedisperse_bits(const uint32_t* bits, size_t pitch_words, con
     BitsParams p;
     p.bits = bits; p.pitchw = pitch_words; p.delays = delays; p.nchans = nchans; p.c0 = chan_begin; p.c1 = chan_end; p.ndms = ndms; p.nt = nt;
     p.ww = window_words; p.D = D; p.dpitch = pitch; p.mode_cnt = mode_cnt; p.mode_cap = mode_cap;
-    const size_t smem = ((size_t)BK_CB * window_words + 2 * BK_CB * BK_DMS) * 4;
+    const size_t smem = ((size_t)BK_CB * window_words + BK_CB * BK_DMS) * 4;
     static bool attr = false;
     if (!attr) {
         const int e = (int)cudaFuncSetAttribute(k_dedisperse_bits, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
