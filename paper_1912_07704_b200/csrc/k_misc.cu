@@ -222,7 +222,8 @@ k_prep_fused(const PrepFused p) {
         uint32_t l[11];
 #pragma unroll
         for (int k = 0; k < 11; ++k) {
-            const int y = (int)(byte_of(w, 2 * k) + byte_of(w, 2 * k + 1)) - oc;
+            /* x_2 - off in ONE instruction: IDP.2A sums the two bytes of a half word into the accumulator (-off) */
+            const int y = (int)((k & 1) ? __dp2a_hi(0x00010001u, w[k >> 1], (unsigned)-oc) : __dp2a_lo(0x00010001u, w[k >> 1], (unsigned)-oc));
             const int v = y < 0 ? 0 : (y > 255 ? 255 : y);
             l[k] = (uint32_t)v;
             const long long t = g * 8 + k;
@@ -241,7 +242,7 @@ k_prep_fused(const PrepFused p) {
         uint32_t l[7];
 #pragma unroll
         for (int k = 0; k < 7; ++k) {
-            const int y = (int)(byte_of(w, 4 * k) + byte_of(w, 4 * k + 1) + byte_of(w, 4 * k + 2) + byte_of(w, 4 * k + 3)) - oc;
+            const int y = (int)__dp4a(w[k], 0x01010101u, (unsigned)-oc);      /* x_4 - off: IDP.4A */
             const int v = y < 0 ? 0 : (y > 255 ? 255 : y);
             l[k] = (uint32_t)v;
             const long long t = g * 4 + k;
@@ -260,13 +261,8 @@ k_prep_fused(const PrepFused p) {
         uint32_t y[5], bit[2] = {0u, 0u};
 #pragma unroll
         for (int k = 0; k < 5; ++k) {
-            int z = -oc;
-            if (k < 4) {
-#pragma unroll
-                for (int j = 0; j < 8; ++j) z += (int)byte_of(w, 8 * k + j);
-            } else {
-                z += (int)__dp4a(n2.x, 0x01010101u, 0u) + (int)__dp4a(n2.y, 0x01010101u, 0u);
-            }
+            const uint32_t wa = k < 4 ? w[2 * k] : n2.x, wb = k < 4 ? w[2 * k + 1] : n2.y;
+            const int z = (int)__dp4a(wa, 0x01010101u, __dp4a(wb, 0x01010101u, (unsigned)-oc));     /* x_8 - off */
             const int h = z >> 1;                                       /* arithmetic: floor(z / 2), z = 2 h + (z & 1) */
             const int v = h < 0 ? 0 : (h > 255 ? 255 : h);
             y[k] = (uint32_t)v;
