@@ -377,3 +377,33 @@ def test_range_whose_tile_window_exceeds_shared_memory_takes_the_global_memory_r
         assert n + og == len(got) and n + oe == sum(len(e) for e in exp)
     finally:
         gpu.close()
+
+
+@pytest.mark.parametrize("bits", [8, 16])
+def test_sparse_exceptions_in_every_offset_form_are_scattered_exactly(bits):
+    """Gaussian noise with rare large spikes (3e-5 of the samples, both signs) in a plan with bin 1, 2, 4 and 8: every offset
+    form stays on its sparse route (exception rate below 4e-4) but has real exceptions with residuals of both signs - the
+    offset-uint8 forms, the half-byte form with its bit plane (8-bit plans) and the offset-uint16 form (16-bit plans). Every row
+    of D must equal the oracle's, in one chunk and with the channel groups of the pipelined copy (>= 256 channels)."""
+    rs = np.random.default_rng(88 + bits)
+    C, N = 288, 24_000
+    mean, top = (127.0, 255) if bits == 8 else (1800.0, 4095)
+    x = np.clip(np.floor(mean + 16.0 * rs.standard_normal((C, N)) + 0.5), 0, top)
+    spikes = rs.random((C, N)) < 3e-5                               # bin 8: 2.4e-4 of the binned samples, below the 4e-4 route limit
+    x[spikes] = np.where(rs.random(int(spikes.sum())) < 0.5, 0, top)
+    x = x.astype(np.uint16 if bits == 16 else np.uint8)
+    nd = 70
+    w = Workload("spikes", C, 1500.0, -0.5, 256e-6, N, ((0.0, 0.05, nd, 1), (3.5, 0.05, nd, 2), (7.0, 0.1, nd, 4), (14.0, 0.2, nd, 8)), (1, 2, 4), 6.0,
+                 seed=1, npulses=0, pulse_dm=(0.0, 0.0), pulse_width_max=1, input_bits=bits, max_value=top)
+    gpu, orc = GpuRun(w, x), OracleRun(w, x)
+    try:
+        desc = gpu.aa.aa_strategy_describe(gpu.h)
+        assert ("half-byte form" in desc) == (bits == 8) and ("offset-uint16 form" in desc) == (bits == 16)
+        gpu.dedisperse()
+        for r, rng in enumerate(w.ranges):
+            check_band(gpu, orc, gpu.chunks[0], r, 0, nd, after_sps=False)
+        gpu.sps()
+        exp = [check_band(gpu, orc, gpu.chunks[0], r, 0, nd, after_sps=True) for r in range(len(w.ranges))]
+        n, og, oe = compare_candidates(gpu.candidates(allow_overflow=True), np.concatenate(exp), w.threshold)
+    finally:
+        gpu.close()
