@@ -407,29 +407,34 @@ static aa_status plan_host(aa_strategy* h, const aa_plan* plan, uint64_t nsamp_t
     /* chunk length under the budget (reading C3): whole observation if it fits, else the largest power of two */
     s.arena.dry = true; s.arena.base = nullptr; s.arena.size = 0;
     auto need = [&](int64_t L) { const bool two = (L < usable); carve(s, L, two); return s.arena.used; };   /* two: double-buffered staging */
+    /* a chunk row stays below 2^28 samples: the sample field of an exception record (k_common.cuh) has 28 bits */
+    const int64_t Lmax = (((int64_t)1 << 28) - 1) / s.B * s.B;
+    auto fits = [&](int64_t L) { return L <= Lmax && (!limit || need(L) <= limit); };
     int64_t L = 0;
     if (chunk_len_hint) {
         L = (int64_t)chunk_len_hint;
         if (L % s.B || L <= s.S) { set_error("aa_strategy_setup: chunk_len_hint = %lld must be a multiple of %d and > overlap %lld", (long long)L, s.B, (long long)s.S); return AA_ERR_INVALID_ARG; }
         if (L > usable) L = usable;
+        if (L > Lmax) { set_error("aa_strategy_setup: chunk_len_hint = %lld exceeds the largest chunk of %lld samples", (long long)L, (long long)Lmax); return AA_ERR_INVALID_ARG; }
         if (limit && need(L) > limit) { set_error("aa_strategy_setup: chunk_len_hint = %lld needs %zu bytes, budget is %zu", (long long)L, need(L), limit); return AA_ERR_BUDGET_TOO_SMALL; }
-    } else if (!limit || need(usable) <= limit) {
+    } else if (fits(usable)) {
         L = usable;
     } else {
         int64_t p2 = 1;
         while (p2 <= s.S) p2 <<= 1;
         if (p2 % s.B) p2 = (int64_t)round_up((size_t)p2, (size_t)s.B);
-        if (p2 >= usable || need(p2) > limit) {
+        if (p2 >= usable || !fits(p2)) {
+            if (p2 > Lmax) { set_error("aa_strategy_setup: the maximum delay (%lld samples) exceeds the largest chunk of %lld samples", (long long)s.S, (long long)Lmax); return AA_ERR_INVALID_ARG; }
             set_error("aa_strategy_setup: budget of %zu bytes is too small: the smallest chunk (%lld samples, overlap %lld) needs %zu bytes",
                       limit, (long long)p2, (long long)s.S, need(std::min(p2, usable)));
             return AA_ERR_BUDGET_TOO_SMALL;
         }
-        while (p2 * 2 < usable && need(p2 * 2) <= limit) p2 *= 2;
+        while (p2 * 2 < usable && fits(p2 * 2)) p2 *= 2;
         L = p2;
         /* then grow in eighths of that power of two while the arena still fits: every chunk recomputes S samples of
-         * overlap, so longer chunks waste less (600 s stream under 40 GB: L = 2^19 -> 9 * 2^16, 19 -> 17 chunks) */
+         * overlap, so longer chunks waste less (600 s stream under 40 GB: L = 2^19 -> 3 * 2^18, 19 -> 13 chunks) */
         const int64_t step = (int64_t)round_up((size_t)std::max<int64_t>(p2 / 8, s.B), (size_t)s.B);
-        while (L + step < usable && need(L + step) <= limit) L += step;
+        while (L + step < usable && fits(L + step)) L += step;
     }
     s.L = L;
     s.n_out = L - s.S;

@@ -279,3 +279,22 @@ def test_input_bits_validation_names_the_limit_and_the_strategy_plans_the_offset
         aa.aa_plan_set_input_bits(big, 8, 0)
     finally:
         aa.aa_plan_destroy(big)
+
+
+def test_chunk_rows_stay_below_the_28_bit_sample_field_of_an_exception_record():
+    """An observation longer than 2^28 samples is chunked even without a budget (exception records carry the sample index in
+    28 bits); a chunk_len_hint beyond that is refused with a message."""
+    plan = aa.aa_plan_create(np.array([1500.0, 1499.0]), 64e-6, ((0.0, 1.0, 4, 2),), (1, 2), 6.0)
+    try:
+        n = (1 << 28) + 4096
+        st = aa.aa_strategy_plan(plan, n)
+        try:
+            info = aa.aa_strategy_get_info(st)
+            assert info["nchunks"] >= 2 and info["chunk_len"] < (1 << 28) and info["chunk_len"] % 2 == 0
+        finally:
+            aa.aa_strategy_destroy(st)
+        with pytest.raises(aa.AaError) as e:
+            aa.aa_strategy_plan(plan, n, chunk_len_hint=(1 << 28) + 2)
+        assert e.value.status == aa.AA_ERR_INVALID_ARG and "largest chunk" in e.value.message
+    finally:
+        aa.aa_plan_destroy(plan)
