@@ -27,12 +27,13 @@ int aak_bin_time(const uint8_t* x, size_t x_pitch, uint16_t* xb, size_t xb_pitch
 int aak_shift_copy(const uint8_t* in, uint8_t* out, size_t pitch, size_t row_bytes, int32_t nrows, int32_t shift_bytes,
                    const unsigned* only_if_cnt, unsigned only_if_above, void* stream);
 
-/* ---- K1c: offset-uint8 form of a binned input (bin 2, 4), see k_misc.cu: x_b = lo + off_c + r with lo a byte and r an
- * exception list. aak_chan_offsets: off_b[c] = clamp(round(b * mean_t x[c][t]) - 128, 0, 255 (b-1)) for rows [0, nrows) and
- * *bias_b += sum of them (either pair may be NULL). aak_prep_fused (below) writes lo[c][t'] and appends the exceptions
- * {c + chan0 | (r + 1024) << 16, t'} at exc[atomicAdd(exc_cnt)] while below cap (the counter keeps counting).
- * aak_scatter_exceptions: D[i][t' - delay(c, i)] += r for every exception and every trial of one range; returns at once
- * if *exc_cnt > cap. k = the plan's delay constants (device doubles). */
+/* ---- K1c: offset forms of a binned input, see k_misc.cu: x_b = lo + off_c + r with lo a byte and r an exception list (bin 2, 4),
+ * x_8 = 2 y + bit + off_c + r (bin 8, half-byte form). aak_chan_offsets: off_b[c] = clamp(round(b * mean_t x[c][t]) - centre, 0, ..)
+ * for rows [0, nrows), centre 128 (bin 2, 4) or 256 (bin 8), and *bias_b += sum of them (any pair may be NULL). aak_prep_fused
+ * (below) writes the forms and appends the exceptions (64-bit records: channel 16 bits, residual r 20 bits two's complement,
+ * binned sample 28 bits; k_common.cuh) at exc[counter++] while the counter is below cap (one atomic per warp; nothing more is
+ * counted once it has passed cap). aak_scatter_exceptions: D[i][t' - delay(c, i)] += r for every exception and every trial of
+ * one range; returns at once if *exc_cnt > cap. k = the plan's delay constants (device doubles). */
 int aak_chan_offsets(const uint8_t* x, size_t pitch, int64_t len, int32_t nrows, int32_t* off2, int32_t* off4, int32_t* off8, int32_t* bias2,
                      int32_t* bias4, int32_t* bias8, void* stream);
 int aak_scatter_exceptions(const uint2* exc, const unsigned* exc_cnt, unsigned cap, const double* k, double dm_low, double dm_step,
@@ -40,8 +41,9 @@ int aak_scatter_exceptions(const uint2* exc, const unsigned* exc_cnt, unsigned c
 
 /* ---- K1 fused: one read of raw rows [0, nrows) (pointers already offset to the first row; chan0 = its channel index)
  * writes the 4 uint8 copies (x4, may be NULL; rows x4_pitch bytes apart, copy k at + k x4_stride), the offset-uint8 forms lo2 / lo4 with their 4 copies and exceptions (may be
- * NULL; off2/off4 offset to the first row; nb = valid binned samples) and the 2 copies of the uint16 bin-8 input (xb8,
- * may be NULL; xb8_pitch in elements, xb8_stride in bytes). ngroups = 16-byte groups per row. */
+ * NULL; off2/off4 offset to the first row; nb = valid binned samples) and, for bin 8, EITHER the half-byte form (hb8, bits8) OR
+ * the 2 copies of the uint16 input (xb8; xb8_pitch in elements, xb8_stride in bytes). ngroups = 16-byte groups per row, a
+ * multiple of 16. */
 typedef struct {
     const uint8_t* raw; size_t pitch; int64_t ngroups; int32_t chan0; unsigned cap;
     uint8_t* x4; size_t x4_pitch, x4_stride;

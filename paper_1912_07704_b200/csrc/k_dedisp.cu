@@ -462,10 +462,12 @@ extern "C" size_t aak_dedisperse_smem_bytes(int32_t chan_block, int32_t window_b
 }
 
 /* The instantiations the strategy can select (aa_strategy.cpp plan_format): bytes (uint8 input and the offset-uint8 form) =
- * 15 compute warps x 2 trials, odd-byte adds on the FMA pipe; binned uint16 = 16 compute warps x 4 adjacent trials with
+ * 15 compute warps x 2 trials, odd-byte adds on the FMA pipe (third parameter 3: the same with every sum doubled, for the
+ * half-byte form of bin 8, k_bits.cu); binned uint16 = 16 compute warps x 4 adjacent trials with
  * equal-delay reuse (third parameter 1: the offset-uint16 form of a 16-bit plan, which adds the sum of the channel offsets -
  * kept apart because the plain uint16 kernel, at 96 registers with spills, loses 8 % to any change of its epilogue);
- * channel block 8, 4 or 2 by window size. The variants measured and rejected are in profiles/r01c_profiles.md. */
+ * channel block 8, 4 or 2 by window size. The variants measured and rejected are in profiles/r01c_profiles.md
+ * and profiles/r02_all_configs.md (IDP.2A accumulators, 16-byte table loads). */
 #define AA_FOR_ALL_VARIANTS(X) \
     X(0, 8, 1, 2, 15) X(0, 4, 1, 2, 15) X(0, 2, 1, 2, 15) \
     X(0, 8, 3, 2, 15) X(0, 4, 3, 2, 15) X(0, 2, 3, 2, 15) \
