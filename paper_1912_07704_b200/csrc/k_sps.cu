@@ -27,7 +27,7 @@ typedef long long i64;
 typedef unsigned __int128 u128;
 
 /* ------------------------------------------------------------------------------------------------ K3 */
-constexpr int STAT_THREADS = 512;
+constexpr int STAT_THREADS = 256;
 constexpr int SPS_MAXW = 16;                 /* aa_plan_create: at most 16 boxcar widths */
 
 __device__ __forceinline__ double u128_to_double_rn(u128 v) {
@@ -156,7 +156,7 @@ __device__ __forceinline__ void split_sample(bool valid, int v, int p, int clo, 
     }
 }
 
-__global__ void __launch_bounds__(STAT_THREADS, 2)
+__global__ void __launch_bounds__(STAT_THREADS, 4)
 k_row_stats(const aak_row_desc* __restrict__ rows, double* __restrict__ mu_sigma, i64* __restrict__ n_iters) {
     extern __shared__ __align__(16) uint8_t stat_raw[];
     StatSmem& sm = *reinterpret_cast<StatSmem*>(stat_raw);
