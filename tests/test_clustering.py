@@ -50,6 +50,38 @@ def test_hand_worked_cases():
     assert e.value.status == aa.AA_ERR_INVALID_ARG and "dm_tol" in e.value.message
 
 
+def test_hand_worked_cases_pin_the_oracle():
+    """The same hand-worked lists through oracle.cluster_candidates ALONE: member sets and representatives are stated here from
+    the definition (reading C10), not taken from either implementation, so a mistake in the oracle's O(n^2) loop (a `<` for a
+    `<=` in any of its three clauses, cliques instead of components, a wrong tie rule) fails without the library's help."""
+    oc = lambda c, dm_tol, gap: tuple(map(list, oracle.cluster_candidates(c, dm_tol, gap)))
+    # boxcars [100,104) and [106,110): 106 <= 100 + 4 + gap iff gap >= 2; |10.5 - 10.0| <= dm_tol iff dm_tol >= 0.5
+    c = _cands([(100, 4, 10.0, 8.0, 0, 100), (106, 4, 10.5, 9.0, 0, 105)])
+    assert oc(c, 0.5, 1) == ([[0], [1]], [0, 1])
+    assert oc(c, 0.5, 2) == ([[0, 1]], [1])                     # inclusive at gap = 2 and at dm_tol = 0.5; best = snr 9.0
+    assert oc(c, 0.49, 2) == ([[0], [1]], [0, 1])
+    # the mirrored clause (the LATER boxcar is listed first): sample_a <= sample_b + width_b + gap at equality
+    c = _cands([(106, 4, 10.5, 9.0, 0, 105), (100, 4, 10.0, 8.0, 0, 100)])
+    assert oc(c, 0.5, 2) == ([[0, 1]], [0])
+    assert oc(c, 0.5, 1) == ([[0], [1]], [0, 1])
+    # a chain A-B, B-C linked, A-C not (24 > 0 + 10 + 2; |3 - 1| > 1): ONE cluster, connected components not cliques
+    c = _cands([(0, 10, 1.0, 7.5, 0, 1), (12, 10, 2.0, 7.2, 0, 2), (24, 10, 3.0, 7.9, 0, 3)])
+    assert oc(c, 1.0, 2) == ([[0, 1, 2]], [2])
+    assert oc(c, 1.0, 1) == ([[0], [1], [2]], [0, 1, 2])        # 12 > 0 + 10 + 1: the chain falls apart
+    # a wide early boxcar [0,1000) reaches the narrow one that starts inside it, not the one at 2000
+    c = _cands([(0, 1000, 5.0, 8.0, 1, 7), (900, 1, 5.0, 8.5, 0, 50), (2000, 1, 5.0, 9.0, 0, 50)])
+    assert oc(c, 0.0, 0) == ([[0, 1], [2]], [1, 2])
+    # touching boxcars [0,1000) and [1000,1001) are linked at gap 0 (1000 <= 0 + 1000 + 0); one sample further is not
+    c = _cands([(0, 1000, 5.0, 8.0, 0, 7), (1000, 1, 5.0, 8.5, 0, 7), (2002, 1, 5.0, 8.5, 0, 7)])
+    assert oc(c, 0.0, 0) == ([[0, 1], [2]], [1, 2])
+    assert oc(c, 0.0, 1000) == ([[0, 1], [2]], [1, 2])          # 2002 > 1000 + 1 + 1000
+    assert oc(c, 0.0, 1001) == ([[0, 1, 2]], [1])               # equal snr 8.5: the earlier sample represents
+    # equal SNR everywhere: the representative is the first by (range, dm_index, sample)
+    c = _cands([(50, 2, 4.0, 8.0, 1, 3), (51, 2, 4.0, 8.0, 0, 9), (500, 2, 4.0, 8.0, 0, 2)])
+    assert oc(c, 0.0, 0) == ([[0, 1], [2]], [1, 2])             # (0, 9, 51) sorts before (1, 3, 50)
+    assert oc(c[:0], 1.0, 1) == ([], [])
+
+
 @pytest.mark.parametrize("seed,n,dm_tol,gap", [(1, 300, 0.6, 3), (2, 500, 0.0, 0), (3, 400, 2.5, 40), (4, 1, 1.0, 1)])
 def test_random_lists_equal_the_written_out_definition(seed, n, dm_tol, gap):
     rs = np.random.default_rng(seed)
