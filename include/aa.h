@@ -278,6 +278,37 @@ aa_status aa_get_row_moments(aa_strategy* s, int32_t range, int64_t* sum_d, int6
 /* Device pointer of D_r for the current chunk and its row pitch in elements (read-only use by other GPU code). */
 aa_status aa_get_dedispersed_device(aa_strategy* s, int32_t range, const int32_t** device_ptr, int64_t* row_pitch);
 
+/* aa_row_moments_static: the same two checksums per row as aa_get_row_moments (sum_t D[i][t] and sum_t t * D[i][t], int64,
+ * wrapping modulo 2^64 like it), on ANY block of int32 rows in device memory, WITHOUT allocating anything - no strategy, no
+ * arena, no cudaMalloc / cudaFree / allocating library call inside.
+ *
+ * Who needs it: code that may not allocate device memory at the moment it wants to check rows of D. (1) A back-end that has
+ * handed out all of the GPU's memory up front (the arena lent to aa_strategy_setup, the capture ring, other stages): a fresh
+ * cudaMalloc there can fail, and the budget forbids it anyway. (2) A watchdog thread that checksums rows while the chunk loop
+ * streams: cudaMalloc and cudaFree synchronise the whole device and would stall the H2D prefetch and the kernels in flight.
+ * aa_get_row_moments does not serve them: it works only on a strategy's own D, out of that strategy's arena.
+ *
+ * Working memory: one array built into the library, 2 x AA_STATIC_MOMENTS_MAX_ROWS x 8 bytes = 256 KiB, present on every
+ * GPU that loads this library's kernels, from load until the process exits, whether this function is ever called or not.
+ *   device_D   (DEVICE, const) nrows rows of int32, row i at device_D + i * row_pitch (elements); e.g. from
+ *              aa_get_dedispersed_device. Must be memory of the CURRENT device.
+ *   nt         samples summed per row, 0 <= nt <= row_pitch.
+ *   nrows      0 <= nrows <= AA_STATIC_MOMENTS_MAX_ROWS (16384). More rows: AA_ERR_INVALID_ARG, nothing is launched, and
+ *              aa_last_error() states the limit - split the rows over several calls.
+ *   host_sum_d, host_sum_td (HOST, caller-owned) nrows int64 each, written before the call returns.
+ *   stream     cudaStream_t (NULL = default stream). The kernels and the two device-to-host copies run on it and the call
+ *              waits for it, so work queued earlier on that stream (the kernel that writes D) is finished first.
+ * First call on each device: the function asks the CUDA runtime for the array's address on the current device
+ * (cudaGetSymbolAddress) and keeps it; later calls on that device reuse it. Make this first call during start-up, with the
+ * intended device current and before any stream capture begins.
+ * Sharing: every call on a GPU uses the SAME array, and it keeps the last call's sums. Each call clears the words it will use
+ * on `stream` before summing, so calls one after another (any stream, any thread) are independent; two calls that are on the
+ * GPU at the same time (two host threads, two streams) add into the same words and both get wrong sums - serialise them.
+ * Results equal aa_get_row_moments' bit for bit (integer sums). Errors: AA_ERR_INVALID_ARG, AA_ERR_CUDA. */
+#define AA_STATIC_MOMENTS_MAX_ROWS 16384
+aa_status aa_row_moments_static(const int32_t* device_D, int64_t row_pitch, int64_t nt, int32_t nrows,
+                                int64_t* host_sum_d, int64_t* host_sum_td, void* stream);
+
 /* Block until everything enqueued on the strategy's streams has finished. */
 aa_status aa_synchronize(aa_strategy* s);
 

@@ -22,6 +22,7 @@ __all__ = [
     "aa_strategy_get_range_info", "aa_strategy_get_chunk", "aa_strategy_get_delay", "aa_strategy_describe",
     "aa_strategy_reset", "aa_strategy_shard", "aa_run_dedispersion", "aa_run_dedispersion_device", "aa_run_sps", "aa_run_pipeline", "aa_get_candidates", "aa_get_clusters", "aa_cluster_candidates", "CLUSTER_DTYPE",
     "aa_get_dedispersed_row", "aa_get_row_stats", "aa_get_row_moments", "aa_get_dedispersed_device", "aa_synchronize",
+    "aa_row_moments_static", "AA_STATIC_MOMENTS_MAX_ROWS",
     "aa_measure_int_add_peak", "aa_measure_int_add_peak3", "aa_get_last_timings", "aa_get_launch_count", "aa_last_error", "aa_version",
     "Plan", "Strategy",
 ]
@@ -30,6 +31,7 @@ AA_OK, AA_STATUS_CHUNK_DONE, AA_STATUS_FINISHED = 0, 1, 2
 AA_ERR_INVALID_ARG, AA_ERR_NOT_READY, AA_ERR_BUDGET_TOO_SMALL, AA_ERR_CUDA = -1, -2, -3, -4
 AA_ERR_CANDIDATE_OVERFLOW, AA_ERR_ORDER, AA_ERR_INTERNAL, AA_ERR_RANGE = -5, -6, -7, -8
 AA_LAYOUT_CHANNEL_MAJOR, AA_LAYOUT_TIME_MAJOR = 0, 1
+AA_STATIC_MOMENTS_MAX_ROWS = 16384      # rows per aa_row_moments_static call (include/aa.h)
 
 CLUSTER_DTYPE = None  # defined below CANDIDATE_DTYPE
 CANDIDATE_DTYPE = np.dtype([("sample", np.uint64), ("dm", np.float32), ("snr", np.float32), ("width", np.uint32),
@@ -117,6 +119,7 @@ def load():
         "aa_get_row_stats": (c_int32, [vp, c_int32, c_int32, POINTER(c_double), POINTER(c_double), POINTER(c_int64), POINTER(c_int32)]),
         "aa_get_row_moments": (c_int32, [vp, c_int32, vp, vp]),
         "aa_get_dedispersed_device": (c_int32, [vp, c_int32, POINTER(vp), POINTER(c_int64)]),
+        "aa_row_moments_static": (c_int32, [vp, c_int64, c_int64, c_int32, vp, vp, vp]),
         "aa_synchronize": (c_int32, [vp]),
         "aa_measure_int_add_peak": (c_int32, [vp, c_int32, POINTER(c_double), POINTER(c_double), POINTER(c_double)]),
         "aa_measure_int_add_peak3": (c_int32, [vp, c_int32, POINTER(c_double), POINTER(c_double), POINTER(c_double), POINTER(c_double)]),
@@ -366,6 +369,20 @@ def aa_get_dedispersed_device(strategy, rng: int):
     p, pitch = c_void_p(), c_int64()
     _check(load().aa_get_dedispersed_device(strategy, rng, byref(p), byref(pitch)))
     return p.value, pitch.value
+
+
+def aa_row_moments_static(device_D, row_pitch: int, nt: int, nrows: int, stream=None):
+    """sum_t D and sum_t t*D of `nrows` int32 rows in device memory (row i at device_D + i*row_pitch elements), computed
+    without any device allocation: the entry point for callers that cannot call cudaMalloc (all device memory already
+    handed out, or a thread that must not stall the streaming loop with an allocation's device-wide synchronisation).
+    At most AA_STATIC_MOMENTS_MAX_ROWS rows per call (AaError beyond that). `device_D` is a device pointer (int) or a
+    torch tensor on the current device. Calls share one built-in scratch array per GPU: do not run two at once."""
+    n = max(0, int(nrows))
+    a = np.zeros(n, dtype=np.int64)
+    b = np.zeros(n, dtype=np.int64)
+    _check(load().aa_row_moments_static(_ptr(device_D), int(row_pitch), int(nt), int(nrows), a.ctypes.data, b.ctypes.data,
+                                        _ptr(stream)))
+    return a, b
 
 
 def aa_synchronize(strategy) -> int:
