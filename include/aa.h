@@ -10,7 +10,10 @@
  * paper's 8-step list (§3.1). The function names and the arithmetic are BASELINE.json `north_star`.
  *
  * Conventions
- *   - Plain C, no exceptions cross the boundary, no global mutable state except a thread-local error string.
+ *   - Plain C, no exceptions cross the boundary. Process-wide state: a thread-local error string, and (aa_row_moments_static
+ *     only) the address of its built-in scratch array per device. Everything else, kernel attributes and the SM count
+ *     included, is set per strategy at aa_strategy_setup for the device that is current there; every aa_run_* / aa_get_* call
+ *     on a strategy must be made with that same device current (AA_ERR_INVALID_ARG naming both devices otherwise).
  *   - Every entry point returns aa_status: >= 0 success / progress, < 0 error. After an error,
  *     aa_last_error() names the offending field ("the API provides user feedback").
  *     Errors raised by aa_run_* are sticky on the strategy.
@@ -42,7 +45,8 @@ typedef enum {
     AA_ERR_CANDIDATE_OVERFLOW = -5,  /* records beyond capacity were dropped, the count is still exact */
     AA_ERR_ORDER = -6,               /* "another module still needs to run" */
     AA_ERR_INTERNAL = -7,
-    AA_ERR_RANGE = -8                /* 16-bit plans only: the data made a boxcar sum leave int32 (see aa_plan_set_input_bits) */
+    AA_ERR_RANGE = -8                /* 16-bit plans only: a sample above max_value, or the data made a boxcar sum leave int32
+                                        (see aa_plan_set_input_bits) */
 } aa_status;
 
 /* One DM range: DM_i = dm_low + i*dm_step for i in [0, ndms); the range is searched on data decimated in time by
@@ -126,7 +130,9 @@ aa_status aa_plan_set_input_layout(aa_plan* plan, int32_t layout);
  * bits) and nchans * max_value * max(bin) < 2^31 (int32 sums). The 8-bit plan's worst-case bound on boxcar sums cannot be
  * given at plan time for 16-bit samples (256 * 4096 * 4095 * 8 is far beyond int32 although real boxcar sums of (D - D[0])
  * are tiny), so it is checked on the DATA instead: if width_max * max|D - D[0]| of a row reaches 2^31, aa_run_sps /
- * aa_get_candidates return AA_ERR_RANGE (sticky) rather than a wrong candidate.
+ * aa_get_candidates return AA_ERR_RANGE (sticky) rather than a wrong candidate. The samples themselves are checked too, in
+ * the kernel that reads every chunk for the per-channel means: a chunk with a sample above max_value (its binned sums would
+ * carry into their neighbours) ends in the same sticky AA_ERR_RANGE at the next aa_run_sps / aa_get_candidates.
  * Speed: noise around a per-channel mean rides the 1-byte dedispersion path whatever the sample type (per-channel offset +
  * exception list); a chunk whose channels spread over more than about +-128 (bin 1, 2, 4) or +-512 (bin 8)
  * around their mean in too many samples falls back to a slow global-memory kernel - still exact.
@@ -202,11 +208,14 @@ aa_status aa_strategy_shard(aa_strategy* s, int32_t rank, int32_t world);
 /* ------------------------------------------------------------------------------------------------ pipeline
  * PAPER.md:47 step 7. One call = one chunk of one module.
  *
- * aa_run_dedispersion: H2D of the cursor's chunk (unless a previous call prefetched it), prefetch of the following chunk
- * into the other input buffer on the copy stream, time binning for ranges with bin > 1, then
+ * aa_run_dedispersion: H2D of the cursor's chunk (unless a previous call prefetched it), prefetch of the following chunk on
+ * the copy stream (channel-major plans have ONE raw input buffer: the prefetch starts as soon as K1, its only reader, has
+ * finished with the current chunk; time-major plans alternate between two staging buffers), time binning for ranges with
+ * bin > 1, then
  *   D_r[i][t'] = sum_c x_b[c][t' + delay(c,r,i)]   (int32, bit-exact)            [north_star]
  * for every range. Asynchronous: returns after enqueueing.
- *   host_input (HOST, const, user-owned, never written): the WHOLE observation, uint8. Channel-major plans:
+ *   host_input (HOST, const, user-owned, never written): the WHOLE observation; uint8 samples, or uint16 samples for a plan
+ *              with aa_plan_set_input_bits(16, ..) (strides stay in bytes). Channel-major plans:
  *              x[c][t], nsamp_total samples per channel, row_stride_bytes between channels. Time-major plans
  *              (aa_plan_set_input_layout): x[t][c], nchans samples per row, row_stride_bytes (>= nchans) between
  *              consecutive time samples. Must stay valid until the

@@ -153,6 +153,10 @@ struct Strategy {
     long long* d_moments = nullptr;          /* [2][max ndms] */
     size_t max_candidates = 0;
 
+    /* the device this strategy was set up on (arena, streams, events and kernel attributes all belong to it) */
+    int device = -1;
+    int nsm = 0;                                      /* its SM count */
+
     /* streams / events */
     cudaStream_t compute = nullptr, copy = nullptr;
     cudaStream_t aux = nullptr;                       /* library-owned: every other DM range's K2 runs here, so that the tail

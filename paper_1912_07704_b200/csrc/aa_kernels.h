@@ -23,7 +23,8 @@ extern "C" {
 int aak_bin_time(const uint8_t* x, size_t x_pitch, uint16_t* xb, size_t xb_pitch_elems, int32_t nchans,
                  int64_t nbinned, int32_t bin, const unsigned* only_if_cnt, unsigned only_if_above, void* stream);
 /* ---- K1b: shifted copy, out[c][j] = in[c][j + shift_bytes] (1..3) for j in [0, row_bytes), rows `pitch` bytes apart.
- * row_bytes and pitch are multiples of 16; the source must be readable up to row_bytes + 4 past each row start. */
+ * row_bytes and pitch are multiples of 16; only [0, row_bytes) of a source row is read, and the last shift_bytes of an output row
+ * (which would come from past the source row) are zero, so out may start right behind the source row (out = in + row_bytes). */
 int aak_shift_copy(const uint8_t* in, uint8_t* out, size_t pitch, size_t row_bytes, int32_t nrows, int32_t shift_bytes,
                    const unsigned* only_if_cnt, unsigned only_if_above, void* stream);
 
@@ -37,7 +38,8 @@ int aak_shift_copy(const uint8_t* in, uint8_t* out, size_t pitch, size_t row_byt
 int aak_chan_offsets(const uint8_t* x, size_t pitch, int64_t len, int32_t nrows, int32_t* off2, int32_t* off4, int32_t* off8, int32_t* bias2,
                      int32_t* bias4, int32_t* bias8, void* stream);
 int aak_scatter_exceptions(const uint2* exc, const unsigned* exc_cnt, unsigned cap, const double* k, double dm_low, double dm_step,
-                           int32_t ndms, int32_t bin, int64_t nt, int32_t* D, int64_t pitch, void* stream);
+                           int32_t ndms, int32_t bin, int64_t nt, int32_t* D, int64_t pitch,
+                           int32_t nsm /* SMs of the strategy's device: the grid is 4 CTAs per SM */, void* stream);
 
 /* ---- K1 fused: one read of raw rows [0, nrows) (pointers already offset to the first row; chan0 = its channel index)
  * writes the 4 uint8 copies (x4, may be NULL; rows x4_pitch bytes apart, copy k at + k x4_stride), the offset-uint8 forms lo2 / lo4 with their 4 copies and exceptions (may be
@@ -61,13 +63,15 @@ int aak_prep_fused(const aak_prep_args* a, int32_t nrows, void* stream);
 
 /* ---- K1 for 16-bit input samples (k_input16.cu): the offset forms x_b = lo + off_b[c] + r of a uint16 chunk.
  * aak_chan_offsets16: off[k][c] = clamp(round(b mean_t x[c][t]) - centre[k], 0, ..) and *bias[k] += off[k][c], k = 0..3 <-> b = 1, 2, 4, 8
- * (NULL entries are skipped; pointers already offset to the first row).
+ * (NULL entries are skipped; pointers already offset to the first row). The same read checks every sample against the plan's
+ * max_value (the packed sums of K1 and the int32 bound on D rely on it).
  * aak_prep16: one read of raw rows writes the byte forms of bin 1, 2, 4 (lo[k], 4 copies, window [0, 255]) and the uint16 form
  * of bin 8 (lo8, 2 copies, window [0, hi8]) with their exception lists; ngroups = 32-byte groups (16 samples) per row.
  * aak_bin_time16: plain x_b as uint16, one copy (the input of the global-memory route); bin in {1, 2, 4, 8}; conditional like
  * aak_bin_time. aak_corner_turn16: x[c][t] = x_tm[t][c] for uint16 samples. */
 int aak_chan_offsets16(const uint16_t* x, size_t pitch_bytes, int64_t len, int32_t nrows, int32_t* const off[4], int32_t* const bias[4],
-                       const int32_t centre[4], void* stream);
+                       const int32_t centre[4], uint32_t input_max,
+                       unsigned* range_flag /* may be NULL; else bit 0 is set if any sample of the rows exceeds input_max */, void* stream);
 typedef struct {
     const uint16_t* raw; size_t pitch_bytes; int64_t ngroups; int32_t chan0; unsigned cap;
     uint8_t* lo[3]; size_t pitch[3], stride[3]; const int32_t* off[3]; uint2* exc[3]; unsigned* cnt[3]; int64_t nb[3];
@@ -134,6 +138,7 @@ int aak_dedisperse_init(void);   /* sets the dynamic shared-memory attribute of 
 int aak_dedisperse_bits(const uint32_t* bits, size_t pitch_words, const int32_t* delays, int32_t nchans, int32_t chan_begin, int32_t chan_end,
                         int32_t ndms, int64_t nt, int32_t window_words, int32_t* D, int64_t pitch, const unsigned* mode_cnt, unsigned mode_cap,
                         void* stream);
+int aak_bits_init(void);         /* sets the dynamic shared-memory attribute (per device: call with the strategy's device current) */
 
 /* One thread per output, global loads (copy 0 of the input, pitch in elements): the route for ranges whose channel window
  * does not fit shared memory, and a cross-check. delays [ndms][nchans] int32; sums channels [chan_begin, chan_end),

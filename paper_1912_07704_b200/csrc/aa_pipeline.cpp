@@ -29,6 +29,16 @@ aa_status check_ready(aa_strategy* h, const char* fn) {
     if (!h) { set_error("%s: strategy is NULL — configure a plan and call aa_strategy_setup first", fn); return AA_ERR_NOT_READY; }
     if (!h->s.ready) { set_error("%s: this strategy was only planned (aa_strategy_plan); call aa_strategy_setup to make it ready", fn); return AA_ERR_NOT_READY; }
     if (h->s.sticky < 0) { return h->s.sticky; }
+    /* arena, streams, events, tensor maps and kernel attributes belong to the device the strategy was set up on: running it with
+     * another device current would launch on the wrong GPU (one arena per device; one strategy per device) */
+    int dev = -1;
+    const cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    if (dev != h->s.device) {
+        set_error("%s: this strategy was set up on CUDA device %d but device %d is current; cudaSetDevice(%d) first (one strategy per device)",
+                  fn, h->s.device, dev, h->s.device);
+        return AA_ERR_INVALID_ARG;
+    }
     return AA_OK;
 }
 
@@ -78,8 +88,10 @@ aa_status enqueue_prep16(Strategy& s, const Chunk& c, int b, int32_t c0, int32_t
         centre[k] = bin == 8 ? (s.lo16_max + 1) / 2 : 128;
         any = any || sparse;
     }
+    /* runs for every 16-bit chunk, also when no bin has an offset form: the same read checks the samples against max_value */
+    AA_LAUNCH(aak_chan_offsets16(raw, s.in_pitch, (int64_t)c.len, n, off, bias, centre, s.plan.input_max, (unsigned*)(s.d_counter + 2), s.compute),
+              "channel offsets (16-bit)");
     if (any) {
-        AA_LAUNCH(aak_chan_offsets16(raw, s.in_pitch, (int64_t)c.len, n, off, bias, centre, s.compute), "channel offsets (16-bit)");
         aak_prep16_args a;
         memset(&a, 0, sizeof a);
         a.raw = raw; a.pitch_bytes = s.in_pitch; a.ngroups = (int64_t)(s.in_pitch / 32); a.chan0 = c0; a.cap = kExcCap;
@@ -199,7 +211,7 @@ aa_status enqueue_k2(Strategy& s, const Chunk& c, int32_t c0, int32_t c1, bool a
                                           rg.pitch, cnt, lim, st), "bit-plane dedispersion");
         if (sparse)
             AA_LAUNCH(aak_scatter_exceptions(s.d_exc[bin] + (size_t)g * kExcCap, s.d_exc_cnt[bin] + g, lim, s.d_k, rg.r.dm_low, rg.r.dm_step,
-                                             rg.r.ndms, bin, a.nt, rg.d_D, rg.pitch, st), "exception scatter");
+                                             rg.r.ndms, bin, a.nt, rg.d_D, rg.pitch, s.nsm, st), "exception scatter");
         if (rg.dense_naive)
             AA_LAUNCH(aak_dedisperse_naive(x0, pitch_elems, 1, rg.d_delays, s.plan.nchans, c0, c1, rg.r.ndms, a.nt, rg.d_D, rg.pitch,
                                            accumulate ? 1 : 0, cnt, lim, st), "dedispersion (global-memory route of an exception-heavy chunk)");
@@ -244,6 +256,8 @@ aa_status enqueue_dedispersion(Strategy& s, int64_t j, int b, const uint8_t* tm_
             AA_LAUNCH(aak_corner_turn(tm_src, tm_stride, s.d_raw[0], s.in_pitch, C, (int64_t)c.len, s.compute), "corner turn");
         b = 0;                                        /* the channel-major copy lives in d_raw[0] */
     }
+    if (s.plan.input_bits == 16)                   /* [2]: "a sample exceeds max_value" flag of this chunk (k_chan_offsets16) */
+        AA_CUDA(cudaMemsetAsync(s.d_counter + 2, 0, sizeof(unsigned long long), s.compute), "cudaMemsetAsync");
     for (int bn = 1; bn <= 8; bn *= 2)             /* exception counters and biases of this chunk's channel groups */
         if (s.d_exc_cnt[bn]) AA_CUDA(cudaMemsetAsync(s.d_exc_cnt[bn], 0, 2 * kMaxGroups * 4, s.compute), "cudaMemsetAsync");
     if (groups) {
@@ -284,6 +298,13 @@ aa_status harvest(Strategy& s) {
     if (!s.harvest_pending) return AA_OK;
     AA_CUDA(cudaEventSynchronize(s.ev_count), "cudaEventSynchronize");
     const unsigned long long found = s.h_counter[0];
+    if (s.plan.input_bits == 16 && (s.h_counter[2] & 1ull)) {
+        s.harvest_pending = false;
+        set_error("aa_run_sps: chunk %lld holds a sample above the plan's max_value = %u (aa_plan_set_input_bits): the binned sums and D of "
+                  "this chunk cannot be trusted", (long long)s.harvest_chunk, s.plan.input_max);
+        s.sticky = AA_ERR_RANGE;
+        return s.sticky;
+    }
     if (s.h_counter[1] & 1ull) {
         s.harvest_pending = false;
         set_error("aa_run_sps: in chunk %lld the widest boxcar times the largest |D - D[0]| of a row reaches 2^31: the int32 boxcar sums cannot be "
@@ -437,7 +458,7 @@ extern "C" aa_status aa_run_sps(aa_strategy* h) {
         AA_CUDA(cudaStreamWaitEvent(s.compute, s.ev_join, 0), "cudaStreamWaitEvent");
     }
     AA_CUDA(cudaEventRecord(s.ev_t[5], s.compute), "cudaEventRecord");
-    AA_CUDA(cudaMemcpyAsync(s.h_counter, s.d_counter, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s.compute), "counter D2H");
+    AA_CUDA(cudaMemcpyAsync(s.h_counter, s.d_counter, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s.compute), "counter D2H");
     AA_CUDA(cudaEventRecord(s.ev_count, s.compute), "cudaEventRecord");
     s.harvest_pending = true; s.harvest_chunk = j; s.stats_timed = true;
     s.pending_sps = false;

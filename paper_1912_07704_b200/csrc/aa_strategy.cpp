@@ -511,6 +511,8 @@ extern "C" aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, u
 
     /* streams, events, pinned counter */
     cudaError_t e;
+    if ((e = cudaGetDevice(&s.device)) != cudaSuccess) return fail(cuda_fail(e, "cudaGetDevice"));
+    if ((e = cudaDeviceGetAttribute(&s.nsm, cudaDevAttrMultiProcessorCount, s.device)) != cudaSuccess || s.nsm < 1) return fail(cuda_fail(e, "cudaDeviceGetAttribute (SM count)"));
     if (compute_stream) s.compute = (cudaStream_t)compute_stream;
     else { if ((e = cudaStreamCreateWithFlags(&s.compute, cudaStreamNonBlocking)) != cudaSuccess) return fail(cuda_fail(e, "cudaStreamCreate")); s.owns_compute = true; }
     if (copy_stream) s.copy = (cudaStream_t)copy_stream;
@@ -533,6 +535,7 @@ extern "C" aa_status aa_strategy_setup(aa_strategy** out, const aa_plan* plan, u
     *s.h_counter = 0;
     if ((e = (cudaError_t)aak_dedisperse_init()) != cudaSuccess) return fail(cuda_fail(e, "kernel attribute setup (dedispersion)"));
     if ((e = (cudaError_t)aak_sps_init()) != cudaSuccess) return fail(cuda_fail(e, "kernel attribute setup (sps)"));
+    if ((e = (cudaError_t)aak_bits_init()) != cudaSuccess) return fail(cuda_fail(e, "kernel attribute setup (bit plane)"));
 
     /* upload tables, build tensor maps and row descriptors */
     std::vector<aak_row_desc> rows_full(s.nrows), rows_last(s.nrows);

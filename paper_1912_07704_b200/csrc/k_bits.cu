@@ -198,14 +198,14 @@ extern "C" int aak_dedisperse_bits(const uint32_t* bits, size_t pitch_words, con
     p.bits = bits; p.pitchw = pitch_words; p.delays = delays; p.nchans = nchans; p.c0 = chan_begin; p.c1 = chan_end; p.ndms = ndms; p.nt = nt;
     p.ww = window_words; p.D = D; p.dpitch = pitch; p.mode_cnt = mode_cnt; p.mode_cap = mode_cap;
     const size_t smem = ((size_t)BK_CB * window_words + BK_CB * BK_DMS) * 4;
-    static bool attr = false;
-    if (!attr) {
-        const int e = (int)cudaFuncSetAttribute(k_dedisperse_bits, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        if (e) return e;
-        attr = true;
-    }
     dim3 grid((unsigned)((nt + BK_T - 1) / BK_T), (unsigned)((ndms + BK_DMS - 1) / BK_DMS));
     if (grid.y > 65535) return (int)cudaErrorInvalidConfiguration;
     k_dedisperse_bits<<<grid, BK_THREADS, smem, (cudaStream_t)stream>>>(p);
     return (int)cudaGetLastError();
+}
+
+/* Function attributes belong to a device: called by aa_strategy_setup with the strategy's device current, like
+ * aak_dedisperse_init and aak_sps_init (no process-wide "already done" flag). */
+extern "C" int aak_bits_init(void) {
+    return (int)cudaFuncSetAttribute(k_dedisperse_bits, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
 }

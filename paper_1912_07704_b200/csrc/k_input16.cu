@@ -22,16 +22,21 @@ namespace {
 struct Off16 { int32_t* off[4]; int32_t* bias[4]; int32_t centre[4]; };
 
 __global__ void __launch_bounds__(256)
-k_chan_offsets16(const uint16_t* __restrict__ x, size_t pitch_bytes, long long len, const Off16 o) {
+k_chan_offsets16(const uint16_t* __restrict__ x, size_t pitch_bytes, long long len, const Off16 o, unsigned input_max,
+                 unsigned* __restrict__ range_flag) {
     __shared__ unsigned long long red[8];
     const uint16_t* row = reinterpret_cast<const uint16_t*>(reinterpret_cast<const uint8_t*>(x) + (size_t)blockIdx.x * pitch_bytes);
     unsigned long long s = 0;
+    unsigned mx2 = 0;                        /* largest sample seen, per 16-bit half */
     const long long nvec = len >> 3;
     for (long long q = threadIdx.x; q < nvec; q += 256) {
         const uint4 v = *reinterpret_cast<const uint4*>(row + q * 8);
         s += (v.x & 0xFFFFu) + (v.x >> 16) + (v.y & 0xFFFFu) + (v.y >> 16) + (v.z & 0xFFFFu) + (v.z >> 16) + (v.w & 0xFFFFu) + (v.w >> 16);
+        mx2 = __vmaxu2(__vmaxu2(mx2, v.x), __vmaxu2(__vmaxu2(v.y, v.z), v.w));
     }
-    for (long long t = (nvec << 3) + threadIdx.x; t < len; t += 256) s += row[t];
+    for (long long t = (nvec << 3) + threadIdx.x; t < len; t += 256) { const unsigned v = row[t]; s += v; mx2 = __vmaxu2(mx2, v); }
+    /* a sample above the plan's max_value breaks the packed 16-bit sums of K1 and the int32 bound on D: flag the chunk */
+    if (range_flag && max(mx2 & 0xFFFFu, mx2 >> 16) > input_max) atomicOr(range_flag, 1u);
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) s += __shfl_down_sync(0xffffffffu, s, d);
     if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
@@ -203,11 +208,11 @@ k_corner_turn16(const uint16_t* __restrict__ in, size_t in_stride_bytes, uint16_
 }  // namespace
 
 extern "C" int aak_chan_offsets16(const uint16_t* x, size_t pitch_bytes, int64_t len, int32_t nrows, int32_t* const off[4], int32_t* const bias[4],
-                                  const int32_t centre[4], void* stream) {
+                                  const int32_t centre[4], uint32_t input_max, unsigned* range_flag, void* stream) {
     if (nrows <= 0) return 0;
     Off16 o;
     for (int k = 0; k < 4; ++k) { o.off[k] = off[k]; o.bias[k] = bias[k]; o.centre[k] = centre[k]; }
-    k_chan_offsets16<<<(unsigned)nrows, 256, 0, (cudaStream_t)stream>>>(x, pitch_bytes, len, o);
+    k_chan_offsets16<<<(unsigned)nrows, 256, 0, (cudaStream_t)stream>>>(x, pitch_bytes, len, o, input_max, range_flag);
     return (int)cudaGetLastError();
 }
 

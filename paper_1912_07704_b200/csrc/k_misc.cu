@@ -63,7 +63,10 @@ k_shift_copy(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, size_t p
     if (g >= ngroups) return;
     const uint8_t* src = in + (size_t)blockIdx.y * pitch + (size_t)g * 16;
     const uint4 a = *reinterpret_cast<const uint4*>(src);
-    const uint32_t nx = *reinterpret_cast<const uint32_t*>(src + 16);
+    /* The last group of a row has no look-ahead word: its last `shift` output bytes would be in[row_bytes ..], which lie past the
+     * row (padding no reader uses) and are written as zero. Reading src + 16 there would also be a data race when the copies are
+     * interleaved in one buffer (out = in + row_bytes, the uint16 forms): that word is the first word of THIS launch's output. */
+    const uint32_t nx = g + 1 < ngroups ? *reinterpret_cast<const uint32_t*>(src + 16) : 0u;
     const int bs = shift * 8;
     uint4 o;
     o.x = __funnelshift_r(a.x, a.y, bs);
@@ -414,12 +417,9 @@ extern "C" int aak_chan_offsets(const uint8_t* x, size_t pitch, int64_t len, int
 }
 
 extern "C" int aak_scatter_exceptions(const uint2* exc, const unsigned* exc_cnt, unsigned cap, const double* k, double dm_low,
-                                      double dm_step, int32_t ndms, int32_t bin, int64_t nt, int32_t* D, int64_t pitch, void* stream) {
-    static int nsm = 0;
-    if (!nsm) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) nsm = 148;
-    }
+                                      double dm_step, int32_t ndms, int32_t bin, int64_t nt, int32_t* D, int64_t pitch, int32_t nsm,
+                                      void* stream) {
+    if (nsm < 1) return (int)cudaErrorInvalidValue;
     k_scatter_exceptions<<<nsm * 4, 256, 0, (cudaStream_t)stream>>>(exc, exc_cnt, cap, k, dm_low, dm_step, ndms, bin, nt, D, pitch);
     return (int)cudaGetLastError();
 }

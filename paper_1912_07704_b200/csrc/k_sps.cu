@@ -650,11 +650,14 @@ k_sps_peaks(const SpsParams p) {
                     inv = __ddiv_rn(1.0, __dmul_rn(__dsqrt_rn(w), sg_c));
                 }
                 rc.a[tid] = a; rc.inv[tid] = inv; if (PW) rc.q[tid] = q;
-                const double x = qd + a + p.threshold / inv;         /* real-valued bound on B_w - w p; margin below */
+                /* x = the computed value of X = q + a + threshold/inv, the real-valued bound on e = B_w - w p. DESIGN.md §2 "K4
+                 * prefilter margin" proves SNR_w > threshold => e >= floor(x): the rounding of the SNR expression and of x together
+                 * move the bound by < 2^-16 while e is an integer; the kernel keeps 2 whole units of slack on top. */
+                const double x = qd + a + p.threshold / inv;
                 int bm;
                 if (!(inv > 0.0)) bm = INT32_MAX;                    /* no SNR from this width: never flagged */
                 else if (x != x) bm = INT32_MIN;
-                else if (x >= 2147483000.0) bm = INT32_MAX;
+                else if (x >= 2147483000.0) bm = 2147482998;         /* e > x - 2^-16 is still possible up to INT32_MAX: keep the rule */
                 else if (x <= -2147483000.0) bm = INT32_MIN;
                 else bm = (int)floor(x) - 2;
                 rc.bmin[tid] = bm;

@@ -127,6 +127,33 @@ def test_16bit_boxcar_sums_beyond_int32_are_an_error_not_a_wrong_candidate():
     assert info["input_bits"] == 16
 
 
+def test_16bit_sample_above_max_value_is_an_error_not_a_wrong_row():
+    """The plan states max_value = 4095; ONE sample of the chunk is 4096. K1 packs binned sums into 16-bit lanes that rely on the
+    bound, so the chunk must end in AA_ERR_RANGE (sticky) naming max_value, on the offset-form route and on the route of an
+    exception-heavy chunk alike; the same data under a plan that admits the value runs clean."""
+    import paper_1912_07704_b200 as aa
+    for sigma in (16.0, 600.0):                                    # 600: every group is over the exception rate (global-memory route)
+        w = Workload("range16", 256, 1500.0, -0.5, 64e-6, 20000, ((0.0, 1.0, 24, 1), (24.0, 2.0, 16, 4)), (1, 4), 6.0, seed=5, npulses=0,
+                     pulse_dm=(0.0, 0.0), pulse_width_max=1, noise_mean=1800.0, noise_sigma=sigma, input_bits=16, max_value=4095)
+        x, _ = make_input(w)
+        assert int(x.max()) <= 4095
+        x[131, 7777] = 4096
+        gpu = GpuRun(w, x)
+        try:
+            gpu.dedisperse()
+            gpu.sps()
+            with pytest.raises(aa.AaError) as e:
+                gpu.candidates()
+            assert e.value.status == aa.AA_ERR_RANGE and "max_value = 4095" in e.value.message
+            with pytest.raises(aa.AaError) as e:                    # sticky
+                gpu.dedisperse()
+            assert e.value.status == aa.AA_ERR_RANGE
+        finally:
+            gpu.close()
+        info, got, _ = _every_row(scaled(w, max_value=8191, name="range16_wider"), x)
+        assert info["input_max"] == 8191
+
+
 def test_16bit_device_entry_point_and_host_array_checks():
     """aa_run_dedispersion_device with a resident uint16 chunk gives the host-path result; the binding refuses a uint8 array for
     a 16-bit plan (and vice versa) instead of reading it as raw bytes."""
