@@ -113,20 +113,22 @@ def row_moments_all_ranges(x: np.ndarray, k: np.ndarray, ranges, start: int, len
     def block(b, c0):
         c1 = min(C, c0 + chan_block)
         nb = length // b
-        xb = oracle.bin_time(x[c0:c1], start, nb, b).astype(np.int64)
+        xb = oracle.bin_time(x[c0:c1], start, nb, b)
+        # P[n] = sum_{t<n} x[t]; the first-moment prefix Q[n] = sum_{t<n} t x[t] is n P[n] - R[n] with R[n] = sum_{m<=n} P[m]
+        # (sum_{m=1..n} P[m] = sum_{t<n} (n - t) x[t]), so two cumulative sums serve both moments and Q is only formed at the
+        # gathered indices. int64 modulo 2^64 throughout, like the GPU's sums.
         P = np.zeros((c1 - c0, nb + 1), np.int64)
-        Q = np.zeros((c1 - c0, nb + 1), np.int64)
-        np.cumsum(xb, axis=1, out=P[:, 1:])
-        xb *= np.arange(nb, dtype=np.int64)
-        np.cumsum(xb, axis=1, out=Q[:, 1:])
+        np.cumsum(xb, axis=1, dtype=np.int64, out=P[:, 1:])
+        R = np.cumsum(P, axis=1)
         ch = np.arange(c1 - c0)[None, :]
         res = {}
         with np.errstate(over="ignore"):
             for r in by_bin[b]:
                 T = n_out // b
                 d = tables[r][:, c0:c1]
-                dP = P[ch, d + T] - P[ch, d]
-                dQ = Q[ch, d + T] - Q[ch, d]
+                P1, P0 = P[ch, d + T], P[ch, d]
+                dP = P1 - P0
+                dQ = ((d + T) * P1 - R[ch, d + T]) - (d * P0 - R[ch, d])
                 res[r] = (dP.sum(axis=1), (dQ - d * dP).sum(axis=1))
         return res
 

@@ -151,6 +151,15 @@ def test_ska_full_size_whole_oracle():
         gpu.close()
 
 
+def test_ska16_full_size():
+    """The SKA-like configuration delivered as 16-bit samples of 12-bit depth (PAPER.md:47 step 1) at full size:
+    offset-uint8 forms at bin 1/2/4 on 4096 channels, the offset-uint16 kernel on the bin-8 range, the 4.29 GB chunk through
+    the 3-group copy. All-row moments, sampled outputs and bands; the pulses are the ska workload's (same seed), so the list
+    has the same length as the 8-bit run's."""
+    info, ncand, nb = _fullsize("ska16", points_per_range=60, pulse_bands=1)
+    assert info["input_bits"] == 16 and info["input_max"] == 4095 and nb >= 15 and ncand > 0
+
+
 def test_lowf_full_size():
     """BASELINE.json configs[3] at full size (4096 channels x 2^21 samples, 6000 DM trials, delays up to 545 316 samples):
     all-row moments, sampled outputs and bands (first / middle / last of each range + one pulse band)."""
@@ -159,9 +168,11 @@ def test_lowf_full_size():
 
 
 def test_stream_full_size_selected_chunks():
-    """BASELINE.json configs[4] at full size (600 s, 40 GB budget, double-buffered H2D): the whole chunk loop runs; the first,
-    a middle and the last (short) chunk get the all-row moment identity, sampled outputs and one band per range, and the
-    candidate lists of those bands are compared; status codes are checked on every chunk."""
+    """BASELINE.json configs[4] at full size (600 s, 40 GB budget, double-buffered H2D): the whole chunk loop runs; EVERY chunk
+    gets the all-row moment identity ("every row of every chunk"; the oracle side of chunk j runs on a worker thread
+    while the GPU works on the chunks after it); the first, a middle and the last (short) chunk also get sampled outputs and one
+    band per range, and the candidate lists of those bands are compared; status codes are checked on every chunk."""
+    from concurrent.futures import ThreadPoolExecutor
     w = datagen.get_workload("stream")
     x, pinned = make_input(w, pinned=True)
     gpu, orc = GpuRun(w, x, budget_bytes=w.budget_bytes, max_candidates=1 << 23), OracleRun(w, x)
@@ -171,9 +182,14 @@ def test_stream_full_size_selected_chunks():
         check = {0, n // 2, n - 1}
         rs = np.random.default_rng(w.seed)
         exp_bands = []
+        pool, pending = ThreadPoolExecutor(max_workers=1), []
         for j, chunk in enumerate(gpu.chunks):
             start, length, n_out = chunk
             gpu.dedisperse()
+            if j not in check:                    # all-row moments of this chunk: GPU sums now (D is overwritten by the next chunk),
+                got_m = [gpu.moments(r) for r in range(len(w.ranges))]            # the oracle's side in the background
+                pending.append((j, got_m, pool.submit(row_moments_all_ranges, x[:, start:start + length], orc.k, w.ranges, 0, length,
+                                                      n_out, 32, None)))
             if j in check:
                 exp = row_moments_all_ranges(x[:, start:start + length], orc.k, w.ranges, 0, length, n_out)
                 for r, rng in enumerate(w.ranges):
@@ -198,5 +214,11 @@ def test_stream_full_size_selected_chunks():
             sel = (got["range"] == r) & (got["dm_index"] >= i0) & (got["dm_index"] < i1) & (got["sample"] >= start) & (got["sample"] < start + n_out)
             compare_candidates(got[sel], e, w.threshold)
         assert len(got) > 0
+        assert len(pending) + len(check) == n
+        for (j, got_m, fut) in pending:
+            exp = fut.result()
+            for r in range(len(w.ranges)):
+                assert np.array_equal(got_m[r][0], exp[r][0]) and np.array_equal(got_m[r][1], exp[r][1]), (j, r)
+        pool.shutdown()
     finally:
         gpu.close()

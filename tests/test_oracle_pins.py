@@ -644,3 +644,26 @@ def test_generator_16bit_matches_its_recipe():
     assert np.array_equal(a[ok].astype(np.int64) - 127, b[ok].astype(np.int64) - 1800)
     c = datagen.generate(77, 5, 4096, mean=4090.0, sigma=16.0, bits=16, max_value=4095)
     assert int(c.max()) == 4095 and np.mean(c == 4095) > 0.3
+
+
+def test_moment_helpers_equal_the_moments_of_the_oracle_rows():
+    """tests/helpers.py derives sum_t D and sum_t t*D of every row from prefix sums of the INPUT (the all-rows check of the
+    full-size GPU tests). Here both helpers are held against the moments of the rows the oracle dedisperses, on a case with
+    three binning factors, a chunk that starts inside the observation and channel blocks that do not divide the channel count."""
+    from helpers import row_moments_all_ranges, row_moments_from_input
+    rs = np.random.default_rng(77)
+    C, N = 37, 4096
+    x = rs.integers(0, 256, size=(C, N), dtype=np.uint8)
+    freqs = 1400.0 - 0.7 * np.arange(C)
+    k = oracle.delay_constants(freqs, 512e-6)
+    ranges = ((0.0, 0.8, 9, 1), (7.2, 1.6, 5, 2), (15.2, 3.0, 4, 4))
+    start, length, n_out = 256, 3200, 2400
+    allr = row_moments_all_ranges(x, k, ranges, start, length, n_out, chan_block=8, threads=2)
+    for r, rng in enumerate(ranges):
+        b, T = rng[3], n_out // rng[3]
+        xb = oracle.bin_time(x, start, length // b, b)
+        D = oracle.dedisperse(xb, k, rng, 0, rng[2], T).astype(np.int64)
+        m0, m1 = D.sum(axis=1), (D * np.arange(T, dtype=np.int64)).sum(axis=1)
+        assert np.array_equal(allr[r][0], m0) and np.array_equal(allr[r][1], m1), r
+        e0, e1 = row_moments_from_input(x, k, rng, start, length, T)
+        assert np.array_equal(e0, m0) and np.array_equal(e1, m1), r
