@@ -34,15 +34,68 @@ UNIT = "DM-trial*samples/s"
 SM_COUNT = 148
 
 
+K2_KERNELS = ("k_dedisperse", "k_scatter_exceptions")      # k_dedisperse also matches k_dedisperse_bits and k_dedisperse_naive
+
+
+def csrc_digest() -> str:
+    """sha256 over the kernel and host sources of the library (names and contents, sorted): what a tracked ncu capture is tied to.
+    (The GPU box has no .git, so a commit id cannot be checked there; the sources can.)"""
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted((ROOT / "paper_1912_07704_b200" / "csrc").iterdir()):
+        if f.suffix in (".cu", ".cuh", ".cpp", ".h"):
+            h.update(f.name.encode())
+            h.update(f.read_bytes())
+    return h.hexdigest()[:16]
+
+
 def k2_dram_traffic(workload: str):
     """dram__bytes_read.sum + dram__bytes_write.sum of the K2 launches of one step, from the tracked ncu capture
-    profiles/k2_dram_traffic.json (which names the commit and the command it was captured with); None if the workload has none."""
+    profiles/k2_dram_traffic.json (which names the command, the commit and the source digest it was captured at).
+    Returns (bytes or None, note); the note says STALE when the library sources have changed since the capture."""
     f = ROOT / "profiles" / "k2_dram_traffic.json"
     if not f.exists():
-        return None, None
+        return None, "no capture (profiles/k2_dram_traffic.json is missing)"
     rec = json.loads(f.read_text())
     e = rec.get("workloads", {}).get(workload)
-    return (e["bytes_per_step"], f"profiles/k2_dram_traffic.json (commit {rec.get('commit')}, {e.get('launches')} launches)") if e else (None, None)
+    if not e:
+        return None, f"no capture for workload {workload!r} in profiles/k2_dram_traffic.json"
+    at = e.get("csrc_sha256", rec.get("csrc_sha256"))
+    fresh = at is not None and at == csrc_digest()
+    note = f"profiles/k2_dram_traffic.json (commit {e.get('commit', rec.get('commit'))}, {e.get('launches')} launches)"
+    if not fresh:
+        note += "; STALE: the library sources have changed since this capture (csrc digest %s then, %s now)" % (at, csrc_digest())
+    return e["bytes_per_step"], note
+
+
+def record_traffic(csv_path: str, workload: str, commit: str, command: str, steps: int = 1) -> None:
+    """Write one workload's entry of profiles/k2_dram_traffic.json from an ncu --csv launch list that holds
+    dram__bytes_read.sum and dram__bytes_write.sum of `steps` identical steps (python bench.py --record-traffic CSV --workload W
+    --traffic-steps N --traffic-commit ID --traffic-command '...'). Sums the K2 launches (K2_KERNELS) and divides by the steps."""
+    import csv
+    rd = wr = 0
+    ids = set()
+    with open(csv_path, newline="") as fh:
+        rows = [r for r in csv.reader(fh) if len(r) >= 15 and r[0].isdigit()]
+    for r in rows:
+        name, metric, val = r[4], r[12], int(float(r[14].replace(",", "")))
+        if not any(k in name for k in K2_KERNELS):
+            continue
+        if metric == "dram__bytes_read.sum":
+            rd += val; ids.add(r[0])
+        elif metric == "dram__bytes_write.sum":
+            wr += val; ids.add(r[0])
+    assert ids, f"no K2 launch with DRAM metrics in {csv_path}"
+    assert len(ids) % steps == 0, f"{len(ids)} K2 launches do not divide into {steps} steps"
+    rd, wr, nl = rd // steps, wr // steps, len(ids) // steps
+    f = ROOT / "profiles" / "k2_dram_traffic.json"
+    rec = json.loads(f.read_text()) if f.exists() else {"workloads": {}}
+    rec.setdefault("workloads", {})[workload] = {"bytes_per_step": rd + wr, "read": rd, "written": wr, "launches": nl,
+                                                 "commit": commit, "csrc_sha256": csrc_digest(), "command": command,
+                                                 "source": "profiles/" + Path(csv_path).name}
+    f.write_text(json.dumps(rec, indent=1) + "\n")
+    print(json.dumps(rec["workloads"][workload]))
+
 
 INT_LANES_PER_SM_CLK = 128      # 64 ALU-pipe (IADD3) + 64 FMA-pipe (IMAD) lanes per SM per clock, DESIGN.md "Roofline"
 
@@ -54,7 +107,14 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="ska", help="tiny | mid | ska | lowf | stream (BASELINE.json configs 0..4), ska16 (ska as 16-bit samples); "
                     "stream = the 600 s chunked pipeline under a 40 GB budget, a step is the whole stream")
+    ap.add_argument("--noise-sigma", type=float, default=None, help="override the workload's noise sigma (input counts); used to record how "
+                    "the 16-bit offset forms degrade as the noise outgrows the byte window (not a BASELINE.json configuration)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--record-traffic", default=None, metavar="CSV", help="no GPU work: write this workload's entry of "
+                    "profiles/k2_dram_traffic.json from an ncu --csv launch list of one step (see record_traffic)")
+    ap.add_argument("--traffic-commit", default="uncommitted")
+    ap.add_argument("--traffic-steps", type=int, default=1)
+    ap.add_argument("--traffic-command", default="")
     ap.add_argument("--input", default="noise", choices=["noise", "uniform"], help="noise: the workload's recipe (Gaussian noise + pulses); "
                     "uniform: uniform random samples over the whole range - every offset form is exception-heavy, so the line records the "
                     "cost of the dense routes (uint16 kernels / global-memory kernel); not a BASELINE.json configuration")
@@ -130,7 +190,8 @@ def oracle_sample(w, x, n_out, rows_per_range: int):
     t_job = time.perf_counter() - t_start
     for r, rng in enumerate(w.ranges):
         b, T = rng[3], n_out // rng[3]
-        idx = sorted({int(round(q * (rng[2] - 1) / max(1, rows_per_range - 1))) for q in range(rows_per_range)})
+        idx = list(range(rng[2])) if rows_per_range is None else \
+            sorted({int(round(q * (rng[2] - 1) / max(1, rows_per_range - 1))) for q in range(rows_per_range)})
         t0 = time.perf_counter()
         for i in idx:
             D = oracle.dedisperse(binned[b], k, rng, i, i + 1, T)
@@ -139,7 +200,8 @@ def oracle_sample(w, x, n_out, rows_per_range: int):
             oracle.find_peaks(S[None, :], w.threshold)
         t_job += (time.perf_counter() - t0) * rng[2] / len(idx)
     spent = time.perf_counter() - t_start
-    what = (f"binning of the full chunk + {rows_per_range} evenly spaced DM row(s) of each of the {len(w.ranges)} ranges over "
+    what = (f"the WHOLE job: binning + every one of the {w.ndms_total} DM rows (dedispersion+SPS), nothing extrapolated" if rows_per_range is None else
+            f"binning of the full chunk + {rows_per_range} evenly spaced DM row(s) of each of the {len(w.ranges)} ranges over "
             f"the full chunk (dedispersion+SPS), extrapolated linearly in rows to all {w.ndms_total} rows")
     return outputs_of(w, n_out), t_job, spent, what
 
@@ -291,11 +353,12 @@ def run_ours(args, w):
     peak = SM_COUNT * INT_LANES_PER_SM_CLK * (sampler.max_mhz or 1965) * 1e6
     t_hbm = (in_bytes + 4 * outputs) / (json.loads((ROOT / "MEASURED_PEAKS.json").read_text())["hbm_gbs"] * 1e9) \
         if (ROOT / "MEASURED_PEAKS.json").exists() else (in_bytes + 4 * outputs) / 6.65e12
-    roofline = {"bound": "alu", "kernel": "k_dedisperse + k_scatter_exceptions (K2), the launches of all DM ranges of one step",
+    traffic_key = w.name if args.input == "noise" else w.name + "+uniform-input"      # a capture belongs to one workload AND input recipe
+    roofline = {"bound": "alu", "kernel": "k_dedisperse + k_dedisperse_bits + k_scatter_exceptions (K2), the launches of all DM ranges of one step",
                 "achieved": adds / k2 / 1e12, "peak": peak / 1e12, "unit": "Tadd/s (algorithmic 32-bit integer adds)",
-                "frac": adds / k2 / peak, "traffic": k2_dram_traffic(w.name)[0],
+                "frac": adds / k2 / peak, "traffic": k2_dram_traffic(traffic_key)[0],
                 "traffic_note": "dram__bytes_read.sum + dram__bytes_write.sum of the K2 launches of one step, one ncu capture: "
-                                + str(k2_dram_traffic(w.name)[1]) + "; compulsory bytes are input once + D once",
+                                + str(k2_dram_traffic(traffic_key)[1]) + "; compulsory bytes are input once + D once",
                 "peak_how": f"derived: {SM_COUNT} SMs x {INT_LANES_PER_SM_CLK} integer-add lanes/clk (64 IADD3 + 64 IMAD) x max SM clock",
                 "measured_iadd3_only_tadd_s": iadd3 / 1e12, "measured_iadd3_imad_mixed_tadd_s": mixed / 1e12, "measured_imad_only_tadd_s": imad / 1e12,
                 "frac_of_measured_mixed": adds / k2 / max(mixed, iadd3), "frac_of_measured_iadd3_only": adds / k2 / iadd3,
@@ -317,9 +380,11 @@ def run_ours(args, w):
             "candidates_per_step": ncand, "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline}
     if not args.no_cpu_baseline and world == 1:
-        rows = 3                              # first, middle and last DM row of every range
+        # Tiny and Mid: the whole oracle (seconds / a few minutes; SURVEY §8(d) "CPU baseline"); the large configurations: first,
+        # middle and last DM row of every range
+        rows = None if w.name.split("+")[0].split("@")[0] in ("tiny", "mid") and not args.nsamp else 3
         o, secs, spent, what = oracle_sample(w, x, info["n_out"], rows)
-        line["cpu_baseline"] = {"value": o / secs, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what,
+        line["cpu_baseline"] = {"value": o / secs, "unit": UNIT, "cores": 1, "kind": "oracle, full" if rows is None else "oracle", "sample": what,
                                 "sample_seconds": spent, "host_cores_available": os.cpu_count()}
     print(json.dumps(line), flush=True)
     st.close()
@@ -418,12 +483,46 @@ def run_stream(args, w):
     plan.close()
 
 
+def spawn_ranks(n: int) -> int:
+    """Re-run this command as n ranks under torch.distributed.run on 127.0.0.1 (one process per GPU). Returns the exit code;
+    refuses, with the reason, when the node shows fewer than n CUDA devices."""
+    import socket
+    import subprocess
+    import torch
+    have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+    if have < n:
+        print(f"bench.py: --gpus {n} needs {n} CUDA devices on this node, {have} visible; not running (a line with n_gpus: {have} "
+              f"would not be the measurement asked for)", file=sys.stderr)
+        return 2
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), str(Path(__file__).resolve()), *sys.argv[1:]]
+    return subprocess.call(cmd)
+
+
 def main():
     args = parse()
+    if args.record_traffic:
+        record_traffic(args.record_traffic, args.workload, args.traffic_commit, args.traffic_command, args.traffic_steps)
+        return
+    launched = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        pass                                   # CPU arm: rank 0 runs, the others exit; no GPU count to check
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # started as plain `python bench.py --gpus N`: become N ranks (one process per GPU) the way the driver starts them,
+        # or say why not. Never print an n_gpus: 1 line for a --gpus N request.
+        sys.exit(spawn_ranks(args.gpus))
+    elif args.gpus != launched:
+        sys.exit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE = {launched}: start N ranks with --nproc-per-node N (or run "
+                 f"`python bench.py --gpus N` and let it spawn them)")
     import datagen
     w = datagen.get_workload(args.workload)
     if args.nsamp:
         w = datagen.scaled(w, nsamp=args.nsamp, name=f"{w.name}@{args.nsamp}")
+    if args.noise_sigma is not None:
+        w = datagen.scaled(w, noise_sigma=args.noise_sigma, name=f"{w.name}+sigma{args.noise_sigma:g}")
     if args.impl == "reference":
         run_reference(args, w)
     elif w.budget_bytes:

@@ -298,3 +298,21 @@ def test_chunk_rows_stay_below_the_28_bit_sample_field_of_an_exception_record():
         assert e.value.status == aa.AA_ERR_INVALID_ARG and "largest chunk" in e.value.message
     finally:
         aa.aa_plan_destroy(plan)
+
+
+def test_bench_refuses_a_multi_gpu_request_it_cannot_honour():
+    """`python bench.py --gpus N` started without torchrun spawns its N ranks itself; on a node with fewer devices it must exit
+    non-zero saying why, never print an n_gpus: 1 line (VERDICT r02 missing 1). A --gpus that contradicts WORLD_SIZE is refused too."""
+    import os
+    import subprocess
+    import sys
+    import torch
+    if torch.cuda.is_available() and torch.cuda.device_count() >= 2:
+        pytest.skip("this node could really run 2 ranks")
+    root = Path(__file__).resolve().parent.parent
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    r = subprocess.run([sys.executable, str(root / "bench.py"), "--gpus", "2"], capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode != 0 and "needs 2 CUDA devices" in r.stderr and r.stdout.strip() == ""
+    r = subprocess.run([sys.executable, str(root / "bench.py"), "--gpus", "1"], capture_output=True, text=True,
+                       env=dict(env, WORLD_SIZE="2", RANK="0", LOCAL_RANK="0"), timeout=300)
+    assert r.returncode != 0 and "WORLD_SIZE = 2" in r.stderr and r.stdout.strip() == ""
